@@ -1,0 +1,147 @@
+/*
+ * hr.h -- C ABI of the B200-native Wilson-Dirac hopping term for higher-representation SU(N) fermions.
+ *
+ * What the library computes (BASELINE.json:north_star; workload: section 3.1 "Wilson-Dirac
+ * operator in single and double precision for general higher representations of SU(N_c)", even-odd;
+ * the represented link is a d_R x d_R matrix acting on the colour index of the spinor):
+ *
+ *   Dphi psi (x) = -1/2 sum_{mu=0..3} [ (1 - gamma_mu) s+_mu(x) U^R_mu(x)            psi(x + mu)
+ *                                     + (1 + gamma_mu) s-_mu(x) U^R_mu(x - mu)^dagger psi(x - mu) ]
+ *   D psi (x)    = (4 + m0) psi(x) + Dphi psi (x)
+ *
+ * on a periodic T x X x Y x Z lattice, s+-_mu(x) = bc[mu] on the hop that crosses the seam between
+ * x_mu = L_mu-1 and 0, else 1 (antiperiodic fermions: bc = -1), and the link map U -> U^R
+ * (fundamental, adjoint [real], two-index symmetric / antisymmetric).  Everything the paper is silent
+ * on (gamma basis, site order, parity, generator and tensor bases) is fixed in DESIGN.md "Readings"
+ * (C1..C19); the ones a caller needs are restated below.
+ *
+ * CANONICAL (interchange) LAYOUT, used only by the import/export calls (reading C4):
+ *   dims = {T, X, Y, Z}, mu = 0,1,2,3 = t,x,y,z.  Full-lattice site index i = ((t*X + x)*Y + y)*Z + z.
+ *   parity(i) = (t+x+y+z) & 1.  A parity-p half field lists the parity-p sites by increasing i, so its
+ *   half index is i >> 1 (every extent is even).
+ *   spinor site  = [spin alpha = 0..3][colour a = 0..d_R-1] complex (re, im)
+ *   gauge field  = [site i][mu][row][col] complex (re, im), row-major; a REPRESENTED ADJOINT field is
+ *                  real: [site i][mu][row][col] real.
+ * INTERNAL device layout (private): per parity, per 16-byte vector
+ * plane, contiguous in the half index.  Spinor buffers passed to hr_dphi_eo / hr_dirac are in the
+ * internal layout: fill them with hr_spinor_import, read them with hr_spinor_export.  Their size is
+ * hr_spinor_bytes() per parity (the same number of bytes as the canonical half field).
+ *
+ * Pointers: every `void *` spinor/gauge buffer handed to a compute call is DEVICE memory owned by the
+ * caller (e.g. a torch tensor's data_ptr()), 16-byte aligned.  `canon` pointers of import/export may
+ * be HOST or DEVICE memory (detected).  `stream` is a cudaStream_t passed as void* (NULL = default
+ * stream).  All device work is enqueued on that stream; the compute calls never synchronise and never
+ * allocate.  No call throws or exits: each returns an hr_status, and hr_last_error() gives the text.
+ * There is NO CPU fallback: without a usable CUDA device every compute call returns HR_ECUDA.
+ */
+#ifndef HR_H
+#define HR_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { HR_OK = 0, HR_EINVAL = -1, HR_EUNSUPPORTED = -2, HR_ECUDA = -3, HR_ENOMEM = -4 } hr_status;
+typedef enum { HR_F64 = 0, HR_F32 = 1 } hr_prec;
+typedef enum { HR_REP_FUND = 0, HR_REP_ADJ = 1, HR_REP_SYM = 2, HR_REP_ASYM = 3 } hr_rep;
+
+typedef struct hr_ctx hr_ctx;     /* immutable problem description: dims, bc, N, rep, device            */
+typedef struct hr_gauge hr_gauge; /* one link field: fundamental (N x N) or represented (d_R x d_R), one precision */
+
+/* Library version string, e.g. "hr-dphi 0.1 (sm_100a)". */
+const char *hr_version(void);
+/* Text of the last error raised on the calling thread ("" if none); valid until the next call. */
+const char *hr_last_error(void);
+
+/*
+ * Describe the problem.  dims[mu] even and >= 2 (reading C11: odd extents break the even/odd
+ * bipartition), bc[mu] in {+1,-1}, N in {2,3,4}.  Supported (N, rep): N=2: FUND, ADJ, SYM;
+ * N=3: FUND, ADJ, SYM, ASYM; N=4: FUND, ASYM.  Anything else (e.g. ASYM for N=2, d_R = 1)
+ * -> HR_EUNSUPPORTED.  Does not touch the GPU; `device` is the CUDA ordinal later calls run on.
+ */
+hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N, hr_rep rep, int device);
+void hr_ctx_destroy(hr_ctx *ctx); /* also frees the host-path workspace, if one was created */
+
+int hr_rep_dim(const hr_ctx *ctx);          /* d_R */
+int hr_links_are_real(const hr_ctx *ctx);   /* 1 for the adjoint (reading C7), else 0 */
+size_t hr_half_volume(const hr_ctx *ctx);   /* V/2 = output sites of one hr_dphi_eo */
+size_t hr_gauge_bytes(const hr_ctx *ctx, int represented, hr_prec prec); /* whole field, both parities */
+size_t hr_spinor_bytes(const hr_ctx *ctx, hr_prec prec);                 /* ONE parity: V/2 sites      */
+
+/*
+ * hr_gauge_alloc -- make a link-field handle (BASELINE.json:north_star "hr_gauge_alloc").
+ * represented = 0: fundamental N x N complex links; 1: represented d_R x d_R links (real for ADJ).
+ * dev_mem == NULL: the library allocates hr_gauge_bytes() of device memory and owns it;
+ * else it borrows caller memory (>= hr_gauge_bytes(), 16-byte aligned), which must outlive the handle.
+ * Contents are undefined until hr_gauge_import / hr_represent_links writes them.
+ */
+hr_status hr_gauge_alloc(const hr_ctx *ctx, int represented, hr_prec prec, void *dev_mem, hr_gauge **out);
+void hr_gauge_free(hr_gauge *g);
+void *hr_gauge_data(const hr_gauge *g);  /* device pointer of the internal-layout storage */
+
+/* canonical <-> internal.  canon_prec is the precision of the canonical array; conversion (one
+ * rounding) happens in the pack kernel.  For host `canon` the copy is staged through device memory
+ * the call allocates and frees (set-up path, not a hot call); the call returns after the data has
+ * left / reached `canon` (it synchronises the stream when `canon` is host memory). */
+hr_status hr_gauge_import(hr_gauge *dst, const void *canon, hr_prec canon_prec, void *stream);
+hr_status hr_gauge_export(const hr_gauge *src, void *canon, hr_prec canon_prec, void *stream);
+hr_status hr_spinor_import(const hr_ctx *ctx, void *dst_dev, hr_prec prec, const void *canon,
+                           hr_prec canon_prec, int parity, void *stream);
+hr_status hr_spinor_export(const hr_ctx *ctx, const void *src_dev, hr_prec prec, void *canon,
+                           hr_prec canon_prec, int parity, void *stream);
+
+/*
+ * hr_represent_links -- the link map U -> U^R, one kernel launch over the 4V links
+ * (BASELINE.json:north_star "fundamental-to-representation link map"; configs[2]:
+ * U^adj_ab = 2 tr(T_a U T_b U^dagger), T_a = lambda_a/2 in the nested Gell-Mann order, reading C6;
+ * configs[3]: two-index symmetric basis e^(ij), pairs lexicographic i<=j, reading C8:
+ * R_(ij),(kl) = n_ij n_kl (U_ik U_jl +- U_il U_jk), n = 1/sqrt2 on diagonal pairs; FUND = copy).
+ * fund_in: fundamental field, repr_out: represented field of the same ctx; precisions may differ
+ * (arithmetic in fund_in's precision, one rounding on store).
+ */
+hr_status hr_represent_links(hr_gauge *repr_out, const hr_gauge *fund_in, void *stream);
+
+/*
+ * hr_dphi_eo -- the even-odd hopping term, ONE kernel launch over the V/2 output sites
+ * (BASELINE.json:north_star "hr_dphi_eo(out, in, links, parity, stream)").
+ * parity = parity of the OUTPUT sites (reading C5).  out: parity-`parity` half field, in:
+ * parity-(1-parity) half field, both internal layout, precision = precision of `links`
+ * (a represented field).  out must not alias in.
+ */
+hr_status hr_dphi_eo(void *out, const void *in, const hr_gauge *links, int parity, void *stream);
+
+/*
+ * hr_dirac -- D = (4+m0) + Dphi on full fields (BASELINE.json:north_star "hr_dirac(m0)").
+ * Full field = [even half | odd half], each half in the internal layout (2 * hr_spinor_bytes()).
+ * Two launches (one per output parity) with the (4+m0) psi(x) term fused.  out_full != in_full.
+ */
+hr_status hr_dirac(double m0, void *out_full, const void *in_full, const hr_gauge *links, void *stream);
+
+/*
+ * hr_dphi_eo_host -- the same operation end to end from HOST memory: copies the canonical parity-
+ * (1-parity) half spinor `in_canon` (host, ideally pinned) to the device, packs it, runs hr_dphi_eo,
+ * unpacks and copies the canonical result into `out_canon` (host).  `links` stays resident on the
+ * device (a gauge field changes once per molecular-dynamics step, a spinor every call).  The
+ * workspace (two internal half spinors + one staging buffer) is created on first use and cached in
+ * the ctx.  Synchronises `stream` before returning.
+ */
+hr_status hr_dphi_eo_host(hr_ctx *ctx, void *out_canon, const void *in_canon, hr_prec canon_prec,
+                          const hr_gauge *links, int parity, void *stream);
+
+/*
+ * Kernel tuning (experiments and ncu evidence; defaults are chosen per (d_R, precision) from
+ * measurements).  key: "variant" (kernel variant id, -1 = default table),
+ * "block" (threads per CTA, 0 = default).  Unknown key or value -> HR_EINVAL.
+ */
+hr_status hr_ctx_set_tuning(hr_ctx *ctx, const char *key, int value);
+/* Name of the Dphi kernel variant a call with this precision would launch (for logs/bench). */
+const char *hr_dphi_variant_name(const hr_ctx *ctx, hr_prec prec);
+/* Number of kernel launches this library has enqueued since load (all threads). */
+unsigned long long hr_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HR_H */

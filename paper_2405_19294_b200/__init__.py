@@ -1,0 +1,288 @@
+"""Python binding of libhr (include/hr.h): the B200-native Wilson-Dirac hopping term Dphi for
+higher-representation SU(N) fermions (arxiv 2405.19294 hot path; BASELINE.json:north_star).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of libhr.so.  The
+functions below carry the names of the C ABI (hr_ctx_create, hr_gauge_alloc, hr_represent_links,
+hr_dphi_eo, hr_dirac, ...) and raise HrError on any non-zero hr_status.  `Lattice` is a small
+convenience wrapper that owns the handles and uses torch only for device memory and streams.
+
+There is NO CPU fallback: if libhr.so has not been built (python -m paper_2405_19294_b200.build)
+importing this package raises, and on a box without a CUDA device every compute call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhr.so")
+
+HR_OK, HR_EINVAL, HR_EUNSUPPORTED, HR_ECUDA, HR_ENOMEM = 0, -1, -2, -3, -4
+HR_F64, HR_F32 = 0, 1
+HR_REP_FUND, HR_REP_ADJ, HR_REP_SYM, HR_REP_ASYM = 0, 1, 2, 3
+REP_NAMES = {"fund": HR_REP_FUND, "adj": HR_REP_ADJ, "sym": HR_REP_SYM, "asym": HR_REP_ASYM}
+PREC_NAMES = {"f64": HR_F64, "f32": HR_F32}
+
+
+class HrError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__(f"libhr status {status}: {text}")
+        self.status = status
+
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -m paper_2405_19294_b200.build` "
+        "(there is no CPU fallback for the CUDA path)")
+
+_lib = ctypes.CDLL(LIB_PATH)
+_vp, _ci, _cd, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+_I4 = ctypes.c_int * 4
+
+# every symbol include/hr.h declares: name -> (restype, argtypes)
+_SIGNATURES = {
+    "hr_version": (ctypes.c_char_p, []),
+    "hr_last_error": (ctypes.c_char_p, []),
+    "hr_ctx_create": (_ci, [ctypes.POINTER(_vp), _I4, _I4, _ci, _ci, _ci]),
+    "hr_ctx_destroy": (None, [_vp]),
+    "hr_rep_dim": (_ci, [_vp]),
+    "hr_links_are_real": (_ci, [_vp]),
+    "hr_half_volume": (_sz, [_vp]),
+    "hr_gauge_bytes": (_sz, [_vp, _ci, _ci]),
+    "hr_spinor_bytes": (_sz, [_vp, _ci]),
+    "hr_gauge_alloc": (_ci, [_vp, _ci, _ci, _vp, ctypes.POINTER(_vp)]),
+    "hr_gauge_free": (None, [_vp]),
+    "hr_gauge_data": (_vp, [_vp]),
+    "hr_gauge_import": (_ci, [_vp, _vp, _ci, _vp]),
+    "hr_gauge_export": (_ci, [_vp, _vp, _ci, _vp]),
+    "hr_spinor_import": (_ci, [_vp, _vp, _ci, _vp, _ci, _ci, _vp]),
+    "hr_spinor_export": (_ci, [_vp, _vp, _ci, _vp, _ci, _ci, _vp]),
+    "hr_represent_links": (_ci, [_vp, _vp, _vp]),
+    "hr_dphi_eo": (_ci, [_vp, _vp, _vp, _ci, _vp]),
+    "hr_dirac": (_ci, [_cd, _vp, _vp, _vp, _vp]),
+    "hr_dphi_eo_host": (_ci, [_vp, _vp, _vp, _ci, _vp, _ci, _vp]),
+    "hr_ctx_set_tuning": (_ci, [_vp, ctypes.c_char_p, _ci]),
+    "hr_dphi_variant_name": (ctypes.c_char_p, [_vp, _ci]),
+    "hr_launch_count": (ctypes.c_ulonglong, []),
+}
+for _name, (_res, _args) in _SIGNATURES.items():
+    _f = getattr(_lib, _name)  # AttributeError here = the library does not export the header's symbol
+    _f.restype = _res
+    _f.argtypes = _args
+
+
+def _check(status: int) -> None:
+    if status != HR_OK:
+        raise HrError(status, _lib.hr_last_error().decode())
+
+
+def _ptr(x) -> int:
+    """Raw address of a torch tensor / numpy array / int / None."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        if not x.flags.c_contiguous:
+            raise ValueError("numpy buffer must be C-contiguous")
+        return x.ctypes.data
+    if hasattr(x, "data_ptr"):
+        if not x.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        return x.data_ptr()
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+# ---- the C ABI, same names --------------------------------------------------------------------
+
+def hr_version() -> str:
+    return _lib.hr_version().decode()
+
+
+def hr_last_error() -> str:
+    return _lib.hr_last_error().decode()
+
+
+def hr_launch_count() -> int:
+    return int(_lib.hr_launch_count())
+
+
+def hr_ctx_create(dims, bc, N: int, rep: int, device: int = 0) -> int:
+    h = _vp()
+    _check(_lib.hr_ctx_create(ctypes.byref(h), _I4(*[int(v) for v in dims]), _I4(*[int(v) for v in bc]), N, rep, device))
+    return h.value
+
+
+def hr_ctx_destroy(ctx: int) -> None:
+    _lib.hr_ctx_destroy(ctx)
+
+
+def hr_rep_dim(ctx: int) -> int:
+    return _lib.hr_rep_dim(ctx)
+
+
+def hr_links_are_real(ctx: int) -> int:
+    return _lib.hr_links_are_real(ctx)
+
+
+def hr_half_volume(ctx: int) -> int:
+    return _lib.hr_half_volume(ctx)
+
+
+def hr_gauge_bytes(ctx: int, represented: int, prec: int) -> int:
+    return _lib.hr_gauge_bytes(ctx, represented, prec)
+
+
+def hr_spinor_bytes(ctx: int, prec: int) -> int:
+    return _lib.hr_spinor_bytes(ctx, prec)
+
+
+def hr_gauge_alloc(ctx: int, represented: int, prec: int, dev_mem=None) -> int:
+    g = _vp()
+    _check(_lib.hr_gauge_alloc(ctx, represented, prec, _ptr(dev_mem), ctypes.byref(g)))
+    return g.value
+
+
+def hr_gauge_free(g: int) -> None:
+    _lib.hr_gauge_free(g)
+
+
+def hr_gauge_data(g: int) -> int:
+    return _lib.hr_gauge_data(g) or 0
+
+
+def hr_gauge_import(g: int, canon, canon_prec: int, stream: int = 0) -> None:
+    _check(_lib.hr_gauge_import(g, _ptr(canon), canon_prec, stream))
+
+
+def hr_gauge_export(g: int, canon, canon_prec: int, stream: int = 0) -> None:
+    _check(_lib.hr_gauge_export(g, _ptr(canon), canon_prec, stream))
+
+
+def hr_spinor_import(ctx: int, dst_dev, prec: int, canon, canon_prec: int, parity: int, stream: int = 0) -> None:
+    _check(_lib.hr_spinor_import(ctx, _ptr(dst_dev), prec, _ptr(canon), canon_prec, parity, stream))
+
+
+def hr_spinor_export(ctx: int, src_dev, prec: int, canon, canon_prec: int, parity: int, stream: int = 0) -> None:
+    _check(_lib.hr_spinor_export(ctx, _ptr(src_dev), prec, _ptr(canon), canon_prec, parity, stream))
+
+
+def hr_represent_links(repr_out: int, fund_in: int, stream: int = 0) -> None:
+    _check(_lib.hr_represent_links(repr_out, fund_in, stream))
+
+
+def hr_dphi_eo(out, inp, links: int, parity: int, stream: int = 0) -> None:
+    _check(_lib.hr_dphi_eo(_ptr(out), _ptr(inp), links, parity, stream))
+
+
+def hr_dirac(m0: float, out_full, in_full, links: int, stream: int = 0) -> None:
+    _check(_lib.hr_dirac(float(m0), _ptr(out_full), _ptr(in_full), links, stream))
+
+
+def hr_dphi_eo_host(ctx: int, out_canon, in_canon, canon_prec: int, links: int, parity: int, stream: int = 0) -> None:
+    _check(_lib.hr_dphi_eo_host(ctx, _ptr(out_canon), _ptr(in_canon), canon_prec, links, parity, stream))
+
+
+def hr_ctx_set_tuning(ctx: int, key: str, value: int) -> None:
+    _check(_lib.hr_ctx_set_tuning(ctx, key.encode(), int(value)))
+
+
+def hr_dphi_variant_name(ctx: int, prec: int) -> str:
+    return _lib.hr_dphi_variant_name(ctx, prec).decode()
+
+
+# ---- convenience wrapper (handles + torch device memory; no arithmetic) ------------------------
+
+_NP_REAL = {HR_F64: np.float64, HR_F32: np.float32}
+_NP_CPLX = {HR_F64: np.complex128, HR_F32: np.complex64}
+
+
+class Lattice:
+    """Owns an hr_ctx and its gauge handles; spinors are torch uint8 tensors in the internal layout."""
+
+    def __init__(self, dims, bc=(-1, 1, 1, 1), N: int = 3, rep="fund", device: int = 0):
+        import torch  # device memory and streams only
+
+        self._torch = torch
+        self.dims = tuple(int(v) for v in dims)
+        self.bc = tuple(int(v) for v in bc)
+        self.N = N
+        self.rep = REP_NAMES[rep] if isinstance(rep, str) else int(rep)
+        self.device = device
+        self.ctx = hr_ctx_create(self.dims, self.bc, N, self.rep, device)
+        self.d = hr_rep_dim(self.ctx)
+        self.real_links = bool(hr_links_are_real(self.ctx))
+        self.vh = hr_half_volume(self.ctx)
+        self._gauges = []
+
+    # -- plumbing
+    def stream(self) -> int:
+        return int(self._torch.cuda.current_stream(self.device).cuda_stream)
+
+    def close(self) -> None:
+        for g in self._gauges:
+            hr_gauge_free(g["handle"])
+        self._gauges = []
+        if self.ctx:
+            hr_ctx_destroy(self.ctx)
+            self.ctx = 0
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- fields
+    def gauge(self, represented: bool, prec: int) -> int:
+        """hr_gauge_alloc on torch-owned device memory; returns the handle."""
+        nbytes = hr_gauge_bytes(self.ctx, int(represented), prec)
+        mem = self._torch.empty(nbytes, dtype=self._torch.uint8, device=f"cuda:{self.device}")
+        h = hr_gauge_alloc(self.ctx, int(represented), prec, mem)
+        self._gauges.append({"handle": h, "mem": mem})
+        return h
+
+    def spinor(self, prec: int, full: bool = False):
+        nbytes = hr_spinor_bytes(self.ctx, prec) * (2 if full else 1)
+        return self._torch.empty(nbytes, dtype=self._torch.uint8, device=f"cuda:{self.device}")
+
+    def import_gauge(self, g: int, canon: np.ndarray) -> None:
+        prec = HR_F64 if canon.dtype in (np.complex128, np.float64) else HR_F32
+        hr_gauge_import(g, np.ascontiguousarray(canon), prec, self.stream())
+
+    def export_gauge(self, g: int, represented: bool, prec: int = HR_F64) -> np.ndarray:
+        V = 2 * self.vh
+        if represented and self.real_links:
+            out = np.empty((V, 4, self.d, self.d), dtype=_NP_REAL[prec])
+        else:
+            n = self.d if represented else self.N
+            out = np.empty((V, 4, n, n), dtype=_NP_CPLX[prec])
+        hr_gauge_export(g, out, prec, self.stream())
+        return out
+
+    def import_spinor(self, dst, prec: int, canon: np.ndarray, parity: int) -> None:
+        cprec = HR_F64 if canon.dtype == np.complex128 else HR_F32
+        hr_spinor_import(self.ctx, dst, prec, np.ascontiguousarray(canon), cprec, parity, self.stream())
+
+    def export_spinor(self, src, prec: int, parity: int, out_prec: int = HR_F64) -> np.ndarray:
+        out = np.empty((self.vh, 4, self.d), dtype=_NP_CPLX[out_prec])
+        hr_spinor_export(self.ctx, src, prec, out, out_prec, parity, self.stream())
+        return out
+
+    # -- the hot path
+    def represent_links(self, repr_out: int, fund_in: int) -> None:
+        hr_represent_links(repr_out, fund_in, self.stream())
+
+    def dphi_eo(self, out, inp, links: int, parity: int) -> None:
+        hr_dphi_eo(out, inp, links, parity, self.stream())
+
+    def dirac(self, m0: float, out_full, in_full, links: int) -> None:
+        hr_dirac(m0, out_full, in_full, links, self.stream())
+
+    def set_tuning(self, key: str, value: int) -> None:
+        hr_ctx_set_tuning(self.ctx, key, value)
+
+    def variant_name(self, prec: int) -> str:
+        return hr_dphi_variant_name(self.ctx, prec)

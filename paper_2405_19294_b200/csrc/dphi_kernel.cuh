@@ -1,0 +1,285 @@
+// dphi_kernel.cuh -- the even-odd Wilson hopping term for sm_100a.
+//
+//   out(x) = -1/2 sum_mu [ (1-gamma_mu) s+ U_mu(x) psi(x+mu) + (1+gamma_mu) s- U_mu(x-mu)^dag psi(x-mu) ]
+//            (+ (4+m0) psi(x) when MASS)                                  BASELINE.json:north_star
+//
+// Design:
+//  * a3  site -> coordinates -> 8 neighbour half-indices and seam signs by integer arithmetic in the
+//        kernel; no neighbour tables, no halo (north_star: "periodic/antiperiodic boundaries resolved by
+//        in-kernel index arithmetic").
+//  * a4  spin projection to a half spinor BEFORE the colour multiply (the paper's half-spinor idea,
+//        PAPER.md:64, moved inside the kernel).  In the chiral basis of reading C1 every projector has
+//        the form   h_k = psi_k + c_k psi_{p(k)},  k = 0,1,  c_k in {+-1, +-i},
+//        and the reconstruction is   out_k += chi_k,  out_{p(k)} += conj(c_k) chi_k :
+//            mu   p(0) p(1)   c_0 (forward)  c_1 (forward)       (backward: both negated)
+//            0     2    3        1              1
+//            1     3    2        i              i
+//            2     3    2        1             -1
+//            3     2    3        i             -i
+//        so the whole spin algebra is additions; the seam sign rides on the FMA that accumulates chi.
+//  * a5  colour multiply chi_k = U h_k / U^dagger h_k with the d_R x d_R link (real for the adjoint),
+//        fully unrolled on compile-time D.
+//  * a6  accumulate, scale by -1/2, optional (4+m0) psi(x), store.
+//  * KSPLIT = 1: one thread per site.  KSPLIT = 2: two threads per site, thread k owns half-spinor
+//        component k (loads psi_k and psi_{p(k)}: no redundant spinor traffic; both lanes read the same
+//        link addresses, which the coalescer merges) -- the register-pressure answer to the paper's
+//        large-N_f problem at d_R >= 6.
+//  * loads are 128-bit, coalesced over the half index (hr_internal.h); links are streamed past L1
+//        (and optionally evict-first in L2), neighbour spinors are left to L1/L2 for re-use.
+#pragma once
+#include "hr_internal.h"
+
+namespace hr {
+
+template <int CRE, int CIM, typename Real>
+__device__ __forceinline__ void add_c(Real &ore, Real &oim, Real are, Real aim, Real bre, Real bim, Real sk)
+{
+    // o = a + sk * c * b,  c = CRE + i CIM, exactly one of CRE, CIM non-zero, sk = +-1 (real)
+    if constexpr (CRE != 0) {
+        ore = fma((Real)CRE * sk, bre, are);
+        oim = fma((Real)CRE * sk, bim, aim);
+    } else {
+        ore = fma((Real)(-CIM) * sk, bim, are);
+        oim = fma((Real)CIM * sk, bre, aim);
+    }
+}
+
+template <int CRE, int CIM, typename Real>
+__device__ __forceinline__ void acc_conj_c(Real &ore, Real &oim, Real xre, Real xim, Real w)
+{
+    // o += w * conj(c) * x,  conj(c) = CRE - i CIM
+    if constexpr (CRE != 0) {
+        ore = fma((Real)CRE * w, xre, ore);
+        oim = fma((Real)CRE * w, xim, oim);
+    } else {
+        ore = fma((Real)CIM * w, xim, ore);
+        oim = fma((Real)(-CIM) * w, xre, oim);
+    }
+}
+
+// chi = U h (DAG = false) or U^dagger h (DAG = true); U complex [D][D] (re,im) or real [D][D]
+template <int D, bool RL, bool DAG, typename Real>
+__device__ __forceinline__ void colour_mul(Real (&chi)[2 * D], const Real *u, const Real (&h)[2 * D])
+{
+#pragma unroll
+    for (int i = 0; i < D; ++i) {
+        Real re = 0, im = 0;
+#pragma unroll
+        for (int j = 0; j < D; ++j) {
+            if constexpr (RL) {
+                const Real r = DAG ? u[j * D + i] : u[i * D + j];
+                re = fma(r, h[2 * j], re);
+                im = fma(r, h[2 * j + 1], im);
+            } else {
+                const int e = DAG ? 2 * (j * D + i) : 2 * (i * D + j);
+                const Real ur = u[e], ui = u[e + 1];
+                if constexpr (!DAG) {
+                    re = fma(ur, h[2 * j], re);
+                    re = fma(-ui, h[2 * j + 1], re);
+                    im = fma(ur, h[2 * j + 1], im);
+                    im = fma(ui, h[2 * j], im);
+                } else {
+                    re = fma(ur, h[2 * j], re);
+                    re = fma(ui, h[2 * j + 1], re);
+                    im = fma(ur, h[2 * j + 1], im);
+                    im = fma(-ui, h[2 * j], im);
+                }
+            }
+        }
+        chi[2 * i] = re;
+        chi[2 * i + 1] = im;
+    }
+}
+
+// one half-spinor component of one hop:  h = a + sk c0 b ; chi = U(^dag) h ; outK += sgn chi ;
+// outP += sgn sk conj(c0) chi.   c0 = (DIR ? -1 : +1) * (MU in {0,2} ? 1 : i)
+template <int MU, int DIR, int D, bool RL, typename Real>
+__device__ __forceinline__ void hop_component(const Real *u, const Real *a, const Real *b, Real sk, Real sgn,
+                                              Real *outK, Real *outP)
+{
+    constexpr int S = DIR ? -1 : 1;
+    constexpr int CRE = (MU == 0 || MU == 2) ? S : 0;
+    constexpr int CIM = (MU == 0 || MU == 2) ? 0 : S;
+    Real h[2 * D], chi[2 * D];
+#pragma unroll
+    for (int c = 0; c < D; ++c) add_c<CRE, CIM>(h[2 * c], h[2 * c + 1], a[2 * c], a[2 * c + 1], b[2 * c], b[2 * c + 1], sk);
+    colour_mul<D, RL, DIR == 1>(chi, u, h);
+    const Real w = sgn * sk;
+#pragma unroll
+    for (int c = 0; c < D; ++c) {
+        outK[2 * c] = fma(sgn, chi[2 * c], outK[2 * c]);
+        outK[2 * c + 1] = fma(sgn, chi[2 * c + 1], outK[2 * c + 1]);
+        acc_conj_c<CRE, CIM>(outP[2 * c], outP[2 * c + 1], chi[2 * c], chi[2 * c + 1], w);
+    }
+}
+
+struct SiteGeom {
+    int t, x, y, zh, b; // b = offset bit: z = 2*zh + b
+};
+
+// neighbour half index and seam sign of the hop (MU, DIR) from the site with half index s
+template <int MU, int DIR>
+__device__ __forceinline__ void neighbour(const DphiArgs &a, const SiteGeom &g, long s, long &sn, int &sign)
+{
+    const long sy = a.Zh, sx = (long)a.Y * a.Zh, st = (long)a.X * a.Y * a.Zh;
+    if constexpr (MU == 0) {
+        if constexpr (DIR == 0) { const bool w = g.t == a.T - 1; sn = w ? s - (a.T - 1) * st : s + st; sign = w ? a.bc[0] : 1; }
+        else                    { const bool w = g.t == 0;       sn = w ? s + (a.T - 1) * st : s - st; sign = w ? a.bc[0] : 1; }
+    } else if constexpr (MU == 1) {
+        if constexpr (DIR == 0) { const bool w = g.x == a.X - 1; sn = w ? s - (a.X - 1) * sx : s + sx; sign = w ? a.bc[1] : 1; }
+        else                    { const bool w = g.x == 0;       sn = w ? s + (a.X - 1) * sx : s - sx; sign = w ? a.bc[1] : 1; }
+    } else if constexpr (MU == 2) {
+        if constexpr (DIR == 0) { const bool w = g.y == a.Y - 1; sn = w ? s - (a.Y - 1) * sy : s + sy; sign = w ? a.bc[2] : 1; }
+        else                    { const bool w = g.y == 0;       sn = w ? s + (a.Y - 1) * sy : s - sy; sign = w ? a.bc[2] : 1; }
+    } else {
+        // z = 2 zh + b; the neighbour row has offset bit 1-b
+        if constexpr (DIR == 0) {
+            const bool w = g.zh == a.Zh - 1;
+            sn = g.b ? (w ? s - (a.Zh - 1) : s + 1) : s;
+            sign = (g.b && w) ? a.bc[3] : 1;
+        } else {
+            const bool w = g.zh == 0;
+            sn = g.b ? s : (w ? s + (a.Zh - 1) : s - 1);
+            sign = (!g.b && w) ? a.bc[3] : 1;
+        }
+    }
+}
+
+template <typename Real, int D, bool RL, int KSPLIT, bool MASS, int LHINT, int SHINT, int STHINT, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
+{
+    constexpr int LNREAL = RL ? D * D : 2 * D * D;        // reals per link
+    constexpr int RPV = 16 / (int)sizeof(Real);
+    constexpr int SPV = 2 * D / RPV;                       // 16-byte vectors per spin component
+    static_assert(KSPLIT == 1 || (2 * D) % RPV == 0, "KSPLIT=2 needs vector-aligned spin components");
+    constexpr size_t LB = (size_t)LNREAL * sizeof(Real);  // link bytes per site
+
+    const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    long s = tid / KSPLIT;
+    const int k = (int)(tid % KSPLIT);
+    const bool live = s < a.vh;
+    if (!live) s = a.vh - 1; // keep the pair convergent for the final shuffle; stores are predicated
+
+    SiteGeom g;
+    {
+        long r = s;
+        g.zh = (int)(r % a.Zh); r /= a.Zh;
+        g.y = (int)(r % a.Y); r /= a.Y;
+        g.x = (int)(r % a.X);
+        g.t = (int)(r / a.X);
+        g.b = (g.t + g.x + g.y + a.parity) & 1;
+    }
+    const size_t vh = (size_t)a.vh;
+    const size_t pb = vh * 16; // plane bytes
+    const char *in = (const char *)a.in;
+    const char *lk_own = (const char *)a.links + (size_t)(a.parity * 4) * LB * vh;       // links based at output parity
+    const char *lk_nbr = (const char *)a.links + (size_t)((1 - a.parity) * 4) * LB * vh; // links based at input parity
+
+    uint64_t pol_l = 0, pol_s = 0;
+    if constexpr (LHINT == LD_STREAM_EF) pol_l = make_policy_evict_first();
+    if constexpr (SHINT == LD_KEEP) pol_s = make_policy_evict_last();
+
+    if constexpr (KSPLIT == 1) {
+        Real acc[4][2 * D];
+#pragma unroll
+        for (int al = 0; al < 4; ++al)
+#pragma unroll
+            for (int c = 0; c < 2 * D; ++c) acc[al][c] = 0;
+
+        auto hop = [&](auto mu_c, auto dir_c) {
+            constexpr int MU = decltype(mu_c)::value;
+            constexpr int DIR = decltype(dir_c)::value;
+            long sn; int sign;
+            neighbour<MU, DIR>(a, g, s, sn, sign);
+            Real psi[8 * D];
+            load_record<SHINT, 8 * D>(psi, in, vh, (size_t)sn, pol_s);
+            Real u[LNREAL];
+            if constexpr (DIR == 0) load_record<LHINT, LNREAL>(u, lk_own + (size_t)MU * LB * vh, vh, (size_t)s, pol_l);
+            else                    load_record<LHINT, LNREAL>(u, lk_nbr + (size_t)MU * LB * vh, vh, (size_t)sn, pol_l);
+            constexpr int P0 = (MU == 0 || MU == 3) ? 2 : 3;
+            constexpr int P1 = 5 - P0;
+            const Real sg = (Real)sign;
+            hop_component<MU, DIR, D, RL, Real>(u, psi + 0 * 2 * D, psi + P0 * 2 * D, (Real)1, sg, acc[0], acc[P0]);
+            hop_component<MU, DIR, D, RL, Real>(u, psi + 1 * 2 * D, psi + P1 * 2 * D, (Real)(MU >= 2 ? -1 : 1), sg, acc[1], acc[P1]);
+        };
+        using I0 = std::integral_constant<int, 0>; using I1 = std::integral_constant<int, 1>;
+        using I2 = std::integral_constant<int, 2>; using I3 = std::integral_constant<int, 3>;
+        hop(I0{}, I0{}); hop(I0{}, I1{});
+        hop(I1{}, I0{}); hop(I1{}, I1{});
+        hop(I2{}, I0{}); hop(I2{}, I1{});
+        hop(I3{}, I0{}); hop(I3{}, I1{});
+
+        Real o[8 * D];
+        if constexpr (MASS) {
+            Real self[8 * D];
+            load_record<LD_STREAM, 8 * D>(self, (const char *)a.self, vh, (size_t)s, 0);
+            const Real m = (Real)a.mass;
+#pragma unroll
+            for (int al = 0; al < 4; ++al)
+#pragma unroll
+                for (int c = 0; c < 2 * D; ++c) o[al * 2 * D + c] = fma(m, self[al * 2 * D + c], (Real)-0.5 * acc[al][c]);
+        } else {
+#pragma unroll
+            for (int al = 0; al < 4; ++al)
+#pragma unroll
+                for (int c = 0; c < 2 * D; ++c) o[al * 2 * D + c] = (Real)-0.5 * acc[al][c];
+        }
+        if (live) store_planes<STHINT, 8 * D / RPV>((char *)a.out + (size_t)s * 16, pb, o);
+    } else {
+        // two threads per site: thread k owns h_k.  accK -> out_k, accP -> out_{k+2} (mu = 0,3),
+        // accQ -> out_{3-k} (mu = 1,2), exchanged with the partner lane at the end.
+        Real accK[2 * D], accP[2 * D], accQ[2 * D];
+#pragma unroll
+        for (int c = 0; c < 2 * D; ++c) { accK[c] = 0; accP[c] = 0; accQ[c] = 0; }
+
+        auto hop = [&](auto mu_c, auto dir_c) {
+            constexpr int MU = decltype(mu_c)::value;
+            constexpr int DIR = decltype(dir_c)::value;
+            long sn; int sign;
+            neighbour<MU, DIR>(a, g, s, sn, sign);
+            constexpr bool STRAIGHT = (MU == 0 || MU == 3);
+            const int pk = STRAIGHT ? k + 2 : 3 - k;
+            Real pa[2 * D], pbv[2 * D];
+            const char *base = in + (size_t)sn * 16;
+            load_planes<SHINT, SPV>(pa, base + (size_t)(k * SPV) * pb, pb, pol_s);
+            load_planes<SHINT, SPV>(pbv, base + (size_t)(pk * SPV) * pb, pb, pol_s);
+            Real u[LNREAL];
+            if constexpr (DIR == 0) load_record<LHINT, LNREAL>(u, lk_own + (size_t)MU * LB * vh, vh, (size_t)s, pol_l);
+            else                    load_record<LHINT, LNREAL>(u, lk_nbr + (size_t)MU * LB * vh, vh, (size_t)sn, pol_l);
+            const Real sk = (MU >= 2 && k == 1) ? (Real)-1 : (Real)1;
+            hop_component<MU, DIR, D, RL, Real>(u, pa, pbv, sk, (Real)sign, accK, STRAIGHT ? accP : accQ);
+        };
+        using I0 = std::integral_constant<int, 0>; using I1 = std::integral_constant<int, 1>;
+        using I2 = std::integral_constant<int, 2>; using I3 = std::integral_constant<int, 3>;
+        hop(I0{}, I0{}); hop(I0{}, I1{});
+        hop(I1{}, I0{}); hop(I1{}, I1{});
+        hop(I2{}, I0{}); hop(I2{}, I1{});
+        hop(I3{}, I0{}); hop(I3{}, I1{});
+
+#pragma unroll
+        for (int c = 0; c < 2 * D; ++c) accP[c] += __shfl_xor_sync(0xffffffffu, accQ[c], 1);
+
+        if constexpr (MASS) {
+            Real sa[2 * D], sb[2 * D];
+            const char *base = (const char *)a.self + (size_t)s * 16;
+            load_planes<LD_STREAM, SPV>(sa, base + (size_t)(k * SPV) * pb, pb, 0);
+            load_planes<LD_STREAM, SPV>(sb, base + (size_t)((k + 2) * SPV) * pb, pb, 0);
+            const Real m = (Real)a.mass;
+#pragma unroll
+            for (int c = 0; c < 2 * D; ++c) {
+                accK[c] = fma(m, sa[c], (Real)-0.5 * accK[c]);
+                accP[c] = fma(m, sb[c], (Real)-0.5 * accP[c]);
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < 2 * D; ++c) { accK[c] *= (Real)-0.5; accP[c] *= (Real)-0.5; }
+        }
+        if (live) {
+            char *ob = (char *)a.out + (size_t)s * 16;
+            store_planes<STHINT, SPV>(ob + (size_t)(k * SPV) * pb, pb, accK);
+            store_planes<STHINT, SPV>(ob + (size_t)((k + 2) * SPV) * pb, pb, accP);
+        }
+    }
+}
+
+} // namespace hr

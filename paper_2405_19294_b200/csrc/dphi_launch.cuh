@@ -1,0 +1,91 @@
+// dphi_launch.cuh -- variant table + launcher for one (Real, D, real-link) combination.
+// Each dphi_inst_*.cu includes this and instantiates launch_dphi_t for its combination, so the
+// combinations compile in parallel.
+#pragma once
+#include <type_traits>
+
+#include "dphi_kernel.cuh"
+
+namespace hr {
+
+// Kernel variants (hr_ctx_set_tuning "variant"); names are what bench.py / profiles report.
+//   0 site      one thread per site, links streamed past L1
+//   1 site_ef   + links evict-first in L2, neighbour spinors evict-last (large volumes)
+//   2 pair      two threads per site (one per half-spinor component)
+//   3 pair_ef   pair + the L2 policies of 1
+//   4 site_l1   one thread per site, links through L1 as well (baseline for the cache-policy evidence)
+enum { DPHI_NVARIANTS = 5 };
+static const char *const kDphiVariantNames[DPHI_NVARIANTS] = { "site", "site_ef", "pair", "pair_ef", "site_l1" };
+
+// registers: __launch_bounds__(MAXT, MINB) caps them at 65536 / (MAXT*MINB)
+template <typename Real, int D, bool RL, int KSPLIT> struct Tune {
+    static constexpr int LNREAL = RL ? D * D : 2 * D * D;
+    // live values of a thread, in 32-bit registers (accumulators + one spinor/half + one link)
+    static constexpr int W = (int)sizeof(Real) / 4;
+    static constexpr int LIVE = W * ((KSPLIT == 1 ? 8 * D : 6 * D) + (KSPLIT == 1 ? 8 * D : 4 * D) + LNREAL) + 40;
+    static constexpr int MAXT = 128;
+    static constexpr int MINB = LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? 4 : LIVE <= 168 ? 3 : LIVE <= 255 ? 2 : 1;
+};
+
+template <typename Real, int D, bool RL, int KSPLIT, bool MASS, int LHINT, int SHINT, int STHINT>
+static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
+{
+    using T = Tune<Real, D, RL, KSPLIT>;
+    if (block <= 0) block = T::MAXT;
+    if (block > T::MAXT || (block % 32) != 0) {
+        set_error("block=%d not supported by this variant (multiple of 32, <= %d)", block, T::MAXT);
+        return HR_EINVAL;
+    }
+    const long nthreads = a.vh * KSPLIT;
+    const long grid = (nthreads + block - 1) / block;
+    dphi_kernel<Real, D, RL, KSPLIT, MASS, LHINT, SHINT, STHINT, T::MAXT, T::MINB><<<(unsigned)grid, block, 0, st>>>(a);
+    count_launch();
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) {
+        set_error("dphi kernel launch failed: %s", cudaGetErrorString(e));
+        return HR_ECUDA;
+    }
+    return HR_OK;
+}
+
+template <typename Real, int D, bool RL, bool MASS>
+static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaStream_t st)
+{
+    constexpr int RPV = 16 / (int)sizeof(Real);
+    constexpr bool PAIR_OK = (2 * D) % RPV == 0;
+    switch (variant) {
+    case 0: return launch_one<Real, D, RL, 1, MASS, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+    case 1: return launch_one<Real, D, RL, 1, MASS, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
+    case 2:
+        if constexpr (PAIR_OK) return launch_one<Real, D, RL, 2, MASS, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+        break;
+    case 3:
+        if constexpr (PAIR_OK) return launch_one<Real, D, RL, 2, MASS, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
+        break;
+    case 4: return launch_one<Real, D, RL, 1, MASS, LD_DEFAULT, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+    default: break;
+    }
+    set_error("dphi variant %d not available for d_R=%d, %s", variant, D, sizeof(Real) == 8 ? "fp64" : "fp32");
+    return HR_EUNSUPPORTED;
+}
+
+template <typename Real, int D, bool RL>
+hr_status launch_dphi_t(int variant, int block, const DphiArgs &a, cudaStream_t st)
+{
+    if (a.self) return launch_variant<Real, D, RL, true>(variant, block, a, st);
+    return launch_variant<Real, D, RL, false>(variant, block, a, st);
+}
+
+template <typename Real, int D, bool RL> bool dphi_variant_ok_t(int variant)
+{
+    constexpr int RPV = 16 / (int)sizeof(Real);
+    if (variant < 0 || variant >= DPHI_NVARIANTS) return false;
+    if ((variant == 2 || variant == 3) && (2 * D) % RPV != 0) return false;
+    return true;
+}
+
+#define HR_DPHI_INSTANCE(Real, D, RL)                                                                    \
+    template hr_status launch_dphi_t<Real, D, RL>(int, int, const DphiArgs &, cudaStream_t);             \
+    template bool dphi_variant_ok_t<Real, D, RL>(int);
+
+} // namespace hr

@@ -1,0 +1,417 @@
+// hr_api.cu -- the C-ABI boundary of libhr (include/hr.h): argument checking, handles, canonical
+// import/export, and the three compute calls.  Every step of the path runs in the kernels of this
+// library; there is no CPU fallback (a missing/unusable CUDA device makes every compute call fail
+// with HR_ECUDA).
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "hr_internal.h"
+
+namespace hr {
+
+static thread_local char g_err[512] = "";
+static std::atomic<unsigned long long> g_launches{0};
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+void count_launch(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
+
+static hr_status cuda_fail(const char *what, cudaError_t e)
+{
+    set_error("%s: %s", what, cudaGetErrorString(e));
+    return e == cudaErrorMemoryAllocation ? HR_ENOMEM : HR_ECUDA;
+}
+#define HR_CUDA(call)                                                                                     \
+    do {                                                                                                  \
+        cudaError_t e_ = (call);                                                                          \
+        if (e_ != cudaSuccess) return cuda_fail(#call, e_);                                               \
+    } while (0)
+
+static int rep_dim(int N, int rep)
+{
+    switch (rep) {
+    case HR_REP_FUND: return N;
+    case HR_REP_ADJ: return N * N - 1;
+    case HR_REP_SYM: return N * (N + 1) / 2;
+    case HR_REP_ASYM: return N * (N - 1) / 2;
+    default: return -1;
+    }
+}
+
+static bool combo_supported(int N, int rep)
+{
+    switch (N) {
+    case 2: return rep == HR_REP_FUND || rep == HR_REP_ADJ || rep == HR_REP_SYM;
+    case 3: return rep == HR_REP_FUND || rep == HR_REP_ADJ || rep == HR_REP_SYM || rep == HR_REP_ASYM;
+    case 4: return rep == HR_REP_FUND || rep == HR_REP_ASYM;
+    default: return false;
+    }
+}
+
+static bool valid_prec(int p) { return p == HR_F64 || p == HR_F32; }
+
+// is `p` device-accessible memory (device or managed)?  Host (pinned or pageable) -> false.
+static hr_status pointer_on_device(const void *p, bool *dev)
+{
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return cuda_fail("cudaPointerGetAttributes", e);
+    }
+    *dev = (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged);
+    return HR_OK;
+}
+
+static hr_status use_device(const hr_ctx *c)
+{
+    cudaError_t e = cudaSetDevice(c->device);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return cuda_fail("cudaSetDevice (no usable CUDA device; libhr has no CPU fallback)", e);
+    }
+    return HR_OK;
+}
+
+// Staging chunk for host canonical arrays: at most this many bytes of canonical data per copy.
+static const size_t kStageBytes = (size_t)256 << 20;
+
+enum FieldKind { FIELD_GAUGE, FIELD_SPINOR };
+
+// canonical (host or device) <-> internal.  `nsites_total` = sites of the canonical array
+// (gauge: V full-lattice sites, 4 records each; spinor: Vh half-lattice sites of `parity`).
+static hr_status transfer(const hr_ctx *c, FieldKind kind, bool import, int nreal, void *internal, hr_prec prec,
+                          void *canon, hr_prec cprec, cudaStream_t st)
+{
+    hr_status rc = use_device(c);
+    if (rc != HR_OK) return rc;
+    bool dev = false;
+    rc = pointer_on_device(canon, &dev);
+    if (rc != HR_OK) return rc;
+    const long nsites = kind == FIELD_GAUGE ? c->V : c->Vh;
+    const size_t site_bytes = (size_t)(kind == FIELD_GAUGE ? 4 : 1) * nreal * prec_bytes(cprec);
+
+    auto run = [&](void *canon_dev, long first, long n) -> hr_status {
+        if (kind == FIELD_GAUGE)
+            return import ? launch_pack_gauge(c, nreal, internal, prec, canon_dev, cprec, first, n, st)
+                          : launch_unpack_gauge(c, nreal, internal, prec, canon_dev, cprec, first, n, st);
+        return import ? launch_pack_spinor(c, internal, prec, canon_dev, cprec, first, n, st)
+                      : launch_unpack_spinor(c, internal, prec, canon_dev, cprec, first, n, st);
+    };
+    if (dev) return run(canon, 0, nsites);
+
+    // host canonical array: stage through device memory in chunks (set-up path)
+    long chunk = (long)(kStageBytes / site_bytes);
+    if (chunk < 1) chunk = 1;
+    if (chunk > nsites) chunk = nsites;
+    void *stage = nullptr;
+    HR_CUDA(cudaMalloc(&stage, (size_t)chunk * site_bytes));
+    hr_status out = HR_OK;
+    for (long first = 0; first < nsites && out == HR_OK; first += chunk) {
+        const long n = (nsites - first < chunk) ? nsites - first : chunk;
+        char *h = (char *)canon + (size_t)first * site_bytes;
+        cudaError_t e = cudaSuccess;
+        if (import) {
+            e = cudaMemcpyAsync(stage, h, (size_t)n * site_bytes, cudaMemcpyHostToDevice, st);
+            if (e == cudaSuccess) out = run(stage, first, n);
+        } else {
+            out = run(stage, first, n);
+            if (out == HR_OK) e = cudaMemcpyAsync(h, stage, (size_t)n * site_bytes, cudaMemcpyDeviceToHost, st);
+        }
+        if (e == cudaSuccess && out == HR_OK) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) out = cuda_fail("staged canonical copy", e);
+    }
+    cudaFree(stage);
+    return out;
+}
+
+} // namespace hr
+
+using namespace hr;
+
+extern "C" {
+
+const char *hr_version(void) { return "hr-dphi 0.1 (sm_100a)"; }
+const char *hr_last_error(void) { return g_err; }
+unsigned long long hr_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N, hr_rep rep, int device)
+{
+    if (!ctx || !dims || !bc) { set_error("hr_ctx_create: NULL argument"); return HR_EINVAL; }
+    *ctx = nullptr;
+    for (int m = 0; m < 4; ++m) {
+        if (dims[m] < 2 || (dims[m] & 1)) {
+            set_error("hr_ctx_create: dims[%d]=%d must be even and >= 2 (reading C11)", m, dims[m]);
+            return HR_EINVAL;
+        }
+        if (bc[m] != 1 && bc[m] != -1) { set_error("hr_ctx_create: bc[%d]=%d must be +1 or -1", m, bc[m]); return HR_EINVAL; }
+    }
+    if ((int)rep < 0 || (int)rep > 3) { set_error("hr_ctx_create: unknown representation %d", (int)rep); return HR_EINVAL; }
+    if (device < 0) { set_error("hr_ctx_create: device=%d", device); return HR_EINVAL; }
+    if (!combo_supported(N, rep)) {
+        set_error("hr_ctx_create: SU(%d) representation %d is not instantiated", N, (int)rep);
+        return HR_EUNSUPPORTED;
+    }
+    const double vol = (double)dims[0] * dims[1] * dims[2] * dims[3];
+    if (vol > 2.0e9) { set_error("hr_ctx_create: volume %.3g exceeds the 2^31 index range", vol); return HR_EINVAL; }
+    hr_ctx *c = new (std::nothrow) hr_ctx();
+    if (!c) { set_error("hr_ctx_create: out of host memory"); return HR_ENOMEM; }
+    for (int m = 0; m < 4; ++m) { c->dims[m] = dims[m]; c->bc[m] = bc[m]; }
+    c->N = N;
+    c->rep = (int)rep;
+    c->d = rep_dim(N, rep);
+    c->real_links = (rep == HR_REP_ADJ);
+    c->device = device;
+    c->V = (long)dims[0] * dims[1] * dims[2] * dims[3];
+    c->Vh = c->V / 2;
+    c->variant = -1;
+    c->block = 0;
+    c->ws_in = c->ws_out = c->ws_stage = nullptr;
+    c->ws_spinor_bytes = c->ws_stage_bytes = 0;
+    c->ws_prec = -1;
+    *ctx = c;
+    return HR_OK;
+}
+
+void hr_ctx_destroy(hr_ctx *ctx)
+{
+    if (!ctx) return;
+    if (ctx->ws_in || ctx->ws_out || ctx->ws_stage) {
+        if (cudaSetDevice(ctx->device) == cudaSuccess) {
+            cudaFree(ctx->ws_in);
+            cudaFree(ctx->ws_out);
+            cudaFree(ctx->ws_stage);
+        }
+        cudaGetLastError();
+    }
+    delete ctx;
+}
+
+int hr_rep_dim(const hr_ctx *ctx) { return ctx ? ctx->d : -1; }
+int hr_links_are_real(const hr_ctx *ctx) { return ctx ? ctx->real_links : -1; }
+size_t hr_half_volume(const hr_ctx *ctx) { return ctx ? (size_t)ctx->Vh : 0; }
+
+size_t hr_gauge_bytes(const hr_ctx *ctx, int represented, hr_prec prec)
+{
+    if (!ctx || !valid_prec(prec)) return 0;
+    return (size_t)ctx->V * 4 * link_nreal(ctx, represented) * prec_bytes(prec);
+}
+
+size_t hr_spinor_bytes(const hr_ctx *ctx, hr_prec prec)
+{
+    if (!ctx || !valid_prec(prec)) return 0;
+    return (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec);
+}
+
+hr_status hr_gauge_alloc(const hr_ctx *ctx, int represented, hr_prec prec, void *dev_mem, hr_gauge **out)
+{
+    if (!ctx || !out) { set_error("hr_gauge_alloc: NULL argument"); return HR_EINVAL; }
+    *out = nullptr;
+    if (!valid_prec(prec) || (represented != 0 && represented != 1)) {
+        set_error("hr_gauge_alloc: bad precision or `represented` flag");
+        return HR_EINVAL;
+    }
+    if (dev_mem && ((uintptr_t)dev_mem & 15)) { set_error("hr_gauge_alloc: dev_mem must be 16-byte aligned"); return HR_EINVAL; }
+    hr_gauge *g = new (std::nothrow) hr_gauge();
+    if (!g) { set_error("hr_gauge_alloc: out of host memory"); return HR_ENOMEM; }
+    g->ctx = ctx;
+    g->represented = represented;
+    g->prec = prec;
+    g->bytes = hr_gauge_bytes(ctx, represented, prec);
+    g->nreal = link_nreal(ctx, represented);
+    g->owns = 0;
+    g->data = dev_mem;
+    if (!dev_mem) {
+        hr_status rc = use_device(ctx);
+        if (rc != HR_OK) { delete g; return rc; }
+        cudaError_t e = cudaMalloc(&g->data, g->bytes);
+        if (e != cudaSuccess) { delete g; cudaGetLastError(); return cuda_fail("hr_gauge_alloc: cudaMalloc", e); }
+        g->owns = 1;
+    }
+    *out = g;
+    return HR_OK;
+}
+
+void hr_gauge_free(hr_gauge *g)
+{
+    if (!g) return;
+    if (g->owns && g->data) {
+        if (cudaSetDevice(g->ctx->device) == cudaSuccess) cudaFree(g->data);
+        cudaGetLastError();
+    }
+    delete g;
+}
+
+void *hr_gauge_data(const hr_gauge *g) { return g ? g->data : nullptr; }
+
+hr_status hr_gauge_import(hr_gauge *dst, const void *canon, hr_prec canon_prec, void *stream)
+{
+    if (!dst || !canon || !valid_prec(canon_prec)) { set_error("hr_gauge_import: bad argument"); return HR_EINVAL; }
+    return transfer(dst->ctx, FIELD_GAUGE, true, dst->nreal, dst->data, dst->prec, const_cast<void *>(canon), canon_prec,
+                    (cudaStream_t)stream);
+}
+
+hr_status hr_gauge_export(const hr_gauge *src, void *canon, hr_prec canon_prec, void *stream)
+{
+    if (!src || !canon || !valid_prec(canon_prec)) { set_error("hr_gauge_export: bad argument"); return HR_EINVAL; }
+    return transfer(src->ctx, FIELD_GAUGE, false, src->nreal, src->data, src->prec, canon, canon_prec, (cudaStream_t)stream);
+}
+
+hr_status hr_spinor_import(const hr_ctx *ctx, void *dst_dev, hr_prec prec, const void *canon, hr_prec canon_prec,
+                           int parity, void *stream)
+{
+    if (!ctx || !dst_dev || !canon || !valid_prec(prec) || !valid_prec(canon_prec) || (parity != 0 && parity != 1)) {
+        set_error("hr_spinor_import: bad argument");
+        return HR_EINVAL;
+    }
+    return transfer(ctx, FIELD_SPINOR, true, 8 * ctx->d, dst_dev, prec, const_cast<void *>(canon), canon_prec,
+                    (cudaStream_t)stream);
+}
+
+hr_status hr_spinor_export(const hr_ctx *ctx, const void *src_dev, hr_prec prec, void *canon, hr_prec canon_prec,
+                           int parity, void *stream)
+{
+    if (!ctx || !src_dev || !canon || !valid_prec(prec) || !valid_prec(canon_prec) || (parity != 0 && parity != 1)) {
+        set_error("hr_spinor_export: bad argument");
+        return HR_EINVAL;
+    }
+    return transfer(ctx, FIELD_SPINOR, false, 8 * ctx->d, const_cast<void *>(src_dev), prec, canon, canon_prec,
+                    (cudaStream_t)stream);
+}
+
+hr_status hr_represent_links(hr_gauge *repr_out, const hr_gauge *fund_in, void *stream)
+{
+    if (!repr_out || !fund_in) { set_error("hr_represent_links: NULL argument"); return HR_EINVAL; }
+    if (repr_out->ctx != fund_in->ctx) { set_error("hr_represent_links: fields belong to different contexts"); return HR_EINVAL; }
+    if (!repr_out->represented || fund_in->represented) {
+        set_error("hr_represent_links: need (represented out, fundamental in)");
+        return HR_EINVAL;
+    }
+    if (repr_out->data == fund_in->data) { set_error("hr_represent_links: out aliases in"); return HR_EINVAL; }
+    hr_status rc = use_device(fund_in->ctx);
+    if (rc != HR_OK) return rc;
+    return launch_represent(fund_in->ctx, fund_in->prec, fund_in->data, repr_out->prec, repr_out->data, (cudaStream_t)stream);
+}
+
+static hr_status dphi_args(DphiArgs &a, const hr_ctx *c, void *out, const void *in, const void *self, const hr_gauge *links,
+                           int parity, double mass)
+{
+    a.out = out;
+    a.in = in;
+    a.self = self;
+    a.links = links->data;
+    a.T = c->dims[0];
+    a.X = c->dims[1];
+    a.Y = c->dims[2];
+    a.Zh = c->dims[3] / 2;
+    a.parity = parity;
+    for (int m = 0; m < 4; ++m) a.bc[m] = c->bc[m];
+    a.vh = c->Vh;
+    a.mass = mass;
+    return HR_OK;
+}
+
+hr_status hr_dphi_eo(void *out, const void *in, const hr_gauge *links, int parity, void *stream)
+{
+    if (!out || !in || !links) { set_error("hr_dphi_eo: NULL argument"); return HR_EINVAL; }
+    if (parity != 0 && parity != 1) { set_error("hr_dphi_eo: parity=%d", parity); return HR_EINVAL; }
+    if (!links->represented) { set_error("hr_dphi_eo: `links` must be a represented field (hr_represent_links)"); return HR_EINVAL; }
+    if (out == in) { set_error("hr_dphi_eo: out aliases in"); return HR_EINVAL; }
+    if (((uintptr_t)out | (uintptr_t)in) & 15) { set_error("hr_dphi_eo: spinor buffers must be 16-byte aligned"); return HR_EINVAL; }
+    const hr_ctx *c = links->ctx;
+    hr_status rc = use_device(c);
+    if (rc != HR_OK) return rc;
+    DphiArgs a;
+    dphi_args(a, c, out, in, nullptr, links, parity, 0.0);
+    return launch_dphi(c, links->prec, a, (cudaStream_t)stream);
+}
+
+hr_status hr_dirac(double m0, void *out_full, const void *in_full, const hr_gauge *links, void *stream)
+{
+    if (!out_full || !in_full || !links) { set_error("hr_dirac: NULL argument"); return HR_EINVAL; }
+    if (!links->represented) { set_error("hr_dirac: `links` must be a represented field"); return HR_EINVAL; }
+    if (out_full == in_full) { set_error("hr_dirac: out aliases in"); return HR_EINVAL; }
+    if (((uintptr_t)out_full | (uintptr_t)in_full) & 15) { set_error("hr_dirac: spinor buffers must be 16-byte aligned"); return HR_EINVAL; }
+    const hr_ctx *c = links->ctx;
+    hr_status rc = use_device(c);
+    if (rc != HR_OK) return rc;
+    const size_t half = hr_spinor_bytes(c, links->prec);
+    for (int p = 0; p < 2; ++p) {
+        DphiArgs a;
+        char *o = (char *)out_full + (size_t)p * half;
+        const char *i_other = (const char *)in_full + (size_t)(1 - p) * half;
+        const char *i_self = (const char *)in_full + (size_t)p * half;
+        dphi_args(a, c, o, i_other, i_self, links, p, 4.0 + m0);
+        rc = launch_dphi(c, links->prec, a, (cudaStream_t)stream);
+        if (rc != HR_OK) return rc;
+    }
+    return HR_OK;
+}
+
+hr_status hr_dphi_eo_host(hr_ctx *ctx, void *out_canon, const void *in_canon, hr_prec canon_prec, const hr_gauge *links,
+                          int parity, void *stream)
+{
+    if (!ctx || !out_canon || !in_canon || !links || !valid_prec(canon_prec)) { set_error("hr_dphi_eo_host: bad argument"); return HR_EINVAL; }
+    if (links->ctx != ctx) { set_error("hr_dphi_eo_host: `links` belongs to a different context"); return HR_EINVAL; }
+    if (parity != 0 && parity != 1) { set_error("hr_dphi_eo_host: parity=%d", parity); return HR_EINVAL; }
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t sb = hr_spinor_bytes(ctx, links->prec);
+    const size_t cb = hr_spinor_bytes(ctx, canon_prec);
+    if (ctx->ws_prec != (int)links->prec || ctx->ws_spinor_bytes != sb || ctx->ws_stage_bytes < cb) {
+        cudaFree(ctx->ws_in); cudaFree(ctx->ws_out); cudaFree(ctx->ws_stage);
+        ctx->ws_in = ctx->ws_out = ctx->ws_stage = nullptr;
+        ctx->ws_prec = -1;
+        HR_CUDA(cudaMalloc(&ctx->ws_in, sb));
+        HR_CUDA(cudaMalloc(&ctx->ws_out, sb));
+        HR_CUDA(cudaMalloc(&ctx->ws_stage, cb));
+        ctx->ws_spinor_bytes = sb;
+        ctx->ws_stage_bytes = cb;
+        ctx->ws_prec = (int)links->prec;
+    }
+    HR_CUDA(cudaMemcpyAsync(ctx->ws_stage, in_canon, cb, cudaMemcpyHostToDevice, st));
+    rc = launch_pack_spinor(ctx, ctx->ws_in, links->prec, ctx->ws_stage, canon_prec, 0, ctx->Vh, st);
+    if (rc != HR_OK) return rc;
+    rc = hr_dphi_eo(ctx->ws_out, ctx->ws_in, links, parity, stream);
+    if (rc != HR_OK) return rc;
+    rc = launch_unpack_spinor(ctx, ctx->ws_out, links->prec, ctx->ws_stage, canon_prec, 0, ctx->Vh, st);
+    if (rc != HR_OK) return rc;
+    HR_CUDA(cudaMemcpyAsync(out_canon, ctx->ws_stage, cb, cudaMemcpyDeviceToHost, st));
+    HR_CUDA(cudaStreamSynchronize(st));
+    return HR_OK;
+}
+
+hr_status hr_ctx_set_tuning(hr_ctx *ctx, const char *key, int value)
+{
+    if (!ctx || !key) { set_error("hr_ctx_set_tuning: NULL argument"); return HR_EINVAL; }
+    if (!strcmp(key, "variant")) {
+        if (!dphi_variant_valid(ctx, value)) { set_error("hr_ctx_set_tuning: variant %d not available for d_R=%d", value, ctx->d); return HR_EINVAL; }
+        ctx->variant = value;
+        return HR_OK;
+    }
+    if (!strcmp(key, "block")) {
+        if (value < 0 || value > 1024 || (value % 32)) { set_error("hr_ctx_set_tuning: block=%d", value); return HR_EINVAL; }
+        ctx->block = value;
+        return HR_OK;
+    }
+    set_error("hr_ctx_set_tuning: unknown key '%s'", key);
+    return HR_EINVAL;
+}
+
+const char *hr_dphi_variant_name(const hr_ctx *ctx, hr_prec prec)
+{
+    if (!ctx || !valid_prec(prec)) return "?";
+    return dphi_variant_name(ctx, prec);
+}
+
+} // extern "C"

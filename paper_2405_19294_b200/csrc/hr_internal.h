@@ -1,0 +1,282 @@
+// hr_internal.h -- private structures and device helpers of libhr (sm_100a).
+//
+// INTERNAL DEVICE LAYOUT.  A per-site record of NREAL reals
+// (spinor: 8*d_R; complex link: 2*d^2; real adjoint link: d^2) is cut into 16-byte vectors; vector v
+// of all V/2 sites of one parity is one contiguous "plane":
+//     address(v, s) = base + (v * Vh + s) * 16          v < NV = NREAL*sizeof(Real)/16
+//     tail (NREAL*sizeof(Real) % 16 = 4 or 8 bytes):   base + NV*16*Vh + s*tail_bytes
+// s = half index = ((t*X + x)*Y + y)*(Z/2) + z/2 of the site inside its parity.  A warp that walks
+// consecutive s therefore issues fully coalesced 128-bit loads (512 contiguous bytes per request).
+// Gauge fields hold 8 such record fields, [parity of the link's base site][mu].
+// This replaces the paper's per-real strided layout (Fig. 1), which would need four
+// (fp32) or two (fp64) times as many load instructions for the same bytes.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/hr.h"
+
+struct hr_ctx {
+    int dims[4];
+    int bc[4];
+    int N;
+    int rep;
+    int d;          // d_R
+    int real_links; // adjoint
+    int device;
+    long V, Vh;
+    int variant;    // -1 = default table
+    int block;      // 0 = default
+    // host-path workspace (hr_dphi_eo_host)
+    void *ws_in, *ws_out, *ws_stage;
+    size_t ws_spinor_bytes, ws_stage_bytes;
+    int ws_prec;
+};
+
+struct hr_gauge {
+    const hr_ctx *ctx;
+    int represented;
+    hr_prec prec;
+    void *data;
+    int owns;
+    size_t bytes;
+    int nreal; // reals per link
+};
+
+namespace hr {
+
+void set_error(const char *fmt, ...);
+void count_launch(int n = 1);
+
+static inline size_t prec_bytes(hr_prec p) { return p == HR_F64 ? 8 : 4; }
+static inline int link_nreal(const hr_ctx *c, int represented)
+{
+    if (!represented) return 2 * c->N * c->N;
+    return c->real_links ? c->d * c->d : 2 * c->d * c->d;
+}
+
+// ---- launch entry points implemented in the kernel translation units ----------------------------
+struct DphiArgs {
+    void *out;
+    const void *in;
+    const void *self;  // psi on the output parity, for the (4+m0) term; nullptr for plain Dphi
+    const void *links; // represented field, internal layout
+    int T, X, Y, Zh;
+    int parity;
+    int bc[4];
+    long vh;
+    double mass; // 4 + m0
+};
+
+// returns HR_OK / HR_EUNSUPPORTED / HR_ECUDA
+hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st);
+const char *dphi_variant_name(const hr_ctx *c, hr_prec prec);
+bool dphi_variant_valid(const hr_ctx *c, int variant);
+
+hr_status launch_represent(const hr_ctx *c, hr_prec in_prec, const void *fund, hr_prec out_prec, void *repr,
+                           cudaStream_t st);
+
+// pack / unpack: canonical AoS (device pointer) <-> internal planes
+hr_status launch_pack_spinor(const hr_ctx *c, void *dst, hr_prec prec, const void *canon_dev, hr_prec cprec,
+                             long first_site, long nsites, cudaStream_t st);
+hr_status launch_unpack_spinor(const hr_ctx *c, const void *src, hr_prec prec, void *canon_dev, hr_prec cprec,
+                               long first_site, long nsites, cudaStream_t st);
+hr_status launch_pack_gauge(const hr_ctx *c, int nreal, void *dst, hr_prec prec, const void *canon_dev,
+                            hr_prec cprec, long first_site, long nsites, cudaStream_t st);
+hr_status launch_unpack_gauge(const hr_ctx *c, int nreal, const void *src, hr_prec prec, void *canon_dev,
+                              hr_prec cprec, long first_site, long nsites, cudaStream_t st);
+
+} // namespace hr
+
+// =================================================================================================
+// device-side helpers
+// =================================================================================================
+#ifdef __CUDACC__
+namespace hr {
+
+template <typename Real> struct VecOf;
+template <> struct VecOf<double> { static constexpr int RPV = 2; };
+template <> struct VecOf<float> { static constexpr int RPV = 4; };
+
+// record geometry
+template <typename Real, int NREAL> struct Rec {
+    static constexpr int RPV = 16 / (int)sizeof(Real);
+    static constexpr int NV = NREAL / RPV;
+    static constexpr int TAIL = NREAL - NV * RPV; // reals in the tail plane
+    static constexpr int BYTES = NREAL * (int)sizeof(Real);
+};
+
+// cache-hint flavours of a 16-byte global load (all read-only path, .nc)
+enum : int {
+    LD_DEFAULT = 0,   // ld.global.nc               : allocate in L1 and L2 (neighbour spinors: re-used)
+    LD_STREAM = 1,    // + L1::no_allocate          : touched once per call (links)
+    LD_STREAM_EF = 2, // + L2 evict_first policy    : links must not push spinors out of L2
+    LD_KEEP = 3       // default L1 + L2 evict_last : neighbour spinors at volumes whose time-slice exceeds L2
+};
+
+__device__ __forceinline__ uint64_t make_policy_evict_first()
+{
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t make_policy_evict_last()
+{
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+
+template <int HINT> __device__ __forceinline__ void ld16(double &a, double &b, const void *p, uint64_t pol)
+{
+    if constexpr (HINT == LD_DEFAULT)
+        asm("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(a), "=d"(b) : "l"(p));
+    else if constexpr (HINT == LD_STREAM)
+        asm("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(a), "=d"(b) : "l"(p));
+    else if constexpr (HINT == LD_STREAM_EF)
+        asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;"
+            : "=d"(a), "=d"(b) : "l"(p), "l"(pol));
+    else
+        asm("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(a), "=d"(b) : "l"(p), "l"(pol));
+}
+template <int HINT>
+__device__ __forceinline__ void ld16(float &a, float &b, float &c, float &d, const void *p, uint64_t pol)
+{
+    if constexpr (HINT == LD_DEFAULT)
+        asm("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(a), "=f"(b), "=f"(c), "=f"(d) : "l"(p));
+    else if constexpr (HINT == LD_STREAM)
+        asm("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+            : "=f"(a), "=f"(b), "=f"(c), "=f"(d) : "l"(p));
+    else if constexpr (HINT == LD_STREAM_EF)
+        asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+            : "=f"(a), "=f"(b), "=f"(c), "=f"(d) : "l"(p), "l"(pol));
+    else
+        asm("ld.global.nc.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+            : "=f"(a), "=f"(b), "=f"(c), "=f"(d) : "l"(p), "l"(pol));
+}
+template <int HINT> __device__ __forceinline__ void ld8(double &a, const void *p, uint64_t pol)
+{
+    if constexpr (HINT == LD_DEFAULT)
+        asm("ld.global.nc.f64 %0, [%1];" : "=d"(a) : "l"(p));
+    else if constexpr (HINT == LD_STREAM)
+        asm("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(a) : "l"(p));
+    else if constexpr (HINT == LD_STREAM_EF)
+        asm("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(a) : "l"(p), "l"(pol));
+    else
+        asm("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(a) : "l"(p), "l"(pol));
+}
+template <int HINT> __device__ __forceinline__ void ld8(float &a, float &b, const void *p, uint64_t pol)
+{
+    if constexpr (HINT == LD_DEFAULT)
+        asm("ld.global.nc.v2.f32 {%0,%1}, [%2];" : "=f"(a), "=f"(b) : "l"(p));
+    else if constexpr (HINT == LD_STREAM)
+        asm("ld.global.nc.L1::no_allocate.v2.f32 {%0,%1}, [%2];" : "=f"(a), "=f"(b) : "l"(p));
+    else if constexpr (HINT == LD_STREAM_EF)
+        asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;"
+            : "=f"(a), "=f"(b) : "l"(p), "l"(pol));
+    else
+        asm("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(a), "=f"(b) : "l"(p), "l"(pol));
+}
+template <int HINT> __device__ __forceinline__ void ld4(float &a, const void *p, uint64_t pol)
+{
+    if constexpr (HINT == LD_DEFAULT)
+        asm("ld.global.nc.f32 %0, [%1];" : "=f"(a) : "l"(p));
+    else if constexpr (HINT == LD_STREAM)
+        asm("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(a) : "l"(p));
+    else if constexpr (HINT == LD_STREAM_EF)
+        asm("ld.global.nc.L1::no_allocate.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(a) : "l"(p), "l"(pol));
+    else
+        asm("ld.global.nc.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(a) : "l"(p), "l"(pol));
+}
+
+// NVEC consecutive planes starting at `p` (= address of the first plane's element for this site)
+template <int HINT, int NVEC>
+__device__ __forceinline__ void load_planes(double *dst, const char *p, size_t plane_bytes, uint64_t pol)
+{
+#pragma unroll
+    for (int v = 0; v < NVEC; ++v) ld16<HINT>(dst[2 * v], dst[2 * v + 1], p + v * plane_bytes, pol);
+}
+template <int HINT, int NVEC>
+__device__ __forceinline__ void load_planes(float *dst, const char *p, size_t plane_bytes, uint64_t pol)
+{
+#pragma unroll
+    for (int v = 0; v < NVEC; ++v)
+        ld16<HINT>(dst[4 * v], dst[4 * v + 1], dst[4 * v + 2], dst[4 * v + 3], p + v * plane_bytes, pol);
+}
+
+// whole record of NREAL reals of site s from the record field at `base`
+template <int HINT, int NREAL>
+__device__ __forceinline__ void load_record(double (&dst)[NREAL], const char *base, size_t vh, size_t s, uint64_t pol)
+{
+    using R = Rec<double, NREAL>;
+    load_planes<HINT, R::NV>(dst, base + s * 16, vh * 16, pol);
+    if constexpr (R::TAIL == 1) ld8<HINT>(dst[NREAL - 1], base + (size_t)R::NV * 16 * vh + s * 8, pol);
+}
+template <int HINT, int NREAL>
+__device__ __forceinline__ void load_record(float (&dst)[NREAL], const char *base, size_t vh, size_t s, uint64_t pol)
+{
+    using R = Rec<float, NREAL>;
+    load_planes<HINT, R::NV>(dst, base + s * 16, vh * 16, pol);
+    const char *t = base + (size_t)R::NV * 16 * vh;
+    if constexpr (R::TAIL == 1) ld4<HINT>(dst[NREAL - 1], t + s * 4, pol);
+    if constexpr (R::TAIL == 2) ld8<HINT>(dst[NREAL - 2], dst[NREAL - 1], t + s * 8, pol);
+    if constexpr (R::TAIL == 3) {
+        ld4<HINT>(dst[NREAL - 3], t + s * 12, pol);
+        ld4<HINT>(dst[NREAL - 2], t + s * 12 + 4, pol);
+        ld4<HINT>(dst[NREAL - 1], t + s * 12 + 8, pol);
+    }
+}
+
+// stores (output spinor: written once, never re-read by this kernel -> streaming)
+enum : int { ST_DEFAULT = 0, ST_STREAM = 1 };
+template <int HINT> __device__ __forceinline__ void st16(void *p, double a, double b)
+{
+    if constexpr (HINT == ST_DEFAULT)
+        asm volatile("st.global.v2.f64 [%0], {%1,%2};" ::"l"(p), "d"(a), "d"(b) : "memory");
+    else
+        asm volatile("st.global.cs.v2.f64 [%0], {%1,%2};" ::"l"(p), "d"(a), "d"(b) : "memory");
+}
+template <int HINT> __device__ __forceinline__ void st16(void *p, float a, float b, float c, float d)
+{
+    if constexpr (HINT == ST_DEFAULT)
+        asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+    else
+        asm volatile("st.global.cs.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+template <int HINT, int NVEC>
+__device__ __forceinline__ void store_planes(char *p, size_t plane_bytes, const double *src)
+{
+#pragma unroll
+    for (int v = 0; v < NVEC; ++v) st16<HINT>(p + v * plane_bytes, src[2 * v], src[2 * v + 1]);
+}
+template <int HINT, int NVEC>
+__device__ __forceinline__ void store_planes(char *p, size_t plane_bytes, const float *src)
+{
+#pragma unroll
+    for (int v = 0; v < NVEC; ++v)
+        st16<HINT>(p + v * plane_bytes, src[4 * v], src[4 * v + 1], src[4 * v + 2], src[4 * v + 3]);
+}
+
+
+// whole record of NREAL reals of site s into the record field at `base` (default cache policy)
+template <int NREAL>
+__device__ __forceinline__ void store_record(char *base, size_t vh, size_t s, const double (&src)[NREAL])
+{
+    using R = Rec<double, NREAL>;
+    store_planes<ST_DEFAULT, R::NV>(base + s * 16, vh * 16, src);
+    if constexpr (R::TAIL == 1) *(double *)(base + (size_t)R::NV * 16 * vh + s * 8) = src[NREAL - 1];
+}
+template <int NREAL>
+__device__ __forceinline__ void store_record(char *base, size_t vh, size_t s, const float (&src)[NREAL])
+{
+    using R = Rec<float, NREAL>;
+    store_planes<ST_DEFAULT, R::NV>(base + s * 16, vh * 16, src);
+    float *t = (float *)(base + (size_t)R::NV * 16 * vh) + s * R::TAIL;
+#pragma unroll
+    for (int e = 0; e < R::TAIL; ++e) t[e] = src[R::NV * 4 + e];
+}
+
+} // namespace hr
+#endif // __CUDACC__
