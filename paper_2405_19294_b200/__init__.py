@@ -6,8 +6,9 @@ functions below carry the names of the C ABI (hr_ctx_create, hr_gauge_alloc, hr_
 hr_dphi_eo, hr_dirac, ...) and raise HrError on any non-zero hr_status.  `Lattice` is a small
 convenience wrapper that owns the handles and uses torch only for device memory and streams.
 
-There is NO CPU fallback: if libhr.so has not been built (python -m paper_2405_19294_b200.build)
-importing this package raises, and on a box without a CUDA device every compute call raises.
+There is NO CPU fallback: if libhr.so is missing, importing this package compiles it in-tree with
+nvcc (paper_2405_19294_b200/build.py); if that fails the import raises, and on a box without a CUDA
+device every compute call raises HrError(HR_ECUDA).
 """
 from __future__ import annotations
 
@@ -33,9 +34,13 @@ class HrError(RuntimeError):
 
 
 if not os.path.exists(LIB_PATH):
-    raise ImportError(
-        f"{LIB_PATH} is missing: build it with `python -m paper_2405_19294_b200.build` "
-        "(there is no CPU fallback for the CUDA path)")
+    from . import build as _build  # pure python; compiles csrc/*.cu with nvcc for sm_100a
+    try:
+        _build.build()
+    except Exception as exc:  # no CPU fallback: without the CUDA library there is no product
+        raise ImportError(
+            f"{LIB_PATH} is missing and could not be built ({exc}); "
+            "there is no CPU fallback for the CUDA path") from exc
 
 _lib = ctypes.CDLL(LIB_PATH)
 _vp, _ci, _cd, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
