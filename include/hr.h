@@ -133,7 +133,8 @@ hr_status hr_dphi_eo_host(hr_ctx *ctx, void *out_canon, const void *in_canon, hr
 /*
  * Kernel tuning (experiments and ncu evidence; defaults are chosen per (d_R, precision) from
  * measurements).  key: "variant" (kernel variant id, -1 = default table),
- * "block" (threads per CTA, 0 = default).  Unknown key or value -> HR_EINVAL.
+ * "block" (threads per CTA, 0 = default), "xblock" (x-extent of the thread order's blocks, a divisor
+ * of X; 0 = default from the L2 working-set rule).  Unknown key or value -> HR_EINVAL.
  */
 hr_status hr_ctx_set_tuning(hr_ctx *ctx, const char *key, int value);
 /* Name of the Dphi kernel variant a call with this precision would launch (for logs/bench). */

@@ -14,8 +14,9 @@ static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "sit
 // Default variant per (d_R, link type, precision, volume): filled from measurements.
 static int default_variant(const hr_ctx *c, hr_prec prec)
 {
-    (void)prec;
-    if (c->d >= 6) return 2; // pair: one thread per site would spill
+    // measured on B200 (profiles/r1_variant_sweep.md): at d_R >= 6 fp64 one thread per site spills
+    // and the pair kernel wins; in fp32 the whole site still fits one thread.
+    if (c->d >= 6) return prec == HR_F64 ? 3 : 1;
     return 0;
 }
 

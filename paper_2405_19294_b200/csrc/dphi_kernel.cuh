@@ -160,14 +160,20 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
     const bool live = s < a.vh;
     if (!live) s = a.vh - 1; // keep the pair convergent for the final shuffle; stores are predicated
 
+    // Thread order -> site (a3).  Threads walk the lattice as [x / Xb][t][x % Xb][y][zh] while the
+    // storage order stays [t][x][y][zh]: the +-t neighbours of a site are then Xb*Y*Zh threads away
+    // instead of X*Y*Zh, so the spinors (and nothing else) that one t-slice of an x-block loads are
+    // still in L2 when the next t-slice needs them.  Xb = X is the identity order.
     SiteGeom g;
     {
-        long r = s;
-        g.zh = (int)(r % a.Zh); r /= a.Zh;
-        g.y = (int)(r % a.Y); r /= a.Y;
-        g.x = (int)(r % a.X);
-        g.t = (int)(r / a.X);
+        unsigned r = (unsigned)s; // Vh < 2^31 (hr_ctx_create)
+        g.zh = (int)(r % (unsigned)a.Zh); r /= (unsigned)a.Zh;
+        g.y = (int)(r % (unsigned)a.Y); r /= (unsigned)a.Y;
+        const int xl = (int)(r % (unsigned)a.Xb); r /= (unsigned)a.Xb;
+        g.t = (int)(r % (unsigned)a.T);
+        g.x = (int)(r / (unsigned)a.T) * a.Xb + xl;
         g.b = (g.t + g.x + g.y + a.parity) & 1;
+        s = (((long)g.t * a.X + g.x) * a.Y + g.y) * a.Zh + g.zh;
     }
     const size_t vh = (size_t)a.vh;
     const size_t pb = vh * 16; // plane bytes

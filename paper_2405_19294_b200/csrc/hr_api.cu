@@ -175,6 +175,7 @@ hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N,
     c->Vh = c->V / 2;
     c->variant = -1;
     c->block = 0;
+    c->xblock = 0;
     c->ws_in = c->ws_out = c->ws_stage = nullptr;
     c->ws_spinor_bytes = c->ws_stage_bytes = 0;
     c->ws_prec = -1;
@@ -302,9 +303,25 @@ hr_status hr_represent_links(hr_gauge *repr_out, const hr_gauge *fund_in, void *
     return launch_represent(fund_in->ctx, fund_in->prec, fund_in->data, repr_out->prec, repr_out->data, (cudaStream_t)stream);
 }
 
+// x-block of the thread order (dphi_kernel.cuh): the largest divisor of X whose t-slice working set
+// Xb*Y*Zh*(8L+2S) stays below kSliceBytes, so that +-t neighbour spinors are re-used out of L2.
+// Measured (profiles/): a 25 MB slice (32^3 fp64) is re-used perfectly, a 176 MB one (64^3 fp64) is not.
+static const double kSliceBytes = 32.0 * 1024 * 1024;
+static int default_xblock(const hr_ctx *c, hr_prec prec)
+{
+    const double w = (double)prec_bytes(prec);
+    const double site = 8.0 * link_nreal(c, 1) * w + 2.0 * 8 * c->d * w;
+    const double row = (double)c->dims[2] * (c->dims[3] / 2) * site;
+    int best = 1;
+    for (int xb = 1; xb <= c->dims[1]; ++xb)
+        if (c->dims[1] % xb == 0 && xb * row <= kSliceBytes) best = xb;
+    return best;
+}
+
 static hr_status dphi_args(DphiArgs &a, const hr_ctx *c, void *out, const void *in, const void *self, const hr_gauge *links,
                            int parity, double mass)
 {
+    a.Xb = c->xblock > 0 ? c->xblock : default_xblock(c, links->prec);
     a.out = out;
     a.in = in;
     a.self = self;
@@ -402,6 +419,11 @@ hr_status hr_ctx_set_tuning(hr_ctx *ctx, const char *key, int value)
     if (!strcmp(key, "block")) {
         if (value < 0 || value > 1024 || (value % 32)) { set_error("hr_ctx_set_tuning: block=%d", value); return HR_EINVAL; }
         ctx->block = value;
+        return HR_OK;
+    }
+    if (!strcmp(key, "xblock")) {
+        if (value < 0 || (value > 0 && ctx->dims[1] % value)) { set_error("hr_ctx_set_tuning: xblock=%d must divide X=%d", value, ctx->dims[1]); return HR_EINVAL; }
+        ctx->xblock = value;
         return HR_OK;
     }
     set_error("hr_ctx_set_tuning: unknown key '%s'", key);

@@ -29,6 +29,7 @@ struct hr_ctx {
     long V, Vh;
     int variant;    // -1 = default table
     int block;      // 0 = default
+    int xblock;     // 0 = default (from the L2 working-set rule), else a divisor of X
     // host-path workspace (hr_dphi_eo_host)
     void *ws_in, *ws_out, *ws_stage;
     size_t ws_spinor_bytes, ws_stage_bytes;
@@ -64,6 +65,7 @@ struct DphiArgs {
     const void *self;  // psi on the output parity, for the (4+m0) term; nullptr for plain Dphi
     const void *links; // represented field, internal layout
     int T, X, Y, Zh;
+    int Xb;     // x-block of the thread order (divides X; X = storage order), see dphi_kernel.cuh
     int parity;
     int bc[4];
     long vh;

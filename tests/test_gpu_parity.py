@@ -149,6 +149,27 @@ def test_every_kernel_variant_matches_oracle(hr, N, rep, prec, variant):
     prob.close()
 
 
+@pytest.mark.parametrize("xblock", [1, 2, 3, 6])
+@pytest.mark.parametrize("variant", [0, 2])
+def test_thread_order_xblock_does_not_change_the_result(hr, xblock, variant):
+    """The [x/Xb][t][x%Xb][y][zh] thread order (L2 re-use of +-t neighbours) is only a permutation of
+    which thread computes which site: bit-identical to the storage order Xb = X, and equal to the oracle."""
+    dims = (4, 6, 4, 10)
+    U, psi = make_inputs(dims, 3, 55, 56, 3)
+    prob = GpuProblem(hr, dims, 3, "fund", "f64", U)
+    prob.lat.set_tuning("variant", variant)
+    prob.lat.set_tuning("xblock", 6)
+    base = [prob.dphi_eo(psi, parity) for parity in (0, 1)]
+    prob.lat.set_tuning("xblock", xblock)
+    for parity in (0, 1):
+        got = prob.dphi_eo(psi, parity)
+        assert np.array_equal(got, base[parity])
+        assert rel_l2(got, oracle.dphi_eo(dims, BC_T, U, parity, psi)) <= TOL["f64"]
+    with pytest.raises(hr.HrError):
+        prob.lat.set_tuning("xblock", 4)   # does not divide X = 6
+    prob.close()
+
+
 # config 1 (BASELINE.json:configs[0]): SU(2) fundamental, 4^4, fp64, full D with m0 = -0.5, both parities of Dphi_eo
 def test_config1_su2_fund_4x4_dirac_and_both_parities(hr):
     dims = (4, 4, 4, 4)
