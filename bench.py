@@ -88,6 +88,27 @@ def make_fields(cfg):
     return U, psi
 
 
+def replica_seeds(seeds, rank):
+    """Independent replica per rank (replicas only, no data-path collective)."""
+    return (seeds[0] + 100000 * rank, seeds[1] + 100000 * rank)
+
+
+def max_over_ranks(x, world, device):
+    """MAX over ranks of a locally measured duration (the only collective besides the timing barrier)."""
+    if world == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(step_bytes, world, seconds_per_step):
+    """value = the units all ranks processed / the max-over-ranks time (GB/s)."""
+    return world * step_bytes / seconds_per_step / 1e9
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons of one GPU during the timed region (NVML)."""
 
@@ -220,7 +241,7 @@ def run_ours(args, cfg, prec):
 
     bm = byte_model(cfg, prec)
     P = hr.PREC_NAMES[prec]
-    cfg_r = dict(cfg, seeds=(cfg["seeds"][0] + 100000 * rank, cfg["seeds"][1] + 100000 * rank))  # independent replica per rank
+    cfg_r = dict(cfg, seeds=replica_seeds(cfg["seeds"], rank))
     U, psi = make_fields(cfg_r)
     lat = hr.Lattice(cfg["dims"], BC, cfg["N"], cfg["rep"], device=local)
     fund = lat.gauge(False, P)
@@ -269,13 +290,10 @@ def run_ours(args, cfg, prec):
     rep_ms = statistics.mean(e[0].elapsed_time(e[1]) for e in ev)
     dphi_ms = statistics.mean([e[1].elapsed_time(e[2]) for e in ev] + [e[2].elapsed_time(e[3]) for e in ev])
     dphi_ms_min = min([e[1].elapsed_time(e[2]) for e in ev] + [e[2].elapsed_time(e[3]) for e in ev])
-    if world > 1:
-        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, world, "cuda")
     ms_step = ms_total / args.steps
     step_bytes = 4 * bm["V"] * bm["represent_bytes_per_link"] + bm["V"] * bm["dphi_bytes_per_site"]
-    value = world * step_bytes / (ms_step * 1e-3) / 1e9
+    value = whole_job_value(step_bytes, world, ms_step * 1e-3)
 
     # end to end through the host entry points (pinned host buffers; copies inside the timed region)
     e2e = None
@@ -301,13 +319,10 @@ def run_ours(args, cfg, prec):
             e2e_step()
         sync_all()
         dt = (time.perf_counter() - t0) / ke
-        if world > 1:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dt, world, "cuda")
         h2d = hU.numel() * hU.element_size() + sum(h.numel() * h.element_size() for h in hin)
         d2h = sum(h.numel() * h.element_size() for h in hout)
-        e2e = {"value": world * step_bytes / dt / 1e9, "unit": "GB/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+        e2e = {"value": whole_job_value(step_bytes, world, dt), "unit": "GB/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "ms_per_step": dt * 1e3, "steps": ke}
 
     if rank != 0:

@@ -1,0 +1,73 @@
+"""N > 1 host logic of bench.py on CPU (gloo, world size 2): DESIGN.md section 9 -- the path as specified
+has no exchange step, so ranks are independent replicas; the only collectives are the timing barrier and the
+MAX over ranks of the measured time.  Checked here: replica seeds differ per rank and give different fields,
+max_over_ranks returns the slowest rank's time on every rank, value = units of all ranks / that time, and
+`bench.py --impl reference` lets rank 0 alone print a line."""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    import bench
+    import lattice_inputs as li
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    seeds = bench.replica_seeds(bench.CONFIGS[1]["seeds"], rank)
+    U = li.haar_links(seeds[0], 2, (4, 4, 4, 4))
+    dist.barrier()
+    local_ms = 1.0 + 2.0 * rank            # rank 1 is the slow one
+    ms = bench.max_over_ranks(local_ms, world, "cpu")
+    val = bench.whole_job_value(1e9, world, ms * 1e-3)
+    allU = [torch.zeros(U.size * 2, dtype=torch.float64) for _ in range(world)]
+    dist.all_gather(allU, torch.from_numpy(np.ascontiguousarray(U).view(np.float64).reshape(-1).copy()))
+    q.put((rank, seeds, ms, val, bool(torch.equal(allU[0], allU[1]))))
+    dist.destroy_process_group()
+
+
+def test_replicas_max_over_ranks_gloo_world2():
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (r0, s0, ms0, v0, same0), (r1, s1, ms1, v1, same1) = res
+    assert s0 != s1 and s0 == (1001, 2001) and s1 == (101001, 102001)
+    assert not same0 and not same1                      # different replicas really hold different fields
+    assert ms0 == ms1 == 3.0                            # the slowest rank's time, on every rank
+    assert v0 == v1 == 2 * 1e9 / 3e-3 / 1e9             # units of all ranks / max time
+
+
+def test_reference_arm_only_rank0_prints():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1",
+                        "--steps", "1", "--warmup", "0", "--gpus", "2"], env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0 and r.stdout.strip() == ""
+    env["RANK"] = "0"
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1",
+                        "--steps", "1", "--warmup", "0", "--gpus", "2"], env=env, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["n_gpus"] == 2
