@@ -130,6 +130,75 @@ hr_status hr_dirac(double m0, void *out_full, const void *in_full, const hr_gaug
 hr_status hr_dphi_eo_host(hr_ctx *ctx, void *out_canon, const void *in_canon, hr_prec canon_prec,
                           const hr_gauge *links, int parity, void *stream);
 
+/* =====================================================================================================
+ * Second part -- SURVEY.md section 8(f) NEXT-1: what the hopping term is FOR ("We are
+ * supporting even-odd preconditioning"; section 3.2 "Linear Algebra"
+ * section 3.3 "Conjugate Gradient").  The paper prints no formula for any of these; the definitions are
+ * readings C20-C24 of DESIGN.md, restated at each call.  All spinor buffers are ONE-parity half fields in
+ * the internal layout (hr_spinor_bytes()), device memory owned by the caller, 16-byte aligned.
+ * Calls that reduce (dot, norm2, the CG) use a scratch area the ctx creates on first use (3 MiB, freed by
+ * hr_ctx_destroy): issue them on ONE stream at a time per ctx.
+ * ===================================================================================================== */
+
+/*
+ * Spinor linear algebra (Fig. 7: "Copy spinor field", "g5 application", "g5 mulc add
+ * assign").  One streaming kernel each, no synchronisation, no allocation.
+ *   hr_spinor_lincomb:            out = ca * G(x) + cb * y,  G = gamma5 if g5 != 0 else 1; ca, cb complex
+ *                                 (re, im); y (and cb) may be NULL; out may alias x and/or y.
+ *   hr_spinor_copy:               out = in
+ *   hr_spinor_g5:                 out = gamma5 in            (gamma5 = diag(1,1,-1,-1) on spin, reading C1)
+ *   hr_spinor_mulc_add_assign:    out += c in                (reading C23)
+ *   hr_spinor_g5_mulc_add_assign: out += c gamma5 in         (reading C23)
+ */
+hr_status hr_spinor_lincomb(const hr_ctx *ctx, hr_prec prec, void *out, const double ca[2], int g5, const void *x,
+                            const double cb[2], const void *y, void *stream);
+hr_status hr_spinor_copy(const hr_ctx *ctx, hr_prec prec, void *out, const void *in, void *stream);
+hr_status hr_spinor_g5(const hr_ctx *ctx, hr_prec prec, void *out, const void *in, void *stream);
+hr_status hr_spinor_mulc_add_assign(const hr_ctx *ctx, hr_prec prec, void *out, double c_re, double c_im,
+                                    const void *in, void *stream);
+hr_status hr_spinor_g5_mulc_add_assign(const hr_ctx *ctx, hr_prec prec, void *out, double c_re, double c_im,
+                                       const void *in, void *stream);
+
+/*
+ * Reductions ("inner products and norms"; the paper runs a site-wise kernel and then
+ * cub -- two passes over global memory; here ONE kernel reads the field(s) once).  Reading C22:
+ *   hr_spinor_dot:   result[0] + i result[1] = <x, y> = sum conj(x) y     (2 doubles)
+ *   hr_spinor_norm2: result[0] = <x, x>                                   (1 double)
+ * Sums are accumulated in fp64 for both precisions, in an order fixed by the launch geometry (bitwise
+ * reproducible).  `result` may be DEVICE memory (no synchronisation) or HOST memory (the call
+ * synchronises the stream before returning).
+ */
+hr_status hr_spinor_dot(hr_ctx *ctx, hr_prec prec, const void *x, const void *y, double *result, void *stream);
+hr_status hr_spinor_norm2(hr_ctx *ctx, hr_prec prec, const void *x, double *result, void *stream);
+
+/*
+ * hr_dhat -- the even-odd preconditioned operator on EVEN sites (reading C20):
+ *     out_e = Dhat in_e = (4+m0)^2 in_e - Dphi_eo Dphi_oe in_e          (g5 == 0)
+ *     out_e = gamma5 Dhat in_e                                          (g5 != 0; Hermitian, reading C21)
+ * Two Dphi launches; the diagonal term, the sign and gamma5 are fused into the second one's epilogue.
+ * tmp_o: caller-owned odd-parity half field (overwritten).  out_e, in_e, tmp_o distinct.
+ */
+hr_status hr_dhat(double m0, int g5, void *out_e, const void *in_e, void *tmp_o, const hr_gauge *links, void *stream);
+
+/*
+ * Conjugate gradient (reading C21).  hr_cg_dhat solves Dhat x_e = b_e on the even sites by
+ * the textbook CG on the normal equations Dhat^dagger Dhat x = Dhat^dagger b (Dhat^dagger = gamma5 Dhat
+ * gamma5), x0 = 0, recursive residual, stopping at the first k with |r_k|^2 <= tol^2 |Dhat^dagger b|^2 or
+ * k = maxiter.  alpha, beta, the iteration counter and the stop flag live on the device: iterations are
+ * enqueued in batches and the host synchronises `stream` once per batch (and before returning).
+ *   workspace: hr_cg_workspace_bytes(ctx, prec of links, maxiter) bytes of device memory, 256-byte aligned.
+ *   iters (may be NULL): iterations done.  rel_res2 (may be NULL): |r_k|^2 / |rhs|^2 at exit.
+ *   hist (may be NULL): HOST array of maxiter+1 doubles, receives |r_k|^2 / |rhs|^2 for k = 0..iters.
+ * hr_dirac_solve solves the FULL system D x = b, D = (4+m0) + Dphi, fields [even half | odd half], through
+ * the preconditioned one (reading C24):  Dhat x_e = (4+m0) b_e - Dphi_eo b_o ;  x_o = (b_o - Dphi_oe x_e)/(4+m0).
+ * x must not alias b.  Not converged within maxiter is not an error: check iters / rel_res2.
+ */
+size_t hr_cg_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter);
+hr_status hr_cg_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol, int maxiter,
+                     void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
+hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links, double tol,
+                         int maxiter, void *workspace, int *iters, double *rel_res2, void *stream);
+
 /*
  * Kernel tuning (experiments and ncu evidence; defaults are chosen per (d_R, precision) from
  * measurements).  key: "variant" (kernel variant id, -1 = default table),

@@ -42,9 +42,10 @@ if not os.path.exists(LIB_PATH):
             f"{LIB_PATH} is missing and could not be built ({exc}); "
             "there is no CPU fallback for the CUDA path") from exc
 
-_lib = ctypes.CDLL(LIB_PATH)
 _vp, _ci, _cd, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
 _I4 = ctypes.c_int * 4
+_D2 = ctypes.c_double * 2
+_D2P = ctypes.POINTER(ctypes.c_double)
 
 # every symbol include/hr.h declares: name -> (restype, argtypes)
 _SIGNATURES = {
@@ -68,14 +69,42 @@ _SIGNATURES = {
     "hr_dphi_eo": (_ci, [_vp, _vp, _vp, _ci, _vp]),
     "hr_dirac": (_ci, [_cd, _vp, _vp, _vp, _vp]),
     "hr_dphi_eo_host": (_ci, [_vp, _vp, _vp, _ci, _vp, _ci, _vp]),
+    "hr_spinor_lincomb": (_ci, [_vp, _ci, _vp, _D2, _ci, _vp, _D2P, _vp, _vp]),
+    "hr_spinor_copy": (_ci, [_vp, _ci, _vp, _vp, _vp]),
+    "hr_spinor_g5": (_ci, [_vp, _ci, _vp, _vp, _vp]),
+    "hr_spinor_mulc_add_assign": (_ci, [_vp, _ci, _vp, _cd, _cd, _vp, _vp]),
+    "hr_spinor_g5_mulc_add_assign": (_ci, [_vp, _ci, _vp, _cd, _cd, _vp, _vp]),
+    "hr_spinor_dot": (_ci, [_vp, _ci, _vp, _vp, _vp, _vp]),
+    "hr_spinor_norm2": (_ci, [_vp, _ci, _vp, _vp, _vp]),
+    "hr_dhat": (_ci, [_cd, _ci, _vp, _vp, _vp, _vp, _vp]),
+    "hr_cg_workspace_bytes": (_sz, [_vp, _ci, _ci]),
+    "hr_cg_dhat": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp, _vp]),
+    "hr_dirac_solve": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
     "hr_ctx_set_tuning": (_ci, [_vp, ctypes.c_char_p, _ci]),
     "hr_dphi_variant_name": (ctypes.c_char_p, [_vp, _ci]),
     "hr_launch_count": (ctypes.c_ulonglong, []),
 }
-for _name, (_res, _args) in _SIGNATURES.items():
-    _f = getattr(_lib, _name)  # AttributeError here = the library does not export the header's symbol
-    _f.restype = _res
-    _f.argtypes = _args
+
+
+def _bind():
+    lib = ctypes.CDLL(LIB_PATH)
+    for name, (res, args) in _SIGNATURES.items():
+        f = getattr(lib, name)  # AttributeError here = the library does not export the header's symbol
+        f.restype = res
+        f.argtypes = args
+    return lib
+
+
+def _exports_all() -> bool:
+    blob = open(LIB_PATH, "rb").read()
+    return all(name.encode() + b"\0" in blob for name in _SIGNATURES)
+
+
+if not _exports_all():
+    # a libhr.so older than include/hr.h (left over from an earlier checkout): rebuild BEFORE loading it
+    from . import build as _build
+    _build.build(force=True)
+_lib = _bind()
 
 
 def _check(status: int) -> None:
@@ -190,6 +219,74 @@ def hr_dphi_eo_host(ctx: int, out_canon, in_canon, canon_prec: int, links: int, 
     _check(_lib.hr_dphi_eo_host(ctx, _ptr(out_canon), _ptr(in_canon), canon_prec, links, parity, stream))
 
 
+def hr_spinor_lincomb(ctx: int, prec: int, out, ca: complex, g5: int, x, cb: complex = 0j, y=None, stream: int = 0) -> None:
+    ca, cb = complex(ca), complex(cb)
+    cbp = ctypes.cast(_D2(cb.real, cb.imag), _D2P) if y is not None else None
+    _check(_lib.hr_spinor_lincomb(ctx, prec, _ptr(out), _D2(ca.real, ca.imag), int(g5), _ptr(x), cbp, _ptr(y), stream))
+
+
+def hr_spinor_copy(ctx: int, prec: int, out, inp, stream: int = 0) -> None:
+    _check(_lib.hr_spinor_copy(ctx, prec, _ptr(out), _ptr(inp), stream))
+
+
+def hr_spinor_g5(ctx: int, prec: int, out, inp, stream: int = 0) -> None:
+    _check(_lib.hr_spinor_g5(ctx, prec, _ptr(out), _ptr(inp), stream))
+
+
+def hr_spinor_mulc_add_assign(ctx: int, prec: int, out, c: complex, inp, stream: int = 0) -> None:
+    c = complex(c)
+    _check(_lib.hr_spinor_mulc_add_assign(ctx, prec, _ptr(out), c.real, c.imag, _ptr(inp), stream))
+
+
+def hr_spinor_g5_mulc_add_assign(ctx: int, prec: int, out, c: complex, inp, stream: int = 0) -> None:
+    c = complex(c)
+    _check(_lib.hr_spinor_g5_mulc_add_assign(ctx, prec, _ptr(out), c.real, c.imag, _ptr(inp), stream))
+
+
+def hr_spinor_dot(ctx: int, prec: int, x, y, stream: int = 0, result=None):
+    """<x, y>; result=None: returned as a Python complex (host result, synchronises); else a device buffer."""
+    if result is not None:
+        _check(_lib.hr_spinor_dot(ctx, prec, _ptr(x), _ptr(y), _ptr(result), stream))
+        return None
+    r = _D2()
+    _check(_lib.hr_spinor_dot(ctx, prec, _ptr(x), _ptr(y), ctypes.addressof(r), stream))
+    return complex(r[0], r[1])
+
+
+def hr_spinor_norm2(ctx: int, prec: int, x, stream: int = 0, result=None):
+    if result is not None:
+        _check(_lib.hr_spinor_norm2(ctx, prec, _ptr(x), _ptr(result), stream))
+        return None
+    r = _cd()
+    _check(_lib.hr_spinor_norm2(ctx, prec, _ptr(x), ctypes.addressof(r), stream))
+    return float(r.value)
+
+
+def hr_dhat(m0: float, g5: int, out_e, in_e, tmp_o, links: int, stream: int = 0) -> None:
+    _check(_lib.hr_dhat(float(m0), int(g5), _ptr(out_e), _ptr(in_e), _ptr(tmp_o), links, stream))
+
+
+def hr_cg_workspace_bytes(ctx: int, prec: int, maxiter: int) -> int:
+    return _lib.hr_cg_workspace_bytes(ctx, prec, maxiter)
+
+
+def hr_cg_dhat(ctx: int, m0: float, x_e, b_e, links: int, tol: float, maxiter: int, workspace, stream: int = 0, want_hist: bool = False):
+    """Returns (iterations, |r|^2/|rhs|^2, history or None)."""
+    it, res = _ci(0), _cd(0.0)
+    hist = np.zeros(maxiter + 1, dtype=np.float64) if want_hist else None
+    _check(_lib.hr_cg_dhat(ctx, float(m0), _ptr(x_e), _ptr(b_e), links, float(tol), int(maxiter), _ptr(workspace),
+                           ctypes.byref(it), ctypes.byref(res), _ptr(hist), stream))
+    return it.value, res.value, (hist[:it.value + 1] if want_hist else None)
+
+
+def hr_dirac_solve(ctx: int, m0: float, x_full, b_full, links: int, tol: float, maxiter: int, workspace, stream: int = 0):
+    """Returns (iterations, |r|^2/|rhs|^2 of the preconditioned normal equations)."""
+    it, res = _ci(0), _cd(0.0)
+    _check(_lib.hr_dirac_solve(ctx, float(m0), _ptr(x_full), _ptr(b_full), links, float(tol), int(maxiter), _ptr(workspace),
+                               ctypes.byref(it), ctypes.byref(res), stream))
+    return it.value, res.value
+
+
 def hr_ctx_set_tuning(ctx: int, key: str, value: int) -> None:
     _check(_lib.hr_ctx_set_tuning(ctx, key.encode(), int(value)))
 
@@ -285,6 +382,20 @@ class Lattice:
 
     def dirac(self, m0: float, out_full, in_full, links: int) -> None:
         hr_dirac(m0, out_full, in_full, links, self.stream())
+
+    # -- NEXT-1: linear algebra, preconditioned operator, solver
+    def cg_workspace(self, prec: int, maxiter: int):
+        n = hr_cg_workspace_bytes(self.ctx, prec, maxiter)
+        return self._torch.empty(n, dtype=self._torch.uint8, device=f"cuda:{self.device}")
+
+    def dhat(self, m0: float, g5: bool, out_e, in_e, tmp_o, links: int) -> None:
+        hr_dhat(m0, int(g5), out_e, in_e, tmp_o, links, self.stream())
+
+    def cg_dhat(self, m0, x_e, b_e, links, tol, maxiter, workspace, want_hist=False):
+        return hr_cg_dhat(self.ctx, m0, x_e, b_e, links, tol, maxiter, workspace, self.stream(), want_hist)
+
+    def dirac_solve(self, m0, x_full, b_full, links, tol, maxiter, workspace):
+        return hr_dirac_solve(self.ctx, m0, x_full, b_full, links, tol, maxiter, workspace, self.stream())
 
     def set_tuning(self, key: str, value: int) -> None:
         hr_ctx_set_tuning(self.ctx, key, value)

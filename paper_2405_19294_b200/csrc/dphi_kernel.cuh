@@ -113,6 +113,14 @@ __device__ __forceinline__ void hop_component(const Real *u, const Real *a, cons
     }
 }
 
+// epilogue coefficients in the kernel's precision, straight from the constant bank
+template <typename Real> __device__ __forceinline__ Real coef_alpha(const DphiArgs &a, int i);
+template <> __device__ __forceinline__ double coef_alpha<double>(const DphiArgs &a, int i) { return a.alpha[i]; }
+template <> __device__ __forceinline__ float coef_alpha<float>(const DphiArgs &a, int i) { return a.alphaf[i]; }
+template <typename Real> __device__ __forceinline__ Real coef_beta(const DphiArgs &a, int i);
+template <> __device__ __forceinline__ double coef_beta<double>(const DphiArgs &a, int i) { return a.beta[i]; }
+template <> __device__ __forceinline__ float coef_beta<float>(const DphiArgs &a, int i) { return a.betaf[i]; }
+
 struct SiteGeom {
     int t, x, y, zh, b; // b = offset bit: z = 2*zh + b
 };
@@ -145,9 +153,14 @@ __device__ __forceinline__ void neighbour(const DphiArgs &a, const SiteGeom &g, 
     }
 }
 
-template <typename Real, int D, bool RL, int KSPLIT, bool MASS, int LHINT, int SHINT, int STHINT, int MAXT, int MINB>
+// MASS: the epilogue reads self = psi(x) on the output parity (alpha term); RED: the epilogue also
+// reduces sum |out|^2 and <self, out> over the launch (needs MASS) -- what a CG on gamma5 Dhat needs
+// from its operator, with no extra pass over the fields.
+template <typename Real, int D, bool RL, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
 {
+    static_assert(!RED || MASS, "the fused reduction needs the self field");
+    if (a.skip != nullptr && *a.skip != 0) return;
     constexpr int LNREAL = RL ? D * D : 2 * D * D;        // reals per link
     constexpr int RPV = 16 / (int)sizeof(Real);
     constexpr int SPV = 2 * D / RPV;                       // 16-byte vectors per spin component
@@ -216,21 +229,36 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
         hop(I3{}, I0{}); hop(I3{}, I1{});
 
         Real o[8 * D];
+        [[maybe_unused]] Real n2 = 0, dre = 0, dim = 0;
         if constexpr (MASS) {
+            const Real be[2] = { coef_beta<Real>(a, 0), coef_beta<Real>(a, 1) };
             Real self[8 * D];
             load_record<LD_STREAM, 8 * D>(self, (const char *)a.self, vh, (size_t)s, 0);
-            const Real m = (Real)a.mass;
+            const Real al_[2] = { coef_alpha<Real>(a, 0), coef_alpha<Real>(a, 1) };
 #pragma unroll
             for (int al = 0; al < 4; ++al)
 #pragma unroll
-                for (int c = 0; c < 2 * D; ++c) o[al * 2 * D + c] = fma(m, self[al * 2 * D + c], (Real)-0.5 * acc[al][c]);
+                for (int c = 0; c < 2 * D; ++c) o[al * 2 * D + c] = fma(al_[al >> 1], self[al * 2 * D + c], be[al >> 1] * acc[al][c]);
+            if constexpr (RED) {
+#pragma unroll
+                for (int e = 0; e < 4 * D; ++e) {
+                    const Real sr = self[2 * e], si = self[2 * e + 1], orr = o[2 * e], oi = o[2 * e + 1];
+                    n2 = fma(orr, orr, fma(oi, oi, n2));
+                    dre = fma(sr, orr, fma(si, oi, dre));   // conj(self) * out
+                    dim = fma(sr, oi, fma(-si, orr, dim));
+                }
+            }
         } else {
 #pragma unroll
             for (int al = 0; al < 4; ++al)
 #pragma unroll
-                for (int c = 0; c < 2 * D; ++c) o[al * 2 * D + c] = (Real)-0.5 * acc[al][c];
+                for (int c = 0; c < 2 * D; ++c) o[al * 2 * D + c] = (Real)-0.5 * acc[al][c]; // plain Dphi
         }
         if (live) store_planes<STHINT, 8 * D / RPV>((char *)a.out + (size_t)s * 16, pb, o);
+        if constexpr (RED) {
+            double v[3] = { live ? (double)n2 : 0.0, live ? (double)dre : 0.0, live ? (double)dim : 0.0 };
+            if (grid_reduce<3>(v, a.red_partial, a.red_ticket)) { a.red_result[0] = v[0]; a.red_result[1] = v[1]; a.red_result[2] = v[2]; }
+        }
     } else {
         // two threads per site: thread k owns h_k.  accK -> out_k, accP -> out_{k+2} (mu = 0,3),
         // accQ -> out_{3-k} (mu = 1,2), exchanged with the partner lane at the end.
@@ -265,25 +293,42 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
 #pragma unroll
         for (int c = 0; c < 2 * D; ++c) accP[c] += __shfl_xor_sync(0xffffffffu, accQ[c], 1);
 
+        [[maybe_unused]] Real n2 = 0, dre = 0, dim = 0;
         if constexpr (MASS) {
+            const Real be[2] = { coef_beta<Real>(a, 0), coef_beta<Real>(a, 1) };
             Real sa[2 * D], sb[2 * D];
             const char *base = (const char *)a.self + (size_t)s * 16;
             load_planes<LD_STREAM, SPV>(sa, base + (size_t)(k * SPV) * pb, pb, 0);
             load_planes<LD_STREAM, SPV>(sb, base + (size_t)((k + 2) * SPV) * pb, pb, 0);
-            const Real m = (Real)a.mass;
+            const Real al_[2] = { coef_alpha<Real>(a, 0), coef_alpha<Real>(a, 1) };
 #pragma unroll
             for (int c = 0; c < 2 * D; ++c) {
-                accK[c] = fma(m, sa[c], (Real)-0.5 * accK[c]);
-                accP[c] = fma(m, sb[c], (Real)-0.5 * accP[c]);
+                accK[c] = fma(al_[0], sa[c], be[0] * accK[c]);   // component k   (upper)
+                accP[c] = fma(al_[1], sb[c], be[1] * accP[c]);   // component k+2 (lower)
+            }
+            if constexpr (RED) {
+#pragma unroll
+                for (int e = 0; e < D; ++e) {
+                    n2 = fma(accK[2 * e], accK[2 * e], fma(accK[2 * e + 1], accK[2 * e + 1], n2));
+                    n2 = fma(accP[2 * e], accP[2 * e], fma(accP[2 * e + 1], accP[2 * e + 1], n2));
+                    dre = fma(sa[2 * e], accK[2 * e], fma(sa[2 * e + 1], accK[2 * e + 1], dre));
+                    dre = fma(sb[2 * e], accP[2 * e], fma(sb[2 * e + 1], accP[2 * e + 1], dre));
+                    dim = fma(sa[2 * e], accK[2 * e + 1], fma(-sa[2 * e + 1], accK[2 * e], dim));
+                    dim = fma(sb[2 * e], accP[2 * e + 1], fma(-sb[2 * e + 1], accP[2 * e], dim));
+                }
             }
         } else {
 #pragma unroll
-            for (int c = 0; c < 2 * D; ++c) { accK[c] *= (Real)-0.5; accP[c] *= (Real)-0.5; }
+            for (int c = 0; c < 2 * D; ++c) { accK[c] *= (Real)-0.5; accP[c] *= (Real)-0.5; } // plain Dphi
         }
         if (live) {
             char *ob = (char *)a.out + (size_t)s * 16;
             store_planes<STHINT, SPV>(ob + (size_t)(k * SPV) * pb, pb, accK);
             store_planes<STHINT, SPV>(ob + (size_t)((k + 2) * SPV) * pb, pb, accP);
+        }
+        if constexpr (RED) {
+            double v[3] = { live ? (double)n2 : 0.0, live ? (double)dre : 0.0, live ? (double)dim : 0.0 };
+            if (grid_reduce<3>(v, a.red_partial, a.red_ticket)) { a.red_result[0] = v[0]; a.red_result[1] = v[1]; a.red_result[2] = v[2]; }
         }
     }
 }

@@ -27,7 +27,7 @@ template <typename Real, int D, bool RL, int KSPLIT> struct Tune {
     static constexpr int MINB = LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? 4 : LIVE <= 168 ? 3 : LIVE <= 255 ? 2 : 1;
 };
 
-template <typename Real, int D, bool RL, int KSPLIT, bool MASS, int LHINT, int SHINT, int STHINT>
+template <typename Real, int D, bool RL, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT>
 static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
 {
     using T = Tune<Real, D, RL, KSPLIT>;
@@ -38,7 +38,11 @@ static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
     }
     const long nthreads = a.vh * KSPLIT;
     const long grid = (nthreads + block - 1) / block;
-    dphi_kernel<Real, D, RL, KSPLIT, MASS, LHINT, SHINT, STHINT, T::MAXT, T::MINB><<<(unsigned)grid, block, 0, st>>>(a);
+    if (RED && (unsigned long)grid > kRedMaxBlocks) {
+        set_error("fused Dphi reduction: %ld CTAs exceed the reduction scratch (%u)", grid, kRedMaxBlocks);
+        return HR_EUNSUPPORTED;
+    }
+    dphi_kernel<Real, D, RL, KSPLIT, MASS, RED, LHINT, SHINT, STHINT, T::MAXT, T::MINB><<<(unsigned)grid, block, 0, st>>>(a);
     count_launch();
     cudaError_t e = cudaPeekAtLastError();
     if (e != cudaSuccess) {
@@ -48,21 +52,21 @@ static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
     return HR_OK;
 }
 
-template <typename Real, int D, bool RL, bool MASS>
+template <typename Real, int D, bool RL, bool MASS, bool RED>
 static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaStream_t st)
 {
     constexpr int RPV = 16 / (int)sizeof(Real);
     constexpr bool PAIR_OK = (2 * D) % RPV == 0;
     switch (variant) {
-    case 0: return launch_one<Real, D, RL, 1, MASS, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
-    case 1: return launch_one<Real, D, RL, 1, MASS, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
+    case 0: return launch_one<Real, D, RL, 1, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+    case 1: return launch_one<Real, D, RL, 1, MASS, RED, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
     case 2:
-        if constexpr (PAIR_OK) return launch_one<Real, D, RL, 2, MASS, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+        if constexpr (PAIR_OK) return launch_one<Real, D, RL, 2, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
         break;
     case 3:
-        if constexpr (PAIR_OK) return launch_one<Real, D, RL, 2, MASS, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
+        if constexpr (PAIR_OK) return launch_one<Real, D, RL, 2, MASS, RED, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
         break;
-    case 4: return launch_one<Real, D, RL, 1, MASS, LD_DEFAULT, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+    case 4: return launch_one<Real, D, RL, 1, MASS, RED, LD_DEFAULT, LD_DEFAULT, ST_DEFAULT>(block, a, st);
     default: break;
     }
     set_error("dphi variant %d not available for d_R=%d, %s", variant, D, sizeof(Real) == 8 ? "fp64" : "fp32");
@@ -72,8 +76,9 @@ static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaS
 template <typename Real, int D, bool RL>
 hr_status launch_dphi_t(int variant, int block, const DphiArgs &a, cudaStream_t st)
 {
-    if (a.self) return launch_variant<Real, D, RL, true>(variant, block, a, st);
-    return launch_variant<Real, D, RL, false>(variant, block, a, st);
+    if (a.self && a.red_result) return launch_variant<Real, D, RL, true, true>(variant, block, a, st);
+    if (a.self) return launch_variant<Real, D, RL, true, false>(variant, block, a, st);
+    return launch_variant<Real, D, RL, false, false>(variant, block, a, st);
 }
 
 template <typename Real, int D, bool RL> bool dphi_variant_ok_t(int variant)

@@ -25,7 +25,7 @@ void set_error(const char *fmt, ...)
 }
 void count_launch(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
 
-static hr_status cuda_fail(const char *what, cudaError_t e)
+hr_status cuda_fail(const char *what, cudaError_t e)
 {
     set_error("%s: %s", what, cudaGetErrorString(e));
     return e == cudaErrorMemoryAllocation ? HR_ENOMEM : HR_ECUDA;
@@ -60,7 +60,7 @@ static bool combo_supported(int N, int rep)
 static bool valid_prec(int p) { return p == HR_F64 || p == HR_F32; }
 
 // is `p` device-accessible memory (device or managed)?  Host (pinned or pageable) -> false.
-static hr_status pointer_on_device(const void *p, bool *dev)
+hr_status pointer_on_device(const void *p, bool *dev)
 {
     cudaPointerAttributes at;
     cudaError_t e = cudaPointerGetAttributes(&at, p);
@@ -72,7 +72,7 @@ static hr_status pointer_on_device(const void *p, bool *dev)
     return HR_OK;
 }
 
-static hr_status use_device(const hr_ctx *c)
+hr_status use_device(const hr_ctx *c)
 {
     cudaError_t e = cudaSetDevice(c->device);
     if (e != cudaSuccess) {
@@ -179,6 +179,8 @@ hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N,
     c->ws_in = c->ws_out = c->ws_stage = nullptr;
     c->ws_spinor_bytes = c->ws_stage_bytes = 0;
     c->ws_prec = -1;
+    c->red_scratch = nullptr;
+    c->red_scratch_bytes = 0;
     *ctx = c;
     return HR_OK;
 }
@@ -186,11 +188,12 @@ hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N,
 void hr_ctx_destroy(hr_ctx *ctx)
 {
     if (!ctx) return;
-    if (ctx->ws_in || ctx->ws_out || ctx->ws_stage) {
+    if (ctx->ws_in || ctx->ws_out || ctx->ws_stage || ctx->red_scratch) {
         if (cudaSetDevice(ctx->device) == cudaSuccess) {
             cudaFree(ctx->ws_in);
             cudaFree(ctx->ws_out);
             cudaFree(ctx->ws_stage);
+            cudaFree(ctx->red_scratch);
         }
         cudaGetLastError();
     }
@@ -318,8 +321,12 @@ static int default_xblock(const hr_ctx *c, hr_prec prec)
     return best;
 }
 
-static hr_status dphi_args(DphiArgs &a, const hr_ctx *c, void *out, const void *in, const void *self, const hr_gauge *links,
-                           int parity, double mass)
+} // extern "C"
+
+namespace hr {
+// Fill the launch arguments of one Dphi launch: out = alpha (.) self + beta (.) sum_hops, see DphiArgs.
+void dphi_args(DphiArgs &a, const hr_ctx *c, void *out, const void *in, const void *self, const hr_gauge *links,
+               int parity, const double alpha[2], const double beta[2])
 {
     a.Xb = c->xblock > 0 ? c->xblock : default_xblock(c, links->prec);
     a.out = out;
@@ -333,9 +340,37 @@ static hr_status dphi_args(DphiArgs &a, const hr_ctx *c, void *out, const void *
     a.parity = parity;
     for (int m = 0; m < 4; ++m) a.bc[m] = c->bc[m];
     a.vh = c->Vh;
-    a.mass = mass;
+    a.alpha[0] = alpha[0]; a.alpha[1] = alpha[1];
+    a.beta[0] = beta[0]; a.beta[1] = beta[1];
+    for (int i = 0; i < 2; ++i) { a.alphaf[i] = (float)alpha[i]; a.betaf[i] = (float)beta[i]; }
+    a.red_partial = nullptr;
+    a.red_ticket = nullptr;
+    a.red_result = nullptr;
+    a.skip = nullptr;
+}
+
+// Reduction scratch of the ctx: [3 * kRedMaxBlocks doubles of per-CTA partials][16 doubles of results][ticket].
+hr_status get_red_scratch(hr_ctx *c, RedScratch *r, cudaStream_t st)
+{
+    const size_t pbytes = (size_t)3 * kRedMaxBlocks * sizeof(double);
+    const size_t total = pbytes + 16 * sizeof(double) + 64;
+    if (!c->red_scratch) {
+        void *m = nullptr;
+        cudaError_t e = cudaMalloc(&m, total);
+        if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail("reduction scratch: cudaMalloc", e); }
+        e = cudaMemsetAsync(m, 0, total, st);
+        if (e != cudaSuccess) { cudaFree(m); return cuda_fail("reduction scratch: cudaMemsetAsync", e); }
+        c->red_scratch = m;
+        c->red_scratch_bytes = total;
+    }
+    r->partial = (double *)c->red_scratch;
+    r->result = (double *)((char *)c->red_scratch + pbytes);
+    r->ticket = (unsigned *)((char *)c->red_scratch + pbytes + 16 * sizeof(double));
     return HR_OK;
 }
+} // namespace hr
+
+extern "C" {
 
 hr_status hr_dphi_eo(void *out, const void *in, const hr_gauge *links, int parity, void *stream)
 {
@@ -348,7 +383,8 @@ hr_status hr_dphi_eo(void *out, const void *in, const hr_gauge *links, int parit
     hr_status rc = use_device(c);
     if (rc != HR_OK) return rc;
     DphiArgs a;
-    dphi_args(a, c, out, in, nullptr, links, parity, 0.0);
+    const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 };
+    dphi_args(a, c, out, in, nullptr, links, parity, zero, mhalf);
     return launch_dphi(c, links->prec, a, (cudaStream_t)stream);
 }
 
@@ -367,7 +403,8 @@ hr_status hr_dirac(double m0, void *out_full, const void *in_full, const hr_gaug
         char *o = (char *)out_full + (size_t)p * half;
         const char *i_other = (const char *)in_full + (size_t)(1 - p) * half;
         const char *i_self = (const char *)in_full + (size_t)p * half;
-        dphi_args(a, c, o, i_other, i_self, links, p, 4.0 + m0);
+        const double mass[2] = { 4.0 + m0, 4.0 + m0 }, mhalf[2] = { -0.5, -0.5 };
+        dphi_args(a, c, o, i_other, i_self, links, p, mass, mhalf);
         rc = launch_dphi(c, links->prec, a, (cudaStream_t)stream);
         if (rc != HR_OK) return rc;
     }

@@ -1,0 +1,259 @@
+// hr_api_solver.cu -- C-ABI entry points of the rows SURVEY.md section 8(f) NEXT-1 adds (include/hr.h,
+// second part): spinor linear algebra, the even-odd preconditioned operator Dhat, and the CG / full solve
+// built on them.  Argument checking and launch sequencing only; the arithmetic is in linalg.cu, cg.cu and
+// the Dphi kernels.  No CPU fallback.
+#include <cstring>
+
+#include "hr_internal.h"
+
+using namespace hr;
+
+#define HR_CUDA(call)                                                                                     \
+    do {                                                                                                  \
+        cudaError_t e_ = (call);                                                                          \
+        if (e_ != cudaSuccess) return cuda_fail(#call, e_);                                               \
+    } while (0)
+
+static bool valid_prec(int p) { return p == HR_F64 || p == HR_F32; }
+static bool aligned16(const void *p) { return ((uintptr_t)p & 15) == 0; }
+
+// copy `n` doubles of a device result to `dst`, which may be host (synchronises) or device memory
+static hr_status deliver(double *dst, const double *src_dev, int n, cudaStream_t st)
+{
+    bool dev = false;
+    hr_status rc = pointer_on_device(dst, &dev);
+    if (rc != HR_OK) return rc;
+    HR_CUDA(cudaMemcpyAsync(dst, src_dev, (size_t)n * sizeof(double), dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    if (!dev) HR_CUDA(cudaStreamSynchronize(st));
+    return HR_OK;
+}
+
+// tmp_o = Dphi_oe in ; out = [gamma5] (m^2 in - Dphi_eo tmp_o).  red != null: also reduce |out|^2, <in,out>.
+static hr_status dhat_launches(const hr_ctx *c, double m0, int g5, void *out_e, const void *in_e, void *tmp_o,
+                               const hr_gauge *links, const RedScratch *rs, double *red_result, const int *skip,
+                               cudaStream_t st)
+{
+    const double m = 4.0 + m0;
+    const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 };
+    DphiArgs a;
+    dphi_args(a, c, tmp_o, in_e, nullptr, links, 1, zero, mhalf);
+    a.skip = skip;
+    hr_status rc = launch_dphi(c, links->prec, a, st);
+    if (rc != HR_OK) return rc;
+    const double s = g5 ? -1.0 : 1.0;
+    const double alpha[2] = { m * m, s * m * m }, beta[2] = { 0.5, s * 0.5 }; // -Dphi = +1/2 sum_hops
+    dphi_args(a, c, out_e, tmp_o, in_e, links, 0, alpha, beta);
+    a.skip = skip;
+    if (rs) {
+        a.red_partial = rs->partial;
+        a.red_ticket = rs->ticket;
+        a.red_result = red_result;
+    }
+    return launch_dphi(c, links->prec, a, st);
+}
+
+extern "C" {
+
+hr_status hr_spinor_lincomb(const hr_ctx *ctx, hr_prec prec, void *out, const double ca[2], int g5, const void *x,
+                            const double cb[2], const void *y, void *stream)
+{
+    if (!ctx || !out || !x || !ca || !valid_prec(prec) || (y && !cb)) { set_error("hr_spinor_lincomb: bad argument"); return HR_EINVAL; }
+    if (!aligned16(out) || !aligned16(x) || !aligned16(y)) { set_error("hr_spinor_lincomb: buffers must be 16-byte aligned"); return HR_EINVAL; }
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    const double zero[2] = { 0.0, 0.0 };
+    return launch_lincomb(ctx, prec, out, ca, g5 != 0, x, y ? cb : zero, y, (cudaStream_t)stream);
+}
+
+hr_status hr_spinor_copy(const hr_ctx *ctx, hr_prec prec, void *out, const void *in, void *stream)
+{
+    const double one[2] = { 1.0, 0.0 };
+    return hr_spinor_lincomb(ctx, prec, out, one, 0, in, nullptr, nullptr, stream);
+}
+
+hr_status hr_spinor_g5(const hr_ctx *ctx, hr_prec prec, void *out, const void *in, void *stream)
+{
+    const double one[2] = { 1.0, 0.0 };
+    return hr_spinor_lincomb(ctx, prec, out, one, 1, in, nullptr, nullptr, stream);
+}
+
+hr_status hr_spinor_mulc_add_assign(const hr_ctx *ctx, hr_prec prec, void *out, double c_re, double c_im, const void *in,
+                                    void *stream)
+{
+    const double c[2] = { c_re, c_im }, one[2] = { 1.0, 0.0 };
+    return hr_spinor_lincomb(ctx, prec, out, c, 0, in, one, out, stream);
+}
+
+hr_status hr_spinor_g5_mulc_add_assign(const hr_ctx *ctx, hr_prec prec, void *out, double c_re, double c_im, const void *in,
+                                       void *stream)
+{
+    const double c[2] = { c_re, c_im }, one[2] = { 1.0, 0.0 };
+    return hr_spinor_lincomb(ctx, prec, out, c, 1, in, one, out, stream);
+}
+
+hr_status hr_spinor_dot(hr_ctx *ctx, hr_prec prec, const void *x, const void *y, double *result, void *stream)
+{
+    if (!ctx || !x || !y || !result || !valid_prec(prec)) { set_error("hr_spinor_dot: bad argument"); return HR_EINVAL; }
+    if (!aligned16(x) || !aligned16(y)) { set_error("hr_spinor_dot: buffers must be 16-byte aligned"); return HR_EINVAL; }
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    RedScratch rs;
+    rc = get_red_scratch(ctx, &rs, st);
+    if (rc != HR_OK) return rc;
+    rc = launch_dot(ctx, prec, x, y, rs, rs.result, st);
+    if (rc != HR_OK) return rc;
+    return deliver(result, rs.result, 2, st);
+}
+
+hr_status hr_spinor_norm2(hr_ctx *ctx, hr_prec prec, const void *x, double *result, void *stream)
+{
+    if (!ctx || !x || !result || !valid_prec(prec)) { set_error("hr_spinor_norm2: bad argument"); return HR_EINVAL; }
+    if (!aligned16(x)) { set_error("hr_spinor_norm2: buffer must be 16-byte aligned"); return HR_EINVAL; }
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    RedScratch rs;
+    rc = get_red_scratch(ctx, &rs, st);
+    if (rc != HR_OK) return rc;
+    rc = launch_dot(ctx, prec, x, x, rs, rs.result, st);
+    if (rc != HR_OK) return rc;
+    return deliver(result, rs.result, 1, st);
+}
+
+hr_status hr_dhat(double m0, int g5, void *out_e, const void *in_e, void *tmp_o, const hr_gauge *links, void *stream)
+{
+    if (!out_e || !in_e || !tmp_o || !links) { set_error("hr_dhat: NULL argument"); return HR_EINVAL; }
+    if (!links->represented) { set_error("hr_dhat: `links` must be a represented field"); return HR_EINVAL; }
+    if (out_e == in_e || out_e == tmp_o || in_e == tmp_o) { set_error("hr_dhat: out, in and tmp must be distinct buffers"); return HR_EINVAL; }
+    if (!aligned16(out_e) || !aligned16(in_e) || !aligned16(tmp_o)) { set_error("hr_dhat: buffers must be 16-byte aligned"); return HR_EINVAL; }
+    const hr_ctx *c = links->ctx;
+    hr_status rc = use_device(c);
+    if (rc != HR_OK) return rc;
+    return dhat_launches(c, m0, g5 != 0, out_e, in_e, tmp_o, links, nullptr, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+size_t hr_cg_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter)
+{
+    if (!ctx || !valid_prec(prec) || maxiter < 0) return 0;
+    const size_t sb = (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec);
+    const size_t state = (sizeof(CgState) + ((size_t)maxiter + 2) * sizeof(double) + 255) & ~(size_t)255;
+    return 5 * sb + state;
+}
+
+// CG on (gamma5 Dhat)^2 x = rhs with rhs already in ws.r; see hr.h
+static hr_status cg_run(hr_ctx *c, double m0, void *x_e, const hr_gauge *links, double tol, int maxiter, char *ws,
+                        int *iters, double *rel_res2, double *hist_host, cudaStream_t st)
+{
+    const hr_prec prec = links->prec;
+    const size_t sb = (size_t)c->Vh * 8 * c->d * prec_bytes(prec);
+    void *r = ws, *p = ws + sb, *t = ws + 2 * sb, *ap = ws + 3 * sb, *tmp = ws + 4 * sb;
+    CgState *cs = (CgState *)(ws + 5 * sb);
+    RedScratch rs;
+    hr_status rc = get_red_scratch(c, &rs, st);
+    if (rc != HR_OK) return rc;
+    rc = launch_cg_init(c, prec, cs, tol, maxiter, x_e, p, r, rs, st);
+    if (rc != HR_OK) return rc;
+    CgState h;
+    memset(&h, 0, sizeof h);
+    // iterations are enqueued in batches; the host looks at the device state once per batch.  A batch
+    // that overshoots costs only empty launches (every kernel returns at once when `done` is set).
+    int batch = 4;
+    for (int issued = 0;;) {
+        HR_CUDA(cudaMemcpyAsync(&h, cs, sizeof h, cudaMemcpyDeviceToHost, st));
+        HR_CUDA(cudaStreamSynchronize(st));
+        if (h.done || issued >= maxiter) break;
+        int n = maxiter - issued < batch ? maxiter - issued : batch;
+        for (int i = 0; i < n; ++i) {
+            rc = dhat_launches(c, m0, 1, t, p, tmp, links, &rs, &cs->pap, &cs->done, st);   // t = Q p, pap = |Q p|^2
+            if (rc != HR_OK) return rc;
+            rc = dhat_launches(c, m0, 1, ap, t, tmp, links, nullptr, nullptr, &cs->done, st); // Ap = Q t
+            if (rc != HR_OK) return rc;
+            rc = launch_cg_update_r(c, prec, cs, r, ap, rs, st);
+            if (rc != HR_OK) return rc;
+            rc = launch_cg_update_xp(c, prec, cs, x_e, p, r, st);
+            if (rc != HR_OK) return rc;
+        }
+        issued += n;
+        if (batch < 32) batch *= 2;
+    }
+    if (iters) *iters = h.iter;
+    if (rel_res2 || hist_host) {
+        const int n = h.iter + 1;
+        if (hist_host) {
+            HR_CUDA(cudaMemcpyAsync(hist_host, (const double *)(cs + 1), (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, st));
+            HR_CUDA(cudaStreamSynchronize(st));
+            if (rel_res2) *rel_res2 = h.bb > 0 ? hist_host[h.iter] / h.bb : 0.0;
+            if (h.bb > 0) for (int k = 0; k < n; ++k) hist_host[k] /= h.bb;
+        } else {
+            double last = 0;
+            HR_CUDA(cudaMemcpyAsync(&last, (const double *)(cs + 1) + h.iter, sizeof(double), cudaMemcpyDeviceToHost, st));
+            HR_CUDA(cudaStreamSynchronize(st));
+            *rel_res2 = h.bb > 0 ? last / h.bb : 0.0;
+        }
+    }
+    return HR_OK;
+}
+
+static hr_status cg_check(const char *who, hr_ctx *ctx, const void *x, const void *b, const hr_gauge *links, double tol,
+                          int maxiter, const void *ws)
+{
+    if (!ctx || !x || !b || !links || !ws) { set_error("%s: NULL argument", who); return HR_EINVAL; }
+    if (links->ctx != ctx) { set_error("%s: `links` belongs to a different context", who); return HR_EINVAL; }
+    if (!links->represented) { set_error("%s: `links` must be a represented field", who); return HR_EINVAL; }
+    if (!(tol >= 0.0) || maxiter < 0) { set_error("%s: tol=%g maxiter=%d", who, tol, maxiter); return HR_EINVAL; }
+    if (x == b) { set_error("%s: x aliases b", who); return HR_EINVAL; }
+    if (!aligned16(x) || !aligned16(b) || ((uintptr_t)ws & 255)) { set_error("%s: buffers must be 16-byte (workspace 256-byte) aligned", who); return HR_EINVAL; }
+    return use_device(ctx);
+}
+
+hr_status hr_cg_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol, int maxiter,
+                     void *workspace, int *iters, double *rel_res2, double *hist, void *stream)
+{
+    hr_status rc = cg_check("hr_cg_dhat", ctx, x_e, b_e, links, tol, maxiter, workspace);
+    if (rc != HR_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    char *ws = (char *)workspace;
+    const size_t sb = (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(links->prec);
+    // rhs = Dhat^dagger b = Q gamma5 b  (reading C21): t = gamma5 b ; r = Q t
+    const double one[2] = { 1.0, 0.0 }, zero[2] = { 0.0, 0.0 };
+    rc = launch_lincomb(ctx, links->prec, ws + 2 * sb, one, 1, b_e, zero, nullptr, st);
+    if (rc != HR_OK) return rc;
+    rc = dhat_launches(ctx, m0, 1, ws, ws + 2 * sb, ws + 4 * sb, links, nullptr, nullptr, nullptr, st);
+    if (rc != HR_OK) return rc;
+    return cg_run(ctx, m0, x_e, links, tol, maxiter, ws, iters, rel_res2, hist, st);
+}
+
+hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links, double tol,
+                         int maxiter, void *workspace, int *iters, double *rel_res2, void *stream)
+{
+    hr_status rc = cg_check("hr_dirac_solve", ctx, x_full, b_full, links, tol, maxiter, workspace);
+    if (rc != HR_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const hr_prec prec = links->prec;
+    char *ws = (char *)workspace;
+    const size_t sb = (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec);
+    const double m = 4.0 + m0;
+    char *x_e = (char *)x_full, *x_o = (char *)x_full + sb;
+    const char *b_e = (const char *)b_full, *b_o = (const char *)b_full + sb;
+    // reading C24:  bhat = m b_e - Dphi_eo b_o  (kept in the x_o slot until the end)
+    DphiArgs a;
+    const double am[2] = { m, m }, half[2] = { 0.5, 0.5 };
+    dphi_args(a, ctx, x_o, b_o, b_e, links, 0, am, half);
+    rc = launch_dphi(ctx, prec, a, st);
+    if (rc != HR_OK) return rc;
+    // rhs of the normal equations: r = Q gamma5 bhat
+    const double one[2] = { 1.0, 0.0 }, zero[2] = { 0.0, 0.0 };
+    rc = launch_lincomb(ctx, prec, ws + 2 * sb, one, 1, x_o, zero, nullptr, st);
+    if (rc != HR_OK) return rc;
+    rc = dhat_launches(ctx, m0, 1, ws, ws + 2 * sb, ws + 4 * sb, links, nullptr, nullptr, nullptr, st);
+    if (rc != HR_OK) return rc;
+    rc = cg_run(ctx, m0, x_e, links, tol, maxiter, ws, iters, rel_res2, nullptr, st);
+    if (rc != HR_OK) return rc;
+    // x_o = (b_o - Dphi_oe x_e) / m
+    const double ainv[2] = { 1.0 / m, 1.0 / m }, binv[2] = { 0.5 / m, 0.5 / m };
+    dphi_args(a, ctx, x_o, x_e, b_o, links, 1, ainv, binv);
+    return launch_dphi(ctx, prec, a, st);
+}
+
+} // extern "C"

@@ -34,6 +34,10 @@ struct hr_ctx {
     void *ws_in, *ws_out, *ws_stage;
     size_t ws_spinor_bytes, ws_stage_bytes;
     int ws_prec;
+    // reduction scratch (hr_spinor_dot / norm2, fused Dphi reductions, CG): per-CTA partial sums, the
+    // self-resetting ticket counter and a small result area; created on first use, one stream at a time
+    void *red_scratch;
+    size_t red_scratch_bytes;
 };
 
 struct hr_gauge {
@@ -50,6 +54,12 @@ namespace hr {
 
 void set_error(const char *fmt, ...);
 void count_launch(int n = 1);
+hr_status cuda_fail(const char *what, cudaError_t e);
+hr_status use_device(const hr_ctx *c);
+hr_status pointer_on_device(const void *p, bool *dev);
+struct DphiArgs;
+void dphi_args(DphiArgs &a, const hr_ctx *c, void *out, const void *in, const void *self, const hr_gauge *links,
+               int parity, const double alpha[2], const double beta[2]);
 
 static inline size_t prec_bytes(hr_prec p) { return p == HR_F64 ? 8 : 4; }
 static inline int link_nreal(const hr_ctx *c, int represented)
@@ -69,8 +79,40 @@ struct DphiArgs {
     int parity;
     int bc[4];
     long vh;
-    double mass; // 4 + m0
+    // epilogue: out_alpha = alpha[alpha>>1] * self_alpha + beta[alpha>>1] * (sum over the 8 hops)_alpha;
+    // index 0 = spin components 0,1, index 1 = components 2,3 (gamma5 = diag(1,1,-1,-1) is a sign
+    // pattern on these).  Without self (plain Dphi) the kernel uses beta = -1/2 as a compile-time constant.
+    double alpha[2], beta[2];
+    float alphaf[2], betaf[2]; // the same, rounded once on the host: constant-bank operands of the fp32 kernels
+    // fused reduction of the epilogue (RED): result[0] = sum |out|^2, result[1..2] = <self, out>
+    double *red_partial;   // [gridDim.x][3]
+    unsigned *red_ticket;  // zero before the launch; the last CTA resets it
+    double *red_result;    // [3], device
+    const int *skip;       // if non-null and *skip != 0 the launch does nothing (converged CG)
 };
+
+// device-resident state of the CG (cg.cu); the host only reads it
+struct CgState {
+    double bb;        // |rhs|^2
+    double tol2;      // tol^2
+    double pap;       // <p, A p> of the current iteration  (= |Q p|^2, written by the fused Dphi reduction)
+    double pap_pad[2];
+    int iter;         // completed iterations k
+    int maxiter;
+    int done;         // set by the r-update when rr_k <= tol^2 bb or k == maxiter: later Dphi / r-updates are no-ops
+    int frozen;       // set by the first skipped r-update: later x/p-updates are no-ops (the x/p-update of the
+                      // iteration that detected convergence still runs)
+    // rr[k] = |r_k|^2, k = 0..maxiter, follows this header
+};
+
+// number of CTAs the reduction scratch provides partial-sum slots for
+static const unsigned kRedMaxBlocks = 1u << 20;
+struct RedScratch {
+    double *partial;
+    unsigned *ticket;
+    double *result;
+};
+hr_status get_red_scratch(hr_ctx *c, RedScratch *r, cudaStream_t st);
 
 // returns HR_OK / HR_EUNSUPPORTED / HR_ECUDA
 hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st);
@@ -79,6 +121,21 @@ bool dphi_variant_valid(const hr_ctx *c, int variant);
 
 hr_status launch_represent(const hr_ctx *c, hr_prec in_prec, const void *fund, hr_prec out_prec, void *repr,
                            cudaStream_t st);
+
+// spinor linear algebra on internal-layout half fields (linalg.cu).  nvec = 16-byte vectors per field.
+//   out = ca * G(x) + cb * y   (G = gamma5 if g5 else identity; y may be null; out may alias x or y)
+hr_status launch_lincomb(const hr_ctx *c, hr_prec prec, void *out, const double ca[2], int g5, const void *x,
+                         const double cb[2], const void *y, cudaStream_t st);
+//   result[0..1] = <x, y> (result[0] = |x|^2 when x == y), device pointer
+hr_status launch_dot(const hr_ctx *c, hr_prec prec, const void *x, const void *y, const RedScratch &rs,
+                     double *result_dev, cudaStream_t st);
+// CG building blocks on the device-resident CgState (cg.cu)
+hr_status launch_cg_init(const hr_ctx *c, hr_prec prec, CgState *cs, double tol, int maxiter, void *x, void *p,
+                         const void *r, const RedScratch &rs, cudaStream_t st);
+hr_status launch_cg_update_r(const hr_ctx *c, hr_prec prec, CgState *cs, void *r, const void *Ap,
+                             const RedScratch &rs, cudaStream_t st);
+hr_status launch_cg_update_xp(const hr_ctx *c, hr_prec prec, const CgState *cs, void *x, void *p, const void *r,
+                              cudaStream_t st);
 
 // pack / unpack: canonical AoS (device pointer) <-> internal planes
 hr_status launch_pack_spinor(const hr_ctx *c, void *dst, hr_prec prec, const void *canon_dev, hr_prec cprec,
@@ -278,6 +335,59 @@ __device__ __forceinline__ void store_record(char *base, size_t vh, size_t s, co
     float *t = (float *)(base + (size_t)R::NV * 16 * vh) + s * R::TAIL;
 #pragma unroll
     for (int e = 0; e < R::TAIL; ++e) t[e] = src[R::NV * 4 + e];
+}
+
+// ---- one-pass grid reduction (replaces the paper's two-kernel cub scheme) -------------
+// Every CTA reduces its threads' NRED fp64 partial sums (shuffle tree, then a fixed-order sum over the
+// warps), writes them to partial[blockIdx.x][NRED] and takes a ticket; the CTA that draws the last ticket
+// sums the per-CTA partials in an order that depends only on the launch geometry -- the result is
+// bitwise reproducible run to run (reading C15) -- and leaves the totals in v[] of its thread 0.
+// Returns true on exactly that thread.  atomicInc wraps the ticket back to 0 for the next launch.
+template <int NRED>
+__device__ __forceinline__ bool grid_reduce(double (&v)[NRED], double *partial, unsigned *ticket)
+{
+    __shared__ double sm[32][NRED];
+    __shared__ bool last;
+    const int tid = threadIdx.x + threadIdx.y * blockDim.x;
+    const int nthr = blockDim.x * blockDim.y;
+    const int lane = tid & 31, warp = tid >> 5, nwarp = (nthr + 31) >> 5;
+    auto block_sum = [&]() {
+#pragma unroll
+        for (int i = 0; i < NRED; ++i)
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+        if (lane == 0)
+#pragma unroll
+            for (int i = 0; i < NRED; ++i) sm[warp][i] = v[i];
+        __syncthreads();
+        if (tid == 0)
+#pragma unroll
+            for (int i = 0; i < NRED; ++i) {
+                double t = 0;
+                for (int w = 0; w < nwarp; ++w) t += sm[w][i];
+                v[i] = t;
+            }
+    };
+    block_sum();
+    if (tid == 0) {
+#pragma unroll
+        for (int i = 0; i < NRED; ++i) partial[(size_t)blockIdx.x * NRED + i] = v[i];
+        __threadfence();
+        const unsigned t = atomicInc(ticket, gridDim.x - 1);
+        last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!last) return false;
+    __threadfence();
+#pragma unroll
+    for (int i = 0; i < NRED; ++i) {
+        double t = 0;
+        for (unsigned b = tid; b < gridDim.x; b += nthr) t += __ldcg(&partial[(size_t)b * NRED + i]);
+        v[i] = t;
+    }
+    __syncthreads(); // sm is re-used
+    block_sum();
+    return tid == 0;
 }
 
 } // namespace hr

@@ -1,0 +1,161 @@
+// linalg.cu -- spinor linear algebra on internal-layout half fields (
+// PAPER.md:108-120, Fig. 7: "Copy spinor field", "g5 application", "g5 mulc add assign", inner products
+// and norms).  Readings C22/C23: <a,b> = sum conj(a) b, sums in fp64; "g5 mulc add assign"
+// is out += c gamma5 in.
+//
+// A half field is NV planes of Vh 16-byte vectors (hr_internal.h); every vector holds whole complex
+// numbers, and gamma5 = diag(1,1,-1,-1) is +1 on the first NV/2 planes and -1 on the rest, so all of
+// these are flat streaming kernels over nvec = NV*Vh vectors: 128-bit loads/stores, four independent
+// vectors in flight per thread, grid = a multiple of the SM count.
+// Reductions are ONE kernel (grid_reduce, hr_internal.h) instead of the paper's site-wise kernel followed
+// by a cub reduction: the field is read once and nothing but per-CTA partials is written.
+#include "hr_internal.h"
+
+namespace hr {
+
+template <typename Real> struct Vec16;
+template <> struct Vec16<double> { using type = double2; };
+template <> struct Vec16<float> { using type = float4; };
+
+// a * b for the complex numbers packed in one 16-byte vector; a = (ar, ai) broadcast
+__device__ __forceinline__ double2 cmul(double ar, double ai, double2 b) { return make_double2(ar * b.x - ai * b.y, ar * b.y + ai * b.x); }
+__device__ __forceinline__ float4 cmul(float ar, float ai, float4 b)
+{
+    return make_float4(ar * b.x - ai * b.y, ar * b.y + ai * b.x, ar * b.z - ai * b.w, ar * b.w + ai * b.z);
+}
+__device__ __forceinline__ double2 vadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float4 vadd(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
+__device__ __forceinline__ void dot_acc(double &re, double &im, double2 a, double2 b)
+{
+    re = fma(a.x, b.x, fma(a.y, b.y, re));
+    im = fma(a.x, b.y, fma(-a.y, b.x, im));
+}
+__device__ __forceinline__ void dot_acc(double &re, double &im, float4 a, float4 b)
+{
+    // the products of one vector in fp32 (exact to 2^-24 each), the running sums in fp64 (reading C22)
+    re += (double)(a.x * b.x + a.y * b.y) + (double)(a.z * b.z + a.w * b.w);
+    im += (double)(a.x * b.y - a.y * b.x) + (double)(a.z * b.w - a.w * b.z);
+}
+
+constexpr int LIN_THREADS = 256;
+constexpr int LIN_UNROLL = 4;
+
+// out = ca * G(x) + cb * y
+template <typename Real, bool G5, bool HAS_Y>
+__global__ void __launch_bounds__(LIN_THREADS) lincomb_kernel(typename Vec16<Real>::type *out, const typename Vec16<Real>::type *x,
+                                                              const typename Vec16<Real>::type *y, Real car, Real cai, Real cbr,
+                                                              Real cbi, size_t nvec, size_t half)
+{
+    using V = typename Vec16<Real>::type;
+    const size_t base = (size_t)blockIdx.x * (LIN_THREADS * LIN_UNROLL) + threadIdx.x;
+    V xv[LIN_UNROLL], yv[LIN_UNROLL];
+#pragma unroll
+    for (int u = 0; u < LIN_UNROLL; ++u) {
+        const size_t i = base + (size_t)u * LIN_THREADS;
+        if (i < nvec) {
+            xv[u] = x[i];
+            if constexpr (HAS_Y) yv[u] = y[i];
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < LIN_UNROLL; ++u) {
+        const size_t i = base + (size_t)u * LIN_THREADS;
+        if (i < nvec) {
+            const Real sg = (G5 && i >= half) ? (Real)-1 : (Real)1;
+            V r = cmul(sg * car, sg * cai, xv[u]);
+            if constexpr (HAS_Y) r = vadd(r, cmul(cbr, cbi, yv[u]));
+            out[i] = r;
+        }
+    }
+}
+
+// v[0] + i v[1] = <x, y>; SAME: y == x, one read
+template <typename Real, bool SAME>
+__global__ void __launch_bounds__(LIN_THREADS) dot_kernel(const typename Vec16<Real>::type *x, const typename Vec16<Real>::type *y,
+                                                          size_t nvec, double *partial, unsigned *ticket, double *result)
+{
+    using V = typename Vec16<Real>::type;
+    double v[2] = { 0.0, 0.0 };
+    const size_t stride = (size_t)gridDim.x * (LIN_THREADS * LIN_UNROLL);
+    for (size_t b0 = (size_t)blockIdx.x * (LIN_THREADS * LIN_UNROLL); b0 < nvec; b0 += stride) {
+        V xv[LIN_UNROLL], yv[LIN_UNROLL];
+#pragma unroll
+        for (int u = 0; u < LIN_UNROLL; ++u) {
+            const size_t i = b0 + threadIdx.x + (size_t)u * LIN_THREADS;
+            if (i < nvec) {
+                xv[u] = x[i];
+                if constexpr (!SAME) yv[u] = y[i];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < LIN_UNROLL; ++u) {
+            const size_t i = b0 + threadIdx.x + (size_t)u * LIN_THREADS;
+            if (i < nvec) dot_acc(v[0], v[1], xv[u], SAME ? xv[u] : yv[u]);
+        }
+    }
+    if (grid_reduce<2>(v, partial, ticket)) {
+        result[0] = v[0];
+        result[1] = SAME ? 0.0 : v[1];
+    }
+}
+
+static inline size_t field_nvec(const hr_ctx *c, hr_prec prec) { return (size_t)c->Vh * 8 * c->d * prec_bytes(prec) / 16; }
+
+// CTAs of a grid-stride reduction: enough to fill the machine, never more than the work
+unsigned reduce_grid(size_t nvec)
+{
+    const size_t need = (nvec + LIN_THREADS * LIN_UNROLL - 1) / (LIN_THREADS * LIN_UNROLL);
+    const size_t cap = 148 * 8;
+    return (unsigned)(need < cap ? (need ? need : 1) : cap);
+}
+
+static hr_status check_launch(const char *what)
+{
+    count_launch();
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) {
+        set_error("%s launch failed: %s", what, cudaGetErrorString(e));
+        return HR_ECUDA;
+    }
+    return HR_OK;
+}
+
+template <typename Real>
+static hr_status lincomb_t(void *out, const double ca[2], int g5, const void *x, const double cb[2], const void *y, size_t nvec,
+                           cudaStream_t st)
+{
+    using V = typename Vec16<Real>::type;
+    const unsigned grid = (unsigned)((nvec + LIN_THREADS * LIN_UNROLL - 1) / (LIN_THREADS * LIN_UNROLL));
+    const Real car = (Real)ca[0], cai = (Real)ca[1], cbr = y ? (Real)cb[0] : 0, cbi = y ? (Real)cb[1] : 0;
+#define GO(G5, HY) lincomb_kernel<Real, G5, HY><<<grid, LIN_THREADS, 0, st>>>((V *)out, (const V *)x, (const V *)y, car, cai, cbr, cbi, nvec, nvec / 2)
+    if (g5) { if (y) GO(true, true); else GO(true, false); }
+    else    { if (y) GO(false, true); else GO(false, false); }
+#undef GO
+    return check_launch("lincomb_kernel");
+}
+
+hr_status launch_lincomb(const hr_ctx *c, hr_prec prec, void *out, const double ca[2], int g5, const void *x, const double cb[2],
+                         const void *y, cudaStream_t st)
+{
+    const size_t nvec = field_nvec(c, prec);
+    return prec == HR_F64 ? lincomb_t<double>(out, ca, g5, x, cb, y, nvec, st) : lincomb_t<float>(out, ca, g5, x, cb, y, nvec, st);
+}
+
+template <typename Real>
+static hr_status dot_t(const void *x, const void *y, size_t nvec, const RedScratch &rs, double *result, cudaStream_t st)
+{
+    using V = typename Vec16<Real>::type;
+    const unsigned grid = reduce_grid(nvec);
+    if (x == y) dot_kernel<Real, true><<<grid, LIN_THREADS, 0, st>>>((const V *)x, (const V *)y, nvec, rs.partial, rs.ticket, result);
+    else dot_kernel<Real, false><<<grid, LIN_THREADS, 0, st>>>((const V *)x, (const V *)y, nvec, rs.partial, rs.ticket, result);
+    return check_launch("dot_kernel");
+}
+
+hr_status launch_dot(const hr_ctx *c, hr_prec prec, const void *x, const void *y, const RedScratch &rs, double *result_dev,
+                     cudaStream_t st)
+{
+    const size_t nvec = field_nvec(c, prec);
+    return prec == HR_F64 ? dot_t<double>(x, y, nvec, rs, result_dev, st) : dot_t<float>(x, y, nvec, rs, result_dev, st);
+}
+
+} // namespace hr
