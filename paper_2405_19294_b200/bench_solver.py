@@ -1,0 +1,106 @@
+#!/usr/bin/env python
+"""Measurement of the NEXT-1 rows: the paper's second benchmark, the spinor linear
+algebra of PAPER.md:108-120 / Fig. 7 ("Copy spinor field", "g5 application", "g5 mulc add assign", norms and
+inner products; SU(3) fundamental), plus hr_dhat and one CG iteration.
+
+    python -m paper_2405_19294_b200.bench_solver [--config 2|3|4|5] [--prec f64|f32] [--reps 50]
+
+Prints one JSON line per operation: algorithmic bytes (S = spinor bytes per site, Vh sites: copy/g5 2S,
+g5_mulc_add_assign 3S, norm2 1S, dot 2S; Dhat 2(8L+2S)+S; CG iteration 4(8L+2S) + 2S + 8S), the time per call
+from CUDA events on the launching stream (back to back, fields larger than L2 rotate through 4 buffer sets),
+GB/s and the fraction of the measured copy peak (MEASURED_PEAKS.json).  Inputs: the seeded synthetic fields
+of bench.py's configs.  bench.py stays the headline; this script is the Fig. 7 companion."""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+
+def main():
+    import torch
+    import bench as B
+    import paper_2405_19294_b200 as hr
+
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--reps", type=int, default=50)
+    ap.add_argument("--m0", type=float, default=0.1)
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench_solver: no CUDA device; the product path has no CPU fallback")
+    cfg = B.CONFIGS[args.config]
+    bm = B.byte_model(cfg, args.prec)
+    P = hr.PREC_NAMES[args.prec]
+    peak, peak_src = B.measured_peak()
+    U, psi = B.make_fields(cfg)
+    lat = hr.Lattice(cfg["dims"], B.BC, cfg["N"], cfg["rep"])
+    fund, links = lat.gauge(False, P), lat.gauge(True, P)
+    lat.import_gauge(fund, U)
+    lat.represent_links(links, fund)
+    nset = 4
+    sets = []
+    for k in range(nset):
+        a, b, c = lat.spinor(P), lat.spinor(P), lat.spinor(P)
+        lat.import_spinor(a, P, psi[0], 0)
+        lat.import_spinor(b, P, psi[1], 0)
+        c.zero_()
+        sets.append((a, b, c))
+    ctx, st = lat.ctx, lat.stream()
+    res = torch.zeros(2, dtype=torch.float64, device="cuda")
+    S, L, vh = bm["S"], bm["L"], bm["V"] // 2
+    dphi_c = 8 * L + 2 * S
+
+    def timed(fn, reps):
+        for k in range(5):
+            fn(k)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for k in range(reps):
+            fn(k)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    ops = [
+        ("copy", 2 * S, lambda k: hr.hr_spinor_copy(ctx, P, sets[k % nset][2], sets[k % nset][0], st)),
+        ("g5", 2 * S, lambda k: hr.hr_spinor_g5(ctx, P, sets[k % nset][2], sets[k % nset][0], st)),
+        ("g5_mulc_add_assign", 3 * S, lambda k: hr.hr_spinor_g5_mulc_add_assign(ctx, P, sets[k % nset][2], 0.3 - 0.2j, sets[k % nset][0], st)),
+        ("norm2", S, lambda k: hr.hr_spinor_norm2(ctx, P, sets[k % nset][0], st, result=res)),
+        ("dot", 2 * S, lambda k: hr.hr_spinor_dot(ctx, P, sets[k % nset][0], sets[k % nset][1], st, result=res)),
+        ("dhat", 2 * dphi_c + S, lambda k: hr.hr_dhat(args.m0, 1, sets[k % nset][2], sets[k % nset][0], sets[k % nset][1], links, st)),
+    ]
+    common = {"workload": cfg["name"], "dtype": args.prec, "peak_gbs": peak, "peak_source": peak_src, "sites": vh}
+    for name, bps, fn in ops:
+        ms = timed(fn, args.reps)
+        gbs = bps * vh / (ms * 1e-3) / 1e9
+        print(json.dumps(dict(common, op=name, bytes_per_site=bps, ms=ms, gbs=gbs, frac=gbs / peak)))
+
+    # one CG iteration, measured on a solve that cannot converge (tol = 0): time / iterations
+    maxiter = 40
+    ws = lat.cg_workspace(P, maxiter)
+    x = lat.spinor(P)
+    lat.cg_dhat(args.m0, x, sets[0][0], links, 0.0, 4, ws)
+    torch.cuda.synchronize()
+    n0 = hr.hr_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    it, res2, _ = lat.cg_dhat(args.m0, x, sets[0][0], links, 0.0, maxiter, ws)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / it
+    bps = 4 * dphi_c + 2 * S + 8 * S
+    gbs = bps * vh / (ms * 1e-3) / 1e9
+    print(json.dumps(dict(common, op="cg_iteration", bytes_per_site=bps, ms=ms, gbs=gbs, frac=gbs / peak, iterations=it,
+                          launches_per_iteration=(hr.hr_launch_count() - n0) / it, rel_res2=res2)))
+    lat.close()
+
+
+if __name__ == "__main__":
+    main()
