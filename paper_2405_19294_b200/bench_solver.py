@@ -76,6 +76,15 @@ def main():
         ("dot", 2 * S, lambda k: hr.hr_spinor_dot(ctx, P, sets[k % nset][0], sets[k % nset][1], st, result=res)),
         ("dhat", 2 * dphi_c + S, lambda k: hr.hr_dhat(args.m0, 1, sets[k % nset][2], sets[k % nset][0], sets[k % nset][1], links, st)),
     ]
+    ops.append(("dphi_eo (represented links, compulsory bytes 8L+2S)", dphi_c,
+                lambda k: hr.hr_dphi_eo(sets[k % nset][2], sets[k % nset][0], links, k & 1, st)))
+    if cfg["rep"] in ("sym", "asym"):
+        # NEXT-3: the same operator from the FUNDAMENTAL links (8F+2S bytes per site actually needed)
+        F = bm["F"]
+        ops.append(("dphi_eo on-the-fly (fundamental links, bytes 8F+2S)", 8 * F + 2 * S,
+                    lambda k: hr.hr_dphi_eo(sets[k % nset][2], sets[k % nset][0], fund, k & 1, st)))
+        ops.append(("dhat on-the-fly", 2 * (8 * F + 2 * S) + S,
+                    lambda k: hr.hr_dhat(args.m0, 1, sets[k % nset][2], sets[k % nset][0], sets[k % nset][1], fund, st)))
     common = {"workload": cfg["name"], "dtype": args.prec, "peak_gbs": peak, "peak_source": peak_src, "sites": vh}
     for name, bps, fn in ops:
         ms = timed(fn, args.reps)

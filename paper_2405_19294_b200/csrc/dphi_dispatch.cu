@@ -5,46 +5,62 @@
 
 namespace hr {
 
-template <typename Real, int D, bool RL>
+template <typename Real, int D, int LK>
 hr_status launch_dphi_t(int variant, int block, const DphiArgs &a, cudaStream_t st);
-template <typename Real, int D, bool RL> bool dphi_variant_ok_t(int variant);
+template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant);
 
 static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1" };
 
 // Default variant per (d_R, link type, precision, volume): filled from measurements.
-static int default_variant(const hr_ctx *c, hr_prec prec)
+static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
 {
+    // on-the-fly two-index kernels hold an N x N link, not a d_R x d_R one: a whole site fits one thread
+    if (lk >= 2) return 0;
     // measured on B200 (profiles/r1_variant_sweep.md): at d_R >= 6 fp64 one thread per site spills
     // and the pair kernel wins; in fp32 the whole site still fits one thread.
     if (c->d >= 6) return prec == HR_F64 ? 3 : 1;
     return 0;
 }
 
-static int resolve_variant(const hr_ctx *c, hr_prec prec) { return c->variant >= 0 ? c->variant : default_variant(c, prec); }
+static int resolve_variant(const hr_ctx *c, hr_prec prec, int lk) { return c->variant >= 0 ? c->variant : default_variant(c, prec, lk); }
+
+// link kind (dphi_kernel.cuh): 0 complex d_R x d_R, 1 real d_R x d_R (adjoint), 2 / 3 two-index symmetric /
+// antisymmetric applied on the fly from the fundamental link
+int dphi_link_kind(const hr_ctx *c, bool fundamental_links)
+{
+    if (!fundamental_links || c->rep == HR_REP_FUND) return c->real_links ? 1 : 0; // FUND: both fields are N x N complex
+    if (c->rep == HR_REP_SYM) return 2;
+    if (c->rep == HR_REP_ASYM) return 3;
+    return -1; // adjoint on the fly: not built
+}
 
 #define HR_COMBOS(X)                                                                                      \
-    X(2, false) X(3, false) X(4, false) X(6, false) X(3, true) X(8, true)
+    X(2, 0) X(3, 0) X(4, 0) X(6, 0) X(3, 1) X(8, 1) X(3, 2) X(6, 2) X(3, 3) X(6, 3)
 
-hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st)
+hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st, bool fundamental_links)
 {
-    const int v = resolve_variant(c, prec);
-    const bool rl = c->real_links != 0;
-#define X(D, RL)                                                                                          \
-    if (c->d == D && rl == RL)                                                                            \
-        return prec == HR_F64 ? launch_dphi_t<double, D, RL>(v, c->block, a, st)                         \
-                              : launch_dphi_t<float, D, RL>(v, c->block, a, st);
+    const int lk = dphi_link_kind(c, fundamental_links);
+    if (lk < 0) {
+        set_error("fundamental links given, but this representation has no on-the-fly kernel (use hr_represent_links)");
+        return HR_EUNSUPPORTED;
+    }
+    const int v = resolve_variant(c, prec, lk);
+#define X(D, LK)                                                                                          \
+    if (c->d == D && lk == LK)                                                                            \
+        return prec == HR_F64 ? launch_dphi_t<double, D, LK>(v, c->block, a, st)                         \
+                              : launch_dphi_t<float, D, LK>(v, c->block, a, st);
     HR_COMBOS(X)
 #undef X
-    set_error("no Dphi kernel compiled for d_R=%d (%s links)", c->d, rl ? "real" : "complex");
+    set_error("no Dphi kernel compiled for d_R=%d (link kind %d)", c->d, lk);
     return HR_EUNSUPPORTED;
 }
 
 bool dphi_variant_valid(const hr_ctx *c, int variant)
 {
     if (variant == -1) return true;
-    const bool rl = c->real_links != 0;
-#define X(D, RL)                                                                                          \
-    if (c->d == D && rl == RL) return dphi_variant_ok_t<double, D, RL>(variant) || dphi_variant_ok_t<float, D, RL>(variant);
+    const int lk = c->real_links ? 1 : 0;
+#define X(D, LK)                                                                                          \
+    if (c->d == D && lk == LK) return dphi_variant_ok_t<double, D, LK>(variant) || dphi_variant_ok_t<float, D, LK>(variant);
     HR_COMBOS(X)
 #undef X
     return false;
@@ -52,7 +68,7 @@ bool dphi_variant_valid(const hr_ctx *c, int variant)
 
 const char *dphi_variant_name(const hr_ctx *c, hr_prec prec)
 {
-    const int v = resolve_variant(c, prec);
+    const int v = resolve_variant(c, prec, c->real_links ? 1 : 0);
     return (v >= 0 && v < (int)(sizeof kNames / sizeof kNames[0])) ? kNames[v] : "?";
 }
 

@@ -1,3 +1,3 @@
 // Dphi kernels for d_R = 3, real (adjoint) links, f32.
 #include "dphi_launch.cuh"
-namespace hr { HR_DPHI_INSTANCE(float, 3, true) }
+namespace hr { HR_DPHI_INSTANCE(float, 3, 1) }

@@ -1,3 +1,3 @@
 // Dphi kernels for d_R = 3, complex links, f64.
 #include "dphi_launch.cuh"
-namespace hr { HR_DPHI_INSTANCE(double, 3, false) }
+namespace hr { HR_DPHI_INSTANCE(double, 3, 0) }

@@ -1,3 +1,3 @@
 // Dphi kernels for d_R = 6, complex links, f64.
 #include "dphi_launch.cuh"
-namespace hr { HR_DPHI_INSTANCE(double, 6, false) }
+namespace hr { HR_DPHI_INSTANCE(double, 6, 0) }

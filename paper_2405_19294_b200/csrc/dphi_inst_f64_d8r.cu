@@ -1,3 +1,3 @@
 // Dphi kernels for d_R = 8, real (adjoint) links, f64.
 #include "dphi_launch.cuh"
-namespace hr { HR_DPHI_INSTANCE(double, 8, true) }
+namespace hr { HR_DPHI_INSTANCE(double, 8, 1) }

@@ -91,9 +91,94 @@ __device__ __forceinline__ void colour_mul(Real (&chi)[2 * D], const Real *u, co
     }
 }
 
+// ---- link kinds ------------------------------------------------------------------------------------
+// LK_COMPLEX / LK_REAL: the represented d_R x d_R link is read from memory (hr_represent_links wrote it).
+// LK_SYM_OTF / LK_ASYM_OTF ("on-the-fly representation"): the kernel reads the
+// FUNDAMENTAL N x N link (144 B instead of 576 B for the SU(3) sextet in fp64) and applies the two-index
+// representation without ever forming R(U): with the colour vector written as the (anti)symmetric matrix
+// Psi = sum_a psi_a e_a (basis of reading C8),  R(U) psi <-> U Psi U^T  and  R(U)^dagger psi <-> U^dagger Psi U^*.
+enum : int { LK_COMPLEX = 0, LK_REAL = 1, LK_SYM_OTF = 2, LK_ASYM_OTF = 3 };
+
+template <int LK, int D> struct LinkGeom {
+    // N of the fundamental link for the on-the-fly kinds: D = N(N+1)/2 (sym) or N(N-1)/2 (asym)
+    static constexpr int N = LK == LK_SYM_OTF ? (D == 3 ? 2 : D == 6 ? 3 : D == 10 ? 4 : 0)
+                           : LK == LK_ASYM_OTF ? (D == 3 ? 3 : D == 6 ? 4 : 0) : D;
+    static constexpr int NREAL = LK == LK_REAL ? D * D : LK == LK_COMPLEX ? 2 * D * D : 2 * N * N;
+    static_assert(N > 0, "no such two-index representation");
+};
+
+// chi = R(U) h (DAG = false) or R(U)^dagger h (DAG = true) from the fundamental link u[N][N] (re,im)
+template <int D, int LK, bool DAG, typename Real>
+__device__ __forceinline__ void twoindex_mul(Real (&chi)[2 * D], const Real *u, const Real (&h)[2 * D])
+{
+    constexpr int N = LinkGeom<LK, D>::N;
+    constexpr bool SYM = LK == LK_SYM_OTF;
+    // Psi' = sqrt2 * Psi: off-diagonal entries are the components themselves, diagonal ones (sym only) sqrt2 * h;
+    // then chi_(ij) = M'_ij (i<j), chi_(ii) = M'_ii / sqrt2 with M' = U Psi' U^T.
+    Real pr[N][N], pi[N][N];
+    {
+        int a = 0;
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+#pragma unroll
+            for (int j = i; j < N; ++j) {
+                if (i == j) {
+                    if constexpr (SYM) { pr[i][i] = (Real)1.4142135623730951 * h[2 * a]; pi[i][i] = (Real)1.4142135623730951 * h[2 * a + 1]; ++a; }
+                    else { pr[i][i] = 0; pi[i][i] = 0; }
+                } else {
+                    pr[i][j] = h[2 * a]; pi[i][j] = h[2 * a + 1];
+                    pr[j][i] = SYM ? h[2 * a] : -h[2 * a]; pi[j][i] = SYM ? h[2 * a + 1] : -h[2 * a + 1];
+                    ++a;
+                }
+            }
+    }
+    // W = U (or U^dagger):  wr/wi[i][k], the imaginary part conjugated for the dagger
+    auto wr = [&](int i, int k) -> Real { return DAG ? u[2 * (k * N + i)] : u[2 * (i * N + k)]; };
+    auto wi = [&](int i, int k) -> Real { return DAG ? -u[2 * (k * N + i) + 1] : u[2 * (i * N + k) + 1]; };
+    // A = W Psi'
+    Real ar[N][N], ai[N][N];
+#pragma unroll
+    for (int i = 0; i < N; ++i)
+#pragma unroll
+        for (int l = 0; l < N; ++l) {
+            Real re = 0, im = 0;
+#pragma unroll
+            for (int k = 0; k < N; ++k) {
+                if (!SYM && k == l) continue;
+                re = fma(wr(i, k), pr[k][l], re); re = fma(-wi(i, k), pi[k][l], re);
+                im = fma(wr(i, k), pi[k][l], im); im = fma(wi(i, k), pr[k][l], im);
+            }
+            ar[i][l] = re; ai[i][l] = im;
+        }
+    // M' = A W^T, needed entries only
+    int a = 0;
+#pragma unroll
+    for (int i = 0; i < N; ++i)
+#pragma unroll
+        for (int j = i; j < N; ++j) {
+            if (!SYM && i == j) continue;
+            Real re = 0, im = 0;
+#pragma unroll
+            for (int l = 0; l < N; ++l) {
+                re = fma(ar[i][l], wr(j, l), re); re = fma(-ai[i][l], wi(j, l), re);
+                im = fma(ar[i][l], wi(j, l), im); im = fma(ai[i][l], wr(j, l), im);
+            }
+            if (i == j) { re *= (Real)0.7071067811865476; im *= (Real)0.7071067811865476; }
+            chi[2 * a] = re; chi[2 * a + 1] = im;
+            ++a;
+        }
+}
+
+template <int D, int LK, bool DAG, typename Real>
+__device__ __forceinline__ void link_mul(Real (&chi)[2 * D], const Real *u, const Real (&h)[2 * D])
+{
+    if constexpr (LK == LK_COMPLEX || LK == LK_REAL) colour_mul<D, LK == LK_REAL, DAG>(chi, u, h);
+    else twoindex_mul<D, LK, DAG>(chi, u, h);
+}
+
 // one half-spinor component of one hop:  h = a + sk c0 b ; chi = U(^dag) h ; outK += sgn chi ;
 // outP += sgn sk conj(c0) chi.   c0 = (DIR ? -1 : +1) * (MU in {0,2} ? 1 : i)
-template <int MU, int DIR, int D, bool RL, typename Real>
+template <int MU, int DIR, int D, int LK, typename Real>
 __device__ __forceinline__ void hop_component(const Real *u, const Real *a, const Real *b, Real sk, Real sgn,
                                               Real *outK, Real *outP)
 {
@@ -103,7 +188,7 @@ __device__ __forceinline__ void hop_component(const Real *u, const Real *a, cons
     Real h[2 * D], chi[2 * D];
 #pragma unroll
     for (int c = 0; c < D; ++c) add_c<CRE, CIM>(h[2 * c], h[2 * c + 1], a[2 * c], a[2 * c + 1], b[2 * c], b[2 * c + 1], sk);
-    colour_mul<D, RL, DIR == 1>(chi, u, h);
+    link_mul<D, LK, DIR == 1>(chi, u, h);
     const Real w = sgn * sk;
 #pragma unroll
     for (int c = 0; c < D; ++c) {
@@ -156,12 +241,12 @@ __device__ __forceinline__ void neighbour(const DphiArgs &a, const SiteGeom &g, 
 // MASS: the epilogue reads self = psi(x) on the output parity (alpha term); RED: the epilogue also
 // reduces sum |out|^2 and <self, out> over the launch (needs MASS) -- what a CG on gamma5 Dhat needs
 // from its operator, with no extra pass over the fields.
-template <typename Real, int D, bool RL, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT, int MAXT, int MINB>
+template <typename Real, int D, int LK, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
 {
     static_assert(!RED || MASS, "the fused reduction needs the self field");
     if (a.skip != nullptr && *a.skip != 0) return;
-    constexpr int LNREAL = RL ? D * D : 2 * D * D;        // reals per link
+    constexpr int LNREAL = LinkGeom<LK, D>::NREAL;         // reals per link record read by the kernel
     constexpr int RPV = 16 / (int)sizeof(Real);
     constexpr int SPV = 2 * D / RPV;                       // 16-byte vectors per spin component
     static_assert(KSPLIT == 1 || (2 * D) % RPV == 0, "KSPLIT=2 needs vector-aligned spin components");
@@ -218,8 +303,8 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
             constexpr int P0 = (MU == 0 || MU == 3) ? 2 : 3;
             constexpr int P1 = 5 - P0;
             const Real sg = (Real)sign;
-            hop_component<MU, DIR, D, RL, Real>(u, psi + 0 * 2 * D, psi + P0 * 2 * D, (Real)1, sg, acc[0], acc[P0]);
-            hop_component<MU, DIR, D, RL, Real>(u, psi + 1 * 2 * D, psi + P1 * 2 * D, (Real)(MU >= 2 ? -1 : 1), sg, acc[1], acc[P1]);
+            hop_component<MU, DIR, D, LK, Real>(u, psi + 0 * 2 * D, psi + P0 * 2 * D, (Real)1, sg, acc[0], acc[P0]);
+            hop_component<MU, DIR, D, LK, Real>(u, psi + 1 * 2 * D, psi + P1 * 2 * D, (Real)(MU >= 2 ? -1 : 1), sg, acc[1], acc[P1]);
         };
         using I0 = std::integral_constant<int, 0>; using I1 = std::integral_constant<int, 1>;
         using I2 = std::integral_constant<int, 2>; using I3 = std::integral_constant<int, 3>;
@@ -281,7 +366,7 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
             if constexpr (DIR == 0) load_record<LHINT, LNREAL>(u, lk_own + (size_t)MU * LB * vh, vh, (size_t)s, pol_l);
             else                    load_record<LHINT, LNREAL>(u, lk_nbr + (size_t)MU * LB * vh, vh, (size_t)sn, pol_l);
             const Real sk = (MU >= 2 && k == 1) ? (Real)-1 : (Real)1;
-            hop_component<MU, DIR, D, RL, Real>(u, pa, pbv, sk, (Real)sign, accK, STRAIGHT ? accP : accQ);
+            hop_component<MU, DIR, D, LK, Real>(u, pa, pbv, sk, (Real)sign, accK, STRAIGHT ? accP : accQ);
         };
         using I0 = std::integral_constant<int, 0>; using I1 = std::integral_constant<int, 1>;
         using I2 = std::integral_constant<int, 2>; using I3 = std::integral_constant<int, 3>;

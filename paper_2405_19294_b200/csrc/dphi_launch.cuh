@@ -18,8 +18,8 @@ enum { DPHI_NVARIANTS = 5 };
 static const char *const kDphiVariantNames[DPHI_NVARIANTS] = { "site", "site_ef", "pair", "pair_ef", "site_l1" };
 
 // registers: __launch_bounds__(MAXT, MINB) caps them at 65536 / (MAXT*MINB)
-template <typename Real, int D, bool RL, int KSPLIT> struct Tune {
-    static constexpr int LNREAL = RL ? D * D : 2 * D * D;
+template <typename Real, int D, int LK, int KSPLIT> struct Tune {
+    static constexpr int LNREAL = LinkGeom<LK, D>::NREAL;
     // live values of a thread, in 32-bit registers (accumulators + one spinor/half + one link)
     static constexpr int W = (int)sizeof(Real) / 4;
     static constexpr int LIVE = W * ((KSPLIT == 1 ? 8 * D : 6 * D) + (KSPLIT == 1 ? 8 * D : 4 * D) + LNREAL) + 40;
@@ -27,10 +27,10 @@ template <typename Real, int D, bool RL, int KSPLIT> struct Tune {
     static constexpr int MINB = LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? 4 : LIVE <= 168 ? 3 : LIVE <= 255 ? 2 : 1;
 };
 
-template <typename Real, int D, bool RL, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT>
+template <typename Real, int D, int LK, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT>
 static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
 {
-    using T = Tune<Real, D, RL, KSPLIT>;
+    using T = Tune<Real, D, LK, KSPLIT>;
     if (block <= 0) block = T::MAXT;
     if (block > T::MAXT || (block % 32) != 0) {
         set_error("block=%d not supported by this variant (multiple of 32, <= %d)", block, T::MAXT);
@@ -42,7 +42,7 @@ static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
         set_error("fused Dphi reduction: %ld CTAs exceed the reduction scratch (%u)", grid, kRedMaxBlocks);
         return HR_EUNSUPPORTED;
     }
-    dphi_kernel<Real, D, RL, KSPLIT, MASS, RED, LHINT, SHINT, STHINT, T::MAXT, T::MINB><<<(unsigned)grid, block, 0, st>>>(a);
+    dphi_kernel<Real, D, LK, KSPLIT, MASS, RED, LHINT, SHINT, STHINT, T::MAXT, T::MINB><<<(unsigned)grid, block, 0, st>>>(a);
     count_launch();
     cudaError_t e = cudaPeekAtLastError();
     if (e != cudaSuccess) {
@@ -52,36 +52,36 @@ static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
     return HR_OK;
 }
 
-template <typename Real, int D, bool RL, bool MASS, bool RED>
+template <typename Real, int D, int LK, bool MASS, bool RED>
 static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaStream_t st)
 {
     constexpr int RPV = 16 / (int)sizeof(Real);
     constexpr bool PAIR_OK = (2 * D) % RPV == 0;
     switch (variant) {
-    case 0: return launch_one<Real, D, RL, 1, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
-    case 1: return launch_one<Real, D, RL, 1, MASS, RED, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
+    case 0: return launch_one<Real, D, LK, 1, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+    case 1: return launch_one<Real, D, LK, 1, MASS, RED, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
     case 2:
-        if constexpr (PAIR_OK) return launch_one<Real, D, RL, 2, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+        if constexpr (PAIR_OK) return launch_one<Real, D, LK, 2, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
         break;
     case 3:
-        if constexpr (PAIR_OK) return launch_one<Real, D, RL, 2, MASS, RED, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
+        if constexpr (PAIR_OK) return launch_one<Real, D, LK, 2, MASS, RED, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
         break;
-    case 4: return launch_one<Real, D, RL, 1, MASS, RED, LD_DEFAULT, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+    case 4: return launch_one<Real, D, LK, 1, MASS, RED, LD_DEFAULT, LD_DEFAULT, ST_DEFAULT>(block, a, st);
     default: break;
     }
     set_error("dphi variant %d not available for d_R=%d, %s", variant, D, sizeof(Real) == 8 ? "fp64" : "fp32");
     return HR_EUNSUPPORTED;
 }
 
-template <typename Real, int D, bool RL>
+template <typename Real, int D, int LK>
 hr_status launch_dphi_t(int variant, int block, const DphiArgs &a, cudaStream_t st)
 {
-    if (a.self && a.red_result) return launch_variant<Real, D, RL, true, true>(variant, block, a, st);
-    if (a.self) return launch_variant<Real, D, RL, true, false>(variant, block, a, st);
-    return launch_variant<Real, D, RL, false, false>(variant, block, a, st);
+    if (a.self && a.red_result) return launch_variant<Real, D, LK, true, true>(variant, block, a, st);
+    if (a.self) return launch_variant<Real, D, LK, true, false>(variant, block, a, st);
+    return launch_variant<Real, D, LK, false, false>(variant, block, a, st);
 }
 
-template <typename Real, int D, bool RL> bool dphi_variant_ok_t(int variant)
+template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant)
 {
     constexpr int RPV = 16 / (int)sizeof(Real);
     if (variant < 0 || variant >= DPHI_NVARIANTS) return false;
@@ -89,8 +89,8 @@ template <typename Real, int D, bool RL> bool dphi_variant_ok_t(int variant)
     return true;
 }
 
-#define HR_DPHI_INSTANCE(Real, D, RL)                                                                    \
-    template hr_status launch_dphi_t<Real, D, RL>(int, int, const DphiArgs &, cudaStream_t);             \
-    template bool dphi_variant_ok_t<Real, D, RL>(int);
+#define HR_DPHI_INSTANCE(Real, D, LK)                                                                    \
+    template hr_status launch_dphi_t<Real, D, LK>(int, int, const DphiArgs &, cudaStream_t);             \
+    template bool dphi_variant_ok_t<Real, D, LK>(int);
 
 } // namespace hr

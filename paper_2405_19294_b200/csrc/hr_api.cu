@@ -376,7 +376,11 @@ hr_status hr_dphi_eo(void *out, const void *in, const hr_gauge *links, int parit
 {
     if (!out || !in || !links) { set_error("hr_dphi_eo: NULL argument"); return HR_EINVAL; }
     if (parity != 0 && parity != 1) { set_error("hr_dphi_eo: parity=%d", parity); return HR_EINVAL; }
-    if (!links->represented) { set_error("hr_dphi_eo: `links` must be a represented field (hr_represent_links)"); return HR_EINVAL; }
+    if (!links->represented && dphi_link_kind(links->ctx, true) < 0) {
+        set_error("hr_dphi_eo: `links` must be a represented field (hr_represent_links); fundamental links are accepted "
+                  "only for the fundamental and two-index representations");
+        return HR_EINVAL;
+    }
     if (out == in) { set_error("hr_dphi_eo: out aliases in"); return HR_EINVAL; }
     if (((uintptr_t)out | (uintptr_t)in) & 15) { set_error("hr_dphi_eo: spinor buffers must be 16-byte aligned"); return HR_EINVAL; }
     const hr_ctx *c = links->ctx;
@@ -385,13 +389,13 @@ hr_status hr_dphi_eo(void *out, const void *in, const hr_gauge *links, int parit
     DphiArgs a;
     const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 };
     dphi_args(a, c, out, in, nullptr, links, parity, zero, mhalf);
-    return launch_dphi(c, links->prec, a, (cudaStream_t)stream);
+    return launch_dphi(c, links->prec, a, (cudaStream_t)stream, !links->represented);
 }
 
 hr_status hr_dirac(double m0, void *out_full, const void *in_full, const hr_gauge *links, void *stream)
 {
     if (!out_full || !in_full || !links) { set_error("hr_dirac: NULL argument"); return HR_EINVAL; }
-    if (!links->represented) { set_error("hr_dirac: `links` must be a represented field"); return HR_EINVAL; }
+    if (!links->represented && dphi_link_kind(links->ctx, true) < 0) { set_error("hr_dirac: `links` must be a represented field"); return HR_EINVAL; }
     if (out_full == in_full) { set_error("hr_dirac: out aliases in"); return HR_EINVAL; }
     if (((uintptr_t)out_full | (uintptr_t)in_full) & 15) { set_error("hr_dirac: spinor buffers must be 16-byte aligned"); return HR_EINVAL; }
     const hr_ctx *c = links->ctx;
@@ -405,7 +409,7 @@ hr_status hr_dirac(double m0, void *out_full, const void *in_full, const hr_gaug
         const char *i_self = (const char *)in_full + (size_t)p * half;
         const double mass[2] = { 4.0 + m0, 4.0 + m0 }, mhalf[2] = { -0.5, -0.5 };
         dphi_args(a, c, o, i_other, i_self, links, p, mass, mhalf);
-        rc = launch_dphi(c, links->prec, a, (cudaStream_t)stream);
+        rc = launch_dphi(c, links->prec, a, (cudaStream_t)stream, !links->represented);
         if (rc != HR_OK) return rc;
     }
     return HR_OK;

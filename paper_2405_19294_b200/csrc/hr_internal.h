@@ -115,7 +115,9 @@ struct RedScratch {
 hr_status get_red_scratch(hr_ctx *c, RedScratch *r, cudaStream_t st);
 
 // returns HR_OK / HR_EUNSUPPORTED / HR_ECUDA
-hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st);
+// fundamental_links: a.links is the FUNDAMENTAL field and the representation is applied on the fly (NEXT-3)
+hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st, bool fundamental_links = false);
+int dphi_link_kind(const hr_ctx *c, bool fundamental_links); // -1: no such kernel
 const char *dphi_variant_name(const hr_ctx *c, hr_prec prec);
 bool dphi_variant_valid(const hr_ctx *c, int variant);
 
