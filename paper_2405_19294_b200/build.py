@@ -25,7 +25,7 @@ NVCC_FLAGS = [
     "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC",
     "-I", INCLUDE,
-]
+] + (os.environ.get("HR_EXTRA_NVCC_FLAGS", "").split())
 
 
 def _nvcc() -> str:

@@ -9,7 +9,7 @@ template <typename Real, int D, int LK>
 hr_status launch_dphi_t(int variant, int block, const DphiArgs &a, cudaStream_t st);
 template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant);
 
-static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1" };
+static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf" };
 
 // Default variant per (d_R, link type, precision, volume): filled from measurements.
 static int default_variant(const hr_ctx *c, hr_prec prec, int lk)

@@ -4,7 +4,7 @@
 #pragma once
 #include <type_traits>
 
-#include "dphi_kernel.cuh"
+#include "dphi_pf_kernel.cuh"
 
 namespace hr {
 
@@ -14,8 +14,11 @@ namespace hr {
 //   2 pair      two threads per site (one per half-spinor component)
 //   3 pair_ef   pair + the L2 policies of 1
 //   4 site_l1   one thread per site, links through L1 as well (baseline for the cache-policy evidence)
-enum { DPHI_NVARIANTS = 5 };
-static const char *const kDphiVariantNames[DPHI_NVARIANTS] = { "site", "site_ef", "pair", "pair_ef", "site_l1" };
+//   5 site_pf   one thread per site, the next hop's operands prefetched with cp.async into a private,
+//               double-buffered shared-memory stage (dphi_pf_kernel.cuh)
+enum { DPHI_NVARIANTS = 6 };
+static const char *const kDphiVariantNames[DPHI_NVARIANTS] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf" };
+static const size_t kMaxDynSmem = 227 * 1024;
 
 // registers: __launch_bounds__(MAXT, MINB) caps them at 65536 / (MAXT*MINB)
 template <typename Real, int D, int LK, int KSPLIT> struct Tune {
@@ -24,7 +27,9 @@ template <typename Real, int D, int LK, int KSPLIT> struct Tune {
     static constexpr int W = (int)sizeof(Real) / 4;
     static constexpr int LIVE = W * ((KSPLIT == 1 ? 8 * D : 6 * D) + (KSPLIT == 1 ? 8 * D : 4 * D) + LNREAL) + 40;
     static constexpr int MAXT = 128;
-    static constexpr int MINB = LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? 4 : LIVE <= 168 ? 3 : LIVE <= 255 ? 2 : 1;
+    // measured (profiles/): the fp32 on-the-fly kernels gain 7 % from a 128-register cap (16 warps per SM)
+    static constexpr int MINB = (LK >= 2 && sizeof(Real) == 4 && KSPLIT == 1) ? 4 :
+                                LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? 4 : LIVE <= 168 ? 3 : LIVE <= 255 ? 2 : 1;
 };
 
 template <typename Real, int D, int LK, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT>
@@ -53,6 +58,32 @@ static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
 }
 
 template <typename Real, int D, int LK, bool MASS, bool RED>
+static hr_status launch_pf(int block, const DphiArgs &a, cudaStream_t st)
+{
+    using T = Tune<Real, D, LK, 1>;
+    using G = PfGeom<Real, D, LK>;
+    if (block <= 0) block = G::smem_bytes(T::MAXT) * 2 <= kMaxDynSmem ? T::MAXT : 64; // at least two CTAs per SM
+    if (block > T::MAXT || (block % 32) != 0 || G::smem_bytes(block) > kMaxDynSmem) {
+        set_error("site_pf: block=%d needs %zu bytes of shared memory (max %zu)", block, G::smem_bytes(block), kMaxDynSmem);
+        return HR_EUNSUPPORTED;
+    }
+    auto kern = dphi_pf_kernel<Real, D, LK, MASS, RED, T::MAXT, T::MINB>;
+    static bool attr_set = false; // per instantiation; the attribute is sticky per device context
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
+        if (e != cudaSuccess) { set_error("site_pf: cudaFuncSetAttribute: %s", cudaGetErrorString(e)); cudaGetLastError(); return HR_ECUDA; }
+        attr_set = true;
+    }
+    const long grid = (a.vh + block - 1) / block;
+    if (RED && (unsigned long)grid > kRedMaxBlocks) { set_error("fused Dphi reduction: too many CTAs"); return HR_EUNSUPPORTED; }
+    kern<<<(unsigned)grid, block, G::smem_bytes(block), st>>>(a);
+    count_launch();
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) { set_error("dphi_pf kernel launch failed: %s", cudaGetErrorString(e)); return HR_ECUDA; }
+    return HR_OK;
+}
+
+template <typename Real, int D, int LK, bool MASS, bool RED>
 static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaStream_t st)
 {
     constexpr int RPV = 16 / (int)sizeof(Real);
@@ -67,6 +98,9 @@ static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaS
         if constexpr (PAIR_OK) return launch_one<Real, D, LK, 2, MASS, RED, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
         break;
     case 4: return launch_one<Real, D, LK, 1, MASS, RED, LD_DEFAULT, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+    case 5:
+        if constexpr (PfGeom<Real, D, LK>::smem_bytes(64) <= kMaxDynSmem) return launch_pf<Real, D, LK, MASS, RED>(block, a, st);
+        break;
     default: break;
     }
     set_error("dphi variant %d not available for d_R=%d, %s", variant, D, sizeof(Real) == 8 ? "fp64" : "fp32");
@@ -86,6 +120,7 @@ template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant)
     constexpr int RPV = 16 / (int)sizeof(Real);
     if (variant < 0 || variant >= DPHI_NVARIANTS) return false;
     if ((variant == 2 || variant == 3) && (2 * D) % RPV != 0) return false;
+    if (variant == 5 && PfGeom<Real, D, LK>::smem_bytes(64) > kMaxDynSmem) return false;
     return true;
 }
 

@@ -123,7 +123,7 @@ def test_dphi_eo_boundaries_and_small_extents(hr, dims, bc, parity):
     prob.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("N,rep", [(2, "fund"), (3, "fund"), (2, "adj"), (3, "sym"), (3, "adj")])
 def test_every_kernel_variant_matches_oracle(hr, N, rep, prec, variant):
@@ -239,9 +239,12 @@ def test_argument_errors_on_the_gpu(hr):
     with pytest.raises(hr.HrError) as e:
         hr.hr_dphi_eo(s, t, prob.links, 2, prob.lat.stream())            # parity not in {0,1}
     assert e.value.status == hr.HR_EINVAL
-    with pytest.raises(hr.HrError) as e:
-        hr.hr_dphi_eo(s, t, prob.fund, 0, prob.lat.stream())             # fundamental field is not a represented one
+    U2 = li.haar_links(95, 2, dims)
+    adj = GpuProblem(hr, dims, 2, "adj", "f64", U2)
+    with pytest.raises(hr.HrError) as e:                                 # the adjoint needs its represented field
+        hr.hr_dphi_eo(adj.lat.spinor(hr.HR_F64), adj.lat.spinor(hr.HR_F64), adj.fund, 0, adj.lat.stream())
     assert e.value.status == hr.HR_EINVAL
+    adj.close()
     with pytest.raises(hr.HrError) as e:
         hr.hr_represent_links(prob.fund, prob.links, prob.lat.stream())  # swapped
     assert e.value.status == hr.HR_EINVAL
