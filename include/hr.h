@@ -107,8 +107,14 @@ hr_status hr_represent_links(hr_gauge *repr_out, const hr_gauge *fund_in, void *
  * hr_dphi_eo -- the even-odd hopping term, ONE kernel launch over the V/2 output sites
  * (BASELINE.json:north_star "hr_dphi_eo(out, in, links, parity, stream)").
  * parity = parity of the OUTPUT sites (reading C5).  out: parity-`parity` half field, in:
- * parity-(1-parity) half field, both internal layout, precision = precision of `links`
- * (a represented field).  out must not alias in.
+ * parity-(1-parity) half field, both internal layout, precision = precision of `links`.
+ * out must not alias in.
+ * `links` is a represented field, OR ("on-the-fly representation") the
+ * FUNDAMENTAL field when the representation is two-index symmetric / antisymmetric (or fundamental):
+ * the kernel then reads the N x N link (e.g. 144 instead of 576 bytes for the SU(3) sextet in fp64) and
+ * applies R(U) psi as U Psi U^T, R(U)^dagger psi as U^dagger Psi U^*, Psi = sum_a psi_a e_a in the basis
+ * of reading C8 -- the same operator, never forming R(U).  The adjoint needs its represented (real)
+ * field: a fundamental one -> HR_EINVAL.  The same holds for every call below that takes `links`.
  */
 hr_status hr_dphi_eo(void *out, const void *in, const hr_gauge *links, int parity, void *stream);
 
@@ -198,6 +204,34 @@ hr_status hr_cg_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const h
                      void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
 hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links, double tol,
                          int maxiter, void *workspace, int *iters, double *rel_res2, void *stream);
+
+/* =====================================================================================================
+ * Third part -- SURVEY.md section 8(e)/(f) NEXT-2: the lattice split into slabs along t, one slab per GPU,
+ * with the paper's half-spinor exchange (send buffers, "it is only necessary to send a
+ * half-spinor"; interior sites are computed while the messages travel).
+ * The ctx of a rank describes its LOCAL slab: dims[0] = T_local (even), bc[0] = the sign of the GLOBAL
+ * time seam (applied only by the first / last rank).  Rank r owns global t in [r T_local, (r+1) T_local).
+ * One distributed Dphi_eo(parity p) is, on every rank:
+ *   1. hr_dphi_eo_halo_pack   -> send_up  (for the NEXT rank):     chi = U_0(y)^dagger P+ psi(y), y in my last slice
+ *                                send_dn  (for the PREVIOUS rank): h   = P- psi(y),               y in my first slice
+ *   2. the exchange: my send_up becomes the next rank's recv_prev, my send_dn the previous rank's recv_next
+ *      (NCCL send/recv via torch.distributed -- paper_2405_19294_b200.halo.exchange -- or no copy at all: the
+ *      send pointers may be PEER memory (the neighbour's receive buffers mapped over NVLink), in which case
+ *      the pack kernel's stores ARE the transfer; ordering is then the caller's: an event or barrier
+ *      between pack and apply);
+ *   3. hr_dphi_eo_interior    -> out = Dphi_eo restricted to hops inside the slab (overlaps with 2);
+ *   4. hr_dphi_eo_halo_apply  -> out += the two face contributions, with bc[0] on the global seam.
+ * With one rank (first_rank = last_rank = 1, recv_prev = own send_up, recv_next = own send_dn) steps 1-4
+ * reproduce hr_dphi_eo exactly.  A message holds 2 d_R complex per face site, hr_halo_bytes() in all, in
+ * the plane layout over the X*Y*Z/2 face sites.  `links` as for hr_dphi_eo (represented, or fundamental
+ * for the two-index representations); all buffers device memory, 16-byte aligned; no synchronisation.
+ * ===================================================================================================== */
+size_t hr_halo_bytes(const hr_ctx *ctx, hr_prec prec);
+hr_status hr_dphi_eo_halo_pack(void *send_up, void *send_dn, const void *in, const hr_gauge *links, int parity,
+                               void *stream);
+hr_status hr_dphi_eo_interior(void *out, const void *in, const hr_gauge *links, int parity, void *stream);
+hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *recv_next, const hr_gauge *links,
+                                int parity, int first_rank, int last_rank, void *stream);
 
 /*
  * Kernel tuning (experiments and ncu evidence; defaults are chosen per (d_R, precision) from

@@ -80,6 +80,10 @@ _SIGNATURES = {
     "hr_cg_workspace_bytes": (_sz, [_vp, _ci, _ci]),
     "hr_cg_dhat": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp, _vp]),
     "hr_dirac_solve": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
+    "hr_halo_bytes": (_sz, [_vp, _ci]),
+    "hr_dphi_eo_halo_pack": (_ci, [_vp, _vp, _vp, _vp, _ci, _vp]),
+    "hr_dphi_eo_interior": (_ci, [_vp, _vp, _vp, _ci, _vp]),
+    "hr_dphi_eo_halo_apply": (_ci, [_vp, _vp, _vp, _vp, _ci, _ci, _ci, _vp]),
     "hr_ctx_set_tuning": (_ci, [_vp, ctypes.c_char_p, _ci]),
     "hr_dphi_variant_name": (ctypes.c_char_p, [_vp, _ci]),
     "hr_launch_count": (ctypes.c_ulonglong, []),
@@ -285,6 +289,24 @@ def hr_dirac_solve(ctx: int, m0: float, x_full, b_full, links: int, tol: float, 
     _check(_lib.hr_dirac_solve(ctx, float(m0), _ptr(x_full), _ptr(b_full), links, float(tol), int(maxiter), _ptr(workspace),
                                ctypes.byref(it), ctypes.byref(res), stream))
     return it.value, res.value
+
+
+def hr_halo_bytes(ctx: int, prec: int) -> int:
+    return _lib.hr_halo_bytes(ctx, prec)
+
+
+def hr_dphi_eo_halo_pack(send_up, send_dn, inp, links: int, parity: int, stream: int = 0) -> None:
+    _check(_lib.hr_dphi_eo_halo_pack(_ptr(send_up), _ptr(send_dn), _ptr(inp), links, parity, stream))
+
+
+def hr_dphi_eo_interior(out, inp, links: int, parity: int, stream: int = 0) -> None:
+    _check(_lib.hr_dphi_eo_interior(_ptr(out), _ptr(inp), links, parity, stream))
+
+
+def hr_dphi_eo_halo_apply(out, recv_prev, recv_next, links: int, parity: int, first_rank: bool, last_rank: bool,
+                          stream: int = 0) -> None:
+    _check(_lib.hr_dphi_eo_halo_apply(_ptr(out), _ptr(recv_prev), _ptr(recv_next), links, parity, int(first_rank),
+                                      int(last_rank), stream))
 
 
 def hr_ctx_set_tuning(ctx: int, key: str, value: int) -> None:

@@ -5,6 +5,7 @@
 #include <type_traits>
 
 #include "dphi_pf_kernel.cuh"
+#include "halo_kernel.cuh"
 
 namespace hr {
 
@@ -124,8 +125,23 @@ template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant)
     return true;
 }
 
+template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, const HaloArgs &a, cudaStream_t st)
+{
+    const unsigned grid = (unsigned)((a.nface + 127) / 128);
+    if (pack) halo_pack_kernel<Real, D, LK><<<grid, 128, 0, st>>>(a);
+    else halo_apply_kernel<Real, D, LK><<<grid, 128, 0, st>>>(a);
+    count_launch();
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) {
+        set_error("halo %s kernel launch failed: %s", pack ? "pack" : "apply", cudaGetErrorString(e));
+        return HR_ECUDA;
+    }
+    return HR_OK;
+}
+
 #define HR_DPHI_INSTANCE(Real, D, LK)                                                                    \
     template hr_status launch_dphi_t<Real, D, LK>(int, int, const DphiArgs &, cudaStream_t);             \
-    template bool dphi_variant_ok_t<Real, D, LK>(int);
+    template bool dphi_variant_ok_t<Real, D, LK>(int);                                                    \
+    template hr_status launch_halo_t<Real, D, LK>(bool, const HaloArgs &, cudaStream_t);
 
 } // namespace hr

@@ -1,0 +1,96 @@
+// hr_api_halo.cu -- C-ABI entry points of SURVEY.md section 8(e)/(f) NEXT-2 (include/hr.h, third part):
+// Dphi_eo on a lattice split into slabs along t, one slab per GPU, half-spinor messages.
+// Argument checking and launch sequencing only; the arithmetic is in halo_kernel.cuh and dphi_kernel.cuh.
+#include "hr_internal.h"
+
+using namespace hr;
+
+static bool aligned16(const void *p) { return ((uintptr_t)p & 15) == 0; }
+
+static hr_status check_links(const char *who, const hr_gauge *links, int parity)
+{
+    if (!links) { set_error("%s: NULL links", who); return HR_EINVAL; }
+    if (parity != 0 && parity != 1) { set_error("%s: parity=%d", who, parity); return HR_EINVAL; }
+    if (!links->represented && dphi_link_kind(links->ctx, true) < 0) {
+        set_error("%s: `links` must be a represented field for this representation", who);
+        return HR_EINVAL;
+    }
+    return use_device(links->ctx);
+}
+
+static void halo_common(HaloArgs &a, const hr_ctx *c, const hr_gauge *links, int parity)
+{
+    a.send_up = a.send_dn = nullptr;
+    a.recv_prev = a.recv_next = nullptr;
+    a.in = nullptr;
+    a.out = nullptr;
+    a.links = links->data;
+    a.parity = parity;
+    a.vh = c->Vh;
+    a.nface = (long)c->dims[1] * c->dims[2] * (c->dims[3] / 2);
+    a.Tl = c->dims[0];
+    a.beta[0] = a.beta[1] = -0.5;
+    a.betaf[0] = a.betaf[1] = -0.5f;
+    a.sign_prev = a.sign_next = 1;
+}
+
+extern "C" {
+
+size_t hr_halo_bytes(const hr_ctx *ctx, hr_prec prec)
+{
+    if (!ctx || (prec != HR_F64 && prec != HR_F32)) return 0;
+    return (size_t)ctx->dims[1] * ctx->dims[2] * (ctx->dims[3] / 2) * 4 * ctx->d * prec_bytes(prec);
+}
+
+hr_status hr_dphi_eo_halo_pack(void *send_up, void *send_dn, const void *in, const hr_gauge *links, int parity, void *stream)
+{
+    hr_status rc = check_links("hr_dphi_eo_halo_pack", links, parity);
+    if (rc != HR_OK) return rc;
+    if (!send_up || !send_dn || !in) { set_error("hr_dphi_eo_halo_pack: NULL buffer"); return HR_EINVAL; }
+    if (!aligned16(send_up) || !aligned16(send_dn) || !aligned16(in) || send_up == send_dn) {
+        set_error("hr_dphi_eo_halo_pack: buffers must be distinct and 16-byte aligned");
+        return HR_EINVAL;
+    }
+    HaloArgs a;
+    halo_common(a, links->ctx, links, parity);
+    a.send_up = send_up;
+    a.send_dn = send_dn;
+    a.in = in;
+    return launch_halo(links->ctx, links->prec, true, a, (cudaStream_t)stream, !links->represented);
+}
+
+hr_status hr_dphi_eo_interior(void *out, const void *in, const hr_gauge *links, int parity, void *stream)
+{
+    hr_status rc = check_links("hr_dphi_eo_interior", links, parity);
+    if (rc != HR_OK) return rc;
+    if (!out || !in || out == in || !aligned16(out) || !aligned16(in)) { set_error("hr_dphi_eo_interior: bad buffers"); return HR_EINVAL; }
+    const hr_ctx *c = links->ctx;
+    DphiArgs a;
+    const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 };
+    dphi_args(a, c, out, in, nullptr, links, parity, zero, mhalf);
+    a.bc[0] = 0; // a hop across the slab boundary contributes nothing here: hr_dphi_eo_halo_apply adds it
+    return launch_dphi(c, links->prec, a, (cudaStream_t)stream, !links->represented);
+}
+
+hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *recv_next, const hr_gauge *links, int parity,
+                                int first_rank, int last_rank, void *stream)
+{
+    hr_status rc = check_links("hr_dphi_eo_halo_apply", links, parity);
+    if (rc != HR_OK) return rc;
+    if (!out || !recv_prev || !recv_next) { set_error("hr_dphi_eo_halo_apply: NULL buffer"); return HR_EINVAL; }
+    if (!aligned16(out) || !aligned16(recv_prev) || !aligned16(recv_next)) {
+        set_error("hr_dphi_eo_halo_apply: buffers must be 16-byte aligned");
+        return HR_EINVAL;
+    }
+    const hr_ctx *c = links->ctx;
+    HaloArgs a;
+    halo_common(a, c, links, parity);
+    a.out = out;
+    a.recv_prev = recv_prev;
+    a.recv_next = recv_next;
+    a.sign_prev = first_rank ? c->bc[0] : 1; // the global seam lies below rank 0's first slice ...
+    a.sign_next = last_rank ? c->bc[0] : 1;  // ... and above the last rank's last slice (reading C9)
+    return launch_halo(c, links->prec, false, a, (cudaStream_t)stream, !links->represented);
+}
+
+} // extern "C"

@@ -121,6 +121,24 @@ int dphi_link_kind(const hr_ctx *c, bool fundamental_links); // -1: no such kern
 const char *dphi_variant_name(const hr_ctx *c, hr_prec prec);
 bool dphi_variant_valid(const hr_ctx *c, int variant);
 
+// slab decomposition along t (halo_kernel.cuh)
+struct HaloArgs {
+    void *send_up;         // to the next rank:  chi = U_0^dagger P+ psi of my last slice     (pack)
+    void *send_dn;         // to the previous rank: h = P- psi of my first slice                (pack)
+    const void *recv_prev; // the previous rank's send_up                                       (apply)
+    const void *recv_next; // the next rank's send_dn                                           (apply)
+    const void *in;        // pack: parity-(1-p) half field
+    void *out;             // apply: parity-p half field, already holding the interior result
+    const void *links;
+    int parity;            // p, parity of the OUTPUT sites of the Dphi_eo being assembled
+    long vh, nface;        // V_local/2, X*Y*Zh
+    int Tl;
+    double beta[2];        // coefficient of the hop sum in the interior launch (-1/2 for plain Dphi)
+    float betaf[2];
+    int sign_prev, sign_next; // seam signs of the two faces (+-1)
+};
+hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, const HaloArgs &a, cudaStream_t st, bool fundamental_links);
+
 hr_status launch_represent(const hr_ctx *c, hr_prec in_prec, const void *fund, hr_prec out_prec, void *repr,
                            cudaStream_t st);
 

@@ -228,7 +228,7 @@ def test_cg_edge_cases(hr):
     with pytest.raises(hr.HrError):
         prob.lat.cg_dhat(m0, gb, gb, prob.links, 1e-10, 50, ws)          # x aliases b
     with pytest.raises(hr.HrError):
-        prob.lat.cg_dhat(m0, gx, gb, prob.fund, 1e-10, 50, ws)           # not a represented field
+        prob.lat.cg_dhat(m0, gx, gb, prob.links, 1e-10, -1, ws)          # negative maxiter
     with pytest.raises(hr.HrError):
         prob.lat.cg_dhat(m0, gx, gb, prob.links, -1.0, 50, ws)
     prob.close()

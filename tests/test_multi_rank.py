@@ -71,3 +71,48 @@ def test_reference_arm_only_rank0_prints():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["n_gpus"] == 2
+
+
+# ------------------------------------------------------------------------------------------------------------
+# NEXT-2: routing of the half-spinor messages between t-slabs, world size 2 over gloo.
+def _halo_worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    from paper_2405_19294_b200 import halo
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    plan = halo.slab_plan(rank, world, 8)
+    send_up = torch.full((16,), 10.0 * rank + 1)       # "for the next rank"
+    send_dn = torch.full((16,), 10.0 * rank + 2)       # "for the previous rank"
+    recv_prev, recv_next = torch.zeros(16), torch.zeros(16)
+    halo.exchange(send_up, send_dn, recv_prev, recv_next, plan)
+    q.put((rank, plan, float(recv_prev[0]), float(recv_next[0])))
+    dist.destroy_process_group()
+
+
+def test_halo_exchange_routing_gloo_world2():
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_halo_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted((q.get(timeout=120) for _ in range(world)), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (_, plan0, rp0, rn0), (_, plan1, rp1, rn1) = res
+    assert plan0 == {"T_local": 4, "t0": 0, "prev": 1, "next": 1, "first_rank": True, "last_rank": False}
+    assert plan1 == {"T_local": 4, "t0": 4, "prev": 0, "next": 0, "first_rank": False, "last_rank": True}
+    # recv_prev = the previous rank's send_up, recv_next = the next rank's send_dn
+    assert rp0 == 11.0 and rn0 == 12.0       # rank 0's neighbours are both rank 1
+    assert rp1 == 1.0 and rn1 == 2.0
+
+
+def test_slab_plan_rejects_bad_splits():
+    import pytest
+    sys.path.insert(0, ROOT)
+    from paper_2405_19294_b200 import halo
+    for T, world in ((8, 3), (12, 4), (4, 4)):      # not divisible / odd local extent / local extent 1
+        with pytest.raises(ValueError):
+            halo.slab_plan(0, world, T)
+    assert halo.slab_plan(2, 4, 16) == {"T_local": 4, "t0": 8, "prev": 1, "next": 3, "first_rank": False, "last_rank": False}
