@@ -39,6 +39,8 @@ CONFIGS = {
     3: dict(name="SU(2) adjoint 32^4", dims=(32, 32, 32, 32), N=2, rep="adj", kind="haar", seeds=(1003, 2003)),
     4: dict(name="SU(3) sextet 24^3x48", dims=(48, 24, 24, 24), N=3, rep="sym", kind="haar", seeds=(1004, 2004)),
     5: dict(name="SU(3) fund 64^4", dims=(64, 64, 64, 64), N=3, rep="fund", kind="near", seeds=(1005, 2005)),
+    # not a BASELINE.json config: the local slab of config 5 on 8 GPUs split along t (NEXT-2)
+    6: dict(name="SU(3) fund 64^3x8 slab", dims=(8, 64, 64, 64), N=3, rep="fund", kind="near", seeds=(1006, 2006)),
 }
 REP_DIM = {"fund": lambda N: N, "adj": lambda N: N * N - 1, "sym": lambda N: N * (N + 1) // 2, "asym": lambda N: N * (N - 1) // 2}
 

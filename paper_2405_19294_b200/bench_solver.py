@@ -85,9 +85,24 @@ def main():
                     lambda k: hr.hr_dphi_eo(sets[k % nset][2], sets[k % nset][0], fund, k & 1, st)))
         ops.append(("dhat on-the-fly", 2 * (8 * F + 2 * S) + S,
                     lambda k: hr.hr_dhat(args.m0, 1, sets[k % nset][2], sets[k % nset][0], sets[k % nset][1], fund, st)))
+    # NEXT-2: the slab pipeline of ONE rank (its neighbour is itself): what the decomposition costs on top of
+    # a plain Dphi_eo of the same local volume.  Algorithmic bytes: pack reads 2 slices of spinors and 1 of links
+    # and writes 2 half-spinor faces; apply reads them back, 1 slice of links, and read-modify-writes 2 slices.
+    nface = vh // cfg["dims"][0]
+    nb = hr.hr_halo_bytes(ctx, P)
+    hb = [torch.empty(nb, dtype=torch.uint8, device="cuda") for _ in range(2)]
+    Lk = bm["L"]
+    ops.append(("halo_pack", None, lambda k: hr.hr_dphi_eo_halo_pack(hb[0], hb[1], sets[k % nset][0], links, k & 1, st)))
+    ops.append(("dphi_eo_interior", dphi_c, lambda k: hr.hr_dphi_eo_interior(sets[k % nset][2], sets[k % nset][0], links, k & 1, st)))
+    ops.append(("halo_apply", None, lambda k: hr.hr_dphi_eo_halo_apply(sets[k % nset][2], hb[0], hb[1], links, k & 1, True, True, st)))
+    face_bytes = {"halo_pack": nface * (2 * S + Lk + S), "halo_apply": nface * (S + Lk + 4 * S)}
     common = {"workload": cfg["name"], "dtype": args.prec, "peak_gbs": peak, "peak_source": peak_src, "sites": vh}
     for name, bps, fn in ops:
         ms = timed(fn, args.reps)
+        if bps is None:   # face kernels: bytes are per launch, not per site of the volume
+            gbs = face_bytes[name] / (ms * 1e-3) / 1e9
+            print(json.dumps(dict(common, op=name, bytes_per_launch=face_bytes[name], face_sites=nface, ms=ms, gbs=gbs, frac=gbs / peak)))
+            continue
         gbs = bps * vh / (ms * 1e-3) / 1e9
         print(json.dumps(dict(common, op=name, bytes_per_site=bps, ms=ms, gbs=gbs, frac=gbs / peak)))
 
