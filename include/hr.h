@@ -237,7 +237,9 @@ hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *re
  * Kernel tuning (experiments and ncu evidence; defaults are chosen per (d_R, precision) from
  * measurements).  key: "variant" (kernel variant id, -1 = default table),
  * "block" (threads per CTA, 0 = default), "xblock" (x-extent of the thread order's blocks, a divisor
- * of X; 0 = default from the L2 working-set rule).  Unknown key or value -> HR_EINVAL.
+ * of X; 0 = default from the L2 working-set rule), "cg_graph" (the CG replays one captured iteration as a
+ * CUDA graph: 1 = default, on lattices below 2^19 sites per parity, where launch overhead shows; 2 = always;
+ * 0 = plain kernel launches).  Unknown key or value -> HR_EINVAL.
  */
 hr_status hr_ctx_set_tuning(hr_ctx *ctx, const char *key, int value);
 /* Name of the Dphi kernel variant a call with this precision would launch (for logs/bench). */

@@ -23,7 +23,7 @@ void set_error(const char *fmt, ...)
     vsnprintf(g_err, sizeof g_err, fmt, ap);
     va_end(ap);
 }
-void count_launch(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
+void count_launch(int n) { g_launches.fetch_add((unsigned long long)(long long)n, std::memory_order_relaxed); }
 
 hr_status cuda_fail(const char *what, cudaError_t e)
 {
@@ -176,6 +176,7 @@ hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N,
     c->variant = -1;
     c->block = 0;
     c->xblock = 0;
+    c->cg_graph = 1;
     c->ws_in = c->ws_out = c->ws_stage = nullptr;
     c->ws_spinor_bytes = c->ws_stage_bytes = 0;
     c->ws_prec = -1;
@@ -465,6 +466,11 @@ hr_status hr_ctx_set_tuning(hr_ctx *ctx, const char *key, int value)
     if (!strcmp(key, "xblock")) {
         if (value < 0 || (value > 0 && ctx->dims[1] % value)) { set_error("hr_ctx_set_tuning: xblock=%d must divide X=%d", value, ctx->dims[1]); return HR_EINVAL; }
         ctx->xblock = value;
+        return HR_OK;
+    }
+    if (!strcmp(key, "cg_graph")) {
+        if (value < 0 || value > 2) { set_error("hr_ctx_set_tuning: cg_graph=%d", value); return HR_EINVAL; }
+        ctx->cg_graph = value;
         return HR_OK;
     }
     set_error("hr_ctx_set_tuning: unknown key '%s'", key);

@@ -30,6 +30,7 @@ struct hr_ctx {
     int variant;    // -1 = default table
     int block;      // 0 = default
     int xblock;     // 0 = default (from the L2 working-set rule), else a divisor of X
+    int cg_graph;   // 1 (default): the CG replays one captured iteration as a CUDA graph; 0: plain launches
     // host-path workspace (hr_dphi_eo_host)
     void *ws_in, *ws_out, *ws_stage;
     size_t ws_spinor_bytes, ws_stage_bytes;

@@ -282,3 +282,29 @@ def test_cg_at_config2_volume_converges_and_satisfies_the_equation(hr):
     dhat_x = (4 + m0) ** 2 * x[hidx] - dd
     assert rel_l2(dhat_x, b[hidx]) <= 1e-7
     prob.close()
+
+
+def test_cg_graph_replay_is_bitwise_the_plain_launch_sequence(hr):
+    """tuning key "cg_graph": one CG iteration captured as a CUDA graph and replayed (default) vs the same six kernels
+    launched one by one -- same kernels, same order, same device-resident scalars: identical bits, identical history."""
+    dims, N, m0 = (4, 4, 4, 8), 3, -0.3
+    U = li.haar_links(121, N, dims)
+    b = li.gaussian_spinor(122, li.volume(dims) // 2, 3)
+    prob = GpuProblem(hr, dims, N, "fund", "f64", U)
+    f = Fields(hr, prob)
+    gb = f.put(b)
+    ws = prob.lat.cg_workspace(f.P, 200)
+    res = {}
+    for mode in (2, 1, 0):
+        prob.lat.set_tuning("cg_graph", mode)
+        gx = f.new()
+        n0 = hr.hr_launch_count()
+        it, res2, hist = prob.lat.cg_dhat(m0, gx, gb, prob.links, 1e-10, 200, ws, want_hist=True)
+        res[mode] = (it, res2, hist.copy(), f.get(gx), hr.hr_launch_count() - n0)
+    assert res[0][0] == res[1][0] and res[0][1] == res[1][1]
+    assert np.array_equal(res[0][2], res[1][2]) and np.array_equal(res[0][3], res[1][3])
+    assert res[0][4] == res[1][4]                     # the launch counter counts replayed kernels too
+    assert res[2][0] == res[0][0] and np.array_equal(res[2][3], res[0][3])
+    with pytest.raises(hr.HrError):
+        prob.lat.set_tuning("cg_graph", 3)
+    prob.close()
