@@ -1,0 +1,83 @@
+"""Oracle for SURVEY.md section 8(f) NEXT-4, the clover term -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+PAPER.md:70 lists "clover [17]" improvement of the Wilson-Dirac operator and prints no formula.  Reading C28 of
+DESIGN.md (the Sheikholeslami-Wohlert term in the normalisation of north_star's D = (4+m0) + Dphi):
+
+    D_sw psi(x) = D psi(x) + T(x) psi(x),      T(x) = -(c_sw / 2) sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}(x)
+    sigma_{mu nu} = (i/2) [gamma_mu, gamma_nu]                       (acts on spin)
+    F_{mu nu}(x)  = (Q_{mu nu}(x) - Q_{mu nu}(x)^dagger) / (8 i)     (Hermitian d_R x d_R, acts on colour)
+    Q_{mu nu}(x)  = sum of the four plaquettes ("leaves") of the mu-nu plane that start and end at x, all taken
+                    counter-clockwise (mu -> nu), built from the REPRESENTED links:
+        U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
+      + U_nu(x) U_mu(x-mu+nu)^dag U_nu(x-mu)^dag U_mu(x-mu)
+      + U_mu(x-mu)^dag U_nu(x-mu-nu)^dag U_mu(x-mu-nu) U_nu(x-nu)
+      + U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag
+With U = exp(i A) this gives F_{mu nu} = d_mu A_nu - d_nu A_mu + O(a^2) (pinned by the constant abelian field in
+tests/test_oracle_clover.py).  Links are periodic; the fermionic boundary signs do not enter T (reading C9).
+
+Written with whole-lattice numpy arrays and np.roll, one line per term, nothing blocked or fused; gamma matrices come
+from oracle.gamma (the C tables of reading C1).  Imports nothing from paper_2405_19294_b200.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import dirac, eo_to_lex, gamma, lex_to_eo
+
+
+def _at(field, dims, shifts):
+    """field(x + sum_k shifts[k] e_k) for a lattice-shaped array [T,X,Y,Z,...]; periodic."""
+    out = field
+    for ax, s in enumerate(shifts):
+        if s:
+            out = np.roll(out, -s, axis=ax)
+    return out
+
+
+def _dag(m):
+    return np.conj(np.swapaxes(m, -1, -2))
+
+
+def field_strength(dims, links_R, mu, nu):
+    """F_{mu nu}(x) for all sites, lexicographic [V, d, d] complex (Hermitian)."""
+    dims = tuple(int(v) for v in dims)
+    d = links_R.shape[-1]
+    U = links_R.reshape(dims + (4, d, d))
+    e = lambda k, s=1: tuple(s if a == k else 0 for a in range(4))
+    add = lambda a, b: tuple(x + y for x, y in zip(a, b))
+    Um = lambda sh: _at(U[..., mu, :, :], dims, sh)
+    Un = lambda sh: _at(U[..., nu, :, :], dims, sh)
+    z = (0, 0, 0, 0)
+    q = Um(z) @ Un(e(mu)) @ _dag(Um(e(nu))) @ _dag(Un(z))
+    q = q + Un(z) @ _dag(Um(add(e(mu, -1), e(nu)))) @ _dag(Un(e(mu, -1))) @ Um(e(mu, -1))
+    q = q + _dag(Um(e(mu, -1))) @ _dag(Un(add(e(mu, -1), e(nu, -1)))) @ Um(add(e(mu, -1), e(nu, -1))) @ Un(e(nu, -1))
+    q = q + _dag(Un(e(nu, -1))) @ Um(e(nu, -1)) @ Un(add(e(mu), e(nu, -1))) @ _dag(Um(z))
+    f = (q - _dag(q)) / 8j
+    return f.reshape(-1, d, d)
+
+
+def sigma(mu, nu):
+    g = [gamma(k) for k in range(4)]
+    return 0.5j * (g[mu] @ g[nu] - g[nu] @ g[mu])
+
+
+def clover_term(dims, links_R, csw):
+    """T(x) as [V, 4, d, 4, d] (row spin, row colour, column spin, column colour), lexicographic sites."""
+    d = links_R.shape[-1]
+    V = int(np.prod([int(v) for v in dims]))
+    T = np.zeros((V, 4, d, 4, d), dtype=np.complex128)
+    for mu in range(4):
+        for nu in range(mu + 1, 4):
+            T += -0.5 * csw * np.einsum("st,xab->xsatb", sigma(mu, nu), field_strength(dims, links_R, mu, nu))
+    return T
+
+
+def apply_clover_lex(T, psi_lex):
+    return np.einsum("xsatb,xtb->xsa", T, psi_lex)
+
+
+def dirac_clover(dims, bc, links_R, m0, csw, psi_eo):
+    """D_sw on a full field [even half | odd half]."""
+    T = clover_term(dims, links_R, csw)
+    tpsi = lex_to_eo(dims, apply_clover_lex(T, eo_to_lex(dims, psi_eo)))
+    return dirac(dims, bc, links_R, m0, psi_eo) + tpsi

@@ -1,0 +1,128 @@
+"""Pins of oracle/clover.py (reading C28) against what the physics fixes.  CPU only.
+Closed forms and invariants, none of them the oracle's formula retyped: the constant abelian field (fixes the
+orientation of the leaves, the sign and the 1/8), pure-gauge fields, gauge covariance, antisymmetry in (mu, nu),
+Hermiticity / gamma5-commutation / tracelessness / chiral block structure of T, gamma5-hermiticity of the dense
+D_sw assembled with oracle.dense, and c_sw = 0."""
+import numpy as np
+import pytest
+
+import lattice_inputs as li
+import oracle
+from oracle import clover, dense
+
+BC_T = (-1, 1, 1, 1)
+
+
+def _coords(dims):
+    return np.stack(np.meshgrid(*[np.arange(n) for n in dims], indexing="ij"), axis=-1).reshape(-1, 4)
+
+
+def _gauge_transform(dims, U, g):
+    """U_mu(x) -> g(x) U_mu(x) g(x+mu)^dagger; U [V,4,N,N], g [V,N,N] lexicographic."""
+    dims = tuple(dims)
+    N = U.shape[-1]
+    gl = g.reshape(dims + (N, N))
+    out = np.empty_like(U)
+    for mu in range(4):
+        gs = np.roll(gl, -1, axis=mu).reshape(-1, N, N)
+        out[:, mu] = g @ U[:, mu] @ np.conj(np.swapaxes(gs, -1, -2))
+    return out
+
+
+def test_unit_and_pure_gauge_fields_have_no_field_strength():
+    dims = (4, 2, 4, 6)
+    V = li.volume(dims)
+    one = np.broadcast_to(np.eye(3, dtype=complex), (V, 4, 3, 3)).copy()
+    g = li.haar_links(5, 3, dims)[:, 0]                     # a random SU(3) element per site
+    pure = _gauge_transform(dims, one, g)
+    for U in (one, pure):
+        for mu in range(4):
+            for nu in range(mu + 1, 4):
+                assert np.abs(clover.field_strength(dims, U, mu, nu)).max() < 1e-13
+    assert np.abs(clover.clover_term(dims, pure, 1.7)).max() < 1e-12
+
+
+@pytest.mark.parametrize("mu,nu", [(0, 1), (1, 2), (0, 3), (2, 3)])
+def test_constant_abelian_field_closed_form(mu, nu):
+    """A_nu(x) = B q x_mu, all other A = 0, with B L_mu a multiple of 2 pi: every leaf is exp(i B q), so
+    F_{mu nu} = diag(sin(B q_a)) = d_mu A_nu + O(B^3) exactly at every site, and F_{nu mu} = -F_{mu nu}."""
+    dims = (8, 4, 6, 4)
+    V = li.volume(dims)
+    x = _coords(dims)
+    q = np.array([1.0, -2.0, 3.0])
+    B = 2 * np.pi / dims[mu]
+    U = np.broadcast_to(np.eye(3, dtype=complex), (V, 4, 3, 3)).copy()
+    U[:, nu] = np.exp(1j * B * x[:, mu, None] * q[None, :])[:, :, None] * np.eye(3)
+    F = clover.field_strength(dims, U, mu, nu)
+    want = np.broadcast_to(np.diag(np.sin(B * q)), (V, 3, 3))
+    assert np.abs(F - want).max() < 1e-13
+    assert np.abs(clover.field_strength(dims, U, nu, mu) + want).max() < 1e-13
+    for a in range(4):
+        for b in range(a + 1, 4):
+            if (a, b) != (min(mu, nu), max(mu, nu)):
+                assert np.abs(clover.field_strength(dims, U, a, b)).max() < 1e-13
+    # T = -(c_sw/2) sigma_{mu nu} (x) F_{mu nu} for this field
+    T = clover.clover_term(dims, U, 1.3)
+    s = clover.sigma(mu, nu) if mu < nu else clover.sigma(nu, mu)
+    sign = 1.0 if mu < nu else -1.0
+    wantT = -0.65 * sign * np.einsum("st,ab->satb", s, np.diag(np.sin(B * q)))
+    assert np.abs(T - wantT[None]).max() < 1e-13
+
+
+@pytest.mark.parametrize("N,rep", [(3, "fund"), (2, "adj"), (3, "sym")])
+def test_field_strength_hermitian_antisymmetric_and_gauge_covariant(N, rep):
+    dims = (4, 4, 2, 4)
+    rid = oracle.REP_NAMES[rep]
+    U = li.haar_links(7, N, dims)
+    g = li.haar_links(8, N, dims)[:, 1]
+    R, Rg = oracle.represent(N, rid, U), oracle.represent(N, rid, g)
+    Rt = oracle.represent(N, rid, _gauge_transform(dims, U, g))
+    for mu in range(4):
+        for nu in range(mu + 1, 4):
+            F = clover.field_strength(dims, R, mu, nu)
+            assert np.abs(F - np.conj(np.swapaxes(F, -1, -2))).max() < 1e-13
+            assert np.abs(F + clover.field_strength(dims, R, nu, mu)).max() < 1e-13
+            Ft = clover.field_strength(dims, Rt, mu, nu)
+            assert np.abs(Ft - Rg @ F @ np.conj(np.swapaxes(Rg, -1, -2))).max() < 1e-12
+    assert np.abs(F).max() > 0.1      # a Haar field is far from pure gauge
+
+
+def test_clover_term_structure():
+    dims = (4, 2, 4, 4)
+    U = li.haar_links(9, 3, dims)
+    V, d = li.volume(dims), 3
+    T = clover.clover_term(dims, U, 1.0).reshape(V, 4 * d, 4 * d)
+    assert np.abs(T - np.conj(np.swapaxes(T, -1, -2))).max() < 1e-13                   # Hermitian
+    g5 = np.kron(np.diag([1, 1, -1, -1]), np.eye(d))
+    assert np.abs(T @ g5 - g5 @ T).max() < 1e-13                                       # commutes with gamma5
+    assert np.abs(T[:, :2 * d, 2 * d:]).max() == 0 and np.abs(T[:, 2 * d:, :2 * d]).max() == 0   # chiral blocks
+    Tsc = T.reshape(V, 4, d, 4, d)
+    assert np.abs(np.einsum("xsasb->xab", Tsc)).max() < 1e-13                          # tr_spin sigma = 0
+    assert np.abs(clover.clover_term(dims, U, 0.0)).max() == 0
+    assert np.allclose(clover.clover_term(dims, U, 2.0), 2 * clover.clover_term(dims, U, 1.0))
+    for mu in range(4):                                                                # sigma: Hermitian, (i/2)[g,g]
+        for nu in range(mu + 1, 4):
+            s = clover.sigma(mu, nu)
+            assert np.allclose(s, s.conj().T) and np.allclose(s @ s, np.eye(4))
+            assert np.allclose(s, 1j * oracle.gamma(mu) @ oracle.gamma(nu))
+
+
+def test_dirac_clover_is_gamma5_hermitian_and_reduces_to_dirac():
+    dims = (2, 2, 4, 2)
+    U = li.haar_links(10, 2, dims)
+    R = oracle.represent(2, oracle.REP_ADJ, U)
+    V, d = li.volume(dims), 3
+    m0, csw = -0.4, 1.2
+    g = [oracle.gamma(mu) for mu in range(4)]
+    D = dense.dirac_matrix(dims, BC_T, R, m0, g)                                        # lexicographic (site, spin, colour)
+    T = clover.clover_term(dims, R, csw).reshape(V, 4 * d, 4 * d)
+    Dsw = D.copy()
+    for x in range(V):
+        Dsw[x * 4 * d:(x + 1) * 4 * d, x * 4 * d:(x + 1) * 4 * d] += T[x]
+    G5 = np.kron(np.eye(V), np.kron(np.diag([1, 1, -1, -1]), np.eye(d)))
+    assert np.abs(G5 @ Dsw @ G5 - Dsw.conj().T).max() < 1e-12
+    psi = li.gaussian_spinor(11, V, d)
+    want = oracle.lex_to_eo(dims, (Dsw @ oracle.eo_to_lex(dims, psi).reshape(-1)).reshape(V, 4, d))
+    got = clover.dirac_clover(dims, BC_T, R, m0, csw, psi)
+    assert np.linalg.norm(got - want) <= 1e-13 * np.linalg.norm(want)
+    assert np.array_equal(clover.dirac_clover(dims, BC_T, R, m0, 0.0, psi), oracle.dirac(dims, BC_T, R, m0, psi))
