@@ -233,6 +233,23 @@ hr_status hr_dphi_eo_interior(void *out, const void *in, const hr_gauge *links, 
 hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *recv_next, const hr_gauge *links,
                                 int parity, int first_rank, int last_rank, void *stream);
 
+/* =====================================================================================================
+ * Fourth part -- SURVEY.md section 8(f) NEXT-4: the clover term ("clover [17]").  The paper prints
+ * no formula; reading C28 of DESIGN.md:
+ *     D_sw = D + T,   T(x) = -(c_sw/2) sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}(x),  sigma = (i/2)[gamma_mu, gamma_nu],
+ *     F_{mu nu} = (Q_{mu nu} - Q_{mu nu}^dagger)/(8 i),  Q = the four counter-clockwise plaquettes ("leaves") of the
+ *     mu-nu plane that start and end at x, built from the REPRESENTED links (U = exp(iA) gives F = dA).
+ * hr_clover_build: one launch over all V sites; `clover` is caller-owned device memory of hr_clover_bytes(),
+ *     precision of `links` (a represented field); T is stored as two packed Hermitian 2 d_R x 2 d_R blocks per site
+ *     (the chiral basis makes sigma block diagonal), [even sites | odd sites].
+ * hr_dirac_clover: out = (4+m0) in + Dphi in + T in on full fields [even half | odd half]; the two hr_dirac launches
+ *     followed by one site-local launch per parity.  out != in.
+ * ===================================================================================================== */
+size_t hr_clover_bytes(const hr_ctx *ctx, hr_prec prec);
+hr_status hr_clover_build(void *clover, const hr_gauge *links, double csw, void *stream);
+hr_status hr_dirac_clover(double m0, void *out_full, const void *in_full, const hr_gauge *links, const void *clover,
+                          void *stream);
+
 /*
  * Kernel tuning (experiments and ncu evidence; defaults are chosen per (d_R, precision) from
  * measurements).  key: "variant" (kernel variant id, -1 = default table),

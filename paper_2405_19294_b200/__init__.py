@@ -84,6 +84,9 @@ _SIGNATURES = {
     "hr_dphi_eo_halo_pack": (_ci, [_vp, _vp, _vp, _vp, _ci, _vp]),
     "hr_dphi_eo_interior": (_ci, [_vp, _vp, _vp, _ci, _vp]),
     "hr_dphi_eo_halo_apply": (_ci, [_vp, _vp, _vp, _vp, _ci, _ci, _ci, _vp]),
+    "hr_clover_bytes": (_sz, [_vp, _ci]),
+    "hr_clover_build": (_ci, [_vp, _vp, _cd, _vp]),
+    "hr_dirac_clover": (_ci, [_cd, _vp, _vp, _vp, _vp, _vp]),
     "hr_ctx_set_tuning": (_ci, [_vp, ctypes.c_char_p, _ci]),
     "hr_dphi_variant_name": (ctypes.c_char_p, [_vp, _ci]),
     "hr_launch_count": (ctypes.c_ulonglong, []),
@@ -307,6 +310,18 @@ def hr_dphi_eo_halo_apply(out, recv_prev, recv_next, links: int, parity: int, fi
                           stream: int = 0) -> None:
     _check(_lib.hr_dphi_eo_halo_apply(_ptr(out), _ptr(recv_prev), _ptr(recv_next), links, parity, int(first_rank),
                                       int(last_rank), stream))
+
+
+def hr_clover_bytes(ctx: int, prec: int) -> int:
+    return _lib.hr_clover_bytes(ctx, prec)
+
+
+def hr_clover_build(clover, links: int, csw: float, stream: int = 0) -> None:
+    _check(_lib.hr_clover_build(_ptr(clover), links, float(csw), stream))
+
+
+def hr_dirac_clover(m0: float, out_full, in_full, links: int, clover, stream: int = 0) -> None:
+    _check(_lib.hr_dirac_clover(float(m0), _ptr(out_full), _ptr(in_full), links, _ptr(clover), stream))
 
 
 def hr_ctx_set_tuning(ctx: int, key: str, value: int) -> None:

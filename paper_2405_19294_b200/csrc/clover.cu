@@ -1,0 +1,263 @@
+// clover.cu -- SURVEY.md section 8(f) NEXT-4: the clover (Sheikholeslami-Wohlert) term ("clover [17]").
+// Reading C28:
+//     D_sw = D + T,   T(x) = -(c_sw/2) sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}(x),
+//     F = (Q - Q^dagger)/(8i),  Q = the four counter-clockwise leaves at x from the REPRESENTED links.
+// In the chiral basis of reading C1 sigma_{mu nu} is block diagonal with Pauli-matrix blocks
+//     upper (spin 0,1):  s01 = sx, s02 = sy, s03 = sz, s12 = -sz, s13 = sy, s23 = -sx
+//     lower (spin 2,3):  s01 = -sx, s02 = -sy, s03 = -sz, s12 = -sz, s13 = sy, s23 = -sx
+// so T(x) = diag(T_up, T_dn) with  T_b = -(c_sw/2) [[C, A - iB], [A + iB, -C]]  (d_R x d_R blocks),
+//     up: A = F01 - F23, B = F02 + F13, C = F03 - F12;   dn: A = -F01 - F23, B = -F02 + F13, C = -F03 - F12.
+// CLOVER FIELD LAYOUT: per parity, per site one record of 2 (2 d_R)^2 reals in the plane layout of hr_internal.h:
+// for each block the 2 d_R real diagonal entries, then the strict upper triangle row by row as (re, im).
+//
+// clover_build_kernel: one thread per site, set-up cost (once per gauge field; the Dirac operator is applied
+// hundreds of times per field in a solve), written with runtime loops over d_R.
+// clover_apply_kernel: out += T in, one thread per site, Hermitian block mat-vec unrolled on d_R;
+// algorithmic bytes per site: C + 3S (clover record, in, out read, out written).
+#include "hr_internal.h"
+
+namespace hr {
+
+template <typename Real, int D, bool RL> struct CloverGeom {
+    static constexpr int LNREAL = RL ? D * D : 2 * D * D;
+    static constexpr int BLK = 4 * D * D;   // reals per packed Hermitian 2D x 2D block
+    static constexpr int NREAL = 2 * BLK;
+};
+
+// complex D x D matrices as Real[2*D*D], row-major (re, im)
+template <typename Real, int D, bool DA, bool DB>
+__device__ void cmm(Real *o, const Real *a, const Real *b) // o = op(a) op(b), op = dagger if flagged
+{
+    for (int i = 0; i < D; ++i)
+        for (int j = 0; j < D; ++j) {
+            Real re = 0, im = 0;
+            for (int k = 0; k < D; ++k) {
+                const int ia = DA ? 2 * (k * D + i) : 2 * (i * D + k);
+                const int ib = DB ? 2 * (j * D + k) : 2 * (k * D + j);
+                const Real ar = a[ia], ai = DA ? -a[ia + 1] : a[ia + 1];
+                const Real br = b[ib], bi = DB ? -b[ib + 1] : b[ib + 1];
+                re += ar * br - ai * bi;
+                im += ar * bi + ai * br;
+            }
+            o[2 * (i * D + j)] = re;
+            o[2 * (i * D + j) + 1] = im;
+        }
+}
+
+struct CloverArgs {
+    void *clover;
+    const void *links;
+    const void *in;
+    void *out;
+    int T, X, Y, Z;
+    long vh;
+    double csw;
+};
+
+template <typename Real, int D, bool RL>
+__device__ void load_link(Real *m, const CloverArgs &a, int t, int x, int y, int z, int mu)
+{
+    constexpr int LNREAL = CloverGeom<Real, D, RL>::LNREAL;
+    t = (t + a.T) % a.T; x = (x + a.X) % a.X; y = (y + a.Y) % a.Y; z = (z + a.Z) % a.Z;
+    const int q = (t + x + y + z) & 1;
+    const size_t s = (((size_t)t * a.X + x) * a.Y + y) * (a.Z / 2) + z / 2;
+    const size_t LB = (size_t)LNREAL * sizeof(Real);
+    const char *base = (const char *)a.links + (size_t)(q * 4 + mu) * LB * (size_t)a.vh;
+    Real r[LNREAL];
+    load_record<LD_DEFAULT, LNREAL>(r, base, (size_t)a.vh, s, 0);
+    if constexpr (RL) {
+        for (int e = 0; e < D * D; ++e) { m[2 * e] = r[e]; m[2 * e + 1] = 0; }
+    } else {
+        for (int e = 0; e < 2 * D * D; ++e) m[e] = r[e];
+    }
+}
+
+// q += op(m1) op(m2) op(m3) op(m4)
+template <typename Real, int D, bool D1, bool D2, bool D3, bool D4>
+__device__ void add_leaf(Real *q, const Real *m1, const Real *m2, const Real *m3, const Real *m4)
+{
+    Real p[2 * D * D], r[2 * D * D];
+    cmm<Real, D, D1, D2>(p, m1, m2);
+    cmm<Real, D, false, D3>(r, p, m3);
+    cmm<Real, D, false, D4>(p, r, m4);
+    for (int e = 0; e < 2 * D * D; ++e) q[e] += p[e];
+}
+
+template <typename Real, int D, bool RL>
+__global__ void __launch_bounds__(64) clover_build_kernel(const CloverArgs a)
+{
+    using G = CloverGeom<Real, D, RL>;
+    constexpr int M = 2 * D * D;
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x; // full-lattice lexicographic index
+    if (i >= 2 * a.vh) return;
+    int c[4];
+    {
+        long r = i;
+        c[3] = (int)(r % a.Z); r /= a.Z;
+        c[2] = (int)(r % a.Y); r /= a.Y;
+        c[1] = (int)(r % a.X);
+        c[0] = (int)(r / a.X);
+    }
+    // coefficient matrices of sx, sy, sz in the two chirality blocks
+    Real cf[2][3][M];
+    for (int b = 0; b < 2; ++b)
+        for (int k = 0; k < 3; ++k)
+            for (int e = 0; e < M; ++e) cf[b][k][e] = 0;
+    // plane (mu,nu) -> (Pauli index, sign in the upper block, sign in the lower block)
+    const int pk[6] = { 0, 1, 2, 2, 1, 0 };
+    const int su[6] = { 1, 1, 1, -1, 1, -1 };
+    const int sd[6] = { -1, -1, -1, -1, 1, -1 };
+    int plane = 0;
+    for (int mu = 0; mu < 4; ++mu)
+        for (int nu = mu + 1; nu < 4; ++nu, ++plane) {
+            auto at = [&](int dm, int dn, int dir, Real *m) {
+                int y[4] = { c[0], c[1], c[2], c[3] };
+                y[mu] += dm;
+                y[nu] += dn;
+                load_link<Real, D, RL>(m, a, y[0], y[1], y[2], y[3], dir);
+            };
+            Real q[M], m1[M], m2[M], m3[M], m4[M];
+            for (int e = 0; e < M; ++e) q[e] = 0;
+            // U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
+            at(0, 0, mu, m1); at(1, 0, nu, m2); at(0, 1, mu, m3); at(0, 0, nu, m4);
+            add_leaf<Real, D, false, false, true, true>(q, m1, m2, m3, m4);
+            // U_nu(x) U_mu(x-mu+nu)^dag U_nu(x-mu)^dag U_mu(x-mu)
+            at(0, 0, nu, m1); at(-1, 1, mu, m2); at(-1, 0, nu, m3); at(-1, 0, mu, m4);
+            add_leaf<Real, D, false, true, true, false>(q, m1, m2, m3, m4);
+            // U_mu(x-mu)^dag U_nu(x-mu-nu)^dag U_mu(x-mu-nu) U_nu(x-nu)
+            at(-1, 0, mu, m1); at(-1, -1, nu, m2); at(-1, -1, mu, m3); at(0, -1, nu, m4);
+            add_leaf<Real, D, true, true, false, false>(q, m1, m2, m3, m4);
+            // U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag
+            at(0, -1, nu, m1); at(0, -1, mu, m2); at(1, -1, nu, m3); at(0, 0, mu, m4);
+            add_leaf<Real, D, true, false, false, true>(q, m1, m2, m3, m4);
+            // F = (Q - Q^dag)/(8i):  F_re = Im(Q - Q^dag)/8, F_im = -Re(Q - Q^dag)/8
+            for (int r = 0; r < D; ++r)
+                for (int s = 0; s < D; ++s) {
+                    const Real gre = q[2 * (r * D + s)] - q[2 * (s * D + r)];
+                    const Real gim = q[2 * (r * D + s) + 1] + q[2 * (s * D + r) + 1];
+                    const Real fre = gim * (Real)0.125, fim = -gre * (Real)0.125;
+                    cf[0][pk[plane]][2 * (r * D + s)] += su[plane] * fre;
+                    cf[0][pk[plane]][2 * (r * D + s) + 1] += su[plane] * fim;
+                    cf[1][pk[plane]][2 * (r * D + s)] += sd[plane] * fre;
+                    cf[1][pk[plane]][2 * (r * D + s) + 1] += sd[plane] * fim;
+                }
+        }
+    // T_b = -(c_sw/2) [[C, A - iB], [A + iB, -C]], packed: diagonal, then strict upper triangle (re, im)
+    const Real k = (Real)(-0.5 * a.csw);
+    Real rec[G::NREAL];
+    for (int b = 0; b < 2; ++b) {
+        const Real *A = cf[b][0], *B = cf[b][1], *C = cf[b][2];
+        auto elem = [&](int row, int col, Real &re, Real &im) {
+            const int sr = row / D, ar = row % D, sc = col / D, ac = col % D;
+            const int e = 2 * (ar * D + ac);
+            if (sr == 0 && sc == 0) { re = C[e]; im = C[e + 1]; }
+            else if (sr == 1 && sc == 1) { re = -C[e]; im = -C[e + 1]; }
+            else if (sr == 0 && sc == 1) { re = A[e] + B[e + 1]; im = A[e + 1] - B[e]; }   // A - iB
+            else { re = A[e] - B[e + 1]; im = A[e + 1] + B[e]; }                           // A + iB
+            re *= k; im *= k;
+        };
+        Real *o = rec + b * G::BLK;
+        int w = 0;
+        for (int d = 0; d < 2 * D; ++d) { Real re, im; elem(d, d, re, im); o[w++] = re; }
+        for (int r = 0; r < 2 * D; ++r)
+            for (int s = r + 1; s < 2 * D; ++s) { Real re, im; elem(r, s, re, im); o[w++] = re; o[w++] = im; }
+    }
+    const int qpar = (c[0] + c[1] + c[2] + c[3]) & 1;
+    const size_t hs = (size_t)(i >> 1);
+    char *base = (char *)a.clover + (size_t)qpar * G::NREAL * sizeof(Real) * (size_t)a.vh;
+    store_record<G::NREAL>(base, (size_t)a.vh, hs, rec);
+}
+
+// out += T in on one parity (clover/in/out point at that parity's half fields)
+template <typename Real, int D>
+__global__ void __launch_bounds__(128) clover_apply_kernel(const CloverArgs a)
+{
+    constexpr int BLK = 4 * D * D, NREAL = 2 * BLK, N2 = 2 * D;
+    const long s = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= a.vh) return;
+    const size_t vh = (size_t)a.vh;
+    Real t[NREAL], psi[8 * D], o[8 * D];
+    load_record<LD_STREAM, NREAL>(t, (const char *)a.clover, vh, (size_t)s, 0);
+    load_record<LD_STREAM, 8 * D>(psi, (const char *)a.in, vh, (size_t)s, 0);
+    load_record<LD_STREAM, 8 * D>(o, (const char *)a.out, vh, (size_t)s, 0);
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+        const Real *tb = t + b * BLK;
+        const Real *v = psi + b * 2 * N2; // spin components 2b, 2b+1: N2 complex numbers
+        Real *w = o + b * 2 * N2;
+#pragma unroll
+        for (int r = 0; r < N2; ++r) {
+            w[2 * r] = fma(tb[r], v[2 * r], w[2 * r]);
+            w[2 * r + 1] = fma(tb[r], v[2 * r + 1], w[2 * r + 1]);
+        }
+        int e = N2;
+#pragma unroll
+        for (int r = 0; r < N2; ++r)
+#pragma unroll
+            for (int c = r + 1; c < N2; ++c) {
+                const Real re = tb[e], im = tb[e + 1];
+                e += 2;
+                // row r gets T_rc v_c ; row c gets conj(T_rc) v_r
+                w[2 * r] = fma(re, v[2 * c], fma(-im, v[2 * c + 1], w[2 * r]));
+                w[2 * r + 1] = fma(re, v[2 * c + 1], fma(im, v[2 * c], w[2 * r + 1]));
+                w[2 * c] = fma(re, v[2 * r], fma(im, v[2 * r + 1], w[2 * c]));
+                w[2 * c + 1] = fma(re, v[2 * r + 1], fma(-im, v[2 * r], w[2 * c + 1]));
+            }
+    }
+    constexpr int RPV = 16 / (int)sizeof(Real);
+    store_planes<ST_DEFAULT, 8 * D / RPV>((char *)a.out + (size_t)s * 16, vh * 16, o);
+}
+
+static hr_status launched(const char *what)
+{
+    count_launch();
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) {
+        set_error("%s launch failed: %s", what, cudaGetErrorString(e));
+        return HR_ECUDA;
+    }
+    return HR_OK;
+}
+
+size_t clover_nreal(const hr_ctx *c) { return (size_t)8 * c->d * c->d; }
+
+hr_status launch_clover_build(const hr_ctx *c, hr_prec prec, void *clover, const void *links, double csw, cudaStream_t st)
+{
+    CloverArgs a;
+    a.clover = clover; a.links = links; a.in = nullptr; a.out = nullptr;
+    a.T = c->dims[0]; a.X = c->dims[1]; a.Y = c->dims[2]; a.Z = c->dims[3];
+    a.vh = c->Vh; a.csw = csw;
+    const unsigned grid = (unsigned)((c->V + 63) / 64);
+    const bool rl = c->real_links != 0;
+#define X(D, RL)                                                                                                      \
+    if (c->d == D && rl == RL) {                                                                                      \
+        if (prec == HR_F64) clover_build_kernel<double, D, RL><<<grid, 64, 0, st>>>(a);                              \
+        else clover_build_kernel<float, D, RL><<<grid, 64, 0, st>>>(a);                                              \
+        return launched("clover_build_kernel");                                                                       \
+    }
+    X(2, false) X(3, false) X(4, false) X(6, false) X(3, true) X(8, true)
+#undef X
+    set_error("no clover kernel compiled for d_R=%d", c->d);
+    return HR_EUNSUPPORTED;
+}
+
+hr_status launch_clover_apply(const hr_ctx *c, hr_prec prec, void *out, const void *in, const void *clover_parity, cudaStream_t st)
+{
+    CloverArgs a;
+    a.clover = const_cast<void *>(clover_parity); a.links = nullptr; a.in = in; a.out = out;
+    a.T = c->dims[0]; a.X = c->dims[1]; a.Y = c->dims[2]; a.Z = c->dims[3];
+    a.vh = c->Vh; a.csw = 0;
+    const unsigned grid = (unsigned)((c->Vh + 127) / 128);
+#define X(D)                                                                                                          \
+    if (c->d == D) {                                                                                                  \
+        if (prec == HR_F64) clover_apply_kernel<double, D><<<grid, 128, 0, st>>>(a);                                 \
+        else clover_apply_kernel<float, D><<<grid, 128, 0, st>>>(a);                                                 \
+        return launched("clover_apply_kernel");                                                                       \
+    }
+    X(2) X(3) X(4) X(6) X(8)
+#undef X
+    set_error("no clover kernel compiled for d_R=%d", c->d);
+    return HR_EUNSUPPORTED;
+}
+
+} // namespace hr

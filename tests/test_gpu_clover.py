@@ -1,0 +1,140 @@
+"""GPU parity of SURVEY.md section 8(f) NEXT-4, the clover term (include/hr.h fourth part; reading C28),
+through the C ABI against oracle/clover.py on the same seeded inputs.  The clover field itself is private (packed
+Hermitian blocks), so what is compared is what is unique: T psi, obtained as hr_dirac_clover - hr_dirac, and the full
+D_sw psi.  Tolerances: BASELINE.json:north_star (1e-13 fp64 / 2e-6 fp32, relative L2 vs the fp64 oracle); T alone is a
+sum of 24 products of four links, checked to 20x those."""
+import numpy as np
+import pytest
+
+import lattice_inputs as li
+import oracle
+from oracle import clover
+from gpu_common import BC_T, TOL, GpuProblem, oracle_rep_id, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def hr():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2405_19294_b200 import build
+    build.build()
+    import paper_2405_19294_b200 as hr
+    return hr
+
+
+def _full(prob, psi_eo):
+    lat, P = prob.lat, prob.prec
+    vh = lat.vh
+    half = prob.hr.hr_spinor_bytes(lat.ctx, P)
+    t = lat.spinor(P, full=True)
+    for p in (0, 1):
+        lat.import_spinor(t[p * half:(p + 1) * half], P, psi_eo[p * vh:(p + 1) * vh], p)
+    return t
+
+
+def _get_full(prob, t):
+    lat, P = prob.lat, prob.prec
+    half = prob.hr.hr_spinor_bytes(lat.ctx, P)
+    return np.concatenate([lat.export_spinor(t[p * half:(p + 1) * half], P, p) for p in (0, 1)])
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("N,rep", [(2, "fund"), (3, "fund"), (2, "adj"), (3, "sym"), (3, "adj"), (4, "fund")])
+@pytest.mark.parametrize("dims", [(4, 4, 6, 8), (2, 2, 2, 2), (6, 2, 4, 2)])
+def test_dirac_clover_matches_oracle(hr, dims, N, rep, prec):
+    import torch
+    if rep in ("sym", "adj") and N == 3 and dims != (4, 4, 6, 8) and prec == "f32":
+        pytest.skip("covered by the other sizes")
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(401, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    V = li.volume(dims)
+    psi = li.gaussian_spinor(402, V, d)
+    m0, csw = -0.3, 1.4
+    prob = GpuProblem(hr, dims, N, rep, prec, U)
+    lat, P = prob.lat, prob.prec
+    cl = torch.empty(hr.hr_clover_bytes(lat.ctx, P), dtype=torch.uint8, device="cuda")
+    cl.fill_(0xFF)
+    n0 = hr.hr_launch_count()
+    hr.hr_clover_build(cl, prob.links, csw, lat.stream())
+    assert hr.hr_launch_count() == n0 + 1
+    gin = _full(prob, psi)
+    gout, gref = lat.spinor(P, full=True), lat.spinor(P, full=True)
+    gout.fill_(0xFF)
+    n0 = hr.hr_launch_count()
+    hr.hr_dirac_clover(m0, gout, gin, prob.links, cl, lat.stream())
+    assert hr.hr_launch_count() == n0 + 4                               # 2 Dphi launches + 2 site-local launches
+    got = _get_full(prob, gout)
+    want = clover.dirac_clover(dims, BC_T, R, m0, csw, psi)
+    assert rel_l2(got, want) <= TOL[prec]
+    # the clover part alone: (D_sw - D) psi = T psi
+    lat.dirac(m0, gref, gin, prob.links)
+    tpsi = got - _get_full(prob, gref)
+    T = clover.clover_term(dims, R, csw)
+    want_t = oracle.lex_to_eo(dims, clover.apply_clover_lex(T, oracle.eo_to_lex(dims, psi)))
+    assert np.linalg.norm(tpsi - want_t) <= 20 * TOL[prec] * np.linalg.norm(want)
+    prob.close()
+
+
+def test_clover_vanishes_on_pure_gauge_and_scales_with_csw(hr):
+    import torch
+    dims, N = (4, 4, 4, 4), 3
+    V = li.volume(dims)
+    g = li.haar_links(403, N, dims)[:, 0].reshape(dims + (N, N))
+    pure = np.empty((V, 4, N, N), dtype=complex)
+    for mu in range(4):                                                 # U_mu(x) = g(x) g(x+mu)^dagger
+        gs = np.roll(g, -1, axis=mu)
+        pure[:, mu] = (g @ np.conj(np.swapaxes(gs, -1, -2))).reshape(V, N, N)
+    psi = li.gaussian_spinor(404, V, 3)
+    prob = GpuProblem(hr, dims, N, "fund", "f64", pure)
+    lat, P = prob.lat, prob.prec
+    cl = torch.empty(hr.hr_clover_bytes(lat.ctx, P), dtype=torch.uint8, device="cuda")
+    hr.hr_clover_build(cl, prob.links, 1.9, lat.stream())
+    gin = _full(prob, psi)
+    a, b = lat.spinor(P, full=True), lat.spinor(P, full=True)
+    hr.hr_dirac_clover(0.1, a, gin, prob.links, cl, lat.stream())
+    lat.dirac(0.1, b, gin, prob.links)
+    assert rel_l2(_get_full(prob, a), _get_full(prob, b)) <= 1e-13      # F = 0 on a pure-gauge field
+    prob.close()
+    U = li.haar_links(405, N, dims)
+    prob = GpuProblem(hr, dims, N, "fund", "f64", U)
+    lat = prob.lat
+    gin = _full(prob, psi)
+    outs = []
+    for csw in (0.0, 1.0, 2.0):
+        hr.hr_clover_build(cl, prob.links, csw, lat.stream())
+        o = lat.spinor(P, full=True)
+        hr.hr_dirac_clover(0.1, o, gin, prob.links, cl, lat.stream())
+        outs.append(_get_full(prob, o))
+    lat.dirac(0.1, b, gin, prob.links)
+    assert np.array_equal(outs[0], _get_full(prob, b))                  # c_sw = 0: exactly D
+    assert rel_l2(outs[2] - outs[0], 2 * (outs[1] - outs[0])) <= 1e-12  # linear in c_sw
+    with pytest.raises(hr.HrError):
+        hr.hr_clover_build(cl, prob.fund, 1.0, lat.stream())            # needs the represented field
+    with pytest.raises(hr.HrError):
+        hr.hr_dirac_clover(0.1, gin, gin, prob.links, cl, lat.stream())
+    prob.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_clover_on_a_131072_site_lattice(hr, prec):
+    """SU(3) fundamental 16^3 x 32 (1024 CTAs of the apply kernel, 2048 of the build kernel): every site against the
+    oracle (its whole-lattice numpy arrays take seconds here; at 32^3 x 64 they need minutes and 5 GB)."""
+    import torch
+    dims, N = (32, 16, 16, 16), 3
+    U = li.near_identity_links(406, N, dims, 0.3)
+    V = li.volume(dims)
+    psi = li.gaussian_spinor(407, V, 3)
+    prob = GpuProblem(hr, dims, N, "fund", prec, U)
+    lat, P = prob.lat, prob.prec
+    cl = torch.empty(hr.hr_clover_bytes(lat.ctx, P), dtype=torch.uint8, device="cuda")
+    hr.hr_clover_build(cl, prob.links, 1.0, lat.stream())
+    gin = _full(prob, psi)
+    o = lat.spinor(P, full=True)
+    hr.hr_dirac_clover(-0.2, o, gin, prob.links, cl, lat.stream())
+    got = _get_full(prob, o)
+    want = clover.dirac_clover(dims, BC_T, U, -0.2, 1.0, psi)
+    assert rel_l2(got, want) <= TOL[prec]
+    prob.close()
