@@ -96,6 +96,16 @@ def main():
     ops.append(("dphi_eo_interior", dphi_c, lambda k: hr.hr_dphi_eo_interior(sets[k % nset][2], sets[k % nset][0], links, k & 1, st)))
     ops.append(("halo_apply", None, lambda k: hr.hr_dphi_eo_halo_apply(sets[k % nset][2], hb[0], hb[1], links, k & 1, True, True, st)))
     face_bytes = {"halo_pack": nface * (2 * S + Lk + S), "halo_apply": nface * (S + Lk + 4 * S)}
+    # NEXT-4: clover term.  build: reads the represented links (each link is used by many leaves; algorithmic bytes
+    # 4L + C per site), apply as part of hr_dirac_clover: two Dphi launches with the mass term + two site-local launches
+    # (C + 3S per site each); bytes per site of the full lattice: 2(8L+3S)/2 ... reported per output site of one parity.
+    Cb = 8 * bm["d"] ** 2 * (8 if args.prec == "f64" else 4)
+    cl = torch.empty(hr.hr_clover_bytes(ctx, P), dtype=torch.uint8, device="cuda")
+    full_in, full_out = lat.spinor(P, full=True), lat.spinor(P, full=True)
+    full_in.zero_()
+    ops.append(("clover_build (per site of the FULL lattice: 4L + C)", 2 * (4 * L + Cb), lambda k: hr.hr_clover_build(cl, links, 1.0, st)))
+    ops.append(("dirac (both parities: 2(8L+3S) per site pair)", 2 * (dphi_c + S), lambda k: hr.hr_dirac(args.m0, full_out, full_in, links, st)))
+    ops.append(("dirac_clover (both parities: 2(8L+3S + C+3S))", 2 * (dphi_c + S + Cb + 3 * S), lambda k: hr.hr_dirac_clover(args.m0, full_out, full_in, links, cl, st)))
     common = {"workload": cfg["name"], "dtype": args.prec, "peak_gbs": peak, "peak_source": peak_src, "sites": vh}
     for name, bps, fn in ops:
         ms = timed(fn, args.reps)

@@ -12,7 +12,7 @@
 //
 // clover_build_kernel: one thread per site, set-up cost (once per gauge field; the Dirac operator is applied
 // hundreds of times per field in a solve), written with runtime loops over d_R.
-// clover_apply_kernel: out += T in, one thread per site, Hermitian block mat-vec unrolled on d_R;
+// clover_apply_kernel: out += T in, one thread per (site, chirality block), Hermitian block mat-vec unrolled on d_R;
 // algorithmic bytes per site: C + 3S (clover record, in, out read, out written).
 #include "hr_internal.h"
 
@@ -26,11 +26,15 @@ template <typename Real, int D, bool RL> struct CloverGeom {
 
 // complex D x D matrices as Real[2*D*D], row-major (re, im)
 template <typename Real, int D, bool DA, bool DB>
-__device__ void cmm(Real *o, const Real *a, const Real *b) // o = op(a) op(b), op = dagger if flagged
+__device__ __forceinline__ void cmm(Real *o, const Real *a, const Real *b) // o = op(a) op(b), op = dagger if flagged
 {
+    // d_R <= 4: fully unrolled, operands stay in registers; larger d_R: runtime loops over local arrays (set-up kernel)
+#pragma unroll(D <= 4 ? D : 1)
     for (int i = 0; i < D; ++i)
+#pragma unroll(D <= 4 ? D : 1)
         for (int j = 0; j < D; ++j) {
             Real re = 0, im = 0;
+#pragma unroll(D <= 4 ? D : 1)
             for (int k = 0; k < D; ++k) {
                 const int ia = DA ? 2 * (k * D + i) : 2 * (i * D + k);
                 const int ib = DB ? 2 * (j * D + k) : 2 * (k * D + j);
@@ -168,44 +172,49 @@ __global__ void __launch_bounds__(64) clover_build_kernel(const CloverArgs a)
     store_record<G::NREAL>(base, (size_t)a.vh, hs, rec);
 }
 
-// out += T in on one parity (clover/in/out point at that parity's half fields)
+// out += T in on one parity (clover/in/out point at that parity's half fields).  One thread per (site, chirality
+// block): it holds the block's 2 d_R input and output components and STREAMS the packed Hermitian block through one
+// 16-byte vector at a time (a whole d_R = 6 block is 144 reals -- preloading it spills).
 template <typename Real, int D>
 __global__ void __launch_bounds__(128) clover_apply_kernel(const CloverArgs a)
 {
-    constexpr int BLK = 4 * D * D, NREAL = 2 * BLK, N2 = 2 * D;
-    const long s = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    constexpr int BLK = 4 * D * D, N2 = 2 * D, RPV = 16 / (int)sizeof(Real);
+    constexpr int NVB = BLK / RPV;         // vectors per block record
+    constexpr int NVH = 4 * D / RPV;       // vectors of two spin components of a spinor
+    static_assert(BLK % RPV == 0 && (4 * D) % RPV == 0, "block and half spinor are whole vectors");
+    const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long s = tid >> 1;
+    const int b = (int)(tid & 1);
     if (s >= a.vh) return;
-    const size_t vh = (size_t)a.vh;
-    Real t[NREAL], psi[8 * D], o[8 * D];
-    load_record<LD_STREAM, NREAL>(t, (const char *)a.clover, vh, (size_t)s, 0);
-    load_record<LD_STREAM, 8 * D>(psi, (const char *)a.in, vh, (size_t)s, 0);
-    load_record<LD_STREAM, 8 * D>(o, (const char *)a.out, vh, (size_t)s, 0);
+    const size_t vh = (size_t)a.vh, pb = vh * 16;
+    Real v[4 * D], w[4 * D];
+    load_planes<LD_STREAM, NVH>(v, (const char *)a.in + (size_t)s * 16 + (size_t)(b * NVH) * pb, pb, 0);
+    load_planes<LD_STREAM, NVH>(w, (const char *)a.out + (size_t)s * 16 + (size_t)(b * NVH) * pb, pb, 0);
+    const char *tp = (const char *)a.clover + (size_t)s * 16 + (size_t)(b * NVB) * pb;
+    Real tv[RPV];
+    int idx = 0; // position in the packed block; a compile-time constant at every use once the loops are unrolled
+    auto next = [&]() -> Real {
+        if (idx % RPV == 0) load_planes<LD_STREAM, 1>(tv, tp + (size_t)(idx / RPV) * pb, pb, 0);
+        return tv[idx++ % RPV];
+    };
 #pragma unroll
-    for (int b = 0; b < 2; ++b) {
-        const Real *tb = t + b * BLK;
-        const Real *v = psi + b * 2 * N2; // spin components 2b, 2b+1: N2 complex numbers
-        Real *w = o + b * 2 * N2;
-#pragma unroll
-        for (int r = 0; r < N2; ++r) {
-            w[2 * r] = fma(tb[r], v[2 * r], w[2 * r]);
-            w[2 * r + 1] = fma(tb[r], v[2 * r + 1], w[2 * r + 1]);
-        }
-        int e = N2;
-#pragma unroll
-        for (int r = 0; r < N2; ++r)
-#pragma unroll
-            for (int c = r + 1; c < N2; ++c) {
-                const Real re = tb[e], im = tb[e + 1];
-                e += 2;
-                // row r gets T_rc v_c ; row c gets conj(T_rc) v_r
-                w[2 * r] = fma(re, v[2 * c], fma(-im, v[2 * c + 1], w[2 * r]));
-                w[2 * r + 1] = fma(re, v[2 * c + 1], fma(im, v[2 * c], w[2 * r + 1]));
-                w[2 * c] = fma(re, v[2 * r], fma(im, v[2 * r + 1], w[2 * c]));
-                w[2 * c + 1] = fma(re, v[2 * r + 1], fma(-im, v[2 * r], w[2 * c + 1]));
-            }
+    for (int d = 0; d < N2; ++d) {                            // diagonal entries (real)
+        const Real t = next();
+        w[2 * d] = fma(t, v[2 * d], w[2 * d]);
+        w[2 * d + 1] = fma(t, v[2 * d + 1], w[2 * d + 1]);
     }
-    constexpr int RPV = 16 / (int)sizeof(Real);
-    store_planes<ST_DEFAULT, 8 * D / RPV>((char *)a.out + (size_t)s * 16, vh * 16, o);
+#pragma unroll
+    for (int r = 0; r < N2; ++r)
+#pragma unroll
+        for (int c = r + 1; c < N2; ++c) {                    // T_rc = re + i im, T_cr = its conjugate
+            const Real re = next();
+            const Real im = next();
+            w[2 * r] = fma(re, v[2 * c], fma(-im, v[2 * c + 1], w[2 * r]));
+            w[2 * r + 1] = fma(re, v[2 * c + 1], fma(im, v[2 * c], w[2 * r + 1]));
+            w[2 * c] = fma(re, v[2 * r], fma(im, v[2 * r + 1], w[2 * c]));
+            w[2 * c + 1] = fma(re, v[2 * r + 1], fma(-im, v[2 * r], w[2 * c + 1]));
+        }
+    store_planes<ST_DEFAULT, NVH>((char *)a.out + (size_t)s * 16 + (size_t)(b * NVH) * pb, pb, w);
 }
 
 static hr_status launched(const char *what)
@@ -247,7 +256,7 @@ hr_status launch_clover_apply(const hr_ctx *c, hr_prec prec, void *out, const vo
     a.clover = const_cast<void *>(clover_parity); a.links = nullptr; a.in = in; a.out = out;
     a.T = c->dims[0]; a.X = c->dims[1]; a.Y = c->dims[2]; a.Z = c->dims[3];
     a.vh = c->Vh; a.csw = 0;
-    const unsigned grid = (unsigned)((c->Vh + 127) / 128);
+    const unsigned grid = (unsigned)((2 * c->Vh + 127) / 128);
 #define X(D)                                                                                                          \
     if (c->d == D) {                                                                                                  \
         if (prec == HR_F64) clover_apply_kernel<double, D><<<grid, 128, 0, st>>>(a);                                 \
