@@ -110,3 +110,44 @@ def dirac_solve(dims, bc, links_R, m0, b_eo, tol, maxiter):
     x_e, it, _ = cg_dhat(dims, bc, links_R, m0, rhs, tol, maxiter)
     x_o = (b_o - dphi_eo(dims, bc, links_R, 1, x_e)) / m
     return np.concatenate([x_e, x_o], axis=0), it
+
+
+# ---- stabilised bi-conjugate gradient ("stabilized Bi-Conjugate Gradient [11, 19]"; reading C29) ----
+def bicgstab(apply_A, b, tol, maxiter):
+    """Textbook BiCGstab (van der Vorst) for a general non-singular A, x0 = 0, shadow residual rhat = r0 = b,
+    no preconditioner, no half-step exit; the stopping rule |r_k|^2 <= tol^2 |b|^2 is tested after every full
+    iteration (reading C29).  <.,.> is antilinear in its first slot (reading C22).
+    Returns (x, iterations, [|r_k|^2 / |b|^2 for k = 0..iterations])."""
+    x = np.zeros_like(b)
+    r = b.copy()
+    rhat = b.copy()
+    bb = norm2(b)
+    hist = [1.0 if bb > 0 else 0.0]
+    if bb == 0.0:
+        return x, 0, hist
+    rho_old = alpha = omega = 1.0 + 0.0j
+    v = np.zeros_like(b)
+    p = np.zeros_like(b)
+    rr = bb
+    k = 0
+    while k < maxiter and rr > tol * tol * bb:
+        rho = dot(rhat, r)
+        beta = (rho / rho_old) * (alpha / omega)
+        p = r + beta * (p - omega * v)
+        v = apply_A(p)
+        alpha = rho / dot(rhat, v)
+        s = r - alpha * v
+        t = apply_A(s)
+        omega = dot(t, s) / norm2(t)
+        x = x + alpha * p + omega * s
+        r = s - omega * t
+        rho_old = rho
+        rr = norm2(r)
+        k += 1
+        hist.append(rr / bb)
+    return x, k, hist
+
+
+def bicgstab_dhat(dims, bc, links_R, m0, b_e, tol, maxiter):
+    """Solve Dhat x = b_e on the even sites with BiCGstab applied to Dhat itself (no normal equations)."""
+    return bicgstab(lambda v: dhat(dims, bc, links_R, m0, v), b_e, tol, maxiter)

@@ -126,3 +126,67 @@ def test_dirac_solve_equals_dense_solve(dims, N, rep):
     assert np.linalg.norm(x - want) <= 1e-10 * np.linalg.norm(want)
     # and it really solves the stencil operator
     assert np.linalg.norm(oracle.dirac(dims, BC_T, R, m0, x) - b) <= 1e-10 * np.linalg.norm(b)
+
+
+# ------------------------------------------------------------------------------------------------- BiCGstab
+def _rand_system(n, seed, shift):
+    rng = np.random.default_rng(seed)
+    A = (rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))) / np.sqrt(n) + shift * np.eye(n)   # non-Hermitian
+    b = (rng.normal(size=n) + 1j * rng.normal(size=n)).reshape(n // 12, 4, 3)
+    return A, b
+
+
+def test_bicgstab_solves_a_non_hermitian_system_like_numpy():
+    A, b = _rand_system(96, 1, 3.0)
+    apply_A = lambda v: (A @ v.reshape(-1)).reshape(v.shape)
+    x, it, hist = solver.bicgstab(apply_A, b, 1e-12, 200)
+    assert 2 < it < 100 and hist[0] == 1.0 and len(hist) == it + 1 and hist[-1] <= 1e-24
+    assert np.allclose(x.reshape(-1), np.linalg.solve(A, b.reshape(-1)), rtol=0, atol=1e-9)
+    # the recursively updated residual is the true one
+    assert abs(solver.norm2(b - apply_A(x)) / solver.norm2(b) - hist[-1]) <= 1e-20
+
+
+@pytest.mark.parametrize("k", [2, 3, 5])
+def test_bicgstab_terminates_within_k_steps_for_k_distinct_eigenvalues(k):
+    """r_j = Q_j(A) P_j(A) r_0 with P_j the BiCG residual polynomial: for a diagonalisable A with k distinct
+    eigenvalues P_k is the minimal polynomial, so BiCGstab is exact after at most k iterations (and, generically, not
+    before: the history must still be far from zero at k-1)."""
+    n = 24
+    evs = [2.0 + 1.0j, 0.5 - 0.25j, -1.0 + 0.5j, 1.5 + 2.0j, 3.0 - 1.0j][:k]
+    ev = np.array([evs[i % k] for i in range(n)])
+    b = (np.arange(n) + 1.0 + 0.5j * np.arange(n)[::-1]).reshape(2, 4, 3)
+    apply_A = lambda v: (ev * v.reshape(-1)).reshape(v.shape)
+    x, it, hist = solver.bicgstab(apply_A, b, 1e-12, 20)
+    assert it == k and hist[-1] <= 1e-24 and hist[k - 1] > 1e-12
+    assert np.allclose(x.reshape(-1), b.reshape(-1) / ev, rtol=0, atol=1e-10)
+
+
+def test_bicgstab_iterates_lie_in_the_krylov_spaces():
+    """x_k is in K_{2k}(A, b) = span{b, A b, ..., A^{2k-1} b}: a wrong update formula leaves the space."""
+    A, b = _rand_system(48, 5, 2.5)
+    apply_A = lambda v: (A @ v.reshape(-1)).reshape(v.shape)
+    for k in (1, 2, 3):
+        x, it, _ = solver.bicgstab(apply_A, b, 0.0, k)
+        assert it == k
+        K = np.empty((48, 2 * k), dtype=complex)
+        w = b.reshape(-1).copy()
+        for j in range(2 * k):
+            K[:, j] = w / np.linalg.norm(w)
+            w = A @ K[:, j]
+        coef, res, *_ = np.linalg.lstsq(K, x.reshape(-1), rcond=None)
+        assert np.linalg.norm(K @ coef - x.reshape(-1)) <= 1e-9 * np.linalg.norm(x)
+
+
+@pytest.mark.parametrize("dims,N,rep", [((2, 2, 2, 2), 2, "fund"), ((2, 2, 4, 2), 2, "adj")])
+def test_bicgstab_dhat_equals_dense_schur_solve(dims, N, rep):
+    R, d = _problem(dims, N, rep, 31)
+    m0 = -0.2
+    m = 4 + m0
+    D = _dense_eo(dims, BC_T, R, m0)
+    n = D.shape[0] // 2
+    schur = m * (D[:n, :n] - D[:n, n:] @ np.linalg.inv(D[n:, n:]) @ D[n:, :n])
+    b = li.gaussian_spinor(32, li.volume(dims) // 2, d)
+    x, it, hist = solver.bicgstab_dhat(dims, BC_T, R, m0, b, 1e-13, 500)
+    assert 0 < it < 500
+    want = np.linalg.solve(schur, b.reshape(-1)).reshape(b.shape)
+    assert np.linalg.norm(x - want) <= 1e-10 * np.linalg.norm(want)
