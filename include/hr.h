@@ -200,6 +200,15 @@ hr_status hr_dhat(double m0, int g5, void *out_e, const void *in_e, void *tmp_o,
  * x must not alias b.  Not converged within maxiter is not an error: check iters / rel_res2.
  */
 size_t hr_cg_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter);
+/*
+ * hr_bicgstab_dhat -- the stabilised bi-conjugate gradient ("stabilized Bi-Conjugate Gradient"; reading
+ * C29: textbook BiCGstab applied to Dhat ITSELF, no normal equations, x0 = 0, shadow residual = b, stopping at the
+ * first k with |r_k|^2 <= tol^2 |b|^2 or k = maxiter).  rho, alpha, omega live on the device like the CG's scalars.
+ * Arguments as hr_cg_dhat; workspace of hr_bicgstab_workspace_bytes().  rel_res2 / hist are relative to |b|^2.
+ */
+size_t hr_bicgstab_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter);
+hr_status hr_bicgstab_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol,
+                           int maxiter, void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
 hr_status hr_cg_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol, int maxiter,
                      void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
 hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links, double tol,

@@ -261,6 +261,76 @@ hr_status hr_cg_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const h
     return cg_run(ctx, m0, x_e, links, tol, maxiter, ws, iters, rel_res2, hist, st);
 }
 
+size_t hr_bicgstab_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter)
+{
+    if (!ctx || !valid_prec(prec) || maxiter < 0) return 0;
+    return 7 * (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec) + bicgstab_state_bytes(maxiter);
+}
+
+hr_status hr_bicgstab_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol, int maxiter,
+                           void *workspace, int *iters, double *rel_res2, double *hist, void *stream)
+{
+    hr_status rc = cg_check("hr_bicgstab_dhat", ctx, x_e, b_e, links, tol, maxiter, workspace);
+    if (rc != HR_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const hr_prec prec = links->prec;
+    char *ws = (char *)workspace;
+    const size_t sb = (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec);
+    void *r = ws, *rhat = ws + sb, *p = ws + 2 * sb, *v = ws + 3 * sb, *s = ws + 4 * sb, *t = ws + 5 * sb, *tmp = ws + 6 * sb;
+    void *state = ws + 7 * sb;
+    RedScratch rs;
+    rc = get_red_scratch(ctx, &rs, st);
+    if (rc != HR_OK) return rc;
+    rc = launch_bi_init(ctx, prec, state, tol, maxiter, x_e, r, rhat, p, v, b_e, rs, st);
+    if (rc != HR_OK) return rc;
+    const int *done = bicgstab_done(state);
+    auto one_iteration = [&]() -> hr_status {
+        hr_status e = launch_bi_update_p(ctx, prec, state, p, r, v, st);
+        if (e != HR_OK) return e;
+        e = dhat_launches(ctx, m0, 0, v, p, tmp, links, nullptr, nullptr, done, st);                       // v = Dhat p
+        if (e != HR_OK) return e;
+        e = launch_dot(ctx, prec, rhat, v, rs, bicgstab_rhat_v(state), st);                                 // <rhat, v>
+        if (e != HR_OK) return e;
+        e = launch_bi_update_s(ctx, prec, state, s, r, v, st);
+        if (e != HR_OK) return e;
+        e = dhat_launches(ctx, m0, 0, t, s, tmp, links, &rs, bicgstab_tt_st(state), done, st);             // t = Dhat s, |t|^2, <s,t>
+        if (e != HR_OK) return e;
+        return launch_bi_update_xr(ctx, prec, state, x_e, r, p, s, t, rhat, rs, st);
+    };
+    alignas(8) char hbuf[256];
+    const size_t hb = bicgstab_header_bytes();
+    int it = 0, dn = 0;
+    double bb = 0;
+    int batch = 4;
+    for (int issued = 0;;) {
+        HR_CUDA(cudaMemcpyAsync(hbuf, state, hb, cudaMemcpyDeviceToHost, st));
+        HR_CUDA(cudaStreamSynchronize(st));
+        bicgstab_unpack(hbuf, &it, &dn, &bb);
+        if (dn || issued >= maxiter) break;
+        const int n = maxiter - issued < batch ? maxiter - issued : batch;
+        for (int i = 0; i < n; ++i) {
+            rc = one_iteration();
+            if (rc != HR_OK) return rc;
+        }
+        issued += n;
+        if (batch < 32) batch *= 2;
+    }
+    if (iters) *iters = it;
+    const double *dh = (const double *)((const char *)state + hb);
+    if (hist) {
+        HR_CUDA(cudaMemcpyAsync(hist, dh, (size_t)(it + 1) * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HR_CUDA(cudaStreamSynchronize(st));
+        if (rel_res2) *rel_res2 = bb > 0 ? hist[it] / bb : 0.0;
+        if (bb > 0) for (int k = 0; k <= it; ++k) hist[k] /= bb;
+    } else if (rel_res2) {
+        double last = 0;
+        HR_CUDA(cudaMemcpyAsync(&last, dh + it, sizeof(double), cudaMemcpyDeviceToHost, st));
+        HR_CUDA(cudaStreamSynchronize(st));
+        *rel_res2 = bb > 0 ? last / bb : 0.0;
+    }
+    return HR_OK;
+}
+
 hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links, double tol,
                          int maxiter, void *workspace, int *iters, double *rel_res2, void *stream)
 {

@@ -163,6 +163,20 @@ hr_status launch_cg_update_r(const hr_ctx *c, hr_prec prec, CgState *cs, void *r
 hr_status launch_cg_update_xp(const hr_ctx *c, hr_prec prec, const CgState *cs, void *x, void *p, const void *r,
                               cudaStream_t st);
 
+// BiCGstab building blocks on a device-resident state (bicgstab.cu); the state struct is private to that file
+size_t bicgstab_state_bytes(int maxiter);
+size_t bicgstab_header_bytes();
+double *bicgstab_rhat_v(void *state);
+double *bicgstab_tt_st(void *state);
+const int *bicgstab_done(void *state);
+void bicgstab_unpack(const void *host_copy, int *iter, int *done, double *bb);
+hr_status launch_bi_init(const hr_ctx *c, hr_prec prec, void *state, double tol, int maxiter, void *x, void *r, void *rhat,
+                         void *p, void *v, const void *b, const RedScratch &rs, cudaStream_t st);
+hr_status launch_bi_update_p(const hr_ctx *c, hr_prec prec, const void *state, void *p, const void *r, const void *v, cudaStream_t st);
+hr_status launch_bi_update_s(const hr_ctx *c, hr_prec prec, void *state, void *s, const void *r, const void *v, cudaStream_t st);
+hr_status launch_bi_update_xr(const hr_ctx *c, hr_prec prec, void *state, void *x, void *r, const void *p, const void *s,
+                              const void *t, const void *rhat, const RedScratch &rs, cudaStream_t st);
+
 // pack / unpack: canonical AoS (device pointer) <-> internal planes
 hr_status launch_pack_spinor(const hr_ctx *c, void *dst, hr_prec prec, const void *canon_dev, hr_prec cprec,
                              long first_site, long nsites, cudaStream_t st);

@@ -308,3 +308,63 @@ def test_cg_graph_replay_is_bitwise_the_plain_launch_sequence(hr):
     with pytest.raises(hr.HrError):
         prob.lat.set_tuning("cg_graph", 3)
     prob.close()
+
+
+# ---------------------------------------------------------------------------------------------- BiCGstab
+@pytest.mark.parametrize("dims,N,rep,m0", CG_CASES)
+def test_bicgstab_dhat_fp64_follows_the_oracle(hr, dims, N, rep, m0):
+    """PAPER.md:124 "stabilized Bi-Conjugate Gradient"; reading C29.  Same algorithm and stopping rule on both sides:
+    the residual histories agree while they are well above rounding (BiCGstab amplifies rounding differences faster
+    than CG, so the history is compared for the first iterations and down to 1e-12 only), iteration counts to +-2,
+    solutions to the solver tolerance x condition number."""
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(121, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    b = li.gaussian_spinor(122, li.volume(dims) // 2, d)
+    tol, maxiter = 1e-10, 300
+    x_want, it_want, hist_want = solver.bicgstab_dhat(dims, BC_T, R, m0, b, tol, maxiter)
+    assert 3 < it_want < maxiter
+    prob = GpuProblem(hr, dims, N, rep, "f64", U)
+    f = Fields(hr, prob)
+    gb, gx = f.put(b), f.new()
+    import torch
+    ws = torch.empty(hr.hr_bicgstab_workspace_bytes(prob.lat.ctx, f.P, maxiter), dtype=torch.uint8, device="cuda")
+    it, res2, hist = hr.hr_bicgstab_dhat(prob.lat.ctx, m0, gx, gb, prob.links, tol, maxiter, ws, prob.lat.stream(), want_hist=True)
+    assert abs(it - it_want) <= 2 and hist[0] == 1.0 and len(hist) == it + 1 and res2 == hist[-1] <= tol * tol
+    n = min(it, it_want, 8) + 1
+    assert np.allclose(hist[:n], hist_want[:n], rtol=1e-5, atol=1e-14)
+    x = f.get(gx)
+    assert rel_l2(x, x_want) <= 1e-8
+    assert rel_l2(solver.dhat(dims, BC_T, R, m0, x), b) <= 1e-8         # it solves the oracle's operator
+    # fewer operator applications than the CG on the normal equations for the same accuracy
+    _, it_cg, _ = solver.cg_dhat(dims, BC_T, R, m0, b, tol, 500)
+    assert it <= it_cg
+    # bitwise reproducible
+    gx2 = f.new()
+    it2, res2b, _ = hr.hr_bicgstab_dhat(prob.lat.ctx, m0, gx2, gb, prob.links, tol, maxiter, ws, prob.lat.stream())
+    assert it2 == it and res2b == res2 and np.array_equal(f.get(gx2), x)
+    prob.close()
+
+
+def test_bicgstab_fp32_and_edge_cases(hr):
+    import torch
+    dims, N, m0 = (4, 4, 4, 8), 3, -0.3
+    U = li.haar_links(121, N, dims)
+    b = li.gaussian_spinor(122, li.volume(dims) // 2, 3)
+    x_want, it_want, _ = solver.bicgstab_dhat(dims, BC_T, U, m0, b, 1e-5, 300)
+    prob = GpuProblem(hr, dims, N, "fund", "f32", U)
+    f = Fields(hr, prob)
+    ctx, st = prob.lat.ctx, prob.lat.stream()
+    ws = torch.empty(hr.hr_bicgstab_workspace_bytes(ctx, f.P, 300), dtype=torch.uint8, device="cuda")
+    gb, gx = f.put(b), f.new()
+    it, res2, _ = hr.hr_bicgstab_dhat(ctx, m0, gx, gb, prob.links, 1e-5, 300, ws, st)
+    assert abs(it - it_want) <= 2 and res2 <= 1e-10 and rel_l2(f.get(gx), x_want) <= 1e-4
+    it, res2, hist = hr.hr_bicgstab_dhat(ctx, m0, gx, gb, prob.links, 1e-5, 0, ws, st, want_hist=True)     # maxiter = 0
+    assert it == 0 and res2 == 1.0 and not f.get(gx).any()
+    it, res2, _ = hr.hr_bicgstab_dhat(ctx, m0, gx, f.put(np.zeros_like(b)), prob.links, 1e-5, 50, ws, st)  # b = 0
+    assert it == 0 and res2 == 0.0 and not f.get(gx).any()
+    it, res2, hist = hr.hr_bicgstab_dhat(ctx, m0, gx, gb, prob.links, 1e-12, 3, ws, st, want_hist=True)    # maxiter hit
+    assert it == 3 and len(hist) == 4
+    with pytest.raises(hr.HrError):
+        hr.hr_bicgstab_dhat(ctx, m0, gb, gb, prob.links, 1e-5, 10, ws, st)
+    prob.close()
