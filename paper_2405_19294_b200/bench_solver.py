@@ -133,6 +133,33 @@ def main():
     gbs = bps * vh / (ms * 1e-3) / 1e9
     print(json.dumps(dict(common, op="cg_iteration", bytes_per_site=bps, ms=ms, gbs=gbs, frac=gbs / peak, iterations=it,
                           launches_per_iteration=(hr.hr_launch_count() - n0) / it, rel_res2=res2)))
+    # BiCGstab: one iteration = 4 Dphi launches + 3 vector kernels + 1 dot; algorithmic bytes
+    # 4(8L+2S) + 2S (self reads of the two fused epilogues) + 16S of vector passes
+    wsb = torch.empty(hr.hr_bicgstab_workspace_bytes(ctx, P, maxiter), dtype=torch.uint8, device="cuda")
+    hr.hr_bicgstab_dhat(ctx, args.m0, x, sets[0][0], links, 0.0, 4, wsb, st)
+    torch.cuda.synchronize()
+    n0 = hr.hr_launch_count()
+    e0.record()
+    it, res2, _ = hr.hr_bicgstab_dhat(ctx, args.m0, x, sets[0][0], links, 0.0, maxiter, wsb, st)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / it
+    bps = 4 * dphi_c + 2 * S + 16 * S
+    gbs = bps * vh / (ms * 1e-3) / 1e9
+    print(json.dumps(dict(common, op="bicgstab_iteration", bytes_per_site=bps, ms=ms, gbs=gbs, frac=gbs / peak, iterations=it,
+                          launches_per_iteration=(hr.hr_launch_count() - n0) / it)))
+    # time to solution, same right-hand side, relative residual 1e-8 (fp64) / 1e-5 (fp32): CG on the normal equations
+    # vs BiCGstab on Dhat
+    tol = 1e-8 if args.prec == "f64" else 1e-5
+    for name, fn in (("cg_solve", lambda: lat.cg_dhat(args.m0, x, sets[0][0], links, tol, 2000, lat.cg_workspace(P, 2000))),
+                     ("bicgstab_solve", lambda: hr.hr_bicgstab_dhat(ctx, args.m0, x, sets[0][0], links, tol, 2000,
+                                                                    torch.empty(hr.hr_bicgstab_workspace_bytes(ctx, P, 2000), dtype=torch.uint8, device="cuda"), st))):
+        torch.cuda.synchronize()
+        e0.record()
+        it, res2, _ = fn()
+        e1.record()
+        torch.cuda.synchronize()
+        print(json.dumps(dict(common, op=name, tol=tol, iterations=it, rel_res2=res2, ms=e0.elapsed_time(e1), bytes_per_site=0, gbs=0.0, frac=0.0)))
     lat.close()
 
 
