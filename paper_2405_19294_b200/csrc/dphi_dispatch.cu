@@ -21,6 +21,9 @@ static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
     // measured on B200 (profiles/r1_variant_sweep.md): at d_R >= 6 fp64 one thread per site spills
     // and the pair kernel wins; in fp32 the whole site still fits one thread.
     if (c->d >= 6) return prec == HR_F64 ? 3 : 1;
+    // SU(2) adjoint (real 3x3 links, spinors are 40 % of the compulsory bytes): evict-first links / evict-last
+    // spinors gain 2 % (0.0965 -> 0.0944 ms at 32^4 fp64)
+    if (lk == 1 && c->d == 3) return 1;
     return 0;
 }
 

@@ -28,16 +28,19 @@ template <typename Real, int D, int LK, int KSPLIT> struct Tune {
     static constexpr int W = (int)sizeof(Real) / 4;
     static constexpr int LIVE = W * ((KSPLIT == 1 ? 8 * D : 6 * D) + (KSPLIT == 1 ? 8 * D : 4 * D) + LNREAL) + 40;
     static constexpr int MAXT = 128;
-    // measured (profiles/): the fp32 on-the-fly kernels gain 7 % from a 128-register cap (16 warps per SM)
+    // measured (profiles/): the fp32 on-the-fly kernels gain 7 % from a 128-register cap (16 warps per SM); the fp64
+    // real-link d_R = 3 kernel (LIVE = 154) loses 3 % at a 168-register cap (it spills), hence the 150 threshold
     static constexpr int MINB = (LK >= 2 && sizeof(Real) == 4 && KSPLIT == 1) ? 4 :
-                                LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? 4 : LIVE <= 168 ? 3 : LIVE <= 255 ? 2 : 1;
+                                LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? 4 : LIVE <= 150 ? 3 : LIVE <= 255 ? 2 : 1;
 };
 
 template <typename Real, int D, int LK, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT>
 static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
 {
     using T = Tune<Real, D, LK, KSPLIT>;
-    if (block <= 0) block = T::MAXT;
+    // default CTA: 64 threads for the one-thread-per-site kernels (same warps per SM, finer tail; measured 1-4 %
+    // faster than 128 on every config), 128 for the pair kernels
+    if (block <= 0) block = KSPLIT == 1 ? 64 : T::MAXT;
     if (block > T::MAXT || (block % 32) != 0) {
         set_error("block=%d not supported by this variant (multiple of 32, <= %d)", block, T::MAXT);
         return HR_EINVAL;
