@@ -72,7 +72,8 @@ size_t hr_spinor_bytes(const hr_ctx *ctx, hr_prec prec);                 /* ONE 
 
 /*
  * hr_gauge_alloc -- make a link-field handle (BASELINE.json:north_star "hr_gauge_alloc").
- * represented = 0: fundamental N x N complex links; 1: represented d_R x d_R links (real for ADJ).
+ * represented = 0: fundamental N x N complex links; 1: represented d_R x d_R links (real for ADJ);
+ * 2: fundamental links stored as their first N-1 rows (hr_gauge_compress below; SU(2), SU(3) only).
  * dev_mem == NULL: the library allocates hr_gauge_bytes() of device memory and owns it;
  * else it borrows caller memory (>= hr_gauge_bytes(), 16-byte aligned), which must outlive the handle.
  * Contents are undefined until hr_gauge_import / hr_represent_links writes them.
@@ -91,6 +92,17 @@ hr_status hr_spinor_import(const hr_ctx *ctx, void *dst_dev, hr_prec prec, const
                            hr_prec canon_prec, int parity, void *stream);
 hr_status hr_spinor_export(const hr_ctx *ctx, const void *src_dev, hr_prec prec, void *canon,
                            hr_prec canon_prec, int parity, void *stream);
+
+/*
+ * hr_gauge_compress -- row-compressed fundamental links (reading C30 of DESIGN.md; SU(2) and SU(3)).
+ * hr_gauge_alloc(ctx, 2, prec, ...) makes a field that keeps only the first N-1 rows of every fundamental link
+ * (SU(3): 12 of 18 reals, SU(2): 4 of 8); hr_gauge_compress fills it from a fundamental field of the same precision.
+ * Every compute call that takes `links` accepts it for the FUNDAMENTAL representation (the last row is rebuilt in
+ * registers: conj(row0 x row1), resp. (-conj u01, conj u00)) and for the SU(2) ADJOINT (the real 3x3 link is built from
+ * the four reals of the first row: 32 instead of 72 bytes per link in fp64).  Only for links that ARE special unitary:
+ * the result equals that of the full links up to their unitarity violation.  Such a field cannot be imported/exported.
+ */
+hr_status hr_gauge_compress(hr_gauge *rows_out, const hr_gauge *fund_in, void *stream);
 
 /*
  * hr_represent_links -- the link map U -> U^R, one kernel launch over the 4V links

@@ -66,6 +66,7 @@ _SIGNATURES = {
     "hr_spinor_import": (_ci, [_vp, _vp, _ci, _vp, _ci, _ci, _vp]),
     "hr_spinor_export": (_ci, [_vp, _vp, _ci, _vp, _ci, _ci, _vp]),
     "hr_represent_links": (_ci, [_vp, _vp, _vp]),
+    "hr_gauge_compress": (_ci, [_vp, _vp, _vp]),
     "hr_dphi_eo": (_ci, [_vp, _vp, _vp, _ci, _vp]),
     "hr_dirac": (_ci, [_cd, _vp, _vp, _vp, _vp]),
     "hr_dphi_eo_host": (_ci, [_vp, _vp, _vp, _ci, _vp, _ci, _vp]),
@@ -210,6 +211,10 @@ def hr_spinor_import(ctx: int, dst_dev, prec: int, canon, canon_prec: int, parit
 
 def hr_spinor_export(ctx: int, src_dev, prec: int, canon, canon_prec: int, parity: int, stream: int = 0) -> None:
     _check(_lib.hr_spinor_export(ctx, _ptr(src_dev), prec, _ptr(canon), canon_prec, parity, stream))
+
+
+def hr_gauge_compress(rows_out: int, fund_in: int, stream: int = 0) -> None:
+    _check(_lib.hr_gauge_compress(rows_out, fund_in, stream))
 
 
 def hr_represent_links(repr_out: int, fund_in: int, stream: int = 0) -> None:
@@ -390,8 +395,9 @@ class Lattice:
             pass
 
     # -- fields
-    def gauge(self, represented: bool, prec: int) -> int:
-        """hr_gauge_alloc on torch-owned device memory; returns the handle."""
+    def gauge(self, represented, prec: int) -> int:
+        """hr_gauge_alloc on torch-owned device memory; returns the handle.  represented: False/0 fundamental,
+        True/1 represented, 2 fundamental stored as N-1 rows (fill with compress_links)."""
         nbytes = hr_gauge_bytes(self.ctx, int(represented), prec)
         mem = self._torch.empty(nbytes, dtype=self._torch.uint8, device=f"cuda:{self.device}")
         h = hr_gauge_alloc(self.ctx, int(represented), prec, mem)
@@ -426,6 +432,9 @@ class Lattice:
         return out
 
     # -- the hot path
+    def compress_links(self, rows_out: int, fund_in: int) -> None:
+        hr_gauge_compress(rows_out, fund_in, self.stream())
+
     def represent_links(self, repr_out: int, fund_in: int) -> None:
         hr_represent_links(repr_out, fund_in, self.stream())
 

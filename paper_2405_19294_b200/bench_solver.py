@@ -85,6 +85,15 @@ def main():
                     lambda k: hr.hr_dphi_eo(sets[k % nset][2], sets[k % nset][0], fund, k & 1, st)))
         ops.append(("dhat on-the-fly", 2 * (8 * F + 2 * S) + S,
                     lambda k: hr.hr_dhat(args.m0, 1, sets[k % nset][2], sets[k % nset][0], sets[k % nset][1], fund, st)))
+    if cfg["N"] <= 3 and (cfg["rep"] == "fund" or (cfg["rep"] == "adj" and cfg["N"] == 2)):
+        # row-compressed fundamental links: bytes 8 Lrows + 2S actually needed
+        rows = lat.gauge(2, P)
+        lat.compress_links(rows, fund)
+        lrows = 2 * cfg["N"] * (cfg["N"] - 1) * (8 if args.prec == "f64" else 4)
+        ops.append(("dphi_eo from row-compressed links (bytes 8 Lrows + 2S)", 8 * lrows + 2 * S,
+                    lambda k: hr.hr_dphi_eo(sets[k % nset][2], sets[k % nset][0], rows, k & 1, st)))
+        ops.append(("dhat from row-compressed links", 2 * (8 * lrows + 2 * S) + S,
+                    lambda k: hr.hr_dhat(args.m0, 1, sets[k % nset][2], sets[k % nset][0], sets[k % nset][1], rows, st)))
     # NEXT-2: the slab pipeline of ONE rank (its neighbour is itself): what the decomposition costs on top of
     # a plain Dphi_eo of the same local volume.  Algorithmic bytes: pack reads 2 slices of spinors and 1 of links
     # and writes 2 half-spinor faces; apply reads them back, 1 slice of links, and read-modify-writes 2 slices.

@@ -17,7 +17,8 @@ static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "sit
 static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
 {
     // on-the-fly two-index kernels hold an N x N link, not a d_R x d_R one: a whole site fits one thread
-    if (lk >= 2) return 0;
+    if (lk == 2 || lk == 3 || lk == 4) return 0;
+    if (lk == 5) return 1;
     // measured on B200 (profiles/r1_variant_sweep.md): at d_R >= 6 fp64 one thread per site spills
     // and the pair kernel wins; in fp32 the whole site still fits one thread.
     if (c->d >= 6) return prec == HR_F64 ? 3 : 1;
@@ -31,22 +32,29 @@ static int resolve_variant(const hr_ctx *c, hr_prec prec, int lk) { return c->va
 
 // link kind (dphi_kernel.cuh): 0 complex d_R x d_R, 1 real d_R x d_R (adjoint), 2 / 3 two-index symmetric /
 // antisymmetric applied on the fly from the fundamental link
-int dphi_link_kind(const hr_ctx *c, bool fundamental_links)
+int dphi_link_kind(const hr_ctx *c, int link_src)
 {
-    if (!fundamental_links || c->rep == HR_REP_FUND) return c->real_links ? 1 : 0; // FUND: both fields are N x N complex
-    if (c->rep == HR_REP_SYM) return 2;
-    if (c->rep == HR_REP_ASYM) return 3;
-    return -1; // adjoint on the fly: not built
+    if (link_src == 0) return c->real_links ? 1 : 0;
+    if (link_src == 1) {                                   // full fundamental field
+        if (c->rep == HR_REP_FUND) return 0;               // FUND: both fields are N x N complex
+        if (c->rep == HR_REP_SYM) return 2;
+        if (c->rep == HR_REP_ASYM) return 3;
+        return -1;                                         // adjoint from full fundamental links: not built
+    }
+    if (c->N > 3) return -1;                               // rows: SU(2), SU(3)
+    if (c->rep == HR_REP_FUND) return 4;
+    if (c->rep == HR_REP_ADJ && c->N == 2) return 5;
+    return -1;
 }
 
 #define HR_COMBOS(X)                                                                                      \
-    X(2, 0) X(3, 0) X(4, 0) X(6, 0) X(3, 1) X(8, 1) X(3, 2) X(6, 2) X(3, 3) X(6, 3)
+    X(2, 0) X(3, 0) X(4, 0) X(6, 0) X(3, 1) X(8, 1) X(3, 2) X(6, 2) X(3, 3) X(6, 3) X(2, 4) X(3, 4) X(3, 5)
 
-hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st, bool fundamental_links)
+hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st, int link_src)
 {
-    const int lk = dphi_link_kind(c, fundamental_links);
+    const int lk = dphi_link_kind(c, link_src);
     if (lk < 0) {
-        set_error("fundamental links given, but this representation has no on-the-fly kernel (use hr_represent_links)");
+        set_error("this kind of link field has no kernel for this representation (use hr_represent_links)");
         return HR_EUNSUPPORTED;
     }
     const int v = resolve_variant(c, prec, lk);
@@ -60,9 +68,9 @@ hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStre
     return HR_EUNSUPPORTED;
 }
 
-hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, const HaloArgs &a, cudaStream_t st, bool fundamental_links)
+hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, const HaloArgs &a, cudaStream_t st, int link_src)
 {
-    const int lk = dphi_link_kind(c, fundamental_links);
+    const int lk = dphi_link_kind(c, link_src);
 #define X(D, LK)                                                                                          \
     if (c->d == D && lk == LK)                                                                            \
         return prec == HR_F64 ? launch_halo_t<double, D, LK>(pack, a, st) : launch_halo_t<float, D, LK>(pack, a, st);

@@ -27,6 +27,8 @@
 //  * loads are 128-bit, coalesced over the half index (hr_internal.h); links are streamed past L1
 //        (and optionally evict-first in L2), neighbour spinors are left to L1/L2 for re-use.
 #pragma once
+#include <type_traits>
+
 #include "hr_internal.h"
 
 namespace hr {
@@ -97,13 +99,20 @@ __device__ __forceinline__ void colour_mul(Real (&chi)[2 * D], const Real *u, co
 // FUNDAMENTAL N x N link (144 B instead of 576 B for the SU(3) sextet in fp64) and applies the two-index
 // representation without ever forming R(U): with the colour vector written as the (anti)symmetric matrix
 // Psi = sum_a psi_a e_a (basis of reading C8),  R(U) psi <-> U Psi U^T  and  R(U)^dagger psi <-> U^dagger Psi U^*.
-enum : int { LK_COMPLEX = 0, LK_REAL = 1, LK_SYM_OTF = 2, LK_ASYM_OTF = 3 };
+// LK_ROWS / LK_ADJ2_ROWS: the fundamental link is stored as its first N-1 rows (SU(3): 12 of 18 reals, SU(2): 4 of 8);
+// the last row is rebuilt in registers (SU(3): conj(row0 x row1); SU(2): (-conj u01, conj u00)) -- 25-33 % fewer
+// link bytes for the fundamental representation.  LK_ADJ2_ROWS builds the real 3x3 SU(2) adjoint link from the four
+// reals (a0, a3, a2, a1) = first row of U = a0 + i a.sigma:  R_ab = (a0^2 - a.a) delta_ab + 2 a_a a_b + 2 a0 eps_abc a_c
+// (32 B instead of 72 B per link in fp64).  Valid for links that ARE special unitary (reading C30).
+enum : int { LK_COMPLEX = 0, LK_REAL = 1, LK_SYM_OTF = 2, LK_ASYM_OTF = 3, LK_ROWS = 4, LK_ADJ2_ROWS = 5 };
 
 template <int LK, int D> struct LinkGeom {
     // N of the fundamental link for the on-the-fly kinds: D = N(N+1)/2 (sym) or N(N-1)/2 (asym)
     static constexpr int N = LK == LK_SYM_OTF ? (D == 3 ? 2 : D == 6 ? 3 : D == 10 ? 4 : 0)
-                           : LK == LK_ASYM_OTF ? (D == 3 ? 3 : D == 6 ? 4 : 0) : D;
-    static constexpr int NREAL = LK == LK_REAL ? D * D : LK == LK_COMPLEX ? 2 * D * D : 2 * N * N;
+                           : LK == LK_ASYM_OTF ? (D == 3 ? 3 : D == 6 ? 4 : 0)
+                           : LK == LK_ADJ2_ROWS ? (D == 3 ? 2 : 0) : D;
+    static constexpr int NREAL = LK == LK_REAL ? D * D : LK == LK_COMPLEX ? 2 * D * D
+                               : (LK == LK_ROWS || LK == LK_ADJ2_ROWS) ? 2 * N * (N - 1) : 2 * N * N;
     static_assert(N > 0, "no such two-index representation");
 };
 
@@ -169,11 +178,74 @@ __device__ __forceinline__ void twoindex_mul(Real (&chi)[2 * D], const Real *u, 
         }
 }
 
+// full N x N complex link from its first N-1 rows (N = 2, 3)
+template <int N, typename Real> __device__ __forceinline__ void rebuild_rows(Real (&f)[2 * N * N], const Real *r)
+{
+    static_assert(N == 2 || N == 3, "row reconstruction for SU(2) and SU(3)");
+#pragma unroll
+    for (int e = 0; e < 2 * N * (N - 1); ++e) f[e] = r[e];
+    if constexpr (N == 2) {
+        f[4] = -r[2]; f[5] = r[3];   // -conj(u01)
+        f[6] = r[0];  f[7] = -r[1];  //  conj(u00)
+    } else {
+        // row2_j = conj(row0_k row1_l - row0_l row1_k), (j,k,l) cyclic
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const int k = (j + 1) % 3, l = (j + 2) % 3;
+            const Real ar = r[2 * k], ai = r[2 * k + 1], br = r[6 + 2 * l], bi = r[6 + 2 * l + 1];
+            const Real cr = r[2 * l], ci = r[2 * l + 1], dr = r[6 + 2 * k], di = r[6 + 2 * k + 1];
+            f[12 + 2 * j] = (ar * br - ai * bi) - (cr * dr - ci * di);
+            f[12 + 2 * j + 1] = -((ar * bi + ai * br) - (cr * di + ci * dr));
+        }
+    }
+}
+
+// real 3x3 SU(2) adjoint link from (a0, a3, a2, a1) = the first row of the fundamental link
+template <typename Real> __device__ __forceinline__ void rebuild_adj2(Real (&m)[9], const Real *r)
+{
+    const Real a0 = r[0], a[3] = { r[3], r[2], r[1] };
+    const Real dg = a0 * a0 - (a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) m[3 * i + j] = (Real)2 * a[i] * a[j] + (i == j ? dg : (Real)0);
+    // + 2 a0 eps_ijk a_k
+    m[1] += (Real)2 * a0 * a[2]; m[3] -= (Real)2 * a0 * a[2];
+    m[5] += (Real)2 * a0 * a[0]; m[7] -= (Real)2 * a0 * a[0];
+    m[6] += (Real)2 * a0 * a[1]; m[2] -= (Real)2 * a0 * a[1];
+}
+
 template <int D, int LK, bool DAG, typename Real>
 __device__ __forceinline__ void link_mul(Real (&chi)[2 * D], const Real *u, const Real (&h)[2 * D])
 {
     if constexpr (LK == LK_COMPLEX || LK == LK_REAL) colour_mul<D, LK == LK_REAL, DAG>(chi, u, h);
-    else twoindex_mul<D, LK, DAG>(chi, u, h);
+    else if constexpr (LK == LK_ROWS) {
+        Real f[2 * D * D];
+        rebuild_rows<D>(f, u);     // identical for both half-spinor components of a hop: the compiler merges the two
+        colour_mul<D, false, DAG>(chi, f, h);
+    } else if constexpr (LK == LK_ADJ2_ROWS) {
+        Real m[9];
+        rebuild_adj2(m, u);
+        colour_mul<3, true, DAG>(chi, m, h);
+    } else twoindex_mul<D, LK, DAG>(chi, u, h);
+}
+
+// Run `f(kind, link)` with the link in the form the colour multiply wants: row-compressed kinds are rebuilt ONCE per
+// hop here (both half-spinor components then share the registers), every other kind is passed through.
+template <int D, int LK, typename Real, typename F>
+__device__ __forceinline__ void with_link(const Real *u, F &&f)
+{
+    if constexpr (LK == LK_ROWS) {
+        Real full[2 * D * D];
+        rebuild_rows<D>(full, u);
+        f(std::integral_constant<int, LK_COMPLEX>{}, (const Real *)full);
+    } else if constexpr (LK == LK_ADJ2_ROWS) {
+        Real m[9];
+        rebuild_adj2(m, u);
+        f(std::integral_constant<int, LK_REAL>{}, (const Real *)m);
+    } else {
+        f(std::integral_constant<int, LK>{}, u);
+    }
 }
 
 // one half-spinor component of one hop:  h = a + sk c0 b ; chi = U(^dag) h ; outK += sgn chi ;
@@ -303,8 +375,11 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
             constexpr int P0 = (MU == 0 || MU == 3) ? 2 : 3;
             constexpr int P1 = 5 - P0;
             const Real sg = (Real)sign;
-            hop_component<MU, DIR, D, LK, Real>(u, psi + 0 * 2 * D, psi + P0 * 2 * D, (Real)1, sg, acc[0], acc[P0]);
-            hop_component<MU, DIR, D, LK, Real>(u, psi + 1 * 2 * D, psi + P1 * 2 * D, (Real)(MU >= 2 ? -1 : 1), sg, acc[1], acc[P1]);
+            with_link<D, LK, Real>(u, [&](auto lk_c, const Real *ul) {
+                constexpr int K = decltype(lk_c)::value;
+                hop_component<MU, DIR, D, K, Real>(ul, psi + 0 * 2 * D, psi + P0 * 2 * D, (Real)1, sg, acc[0], acc[P0]);
+                hop_component<MU, DIR, D, K, Real>(ul, psi + 1 * 2 * D, psi + P1 * 2 * D, (Real)(MU >= 2 ? -1 : 1), sg, acc[1], acc[P1]);
+            });
         };
         using I0 = std::integral_constant<int, 0>; using I1 = std::integral_constant<int, 1>;
         using I2 = std::integral_constant<int, 2>; using I3 = std::integral_constant<int, 3>;
@@ -366,7 +441,9 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
             if constexpr (DIR == 0) load_record<LHINT, LNREAL>(u, lk_own + (size_t)MU * LB * vh, vh, (size_t)s, pol_l);
             else                    load_record<LHINT, LNREAL>(u, lk_nbr + (size_t)MU * LB * vh, vh, (size_t)sn, pol_l);
             const Real sk = (MU >= 2 && k == 1) ? (Real)-1 : (Real)1;
-            hop_component<MU, DIR, D, LK, Real>(u, pa, pbv, sk, (Real)sign, accK, STRAIGHT ? accP : accQ);
+            with_link<D, LK, Real>(u, [&](auto lk_c, const Real *ul) {
+                hop_component<MU, DIR, D, decltype(lk_c)::value, Real>(ul, pa, pbv, sk, (Real)sign, accK, STRAIGHT ? accP : accQ);
+            });
         };
         using I0 = std::integral_constant<int, 0>; using I1 = std::integral_constant<int, 1>;
         using I2 = std::integral_constant<int, 2>; using I3 = std::integral_constant<int, 3>;

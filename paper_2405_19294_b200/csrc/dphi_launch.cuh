@@ -30,7 +30,8 @@ template <typename Real, int D, int LK, int KSPLIT> struct Tune {
     static constexpr int MAXT = 128;
     // measured (profiles/): the fp32 on-the-fly kernels gain 7 % from a 128-register cap (16 warps per SM); the fp64
     // real-link d_R = 3 kernel (LIVE = 154) loses 3 % at a 168-register cap (it spills), hence the 150 threshold
-    static constexpr int MINB = (LK >= 2 && sizeof(Real) == 4 && KSPLIT == 1) ? 4 :
+    static constexpr int MINB = ((LK == LK_SYM_OTF || LK == LK_ASYM_OTF) && sizeof(Real) == 4 && KSPLIT == 1) ? 4 :
+                                (LK == LK_ADJ2_ROWS && sizeof(Real) == 8 && KSPLIT == 1) ? 2 :   // as the real-link kernel it expands to
                                 LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? 4 : LIVE <= 150 ? 3 : LIVE <= 255 ? 2 : 1;
 };
 

@@ -135,8 +135,11 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_pf_kernel(const DphiArgs a)
         constexpr int P0 = (MU == 0 || MU == 3) ? 2 : 3;
         constexpr int P1 = 5 - P0;
         const Real sg = (Real)sign;
-        hop_component<MU, DIR, D, LK, Real>(u, psi + 0 * 2 * D, psi + P0 * 2 * D, (Real)1, sg, acc[0], acc[P0]);
-        hop_component<MU, DIR, D, LK, Real>(u, psi + 1 * 2 * D, psi + P1 * 2 * D, (Real)(MU >= 2 ? -1 : 1), sg, acc[1], acc[P1]);
+        with_link<D, LK, Real>(u, [&](auto lk_c, const Real *ul) {
+            constexpr int K = decltype(lk_c)::value;
+            hop_component<MU, DIR, D, K, Real>(ul, psi + 0 * 2 * D, psi + P0 * 2 * D, (Real)1, sg, acc[0], acc[P0]);
+            hop_component<MU, DIR, D, K, Real>(ul, psi + 1 * 2 * D, psi + P1 * 2 * D, (Real)(MU >= 2 ? -1 : 1), sg, acc[1], acc[P1]);
+        });
     };
     using I0 = std::integral_constant<int, 0>; using I1 = std::integral_constant<int, 1>;
     using I2 = std::integral_constant<int, 2>; using I3 = std::integral_constant<int, 3>;

@@ -207,7 +207,7 @@ size_t hr_half_volume(const hr_ctx *ctx) { return ctx ? (size_t)ctx->Vh : 0; }
 
 size_t hr_gauge_bytes(const hr_ctx *ctx, int represented, hr_prec prec)
 {
-    if (!ctx || !valid_prec(prec)) return 0;
+    if (!ctx || !valid_prec(prec) || represented < 0 || represented > 2) return 0;
     return (size_t)ctx->V * 4 * link_nreal(ctx, represented) * prec_bytes(prec);
 }
 
@@ -221,9 +221,13 @@ hr_status hr_gauge_alloc(const hr_ctx *ctx, int represented, hr_prec prec, void 
 {
     if (!ctx || !out) { set_error("hr_gauge_alloc: NULL argument"); return HR_EINVAL; }
     *out = nullptr;
-    if (!valid_prec(prec) || (represented != 0 && represented != 1)) {
+    if (!valid_prec(prec) || represented < 0 || represented > 2) {
         set_error("hr_gauge_alloc: bad precision or `represented` flag");
         return HR_EINVAL;
+    }
+    if (represented == 2 && ctx->N > 3) {
+        set_error("hr_gauge_alloc: row-compressed fundamental links exist for SU(2) and SU(3) only");
+        return HR_EUNSUPPORTED;
     }
     if (dev_mem && ((uintptr_t)dev_mem & 15)) { set_error("hr_gauge_alloc: dev_mem must be 16-byte aligned"); return HR_EINVAL; }
     hr_gauge *g = new (std::nothrow) hr_gauge();
@@ -261,6 +265,7 @@ void *hr_gauge_data(const hr_gauge *g) { return g ? g->data : nullptr; }
 hr_status hr_gauge_import(hr_gauge *dst, const void *canon, hr_prec canon_prec, void *stream)
 {
     if (!dst || !canon || !valid_prec(canon_prec)) { set_error("hr_gauge_import: bad argument"); return HR_EINVAL; }
+    if (dst->represented == 2) { set_error("hr_gauge_import: a row-compressed field is filled by hr_gauge_compress"); return HR_EUNSUPPORTED; }
     return transfer(dst->ctx, FIELD_GAUGE, true, dst->nreal, dst->data, dst->prec, const_cast<void *>(canon), canon_prec,
                     (cudaStream_t)stream);
 }
@@ -268,6 +273,7 @@ hr_status hr_gauge_import(hr_gauge *dst, const void *canon, hr_prec canon_prec, 
 hr_status hr_gauge_export(const hr_gauge *src, void *canon, hr_prec canon_prec, void *stream)
 {
     if (!src || !canon || !valid_prec(canon_prec)) { set_error("hr_gauge_export: bad argument"); return HR_EINVAL; }
+    if (src->represented == 2) { set_error("hr_gauge_export: a row-compressed field has no canonical form; export the fundamental field"); return HR_EUNSUPPORTED; }
     return transfer(src->ctx, FIELD_GAUGE, false, src->nreal, src->data, src->prec, canon, canon_prec, (cudaStream_t)stream);
 }
 
@@ -293,11 +299,23 @@ hr_status hr_spinor_export(const hr_ctx *ctx, const void *src_dev, hr_prec prec,
                     (cudaStream_t)stream);
 }
 
+hr_status hr_gauge_compress(hr_gauge *rows_out, const hr_gauge *fund_in, void *stream)
+{
+    if (!rows_out || !fund_in) { set_error("hr_gauge_compress: NULL argument"); return HR_EINVAL; }
+    if (rows_out->ctx != fund_in->ctx || rows_out->represented != 2 || fund_in->represented != 0 || rows_out->prec != fund_in->prec) {
+        set_error("hr_gauge_compress: need (row-compressed out, fundamental in) of one context and one precision");
+        return HR_EINVAL;
+    }
+    hr_status rc = use_device(fund_in->ctx);
+    if (rc != HR_OK) return rc;
+    return launch_compress(fund_in->ctx, fund_in->prec, rows_out->data, fund_in->data, (cudaStream_t)stream);
+}
+
 hr_status hr_represent_links(hr_gauge *repr_out, const hr_gauge *fund_in, void *stream)
 {
     if (!repr_out || !fund_in) { set_error("hr_represent_links: NULL argument"); return HR_EINVAL; }
     if (repr_out->ctx != fund_in->ctx) { set_error("hr_represent_links: fields belong to different contexts"); return HR_EINVAL; }
-    if (!repr_out->represented || fund_in->represented) {
+    if (repr_out->represented != 1 || fund_in->represented != 0) {
         set_error("hr_represent_links: need (represented out, fundamental in)");
         return HR_EINVAL;
     }
@@ -377,7 +395,7 @@ hr_status hr_dphi_eo(void *out, const void *in, const hr_gauge *links, int parit
 {
     if (!out || !in || !links) { set_error("hr_dphi_eo: NULL argument"); return HR_EINVAL; }
     if (parity != 0 && parity != 1) { set_error("hr_dphi_eo: parity=%d", parity); return HR_EINVAL; }
-    if (!links->represented && dphi_link_kind(links->ctx, true) < 0) {
+    if (dphi_link_kind(links->ctx, link_src(links)) < 0) {
         set_error("hr_dphi_eo: `links` must be a represented field (hr_represent_links); fundamental links are accepted "
                   "only for the fundamental and two-index representations");
         return HR_EINVAL;
@@ -390,13 +408,13 @@ hr_status hr_dphi_eo(void *out, const void *in, const hr_gauge *links, int parit
     DphiArgs a;
     const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 };
     dphi_args(a, c, out, in, nullptr, links, parity, zero, mhalf);
-    return launch_dphi(c, links->prec, a, (cudaStream_t)stream, !links->represented);
+    return launch_dphi(c, links->prec, a, (cudaStream_t)stream, link_src(links));
 }
 
 hr_status hr_dirac(double m0, void *out_full, const void *in_full, const hr_gauge *links, void *stream)
 {
     if (!out_full || !in_full || !links) { set_error("hr_dirac: NULL argument"); return HR_EINVAL; }
-    if (!links->represented && dphi_link_kind(links->ctx, true) < 0) { set_error("hr_dirac: `links` must be a represented field"); return HR_EINVAL; }
+    if (dphi_link_kind(links->ctx, link_src(links)) < 0) { set_error("hr_dirac: `links` must be a represented field"); return HR_EINVAL; }
     if (out_full == in_full) { set_error("hr_dirac: out aliases in"); return HR_EINVAL; }
     if (((uintptr_t)out_full | (uintptr_t)in_full) & 15) { set_error("hr_dirac: spinor buffers must be 16-byte aligned"); return HR_EINVAL; }
     const hr_ctx *c = links->ctx;
@@ -410,7 +428,7 @@ hr_status hr_dirac(double m0, void *out_full, const void *in_full, const hr_gaug
         const char *i_self = (const char *)in_full + (size_t)p * half;
         const double mass[2] = { 4.0 + m0, 4.0 + m0 }, mhalf[2] = { -0.5, -0.5 };
         dphi_args(a, c, o, i_other, i_self, links, p, mass, mhalf);
-        rc = launch_dphi(c, links->prec, a, (cudaStream_t)stream, !links->represented);
+        rc = launch_dphi(c, links->prec, a, (cudaStream_t)stream, link_src(links));
         if (rc != HR_OK) return rc;
     }
     return HR_OK;

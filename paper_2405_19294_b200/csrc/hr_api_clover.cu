@@ -17,7 +17,7 @@ size_t hr_clover_bytes(const hr_ctx *ctx, hr_prec prec)
 hr_status hr_clover_build(void *clover, const hr_gauge *links, double csw, void *stream)
 {
     if (!clover || !links) { set_error("hr_clover_build: NULL argument"); return HR_EINVAL; }
-    if (!links->represented) { set_error("hr_clover_build: `links` must be a represented field (the leaves are products of U^R)"); return HR_EINVAL; }
+    if (links->represented != 1) { set_error("hr_clover_build: `links` must be a represented field (the leaves are products of U^R)"); return HR_EINVAL; }
     if (!aligned16(clover)) { set_error("hr_clover_build: buffer must be 16-byte aligned"); return HR_EINVAL; }
     hr_status rc = use_device(links->ctx);
     if (rc != HR_OK) return rc;

@@ -11,7 +11,7 @@ static hr_status check_links(const char *who, const hr_gauge *links, int parity)
 {
     if (!links) { set_error("%s: NULL links", who); return HR_EINVAL; }
     if (parity != 0 && parity != 1) { set_error("%s: parity=%d", who, parity); return HR_EINVAL; }
-    if (!links->represented && dphi_link_kind(links->ctx, true) < 0) {
+    if (dphi_link_kind(links->ctx, link_src(links)) < 0) {
         set_error("%s: `links` must be a represented field for this representation", who);
         return HR_EINVAL;
     }
@@ -56,7 +56,7 @@ hr_status hr_dphi_eo_halo_pack(void *send_up, void *send_dn, const void *in, con
     a.send_up = send_up;
     a.send_dn = send_dn;
     a.in = in;
-    return launch_halo(links->ctx, links->prec, true, a, (cudaStream_t)stream, !links->represented);
+    return launch_halo(links->ctx, links->prec, true, a, (cudaStream_t)stream, link_src(links));
 }
 
 hr_status hr_dphi_eo_interior(void *out, const void *in, const hr_gauge *links, int parity, void *stream)
@@ -69,7 +69,7 @@ hr_status hr_dphi_eo_interior(void *out, const void *in, const hr_gauge *links, 
     const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 };
     dphi_args(a, c, out, in, nullptr, links, parity, zero, mhalf);
     a.bc[0] = 0; // a hop across the slab boundary contributes nothing here: hr_dphi_eo_halo_apply adds it
-    return launch_dphi(c, links->prec, a, (cudaStream_t)stream, !links->represented);
+    return launch_dphi(c, links->prec, a, (cudaStream_t)stream, link_src(links));
 }
 
 hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *recv_next, const hr_gauge *links, int parity,
@@ -90,7 +90,7 @@ hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *re
     a.recv_next = recv_next;
     a.sign_prev = first_rank ? c->bc[0] : 1; // the global seam lies below rank 0's first slice ...
     a.sign_next = last_rank ? c->bc[0] : 1;  // ... and above the last rank's last slice (reading C9)
-    return launch_halo(c, links->prec, false, a, (cudaStream_t)stream, !links->represented);
+    return launch_halo(c, links->prec, false, a, (cudaStream_t)stream, link_src(links));
 }
 
 } // extern "C"

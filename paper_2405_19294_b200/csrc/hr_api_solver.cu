@@ -38,7 +38,7 @@ static hr_status dhat_launches(const hr_ctx *c, double m0, int g5, void *out_e, 
     DphiArgs a;
     dphi_args(a, c, tmp_o, in_e, nullptr, links, 1, zero, mhalf);
     a.skip = skip;
-    hr_status rc = launch_dphi(c, links->prec, a, st, !links->represented);
+    hr_status rc = launch_dphi(c, links->prec, a, st, link_src(links));
     if (rc != HR_OK) return rc;
     const double s = g5 ? -1.0 : 1.0;
     const double alpha[2] = { m * m, s * m * m }, beta[2] = { 0.5, s * 0.5 }; // -Dphi = +1/2 sum_hops
@@ -49,7 +49,7 @@ static hr_status dhat_launches(const hr_ctx *c, double m0, int g5, void *out_e, 
         a.red_ticket = rs->ticket;
         a.red_result = red_result;
     }
-    return launch_dphi(c, links->prec, a, st, !links->represented);
+    return launch_dphi(c, links->prec, a, st, link_src(links));
 }
 
 extern "C" {
@@ -124,7 +124,7 @@ hr_status hr_spinor_norm2(hr_ctx *ctx, hr_prec prec, const void *x, double *resu
 hr_status hr_dhat(double m0, int g5, void *out_e, const void *in_e, void *tmp_o, const hr_gauge *links, void *stream)
 {
     if (!out_e || !in_e || !tmp_o || !links) { set_error("hr_dhat: NULL argument"); return HR_EINVAL; }
-    if (!links->represented && dphi_link_kind(links->ctx, true) < 0) { set_error("hr_dhat: `links` must be a represented field"); return HR_EINVAL; }
+    if (dphi_link_kind(links->ctx, link_src(links)) < 0) { set_error("hr_dhat: `links` must be a represented field"); return HR_EINVAL; }
     if (out_e == in_e || out_e == tmp_o || in_e == tmp_o) { set_error("hr_dhat: out, in and tmp must be distinct buffers"); return HR_EINVAL; }
     if (!aligned16(out_e) || !aligned16(in_e) || !aligned16(tmp_o)) { set_error("hr_dhat: buffers must be 16-byte aligned"); return HR_EINVAL; }
     const hr_ctx *c = links->ctx;
@@ -237,7 +237,7 @@ static hr_status cg_check(const char *who, hr_ctx *ctx, const void *x, const voi
 {
     if (!ctx || !x || !b || !links || !ws) { set_error("%s: NULL argument", who); return HR_EINVAL; }
     if (links->ctx != ctx) { set_error("%s: `links` belongs to a different context", who); return HR_EINVAL; }
-    if (!links->represented && dphi_link_kind(ctx, true) < 0) { set_error("%s: `links` must be a represented field", who); return HR_EINVAL; }
+    if (dphi_link_kind(ctx, link_src(links)) < 0) { set_error("%s: `links` must be a represented field", who); return HR_EINVAL; }
     if (!(tol >= 0.0) || maxiter < 0) { set_error("%s: tol=%g maxiter=%d", who, tol, maxiter); return HR_EINVAL; }
     if (x == b) { set_error("%s: x aliases b", who); return HR_EINVAL; }
     if (!aligned16(x) || !aligned16(b) || ((uintptr_t)ws & 255)) { set_error("%s: buffers must be 16-byte (workspace 256-byte) aligned", who); return HR_EINVAL; }
@@ -347,7 +347,7 @@ hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_ful
     DphiArgs a;
     const double am[2] = { m, m }, half[2] = { 0.5, 0.5 };
     dphi_args(a, ctx, x_o, b_o, b_e, links, 0, am, half);
-    rc = launch_dphi(ctx, prec, a, st, !links->represented);
+    rc = launch_dphi(ctx, prec, a, st, link_src(links));
     if (rc != HR_OK) return rc;
     // rhs of the normal equations: r = Q gamma5 bhat
     const double one[2] = { 1.0, 0.0 }, zero[2] = { 0.0, 0.0 };
@@ -360,7 +360,7 @@ hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_ful
     // x_o = (b_o - Dphi_oe x_e) / m
     const double ainv[2] = { 1.0 / m, 1.0 / m }, binv[2] = { 0.5 / m, 0.5 / m };
     dphi_args(a, ctx, x_o, x_e, b_o, links, 1, ainv, binv);
-    return launch_dphi(ctx, prec, a, st, !links->represented);
+    return launch_dphi(ctx, prec, a, st, link_src(links));
 }
 
 } // extern "C"

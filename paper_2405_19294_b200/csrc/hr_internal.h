@@ -63,8 +63,11 @@ void dphi_args(DphiArgs &a, const hr_ctx *c, void *out, const void *in, const vo
                int parity, const double alpha[2], const double beta[2]);
 
 static inline size_t prec_bytes(hr_prec p) { return p == HR_F64 ? 8 : 4; }
+// link-field kinds (hr_gauge::represented): 0 fundamental N x N, 1 represented d_R x d_R, 2 fundamental stored as its
+// first N-1 rows (the last row of an SU(N) matrix is fixed by the others; N = 2, 3)
 static inline int link_nreal(const hr_ctx *c, int represented)
 {
+    if (represented == 2) return 2 * c->N * (c->N - 1);
     if (!represented) return 2 * c->N * c->N;
     return c->real_links ? c->d * c->d : 2 * c->d * c->d;
 }
@@ -116,9 +119,12 @@ struct RedScratch {
 hr_status get_red_scratch(hr_ctx *c, RedScratch *r, cudaStream_t st);
 
 // returns HR_OK / HR_EUNSUPPORTED / HR_ECUDA
-// fundamental_links: a.links is the FUNDAMENTAL field and the representation is applied on the fly (NEXT-3)
-hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st, bool fundamental_links = false);
-int dphi_link_kind(const hr_ctx *c, bool fundamental_links); // -1: no such kernel
+// link_src: what a.links holds -- 0 the represented field, 1 the FUNDAMENTAL field (representation applied on the fly,
+// NEXT-3), 2 the fundamental field stored as N-1 rows (last row and representation rebuilt in the kernel)
+hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st, int link_src = 0);
+int dphi_link_kind(const hr_ctx *c, int link_src); // -1: no such kernel
+static inline int link_src(const hr_gauge *g) { return g->represented == 1 ? 0 : g->represented == 0 ? 1 : 2; }
+hr_status launch_compress(const hr_ctx *c, hr_prec prec, void *rows, const void *fund, cudaStream_t st);
 const char *dphi_variant_name(const hr_ctx *c, hr_prec prec);
 bool dphi_variant_valid(const hr_ctx *c, int variant);
 
@@ -138,7 +144,7 @@ struct HaloArgs {
     float betaf[2];
     int sign_prev, sign_next; // seam signs of the two faces (+-1)
 };
-hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, const HaloArgs &a, cudaStream_t st, bool fundamental_links);
+hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, const HaloArgs &a, cudaStream_t st, int link_src);
 
 // clover term (clover.cu): record of 8 d_R^2 reals per site, [parity] fields
 size_t clover_nreal(const hr_ctx *c);

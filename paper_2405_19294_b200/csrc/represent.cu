@@ -149,6 +149,37 @@ static hr_status launch_rep(hr_prec ip, const void *fund, hr_prec op, void *repr
     return HR_OK;
 }
 
+// fundamental field -> its first N-1 rows (link kind LK_ROWS of dphi_kernel.cuh): a permutation copy, one thread per link
+template <int N, typename Real>
+__global__ void __launch_bounds__(128) compress_kernel(const char *__restrict__ fund, char *__restrict__ rows, long vh)
+{
+    constexpr int NIN = 2 * N * N, NOUT = 2 * N * (N - 1);
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= 8 * vh) return;
+    const long q = idx / vh, s = idx - q * vh;
+    Real u[NIN], o[NOUT];
+    load_record<LD_STREAM, NIN>(u, fund + (size_t)q * NIN * sizeof(Real) * vh, (size_t)vh, (size_t)s, 0);
+#pragma unroll
+    for (int e = 0; e < NOUT; ++e) o[e] = u[e];
+    store_record<NOUT>(rows + (size_t)q * NOUT * sizeof(Real) * vh, (size_t)vh, (size_t)s, o);
+}
+
+hr_status launch_compress(const hr_ctx *c, hr_prec prec, void *rows, const void *fund, cudaStream_t st)
+{
+    const unsigned grid = (unsigned)((8 * c->Vh + 127) / 128);
+    const char *f = (const char *)fund;
+    char *r = (char *)rows;
+    if (c->N == 2 && prec == HR_F64) compress_kernel<2, double><<<grid, 128, 0, st>>>(f, r, c->Vh);
+    else if (c->N == 2) compress_kernel<2, float><<<grid, 128, 0, st>>>(f, r, c->Vh);
+    else if (c->N == 3 && prec == HR_F64) compress_kernel<3, double><<<grid, 128, 0, st>>>(f, r, c->Vh);
+    else if (c->N == 3) compress_kernel<3, float><<<grid, 128, 0, st>>>(f, r, c->Vh);
+    else { set_error("row compression exists for SU(2) and SU(3) only"); return HR_EUNSUPPORTED; }
+    count_launch();
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) { set_error("compress kernel launch failed: %s", cudaGetErrorString(e)); return HR_ECUDA; }
+    return HR_OK;
+}
+
 hr_status launch_represent(const hr_ctx *c, hr_prec in_prec, const void *fund, hr_prec out_prec, void *repr, cudaStream_t st)
 {
 #define X(NN, RR) if (c->N == NN && c->rep == RR) return launch_rep<NN, RR>(in_prec, fund, out_prec, repr, c->Vh, st);
