@@ -102,3 +102,23 @@ def test_two_index_closed_form_su3():
                 n = (2 ** -0.5 if i == j else 1.0) * (2 ** -0.5 if k == l else 1.0)
                 want = n * (U[:, i, k] * U[:, j, l] + sign * U[:, i, l] * U[:, j, k])
                 assert np.abs(R[:, a, b] - want).max() < 1e-15
+
+
+def test_last_row_of_a_special_unitary_matrix_is_fixed_by_the_others():
+    """Reading C30 (row-compressed links): for U in SU(3) the third row is conj(row0 x row1), for U in SU(2) the second
+    row is (-conj u01, conj u00); and the SU(2) adjoint link is a function of the first row alone,
+    R_ab = (a0^2 - a.a) delta_ab + 2 a_a a_b + 2 a0 eps_abc a_c with (a0, a3, a2, a1) = (Re u00, Im u00, Re u01, Im u01).
+    Checked on the seeded generator's links against the oracle's trace definition."""
+    U3 = li.haar_links(71, 3, (2, 2, 2, 2)).reshape(-1, 3, 3)
+    assert np.abs(np.conj(np.cross(U3[:, 0], U3[:, 1])) - U3[:, 2]).max() < 1e-14
+    U2 = li.haar_links(72, 2, (2, 2, 2, 2)).reshape(-1, 2, 2)
+    assert np.abs(U2[:, 1, 0] + np.conj(U2[:, 0, 1])).max() < 1e-14 and np.abs(U2[:, 1, 1] - np.conj(U2[:, 0, 0])).max() < 1e-14
+    R = oracle.represent(2, oracle.REP_ADJ, U2).real
+    a0, a3, a2, a1 = U2[:, 0, 0].real, U2[:, 0, 0].imag, U2[:, 0, 1].real, U2[:, 0, 1].imag
+    a = np.stack([a1, a2, a3], axis=-1)
+    eps = np.zeros((3, 3, 3))
+    eps[0, 1, 2] = eps[1, 2, 0] = eps[2, 0, 1] = 1
+    eps[0, 2, 1] = eps[2, 1, 0] = eps[1, 0, 2] = -1
+    want = (a0 ** 2 - np.sum(a * a, -1))[:, None, None] * np.eye(3) + 2 * a[:, :, None] * a[:, None, :] \
+        + 2 * a0[:, None, None] * np.einsum("abc,xc->xab", eps, a)
+    assert np.abs(R - want).max() < 1e-14
