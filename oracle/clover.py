@@ -81,3 +81,24 @@ def dirac_clover(dims, bc, links_R, m0, csw, psi_eo):
     T = clover_term(dims, links_R, csw)
     tpsi = lex_to_eo(dims, apply_clover_lex(T, eo_to_lex(dims, psi_eo)))
     return dirac(dims, bc, links_R, m0, psi_eo) + tpsi
+
+
+# ---- exponentiated clover ("exponentiated clover improvement [8]"; reading C31) -----------------------
+def exp_clover_term(dims, links_R, m0, csw):
+    """Reading C31: the site-diagonal part (4+m0) + T(x) of D_sw is replaced by (4+m0) exp(T(x) / (4+m0)), which is
+    positive definite for every gauge field.  Returned is E(x) = (4+m0) [exp(T(x)/(4+m0)) - 1] as [V, 4, d, 4, d], so
+    that D_exp = D + E; computed from the Hermitian eigendecomposition of the dense 4d x 4d matrix of every site."""
+    m = 4.0 + m0
+    T = clover_term(dims, links_R, csw)
+    V, d = T.shape[0], T.shape[2]
+    Tm = T.reshape(V, 4 * d, 4 * d)
+    w, Q = np.linalg.eigh(Tm)
+    E = (Q * (m * np.expm1(w / m))[:, None, :]) @ np.conj(np.swapaxes(Q, -1, -2))
+    return E.reshape(V, 4, d, 4, d)
+
+
+def dirac_expclover(dims, bc, links_R, m0, csw, psi_eo):
+    """D_exp on a full field [even half | odd half]: Dphi psi + (4+m0) exp(T/(4+m0)) psi."""
+    E = exp_clover_term(dims, links_R, m0, csw)
+    epsi = lex_to_eo(dims, apply_clover_lex(E, eo_to_lex(dims, psi_eo)))
+    return dirac(dims, bc, links_R, m0, psi_eo) + epsi

@@ -126,3 +126,59 @@ def test_dirac_clover_is_gamma5_hermitian_and_reduces_to_dirac():
     got = clover.dirac_clover(dims, BC_T, R, m0, csw, psi)
     assert np.linalg.norm(got - want) <= 1e-13 * np.linalg.norm(want)
     assert np.array_equal(clover.dirac_clover(dims, BC_T, R, m0, 0.0, psi), oracle.dirac(dims, BC_T, R, m0, psi))
+
+
+# ------------------------------------------------------------------------------------------ exponentiated clover
+def test_exp_clover_equals_its_power_series_and_is_positive():
+    dims = (4, 2, 2, 4)
+    U = li.haar_links(12, 3, dims)
+    V, d = li.volume(dims), 3
+    m0, csw = -0.5, 1.5
+    m = 4 + m0
+    T = clover.clover_term(dims, U, csw).reshape(V, 4 * d, 4 * d)
+    E = clover.exp_clover_term(dims, U, m0, csw).reshape(V, 4 * d, 4 * d)
+    series = np.zeros_like(T)
+    term = np.broadcast_to(np.eye(4 * d, dtype=complex), T.shape).copy()
+    for k in range(1, 40):                          # m (exp(T/m) - 1) = sum_{k>=1} T^k / (k! m^(k-1))
+        term = term @ T / (k * m)
+        series = series + m * term
+    assert np.abs(E - series).max() < 1e-12
+    assert np.abs(E - np.conj(np.swapaxes(E, -1, -2))).max() < 1e-13
+    g5 = np.kron(np.diag([1, 1, -1, -1]), np.eye(d))
+    assert np.abs(E @ g5 - g5 @ E).max() < 1e-13
+    assert np.abs(E[:, :2 * d, 2 * d:]).max() < 1e-13
+    # the whole point of the exponential: the diagonal term m + E = m exp(T/m) is positive definite, while m + T need not be
+    assert np.linalg.eigvalsh(m * np.eye(4 * d) + E).min() > 0
+    # small c_sw: E = T + T^2 / (2m) + O(c_sw^3)
+    eps = 1e-3
+    Ts = clover.clover_term(dims, U, eps).reshape(V, 4 * d, 4 * d)
+    Es = clover.exp_clover_term(dims, U, m0, eps).reshape(V, 4 * d, 4 * d)
+    fro = np.linalg.norm(Ts, axis=(1, 2)).max()                      # the remainder is T^3/(6 m^2) + ...: third order
+    assert np.abs(Es - Ts - Ts @ Ts / (2 * m)).max() <= 1.05 * fro ** 3 / (6 * m * m)
+    assert np.abs(Es - Ts).max() > 10 * fro ** 3                       # ... and the second-order term is really there
+
+
+def test_exp_clover_closed_form_on_the_constant_abelian_field():
+    """T = -(c/2) sigma_01 sin(B q): sigma^2 = 1, so exp(t sigma) = cosh t + sigma sinh t."""
+    dims = (8, 4, 2, 2)
+    V = li.volume(dims)
+    x = _coords(dims)
+    q = np.array([1.0, -2.0, 3.0])
+    B = 2 * np.pi / dims[0]
+    U = np.broadcast_to(np.eye(3, dtype=complex), (V, 4, 3, 3)).copy()
+    U[:, 1] = np.exp(1j * B * x[:, 0, None] * q[None, :])[:, :, None] * np.eye(3)
+    m0, csw = 0.2, 1.1
+    m = 4 + m0
+    E = clover.exp_clover_term(dims, U, m0, csw)
+    t = -0.5 * csw * np.sin(B * q) / m
+    s = clover.sigma(0, 1)
+    want = m * (np.einsum("st,ab->satb", np.eye(4), np.diag(np.cosh(t) - 1)) + np.einsum("st,ab->satb", s, np.diag(np.sinh(t))))
+    assert np.abs(E - want[None]).max() < 1e-13
+
+
+def test_dirac_expclover_reduces_to_dirac_without_field_strength():
+    dims = (2, 2, 2, 4)
+    V = li.volume(dims)
+    one = np.broadcast_to(np.eye(2, dtype=complex), (V, 4, 2, 2)).copy()
+    psi = li.gaussian_spinor(13, V, 2)
+    assert np.allclose(clover.dirac_expclover(dims, BC_T, one, -0.1, 1.3, psi), oracle.dirac(dims, BC_T, one, -0.1, psi), atol=1e-14)
