@@ -265,8 +265,13 @@ hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *re
  *     (the chiral basis makes sigma block diagonal), [even sites | odd sites].
  * hr_dirac_clover: out = (4+m0) in + Dphi in + T in on full fields [even half | odd half]; the two hr_dirac launches
  *     followed by one site-local launch per parity.  out != in.
- * ===================================================================================================== */
+ * hr_clover_exp: the exponentiated clover term ("exponentiated clover improvement [8]"; reading C31: the
+ *     site-diagonal part (4+m0) + T of D_sw becomes (4+m0) exp(T/(4+m0)), positive definite on every gauge field).
+ *     Replaces, IN PLACE, the T written by hr_clover_build by E = (4+m0)[exp(T/(4+m0)) - 1]; hr_dirac_clover with the
+ *     same m0 then applies D_exp = Dphi + (4+m0) exp(T/(4+m0)).  One launch over the 2V blocks; 4 + m0 > 0.
+ */
 size_t hr_clover_bytes(const hr_ctx *ctx, hr_prec prec);
+hr_status hr_clover_exp(const hr_ctx *ctx, hr_prec prec, void *clover, double m0, void *stream);
 hr_status hr_clover_build(void *clover, const hr_gauge *links, double csw, void *stream);
 hr_status hr_dirac_clover(double m0, void *out_full, const void *in_full, const hr_gauge *links, const void *clover,
                           void *stream);

@@ -89,6 +89,7 @@ _SIGNATURES = {
     "hr_dphi_eo_halo_apply": (_ci, [_vp, _vp, _vp, _vp, _ci, _ci, _ci, _vp]),
     "hr_clover_bytes": (_sz, [_vp, _ci]),
     "hr_clover_build": (_ci, [_vp, _vp, _cd, _vp]),
+    "hr_clover_exp": (_ci, [_vp, _ci, _vp, _cd, _vp]),
     "hr_dirac_clover": (_ci, [_cd, _vp, _vp, _vp, _vp, _vp]),
     "hr_ctx_set_tuning": (_ci, [_vp, ctypes.c_char_p, _ci]),
     "hr_dphi_variant_name": (ctypes.c_char_p, [_vp, _ci]),
@@ -338,6 +339,10 @@ def hr_clover_bytes(ctx: int, prec: int) -> int:
 
 def hr_clover_build(clover, links: int, csw: float, stream: int = 0) -> None:
     _check(_lib.hr_clover_build(_ptr(clover), links, float(csw), stream))
+
+
+def hr_clover_exp(ctx: int, prec: int, clover, m0: float, stream: int = 0) -> None:
+    _check(_lib.hr_clover_exp(ctx, prec, _ptr(clover), float(m0), stream))
 
 
 def hr_dirac_clover(m0: float, out_full, in_full, links: int, clover, stream: int = 0) -> None:

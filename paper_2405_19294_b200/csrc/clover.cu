@@ -217,6 +217,69 @@ __global__ void __launch_bounds__(128) clover_apply_kernel(const CloverArgs a)
     store_planes<ST_DEFAULT, NVH>((char *)a.out + (size_t)s * 16 + (size_t)(b * NVH) * pb, pb, w);
 }
 
+// In-place  T -> E = m [exp(T/m) - 1]  on the packed Hermitian blocks (reading C31: exponentiated clover).
+// One thread per (site, chirality block): the n x n block (n = 2 d_R <= 16) is unpacked to a dense complex matrix,
+// X = T / (m 2^6) is exponentiated by a 10-term Taylor series of expm1 (|X| < 0.1: remainder < 1e-22) and the result
+// is squared six times in the expm1 form  e(2X) = e(X)^2 + 2 e(X)  (no cancellation against the identity), then
+// packed back.  Set-up kernel: runtime loops over local arrays.
+template <typename Real, int D>
+__global__ void __launch_bounds__(64) clover_exp_kernel(char *clover, long vh, double m)
+{
+    constexpr int N2 = 2 * D, M = 2 * N2 * N2, BLK = 4 * D * D, RPV = 16 / (int)sizeof(Real), NVB = BLK / RPV;
+    const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x; // over 2 parities x vh sites x 2 blocks
+    if (tid >= 4 * vh) return;
+    const int b = (int)(tid & 1);
+    const long site = tid >> 1;                                    // 0 .. 2 vh
+    const long par = site / vh, s = site - par * vh;
+    char *rec = clover + (size_t)par * 2 * BLK * sizeof(Real) * (size_t)vh + (size_t)s * 16 + (size_t)(b * NVB) * (size_t)vh * 16;
+    const size_t pb = (size_t)vh * 16;
+    Real t[BLK];
+    load_planes<LD_DEFAULT, NVB>(t, rec, pb, 0);
+    double x[M], e[M], p[M], q[M];
+    const double sc = 1.0 / (m * 64.0);
+    for (int i = 0; i < M; ++i) x[i] = 0;
+    {
+        int w = 0;
+        for (int d = 0; d < N2; ++d) x[2 * (d * N2 + d)] = (double)t[w++] * sc;
+        for (int r = 0; r < N2; ++r)
+            for (int c = r + 1; c < N2; ++c) {
+                const double re = (double)t[w++] * sc, im = (double)t[w++] * sc;
+                x[2 * (r * N2 + c)] = re; x[2 * (r * N2 + c) + 1] = im;
+                x[2 * (c * N2 + r)] = re; x[2 * (c * N2 + r) + 1] = -im;
+            }
+    }
+    auto mul = [&](double *o, const double *a, const double *bb) {   // o = a bb (dense complex N2 x N2)
+        for (int i = 0; i < N2; ++i)
+            for (int j = 0; j < N2; ++j) {
+                double re = 0, im = 0;
+                for (int k = 0; k < N2; ++k) {
+                    const double ar = a[2 * (i * N2 + k)], ai = a[2 * (i * N2 + k) + 1];
+                    const double br = bb[2 * (k * N2 + j)], bi = bb[2 * (k * N2 + j) + 1];
+                    re += ar * br - ai * bi;
+                    im += ar * bi + ai * br;
+                }
+                o[2 * (i * N2 + j)] = re; o[2 * (i * N2 + j) + 1] = im;
+            }
+    };
+    // e = expm1(X) = X + X^2/2! + ... + X^10/10!
+    for (int i = 0; i < M; ++i) { e[i] = x[i]; p[i] = x[i]; }
+    for (int k = 2; k <= 10; ++k) {
+        mul(q, p, x);
+        for (int i = 0; i < M; ++i) { p[i] = q[i] / k; e[i] += p[i]; }
+    }
+    for (int sq = 0; sq < 6; ++sq) {                                  // expm1(2X) = expm1(X)^2 + 2 expm1(X)
+        mul(q, e, e);
+        for (int i = 0; i < M; ++i) e[i] = q[i] + 2.0 * e[i];
+    }
+    {
+        int w = 0;
+        for (int d = 0; d < N2; ++d) t[w++] = (Real)(m * e[2 * (d * N2 + d)]);
+        for (int r = 0; r < N2; ++r)
+            for (int c = r + 1; c < N2; ++c) { t[w++] = (Real)(m * e[2 * (r * N2 + c)]); t[w++] = (Real)(m * e[2 * (r * N2 + c) + 1]); }
+    }
+    store_planes<ST_DEFAULT, NVB>(rec, pb, t);
+}
+
 static hr_status launched(const char *what)
 {
     count_launch();
@@ -245,6 +308,21 @@ hr_status launch_clover_build(const hr_ctx *c, hr_prec prec, void *clover, const
         return launched("clover_build_kernel");                                                                       \
     }
     X(2, false) X(3, false) X(4, false) X(6, false) X(3, true) X(8, true)
+#undef X
+    set_error("no clover kernel compiled for d_R=%d", c->d);
+    return HR_EUNSUPPORTED;
+}
+
+hr_status launch_clover_exp(const hr_ctx *c, hr_prec prec, void *clover, double m, cudaStream_t st)
+{
+    const unsigned grid = (unsigned)((4 * c->Vh + 63) / 64);
+#define X(D)                                                                                                          \
+    if (c->d == D) {                                                                                                  \
+        if (prec == HR_F64) clover_exp_kernel<double, D><<<grid, 64, 0, st>>>((char *)clover, c->Vh, m);             \
+        else clover_exp_kernel<float, D><<<grid, 64, 0, st>>>((char *)clover, c->Vh, m);                             \
+        return launched("clover_exp_kernel");                                                                         \
+    }
+    X(2) X(3) X(4) X(6) X(8)
 #undef X
     set_error("no clover kernel compiled for d_R=%d", c->d);
     return HR_EUNSUPPORTED;

@@ -24,6 +24,16 @@ hr_status hr_clover_build(void *clover, const hr_gauge *links, double csw, void 
     return launch_clover_build(links->ctx, links->prec, clover, links->data, csw, (cudaStream_t)stream);
 }
 
+hr_status hr_clover_exp(const hr_ctx *ctx, hr_prec prec, void *clover, double m0, void *stream)
+{
+    if (!ctx || !clover || (prec != HR_F64 && prec != HR_F32)) { set_error("hr_clover_exp: bad argument"); return HR_EINVAL; }
+    if (!aligned16(clover)) { set_error("hr_clover_exp: buffer must be 16-byte aligned"); return HR_EINVAL; }
+    if (!(4.0 + m0 > 0.0)) { set_error("hr_clover_exp: 4 + m0 = %g must be positive", 4.0 + m0); return HR_EINVAL; }
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    return launch_clover_exp(ctx, prec, clover, 4.0 + m0, (cudaStream_t)stream);
+}
+
 hr_status hr_dirac_clover(double m0, void *out_full, const void *in_full, const hr_gauge *links, const void *clover, void *stream)
 {
     if (!out_full || !in_full || !links || !clover) { set_error("hr_dirac_clover: NULL argument"); return HR_EINVAL; }

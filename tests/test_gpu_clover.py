@@ -138,3 +138,42 @@ def test_clover_on_a_131072_site_lattice(hr, prec):
     want = clover.dirac_clover(dims, BC_T, U, -0.2, 1.0, psi)
     assert rel_l2(got, want) <= TOL[prec]
     prob.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("N,rep", [(2, "fund"), (3, "fund"), (2, "adj"), (3, "sym"), (3, "adj")])
+def test_dirac_expclover_matches_oracle(hr, N, rep, prec):
+    """PAPER.md:70 "exponentiated clover"; reading C31: hr_clover_build + hr_clover_exp + hr_dirac_clover = D_exp."""
+    import torch
+    dims = (4, 4, 2, 6)
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(411, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    V = li.volume(dims)
+    psi = li.gaussian_spinor(412, V, d)
+    m0, csw = -0.6, 1.7
+    prob = GpuProblem(hr, dims, N, rep, prec, U)
+    lat, P = prob.lat, prob.prec
+    cl = torch.empty(hr.hr_clover_bytes(lat.ctx, P), dtype=torch.uint8, device="cuda")
+    hr.hr_clover_build(cl, prob.links, csw, lat.stream())
+    n0 = hr.hr_launch_count()
+    hr.hr_clover_exp(lat.ctx, P, cl, m0, lat.stream())
+    assert hr.hr_launch_count() == n0 + 1
+    gin = _full(prob, psi)
+    gout, gref = lat.spinor(P, full=True), lat.spinor(P, full=True)
+    hr.hr_dirac_clover(m0, gout, gin, prob.links, cl, lat.stream())
+    got = _get_full(prob, gout)
+    want = clover.dirac_expclover(dims, BC_T, R, m0, csw, psi)
+    assert rel_l2(got, want) <= TOL[prec]
+    # the exponential part alone, E psi = (D_exp - D) psi, and that it differs from the plain clover term at second order
+    lat.dirac(m0, gref, gin, prob.links)
+    epsi = got - _get_full(prob, gref)
+    E = clover.exp_clover_term(dims, R, m0, csw)
+    want_e = oracle.lex_to_eo(dims, clover.apply_clover_lex(E, oracle.eo_to_lex(dims, psi)))
+    assert np.linalg.norm(epsi - want_e) <= 20 * TOL[prec] * np.linalg.norm(want)
+    T = clover.clover_term(dims, R, csw)
+    want_t = oracle.lex_to_eo(dims, clover.apply_clover_lex(T, oracle.eo_to_lex(dims, psi)))
+    assert np.linalg.norm(epsi - want_t) > 1e-3 * np.linalg.norm(want_t)
+    with pytest.raises(hr.HrError):
+        hr.hr_clover_exp(lat.ctx, P, cl, -4.5, lat.stream())            # 4 + m0 <= 0
+    prob.close()
