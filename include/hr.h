@@ -225,6 +225,10 @@ hr_status hr_cg_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const h
                      void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
 hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links, double tol,
                          int maxiter, void *workspace, int *iters, double *rel_res2, void *stream);
+/* The same full solve with hr_bicgstab_dhat as the inner solver (workspace of hr_bicgstab_workspace_bytes();
+ * tol and rel_res2 refer to the preconditioned system Dhat x_e = (4+m0) b_e - Dphi_eo b_o). */
+hr_status hr_dirac_solve_bicgstab(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links,
+                                  double tol, int maxiter, void *workspace, int *iters, double *rel_res2, void *stream);
 
 /* =====================================================================================================
  * Third part -- SURVEY.md section 8(e)/(f) NEXT-2: the lattice split into slabs along t, one slab per GPU,

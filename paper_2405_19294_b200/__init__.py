@@ -91,6 +91,7 @@ _SIGNATURES = {
     "hr_clover_build": (_ci, [_vp, _vp, _cd, _vp]),
     "hr_clover_exp": (_ci, [_vp, _ci, _vp, _cd, _vp]),
     "hr_dirac_clover": (_ci, [_cd, _vp, _vp, _vp, _vp, _vp]),
+    "hr_dirac_solve_bicgstab": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
     "hr_ctx_set_tuning": (_ci, [_vp, ctypes.c_char_p, _ci]),
     "hr_dphi_variant_name": (ctypes.c_char_p, [_vp, _ci]),
     "hr_launch_count": (ctypes.c_ulonglong, []),
@@ -347,6 +348,14 @@ def hr_clover_exp(ctx: int, prec: int, clover, m0: float, stream: int = 0) -> No
 
 def hr_dirac_clover(m0: float, out_full, in_full, links: int, clover, stream: int = 0) -> None:
     _check(_lib.hr_dirac_clover(float(m0), _ptr(out_full), _ptr(in_full), links, _ptr(clover), stream))
+
+
+def hr_dirac_solve_bicgstab(ctx: int, m0: float, x_full, b_full, links: int, tol: float, maxiter: int, workspace, stream: int = 0):
+    """Returns (iterations, |r|^2/|bhat|^2 of the preconditioned system)."""
+    it, res = _ci(0), _cd(0.0)
+    _check(_lib.hr_dirac_solve_bicgstab(ctx, float(m0), _ptr(x_full), _ptr(b_full), links, float(tol), int(maxiter),
+                                        _ptr(workspace), ctypes.byref(it), ctypes.byref(res), stream))
+    return it.value, res.value
 
 
 def hr_ctx_set_tuning(ctx: int, key: str, value: int) -> None:

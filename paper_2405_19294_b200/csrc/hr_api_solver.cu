@@ -363,4 +363,28 @@ hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_ful
     return launch_dphi(ctx, prec, a, st, link_src(links));
 }
 
+hr_status hr_dirac_solve_bicgstab(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links, double tol,
+                                  int maxiter, void *workspace, int *iters, double *rel_res2, void *stream)
+{
+    hr_status rc = cg_check("hr_dirac_solve_bicgstab", ctx, x_full, b_full, links, tol, maxiter, workspace);
+    if (rc != HR_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const hr_prec prec = links->prec;
+    const size_t sb = (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec);
+    const double m = 4.0 + m0;
+    char *x_e = (char *)x_full, *x_o = (char *)x_full + sb;
+    const char *b_e = (const char *)b_full, *b_o = (const char *)b_full + sb;
+    // reading C24:  bhat = m b_e - Dphi_eo b_o  (kept in the x_o slot until the end); BiCGstab on Dhat x_e = bhat
+    DphiArgs a;
+    const double am[2] = { m, m }, half[2] = { 0.5, 0.5 };
+    dphi_args(a, ctx, x_o, b_o, b_e, links, 0, am, half);
+    rc = launch_dphi(ctx, prec, a, st, link_src(links));
+    if (rc != HR_OK) return rc;
+    rc = hr_bicgstab_dhat(ctx, m0, x_e, x_o, links, tol, maxiter, workspace, iters, rel_res2, nullptr, stream);
+    if (rc != HR_OK) return rc;
+    const double ainv[2] = { 1.0 / m, 1.0 / m }, binv[2] = { 0.5 / m, 0.5 / m };
+    dphi_args(a, ctx, x_o, x_e, b_o, links, 1, ainv, binv);
+    return launch_dphi(ctx, prec, a, st, link_src(links));
+}
+
 } // extern "C"

@@ -368,3 +368,27 @@ def test_bicgstab_fp32_and_edge_cases(hr):
     with pytest.raises(hr.HrError):
         hr.hr_bicgstab_dhat(ctx, m0, gb, gb, prob.links, 1e-5, 10, ws, st)
     prob.close()
+
+
+@pytest.mark.parametrize("dims,N,rep,m0", CG_CASES)
+def test_dirac_solve_bicgstab_inverts_the_oracles_dirac_operator(hr, dims, N, rep, m0):
+    import torch
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(131, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    V = li.volume(dims)
+    b = li.gaussian_spinor(132, V, d)
+    x_want, _ = solver.dirac_solve(dims, BC_T, R, m0, b, 1e-11, 1000)
+    prob = GpuProblem(hr, dims, N, rep, "f64", U)
+    lat, P = prob.lat, prob.prec
+    half = hr.hr_spinor_bytes(lat.ctx, P)
+    gb, gx = lat.spinor(P, full=True), lat.spinor(P, full=True)
+    for p in (0, 1):
+        lat.import_spinor(gb[p * half:(p + 1) * half], P, b[p * (V // 2):(p + 1) * (V // 2)], p)
+    ws = torch.empty(hr.hr_bicgstab_workspace_bytes(lat.ctx, P, 500), dtype=torch.uint8, device="cuda")
+    it, res2 = hr.hr_dirac_solve_bicgstab(lat.ctx, m0, gx, gb, prob.links, 1e-11, 500, ws, lat.stream())
+    assert 0 < it < 500 and res2 <= 1e-22
+    x = np.concatenate([lat.export_spinor(gx[p * half:(p + 1) * half], P, p) for p in (0, 1)])
+    assert rel_l2(x, x_want) <= 1e-9
+    assert rel_l2(oracle.dirac(dims, BC_T, R, m0, x), b) <= 1e-9
+    prob.close()
