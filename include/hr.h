@@ -225,6 +225,19 @@ hr_status hr_cg_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const h
                      void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
 hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links, double tol,
                          int maxiter, void *workspace, int *iters, double *rel_res2, void *stream);
+/*
+ * hr_bicgstab_dhat_mixed -- mixed precision (the operator exists "in single and double precision"): defect
+ * correction x += e, Dhat e = r, with the defect equation solved by hr_bicgstab_dhat in fp32 (links32, to inner_tol on
+ * the normalised residual) and the TRUE residual r = b - Dhat x recomputed in fp64 (links64) after every inner solve; stops
+ * when |r|^2 <= tol^2 |b|^2 (fp64, true residual) or after maxiter inner iterations in total.  x_e, b_e: fp64 half
+ * fields; workspace of hr_mixed_workspace_bytes(ctx, maxiter), 256-byte aligned.  iters: inner iterations in total,
+ * outer_steps: number of defect corrections, rel_res2: true |r|^2 / |b|^2.  Synchronises once per outer step.
+ */
+size_t hr_mixed_workspace_bytes(const hr_ctx *ctx, int maxiter);
+hr_status hr_bicgstab_dhat_mixed(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links64,
+                                 const hr_gauge *links32, double tol, double inner_tol, int maxiter, void *workspace,
+                                 int *iters, int *outer_steps, double *rel_res2, void *stream);
+
 /* The same full solve with hr_bicgstab_dhat as the inner solver (workspace of hr_bicgstab_workspace_bytes();
  * tol and rel_res2 refer to the preconditioned system Dhat x_e = (4+m0) b_e - Dphi_eo b_o). */
 hr_status hr_dirac_solve_bicgstab(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links,

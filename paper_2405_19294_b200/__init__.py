@@ -92,6 +92,8 @@ _SIGNATURES = {
     "hr_clover_exp": (_ci, [_vp, _ci, _vp, _cd, _vp]),
     "hr_dirac_clover": (_ci, [_cd, _vp, _vp, _vp, _vp, _vp]),
     "hr_dirac_solve_bicgstab": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
+    "hr_mixed_workspace_bytes": (_sz, [_vp, _ci]),
+    "hr_bicgstab_dhat_mixed": (_ci, [_vp, _cd, _vp, _vp, _vp, _vp, _cd, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
     "hr_ctx_set_tuning": (_ci, [_vp, ctypes.c_char_p, _ci]),
     "hr_dphi_variant_name": (ctypes.c_char_p, [_vp, _ci]),
     "hr_launch_count": (ctypes.c_ulonglong, []),
@@ -356,6 +358,19 @@ def hr_dirac_solve_bicgstab(ctx: int, m0: float, x_full, b_full, links: int, tol
     _check(_lib.hr_dirac_solve_bicgstab(ctx, float(m0), _ptr(x_full), _ptr(b_full), links, float(tol), int(maxiter),
                                         _ptr(workspace), ctypes.byref(it), ctypes.byref(res), stream))
     return it.value, res.value
+
+
+def hr_mixed_workspace_bytes(ctx: int, maxiter: int) -> int:
+    return _lib.hr_mixed_workspace_bytes(ctx, maxiter)
+
+
+def hr_bicgstab_dhat_mixed(ctx: int, m0: float, x_e, b_e, links64: int, links32: int, tol: float, inner_tol: float, maxiter: int,
+                           workspace, stream: int = 0):
+    """Returns (inner iterations in total, outer steps, true |r|^2/|b|^2)."""
+    it, outer, res = _ci(0), _ci(0), _cd(0.0)
+    _check(_lib.hr_bicgstab_dhat_mixed(ctx, float(m0), _ptr(x_e), _ptr(b_e), links64, links32, float(tol), float(inner_tol),
+                                       int(maxiter), _ptr(workspace), ctypes.byref(it), ctypes.byref(outer), ctypes.byref(res), stream))
+    return it.value, outer.value, res.value
 
 
 def hr_ctx_set_tuning(ctx: int, key: str, value: int) -> None:

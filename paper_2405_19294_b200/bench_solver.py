@@ -169,6 +169,19 @@ def main():
         e1.record()
         torch.cuda.synchronize()
         print(json.dumps(dict(common, op=name, tol=tol, iterations=it, rel_res2=res2, ms=e0.elapsed_time(e1), bytes_per_site=0, gbs=0.0, frac=0.0)))
+    if args.prec == "f64":
+        # mixed precision: fp32 inner BiCGstab (to 1e-4) + fp64 true residual, same right-hand side and target
+        l32 = lat.gauge(True, hr.HR_F32)
+        lat.represent_links(l32, fund)
+        wsm = torch.empty(hr.hr_mixed_workspace_bytes(ctx, 2000), dtype=torch.uint8, device="cuda")
+        hr.hr_bicgstab_dhat_mixed(ctx, args.m0, x, sets[0][0], links, l32, tol, 1e-4, 2000, wsm, st)
+        torch.cuda.synchronize()
+        e0.record()
+        it, outer, res2 = hr.hr_bicgstab_dhat_mixed(ctx, args.m0, x, sets[0][0], links, l32, tol, 1e-4, 2000, wsm, st)
+        e1.record()
+        torch.cuda.synchronize()
+        print(json.dumps(dict(common, op="mixed_bicgstab_solve", tol=tol, iterations=it, outer_steps=outer, rel_res2=res2,
+                              ms=e0.elapsed_time(e1), bytes_per_site=0, gbs=0.0, frac=0.0)))
     lat.close()
 
 

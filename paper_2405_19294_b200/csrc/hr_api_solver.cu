@@ -2,6 +2,7 @@
 // second part): spinor linear algebra, the even-odd preconditioned operator Dhat, and the CG / full solve
 // built on them.  Argument checking and launch sequencing only; the arithmetic is in linalg.cu, cg.cu and
 // the Dphi kernels.  No CPU fallback.
+#include <cmath>
 #include <cstring>
 
 #include "hr_internal.h"
@@ -385,6 +386,70 @@ hr_status hr_dirac_solve_bicgstab(hr_ctx *ctx, double m0, void *x_full, const vo
     const double ainv[2] = { 1.0 / m, 1.0 / m }, binv[2] = { 0.5 / m, 0.5 / m };
     dphi_args(a, ctx, x_o, x_e, b_o, links, 1, ainv, binv);
     return launch_dphi(ctx, prec, a, st, link_src(links));
+}
+
+size_t hr_mixed_workspace_bytes(const hr_ctx *ctx, int maxiter)
+{
+    if (!ctx || maxiter < 0) return 0;
+    const size_t s64 = (size_t)ctx->Vh * 8 * ctx->d * 8, s32 = s64 / 2;
+    return 3 * s64 + 2 * s32 + hr_bicgstab_workspace_bytes(ctx, HR_F32, maxiter);
+}
+
+hr_status hr_bicgstab_dhat_mixed(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links64,
+                                 const hr_gauge *links32, double tol, double inner_tol, int maxiter, void *workspace,
+                                 int *iters, int *outer_steps, double *rel_res2, void *stream)
+{
+    hr_status rc = cg_check("hr_bicgstab_dhat_mixed", ctx, x_e, b_e, links64, tol, maxiter, workspace);
+    if (rc != HR_OK) return rc;
+    if (!links32 || links32->ctx != ctx || links64->prec != HR_F64 || links32->prec != HR_F32 ||
+        dphi_link_kind(ctx, link_src(links32)) < 0 || !(inner_tol > 0.0 && inner_tol < 1.0)) {
+        set_error("hr_bicgstab_dhat_mixed: need an fp64 and an fp32 link field of this context and 0 < inner_tol < 1");
+        return HR_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    char *ws = (char *)workspace;
+    const size_t s64 = (size_t)ctx->Vh * 8 * ctx->d * 8, s32 = s64 / 2;
+    void *r = ws, *ax = ws + s64, *tmp = ws + 2 * s64, *r32 = ws + 3 * s64, *e32 = ws + 3 * s64 + s32;
+    void *inner_ws = ws + 3 * s64 + 2 * s32;
+    const double one[2] = { 1.0, 0.0 }, zero[2] = { 0.0, 0.0 }, mone[2] = { -1.0, 0.0 };
+    RedScratch rs;
+    rc = get_red_scratch(ctx, &rs, st);
+    if (rc != HR_OK) return rc;
+    // x = 0, r = b
+    rc = launch_lincomb(ctx, HR_F64, x_e, zero, 0, b_e, zero, nullptr, st);
+    if (rc != HR_OK) return rc;
+    rc = launch_lincomb(ctx, HR_F64, r, one, 0, b_e, zero, nullptr, st);
+    if (rc != HR_OK) return rc;
+    double bb = -1.0, rr = 0.0;
+    int total = 0, outer = 0;
+    for (;;) {
+        rc = launch_dot(ctx, HR_F64, r, r, rs, rs.result, st);
+        if (rc != HR_OK) return rc;
+        HR_CUDA(cudaMemcpyAsync(&rr, rs.result, sizeof(double), cudaMemcpyDeviceToHost, st));
+        HR_CUDA(cudaStreamSynchronize(st));
+        if (bb < 0) bb = rr;
+        if (!(rr > tol * tol * bb) || total >= maxiter || outer >= 100) break;
+        // defect equation Dhat e = r, solved in fp32 on the normalised residual
+        const double nrm = sqrt(rr);
+        rc = launch_cvt(ctx, true, r32, r, 1.0 / nrm, st);
+        if (rc != HR_OK) return rc;
+        int it = 0;
+        rc = hr_bicgstab_dhat(ctx, m0, e32, r32, links32, inner_tol, maxiter - total, inner_ws, &it, nullptr, nullptr, stream);
+        if (rc != HR_OK) return rc;
+        total += it;
+        ++outer;
+        rc = launch_cvt(ctx, false, x_e, e32, nrm, st);                                               // x += |r| e
+        if (rc != HR_OK) return rc;
+        rc = dhat_launches(ctx, m0, 0, ax, x_e, tmp, links64, nullptr, nullptr, nullptr, st);         // fp64 true residual
+        if (rc != HR_OK) return rc;
+        rc = launch_lincomb(ctx, HR_F64, r, one, 0, b_e, mone, ax, st);                               // r = b - Dhat x
+        if (rc != HR_OK) return rc;
+        if (it == 0) break;                                                                           // no progress possible
+    }
+    if (iters) *iters = total;
+    if (outer_steps) *outer_steps = outer;
+    if (rel_res2) *rel_res2 = bb > 0 ? rr / bb : 0.0;
+    return HR_OK;
 }
 
 } // extern "C"

@@ -159,6 +159,8 @@ hr_status launch_represent(const hr_ctx *c, hr_prec in_prec, const void *fund, h
 //   out = ca * G(x) + cb * y   (G = gamma5 if g5 else identity; y may be null; out may alias x or y)
 hr_status launch_lincomb(const hr_ctx *c, hr_prec prec, void *out, const double ca[2], int g5, const void *x,
                          const double cb[2], const void *y, cudaStream_t st);
+// half field fp64 -> fp32 (dst = (float)(scale * src)) when down, else fp64 accumulate dst += scale * (double) src
+hr_status launch_cvt(const hr_ctx *c, bool down, void *dst, const void *src, double scale, cudaStream_t st);
 //   result[0..1] = <x, y> (result[0] = |x|^2 when x == y), device pointer
 hr_status launch_dot(const hr_ctx *c, hr_prec prec, const void *x, const void *y, const RedScratch &rs,
                      double *result_dev, cudaStream_t st);

@@ -99,6 +99,30 @@ __global__ void __launch_bounds__(LIN_THREADS) dot_kernel(const typename Vec16<R
     }
 }
 
+// ---- precision conversion of half fields in the internal layout (mixed-precision solver) -----------------------
+// fp32 vector v' of site s holds the reals 4v'..4v'+3, i.e. the fp64 vectors 2v' and 2v'+1 of the same site.
+__global__ void __launch_bounds__(LIN_THREADS) cvt_down_kernel(float4 *out, const double2 *in, double scale, size_t vh, size_t nvec32)
+{
+    const size_t i = (size_t)blockIdx.x * LIN_THREADS + threadIdx.x; // = v' * vh + s
+    if (i >= nvec32) return;
+    const size_t v = i / vh, s = i - v * vh;
+    const double2 a = in[(2 * v) * vh + s], b = in[(2 * v + 1) * vh + s];
+    out[i] = make_float4((float)(scale * a.x), (float)(scale * a.y), (float)(scale * b.x), (float)(scale * b.y));
+}
+// x64 += scale * (double) e32
+__global__ void __launch_bounds__(LIN_THREADS) cvt_up_axpy_kernel(double2 *x, const float4 *e, double scale, size_t vh, size_t nvec32)
+{
+    const size_t i = (size_t)blockIdx.x * LIN_THREADS + threadIdx.x;
+    if (i >= nvec32) return;
+    const size_t v = i / vh, s = i - v * vh;
+    const float4 ev = e[i];
+    double2 a = x[(2 * v) * vh + s], b = x[(2 * v + 1) * vh + s];
+    a.x = fma(scale, (double)ev.x, a.x); a.y = fma(scale, (double)ev.y, a.y);
+    b.x = fma(scale, (double)ev.z, b.x); b.y = fma(scale, (double)ev.w, b.y);
+    x[(2 * v) * vh + s] = a;
+    x[(2 * v + 1) * vh + s] = b;
+}
+
 static inline size_t field_nvec(const hr_ctx *c, hr_prec prec) { return (size_t)c->Vh * 8 * c->d * prec_bytes(prec) / 16; }
 
 // CTAs of a grid-stride reduction: enough to fill the machine, never more than the work
@@ -132,6 +156,15 @@ static hr_status lincomb_t(void *out, const double ca[2], int g5, const void *x,
     else    { if (y) GO(false, true); else GO(false, false); }
 #undef GO
     return check_launch("lincomb_kernel");
+}
+
+hr_status launch_cvt(const hr_ctx *c, bool down, void *dst, const void *src, double scale, cudaStream_t st)
+{
+    const size_t nvec32 = (size_t)c->Vh * 8 * c->d * 4 / 16;
+    const unsigned grid = (unsigned)((nvec32 + LIN_THREADS - 1) / LIN_THREADS);
+    if (down) cvt_down_kernel<<<grid, LIN_THREADS, 0, st>>>((float4 *)dst, (const double2 *)src, scale, (size_t)c->Vh, nvec32);
+    else cvt_up_axpy_kernel<<<grid, LIN_THREADS, 0, st>>>((double2 *)dst, (const float4 *)src, scale, (size_t)c->Vh, nvec32);
+    return check_launch(down ? "cvt_down_kernel" : "cvt_up_axpy_kernel");
 }
 
 hr_status launch_lincomb(const hr_ctx *c, hr_prec prec, void *out, const double ca[2], int g5, const void *x, const double cb[2],

@@ -392,3 +392,33 @@ def test_dirac_solve_bicgstab_inverts_the_oracles_dirac_operator(hr, dims, N, re
     assert rel_l2(x, x_want) <= 1e-9
     assert rel_l2(oracle.dirac(dims, BC_T, R, m0, x), b) <= 1e-9
     prob.close()
+
+
+@pytest.mark.parametrize("dims,N,rep,m0", CG_CASES)
+def test_mixed_precision_bicgstab_reaches_fp64_accuracy(hr, dims, N, rep, m0):
+    """hr_bicgstab_dhat_mixed: fp32 inner solves + fp64 true residual.  What it reaches has a plain definition, the
+    solution of Dhat x = b: compared with the oracle's fp64 solution, and its true residual with the oracle's Dhat."""
+    import torch
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(121, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    b = li.gaussian_spinor(122, li.volume(dims) // 2, d)
+    x_want, _, _ = solver.bicgstab_dhat(dims, BC_T, R, m0, b, 1e-12, 500)
+    prob = GpuProblem(hr, dims, N, rep, "f64", U)
+    lat = prob.lat
+    l32 = lat.gauge(True, hr.HR_F32)
+    lat.represent_links(l32, prob.fund)                     # fp64 fundamental -> fp32 represented (one rounding on store)
+    f = Fields(hr, prob)
+    gb, gx = f.put(b), f.new()
+    ws = torch.empty(hr.hr_mixed_workspace_bytes(lat.ctx, 500), dtype=torch.uint8, device="cuda")
+    it, outer, res2 = hr.hr_bicgstab_dhat_mixed(lat.ctx, m0, gx, gb, prob.links, l32, 1e-10, 1e-4, 500, ws, lat.stream())
+    assert 0 < it < 500 and 2 <= outer <= 6 and res2 <= 1e-20
+    x = f.get(gx)
+    assert rel_l2(x, x_want) <= 1e-8
+    assert rel_l2(solver.dhat(dims, BC_T, R, m0, x), b) <= 2e-10        # TRUE residual, oracle's operator
+    # argument errors: precisions swapped
+    with pytest.raises(hr.HrError):
+        hr.hr_bicgstab_dhat_mixed(lat.ctx, m0, gx, gb, l32, prob.links, 1e-10, 1e-4, 500, ws, lat.stream())
+    with pytest.raises(hr.HrError):
+        hr.hr_bicgstab_dhat_mixed(lat.ctx, m0, gx, gb, prob.links, l32, 1e-10, 1.5, 500, ws, lat.stream())
+    prob.close()
