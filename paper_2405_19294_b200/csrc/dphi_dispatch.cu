@@ -18,6 +18,7 @@ static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
 {
     // on-the-fly two-index kernels hold an N x N link, not a d_R x d_R one: a whole site fits one thread
     if (lk == 2 || lk == 3 || lk == 4) return 0;
+    if (lk == 6 || lk == 7) return prec == HR_F64 ? 2 : 0; // fp64 d_R = 8: two threads per site (measured)
     if (lk == 5) return 1;
     // measured on B200 (profiles/r1_variant_sweep.md): at d_R >= 6 fp64 one thread per site spills
     // and the pair kernel wins; in fp32 the whole site still fits one thread.
@@ -39,16 +40,18 @@ int dphi_link_kind(const hr_ctx *c, int link_src)
         if (c->rep == HR_REP_FUND) return 0;               // FUND: both fields are N x N complex
         if (c->rep == HR_REP_SYM) return 2;
         if (c->rep == HR_REP_ASYM) return 3;
-        return -1;                                         // adjoint from full fundamental links: not built
+        if (c->rep == HR_REP_ADJ && c->N == 3) return 6;   // SU(3) adjoint on the fly
+        return -1;                                         // SU(2) adjoint: from the row-compressed field (kind 5)
     }
     if (c->N > 3) return -1;                               // rows: SU(2), SU(3)
     if (c->rep == HR_REP_FUND) return 4;
     if (c->rep == HR_REP_ADJ && c->N == 2) return 5;
+    if (c->rep == HR_REP_ADJ && c->N == 3) return 7;
     return -1;
 }
 
 #define HR_COMBOS(X)                                                                                      \
-    X(2, 0) X(3, 0) X(4, 0) X(6, 0) X(3, 1) X(8, 1) X(3, 2) X(6, 2) X(3, 3) X(6, 3) X(2, 4) X(3, 4) X(3, 5)
+    X(2, 0) X(3, 0) X(4, 0) X(6, 0) X(3, 1) X(8, 1) X(3, 2) X(6, 2) X(3, 3) X(6, 3) X(2, 4) X(3, 4) X(3, 5) X(8, 6) X(8, 7)
 
 hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st, int link_src)
 {

@@ -104,15 +104,21 @@ __device__ __forceinline__ void colour_mul(Real (&chi)[2 * D], const Real *u, co
 // link bytes for the fundamental representation.  LK_ADJ2_ROWS builds the real 3x3 SU(2) adjoint link from the four
 // reals (a0, a3, a2, a1) = first row of U = a0 + i a.sigma:  R_ab = (a0^2 - a.a) delta_ab + 2 a_a a_b + 2 a0 eps_abc a_c
 // (32 B instead of 72 B per link in fp64).  Valid for links that ARE special unitary (reading C30).
-enum : int { LK_COMPLEX = 0, LK_REAL = 1, LK_SYM_OTF = 2, LK_ASYM_OTF = 3, LK_ROWS = 4, LK_ADJ2_ROWS = 5 };
+// LK_ADJ3_OTF / LK_ADJ3_ROWS: the SU(3) ADJOINT (d_R = 8) applied on the fly from the fundamental link (18 reals, or its
+// first two rows): with Psi = sum_a psi_a T_a (T_a = lambda_a/2, nested Gell-Mann order of reading C6),
+// (R psi)_a = 2 tr(T_a U Psi U^dagger) and (R^T psi)_a = 2 tr(T_a U^dagger Psi U) -- the 8 x 8 real link (512 B in
+// fp64, the paper's large-N_f register problem) is never formed: 144 or 96 B are read instead.
+enum : int { LK_COMPLEX = 0, LK_REAL = 1, LK_SYM_OTF = 2, LK_ASYM_OTF = 3, LK_ROWS = 4, LK_ADJ2_ROWS = 5, LK_ADJ3_OTF = 6,
+             LK_ADJ3_ROWS = 7 };
 
 template <int LK, int D> struct LinkGeom {
     // N of the fundamental link for the on-the-fly kinds: D = N(N+1)/2 (sym) or N(N-1)/2 (asym)
     static constexpr int N = LK == LK_SYM_OTF ? (D == 3 ? 2 : D == 6 ? 3 : D == 10 ? 4 : 0)
                            : LK == LK_ASYM_OTF ? (D == 3 ? 3 : D == 6 ? 4 : 0)
-                           : LK == LK_ADJ2_ROWS ? (D == 3 ? 2 : 0) : D;
+                           : LK == LK_ADJ2_ROWS ? (D == 3 ? 2 : 0)
+                           : (LK == LK_ADJ3_OTF || LK == LK_ADJ3_ROWS) ? (D == 8 ? 3 : 0) : D;
     static constexpr int NREAL = LK == LK_REAL ? D * D : LK == LK_COMPLEX ? 2 * D * D
-                               : (LK == LK_ROWS || LK == LK_ADJ2_ROWS) ? 2 * N * (N - 1) : 2 * N * N;
+                               : (LK == LK_ROWS || LK == LK_ADJ2_ROWS || LK == LK_ADJ3_ROWS) ? 2 * N * (N - 1) : 2 * N * N;
     static_assert(N > 0, "no such two-index representation");
 };
 
@@ -215,6 +221,62 @@ template <typename Real> __device__ __forceinline__ void rebuild_adj2(Real (&m)[
     m[6] += (Real)2 * a0 * a[1]; m[2] -= (Real)2 * a0 * a[1];
 }
 
+// chi = R^adj(U) h (DAG = false) or R^adj(U)^T h (DAG = true) for SU(3), from the fundamental link u[3][3] (re,im);
+// components in the nested Gell-Mann order: 0 S01, 1 A01, 2 D1, 3 S02, 4 A02, 5 S12, 6 A12, 7 D2
+template <bool DAG, typename Real>
+__device__ __forceinline__ void adj3_mul(Real (&chi)[16], const Real *u, const Real (&h)[16])
+{
+    constexpr Real IS3 = (Real)0.57735026918962576451; // 1/sqrt(3)
+    // Psi = (1/2) sum_a h_a lambda_a  (the factor 1/2 is applied at the end together with the 2 of 2 tr(T_a .))
+    Real pr[3][3], pi[3][3];
+    auto offd = [&](int i, int m, int s, int a) { // Psi_im = h_S - i h_A, Psi_mi = h_S + i h_A
+        pr[i][m] = h[2 * s] + h[2 * a + 1]; pi[i][m] = h[2 * s + 1] - h[2 * a];
+        pr[m][i] = h[2 * s] - h[2 * a + 1]; pi[m][i] = h[2 * s + 1] + h[2 * a];
+    };
+    offd(0, 1, 0, 1); offd(0, 2, 3, 4); offd(1, 2, 5, 6);
+    pr[0][0] = h[4] + IS3 * h[14]; pi[0][0] = h[5] + IS3 * h[15];
+    pr[1][1] = -h[4] + IS3 * h[14]; pi[1][1] = -h[5] + IS3 * h[15];
+    pr[2][2] = (Real)-2 * IS3 * h[14]; pi[2][2] = (Real)-2 * IS3 * h[15];
+    auto wr = [&](int i, int k) -> Real { return DAG ? u[2 * (k * 3 + i)] : u[2 * (i * 3 + k)]; };
+    auto wi = [&](int i, int k) -> Real { return DAG ? -u[2 * (k * 3 + i) + 1] : u[2 * (i * 3 + k) + 1]; };
+    Real ar[3][3], ai[3][3], mr[3][3], mi[3][3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int l = 0; l < 3; ++l) {
+            Real re = 0, im = 0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                re = fma(wr(i, k), pr[k][l], re); re = fma(-wi(i, k), pi[k][l], re);
+                im = fma(wr(i, k), pi[k][l], im); im = fma(wi(i, k), pr[k][l], im);
+            }
+            ar[i][l] = re; ai[i][l] = im;
+        }
+    // M = A W^dagger: M_ij = sum_l A_il conj(W_jl)
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            Real re = 0, im = 0;
+#pragma unroll
+            for (int l = 0; l < 3; ++l) {
+                re = fma(ar[i][l], wr(j, l), re); re = fma(ai[i][l], wi(j, l), re);
+                im = fma(ai[i][l], wr(j, l), im); im = fma(-ar[i][l], wi(j, l), im);
+            }
+            mr[i][j] = re; mi[i][j] = im;
+        }
+    // chi_a = tr(lambda_a M) / 2 ... with Psi carrying no 1/2: chi_a = (1/2) tr(lambda_a M)
+    auto ext = [&](int i, int m, int s, int a) {
+        chi[2 * s] = (Real)0.5 * (mr[m][i] + mr[i][m]); chi[2 * s + 1] = (Real)0.5 * (mi[m][i] + mi[i][m]);
+        // i (M_im - M_mi)
+        chi[2 * a] = (Real)-0.5 * (mi[i][m] - mi[m][i]); chi[2 * a + 1] = (Real)0.5 * (mr[i][m] - mr[m][i]);
+    };
+    ext(0, 1, 0, 1); ext(0, 2, 3, 4); ext(1, 2, 5, 6);
+    chi[4] = (Real)0.5 * (mr[0][0] - mr[1][1]); chi[5] = (Real)0.5 * (mi[0][0] - mi[1][1]);
+    chi[14] = (Real)0.5 * IS3 * (mr[0][0] + mr[1][1] - (Real)2 * mr[2][2]);
+    chi[15] = (Real)0.5 * IS3 * (mi[0][0] + mi[1][1] - (Real)2 * mi[2][2]);
+}
+
 template <int D, int LK, bool DAG, typename Real>
 __device__ __forceinline__ void link_mul(Real (&chi)[2 * D], const Real *u, const Real (&h)[2 * D])
 {
@@ -227,6 +289,12 @@ __device__ __forceinline__ void link_mul(Real (&chi)[2 * D], const Real *u, cons
         Real m[9];
         rebuild_adj2(m, u);
         colour_mul<3, true, DAG>(chi, m, h);
+    } else if constexpr (LK == LK_ADJ3_OTF) {
+        adj3_mul<DAG>(chi, u, h);
+    } else if constexpr (LK == LK_ADJ3_ROWS) {
+        Real f[18];
+        rebuild_rows<3>(f, u);
+        adj3_mul<DAG>(chi, f, h);
     } else twoindex_mul<D, LK, DAG>(chi, u, h);
 }
 
@@ -243,6 +311,10 @@ __device__ __forceinline__ void with_link(const Real *u, F &&f)
         Real m[9];
         rebuild_adj2(m, u);
         f(std::integral_constant<int, LK_REAL>{}, (const Real *)m);
+    } else if constexpr (LK == LK_ADJ3_ROWS) {
+        Real full[18];
+        rebuild_rows<3>(full, u);
+        f(std::integral_constant<int, LK_ADJ3_OTF>{}, (const Real *)full);
     } else {
         f(std::integral_constant<int, LK>{}, u);
     }

@@ -13,7 +13,7 @@ from gpu_common import BC_T, TOL, GpuProblem, oracle_rep_id, rel_l2
 
 pytestmark = pytest.mark.gpu
 
-OTF_COMBOS = [(2, "sym"), (3, "sym"), (3, "asym"), (4, "asym")]
+OTF_COMBOS = [(2, "sym"), (3, "sym"), (3, "asym"), (4, "asym"), (3, "adj")]
 
 
 @pytest.fixture(scope="module")

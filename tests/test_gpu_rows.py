@@ -11,7 +11,7 @@ from oracle import solver
 from gpu_common import BC_T, TOL, GpuProblem, oracle_rep_id, rel_l2
 
 pytestmark = pytest.mark.gpu
-COMBOS = [(2, "fund"), (3, "fund"), (2, "adj")]
+COMBOS = [(2, "fund"), (3, "fund"), (2, "adj"), (3, "adj")]
 
 
 @pytest.fixture(scope="module")
