@@ -98,8 +98,9 @@ hr_status hr_spinor_export(const hr_ctx *ctx, const void *src_dev, hr_prec prec,
  * hr_gauge_alloc(ctx, 2, prec, ...) makes a field that keeps only the first N-1 rows of every fundamental link
  * (SU(3): 12 of 18 reals, SU(2): 4 of 8); hr_gauge_compress fills it from a fundamental field of the same precision.
  * Every compute call that takes `links` accepts it for the FUNDAMENTAL representation (the last row is rebuilt in
- * registers: conj(row0 x row1), resp. (-conj u01, conj u00)) and for the SU(2) ADJOINT (the real 3x3 link is built from
- * the four reals of the first row: 32 instead of 72 bytes per link in fp64).  Only for links that ARE special unitary:
+ * registers: conj(row0 x row1), resp. (-conj u01, conj u00)), for the SU(2) ADJOINT (the real 3x3 link is built from
+ * the four reals of the first row: 32 instead of 72 bytes per link in fp64) and for the SU(3) ADJOINT (applied on the
+ * fly, 96 instead of 512 bytes).  Only for links that ARE special unitary:
  * the result equals that of the full links up to their unitarity violation.  Such a field cannot be imported/exported.
  */
 hr_status hr_gauge_compress(hr_gauge *rows_out, const hr_gauge *fund_in, void *stream);
@@ -125,8 +126,11 @@ hr_status hr_represent_links(hr_gauge *repr_out, const hr_gauge *fund_in, void *
  * FUNDAMENTAL field when the representation is two-index symmetric / antisymmetric (or fundamental):
  * the kernel then reads the N x N link (e.g. 144 instead of 576 bytes for the SU(3) sextet in fp64) and
  * applies R(U) psi as U Psi U^T, R(U)^dagger psi as U^dagger Psi U^*, Psi = sum_a psi_a e_a in the basis
- * of reading C8 -- the same operator, never forming R(U).  The adjoint needs its represented (real)
- * field: a fundamental one -> HR_EINVAL.  The same holds for every call below that takes `links`.
+ * of reading C8 -- the same operator, never forming R(U).  The SU(3) adjoint likewise accepts the
+ * fundamental field ((R psi)_a = 2 tr(T_a U Psi U^dagger), Psi = sum_a psi_a T_a: 144 instead of 512 bytes
+ * per link in fp64); the SU(2) adjoint accepts the row-compressed field of hr_gauge_compress (32 instead of
+ * 72 bytes) but not the full fundamental one (-> HR_EINVAL).  The same holds for every call below that
+ * takes `links`.
  */
 hr_status hr_dphi_eo(void *out, const void *in, const hr_gauge *links, int parity, void *stream);
 
