@@ -102,3 +102,54 @@ def dirac_expclover(dims, bc, links_R, m0, csw, psi_eo):
     E = exp_clover_term(dims, links_R, m0, csw)
     epsi = lex_to_eo(dims, apply_clover_lex(E, eo_to_lex(dims, psi_eo)))
     return dirac(dims, bc, links_R, m0, psi_eo) + epsi
+
+
+# ---- even-odd preconditioning WITH the clover term ("even-odd preconditioning, clover"; reading C32) ----
+def site_term(dims, links_R, m0, csw, exponentiated=False):
+    """The site-diagonal part A(x) of the improved operator as dense [V, 4d, 4d] matrices (lexicographic sites):
+    A = (4+m0) + T (clover) or (4+m0) exp(T/(4+m0)) (exponentiated clover)."""
+    m = 4.0 + m0
+    X = exp_clover_term(dims, links_R, m0, csw) if exponentiated else clover_term(dims, links_R, csw)
+    V, d = X.shape[0], X.shape[2]
+    return X.reshape(V, 4 * d, 4 * d) + m * np.eye(4 * d)[None]
+
+
+def _halves(dims, A_lex):
+    """[V, n, n] lexicographic -> (even sites, odd sites) in canonical half-field order."""
+    eo = lex_to_eo(dims, A_lex)
+    vh = A_lex.shape[0] // 2
+    return eo[:vh], eo[vh:]
+
+
+def _blockmul(A_half, psi_half):
+    n = A_half.shape[-1]
+    return (A_half @ psi_half.reshape(psi_half.shape[0], n, 1)).reshape(psi_half.shape)
+
+
+def dhat_clover(dims, bc, links_R, m0, csw, psi_e, exponentiated=False):
+    """Reading C32: with D_sw = [[A_ee, Dphi_eo], [Dphi_oe, A_oo]] the even-odd preconditioned operator is the Schur
+    complement on the even sites,  Dhat_sw = A_ee - Dphi_eo A_oo^{-1} Dphi_oe  (not multiplied by anything: A is a
+    matrix now, not the number 4+m0 of reading C20)."""
+    from . import dphi_eo
+    Ae, Ao = _halves(dims, site_term(dims, links_R, m0, csw, exponentiated))
+    t = dphi_eo(dims, bc, links_R, 1, psi_e)                                   # odd sites
+    n = Ao.shape[-1]
+    t = np.linalg.solve(Ao, t.reshape(t.shape[0], n, 1)).reshape(t.shape)       # A_oo^{-1}
+    return _blockmul(Ae, psi_e) - dphi_eo(dims, bc, links_R, 0, t)
+
+
+def dirac_clover_solve(dims, bc, links_R, m0, csw, b_eo, tol, maxiter, exponentiated=False):
+    """x = D_sw^{-1} b through the preconditioned system (BiCGstab of oracle.solver on Dhat_sw):
+    Dhat_sw x_e = b_e - Dphi_eo A_oo^{-1} b_o,   x_o = A_oo^{-1} (b_o - Dphi_oe x_e).  Returns (x_eo, iterations)."""
+    from . import dphi_eo
+    from .solver import bicgstab
+    Ae, Ao = _halves(dims, site_term(dims, links_R, m0, csw, exponentiated))
+    n = Ao.shape[-1]
+    ainv = lambda v: np.linalg.solve(Ao, v.reshape(v.shape[0], n, 1)).reshape(v.shape)
+    vh = b_eo.shape[0] // 2
+    b_e, b_o = b_eo[:vh], b_eo[vh:]
+    rhs = b_e - dphi_eo(dims, bc, links_R, 0, ainv(b_o))
+    op = lambda v: dhat_clover(dims, bc, links_R, m0, csw, v, exponentiated)
+    x_e, it, _ = bicgstab(op, rhs, tol, maxiter)
+    x_o = ainv(b_o - dphi_eo(dims, bc, links_R, 1, x_e))
+    return np.concatenate([x_e, x_o], axis=0), it

@@ -182,3 +182,41 @@ def test_dirac_expclover_reduces_to_dirac_without_field_strength():
     one = np.broadcast_to(np.eye(2, dtype=complex), (V, 4, 2, 2)).copy()
     psi = li.gaussian_spinor(13, V, 2)
     assert np.allclose(clover.dirac_expclover(dims, BC_T, one, -0.1, 1.3, psi), oracle.dirac(dims, BC_T, one, -0.1, psi), atol=1e-14)
+
+
+# ------------------------------------------------------------------------------ even-odd preconditioning with clover
+def _dense_dsw_eo(dims, bc, R, m0, csw, exponentiated):
+    """Dense D_sw (oracle.dense + per-site blocks), rows/columns in [even sites | odd sites] order."""
+    V, d = li.volume(dims), R.shape[-1]
+    g = [oracle.gamma(mu) for mu in range(4)]
+    D = dense.dirac_matrix(dims, bc, R, m0, g, hopping_only=True)
+    A = clover.site_term(dims, R, m0, csw, exponentiated)
+    for x in range(V):
+        D[x * 4 * d:(x + 1) * 4 * d, x * 4 * d:(x + 1) * 4 * d] += A[x]
+    site_eo = oracle.lex_to_eo(dims, np.arange(V))
+    idx = (site_eo[:, None] * (4 * d) + np.arange(4 * d)[None, :]).reshape(-1)
+    return D[np.ix_(idx, idx)]
+
+
+@pytest.mark.parametrize("exponentiated", [False, True])
+@pytest.mark.parametrize("dims,N,rep", [((2, 2, 2, 2), 2, "fund"), ((2, 2, 4, 2), 2, "adj"), ((2, 2, 2, 2), 3, "fund")])
+def test_dhat_clover_is_the_dense_schur_complement_and_the_solve_is_the_dense_solve(dims, N, rep, exponentiated):
+    U = li.haar_links(21, N, dims)
+    R = oracle.represent(N, oracle.REP_NAMES[rep], U)
+    d, V = R.shape[-1], li.volume(dims)
+    m0, csw = -0.3, 1.2
+    D = _dense_dsw_eo(dims, BC_T, R, m0, csw, exponentiated)
+    n = D.shape[0] // 2
+    schur = D[:n, :n] - D[:n, n:] @ np.linalg.inv(D[n:, n:]) @ D[n:, :n]
+    psi = li.gaussian_spinor(22, V // 2, d)
+    want = (schur @ psi.reshape(-1)).reshape(psi.shape)
+    got = clover.dhat_clover(dims, BC_T, R, m0, csw, psi, exponentiated)
+    assert np.linalg.norm(got - want) <= 1e-12 * np.linalg.norm(want)
+    b = li.gaussian_spinor(23, V, d)
+    x, it = clover.dirac_clover_solve(dims, BC_T, R, m0, csw, b, 1e-13, 500, exponentiated)
+    xs = np.linalg.solve(D, b.reshape(-1)).reshape(b.shape)
+    assert 0 < it < 500 and np.linalg.norm(x - xs) <= 1e-9 * np.linalg.norm(xs)
+    # c_sw = 0: A = 4 + m0 and Dhat_sw = Dhat / (4 + m0) of reading C20
+    from oracle import solver
+    z = clover.dhat_clover(dims, BC_T, R, m0, 0.0, psi, exponentiated)
+    assert np.allclose(z * (4 + m0), solver.dhat(dims, BC_T, R, m0, psi), atol=1e-12)
