@@ -290,8 +290,27 @@ hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *re
  *     site-diagonal part (4+m0) + T of D_sw becomes (4+m0) exp(T/(4+m0)), positive definite on every gauge field).
  *     Replaces, IN PLACE, the T written by hr_clover_build by E = (4+m0)[exp(T/(4+m0)) - 1]; hr_dirac_clover with the
  *     same m0 then applies D_exp = Dphi + (4+m0) exp(T/(4+m0)).  One launch over the 2V blocks; 4 + m0 > 0.
+ * Even-odd preconditioning WITH the clover term ("even-odd preconditioning, clover"; reading C32): with
+ * A(x) = (4+m0) + T(x)  [or (4+m0) exp(T/(4+m0)) after hr_clover_exp]  and  D_sw = [[A_ee, Dphi_eo], [Dphi_oe, A_oo]],
+ *     Dhat_sw = A_ee - Dphi_eo A_oo^{-1} Dphi_oe                                  (Schur complement on the even sites).
+ * hr_clover_finalize: IN PLACE site_term (T or E, as written by hr_clover_build / hr_clover_exp) -> A = (4+m0) + it, and
+ *     A^{-1} (every 2 d_R x 2 d_R block inverted by Gauss-Jordan elimination in fp64) into site_inverse, a second buffer
+ *     of hr_clover_bytes().  After this call the buffers serve hr_dhat_clover / hr_dirac_clover_solve (NOT
+ *     hr_dirac_clover, which expects T and adds 4+m0 itself).
+ * hr_dhat_clover: out_e = Dhat_sw in_e; two Dphi launches and two site-local launches; tmp_o, tmp2_o: odd-parity half
+ *     fields owned by the caller; the four spinor buffers distinct.
+ * hr_dirac_clover_solve: x = D_sw^{-1} b on full fields [even half | odd half] through
+ *     Dhat_sw x_e = b_e - Dphi_eo A_oo^{-1} b_o,  x_o = A_oo^{-1} (b_o - Dphi_oe x_e),  the preconditioned system solved
+ *     by BiCGstab (reading C29; tol, iters and rel_res2 refer to it); workspace of hr_clover_solve_workspace_bytes().
  */
 size_t hr_clover_bytes(const hr_ctx *ctx, hr_prec prec);
+hr_status hr_clover_finalize(const hr_ctx *ctx, hr_prec prec, void *site_term, void *site_inverse, double m0, void *stream);
+hr_status hr_dhat_clover(void *out_e, const void *in_e, void *tmp_o, void *tmp2_o, const hr_gauge *links,
+                         const void *site_term, const void *site_inverse, void *stream);
+size_t hr_clover_solve_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter);
+hr_status hr_dirac_clover_solve(hr_ctx *ctx, void *x_full, const void *b_full, const hr_gauge *links, const void *site_term,
+                                const void *site_inverse, double tol, int maxiter, void *workspace, int *iters,
+                                double *rel_res2, void *stream);
 hr_status hr_clover_exp(const hr_ctx *ctx, hr_prec prec, void *clover, double m0, void *stream);
 hr_status hr_clover_build(void *clover, const hr_gauge *links, double csw, void *stream);
 hr_status hr_dirac_clover(double m0, void *out_full, const void *in_full, const hr_gauge *links, const void *clover,

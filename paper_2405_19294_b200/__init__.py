@@ -91,6 +91,10 @@ _SIGNATURES = {
     "hr_clover_build": (_ci, [_vp, _vp, _cd, _vp]),
     "hr_clover_exp": (_ci, [_vp, _ci, _vp, _cd, _vp]),
     "hr_dirac_clover": (_ci, [_cd, _vp, _vp, _vp, _vp, _vp]),
+    "hr_clover_finalize": (_ci, [_vp, _ci, _vp, _vp, _cd, _vp]),
+    "hr_dhat_clover": (_ci, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "hr_clover_solve_workspace_bytes": (_sz, [_vp, _ci, _ci]),
+    "hr_dirac_clover_solve": (_ci, [_vp, _vp, _vp, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
     "hr_dirac_solve_bicgstab": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
     "hr_mixed_workspace_bytes": (_sz, [_vp, _ci]),
     "hr_bicgstab_dhat_mixed": (_ci, [_vp, _cd, _vp, _vp, _vp, _vp, _cd, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
@@ -371,6 +375,26 @@ def hr_bicgstab_dhat_mixed(ctx: int, m0: float, x_e, b_e, links64: int, links32:
     _check(_lib.hr_bicgstab_dhat_mixed(ctx, float(m0), _ptr(x_e), _ptr(b_e), links64, links32, float(tol), float(inner_tol),
                                        int(maxiter), _ptr(workspace), ctypes.byref(it), ctypes.byref(outer), ctypes.byref(res), stream))
     return it.value, outer.value, res.value
+
+
+def hr_clover_finalize(ctx: int, prec: int, site_term, site_inverse, m0: float, stream: int = 0) -> None:
+    _check(_lib.hr_clover_finalize(ctx, prec, _ptr(site_term), _ptr(site_inverse), float(m0), stream))
+
+
+def hr_dhat_clover(out_e, in_e, tmp_o, tmp2_o, links: int, site_term, site_inverse, stream: int = 0) -> None:
+    _check(_lib.hr_dhat_clover(_ptr(out_e), _ptr(in_e), _ptr(tmp_o), _ptr(tmp2_o), links, _ptr(site_term), _ptr(site_inverse), stream))
+
+
+def hr_clover_solve_workspace_bytes(ctx: int, prec: int, maxiter: int) -> int:
+    return _lib.hr_clover_solve_workspace_bytes(ctx, prec, maxiter)
+
+
+def hr_dirac_clover_solve(ctx: int, x_full, b_full, links: int, site_term, site_inverse, tol: float, maxiter: int, workspace, stream: int = 0):
+    """Returns (iterations, |r|^2/|bhat|^2 of the preconditioned system)."""
+    it, res = _ci(0), _cd(0.0)
+    _check(_lib.hr_dirac_clover_solve(ctx, _ptr(x_full), _ptr(b_full), links, _ptr(site_term), _ptr(site_inverse), float(tol),
+                                      int(maxiter), _ptr(workspace), ctypes.byref(it), ctypes.byref(res), stream))
+    return it.value, res.value
 
 
 def hr_ctx_set_tuning(ctx: int, key: str, value: int) -> None:

@@ -175,7 +175,8 @@ __global__ void __launch_bounds__(64) clover_build_kernel(const CloverArgs a)
 // out += T in on one parity (clover/in/out point at that parity's half fields).  One thread per (site, chirality
 // block): it holds the block's 2 d_R input and output components and STREAMS the packed Hermitian block through one
 // 16-byte vector at a time (a whole d_R = 6 block is 144 reals -- preloading it spills).
-template <typename Real, int D>
+// MODE: +1  out += T in;   0  out = T in (out is not read);   -1  out = T in - out
+template <typename Real, int D, int MODE>
 __global__ void __launch_bounds__(128) clover_apply_kernel(const CloverArgs a)
 {
     constexpr int BLK = 4 * D * D, N2 = 2 * D, RPV = 16 / (int)sizeof(Real);
@@ -189,7 +190,16 @@ __global__ void __launch_bounds__(128) clover_apply_kernel(const CloverArgs a)
     const size_t vh = (size_t)a.vh, pb = vh * 16;
     Real v[4 * D], w[4 * D];
     load_planes<LD_STREAM, NVH>(v, (const char *)a.in + (size_t)s * 16 + (size_t)(b * NVH) * pb, pb, 0);
-    load_planes<LD_STREAM, NVH>(w, (const char *)a.out + (size_t)s * 16 + (size_t)(b * NVH) * pb, pb, 0);
+    if constexpr (MODE == 0) {
+#pragma unroll
+        for (int e = 0; e < 4 * D; ++e) w[e] = 0;
+    } else {
+        load_planes<LD_STREAM, NVH>(w, (const char *)a.out + (size_t)s * 16 + (size_t)(b * NVH) * pb, pb, 0);
+        if constexpr (MODE < 0) {
+#pragma unroll
+            for (int e = 0; e < 4 * D; ++e) w[e] = -w[e];
+        }
+    }
     const char *tp = (const char *)a.clover + (size_t)s * 16 + (size_t)(b * NVB) * pb;
     Real tv[RPV];
     int idx = 0; // position in the packed block; a compile-time constant at every use once the loops are unrolled
@@ -280,6 +290,76 @@ __global__ void __launch_bounds__(64) clover_exp_kernel(char *clover, long vh, d
     store_planes<ST_DEFAULT, NVB>(rec, pb, t);
 }
 
+// T (or E) -> A = (4+m0) + T in place, and A^{-1} into a second field of the same layout (reading C32: the even-odd
+// preconditioned operator with a clover term needs A_oo^{-1}).  One thread per (site, chirality block); the n x n
+// block (n = 2 d_R <= 16) is inverted by Gauss-Jordan elimination with partial pivoting in fp64 (the inverse of a
+// Hermitian matrix is Hermitian, so it packs the same way).  Set-up kernel.
+template <typename Real, int D>
+__global__ void __launch_bounds__(64) clover_finalize_kernel(char *clover, char *inverse, long vh, double m)
+{
+    constexpr int N2 = 2 * D, M = 2 * N2 * N2, BLK = 4 * D * D, RPV = 16 / (int)sizeof(Real), NVB = BLK / RPV;
+    const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= 4 * vh) return;
+    const int b = (int)(tid & 1);
+    const long site = tid >> 1;
+    const long par = site / vh, s = site - par * vh;
+    const size_t off = (size_t)par * 2 * BLK * sizeof(Real) * (size_t)vh + (size_t)s * 16 + (size_t)(b * NVB) * (size_t)vh * 16;
+    const size_t pb = (size_t)vh * 16;
+    Real t[BLK];
+    load_planes<LD_DEFAULT, NVB>(t, clover + off, pb, 0);
+    double x[M], y[M];
+    for (int i = 0; i < M; ++i) { x[i] = 0; y[i] = 0; }
+    {
+        int w = 0;
+        for (int d = 0; d < N2; ++d) { t[w] = (Real)((double)t[w] + m); x[2 * (d * N2 + d)] = (double)t[w]; y[2 * (d * N2 + d)] = 1.0; ++w; }
+        for (int r = 0; r < N2; ++r)
+            for (int c = r + 1; c < N2; ++c) {
+                const double re = (double)t[w++], im = (double)t[w++];
+                x[2 * (r * N2 + c)] = re; x[2 * (r * N2 + c) + 1] = im;
+                x[2 * (c * N2 + r)] = re; x[2 * (c * N2 + r) + 1] = -im;
+            }
+    }
+    store_planes<ST_DEFAULT, NVB>(clover + off, pb, t);   // A = m + T
+    for (int col = 0; col < N2; ++col) {
+        int piv = col;
+        double best = -1.0;
+        for (int r = col; r < N2; ++r) {
+            const double v = x[2 * (r * N2 + col)] * x[2 * (r * N2 + col)] + x[2 * (r * N2 + col) + 1] * x[2 * (r * N2 + col) + 1];
+            if (v > best) { best = v; piv = r; }
+        }
+        if (piv != col)
+            for (int k = 0; k < 2 * N2; ++k) {
+                double tmp = x[2 * col * N2 + k]; x[2 * col * N2 + k] = x[2 * piv * N2 + k]; x[2 * piv * N2 + k] = tmp;
+                tmp = y[2 * col * N2 + k]; y[2 * col * N2 + k] = y[2 * piv * N2 + k]; y[2 * piv * N2 + k] = tmp;
+            }
+        const double pr = x[2 * (col * N2 + col)], pi = x[2 * (col * N2 + col) + 1];
+        const double den = pr * pr + pi * pi, ir = pr / den, ii = -pi / den; // 1 / pivot
+        for (int k = 0; k < N2; ++k) {
+            double re = x[2 * (col * N2 + k)], im = x[2 * (col * N2 + k) + 1];
+            x[2 * (col * N2 + k)] = re * ir - im * ii; x[2 * (col * N2 + k) + 1] = re * ii + im * ir;
+            re = y[2 * (col * N2 + k)]; im = y[2 * (col * N2 + k) + 1];
+            y[2 * (col * N2 + k)] = re * ir - im * ii; y[2 * (col * N2 + k) + 1] = re * ii + im * ir;
+        }
+        for (int r = 0; r < N2; ++r) {
+            if (r == col) continue;
+            const double fr = x[2 * (r * N2 + col)], fi = x[2 * (r * N2 + col) + 1];
+            for (int k = 0; k < N2; ++k) {
+                const double ar = x[2 * (col * N2 + k)], ai = x[2 * (col * N2 + k) + 1];
+                x[2 * (r * N2 + k)] -= fr * ar - fi * ai; x[2 * (r * N2 + k) + 1] -= fr * ai + fi * ar;
+                const double br = y[2 * (col * N2 + k)], bi = y[2 * (col * N2 + k) + 1];
+                y[2 * (r * N2 + k)] -= fr * br - fi * bi; y[2 * (r * N2 + k) + 1] -= fr * bi + fi * br;
+            }
+        }
+    }
+    {
+        int w = 0;
+        for (int d = 0; d < N2; ++d) t[w++] = (Real)y[2 * (d * N2 + d)];
+        for (int r = 0; r < N2; ++r)
+            for (int c = r + 1; c < N2; ++c) { t[w++] = (Real)y[2 * (r * N2 + c)]; t[w++] = (Real)y[2 * (r * N2 + c) + 1]; }
+    }
+    store_planes<ST_DEFAULT, NVB>(inverse + off, pb, t);
+}
+
 static hr_status launched(const char *what)
 {
     count_launch();
@@ -328,21 +408,43 @@ hr_status launch_clover_exp(const hr_ctx *c, hr_prec prec, void *clover, double 
     return HR_EUNSUPPORTED;
 }
 
-hr_status launch_clover_apply(const hr_ctx *c, hr_prec prec, void *out, const void *in, const void *clover_parity, cudaStream_t st)
+hr_status launch_clover_finalize(const hr_ctx *c, hr_prec prec, void *clover, void *inverse, double m, cudaStream_t st)
+{
+    const unsigned grid = (unsigned)((4 * c->Vh + 63) / 64);
+#define X(D)                                                                                                          \
+    if (c->d == D) {                                                                                                  \
+        if (prec == HR_F64) clover_finalize_kernel<double, D><<<grid, 64, 0, st>>>((char *)clover, (char *)inverse, c->Vh, m); \
+        else clover_finalize_kernel<float, D><<<grid, 64, 0, st>>>((char *)clover, (char *)inverse, c->Vh, m);       \
+        return launched("clover_finalize_kernel");                                                                    \
+    }
+    X(2) X(3) X(4) X(6) X(8)
+#undef X
+    set_error("no clover kernel compiled for d_R=%d", c->d);
+    return HR_EUNSUPPORTED;
+}
+
+// out (+)= T in on one parity; mode +1: out += T in, 0: out = T in, -1: out = T in - out
+hr_status launch_clover_apply(const hr_ctx *c, hr_prec prec, void *out, const void *in, const void *clover_parity, cudaStream_t st, int mode)
 {
     CloverArgs a;
     a.clover = const_cast<void *>(clover_parity); a.links = nullptr; a.in = in; a.out = out;
     a.T = c->dims[0]; a.X = c->dims[1]; a.Y = c->dims[2]; a.Z = c->dims[3];
     a.vh = c->Vh; a.csw = 0;
     const unsigned grid = (unsigned)((2 * c->Vh + 127) / 128);
+#define GO(Real, D)                                                                                                   \
+    do {                                                                                                              \
+        if (mode > 0) clover_apply_kernel<Real, D, 1><<<grid, 128, 0, st>>>(a);                                      \
+        else if (mode == 0) clover_apply_kernel<Real, D, 0><<<grid, 128, 0, st>>>(a);                                \
+        else clover_apply_kernel<Real, D, -1><<<grid, 128, 0, st>>>(a);                                              \
+    } while (0)
 #define X(D)                                                                                                          \
     if (c->d == D) {                                                                                                  \
-        if (prec == HR_F64) clover_apply_kernel<double, D><<<grid, 128, 0, st>>>(a);                                 \
-        else clover_apply_kernel<float, D><<<grid, 128, 0, st>>>(a);                                                 \
+        if (prec == HR_F64) GO(double, D); else GO(float, D);                                                         \
         return launched("clover_apply_kernel");                                                                       \
     }
     X(2) X(3) X(4) X(6) X(8)
 #undef X
+#undef GO
     set_error("no clover kernel compiled for d_R=%d", c->d);
     return HR_EUNSUPPORTED;
 }

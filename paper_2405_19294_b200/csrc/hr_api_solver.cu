@@ -4,6 +4,7 @@
 // the Dphi kernels.  No CPU fallback.
 #include <cmath>
 #include <cstring>
+#include <functional>
 
 #include "hr_internal.h"
 
@@ -268,19 +269,21 @@ size_t hr_bicgstab_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter)
     return 7 * (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec) + bicgstab_state_bytes(maxiter);
 }
 
-hr_status hr_bicgstab_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol, int maxiter,
-                           void *workspace, int *iters, double *rel_res2, double *hist, void *stream)
+} // extern "C"
+
+// The operator of a BiCGstab run: out = Op in.  reduce: also leave |out|^2 and <in, out> in red[0..2] (the Dphi
+// epilogue does it for Dhat; operators that end in another kernel use two dot launches).  skip: device flag, non-zero =
+// converged (kernels that know about it return at once).
+typedef std::function<hr_status(void *out, const void *in, bool reduce, double *red, const int *skip)> BiOp;
+
+// textbook BiCGstab on device-resident scalars (bicgstab.cu); ws holds r, rhat, p, v, s, t (6 half spinors) and the state
+static hr_status bicgstab_core(hr_ctx *ctx, hr_prec prec, void *x_e, const void *b_e, double tol, int maxiter, char *ws,
+                               void *state, const BiOp &op, int *iters, double *rel_res2, double *hist, cudaStream_t st)
 {
-    hr_status rc = cg_check("hr_bicgstab_dhat", ctx, x_e, b_e, links, tol, maxiter, workspace);
-    if (rc != HR_OK) return rc;
-    cudaStream_t st = (cudaStream_t)stream;
-    const hr_prec prec = links->prec;
-    char *ws = (char *)workspace;
     const size_t sb = (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec);
-    void *r = ws, *rhat = ws + sb, *p = ws + 2 * sb, *v = ws + 3 * sb, *s = ws + 4 * sb, *t = ws + 5 * sb, *tmp = ws + 6 * sb;
-    void *state = ws + 7 * sb;
+    void *r = ws, *rhat = ws + sb, *p = ws + 2 * sb, *v = ws + 3 * sb, *s = ws + 4 * sb, *t = ws + 5 * sb;
     RedScratch rs;
-    rc = get_red_scratch(ctx, &rs, st);
+    hr_status rc = get_red_scratch(ctx, &rs, st);
     if (rc != HR_OK) return rc;
     rc = launch_bi_init(ctx, prec, state, tol, maxiter, x_e, r, rhat, p, v, b_e, rs, st);
     if (rc != HR_OK) return rc;
@@ -288,13 +291,13 @@ hr_status hr_bicgstab_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, c
     auto one_iteration = [&]() -> hr_status {
         hr_status e = launch_bi_update_p(ctx, prec, state, p, r, v, st);
         if (e != HR_OK) return e;
-        e = dhat_launches(ctx, m0, 0, v, p, tmp, links, nullptr, nullptr, done, st);                       // v = Dhat p
+        e = op(v, p, false, nullptr, done);                                                                  // v = Op p
         if (e != HR_OK) return e;
         e = launch_dot(ctx, prec, rhat, v, rs, bicgstab_rhat_v(state), st);                                 // <rhat, v>
         if (e != HR_OK) return e;
         e = launch_bi_update_s(ctx, prec, state, s, r, v, st);
         if (e != HR_OK) return e;
-        e = dhat_launches(ctx, m0, 0, t, s, tmp, links, &rs, bicgstab_tt_st(state), done, st);             // t = Dhat s, |t|^2, <s,t>
+        e = op(t, s, true, bicgstab_tt_st(state), done);                                                    // t = Op s, |t|^2, <s,t>
         if (e != HR_OK) return e;
         return launch_bi_update_xr(ctx, prec, state, x_e, r, p, s, t, rhat, rs, st);
     };
@@ -330,6 +333,126 @@ hr_status hr_bicgstab_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, c
         *rel_res2 = bb > 0 ? last / bb : 0.0;
     }
     return HR_OK;
+}
+
+// Dhat_sw = A_ee - Dphi_eo A_oo^{-1} Dphi_oe (reading C32): 2 Dphi launches + 2 site-local launches
+static hr_status dhat_clover_launches(const hr_ctx *c, void *out_e, const void *in_e, void *tmp_o, void *tmp2_o,
+                                      const hr_gauge *links, const void *site, const void *site_inv, const int *skip, cudaStream_t st)
+{
+    const size_t chalf = (size_t)c->Vh * clover_nreal(c) * prec_bytes(links->prec);
+    const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 };
+    DphiArgs a;
+    dphi_args(a, c, tmp_o, in_e, nullptr, links, 1, zero, mhalf);
+    a.skip = skip;
+    hr_status rc = launch_dphi(c, links->prec, a, st, link_src(links));                                     // tmp = Dphi_oe in
+    if (rc != HR_OK) return rc;
+    rc = launch_clover_apply(c, links->prec, tmp2_o, tmp_o, (const char *)site_inv + chalf, st, 0);        // tmp2 = A_oo^{-1} tmp
+    if (rc != HR_OK) return rc;
+    dphi_args(a, c, out_e, tmp2_o, nullptr, links, 0, zero, mhalf);
+    a.skip = skip;
+    rc = launch_dphi(c, links->prec, a, st, link_src(links));                                               // out = Dphi_eo tmp2
+    if (rc != HR_OK) return rc;
+    return launch_clover_apply(c, links->prec, out_e, in_e, site, st, -1);                                  // out = A_ee in - out
+}
+
+extern "C" {
+
+hr_status hr_bicgstab_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol, int maxiter,
+                           void *workspace, int *iters, double *rel_res2, double *hist, void *stream)
+{
+    hr_status rc = cg_check("hr_bicgstab_dhat", ctx, x_e, b_e, links, tol, maxiter, workspace);
+    if (rc != HR_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    char *ws = (char *)workspace;
+    const size_t sb = (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(links->prec);
+    void *tmp = ws + 6 * sb;
+    RedScratch rs;
+    rc = get_red_scratch(ctx, &rs, st);
+    if (rc != HR_OK) return rc;
+    BiOp op = [&](void *out, const void *in, bool reduce, double *red, const int *skip) -> hr_status {
+        return dhat_launches(ctx, m0, 0, out, in, tmp, links, reduce ? &rs : nullptr, red, skip, st);
+    };
+    return bicgstab_core(ctx, links->prec, x_e, b_e, tol, maxiter, ws, ws + 7 * sb, op, iters, rel_res2, hist, st);
+}
+
+hr_status hr_clover_finalize(const hr_ctx *ctx, hr_prec prec, void *site_term, void *site_inverse, double m0, void *stream)
+{
+    if (!ctx || !site_term || !site_inverse || !valid_prec(prec) || site_term == site_inverse) { set_error("hr_clover_finalize: bad argument"); return HR_EINVAL; }
+    if (!aligned16(site_term) || !aligned16(site_inverse)) { set_error("hr_clover_finalize: buffers must be 16-byte aligned"); return HR_EINVAL; }
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    return launch_clover_finalize(ctx, prec, site_term, site_inverse, 4.0 + m0, (cudaStream_t)stream);
+}
+
+hr_status hr_dhat_clover(void *out_e, const void *in_e, void *tmp_o, void *tmp2_o, const hr_gauge *links, const void *site_term,
+                         const void *site_inverse, void *stream)
+{
+    if (!out_e || !in_e || !tmp_o || !tmp2_o || !links || !site_term || !site_inverse) { set_error("hr_dhat_clover: NULL argument"); return HR_EINVAL; }
+    if (dphi_link_kind(links->ctx, link_src(links)) < 0) { set_error("hr_dhat_clover: no kernel for this kind of link field"); return HR_EINVAL; }
+    if (out_e == in_e || out_e == tmp_o || out_e == tmp2_o || in_e == tmp_o || in_e == tmp2_o || tmp_o == tmp2_o) {
+        set_error("hr_dhat_clover: out, in and the two temporaries must be distinct buffers");
+        return HR_EINVAL;
+    }
+    if (!aligned16(out_e) || !aligned16(in_e) || !aligned16(tmp_o) || !aligned16(tmp2_o) || !aligned16(site_term) || !aligned16(site_inverse)) {
+        set_error("hr_dhat_clover: buffers must be 16-byte aligned");
+        return HR_EINVAL;
+    }
+    hr_status rc = use_device(links->ctx);
+    if (rc != HR_OK) return rc;
+    return dhat_clover_launches(links->ctx, out_e, in_e, tmp_o, tmp2_o, links, site_term, site_inverse, nullptr, (cudaStream_t)stream);
+}
+
+size_t hr_clover_solve_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter)
+{
+    if (!ctx || !valid_prec(prec) || maxiter < 0) return 0;
+    return 8 * (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec) + bicgstab_state_bytes(maxiter);
+}
+
+hr_status hr_dirac_clover_solve(hr_ctx *ctx, void *x_full, const void *b_full, const hr_gauge *links, const void *site_term,
+                                const void *site_inverse, double tol, int maxiter, void *workspace, int *iters, double *rel_res2,
+                                void *stream)
+{
+    hr_status rc = cg_check("hr_dirac_clover_solve", ctx, x_full, b_full, links, tol, maxiter, workspace);
+    if (rc != HR_OK) return rc;
+    if (!site_term || !site_inverse || !aligned16(site_term) || !aligned16(site_inverse)) { set_error("hr_dirac_clover_solve: bad site-term buffers"); return HR_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const hr_prec prec = links->prec;
+    char *ws = (char *)workspace;
+    const size_t sb = (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec);
+    const size_t chalf = (size_t)ctx->Vh * clover_nreal(ctx) * prec_bytes(prec);
+    void *tmp = ws + 6 * sb, *tmp2 = ws + 7 * sb, *state = ws + 8 * sb;
+    char *x_e = (char *)x_full, *x_o = (char *)x_full + sb;
+    const char *b_e = (const char *)b_full, *b_o = (const char *)b_full + sb;
+    const char *ainv_o = (const char *)site_inverse + chalf;
+    const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 }, one[2] = { 1.0, 0.0 }, mone[2] = { -1.0, 0.0 };
+    RedScratch rs;
+    rc = get_red_scratch(ctx, &rs, st);
+    if (rc != HR_OK) return rc;
+    // reading C32: bhat = b_e - Dphi_eo A_oo^{-1} b_o, kept in the x_o slot until the end
+    rc = launch_clover_apply(ctx, prec, tmp2, b_o, ainv_o, st, 0);
+    if (rc != HR_OK) return rc;
+    DphiArgs a;
+    dphi_args(a, ctx, x_o, tmp2, nullptr, links, 0, zero, mhalf);
+    rc = launch_dphi(ctx, prec, a, st, link_src(links));
+    if (rc != HR_OK) return rc;
+    rc = launch_lincomb(ctx, prec, x_o, one, 0, b_e, mone, x_o, st);
+    if (rc != HR_OK) return rc;
+    BiOp op = [&](void *out, const void *in, bool reduce, double *red, const int *skip) -> hr_status {
+        hr_status e = dhat_clover_launches(ctx, out, in, tmp, tmp2, links, site_term, site_inverse, skip, st);
+        if (e != HR_OK || !reduce) return e;
+        e = launch_dot(ctx, prec, out, out, rs, red, st);          // red[0] = |out|^2 (red[1] = 0, overwritten next)
+        if (e != HR_OK) return e;
+        return launch_dot(ctx, prec, in, out, rs, red + 1, st);    // red[1..2] = <in, out>
+    };
+    rc = bicgstab_core(ctx, prec, x_e, x_o, tol, maxiter, ws, state, op, iters, rel_res2, nullptr, st);
+    if (rc != HR_OK) return rc;
+    // x_o = A_oo^{-1} (b_o - Dphi_oe x_e)
+    dphi_args(a, ctx, tmp, x_e, nullptr, links, 1, zero, mhalf);
+    rc = launch_dphi(ctx, prec, a, st, link_src(links));
+    if (rc != HR_OK) return rc;
+    rc = launch_lincomb(ctx, prec, tmp, one, 0, b_o, mone, tmp, st);
+    if (rc != HR_OK) return rc;
+    return launch_clover_apply(ctx, prec, x_o, tmp, ainv_o, st, 0);
 }
 
 hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links, double tol,

@@ -150,7 +150,9 @@ hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, const HaloArgs &
 size_t clover_nreal(const hr_ctx *c);
 hr_status launch_clover_build(const hr_ctx *c, hr_prec prec, void *clover, const void *links, double csw, cudaStream_t st);
 hr_status launch_clover_exp(const hr_ctx *c, hr_prec prec, void *clover, double m, cudaStream_t st);
-hr_status launch_clover_apply(const hr_ctx *c, hr_prec prec, void *out, const void *in, const void *clover_parity, cudaStream_t st);
+hr_status launch_clover_apply(const hr_ctx *c, hr_prec prec, void *out, const void *in, const void *clover_parity, cudaStream_t st,
+                              int mode = 1);
+hr_status launch_clover_finalize(const hr_ctx *c, hr_prec prec, void *clover, void *inverse, double m, cudaStream_t st);
 
 hr_status launch_represent(const hr_ctx *c, hr_prec in_prec, const void *fund, hr_prec out_prec, void *repr,
                            cudaStream_t st);

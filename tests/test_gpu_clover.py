@@ -177,3 +177,77 @@ def test_dirac_expclover_matches_oracle(hr, N, rep, prec):
     with pytest.raises(hr.HrError):
         hr.hr_clover_exp(lat.ctx, P, cl, -4.5, lat.stream())            # 4 + m0 <= 0
     prob.close()
+
+
+@pytest.mark.parametrize("exponentiated", [False, True])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("N,rep", [(3, "fund"), (2, "adj"), (3, "sym")])
+def test_dhat_clover_matches_oracle(hr, N, rep, prec, exponentiated):
+    """Reading C32: Dhat_sw = A_ee - Dphi_eo A_oo^{-1} Dphi_oe with A from hr_clover_build [+ hr_clover_exp] +
+    hr_clover_finalize, against the oracle (dense per-site blocks, numpy.linalg.solve for A^{-1})."""
+    import torch
+    dims = (4, 4, 2, 6)
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(421, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    V = li.volume(dims)
+    psi = li.gaussian_spinor(422, V // 2, d)
+    m0, csw = -0.3, 1.1
+    want = clover.dhat_clover(dims, BC_T, R, m0, csw, psi, exponentiated)
+    prob = GpuProblem(hr, dims, N, rep, prec, U)
+    lat, P = prob.lat, prob.prec
+    nb = hr.hr_clover_bytes(lat.ctx, P)
+    A = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    Ainv = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    Ainv.fill_(0xFF)
+    hr.hr_clover_build(A, prob.links, csw, lat.stream())
+    if exponentiated:
+        hr.hr_clover_exp(lat.ctx, P, A, m0, lat.stream())
+    hr.hr_clover_finalize(lat.ctx, P, A, Ainv, m0, lat.stream())
+    gin = lat.spinor(P)
+    lat.import_spinor(gin, P, psi, 0)
+    out, t1, t2 = lat.spinor(P), lat.spinor(P), lat.spinor(P)
+    out.fill_(0xFF)
+    n0 = hr.hr_launch_count()
+    hr.hr_dhat_clover(out, gin, t1, t2, prob.links, A, Ainv, lat.stream())
+    assert hr.hr_launch_count() == n0 + 4
+    # fp32: A^{-1} amplifies the input rounding by the condition number of the blocks (a few units here)
+    assert rel_l2(lat.export_spinor(out, P, 0), want) <= (TOL[prec] if prec == "f64" else 5 * TOL[prec])
+    with pytest.raises(hr.HrError):
+        hr.hr_dhat_clover(out, gin, t1, t1, prob.links, A, Ainv, lat.stream())
+    prob.close()
+
+
+@pytest.mark.parametrize("exponentiated", [False, True])
+@pytest.mark.parametrize("N,rep", [(3, "fund"), (2, "adj")])
+def test_dirac_clover_solve_inverts_the_oracles_operator(hr, N, rep, exponentiated):
+    import torch
+    dims = (4, 4, 4, 4)
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(431, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    V = li.volume(dims)
+    b = li.gaussian_spinor(432, V, d)
+    m0, csw = -0.2, 1.0
+    x_want, it_want = clover.dirac_clover_solve(dims, BC_T, R, m0, csw, b, 1e-11, 500, exponentiated)
+    prob = GpuProblem(hr, dims, N, rep, "f64", U)
+    lat, P = prob.lat, prob.prec
+    nb = hr.hr_clover_bytes(lat.ctx, P)
+    A = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    Ainv = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    hr.hr_clover_build(A, prob.links, csw, lat.stream())
+    if exponentiated:
+        hr.hr_clover_exp(lat.ctx, P, A, m0, lat.stream())
+    hr.hr_clover_finalize(lat.ctx, P, A, Ainv, m0, lat.stream())
+    gb = _full(prob, b)
+    gx = lat.spinor(P, full=True)
+    gx.fill_(0xFF)
+    ws = torch.empty(hr.hr_clover_solve_workspace_bytes(lat.ctx, P, 500), dtype=torch.uint8, device="cuda")
+    it, res2 = hr.hr_dirac_clover_solve(lat.ctx, gx, gb, prob.links, A, Ainv, 1e-11, 500, ws, lat.stream())
+    assert abs(it - it_want) <= 2 and res2 <= 1e-22
+    x = _get_full(prob, gx)
+    assert rel_l2(x, x_want) <= 1e-9
+    # the oracle's full operator applied to the GPU's solution gives back b
+    Dx = clover.dirac_expclover(dims, BC_T, R, m0, csw, x) if exponentiated else clover.dirac_clover(dims, BC_T, R, m0, csw, x)
+    assert rel_l2(Dx, b) <= 1e-9
+    prob.close()
