@@ -115,6 +115,15 @@ def main():
     ops.append(("clover_build (per site of the FULL lattice: 4L + C)", 2 * (4 * L + Cb), lambda k: hr.hr_clover_build(cl, links, 1.0, st)))
     ops.append(("dirac (both parities: 2(8L+3S) per site pair)", 2 * (dphi_c + S), lambda k: hr.hr_dirac(args.m0, full_out, full_in, links, st)))
     ops.append(("dirac_clover (both parities: 2(8L+3S + C+3S))", 2 * (dphi_c + S + Cb + 3 * S), lambda k: hr.hr_dirac_clover(args.m0, full_out, full_in, links, cl, st)))
+    # even-odd preconditioned clover operator: 2 Dphi + 2 site-local launches;
+    # algorithmic bytes per even site: 2(8L+2S) + (C+2S) + (C+3S)
+    Ainv = torch.empty(hr.hr_clover_bytes(ctx, P), dtype=torch.uint8, device="cuda")
+    Asite = torch.empty(hr.hr_clover_bytes(ctx, P), dtype=torch.uint8, device="cuda")
+    hr.hr_clover_build(Asite, links, 1.0, st)
+    hr.hr_clover_finalize(ctx, P, Asite, Ainv, args.m0, st)
+    t2 = lat.spinor(P)
+    ops.append(("dhat_clover", 2 * dphi_c + 2 * Cb + 5 * S,
+                lambda k: hr.hr_dhat_clover(sets[k % nset][2], sets[k % nset][0], sets[k % nset][1], t2, links, Asite, Ainv, st)))
     common = {"workload": cfg["name"], "dtype": args.prec, "peak_gbs": peak, "peak_source": peak_src, "sites": vh}
     for name, bps, fn in ops:
         ms = timed(fn, args.reps)
