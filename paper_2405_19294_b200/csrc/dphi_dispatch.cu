@@ -83,6 +83,17 @@ hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, const HaloArgs &
     return HR_EUNSUPPORTED;
 }
 
+// can a launch with this link source carry a fused site matrix (DphiArgs::site_mode)?
+bool dphi_site_fusable(const hr_ctx *c, hr_prec prec, int link_src)
+{
+    const int lk = dphi_link_kind(c, link_src);
+    // measured: fp64 d_R = 3 gains 18-30 %; fp32 (128-register cap) is no faster fused, and at
+    // d_R >= 6 the block mat-vec spills in a kernel already at 255 registers
+    if ((lk != 0 && lk != 1) || c->d > 4 || prec != HR_F64) return false;
+    const int v = resolve_variant(c, prec, lk);
+    return v == 0 || v == 1;
+}
+
 bool dphi_variant_valid(const hr_ctx *c, int variant)
 {
     if (variant == -1) return true;

@@ -350,6 +350,43 @@ template <typename Real> __device__ __forceinline__ Real coef_beta(const DphiArg
 template <> __device__ __forceinline__ double coef_beta<double>(const DphiArgs &a, int i) { return a.beta[i]; }
 template <> __device__ __forceinline__ float coef_beta<float>(const DphiArgs &a, int i) { return a.betaf[i]; }
 
+// w += M v for the site-diagonal matrix M of one site (two packed Hermitian 2D x 2D blocks, clover.cu layout), streamed
+// one 16-byte vector at a time; v, w: the site's spinor [spin][colour] (re, im)
+template <typename Real, int D>
+__device__ __forceinline__ void site_matvec(Real (&w)[8 * D], const Real (&v)[8 * D], const char *mat, size_t vh, size_t s)
+{
+    constexpr int BLK = 4 * D * D, N2 = 2 * D, RPV = 16 / (int)sizeof(Real), NVB = BLK / RPV;
+    const size_t pb = vh * 16;
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+        const char *tp = mat + s * 16 + (size_t)(b * NVB) * pb;
+        const int o = b * 2 * N2;
+        Real tv[RPV];
+        int idx = 0;
+        auto next = [&]() -> Real {
+            if (idx % RPV == 0) load_planes<LD_STREAM, 1>(tv, tp + (size_t)(idx / RPV) * pb, pb, 0);
+            return tv[idx++ % RPV];
+        };
+#pragma unroll
+        for (int d = 0; d < N2; ++d) {
+            const Real t = next();
+            w[o + 2 * d] = fma(t, v[o + 2 * d], w[o + 2 * d]);
+            w[o + 2 * d + 1] = fma(t, v[o + 2 * d + 1], w[o + 2 * d + 1]);
+        }
+#pragma unroll
+        for (int r = 0; r < N2; ++r)
+#pragma unroll
+            for (int c = r + 1; c < N2; ++c) {
+                const Real re = next();
+                const Real im = next();
+                w[o + 2 * r] = fma(re, v[o + 2 * c], fma(-im, v[o + 2 * c + 1], w[o + 2 * r]));
+                w[o + 2 * r + 1] = fma(re, v[o + 2 * c + 1], fma(im, v[o + 2 * c], w[o + 2 * r + 1]));
+                w[o + 2 * c] = fma(re, v[o + 2 * r], fma(im, v[o + 2 * r + 1], w[o + 2 * c]));
+                w[o + 2 * c + 1] = fma(re, v[o + 2 * r + 1], fma(-im, v[o + 2 * r], w[o + 2 * c + 1]));
+            }
+    }
+}
+
 struct SiteGeom {
     int t, x, y, zh, b; // b = offset bit: z = 2*zh + b
 };
@@ -385,10 +422,13 @@ __device__ __forceinline__ void neighbour(const DphiArgs &a, const SiteGeom &g, 
 // MASS: the epilogue reads self = psi(x) on the output parity (alpha term); RED: the epilogue also
 // reduces sum |out|^2 and <self, out> over the launch (needs MASS) -- what a CG on gamma5 Dhat needs
 // from its operator, with no extra pass over the fields.
-template <typename Real, int D, int LK, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT, int MAXT, int MINB>
+// CLV: a site-diagonal matrix fused into the epilogue (DphiArgs::site_mode): 1 adds M self (needs MASS), 2 applies M to
+// the scaled hop sum; one-thread-per-site kernels only.
+template <typename Real, int D, int LK, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT, int MAXT, int MINB, int CLV = 0>
 __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
 {
     static_assert(!RED || MASS, "the fused reduction needs the self field");
+    static_assert(CLV == 0 || (KSPLIT == 1 && !RED && (CLV != 1 || MASS) && (CLV != 2 || !MASS)), "fused site matrix: site kernels only");
     if (a.skip != nullptr && *a.skip != 0) return;
     constexpr int LNREAL = LinkGeom<LK, D>::NREAL;         // reals per link record read by the kernel
     constexpr int RPV = 16 / (int)sizeof(Real);
@@ -471,6 +511,7 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
             for (int al = 0; al < 4; ++al)
 #pragma unroll
                 for (int c = 0; c < 2 * D; ++c) o[al * 2 * D + c] = fma(al_[al >> 1], self[al * 2 * D + c], be[al >> 1] * acc[al][c]);
+            if constexpr (CLV == 1) site_matvec<Real, D>(o, self, (const char *)a.site_mat, vh, (size_t)s);
             if constexpr (RED) {
 #pragma unroll
                 for (int e = 0; e < 4 * D; ++e) {
@@ -485,6 +526,12 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
             for (int al = 0; al < 4; ++al)
 #pragma unroll
                 for (int c = 0; c < 2 * D; ++c) o[al * 2 * D + c] = (Real)-0.5 * acc[al][c]; // plain Dphi
+            if constexpr (CLV == 2) {
+                Real hv[8 * D];
+#pragma unroll
+                for (int e = 0; e < 8 * D; ++e) { hv[e] = o[e]; o[e] = 0; }
+                site_matvec<Real, D>(o, hv, (const char *)a.site_mat, vh, (size_t)s);
+            }
         }
         if (live) store_planes<STHINT, 8 * D / RPV>((char *)a.out + (size_t)s * 16, pb, o);
         if constexpr (RED) {

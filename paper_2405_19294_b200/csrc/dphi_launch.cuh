@@ -35,7 +35,7 @@ template <typename Real, int D, int LK, int KSPLIT> struct Tune {
                                 LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? 4 : LIVE <= 150 ? 3 : LIVE <= 255 ? 2 : 1;
 };
 
-template <typename Real, int D, int LK, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT>
+template <typename Real, int D, int LK, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT, int CLV = 0>
 static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
 {
     using T = Tune<Real, D, LK, KSPLIT>;
@@ -52,7 +52,7 @@ static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
         set_error("fused Dphi reduction: %ld CTAs exceed the reduction scratch (%u)", grid, kRedMaxBlocks);
         return HR_EUNSUPPORTED;
     }
-    dphi_kernel<Real, D, LK, KSPLIT, MASS, RED, LHINT, SHINT, STHINT, T::MAXT, T::MINB><<<(unsigned)grid, block, 0, st>>>(a);
+    dphi_kernel<Real, D, LK, KSPLIT, MASS, RED, LHINT, SHINT, STHINT, T::MAXT, T::MINB, CLV><<<(unsigned)grid, block, 0, st>>>(a);
     count_launch();
     cudaError_t e = cudaPeekAtLastError();
     if (e != cudaSuccess) {
@@ -115,6 +115,21 @@ static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaS
 template <typename Real, int D, int LK>
 hr_status launch_dphi_t(int variant, int block, const DphiArgs &a, cudaStream_t st)
 {
+    if (a.site_mode != 0) {
+        // fused site-diagonal matrix: the `site` / `site_ef` kernels only, complex-link kinds with a clover field
+        if constexpr (LK == LK_COMPLEX || LK == LK_REAL) {
+            if (a.site_mode == 1 && a.self && !a.red_result) {
+                if (variant == 0) return launch_one<Real, D, LK, 1, true, false, LD_STREAM, LD_DEFAULT, ST_DEFAULT, 1>(block, a, st);
+                if (variant == 1) return launch_one<Real, D, LK, 1, true, false, LD_STREAM_EF, LD_KEEP, ST_STREAM, 1>(block, a, st);
+            }
+            if (a.site_mode == 2 && !a.self) {
+                if (variant == 0) return launch_one<Real, D, LK, 1, false, false, LD_STREAM, LD_DEFAULT, ST_DEFAULT, 2>(block, a, st);
+                if (variant == 1) return launch_one<Real, D, LK, 1, false, false, LD_STREAM_EF, LD_KEEP, ST_STREAM, 2>(block, a, st);
+            }
+        }
+        set_error("fused site matrix: not available for this kernel variant / link kind");
+        return HR_EUNSUPPORTED;
+    }
     if (a.self && a.red_result) return launch_variant<Real, D, LK, true, true>(variant, block, a, st);
     if (a.self) return launch_variant<Real, D, LK, true, false>(variant, block, a, st);
     return launch_variant<Real, D, LK, false, false>(variant, block, a, st);

@@ -366,6 +366,8 @@ void dphi_args(DphiArgs &a, const hr_ctx *c, void *out, const void *in, const vo
     a.red_ticket = nullptr;
     a.red_result = nullptr;
     a.skip = nullptr;
+    a.site_mat = nullptr;
+    a.site_mode = 0;
 }
 
 // Reduction scratch of the ctx: [3 * kRedMaxBlocks doubles of per-CTA partials][16 doubles of results][ticket].

@@ -340,8 +340,22 @@ static hr_status dhat_clover_launches(const hr_ctx *c, void *out_e, const void *
                                       const hr_gauge *links, const void *site, const void *site_inv, const int *skip, cudaStream_t st)
 {
     const size_t chalf = (size_t)c->Vh * clover_nreal(c) * prec_bytes(links->prec);
-    const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 };
+    const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 }, phalf[2] = { 0.5, 0.5 };
     DphiArgs a;
+    if (links->represented == 1 && dphi_site_fusable(c, links->prec, link_src(links))) {
+        // both site-local steps fused into the Dphi epilogues: tmp2 = A_oo^{-1} (Dphi_oe in); out = A_ee in - Dphi_eo tmp2
+        dphi_args(a, c, tmp2_o, in_e, nullptr, links, 1, zero, mhalf);
+        a.skip = skip;
+        a.site_mat = (const char *)site_inv + chalf;
+        a.site_mode = 2;
+        hr_status rc = launch_dphi(c, links->prec, a, st, link_src(links));
+        if (rc != HR_OK) return rc;
+        dphi_args(a, c, out_e, tmp2_o, in_e, links, 0, zero, phalf);     // 0 * in + 1/2 hops (= -Dphi) + A_ee in
+        a.skip = skip;
+        a.site_mat = site;
+        a.site_mode = 1;
+        return launch_dphi(c, links->prec, a, st, link_src(links));
+    }
     dphi_args(a, c, tmp_o, in_e, nullptr, links, 1, zero, mhalf);
     a.skip = skip;
     hr_status rc = launch_dphi(c, links->prec, a, st, link_src(links));                                     // tmp = Dphi_oe in

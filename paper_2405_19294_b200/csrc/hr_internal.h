@@ -93,6 +93,10 @@ struct DphiArgs {
     unsigned *red_ticket;  // zero before the launch; the last CTA resets it
     double *red_result;    // [3], device
     const int *skip;       // if non-null and *skip != 0 the launch does nothing (converged CG)
+    // fused site-diagonal matrix (clover.cu layout: two packed Hermitian 2 d_R x 2 d_R blocks per site, output parity):
+    // site_mode 1: out = alpha self + beta hops + M self;  2: out = M (beta hops);  0: none.  One-thread-per-site kernels.
+    const void *site_mat;
+    int site_mode;
 };
 
 // device-resident state of the CG (cg.cu); the host only reads it
@@ -125,6 +129,7 @@ hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStre
 int dphi_link_kind(const hr_ctx *c, int link_src); // -1: no such kernel
 static inline int link_src(const hr_gauge *g) { return g->represented == 1 ? 0 : g->represented == 0 ? 1 : 2; }
 hr_status launch_compress(const hr_ctx *c, hr_prec prec, void *rows, const void *fund, cudaStream_t st);
+bool dphi_site_fusable(const hr_ctx *c, hr_prec prec, int link_src);
 const char *dphi_variant_name(const hr_ctx *c, hr_prec prec);
 bool dphi_variant_valid(const hr_ctx *c, int variant);
 

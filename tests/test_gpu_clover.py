@@ -65,7 +65,7 @@ def test_dirac_clover_matches_oracle(hr, dims, N, rep, prec):
     gout.fill_(0xFF)
     n0 = hr.hr_launch_count()
     hr.hr_dirac_clover(m0, gout, gin, prob.links, cl, lat.stream())
-    assert hr.hr_launch_count() == n0 + 4                               # 2 Dphi launches + 2 site-local launches
+    assert hr.hr_launch_count() - n0 in (2, 4)                          # fused into the Dphi epilogues where d_R <= 4
     got = _get_full(prob, gout)
     want = clover.dirac_clover(dims, BC_T, R, m0, csw, psi)
     assert rel_l2(got, want) <= TOL[prec]
@@ -210,7 +210,7 @@ def test_dhat_clover_matches_oracle(hr, N, rep, prec, exponentiated):
     out.fill_(0xFF)
     n0 = hr.hr_launch_count()
     hr.hr_dhat_clover(out, gin, t1, t2, prob.links, A, Ainv, lat.stream())
-    assert hr.hr_launch_count() == n0 + 4
+    assert hr.hr_launch_count() - n0 in (2, 4)
     # fp32: A^{-1} amplifies the input rounding by the condition number of the blocks (a few units here)
     assert rel_l2(lat.export_spinor(out, P, 0), want) <= (TOL[prec] if prec == "f64" else 5 * TOL[prec])
     with pytest.raises(hr.HrError):
@@ -250,4 +250,38 @@ def test_dirac_clover_solve_inverts_the_oracles_operator(hr, N, rep, exponentiat
     # the oracle's full operator applied to the GPU's solution gives back b
     Dx = clover.dirac_expclover(dims, BC_T, R, m0, csw, x) if exponentiated else clover.dirac_clover(dims, BC_T, R, m0, csw, x)
     assert rel_l2(Dx, b) <= 1e-9
+    prob.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2, 4])
+def test_fused_and_unfused_clover_paths_agree(hr, variant):
+    """hr_dirac_clover / hr_dhat_clover fuse the site-diagonal matrix into the Dphi epilogue for the `site` / `site_ef`
+    kernels (d_R <= 4) and fall back to separate site-local launches otherwise: same operator either way."""
+    import torch
+    dims, N, rep, m0, csw = (4, 4, 2, 6), 3, "fund", -0.3, 1.1
+    U = li.haar_links(441, N, dims)
+    V = li.volume(dims)
+    psi = li.gaussian_spinor(442, V, 3)
+    prob = GpuProblem(hr, dims, N, rep, "f64", U)
+    lat, P = prob.lat, prob.prec
+    lat.set_tuning("variant", variant)
+    nb = hr.hr_clover_bytes(lat.ctx, P)
+    T = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    A = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    Ainv = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    hr.hr_clover_build(T, prob.links, csw, lat.stream())
+    A.copy_(T)
+    hr.hr_clover_finalize(lat.ctx, P, A, Ainv, m0, lat.stream())
+    gin = _full(prob, psi)
+    gout = lat.spinor(P, full=True)
+    n0 = hr.hr_launch_count()
+    hr.hr_dirac_clover(m0, gout, gin, prob.links, T, lat.stream())
+    assert hr.hr_launch_count() - n0 == (2 if variant in (0, 1) else 4)
+    assert rel_l2(_get_full(prob, gout), clover.dirac_clover(dims, BC_T, U, m0, csw, psi)) <= TOL["f64"]
+    half = hr.hr_spinor_bytes(lat.ctx, P)
+    out, t1, t2 = lat.spinor(P), lat.spinor(P), lat.spinor(P)
+    n0 = hr.hr_launch_count()
+    hr.hr_dhat_clover(out, gin[:half], t1, t2, prob.links, A, Ainv, lat.stream())
+    assert hr.hr_launch_count() - n0 == (2 if variant in (0, 1) else 4)
+    assert rel_l2(lat.export_spinor(out, P, 0), clover.dhat_clover(dims, BC_T, U, m0, csw, psi[:V // 2])) <= TOL["f64"]
     prob.close()
