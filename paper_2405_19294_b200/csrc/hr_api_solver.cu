@@ -274,7 +274,7 @@ size_t hr_bicgstab_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter)
 // The operator of a BiCGstab run: out = Op in.  reduce: also leave |out|^2 and <in, out> in red[0..2] (the Dphi
 // epilogue does it for Dhat; operators that end in another kernel use two dot launches).  skip: device flag, non-zero =
 // converged (kernels that know about it return at once).
-typedef std::function<hr_status(void *out, const void *in, bool reduce, double *red, const int *skip)> BiOp;
+typedef std::function<hr_status(void *out, const void *in, bool reduce, double *red, const int *skip, cudaStream_t q)> BiOp;
 
 // textbook BiCGstab on device-resident scalars (bicgstab.cu); ws holds r, rhat, p, v, s, t (6 half spinors) and the state
 static hr_status bicgstab_core(hr_ctx *ctx, hr_prec prec, void *x_e, const void *b_e, double tol, int maxiter, char *ws,
@@ -288,19 +288,40 @@ static hr_status bicgstab_core(hr_ctx *ctx, hr_prec prec, void *x_e, const void 
     rc = launch_bi_init(ctx, prec, state, tol, maxiter, x_e, r, rhat, p, v, b_e, rs, st);
     if (rc != HR_OK) return rc;
     const int *done = bicgstab_done(state);
-    auto one_iteration = [&]() -> hr_status {
-        hr_status e = launch_bi_update_p(ctx, prec, state, p, r, v, st);
+    auto one_iteration = [&](cudaStream_t q) -> hr_status {
+        hr_status e = launch_bi_update_p(ctx, prec, state, p, r, v, q);
         if (e != HR_OK) return e;
-        e = op(v, p, false, nullptr, done);                                                                  // v = Op p
+        e = op(v, p, false, nullptr, done, q);                                                               // v = Op p
         if (e != HR_OK) return e;
-        e = launch_dot(ctx, prec, rhat, v, rs, bicgstab_rhat_v(state), st);                                 // <rhat, v>
+        e = launch_dot(ctx, prec, rhat, v, rs, bicgstab_rhat_v(state), q);                                  // <rhat, v>
         if (e != HR_OK) return e;
-        e = launch_bi_update_s(ctx, prec, state, s, r, v, st);
+        e = launch_bi_update_s(ctx, prec, state, s, r, v, q);
         if (e != HR_OK) return e;
-        e = op(t, s, true, bicgstab_tt_st(state), done);                                                    // t = Op s, |t|^2, <s,t>
+        e = op(t, s, true, bicgstab_tt_st(state), done, q);                                                 // t = Op s, |t|^2, <s,t>
         if (e != HR_OK) return e;
-        return launch_bi_update_xr(ctx, prec, state, x_e, r, p, s, t, rhat, rs, st);
+        return launch_bi_update_xr(ctx, prec, state, x_e, r, p, s, t, rhat, rs, q);
     };
+    // as in the CG: an iteration is host-invariant, so on small lattices it is captured once and replayed as a graph
+    cudaGraphExec_t gexec = nullptr;
+    int launches_per_iteration = 0;
+    if (ctx->cg_graph == 2 || (ctx->cg_graph == 1 && ctx->Vh <= (1L << 19))) {
+        cudaStream_t cap = nullptr;
+        cudaGraph_t graph = nullptr;
+        const unsigned long long before = hr_launch_count();
+        bool ok = cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) == cudaSuccess;
+        if (ok) ok = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+        if (ok) {
+            const hr_status e = one_iteration(cap);
+            const cudaError_t ce = cudaStreamEndCapture(cap, &graph);
+            ok = e == HR_OK && ce == cudaSuccess && graph != nullptr;
+        }
+        if (ok) ok = cudaGraphInstantiate(&gexec, graph, 0) == cudaSuccess;
+        if (graph) cudaGraphDestroy(graph);
+        if (cap) cudaStreamDestroy(cap);
+        launches_per_iteration = (int)(hr_launch_count() - before);
+        count_launch(-launches_per_iteration); // captured, not launched
+        if (!ok) { gexec = nullptr; cudaGetLastError(); }
+    }
     alignas(8) char hbuf[256];
     const size_t hb = bicgstab_header_bytes();
     int it = 0, dn = 0;
@@ -313,12 +334,19 @@ static hr_status bicgstab_core(hr_ctx *ctx, hr_prec prec, void *x_e, const void 
         if (dn || issued >= maxiter) break;
         const int n = maxiter - issued < batch ? maxiter - issued : batch;
         for (int i = 0; i < n; ++i) {
-            rc = one_iteration();
-            if (rc != HR_OK) return rc;
+            if (gexec) {
+                const cudaError_t ce = cudaGraphLaunch(gexec, st);
+                if (ce != cudaSuccess) { cudaGraphExecDestroy(gexec); return cuda_fail("cudaGraphLaunch (BiCGstab iteration)", ce); }
+                count_launch(launches_per_iteration);
+            } else {
+                rc = one_iteration(st);
+                if (rc != HR_OK) return rc;
+            }
         }
         issued += n;
         if (batch < 32) batch *= 2;
     }
+    if (gexec) cudaGraphExecDestroy(gexec);
     if (iters) *iters = it;
     const double *dh = (const double *)((const char *)state + hb);
     if (hist) {
@@ -383,8 +411,8 @@ hr_status hr_bicgstab_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, c
     RedScratch rs;
     rc = get_red_scratch(ctx, &rs, st);
     if (rc != HR_OK) return rc;
-    BiOp op = [&](void *out, const void *in, bool reduce, double *red, const int *skip) -> hr_status {
-        return dhat_launches(ctx, m0, 0, out, in, tmp, links, reduce ? &rs : nullptr, red, skip, st);
+    BiOp op = [&](void *out, const void *in, bool reduce, double *red, const int *skip, cudaStream_t q) -> hr_status {
+        return dhat_launches(ctx, m0, 0, out, in, tmp, links, reduce ? &rs : nullptr, red, skip, q);
     };
     return bicgstab_core(ctx, links->prec, x_e, b_e, tol, maxiter, ws, ws + 7 * sb, op, iters, rel_res2, hist, st);
 }
@@ -451,12 +479,12 @@ hr_status hr_dirac_clover_solve(hr_ctx *ctx, void *x_full, const void *b_full, c
     if (rc != HR_OK) return rc;
     rc = launch_lincomb(ctx, prec, x_o, one, 0, b_e, mone, x_o, st);
     if (rc != HR_OK) return rc;
-    BiOp op = [&](void *out, const void *in, bool reduce, double *red, const int *skip) -> hr_status {
-        hr_status e = dhat_clover_launches(ctx, out, in, tmp, tmp2, links, site_term, site_inverse, skip, st);
+    BiOp op = [&](void *out, const void *in, bool reduce, double *red, const int *skip, cudaStream_t q) -> hr_status {
+        hr_status e = dhat_clover_launches(ctx, out, in, tmp, tmp2, links, site_term, site_inverse, skip, q);
         if (e != HR_OK || !reduce) return e;
-        e = launch_dot(ctx, prec, out, out, rs, red, st);          // red[0] = |out|^2 (red[1] = 0, overwritten next)
+        e = launch_dot(ctx, prec, out, out, rs, red, q);           // red[0] = |out|^2 (red[1] = 0, overwritten next)
         if (e != HR_OK) return e;
-        return launch_dot(ctx, prec, in, out, rs, red + 1, st);    // red[1..2] = <in, out>
+        return launch_dot(ctx, prec, in, out, rs, red + 1, q);     // red[1..2] = <in, out>
     };
     rc = bicgstab_core(ctx, prec, x_e, x_o, tol, maxiter, ws, state, op, iters, rel_res2, nullptr, st);
     if (rc != HR_OK) return rc;

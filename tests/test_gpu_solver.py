@@ -422,3 +422,24 @@ def test_mixed_precision_bicgstab_reaches_fp64_accuracy(hr, dims, N, rep, m0):
     with pytest.raises(hr.HrError):
         hr.hr_bicgstab_dhat_mixed(lat.ctx, m0, gx, gb, prob.links, l32, 1e-10, 1.5, 500, ws, lat.stream())
     prob.close()
+
+
+def test_bicgstab_graph_replay_is_bitwise_the_plain_launch_sequence(hr):
+    import torch
+    dims, N, m0 = (4, 4, 4, 8), 3, -0.3
+    U = li.haar_links(121, N, dims)
+    b = li.gaussian_spinor(122, li.volume(dims) // 2, 3)
+    prob = GpuProblem(hr, dims, N, "fund", "f64", U)
+    f = Fields(hr, prob)
+    gb = f.put(b)
+    ws = torch.empty(hr.hr_bicgstab_workspace_bytes(prob.lat.ctx, f.P, 200), dtype=torch.uint8, device="cuda")
+    res = {}
+    for mode in (2, 0):
+        prob.lat.set_tuning("cg_graph", mode)
+        gx = f.new()
+        n0 = hr.hr_launch_count()
+        it, res2, hist = hr.hr_bicgstab_dhat(prob.lat.ctx, m0, gx, gb, prob.links, 1e-10, 200, ws, prob.lat.stream(), want_hist=True)
+        res[mode] = (it, res2, hist.copy(), f.get(gx), hr.hr_launch_count() - n0)
+    assert res[0][0] == res[2][0] and res[0][1] == res[2][1] and res[0][4] == res[2][4]
+    assert np.array_equal(res[0][2], res[2][2]) and np.array_equal(res[0][3], res[2][3])
+    prob.close()
