@@ -269,6 +269,20 @@ hr_status hr_dirac_solve_bicgstab(hr_ctx *ctx, double m0, void *x_full, const vo
  * for the two-index representations); all buffers device memory, 16-byte aligned; no synchronisation.
  * ===================================================================================================== */
 size_t hr_halo_bytes(const hr_ctx *ctx, hr_prec prec);
+/*
+ * Peer memory for the messages (the fused projection + transfer of step 2): hr_halo_buffers_alloc makes ONE cudaMalloc
+ * allocation of 6 hr_halo_bytes(): [send_up | send_dn | recv_prev[0] | recv_next[0] | recv_prev[1] | recv_next[1]]
+ * (receive buffers double-buffered by call parity); hr_ipc_export / hr_ipc_open / hr_ipc_close wrap
+ * cudaIpcGetMemHandle / OpenMemHandle / CloseMemHandle (64-byte handle) so that a neighbouring PROCESS -- on another
+ * GPU over NVLink, or on the same GPU -- maps the allocation and passes  peer_base + offset  as the send pointers of
+ * hr_dphi_eo_halo_pack.  Ordering between the neighbour's pack and the own apply is the caller's (halo.py:
+ * PeerSlabDphi uses one barrier per call).
+ */
+hr_status hr_halo_buffers_alloc(const hr_ctx *ctx, hr_prec prec, void **base);
+void hr_halo_buffers_free(const hr_ctx *ctx, void *base);
+hr_status hr_ipc_export(const hr_ctx *ctx, const void *base, unsigned char handle[64]);
+hr_status hr_ipc_open(const hr_ctx *ctx, const unsigned char handle[64], void **peer_base);
+hr_status hr_ipc_close(const hr_ctx *ctx, void *peer_base);
 hr_status hr_dphi_eo_halo_pack(void *send_up, void *send_dn, const void *in, const hr_gauge *links, int parity,
                                void *stream);
 hr_status hr_dphi_eo_interior(void *out, const void *in, const hr_gauge *links, int parity, void *stream);

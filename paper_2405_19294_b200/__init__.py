@@ -84,6 +84,11 @@ _SIGNATURES = {
     "hr_bicgstab_dhat": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp, _vp]),
     "hr_dirac_solve": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
     "hr_halo_bytes": (_sz, [_vp, _ci]),
+    "hr_halo_buffers_alloc": (_ci, [_vp, _ci, ctypes.POINTER(_vp)]),
+    "hr_halo_buffers_free": (None, [_vp, _vp]),
+    "hr_ipc_export": (_ci, [_vp, _vp, ctypes.c_char_p]),
+    "hr_ipc_open": (_ci, [_vp, ctypes.c_char_p, ctypes.POINTER(_vp)]),
+    "hr_ipc_close": (_ci, [_vp, _vp]),
     "hr_dphi_eo_halo_pack": (_ci, [_vp, _vp, _vp, _vp, _ci, _vp]),
     "hr_dphi_eo_interior": (_ci, [_vp, _vp, _vp, _ci, _vp]),
     "hr_dphi_eo_halo_apply": (_ci, [_vp, _vp, _vp, _vp, _ci, _ci, _ci, _vp]),
@@ -324,6 +329,32 @@ def hr_dirac_solve(ctx: int, m0: float, x_full, b_full, links: int, tol: float, 
 
 def hr_halo_bytes(ctx: int, prec: int) -> int:
     return _lib.hr_halo_bytes(ctx, prec)
+
+
+def hr_halo_buffers_alloc(ctx: int, prec: int) -> int:
+    p = _vp()
+    _check(_lib.hr_halo_buffers_alloc(ctx, prec, ctypes.byref(p)))
+    return p.value
+
+
+def hr_halo_buffers_free(ctx: int, base: int) -> None:
+    _lib.hr_halo_buffers_free(ctx, base)
+
+
+def hr_ipc_export(ctx: int, base: int) -> bytes:
+    buf = ctypes.create_string_buffer(64)
+    _check(_lib.hr_ipc_export(ctx, base, buf))
+    return buf.raw
+
+
+def hr_ipc_open(ctx: int, handle: bytes) -> int:
+    p = _vp()
+    _check(_lib.hr_ipc_open(ctx, ctypes.create_string_buffer(bytes(handle), 64), ctypes.byref(p)))
+    return p.value
+
+
+def hr_ipc_close(ctx: int, peer_base: int) -> None:
+    _check(_lib.hr_ipc_close(ctx, peer_base))
 
 
 def hr_dphi_eo_halo_pack(send_up, send_dn, inp, links: int, parity: int, stream: int = 0) -> None:

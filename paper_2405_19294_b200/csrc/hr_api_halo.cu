@@ -1,6 +1,8 @@
 // hr_api_halo.cu -- C-ABI entry points of SURVEY.md section 8(e)/(f) NEXT-2 (include/hr.h, third part):
 // Dphi_eo on a lattice split into slabs along t, one slab per GPU, half-spinor messages.
 // Argument checking and launch sequencing only; the arithmetic is in halo_kernel.cuh and dphi_kernel.cuh.
+#include <cstring>
+
 #include "hr_internal.h"
 
 using namespace hr;
@@ -91,6 +93,64 @@ hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *re
     a.sign_prev = first_rank ? c->bc[0] : 1; // the global seam lies below rank 0's first slice ...
     a.sign_next = last_rank ? c->bc[0] : 1;  // ... and above the last rank's last slice (reading C9)
     return launch_halo(c, links->prec, false, a, (cudaStream_t)stream, link_src(links));
+}
+
+// ---- face buffers in peer-accessible memory ---------------------------------------------------------------------
+// One cudaMalloc allocation of 6 face messages: [send_up | send_dn | recv_prev[0] | recv_next[0] | recv_prev[1] |
+// recv_next[1]] (the receive buffers are double-buffered by call parity, see halo.py).  A plain cudaMalloc base pointer
+// is what cudaIpcGetMemHandle wants; torch's caching allocator hands out sub-blocks.
+hr_status hr_halo_buffers_alloc(const hr_ctx *ctx, hr_prec prec, void **base)
+{
+    if (!ctx || !base || (prec != HR_F64 && prec != HR_F32)) { set_error("hr_halo_buffers_alloc: bad argument"); return HR_EINVAL; }
+    *base = nullptr;
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    cudaError_t e = cudaMalloc(base, 6 * hr_halo_bytes(ctx, prec));
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail("hr_halo_buffers_alloc: cudaMalloc", e); }
+    return HR_OK;
+}
+
+void hr_halo_buffers_free(const hr_ctx *ctx, void *base)
+{
+    if (!ctx || !base) return;
+    if (cudaSetDevice(ctx->device) == cudaSuccess) cudaFree(base);
+    cudaGetLastError();
+}
+
+hr_status hr_ipc_export(const hr_ctx *ctx, const void *base, unsigned char handle[64])
+{
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "cudaIpcMemHandle_t is 64 bytes");
+    if (!ctx || !base || !handle) { set_error("hr_ipc_export: NULL argument"); return HR_EINVAL; }
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    cudaIpcMemHandle_t h;
+    cudaError_t e = cudaIpcGetMemHandle(&h, const_cast<void *>(base));
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail("hr_ipc_export: cudaIpcGetMemHandle", e); }
+    memcpy(handle, &h, 64);
+    return HR_OK;
+}
+
+hr_status hr_ipc_open(const hr_ctx *ctx, const unsigned char handle[64], void **peer_base)
+{
+    if (!ctx || !handle || !peer_base) { set_error("hr_ipc_open: NULL argument"); return HR_EINVAL; }
+    *peer_base = nullptr;
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, 64);
+    cudaError_t e = cudaIpcOpenMemHandle(peer_base, h, cudaIpcMemLazyEnablePeerAccess);
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail("hr_ipc_open: cudaIpcOpenMemHandle", e); }
+    return HR_OK;
+}
+
+hr_status hr_ipc_close(const hr_ctx *ctx, void *peer_base)
+{
+    if (!ctx || !peer_base) { set_error("hr_ipc_close: NULL argument"); return HR_EINVAL; }
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    cudaError_t e = cudaIpcCloseMemHandle(peer_base);
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail("hr_ipc_close: cudaIpcCloseMemHandle", e); }
+    return HR_OK;
 }
 
 } // extern "C"

@@ -55,3 +55,80 @@ class SlabDphi:
         hr_dphi_eo_interior(out, inp, links, parity, st)      # enqueued first: NCCL's transfer overlaps with it
         exchange(self.send_up, self.send_dn, self.recv_prev, self.recv_next, self.plan, self.group)
         hr_dphi_eo_halo_apply(out, self.recv_prev, self.recv_next, links, parity, self.plan["first_rank"], self.plan["last_rank"], st)
+
+
+class PeerSlabDphi:
+    """Distributed Dphi_eo of one rank with the messages written STRAIGHT INTO THE NEIGHBOURS' receive buffers by the pack
+    kernel (peer memory mapped with CUDA IPC: over NVLink between GPUs, or inside one GPU between processes): projection
+    and transfer are one kernel, there is no send/recv.  Receive buffers are double-buffered by call parity and one
+    barrier per call orders the neighbours' stores before the own apply (fence()).  One rank: its own buffers."""
+
+    def __init__(self, lat, prec: int, plan: dict, group=None):
+        import torch.distributed as dist
+        from . import hr_halo_buffers_alloc, hr_halo_bytes, hr_ipc_export, hr_ipc_open
+        self.lat, self.prec, self.plan, self.group = lat, prec, plan, group
+        self.nb = hr_halo_bytes(lat.ctx, prec)
+        self.base = hr_halo_buffers_alloc(lat.ctx, prec)
+        self.calls = 0
+        self.world = dist.get_world_size(group) if dist.is_available() and dist.is_initialized() else 1
+        self._opened = []
+        if self.world == 1:
+            self.prev_base = self.next_base = self.base
+            return
+        rank = dist.get_rank(group)
+        handles = [None] * self.world
+        dist.all_gather_object(handles, hr_ipc_export(lat.ctx, self.base), group=group)
+
+        def peer(r):
+            if r == rank:
+                return self.base
+            p = hr_ipc_open(lat.ctx, handles[r])
+            self._opened.append(p)
+            return p
+
+        self.prev_base = peer(plan["prev"])
+        self.next_base = self.prev_base if plan["next"] == plan["prev"] else peer(plan["next"])
+
+    # offsets inside an allocation: [send_up | send_dn | recv_prev[0] | recv_next[0] | recv_prev[1] | recv_next[1]]
+    def _recv_prev(self, base, k):
+        return base + (2 + 2 * k) * self.nb
+
+    def _recv_next(self, base, k):
+        return base + (3 + 2 * k) * self.nb
+
+    def fence(self):
+        """Every rank's pack stores are complete and visible before anyone applies."""
+        import torch
+        import torch.distributed as dist
+        if self.world == 1:
+            return
+        if dist.get_backend(self.group) == "nccl":
+            if not hasattr(self, "_token"):
+                self._token = torch.zeros(1, device=f"cuda:{self.lat.device}")
+            dist.all_reduce(self._token, group=self.group)       # on the stream: ordered after the pack kernel, no host wait
+        else:
+            torch.cuda.synchronize(self.lat.device)
+            dist.barrier(group=self.group)
+
+    def dphi_eo(self, out, inp, links: int, parity: int) -> None:
+        from . import hr_dphi_eo_halo_apply, hr_dphi_eo_halo_pack, hr_dphi_eo_interior
+        st = self.lat.stream()
+        k = self.calls & 1
+        self.calls += 1
+        # my "up" message is the NEXT rank's recv_prev, my "down" message the PREVIOUS rank's recv_next: peer stores
+        hr_dphi_eo_halo_pack(self._recv_prev(self.next_base, k), self._recv_next(self.prev_base, k), inp, links, parity, st)
+        hr_dphi_eo_interior(out, inp, links, parity, st)
+        self.fence()
+        hr_dphi_eo_halo_apply(out, self._recv_prev(self.base, k), self._recv_next(self.base, k), links, parity,
+                              self.plan["first_rank"], self.plan["last_rank"], st)
+
+    def close(self):
+        from . import hr_halo_buffers_free, hr_ipc_close
+        import torch
+        torch.cuda.synchronize(self.lat.device)
+        for p in self._opened:
+            hr_ipc_close(self.lat.ctx, p)
+        self._opened = []
+        if self.base:
+            hr_halo_buffers_free(self.lat.ctx, self.base)
+            self.base = 0

@@ -1,0 +1,137 @@
+"""GPU parity of the peer-memory halo path (include/hr.h third part: hr_halo_buffers_alloc / hr_ipc_*; halo.PeerSlabDphi;
+PAPER.md:46-64): the pack kernel of one PROCESS stores its half-spinor messages straight into the receive buffers of
+its neighbours, mapped with CUDA IPC.  (a) one rank (neighbour = itself) against the oracle; (b) TWO processes, each
+owning one slab of a global lattice, both on cuda:0 -- IPC works inside one GPU as it does over NVLink -- with the
+ordering done on the host (synchronize + gloo barrier; no kernel of one rank waits on a kernel of the other), results
+stitched and compared with the oracle on the global lattice.  Tolerances: BASELINE.json:north_star."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+import lattice_inputs as li
+import oracle
+from gpu_common import BC_T, TOL, GpuProblem, oracle_rep_id, rel_l2
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def hr():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2405_19294_b200 import build
+    build.build()
+    import paper_2405_19294_b200 as hr
+    return hr
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("N,rep,fundlinks", [(3, "fund", False), (3, "sym", True)])
+def test_single_rank_peer_buffers_reproduce_the_oracle(hr, N, rep, fundlinks, prec):
+    from paper_2405_19294_b200 import halo
+    dims = (4, 4, 6, 8)
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(341, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    prob = GpuProblem(hr, dims, N, rep, prec, U)
+    slab = halo.PeerSlabDphi(prob.lat, prob.prec, halo.slab_plan(0, 1, dims[0]))
+    for rounds in range(2):                                          # both halves of the double buffer
+        for parity in (0, 1):
+            psi = li.gaussian_spinor(342 + parity + 2 * rounds, li.volume(dims) // 2, d)
+            gin, out = prob.lat.spinor(prob.prec), prob.lat.spinor(prob.prec)
+            prob.lat.import_spinor(gin, prob.prec, psi, 1 - parity)
+            out.fill_(0xFF)
+            slab.dphi_eo(out, gin, prob.fund if fundlinks else prob.links, parity)
+            assert rel_l2(prob.lat.export_spinor(out, prob.prec, parity), oracle.dphi_eo(dims, BC_T, R, parity, psi)) <= TOL[prec]
+    slab.close()
+    prob.close()
+
+
+def test_ipc_handle_round_trip_inside_one_process_is_refused_or_maps(hr):
+    """cudaIpcOpenMemHandle of an allocation of the SAME process is an error in CUDA; the binding must surface it as an
+    HrError (not crash), and export must give a 64-byte handle."""
+    prob = GpuProblem(hr, (4, 4, 4, 4), 3, "fund", "f64", li.haar_links(343, 3, (4, 4, 4, 4)))
+    base = hr.hr_halo_buffers_alloc(prob.lat.ctx, hr.HR_F64)
+    h = hr.hr_ipc_export(prob.lat.ctx, base)
+    assert isinstance(h, bytes) and len(h) == 64
+    try:
+        p = hr.hr_ipc_open(prob.lat.ctx, h)
+        hr.hr_ipc_close(prob.lat.ctx, p)
+    except hr.HrError as e:
+        assert e.status == hr.HR_ECUDA
+    hr.hr_halo_buffers_free(prob.lat.ctx, base)
+    prob.close()
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _peer_worker(rank, world, port, q, case):
+    sys.path.insert(0, ROOT)
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import torch.distributed as dist
+    import paper_2405_19294_b200 as hr
+    from paper_2405_19294_b200 import halo
+    from gpu_common import GpuProblem
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    dims, N, rep, fundlinks, prec = case
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    V = li.volume(dims)
+    U = li.haar_links(351, N, dims)
+    ldims = (dims[0] // world,) + tuple(dims[1:])
+    Ul = np.ascontiguousarray(U[rank * (V // world):(rank + 1) * (V // world)])       # t slowest: slabs are contiguous
+    prob = GpuProblem(hr, ldims, N, rep, prec, Ul)
+    slab = halo.PeerSlabDphi(prob.lat, prob.prec, halo.slab_plan(rank, world, dims[0]))
+    lk = prob.fund if fundlinks else prob.links
+    res = {}
+    for rounds in range(2):
+        for parity in (0, 1):
+            psi = li.gaussian_spinor(352 + parity + 2 * rounds, V // 2, d)
+            per = (V // 2) // world
+            gin, out = prob.lat.spinor(prob.prec), prob.lat.spinor(prob.prec)
+            prob.lat.import_spinor(gin, prob.prec, np.ascontiguousarray(psi[rank * per:(rank + 1) * per]), 1 - parity)
+            out.fill_(0xFF)
+            slab.dphi_eo(out, gin, lk, parity)
+            res[(rounds, parity)] = prob.lat.export_spinor(out, prob.prec, parity)
+    dist.barrier()
+    slab.close()
+    prob.close()
+    q.put((rank, res))
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("case", [((8, 4, 2, 6), 3, "fund", False, "f64"), ((8, 4, 2, 6), 3, "sym", True, "f32"),
+                                  ((4, 4, 4, 4), 2, "adj", False, "f64")])
+def test_two_processes_store_into_each_others_buffers(case):
+    import torch
+    import torch.multiprocessing as mp
+    assert torch.cuda.is_available()
+    from paper_2405_19294_b200 import build
+    build.build()
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_peer_worker, args=(r, world, port, q, case)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = dict(q.get(timeout=300) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    dims, N, rep, _, prec = case
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    R = oracle.represent(N, oracle_rep_id(rep), li.haar_links(351, N, dims))
+    for rounds in range(2):
+        for parity in (0, 1):
+            psi = li.gaussian_spinor(352 + parity + 2 * rounds, li.volume(dims) // 2, d)
+            want = oracle.dphi_eo(dims, BC_T, R, parity, psi)
+            stitched = np.concatenate([got[r][(rounds, parity)] for r in range(world)])
+            assert rel_l2(stitched, want) <= TOL[prec], (rounds, parity)
