@@ -132,3 +132,71 @@ class PeerSlabDphi:
         if self.base:
             hr_halo_buffers_free(self.lat.ctx, self.base)
             self.base = 0
+
+
+class SlabCG:
+    """Dhat x = b on a lattice cut into t-slabs (one per rank): CG on Dhat^dag Dhat x = Dhat^dag b (the
+    algorithm of hr_cg_dhat, readings C20-C22), every vector operation one of the library's kernels on the LOCAL slab,
+    the operator through `slab` (SlabDphi or PeerSlabDphi: two distributed Dphi_eo per Dhat), and the two scalars of an
+    iteration summed over the ranks with an all-reduce.  Host-driven (one scalar read per reduction): this is the
+    distributed counterpart of the single-GPU solver, not its tuned form."""
+
+    def __init__(self, slab, links: int, m0: float, group=None):
+        self.slab, self.links, self.m0, self.group = slab, links, float(m0), group
+        self.lat, self.prec = slab.lat, slab.prec
+        self.tmp_o = self.lat.spinor(self.prec)
+        self.tmp_e = self.lat.spinor(self.prec)
+
+    def allsum(self, v: float) -> float:
+        import torch
+        import torch.distributed as dist
+        if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(self.group) == 1:
+            return v
+        dev = f"cuda:{self.lat.device}" if dist.get_backend(self.group) == "nccl" else "cpu"
+        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, group=self.group)
+        return float(t.item())
+
+    def g5dhat(self, out, inp) -> None:
+        """out = gamma5 Dhat inp,  Dhat = (4+m0)^2 - Dphi_eo Dphi_oe  (Hermitian, reading C21)."""
+        from . import hr_spinor_g5, hr_spinor_lincomb
+        ctx, P, st = self.lat.ctx, self.prec, self.lat.stream()
+        self.slab.dphi_eo(self.tmp_o, inp, self.links, 1)
+        self.slab.dphi_eo(self.tmp_e, self.tmp_o, self.links, 0)
+        m = 4.0 + self.m0
+        hr_spinor_lincomb(ctx, P, self.tmp_e, m * m, 0, inp, -1.0, self.tmp_e, st)
+        hr_spinor_g5(ctx, P, out, self.tmp_e, st)
+
+    def norm2(self, v) -> float:
+        from . import hr_spinor_norm2
+        return self.allsum(hr_spinor_norm2(self.lat.ctx, self.prec, v, self.lat.stream()))
+
+    def redot(self, a, b) -> float:
+        from . import hr_spinor_dot
+        return self.allsum(hr_spinor_dot(self.lat.ctx, self.prec, a, b, self.lat.stream()).real)
+
+    def solve(self, x, b, tol: float, maxiter: int):
+        """x = Dhat^{-1} b (x0 = 0).  Returns (iterations, [|r_k|^2 / |rhs|^2])."""
+        from . import hr_spinor_copy, hr_spinor_g5, hr_spinor_lincomb, hr_spinor_mulc_add_assign
+        lat, ctx, P, st = self.lat, self.lat.ctx, self.prec, self.lat.stream()
+        r, p, ap, w = (lat.spinor(P) for _ in range(4))
+        # rhs = Dhat^dag b = g5 Dhat g5 b;  A = Dhat^dag Dhat = (g5 Dhat)^2
+        hr_spinor_g5(ctx, P, w, b, st)
+        self.g5dhat(r, w)
+        hr_spinor_copy(ctx, P, p, r, st)
+        hr_spinor_lincomb(ctx, P, x, 0.0, 0, r, stream=st)
+        rr = bb = self.norm2(r)
+        hist = [1.0 if bb > 0 else 0.0]
+        k = 0
+        while bb > 0 and k < maxiter and rr > tol * tol * bb:
+            self.g5dhat(w, p)
+            self.g5dhat(ap, w)
+            alpha = rr / self.redot(p, ap)
+            hr_spinor_mulc_add_assign(ctx, P, x, alpha, p, st)
+            hr_spinor_mulc_add_assign(ctx, P, r, -alpha, ap, st)
+            rr_new = self.norm2(r)
+            hr_spinor_lincomb(ctx, P, p, 1.0, 0, r, rr_new / rr, p, st)
+            rr = rr_new
+            k += 1
+            hist.append(rr / bb)
+        return k, hist

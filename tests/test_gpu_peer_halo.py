@@ -74,6 +74,14 @@ def _free_port():
 
 
 def _peer_worker(rank, world, port, q, case):
+    try:
+        _peer_worker_body(rank, world, port, q, case)
+    except BaseException as e:                                       # the parent must not wait for a dead rank
+        q.put((rank, {"error": repr(e)}))
+        raise
+
+
+def _peer_worker_body(rank, world, port, q, case):
     sys.path.insert(0, ROOT)
     sys.path.insert(0, os.path.join(ROOT, "tests"))
     import torch.distributed as dist
@@ -101,6 +109,15 @@ def _peer_worker(rank, world, port, q, case):
             out.fill_(0xFF)
             slab.dphi_eo(out, gin, lk, parity)
             res[(rounds, parity)] = prob.lat.export_spinor(out, prob.prec, parity)
+    if case[2] == "fund" or world == 1:                              # distributed CG on the slabs (SlabCG)
+        m0 = -0.2
+        b = li.gaussian_spinor(361, V // 2, d)
+        per = (V // 2) // world
+        gb, gx = prob.lat.spinor(prob.prec), prob.lat.spinor(prob.prec)
+        prob.lat.import_spinor(gb, prob.prec, np.ascontiguousarray(b[rank * per:(rank + 1) * per]), 0)
+        gx.fill_(0xFF)
+        it, hist = halo.SlabCG(slab, lk, m0).solve(gx, gb, 1e-10, 400)
+        res["cg"] = (it, hist, prob.lat.export_spinor(gx, prob.prec, 0))
     dist.barrier()
     slab.close()
     prob.close()
@@ -122,7 +139,16 @@ def test_two_processes_store_into_each_others_buffers(case):
     procs = [ctx.Process(target=_peer_worker, args=(r, world, port, q, case)) for r in range(world)]
     for p in procs:
         p.start()
-    got = dict(q.get(timeout=300) for _ in range(world))
+    got = {}
+    for _ in range(world):
+        r, res = q.get(timeout=240)
+        if "error" in res:
+            for p in procs:
+                p.join(timeout=5)
+                if p.is_alive():
+                    p.terminate()                                    # the surviving rank sits in a barrier
+            pytest.fail(f"rank {r}: {res['error']}")
+        got[r] = res
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
@@ -135,3 +161,13 @@ def test_two_processes_store_into_each_others_buffers(case):
             want = oracle.dphi_eo(dims, BC_T, R, parity, psi)
             stitched = np.concatenate([got[r][(rounds, parity)] for r in range(world)])
             assert rel_l2(stitched, want) <= TOL[prec], (rounds, parity)
+    if "cg" in got[0]:
+        from oracle import solver
+        b = li.gaussian_spinor(361, li.volume(dims) // 2, d)
+        x_want, it_want, hist_want = solver.cg_dhat(dims, BC_T, R, -0.2, b, 1e-10, 400)
+        assert got[0]["cg"][0] == got[1]["cg"][0] and abs(got[0]["cg"][0] - it_want) <= 1
+        n = min(got[0]["cg"][0], it_want) + 1
+        assert np.allclose(got[0]["cg"][1][:n], hist_want[:n], rtol=1e-6, atol=0)
+        assert got[0]["cg"][1] == got[1]["cg"][1]                    # both ranks saw the same all-reduced scalars
+        x = np.concatenate([got[r]["cg"][2] for r in range(world)])
+        assert rel_l2(x, x_want) <= 1e-8
