@@ -11,7 +11,7 @@ template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant);
 
 template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, const HaloArgs &a, cudaStream_t st);
 
-static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf" };
+static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour" };
 
 // Default variant per (d_R, link type, precision, volume): filled from measurements.
 static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
@@ -20,9 +20,13 @@ static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
     if (lk == 2 || lk == 3 || lk == 4) return 0;
     if (lk == 6 || lk == 7) return prec == HR_F64 ? 2 : 0; // fp64 d_R = 8: two threads per site (measured)
     if (lk == 5) return 1;
+    // d_R > 8 (SU(4) sym / adj): a site no longer fits a thread at all -- the colour-parallel kernel
+    if (c->d > 8) return 6;
     // measured on B200 (profiles/r1_variant_sweep.md): at d_R >= 6 fp64 one thread per site spills
     // and the pair kernel wins; in fp32 the whole site still fits one thread.
-    if (c->d >= 6) return prec == HR_F64 ? 3 : 1;
+    // ... and (bench_large_n, profiles/r1_large_n.md) the colour-parallel kernel beats both: SU(3) sextet 24^3x48 fp64
+    // 0.301 ms against 0.331 (site) / 0.332 (pair); SU(3) adjoint 0.347 against 0.363 (pair_ef)
+    if (c->d >= 6) return prec == HR_F64 ? 6 : 1;
     // SU(2) adjoint (real 3x3 links, spinors are 40 % of the compulsory bytes): evict-first links / evict-last
     // spinors gain 2 % (0.0965 -> 0.0944 ms at 32^4 fp64)
     if (lk == 1 && c->d == 3) return 1;
@@ -51,7 +55,7 @@ int dphi_link_kind(const hr_ctx *c, int link_src)
 }
 
 #define HR_COMBOS(X)                                                                                      \
-    X(2, 0) X(3, 0) X(4, 0) X(6, 0) X(3, 1) X(8, 1) X(3, 2) X(6, 2) X(3, 3) X(6, 3) X(2, 4) X(3, 4) X(3, 5) X(8, 6) X(8, 7)
+    X(2, 0) X(3, 0) X(4, 0) X(6, 0) X(3, 1) X(8, 1) X(3, 2) X(6, 2) X(3, 3) X(6, 3) X(2, 4) X(3, 4) X(3, 5) X(8, 6) X(8, 7) X(10, 0) X(15, 1)
 
 hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st, int link_src)
 {

@@ -5,6 +5,7 @@
 #include <type_traits>
 
 #include "dphi_pf_kernel.cuh"
+#include "dphi_cp_kernel.cuh"
 #include "halo_kernel.cuh"
 
 namespace hr {
@@ -17,8 +18,10 @@ namespace hr {
 //   4 site_l1   one thread per site, links through L1 as well (baseline for the cache-policy evidence)
 //   5 site_pf   one thread per site, the next hop's operands prefetched with cp.async into a private,
 //               double-buffered shared-memory stage (dphi_pf_kernel.cuh)
-enum { DPHI_NVARIANTS = 6 };
-static const char *const kDphiVariantNames[DPHI_NVARIANTS] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf" };
+//   6 colour    one thread per (site, colour row): the large-d_R kernel (dphi_cp_kernel.cuh; represented links)
+// d_R > 8 (SU(4) two-index symmetric, adjoint) compiles only 0 (the paper's "unimproved" kernel, for comparison) and 6.
+enum { DPHI_NVARIANTS = 7 };
+static const char *const kDphiVariantNames[DPHI_NVARIANTS] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour" };
 static const size_t kMaxDynSmem = 227 * 1024;
 
 // registers: __launch_bounds__(MAXT, MINB) caps them at 65536 / (MAXT*MINB)
@@ -93,6 +96,13 @@ static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaS
 {
     constexpr int RPV = 16 / (int)sizeof(Real);
     constexpr bool PAIR_OK = (2 * D) % RPV == 0;
+    constexpr bool CP_OK = (LK == LK_COMPLEX || LK == LK_REAL);
+    if constexpr (CP_OK) {
+        if (variant == 6) return launch_cp<Real, D, LK, MASS, RED>(a, st);
+    }
+    if constexpr (D > 8) {
+        if (variant == 0) return launch_one<Real, D, LK, 1, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
+    } else
     switch (variant) {
     case 0: return launch_one<Real, D, LK, 1, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
     case 1: return launch_one<Real, D, LK, 1, MASS, RED, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
@@ -117,7 +127,7 @@ hr_status launch_dphi_t(int variant, int block, const DphiArgs &a, cudaStream_t 
 {
     if (a.site_mode != 0) {
         // fused site-diagonal matrix: the `site` / `site_ef` kernels only, complex-link kinds with a clover field
-        if constexpr (LK == LK_COMPLEX || LK == LK_REAL) {
+        if constexpr ((LK == LK_COMPLEX || LK == LK_REAL) && D <= 8) {
             if (a.site_mode == 1 && a.self && !a.red_result) {
                 if (variant == 0) return launch_one<Real, D, LK, 1, true, false, LD_STREAM, LD_DEFAULT, ST_DEFAULT, 1>(block, a, st);
                 if (variant == 1) return launch_one<Real, D, LK, 1, true, false, LD_STREAM_EF, LD_KEEP, ST_STREAM, 1>(block, a, st);
@@ -139,6 +149,8 @@ template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant)
 {
     constexpr int RPV = 16 / (int)sizeof(Real);
     if (variant < 0 || variant >= DPHI_NVARIANTS) return false;
+    if (variant == 6) return LK == LK_COMPLEX || LK == LK_REAL;
+    if (D > 8) return variant == 0;
     if ((variant == 2 || variant == 3) && (2 * D) % RPV != 0) return false;
     if (variant == 5 && PfGeom<Real, D, LK>::smem_bytes(64) > kMaxDynSmem) return false;
     return true;

@@ -52,7 +52,7 @@ static bool combo_supported(int N, int rep)
     switch (N) {
     case 2: return rep == HR_REP_FUND || rep == HR_REP_ADJ || rep == HR_REP_SYM;
     case 3: return rep == HR_REP_FUND || rep == HR_REP_ADJ || rep == HR_REP_SYM || rep == HR_REP_ASYM;
-    case 4: return rep == HR_REP_FUND || rep == HR_REP_ASYM;
+    case 4: return rep == HR_REP_FUND || rep == HR_REP_ASYM || rep == HR_REP_SYM || rep == HR_REP_ADJ;
     default: return false;
     }
 }

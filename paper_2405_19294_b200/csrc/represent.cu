@@ -185,7 +185,7 @@ hr_status launch_represent(const hr_ctx *c, hr_prec in_prec, const void *fund, h
 #define X(NN, RR) if (c->N == NN && c->rep == RR) return launch_rep<NN, RR>(in_prec, fund, out_prec, repr, c->Vh, st);
     X(2, HR_REP_FUND) X(2, HR_REP_ADJ) X(2, HR_REP_SYM)
     X(3, HR_REP_FUND) X(3, HR_REP_ADJ) X(3, HR_REP_SYM) X(3, HR_REP_ASYM)
-    X(4, HR_REP_FUND) X(4, HR_REP_ASYM)
+    X(4, HR_REP_FUND) X(4, HR_REP_ASYM) X(4, HR_REP_SYM) X(4, HR_REP_ADJ)
 #undef X
     set_error("no link-map kernel compiled for SU(%d) representation %d", c->N, c->rep);
     return HR_EUNSUPPORTED;

@@ -9,7 +9,7 @@ BC_T = (-1, 1, 1, 1)             # periodic in space, antiperiodic in time (BASE
 TOL = {"f64": 1e-13, "f32": 2e-6}  # BASELINE.json:north_star: relative L2 vs the fp64 oracle
 
 # (N, rep name, oracle rep id)
-COMBOS = [(2, "fund"), (2, "adj"), (2, "sym"), (3, "fund"), (3, "adj"), (3, "sym"), (3, "asym"), (4, "fund"), (4, "asym")]
+COMBOS = [(2, "fund"), (2, "adj"), (2, "sym"), (3, "fund"), (3, "adj"), (3, "sym"), (3, "asym"), (4, "fund"), (4, "asym"), (4, "sym"), (4, "adj")]
 
 
 def rel_l2(a, b):

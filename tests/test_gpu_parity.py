@@ -123,9 +123,9 @@ def test_dphi_eo_boundaries_and_small_extents(hr, dims, bc, parity):
     prob.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("N,rep", [(2, "fund"), (3, "fund"), (2, "adj"), (3, "sym"), (3, "adj")])
+@pytest.mark.parametrize("N,rep", [(2, "fund"), (3, "fund"), (2, "adj"), (3, "sym"), (3, "adj"), (4, "sym"), (4, "adj")])
 def test_every_kernel_variant_matches_oracle(hr, N, rep, prec, variant):
     dims = (4, 4, 6, 8)
     d = oracle.rep_dim(N, oracle_rep_id(rep))
@@ -266,3 +266,37 @@ def test_launch_counter_counts_our_kernels(hr):
     prob.lat.dirac(0.1, full_out, full_in, prob.links)
     assert hr.hr_launch_count() == n0 + 2        # hr_dirac: one launch per output parity
     prob.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# the colour-parallel kernel (variant 6): ragged CTA tails, boundary signs, mass term
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("N,rep", [(3, "fund"), (2, "adj"), (3, "sym"), (3, "adj"), (4, "sym"), (4, "adj")])
+@pytest.mark.parametrize("dims,bc", [((2, 2, 2, 2), BC_T), ((4, 6, 2, 10), (1, -1, 1, -1)), ((6, 2, 6, 6), (-1, -1, -1, -1))])
+def test_colour_parallel_kernel_matches_oracle(hr, dims, bc, N, rep, prec):
+    """Vh = 8, 240, 216: less than one CTA of 32 sites, and ragged tails; odd d_R in fp32 and real links exercise the
+    unaligned element loads and the tail planes of the record layout."""
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(61, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    V = li.volume(dims)
+    prob = GpuProblem(hr, dims, N, rep, prec, U, bc=bc)
+    prob.lat.set_tuning("variant", 6)
+    assert hr.hr_dphi_variant_name(prob.lat.ctx, prob.prec) == "colour"
+    for parity in (0, 1):
+        psi = li.gaussian_spinor(62 + parity, V // 2, d)
+        assert rel_l2(prob.dphi_eo(psi, parity), oracle.dphi_eo(dims, bc, R, parity, psi)) <= TOL[prec], parity
+    psi = li.gaussian_spinor(64, V, d)
+    assert rel_l2(prob.dirac(-0.3, psi), oracle.dirac(dims, bc, R, -0.3, psi)) <= TOL[prec]
+    prob.close()
+
+
+def test_large_representations_default_to_the_colour_kernel(hr):
+    for N, rep in ((4, "sym"), (4, "adj")):
+        lat = hr.Lattice((4, 4, 4, 4), BC_T, N, rep)
+        assert lat.d == (10 if rep == "sym" else 15)
+        assert hr.hr_dphi_variant_name(lat.ctx, hr.HR_F64) == "colour" and hr.hr_dphi_variant_name(lat.ctx, hr.HR_F32) == "colour"
+        with pytest.raises(hr.HrError):
+            lat.set_tuning("variant", 2)            # no pair kernel at d_R > 8
+        lat.close()

@@ -47,7 +47,7 @@ class Fields:
 # dims chosen so that V/2 * (16-byte vectors per site) is NOT a multiple of the 1024-vector CTA tile (ragged
 # tail) and spans several CTAs
 LA_CASES = [((4, 2, 6, 2), 2, "fund"), ((4, 6, 6, 10), 3, "fund"), ((6, 4, 2, 10), 2, "adj"), ((4, 4, 6, 2), 3, "sym"),
-            ((2, 2, 2, 2), 3, "adj")]
+            ((2, 2, 2, 2), 3, "adj"), ((4, 2, 2, 6), 4, "sym"), ((2, 4, 2, 6), 4, "adj")]
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
@@ -118,7 +118,7 @@ def test_reductions_match_oracle_and_are_deterministic(hr, dims, N, rep, prec):
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("g5", [0, 1])
 @pytest.mark.parametrize("dims,N,rep", [((4, 4, 6, 8), 3, "fund"), ((6, 4, 4, 4), 2, "adj"), ((4, 4, 4, 6), 3, "sym"),
-                                        ((2, 2, 2, 2), 2, "fund"), ((4, 2, 6, 4), 3, "asym")])
+                                        ((2, 2, 2, 2), 2, "fund"), ((4, 2, 6, 4), 3, "asym"), ((4, 2, 4, 6), 4, "sym"), ((2, 4, 6, 2), 4, "adj")])
 def test_dhat_matches_oracle(hr, dims, N, rep, g5, prec):
     d = oracle.rep_dim(N, oracle_rep_id(rep))
     U = li.haar_links(111, N, dims)
@@ -136,7 +136,7 @@ def test_dhat_matches_oracle(hr, dims, N, rep, g5, prec):
     assert hr.hr_launch_count() == n0 + 2          # two Dphi launches, diagonal term and gamma5 fused
     assert rel_l2(f.get(out), want) <= TOL[prec]
     # every kernel variant computes the same operator
-    for variant in (0, 1, 2, 3, 4, 5):
+    for variant in (0, 1, 2, 3, 4, 5, 6):
         try:
             prob.lat.set_tuning("variant", variant)
             out2 = f.new()
@@ -150,7 +150,8 @@ def test_dhat_matches_oracle(hr, dims, N, rep, g5, prec):
 
 
 # ---------------------------------------------------------------------------------------------- CG
-CG_CASES = [((4, 4, 4, 8), 3, "fund", -0.3), ((4, 4, 6, 4), 2, "adj", -0.5), ((4, 4, 4, 4), 3, "sym", -0.2)]
+CG_CASES = [((4, 4, 4, 8), 3, "fund", -0.3), ((4, 4, 6, 4), 2, "adj", -0.5), ((4, 4, 4, 4), 3, "sym", -0.2),
+            ((4, 2, 4, 6), 4, "sym", -0.25)]          # d_R = 10: the colour-parallel kernel with the fused reduction
 
 
 @pytest.mark.parametrize("dims,N,rep,m0", CG_CASES)
