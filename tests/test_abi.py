@@ -68,7 +68,7 @@ def test_ctx_geometry_and_sizes(hr, N, rep, d, real):
     ((4, 4, 4, 4), (1, 1, 1, 1), 3, 7, -1),     # unknown rep
     ((4, 4, 4, 4), (1, 1, 1, 1), 2, 3, -2),     # SU(2) antisymmetric: d_R = 1, not instantiated
     ((4, 4, 4, 4), (1, 1, 1, 1), 5, 0, -2),     # SU(5) not instantiated
-    ((4, 4, 4, 4), (1, 1, 1, 1), 4, 2, -2),     # SU(4) symmetric (d_R = 10) not instantiated
+    ((4, 4, 4, 4), (1, 1, 1, 1), 6, 2, -2),     # SU(6) symmetric (d_R = 21) not instantiated
 ])
 def test_ctx_create_rejects_bad_arguments(hr, dims, bc, N, rep, status):
     with pytest.raises(hr.HrError) as e:
