@@ -58,7 +58,8 @@ const char *hr_last_error(void);
 /*
  * Describe the problem.  dims[mu] even and >= 2 (reading C11: odd extents break the even/odd
  * bipartition), bc[mu] in {+1,-1}, N in {2,3,4}.  Supported (N, rep): N=2: FUND, ADJ, SYM;
- * N=3: FUND, ADJ, SYM, ASYM; N=4: FUND, ASYM.  Anything else (e.g. ASYM for N=2, d_R = 1)
+ * N=3: FUND, ADJ, SYM, ASYM; N=4: FUND, ASYM, SYM (d_R = 10), ADJ (d_R = 15; these two run on the colour-parallel
+ * kernel of PAPER.md:92-96 and have no clover / on-the-fly-link kernels).  Anything else (e.g. ASYM for N=2, d_R = 1)
  * -> HR_EUNSUPPORTED.  Does not touch the GPU; `device` is the CUDA ordinal later calls run on.
  */
 hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N, hr_rep rep, int device);
@@ -332,7 +333,8 @@ hr_status hr_dirac_clover(double m0, void *out_full, const void *in_full, const 
 
 /*
  * Kernel tuning (experiments and ncu evidence; defaults are chosen per (d_R, precision) from
- * measurements).  key: "variant" (kernel variant id, -1 = default table),
+ * measurements).  key: "variant" (kernel variant id, -1 = default table; 0 site, 1 site_ef,
+ * 2 pair, 3 pair_ef, 4 site_l1, 5 site_pf, 6 colour = one thread per (site, colour row)),
  * "block" (threads per CTA, 0 = default), "xblock" (x-extent of the thread order's blocks, a divisor
  * of X; 0 = default from the L2 working-set rule), "cg_graph" (the CG replays one captured iteration as a
  * CUDA graph: 1 = default, on lattices below 2^19 sites per parity, where launch overhead shows; 2 = always;

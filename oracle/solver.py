@@ -15,6 +15,8 @@ written out below are their plain definitions under the readings C20-C24 of DESI
   C24  full solve D x = b through the preconditioned system:
        Dhat x_e = m b_e - Dphi_eo b_o,   x_o = (b_o - Dphi_oe x_e) / m.
 
+  C29  BiCGstab (below);  C33  gamma5-QMR (below): both written out at their definitions further down.
+
 Every function is numpy on canonical half fields [V/2][4][d] complex128 and calls oracle.dphi_eo (the C
 definition of the hopping term) as its only non-trivial step; the CG is the textbook algorithm, one line per
 step, no fusion.  Pins: tests/test_oracle_solver.py (dense Schur complement and numpy.linalg.solve through
@@ -151,3 +153,93 @@ def bicgstab(apply_A, b, tol, maxiter):
 def bicgstab_dhat(dims, bc, links_R, m0, b_e, tol, maxiter):
     """Solve Dhat x = b_e on the even sites with BiCGstab applied to Dhat itself (no normal equations)."""
     return bicgstab(lambda v: dhat(dims, bc, links_R, m0, v), b_e, tol, maxiter)
+
+
+# ---- QMR for gamma5-hermitian operators (PAPER.md:124 "QMR gamma_5 inverters"; reading C33) ------------------------------
+def qmr_j(apply_A, apply_J, b, tol, maxiter, debug=False):
+    """Quasi-minimal residual method without look-ahead for an operator that is self-adjoint in the indefinite inner
+    product (x, y)_J = <x, J y>, J a Hermitian involution (gamma5 for the Wilson-Dirac operator and for Dhat, reading
+    C21): A^dagger = J A J.  The paper names the method and prints nothing (reading C33); this is the method written out
+    from its definition:
+
+      Lanczos in the J-inner product (ONE operator application per step, no A^dagger): v_1 = b / rho_1, rho_1 = |b|,
+          delta_k = (v_k, v_k)_J                                    (real)
+          alpha_k = (v_k, A v_k)_J / delta_k                        (real)
+          beta_k  = rho_k delta_k / delta_{k-1},  beta_1 = 0
+          vt      = A v_k - alpha_k v_k - beta_k v_{k-1};   rho_{k+1} = |vt|;   v_{k+1} = vt / rho_{k+1}
+      so that A V_k = V_{k+1} T_k with T_k tridiagonal: T[k-1,k] = beta_k, T[k,k] = alpha_k, T[k+1,k] = rho_{k+1},
+      and V_k^dagger J V_k = diag(delta).
+      Quasi-minimisation: x_k = V_k y_k with y_k = argmin | rho_1 e_1 - T_k y |, by Givens rotations (QR of T_k):
+          theta_k = s_{k-2} beta_k;   t = c_{k-2} beta_k
+          eps_k   = c_{k-1} t + s_{k-1} alpha_k;   zt = -s_{k-1} t + c_{k-1} alpha_k
+          zeta_k  = sqrt(zt^2 + rho_{k+1}^2);   c_k = zt / zeta_k;   s_k = rho_{k+1} / zeta_k
+          p_k = (v_k - eps_k p_{k-1} - theta_k p_{k-2}) / zeta_k
+          x_k = x_{k-1} + c_k eta p_k;   eta <- -s_k eta             (eta starts at rho_1)
+      |eta| is the norm of the QUASI-residual; |b - A x_k| <= sqrt(k+1) |eta| because the v_k are not orthonormal.
+    Stopping (reading C33): x0 = 0; after step k, if |eta| <= tol |b| the TRUE residual b - A x_k is computed (one more
+    operator application) and the iteration ends when |b - A x_k| <= tol |b|; it also ends at k = maxiter, at
+    rho_{k+1} = 0 (Krylov space exhausted: x_k is exact) and at a Lanczos breakdown delta_k = 0.
+    Returns (x, iterations, [|eta_k| / |b| for k = 0..iterations], |b - A x|^2 / |b|^2) -- plus the Lanczos data when debug."""
+    x = np.zeros_like(b)
+    bnorm = np.sqrt(norm2(b))
+    hist = [1.0 if bnorm > 0 else 0.0]
+    if bnorm == 0.0:
+        return (x, 0, hist, 0.0) + (({},) if debug else ())
+    v_prev = np.zeros_like(b)
+    v = b / bnorm
+    p1 = np.zeros_like(b)            # p_{k-1}
+    p2 = np.zeros_like(b)            # p_{k-2}
+    c1, s1, c2, s2 = 1.0, 0.0, 1.0, 0.0   # (c_{k-1}, s_{k-1}), (c_{k-2}, s_{k-2})
+    eta = bnorm
+    rho = bnorm
+    delta_prev = 1.0
+    delta = dot(v, apply_J(v)).real
+    V, alphas, betas, rhos, deltas = [v], [], [], [rho], [delta]
+    k = 0
+    res2 = 1.0
+    while k < maxiter:
+        if delta == 0.0:
+            break                                                   # Lanczos breakdown
+        w = apply_A(v)
+        alpha = dot(v, apply_J(w)).real / delta
+        beta = rho * delta / delta_prev if k > 0 else 0.0
+        vt = w - alpha * v - beta * v_prev
+        rho_next = np.sqrt(norm2(vt))
+        theta = s2 * beta
+        t = c2 * beta
+        eps = c1 * t + s1 * alpha
+        zt = -s1 * t + c1 * alpha
+        zeta = np.sqrt(zt * zt + rho_next * rho_next)
+        if zeta == 0.0:
+            break
+        c, s = zt / zeta, rho_next / zeta
+        p = (v - eps * p1 - theta * p2) / zeta
+        x = x + (c * eta) * p
+        eta = -s * eta
+        k += 1
+        hist.append(abs(eta) / bnorm)
+        alphas.append(alpha); betas.append(beta); rhos.append(rho_next)
+        p2, p1 = p1, p
+        c2, s2, c1, s1 = c1, s1, c, s
+        if rho_next == 0.0:
+            res2 = norm2(b - apply_A(x)) / (bnorm * bnorm)
+            break
+        if abs(eta) <= tol * bnorm:
+            res2 = norm2(b - apply_A(x)) / (bnorm * bnorm)
+            if res2 <= tol * tol:
+                break
+        v_prev, v = v, vt / rho_next
+        delta_prev, delta, rho = delta, dot(v, apply_J(v)).real, rho_next
+        V.append(v); deltas.append(delta)
+    else:
+        res2 = norm2(b - apply_A(x)) / (bnorm * bnorm)
+    if k == maxiter or delta == 0.0:
+        res2 = norm2(b - apply_A(x)) / (bnorm * bnorm)
+    if debug:
+        return x, k, hist, res2, dict(V=V, alpha=alphas, beta=betas, rho=rhos, delta=deltas)
+    return x, k, hist, res2
+
+
+def qmr_dhat(dims, bc, links_R, m0, b_e, tol, maxiter):
+    """Solve Dhat x = b_e on the even sites with the gamma5-QMR (Dhat^dagger = gamma5 Dhat gamma5, reading C21)."""
+    return qmr_j(lambda v: dhat(dims, bc, links_R, m0, v), g5, b_e, tol, maxiter)

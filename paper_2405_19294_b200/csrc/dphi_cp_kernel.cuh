@@ -296,11 +296,13 @@ static hr_status launch_cp(const DphiArgs &a, cudaStream_t st)
     static_assert(LK == LK_COMPLEX || LK == LK_REAL, "colour-parallel kernel: represented links");
     using G = CpGeom<Real, D, LK == LK_REAL>;
     auto kern = dphi_cp_kernel<Real, D, LK == LK_REAL, MASS, RED>;
-    static bool attr_set = false;
-    if (!attr_set && G::smem_bytes() > 48 * 1024) {
+    static bool attr_set[64] = {};                   // per instantiation and device (the attribute lives in the device's context)
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (G::smem_bytes() > 48 * 1024 && !(dev >= 0 && dev < 64 && attr_set[dev])) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes());
         if (e != cudaSuccess) { set_error("colour kernel: cudaFuncSetAttribute: %s", cudaGetErrorString(e)); cudaGetLastError(); return HR_ECUDA; }
-        attr_set = true;
+        if (dev >= 0 && dev < 64) attr_set[dev] = true;
     }
     const long grid = (a.vh + G::SITES - 1) / G::SITES;
     if (RED && (unsigned long)grid > kRedMaxBlocks) { set_error("fused Dphi reduction: too many CTAs"); return HR_EUNSUPPORTED; }

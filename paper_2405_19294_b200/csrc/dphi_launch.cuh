@@ -76,11 +76,13 @@ static hr_status launch_pf(int block, const DphiArgs &a, cudaStream_t st)
         return HR_EUNSUPPORTED;
     }
     auto kern = dphi_pf_kernel<Real, D, LK, MASS, RED, T::MAXT, T::MINB>;
-    static bool attr_set = false; // per instantiation; the attribute is sticky per device context
-    if (!attr_set) {
+    static bool attr_set[64] = {}; // per instantiation and device (the attribute lives in the device's context)
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!(dev >= 0 && dev < 64 && attr_set[dev])) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxDynSmem);
         if (e != cudaSuccess) { set_error("site_pf: cudaFuncSetAttribute: %s", cudaGetErrorString(e)); cudaGetLastError(); return HR_ECUDA; }
-        attr_set = true;
+        if (dev >= 0 && dev < 64) attr_set[dev] = true;
     }
     const long grid = (a.vh + block - 1) / block;
     if (RED && (unsigned long)grid > kRedMaxBlocks) { set_error("fused Dphi reduction: too many CTAs"); return HR_EUNSUPPORTED; }

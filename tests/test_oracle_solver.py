@@ -190,3 +190,133 @@ def test_bicgstab_dhat_equals_dense_schur_solve(dims, N, rep):
     assert 0 < it < 500
     want = np.linalg.solve(schur, b.reshape(-1)).reshape(b.shape)
     assert np.linalg.norm(x - want) <= 1e-10 * np.linalg.norm(want)
+
+
+# ---- QMR for J-hermitian operators ("QMR gamma_5"; reading C33) -----------------------------------------
+def _j_system(n, seed, shift):
+    """A = J H with H Hermitian (so A^dagger = J A J), J = diag(+1 x n/2, -1 x n/2); b complex."""
+    rng = np.random.default_rng(seed)
+    J = np.diag([1.0] * (n // 2) + [-1.0] * (n - n // 2)).astype(complex)
+    H = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    H = H + H.conj().T + shift * np.eye(n)
+    b = (rng.normal(size=n) + 1j * rng.normal(size=n)).reshape(n // 4, 4, 1)
+    return J @ H, J, b
+
+
+def _ops(A, J):
+    n = A.shape[0]
+    return (lambda v: (A @ v.reshape(n)).reshape(v.shape)), (lambda v: (J @ v.reshape(n)).reshape(v.shape))
+
+
+def test_qmr_solves_a_j_hermitian_indefinite_system_like_numpy():
+    A, J, b = _j_system(40, 5, 9.0)
+    assert np.allclose(A.conj().T, J @ A @ J) and not np.allclose(A, A.conj().T)
+    apply_A, apply_J = _ops(A, J)
+    x, it, hist, res2 = solver.qmr_j(apply_A, apply_J, b, 1e-11, 200)
+    want = np.linalg.solve(A, b.reshape(-1))
+    assert 0 < it < 200 and res2 <= 1e-22
+    assert np.linalg.norm(x.reshape(-1) - want) <= 1e-9 * np.linalg.norm(want)
+    # the reported residual is the true one
+    assert np.isclose(res2, np.linalg.norm(b.reshape(-1) - A @ x.reshape(-1)) ** 2 / np.linalg.norm(b) ** 2, rtol=1e-6)
+
+
+def test_qmr_lanczos_vectors_are_j_orthogonal_and_satisfy_the_three_term_relation():
+    """A V_k = V_{k+1} T_k with the tridiagonal T of (beta, alpha, rho) and V^dagger J V = diag(delta): the two defining
+    properties of the J-Lanczos process, checked on the vectors the solver actually built."""
+    n = 24
+    A, J, b = _j_system(n, 6, 7.0)
+    apply_A, apply_J = _ops(A, J)
+    x, it, hist, res2, dbg = solver.qmr_j(apply_A, apply_J, b, 1e-30, 10, debug=True)
+    assert it == 10
+    V = np.stack([v.reshape(n) for v in dbg["V"]], axis=1)          # n x (k+1)
+    k = 10
+    assert V.shape[1] == k + 1 or V.shape[1] == k                  # the last v_{k+1} is built only if the loop continues
+    G = V.conj().T @ J @ V
+    assert np.abs(G - np.diag(np.diag(G))).max() <= 1e-10
+    assert np.allclose(np.diag(G).real, dbg["delta"][:V.shape[1]], atol=1e-12) and np.abs(np.diag(G).imag).max() <= 1e-12
+    assert np.allclose(np.linalg.norm(V, axis=0), 1.0)
+    kk = V.shape[1] - 1
+    T = np.zeros((kk + 1, kk))
+    for j in range(kk):
+        T[j, j] = dbg["alpha"][j]
+        T[j + 1, j] = dbg["rho"][j + 1]
+        if j > 0:
+            T[j - 1, j] = dbg["beta"][j]
+    assert np.abs(A @ V[:, :kk] - V @ T).max() <= 1e-10
+
+
+def test_qmr_with_j_identity_is_minres_and_eta_is_the_true_residual_norm():
+    """J = 1, A Hermitian (indefinite): the Lanczos vectors are orthonormal, so the quasi-residual IS the residual:
+    |eta_k| = |b - A x_k| at every k, and it never increases (minimal residual over the Krylov space)."""
+    n = 32
+    rng = np.random.default_rng(7)
+    H = rng.normal(size=(n, n)) + 1j * rng.normal(size=(n, n))
+    H = H + H.conj().T                                                        # indefinite
+    b = (rng.normal(size=n) + 1j * rng.normal(size=n)).reshape(n // 4, 4, 1)
+    apply_A = lambda v: (H @ v.reshape(n)).reshape(v.shape)
+    ident = lambda v: v
+    bn = np.linalg.norm(b)
+    prev = 1.0
+    for k in (1, 2, 5, 9, 17):
+        x, it, hist, res2 = solver.qmr_j(apply_A, ident, b, 1e-30, k)
+        assert it == k
+        true = np.linalg.norm(b.reshape(-1) - H @ x.reshape(-1)) / bn
+        assert np.isclose(hist[-1], true, rtol=1e-8)
+        # minimal residual: no other vector of the Krylov space does better
+        K = np.stack([np.linalg.matrix_power(H, j) @ b.reshape(-1) for j in range(k)], axis=1)
+        Q, _ = np.linalg.qr(K)
+        y = np.linalg.lstsq(H @ Q, b.reshape(-1), rcond=None)[0]
+        assert np.isclose(true, np.linalg.norm(b.reshape(-1) - H @ Q @ y) / bn, rtol=1e-6)
+        assert true <= prev * (1 + 1e-12)
+        prev = true
+
+
+def test_qmr_iterates_lie_in_the_krylov_space_and_bound_the_true_residual():
+    n = 28
+    A, J, b = _j_system(n, 8, 8.0)
+    apply_A, apply_J = _ops(A, J)
+    bn = np.linalg.norm(b)
+    for k in (1, 3, 6):
+        x, it, hist, res2 = solver.qmr_j(apply_A, apply_J, b, 1e-30, k)
+        K = np.stack([np.linalg.matrix_power(A, j) @ b.reshape(-1) for j in range(k)], axis=1)
+        Q, _ = np.linalg.qr(K)
+        xv = x.reshape(-1)
+        assert np.linalg.norm(xv - Q @ (Q.conj().T @ xv)) <= 1e-9 * np.linalg.norm(xv)
+        assert np.sqrt(res2) <= np.sqrt(k + 1) * hist[-1] * (1 + 1e-9)       # |r_k| <= sqrt(k+1) |eta_k|
+
+
+def test_qmr_terminates_when_the_krylov_space_is_exhausted():
+    """k distinct eigenvalues of a J-hermitian diagonalisable A: rho_{k+1} = 0 and x_k is exact."""
+    n = 16
+    J = np.diag([1.0] * 8 + [-1.0] * 8)
+    d = np.array([2.0, -1.5, 0.75] * 6)[:n]                    # A = J diag(J d) = diag(d): J-hermitian, 3 eigenvalues
+    b = (np.arange(n) + 1.0 - 0.5j * np.arange(n)[::-1]).reshape(4, 4, 1)
+    apply_A = lambda v: (d * v.reshape(-1)).reshape(v.shape)
+    apply_J = lambda v: (np.diag(J) * v.reshape(-1)).reshape(v.shape)
+    x, it, hist, res2 = solver.qmr_j(apply_A, apply_J, b, 1e-13, 50)
+    assert it <= 4 and res2 <= 1e-24
+    assert np.allclose(x.reshape(-1), b.reshape(-1) / d, atol=1e-10)
+
+
+def test_qmr_zero_rhs_and_maxiter_zero():
+    A, J, b = _j_system(8, 9, 5.0)
+    apply_A, apply_J = _ops(A, J)
+    x, it, hist, res2 = solver.qmr_j(apply_A, apply_J, 0 * b, 1e-10, 10)
+    assert it == 0 and res2 == 0.0 and not x.any()
+    x, it, hist, res2 = solver.qmr_j(apply_A, apply_J, b, 1e-10, 0)
+    assert it == 0 and np.isclose(res2, 1.0) and not x.any()
+
+
+@pytest.mark.parametrize("dims,N,rep", [((2, 2, 2, 2), 2, "fund"), ((2, 2, 4, 2), 2, "adj")])
+def test_qmr_dhat_equals_dense_schur_solve(dims, N, rep):
+    R, d = _problem(dims, N, rep, 41)
+    m0 = -0.2
+    m = 4 + m0
+    D = _dense_eo(dims, BC_T, R, m0)
+    n = D.shape[0] // 2
+    schur = m * (D[:n, :n] - D[:n, n:] @ np.linalg.inv(D[n:, n:]) @ D[n:, :n])
+    b = li.gaussian_spinor(42, li.volume(dims) // 2, d)
+    x, it, hist, res2 = solver.qmr_dhat(dims, BC_T, R, m0, b, 1e-12, 500)
+    assert 0 < it < 500 and res2 <= 1e-24
+    want = np.linalg.solve(schur, b.reshape(-1)).reshape(b.shape)
+    assert np.linalg.norm(x - want) <= 1e-9 * np.linalg.norm(want)
