@@ -228,6 +228,20 @@ hr_status hr_bicgstab_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, c
                            int maxiter, void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
 hr_status hr_cg_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol, int maxiter,
                      void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
+/*
+ * hr_qmr_dhat -- the gamma5-QMR ("QMR gamma_5 inverters"; reading C33): quasi-minimal residual method without
+ * look-ahead on Dhat ITSELF, built on the Lanczos process in the indefinite inner product (x, y)_J = <x, gamma5 y>, in which
+ * Dhat is self-adjoint (reading C21) -- ONE operator application per iteration, no Dhat^dagger.  x0 = 0.  After step k,
+ * |eta_k| is the norm of the quasi-residual (|b - Dhat x_k| <= sqrt(k+1) |eta_k|); when |eta_k| <= tol |b| the TRUE
+ * residual is computed (one more operator application) and the iteration ends if |b - Dhat x_k| <= tol |b|; it also ends at
+ * k = maxiter, when the Krylov space is exhausted and at a Lanczos breakdown ((v_k, v_k)_J = 0).  The Lanczos scalars and the
+ * Givens rotations live on the HOST: two synchronisations of `stream` per iteration (the correct first form of the
+ * method, not a tuned one).  Arguments as hr_cg_dhat; workspace of hr_qmr_workspace_bytes(), 256-byte aligned.
+ *   rel_res2: TRUE |b - Dhat x|^2 / |b|^2 at exit.  hist (HOST, maxiter+1 doubles): |eta_k| / |b| for k = 0..iters.
+ */
+size_t hr_qmr_workspace_bytes(const hr_ctx *ctx, hr_prec prec);
+hr_status hr_qmr_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol, int maxiter,
+                      void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
 hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_full, const hr_gauge *links, double tol,
                          int maxiter, void *workspace, int *iters, double *rel_res2, void *stream);
 /*

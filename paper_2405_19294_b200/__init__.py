@@ -82,6 +82,8 @@ _SIGNATURES = {
     "hr_cg_dhat": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp, _vp]),
     "hr_bicgstab_workspace_bytes": (_sz, [_vp, _ci, _ci]),
     "hr_bicgstab_dhat": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp, _vp]),
+    "hr_qmr_workspace_bytes": (_sz, [_vp, _ci]),
+    "hr_qmr_dhat": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp, _vp]),
     "hr_dirac_solve": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
     "hr_halo_bytes": (_sz, [_vp, _ci]),
     "hr_halo_buffers_alloc": (_ci, [_vp, _ci, ctypes.POINTER(_vp)]),
@@ -316,6 +318,19 @@ def hr_bicgstab_dhat(ctx: int, m0: float, x_e, b_e, links: int, tol: float, maxi
     hist = np.zeros(maxiter + 1, dtype=np.float64) if want_hist else None
     _check(_lib.hr_bicgstab_dhat(ctx, float(m0), _ptr(x_e), _ptr(b_e), links, float(tol), int(maxiter), _ptr(workspace),
                                  ctypes.byref(it), ctypes.byref(res), _ptr(hist), stream))
+    return it.value, res.value, (hist[:it.value + 1] if want_hist else None)
+
+
+def hr_qmr_workspace_bytes(ctx: int, prec: int) -> int:
+    return _lib.hr_qmr_workspace_bytes(ctx, prec)
+
+
+def hr_qmr_dhat(ctx: int, m0: float, x_e, b_e, links: int, tol: float, maxiter: int, workspace, stream: int = 0, want_hist: bool = False):
+    """Returns (iterations, true |b - Dhat x|^2/|b|^2, history of |eta_k|/|b| or None)."""
+    it, res = _ci(0), _cd(0.0)
+    hist = np.zeros(maxiter + 1, dtype=np.float64) if want_hist else None
+    _check(_lib.hr_qmr_dhat(ctx, float(m0), _ptr(x_e), _ptr(b_e), links, float(tol), int(maxiter), _ptr(workspace),
+                            ctypes.byref(it), ctypes.byref(res), _ptr(hist), stream))
     return it.value, res.value, (hist[:it.value + 1] if want_hist else None)
 
 

@@ -167,11 +167,13 @@ def main():
     print(json.dumps(dict(common, op="bicgstab_iteration", bytes_per_site=bps, ms=ms, gbs=gbs, frac=gbs / peak, iterations=it,
                           launches_per_iteration=(hr.hr_launch_count() - n0) / it)))
     # time to solution, same right-hand side, relative residual 1e-8 (fp64) / 1e-5 (fp32): CG on the normal equations
-    # vs BiCGstab on Dhat
+    # vs BiCGstab on Dhat vs the gamma5-QMR on Dhat (host-driven scalars)
     tol = 1e-8 if args.prec == "f64" else 1e-5
     for name, fn in (("cg_solve", lambda: lat.cg_dhat(args.m0, x, sets[0][0], links, tol, 2000, lat.cg_workspace(P, 2000))),
                      ("bicgstab_solve", lambda: hr.hr_bicgstab_dhat(ctx, args.m0, x, sets[0][0], links, tol, 2000,
-                                                                    torch.empty(hr.hr_bicgstab_workspace_bytes(ctx, P, 2000), dtype=torch.uint8, device="cuda"), st))):
+                                                                    torch.empty(hr.hr_bicgstab_workspace_bytes(ctx, P, 2000), dtype=torch.uint8, device="cuda"), st)),
+                     ("qmr_solve", lambda: hr.hr_qmr_dhat(ctx, args.m0, x, sets[0][0], links, tol, 2000,
+                                                          torch.empty(hr.hr_qmr_workspace_bytes(ctx, P), dtype=torch.uint8, device="cuda"), st))):
         torch.cuda.synchronize()
         e0.record()
         it, res2, _ = fn()

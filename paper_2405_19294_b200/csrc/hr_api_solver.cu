@@ -417,6 +417,138 @@ hr_status hr_bicgstab_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, c
     return bicgstab_core(ctx, links->prec, x_e, b_e, tol, maxiter, ws, ws + 7 * sb, op, iters, rel_res2, hist, st);
 }
 
+size_t hr_qmr_workspace_bytes(const hr_ctx *ctx, hr_prec prec)
+{
+    if (!ctx || !valid_prec(prec)) return 0;
+    return 6 * (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec);
+}
+
+// gamma5-QMR on Dhat (include/hr.h; reading C33).  Host-driven: the Lanczos scalars and the Givens rotations live on the
+// host, two stream synchronisations per iteration; every vector operation is a library kernel.
+hr_status hr_qmr_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol, int maxiter,
+                      void *workspace, int *iters, double *rel_res2, double *hist, void *stream)
+{
+    hr_status rc = cg_check("hr_qmr_dhat", ctx, x_e, b_e, links, tol, maxiter, workspace);
+    if (rc != HR_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const hr_prec P = links->prec;
+    const size_t sb = (size_t)ctx->Vh * 8 * ctx->d * prec_bytes(P);
+    const size_t nvec = sb / 16, half = nvec / 2;
+    char *ws = (char *)workspace;
+    void *v = ws, *vp = ws + sb, *p1 = ws + 2 * sb, *p2 = ws + 3 * sb, *w = ws + 4 * sb, *tmp = ws + 5 * sb;
+    RedScratch rs;
+    rc = get_red_scratch(ctx, &rs, st);
+    if (rc != HR_OK) return rc;
+    const double zero[2] = { 0.0, 0.0 }, one[2] = { 1.0, 0.0 };
+    double h[8];
+    // |x_upper|^2 and |x_lower|^2 of a field: its norm and its gamma5 "norm" <x, gamma5 x> in one read each half
+    auto halves = [&](const void *f, double *up, double *lo) -> hr_status {
+        hr_status r = launch_dot_range(ctx, P, f, f, 0, half, rs, rs.result, st);
+        if (r != HR_OK) return r;
+        r = launch_dot_range(ctx, P, f, f, half, half, rs, rs.result + 2, st);
+        if (r != HR_OK) return r;
+        HR_CUDA(cudaMemcpyAsync(h, rs.result, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HR_CUDA(cudaStreamSynchronize(st));
+        *up = h[0]; *lo = h[2];
+        return HR_OK;
+    };
+    auto true_res2 = [&](double bb, double *out) -> hr_status {      // |b - Dhat x|^2 / |b|^2, through w and tmp
+        hr_status r = dhat_launches(ctx, m0, 0, w, x_e, tmp, links, nullptr, nullptr, nullptr, st);
+        if (r != HR_OK) return r;
+        const double m1[2] = { -1.0, 0.0 };
+        r = launch_lincomb(ctx, P, w, one, 0, b_e, m1, w, st);
+        if (r != HR_OK) return r;
+        double up, lo;
+        r = halves(w, &up, &lo);
+        if (r != HR_OK) return r;
+        *out = (up + lo) / bb;
+        return HR_OK;
+    };
+    rc = launch_lincomb(ctx, P, x_e, zero, 0, b_e, zero, nullptr, st);                    // x = 0
+    if (rc != HR_OK) return rc;
+    double up, lo;
+    rc = halves(b_e, &up, &lo);
+    if (rc != HR_OK) return rc;
+    const double bb = up + lo, bnorm = sqrt(bb);
+    if (hist) hist[0] = bb > 0.0 ? 1.0 : 0.0;
+    if (iters) *iters = 0;
+    if (rel_res2) *rel_res2 = bb > 0.0 ? 1.0 : 0.0;
+    if (bb == 0.0) return HR_OK;
+    const double inv[2] = { 1.0 / bnorm, 0.0 };
+    rc = launch_lincomb(ctx, P, v, inv, 0, b_e, zero, nullptr, st);                       // v_1 = b / rho_1
+    if (rc != HR_OK) return rc;
+    rc = launch_lincomb(ctx, P, p1, zero, 0, b_e, zero, nullptr, st);                     // p_0 = p_{-1} = 0
+    if (rc != HR_OK) return rc;
+    rc = launch_lincomb(ctx, P, p2, zero, 0, b_e, zero, nullptr, st);
+    if (rc != HR_OK) return rc;
+    double c1 = 1.0, s1 = 0.0, c2 = 1.0, s2 = 0.0, eta = bnorm, rho = bnorm;
+    double delta_prev = 1.0, delta = (up - lo) / bb;
+    double res2 = 1.0;
+    bool have_res = false;
+    int k = 0;
+    while (k < maxiter) {
+        if (delta == 0.0) break;                                                           // Lanczos breakdown
+        // w = gamma5 Dhat v, and <v, w> = (v, Dhat v)_J from the fused reduction of the second Dphi launch
+        rc = dhat_launches(ctx, m0, 1, w, v, tmp, links, &rs, rs.result + 4, nullptr, st);
+        if (rc != HR_OK) return rc;
+        HR_CUDA(cudaMemcpyAsync(h + 4, rs.result + 4, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HR_CUDA(cudaStreamSynchronize(st));
+        const double alpha = h[5] / delta;
+        const double beta = k > 0 ? rho * delta / delta_prev : 0.0;
+        // vt = Dhat v - alpha v - beta v_prev = gamma5 w - alpha v - beta v_prev   (into w)
+        const double ma[2] = { -alpha, 0.0 }, mb[2] = { -beta, 0.0 };
+        rc = launch_lincomb(ctx, P, w, one, 1, w, ma, v, st);
+        if (rc != HR_OK) return rc;
+        if (k > 0) {
+            rc = launch_lincomb(ctx, P, w, one, 0, w, mb, vp, st);
+            if (rc != HR_OK) return rc;
+        }
+        rc = halves(w, &up, &lo);
+        if (rc != HR_OK) return rc;
+        const double rho_next = sqrt(up + lo);
+        const double theta = s2 * beta, t = c2 * beta;
+        const double eps = c1 * t + s1 * alpha, zt = -s1 * t + c1 * alpha;
+        const double zeta = sqrt(zt * zt + rho_next * rho_next);
+        if (zeta == 0.0) break;
+        const double c = zt / zeta, s = rho_next / zeta;
+        // p = (v - eps p1 - theta p2) / zeta, into p2's buffer (p_{k-2} is not needed again)
+        const double iz[2] = { 1.0 / zeta, 0.0 }, mt[2] = { -theta / zeta, 0.0 }, me[2] = { -eps / zeta, 0.0 };
+        rc = launch_lincomb(ctx, P, p2, iz, 0, v, mt, p2, st);
+        if (rc != HR_OK) return rc;
+        rc = launch_lincomb(ctx, P, p2, one, 0, p2, me, p1, st);
+        if (rc != HR_OK) return rc;
+        const double ce[2] = { c * eta, 0.0 };
+        rc = launch_lincomb(ctx, P, x_e, one, 0, x_e, ce, p2, st);                        // x += c eta p
+        if (rc != HR_OK) return rc;
+        eta = -s * eta;
+        ++k;
+        if (hist) hist[k] = fabs(eta) / bnorm;
+        { void *q = p1; p1 = p2; p2 = q; }
+        c2 = c1; s2 = s1; c1 = c; s1 = s;
+        if (rho_next == 0.0) { rc = true_res2(bb, &res2); if (rc != HR_OK) return rc; have_res = true; break; }
+        // v_{k+1} = vt / rho_{k+1} into the old v_prev buffer (before the residual check below, which re-uses w);
+        // delta_{k+1} = (|vt_up|^2 - |vt_lo|^2) / rho_{k+1}^2
+        const double ir[2] = { 1.0 / rho_next, 0.0 };
+        rc = launch_lincomb(ctx, P, vp, ir, 0, w, zero, nullptr, st);
+        if (rc != HR_OK) return rc;
+        { void *q = v; v = vp; vp = q; }
+        delta_prev = delta;
+        delta = (up - lo) / (up + lo);
+        rho = rho_next;
+        if (fabs(eta) <= tol * bnorm) {
+            rc = true_res2(bb, &res2);
+            if (rc != HR_OK) return rc;
+            have_res = true;
+            if (res2 <= tol * tol) break;
+            have_res = false;
+        }
+    }
+    if (!have_res) { rc = true_res2(bb, &res2); if (rc != HR_OK) return rc; }
+    if (iters) *iters = k;
+    if (rel_res2) *rel_res2 = res2;
+    return HR_OK;
+}
+
 hr_status hr_clover_finalize(const hr_ctx *ctx, hr_prec prec, void *site_term, void *site_inverse, double m0, void *stream)
 {
     if (!ctx || !site_term || !site_inverse || !valid_prec(prec) || site_term == site_inverse) { set_error("hr_clover_finalize: bad argument"); return HR_EINVAL; }

@@ -171,6 +171,8 @@ hr_status launch_cvt(const hr_ctx *c, bool down, void *dst, const void *src, dou
 //   result[0..1] = <x, y> (result[0] = |x|^2 when x == y), device pointer
 hr_status launch_dot(const hr_ctx *c, hr_prec prec, const void *x, const void *y, const RedScratch &rs,
                      double *result_dev, cudaStream_t st);
+hr_status launch_dot_range(const hr_ctx *c, hr_prec prec, const void *x, const void *y, size_t first, size_t nvec,
+                           const RedScratch &rs, double *result_dev, cudaStream_t st);
 // CG building blocks on the device-resident CgState (cg.cu)
 hr_status launch_cg_init(const hr_ctx *c, hr_prec prec, CgState *cs, double tol, int maxiter, void *x, void *p,
                          const void *r, const RedScratch &rs, cudaStream_t st);

@@ -191,4 +191,14 @@ hr_status launch_dot(const hr_ctx *c, hr_prec prec, const void *x, const void *y
     return prec == HR_F64 ? dot_t<double>(x, y, nvec, rs, result_dev, st) : dot_t<float>(x, y, nvec, rs, result_dev, st);
 }
 
+// <x, y> over the vectors [first, first + nvec) of the two fields (the upper / lower spin halves of a field are the first
+// and second half of its vectors: gamma5 is a sign pattern on them)
+hr_status launch_dot_range(const hr_ctx *c, hr_prec prec, const void *x, const void *y, size_t first, size_t nvec,
+                           const RedScratch &rs, double *result_dev, cudaStream_t st)
+{
+    (void)c;
+    const char *xp = (const char *)x + first * 16, *yp = (const char *)y + first * 16;
+    return prec == HR_F64 ? dot_t<double>(xp, yp, nvec, rs, result_dev, st) : dot_t<float>(xp, yp, nvec, rs, result_dev, st);
+}
+
 } // namespace hr

@@ -444,3 +444,68 @@ def test_bicgstab_graph_replay_is_bitwise_the_plain_launch_sequence(hr):
     assert res[0][0] == res[2][0] and res[0][1] == res[2][1] and res[0][4] == res[2][4]
     assert np.array_equal(res[0][2], res[2][2]) and np.array_equal(res[0][3], res[2][3])
     prob.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# gamma5-QMR ("QMR gamma_5 inverters"; reading C33)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims,N,rep,m0", CG_CASES)
+def test_qmr_dhat_fp64_follows_the_oracle(hr, dims, N, rep, m0):
+    """Same Lanczos process, same rotations, same stopping rule on both sides: the quasi-residual history |eta_k| / |b|
+    agrees while it is well above rounding, iteration counts to +-1, the reported residual is the true one, the solution
+    solves the oracle's operator."""
+    import torch
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(121, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    b = li.gaussian_spinor(122, li.volume(dims) // 2, d)
+    tol, maxiter = 1e-10, 300
+    x_want, it_want, hist_want, res2_want = solver.qmr_dhat(dims, BC_T, R, m0, b, tol, maxiter)
+    assert 3 < it_want < maxiter and res2_want <= tol * tol
+    prob = GpuProblem(hr, dims, N, rep, "f64", U)
+    f = Fields(hr, prob)
+    gb, gx = f.put(b), f.new()
+    ws = torch.empty(hr.hr_qmr_workspace_bytes(prob.lat.ctx, f.P), dtype=torch.uint8, device="cuda")
+    ws.fill_(0xFF)
+    it, res2, hist = hr.hr_qmr_dhat(prob.lat.ctx, m0, gx, gb, prob.links, tol, maxiter, ws, prob.lat.stream(), want_hist=True)
+    assert abs(it - it_want) <= 1 and hist[0] == 1.0 and len(hist) == it + 1 and res2 <= tol * tol
+    n = min(it, it_want) + 1
+    assert np.allclose(hist[:n], hist_want[:n], rtol=1e-5, atol=1e-13)
+    x = f.get(gx)
+    assert rel_l2(x, x_want) <= 1e-8
+    r = b - solver.dhat(dims, BC_T, R, m0, x)
+    assert np.isclose(res2, solver.norm2(r) / solver.norm2(b), rtol=1e-3, atol=1e-26)   # the TRUE residual
+    # one operator application per iteration: no more iterations than twice the CG's on the normal equations
+    _, it_cg, _ = solver.cg_dhat(dims, BC_T, R, m0, b, tol, 500)
+    assert it <= 2 * it_cg
+    # bitwise reproducible
+    gx2 = f.new()
+    it2, res2b, _ = hr.hr_qmr_dhat(prob.lat.ctx, m0, gx2, gb, prob.links, tol, maxiter, ws, prob.lat.stream())
+    assert it2 == it and res2b == res2 and np.array_equal(f.get(gx2), x)
+    prob.close()
+
+
+def test_qmr_fp32_on_the_fly_links_and_edge_cases(hr):
+    import torch
+    dims, N, m0 = (4, 4, 4, 8), 3, -0.3
+    U = li.haar_links(121, N, dims)
+    R = oracle.represent(N, oracle.REP_SYM, U)
+    b = li.gaussian_spinor(122, li.volume(dims) // 2, 6)
+    x_want, it_want, _, _ = solver.qmr_dhat(dims, BC_T, R, m0, b, 1e-5, 300)
+    prob = GpuProblem(hr, dims, N, "sym", "f32", U)
+    f = Fields(hr, prob)
+    ctx, st = prob.lat.ctx, prob.lat.stream()
+    ws = torch.empty(hr.hr_qmr_workspace_bytes(ctx, f.P), dtype=torch.uint8, device="cuda")
+    gb, gx = f.put(b), f.new()
+    for links in (prob.links, prob.fund):                                                     # represented / on the fly
+        it, res2, _ = hr.hr_qmr_dhat(ctx, m0, gx, gb, links, 1e-5, 300, ws, st)
+        assert abs(it - it_want) <= 2 and res2 <= 1e-10 and rel_l2(f.get(gx), x_want) <= 1e-4
+    it, res2, hist = hr.hr_qmr_dhat(ctx, m0, gx, gb, prob.links, 1e-5, 0, ws, st, want_hist=True)        # maxiter = 0
+    assert it == 0 and abs(res2 - 1.0) <= 1e-6 and not f.get(gx).any()
+    it, res2, _ = hr.hr_qmr_dhat(ctx, m0, gx, f.put(np.zeros_like(b)), prob.links, 1e-5, 50, ws, st)     # b = 0
+    assert it == 0 and res2 == 0.0 and not f.get(gx).any()
+    it, res2, hist = hr.hr_qmr_dhat(ctx, m0, gx, gb, prob.links, 1e-12, 3, ws, st, want_hist=True)       # maxiter hit
+    assert it == 3 and len(hist) == 4 and res2 > 1e-12
+    with pytest.raises(hr.HrError):
+        hr.hr_qmr_dhat(ctx, m0, gb, gb, prob.links, 1e-5, 10, ws, st)
+    prob.close()
