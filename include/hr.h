@@ -293,6 +293,21 @@ size_t hr_halo_bytes(const hr_ctx *ctx, hr_prec prec);
  * hr_dphi_eo_halo_pack.  Ordering between the neighbour's pack and the own apply is the caller's (halo.py:
  * PeerSlabDphi uses one barrier per call).
  */
+/*
+ * 4-D block decomposition ("4-D block partition, split t first, then z, y, x"): the same three steps
+ * for any direction mu in {0: t, 1: x, 2: y, 3: z}.  hr_face_bytes(ctx, prec, mu) = bytes of one message of that direction
+ * (V_local/2 / L_mu face sites x 2 d_R complex); hr_dphi_eo_face_pack / _face_apply are hr_dphi_eo_halo_pack / _halo_apply
+ * for direction mu (the seam sign is bc[mu]); hr_dphi_eo_interior_mask drops the hops across the boundaries of every
+ * direction whose bit is set in split_mask (bit mu).  A rank packs every split direction from the SAME input field, runs
+ * the interior launch, and applies the directions one after the other on the same stream (edge and corner sites receive
+ * a term from each).  Local extents stay even (site parity is global); a split in z needs an even local Y.
+ */
+size_t hr_face_bytes(const hr_ctx *ctx, hr_prec prec, int mu);
+hr_status hr_dphi_eo_face_pack(int mu, void *send_up, void *send_dn, const void *in, const hr_gauge *links, int parity,
+                               void *stream);
+hr_status hr_dphi_eo_interior_mask(void *out, const void *in, const hr_gauge *links, int parity, int split_mask, void *stream);
+hr_status hr_dphi_eo_face_apply(int mu, void *out, const void *recv_prev, const void *recv_next, const hr_gauge *links,
+                                int parity, int first_rank, int last_rank, void *stream);
 hr_status hr_halo_buffers_alloc(const hr_ctx *ctx, hr_prec prec, void **base);
 void hr_halo_buffers_free(const hr_ctx *ctx, void *base);
 hr_status hr_ipc_export(const hr_ctx *ctx, const void *base, unsigned char handle[64]);

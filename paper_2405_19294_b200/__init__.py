@@ -86,6 +86,10 @@ _SIGNATURES = {
     "hr_qmr_dhat": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp, _vp]),
     "hr_dirac_solve": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
     "hr_halo_bytes": (_sz, [_vp, _ci]),
+    "hr_face_bytes": (_sz, [_vp, _ci, _ci]),
+    "hr_dphi_eo_face_pack": (_ci, [_ci, _vp, _vp, _vp, _vp, _ci, _vp]),
+    "hr_dphi_eo_interior_mask": (_ci, [_vp, _vp, _vp, _ci, _ci, _vp]),
+    "hr_dphi_eo_face_apply": (_ci, [_ci, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _vp]),
     "hr_halo_buffers_alloc": (_ci, [_vp, _ci, ctypes.POINTER(_vp)]),
     "hr_halo_buffers_free": (None, [_vp, _vp]),
     "hr_ipc_export": (_ci, [_vp, _vp, ctypes.c_char_p]),
@@ -344,6 +348,24 @@ def hr_dirac_solve(ctx: int, m0: float, x_full, b_full, links: int, tol: float, 
 
 def hr_halo_bytes(ctx: int, prec: int) -> int:
     return _lib.hr_halo_bytes(ctx, prec)
+
+
+def hr_face_bytes(ctx: int, prec: int, mu: int) -> int:
+    return _lib.hr_face_bytes(ctx, prec, mu)
+
+
+def hr_dphi_eo_face_pack(mu: int, send_up, send_dn, inp, links: int, parity: int, stream: int = 0) -> None:
+    _check(_lib.hr_dphi_eo_face_pack(mu, _ptr(send_up), _ptr(send_dn), _ptr(inp), links, parity, stream))
+
+
+def hr_dphi_eo_interior_mask(out, inp, links: int, parity: int, split_mask: int, stream: int = 0) -> None:
+    _check(_lib.hr_dphi_eo_interior_mask(_ptr(out), _ptr(inp), links, parity, split_mask, stream))
+
+
+def hr_dphi_eo_face_apply(mu: int, out, recv_prev, recv_next, links: int, parity: int, first_rank: int, last_rank: int,
+                          stream: int = 0) -> None:
+    _check(_lib.hr_dphi_eo_face_apply(mu, _ptr(out), _ptr(recv_prev), _ptr(recv_next), links, parity, int(first_rank),
+                                      int(last_rank), stream))
 
 
 def hr_halo_buffers_alloc(ctx: int, prec: int) -> int:

@@ -105,6 +105,20 @@ def main():
     ops.append(("dphi_eo_interior", dphi_c, lambda k: hr.hr_dphi_eo_interior(sets[k % nset][2], sets[k % nset][0], links, k & 1, st)))
     ops.append(("halo_apply", None, lambda k: hr.hr_dphi_eo_halo_apply(sets[k % nset][2], hb[0], hb[1], links, k & 1, True, True, st)))
     face_bytes = {"halo_pack": nface * (2 * S + Lk + S), "halo_apply": nface * (S + Lk + 4 * S)}
+    face_sites = {"halo_pack": nface, "halo_apply": nface}
+    # 4-D block decomposition: the face kernels of the other directions (strided faces) and the interior launch with all
+    # four directions masked
+    fb = {}
+    for mu, nm in ((1, "x"), (2, "y"), (3, "z")):
+        nf_mu = vh // cfg["dims"][mu]
+        fb[mu] = [torch.empty(hr.hr_face_bytes(ctx, P, mu), dtype=torch.uint8, device="cuda") for _ in range(2)]
+        ops.append((f"face_pack {nm}", None, lambda k, mu=mu: hr.hr_dphi_eo_face_pack(mu, fb[mu][0], fb[mu][1], sets[k % nset][0], links, k & 1, st)))
+        ops.append((f"face_apply {nm}", None, lambda k, mu=mu: hr.hr_dphi_eo_face_apply(mu, sets[k % nset][2], fb[mu][0], fb[mu][1], links, k & 1, True, True, st)))
+        face_bytes[f"face_pack {nm}"] = nf_mu * (2 * S + Lk + S)
+        face_bytes[f"face_apply {nm}"] = nf_mu * (S + Lk + 4 * S)
+        face_sites[f"face_pack {nm}"] = face_sites[f"face_apply {nm}"] = nf_mu
+    ops.append(("dphi_eo_interior, all four directions masked", dphi_c,
+                lambda k: hr.hr_dphi_eo_interior_mask(sets[k % nset][2], sets[k % nset][0], links, k & 1, 15, st)))
     # NEXT-4: clover term.  build: reads the represented links (each link is used by many leaves; algorithmic bytes
     # 4L + C per site), apply as part of hr_dirac_clover: two Dphi launches with the mass term + two site-local launches
     # (C + 3S per site each); bytes per site of the full lattice: 2(8L+3S)/2 ... reported per output site of one parity.
@@ -129,7 +143,7 @@ def main():
         ms = timed(fn, args.reps)
         if bps is None:   # face kernels: bytes are per launch, not per site of the volume
             gbs = face_bytes[name] / (ms * 1e-3) / 1e9
-            print(json.dumps(dict(common, op=name, bytes_per_launch=face_bytes[name], face_sites=nface, ms=ms, gbs=gbs, frac=gbs / peak)))
+            print(json.dumps(dict(common, op=name, bytes_per_launch=face_bytes[name], face_sites=face_sites[name], ms=ms, gbs=gbs, frac=gbs / peak)))
             continue
         gbs = bps * vh / (ms * 1e-3) / 1e9
         print(json.dumps(dict(common, op=name, bytes_per_site=bps, ms=ms, gbs=gbs, frac=gbs / peak)))

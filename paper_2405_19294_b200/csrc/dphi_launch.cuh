@@ -158,11 +158,19 @@ template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant)
     return true;
 }
 
-template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, const HaloArgs &a, cudaStream_t st)
+template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, int mu, const HaloArgs &a, cudaStream_t st)
 {
     const unsigned grid = (unsigned)((a.nface + 127) / 128);
-    if (pack) halo_pack_kernel<Real, D, LK><<<grid, 128, 0, st>>>(a);
-    else halo_apply_kernel<Real, D, LK><<<grid, 128, 0, st>>>(a);
+#define HR_HALO_MU(M)                                                                                     \
+    case M:                                                                                               \
+        if (pack) halo_pack_kernel<Real, D, LK, M><<<grid, 128, 0, st>>>(a);                              \
+        else halo_apply_kernel<Real, D, LK, M><<<grid, 128, 0, st>>>(a);                                  \
+        break;
+    switch (mu) {
+        HR_HALO_MU(0) HR_HALO_MU(1) HR_HALO_MU(2) HR_HALO_MU(3)
+    default: set_error("halo kernels: direction %d", mu); return HR_EINVAL;
+    }
+#undef HR_HALO_MU
     count_launch();
     cudaError_t e = cudaPeekAtLastError();
     if (e != cudaSuccess) {
@@ -175,6 +183,6 @@ template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, const
 #define HR_DPHI_INSTANCE(Real, D, LK)                                                                    \
     template hr_status launch_dphi_t<Real, D, LK>(int, int, const DphiArgs &, cudaStream_t);             \
     template bool dphi_variant_ok_t<Real, D, LK>(int);                                                    \
-    template hr_status launch_halo_t<Real, D, LK>(bool, const HaloArgs &, cudaStream_t);
+    template hr_status launch_halo_t<Real, D, LK>(bool, int, const HaloArgs &, cudaStream_t);
 
 } // namespace hr

@@ -16,39 +16,89 @@
 //                      contribute nothing; runs while the messages travel.
 //   halo_apply_kernel  one thread per face site: out(t=0) += beta s_prev R+(chi_recv), out(t=T_l-1) += beta s_next
 //                      R-(U_0(x) h_recv); s = bc[0] on the global seam (rank 0's first / last rank's last slice).
-// Face buffers use the plane layout of hr_internal.h: [16-byte vector v][face site f], f = (x*Y + y)*Zh + zh.
+// Face buffers use the plane layout of hr_internal.h: [16-byte vector v][face site f].
+//
+// 4-D block decomposition: the same two kernels for every direction MU.  With the projector table of dphi_kernel.cuh
+// (h_k = psi_k + sk_k c psi_{p(k)}, c = +c0 forward / -c0 backward, c0 = 1 (mu = 0,2) or i (mu = 1,3)):
+//   "down" message (to the previous rank in MU): h = P^-_mu psi of my FIRST slice x_mu = 0 (forward projector);
+//   "up" message (to the next rank in MU): chi = U_mu(y)^dagger P^+_mu psi of my LAST slice x_mu = L_mu - 1.
+// Face sites of direction MU are enumerated as f = the half index with the coordinate x_mu dropped (mu = 0,1,2: one site
+// per (other coordinates, zh)); for mu = 3 the face z = 0 holds the sites with offset bit b = 0 and the face z = Z-1 those
+// with b = 1, one per (t, x, y/2), y's parity fixed by the site parity -- sender and receiver enumerate them alike.
 #pragma once
 #include "dphi_kernel.cuh"
 
 namespace hr {
 
+// half index of face site f of direction MU on the first (side 0) or last (side 1) slice, for sites of parity `par`
+template <int MU> __device__ __forceinline__ size_t face_site(const HaloArgs &a, int par, int side, long f)
+{
+    const unsigned X = (unsigned)a.X, Y = (unsigned)a.Y, Zh = (unsigned)a.Zh;
+    unsigned r = (unsigned)f;
+    if constexpr (MU == 0) {
+        return (size_t)f + (side ? (size_t)(a.T - 1) * X * Y * Zh : 0);
+    } else if constexpr (MU == 1) {
+        const unsigned zh = r % Zh; r /= Zh;
+        const unsigned y = r % Y, t = r / Y, x = side ? X - 1 : 0;
+        return (((size_t)t * X + x) * Y + y) * Zh + zh;
+    } else if constexpr (MU == 2) {
+        const unsigned zh = r % Zh; r /= Zh;
+        const unsigned x = r % X, t = r / X, y = side ? Y - 1 : 0;
+        return (((size_t)t * X + x) * Y + y) * Zh + zh;
+    } else {
+        const unsigned Yh = Y / 2;
+        const unsigned yh = r % Yh; r /= Yh;
+        const unsigned x = r % X, t = r / X;
+        const unsigned y = 2 * yh + ((t + x + (unsigned)par + (unsigned)side) & 1u);   // offset bit b = side
+        return (((size_t)t * X + x) * Y + y) * Zh + (side ? Zh - 1 : 0);
+    }
+}
 
-template <typename Real, int D, int LK>
+template <int MU> struct HopTable {
+    static constexpr int CRE = (MU == 0 || MU == 2) ? 1 : 0;   // c0
+    static constexpr int CIM = (MU == 0 || MU == 2) ? 0 : 1;
+    static constexpr int P0 = (MU == 0 || MU == 3) ? 2 : 3;
+    static constexpr int P1 = 5 - P0;
+};
+
+template <typename Real, int D, int LK, int MU>
 __global__ void __launch_bounds__(128) halo_pack_kernel(const HaloArgs a)
 {
     constexpr int LNREAL = LinkGeom<LK, D>::NREAL;
     constexpr int RPV = 16 / (int)sizeof(Real);
     constexpr size_t LB = (size_t)LNREAL * sizeof(Real);
+    using H = HopTable<MU>;
     const long f = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (f >= a.nface) return;
     const size_t vh = (size_t)a.vh, nf = (size_t)a.nface;
     const char *in = (const char *)a.in;
-    // down message: first slice, h = (psi0 + psi2, psi1 + psi3)
+    const int q = 1 - a.parity;                         // parity of the input sites
+    const Real sk1 = (Real)(MU >= 2 ? -1 : 1);
+    // down message: first slice, forward projector h_k = psi_k + sk_k c0 psi_{p(k)}
     {
+        const size_t sy = face_site<MU>(a, q, 0, f);
         Real psi[8 * D], h[4 * D];
-        load_record<LD_DEFAULT, 8 * D>(psi, in, vh, (size_t)f, 0);
+        load_record<LD_DEFAULT, 8 * D>(psi, in, vh, sy, 0);
 #pragma unroll
-        for (int c = 0; c < 2 * D; ++c) { h[c] = psi[c] + psi[4 * D + c]; h[2 * D + c] = psi[2 * D + c] + psi[6 * D + c]; }
+        for (int c = 0; c < D; ++c) {
+            add_c<H::CRE, H::CIM>(h[2 * c], h[2 * c + 1], psi[2 * c], psi[2 * c + 1], psi[H::P0 * 2 * D + 2 * c], psi[H::P0 * 2 * D + 2 * c + 1], (Real)1);
+            add_c<H::CRE, H::CIM>(h[2 * D + 2 * c], h[2 * D + 2 * c + 1], psi[2 * D + 2 * c], psi[2 * D + 2 * c + 1],
+                                  psi[H::P1 * 2 * D + 2 * c], psi[H::P1 * 2 * D + 2 * c + 1], sk1);
+        }
         store_planes<ST_DEFAULT, 4 * D / RPV>((char *)a.send_dn + (size_t)f * 16, nf * 16, h);
     }
-    // up message: last slice, chi = U_0(y)^dagger (psi0 - psi2, psi1 - psi3); U_0(y) is based at the INPUT parity
+    // up message: last slice, chi = U_mu(y)^dagger (psi_k - sk_k c0 psi_{p(k)}); U_mu(y) is based at the INPUT parity
     {
-        const size_t sy = (size_t)(a.Tl - 1) * nf + (size_t)f;
+        const size_t sy = face_site<MU>(a, q, 1, f);
         Real psi[8 * D], u[LNREAL], h0[2 * D], h1[2 * D], c0[2 * D], c1[2 * D], chi[4 * D];
         load_record<LD_DEFAULT, 8 * D>(psi, in, vh, sy, 0);
-        load_record<LD_STREAM, LNREAL>(u, (const char *)a.links + (size_t)((1 - a.parity) * 4) * LB * vh, vh, sy, 0);
+        load_record<LD_STREAM, LNREAL>(u, (const char *)a.links + (size_t)(q * 4 + MU) * LB * vh, vh, sy, 0);
 #pragma unroll
-        for (int c = 0; c < 2 * D; ++c) { h0[c] = psi[c] - psi[4 * D + c]; h1[c] = psi[2 * D + c] - psi[6 * D + c]; }
+        for (int c = 0; c < D; ++c) {
+            add_c<-H::CRE, -H::CIM>(h0[2 * c], h0[2 * c + 1], psi[2 * c], psi[2 * c + 1], psi[H::P0 * 2 * D + 2 * c], psi[H::P0 * 2 * D + 2 * c + 1], (Real)1);
+            add_c<-H::CRE, -H::CIM>(h1[2 * c], h1[2 * c + 1], psi[2 * D + 2 * c], psi[2 * D + 2 * c + 1],
+                                    psi[H::P1 * 2 * D + 2 * c], psi[H::P1 * 2 * D + 2 * c + 1], sk1);
+        }
         link_mul<D, LK, true>(c0, u, h0);
         link_mul<D, LK, true>(c1, u, h1);
 #pragma unroll
@@ -57,35 +107,45 @@ __global__ void __launch_bounds__(128) halo_pack_kernel(const HaloArgs a)
     }
 }
 
-template <typename Real, int D, int LK>
+template <typename Real, int D, int LK, int MU>
 __global__ void __launch_bounds__(128) halo_apply_kernel(const HaloArgs a)
 {
     constexpr int LNREAL = LinkGeom<LK, D>::NREAL;
     constexpr int RPV = 16 / (int)sizeof(Real);
     constexpr size_t LB = (size_t)LNREAL * sizeof(Real);
+    using H = HopTable<MU>;
     const long f = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (f >= a.nface) return;
     const size_t vh = (size_t)a.vh, nf = (size_t)a.nface;
     Real be[2];
     if constexpr (sizeof(Real) == 8) { be[0] = (Real)a.beta[0]; be[1] = (Real)a.beta[1]; }
     else { be[0] = a.betaf[0]; be[1] = a.betaf[1]; }
+    const Real sk1 = (Real)(MU >= 2 ? -1 : 1);
     char *out = (char *)a.out;
-    // slice 0: backward hop from the previous rank, (1+gamma_0) chi = (chi0, chi1, -chi0, -chi1)
+    // first slice: backward hop from the previous rank; reconstruct with c = -c0:  out_k += chi_k, out_{p(k)} += sk_k conj(-c0) chi_k
     {
+        const size_t sx = face_site<MU>(a, a.parity, 0, f);
         Real chi[4 * D], o[8 * D];
         load_planes<LD_STREAM, 4 * D / RPV>(chi, (const char *)a.recv_prev + (size_t)f * 16, nf * 16, 0);
-        load_record<LD_DEFAULT, 8 * D>(o, out, vh, (size_t)f, 0);
+        load_record<LD_DEFAULT, 8 * D>(o, out, vh, sx, 0);
         const Real s0 = be[0] * (Real)a.sign_prev, s1 = be[1] * (Real)a.sign_prev;
 #pragma unroll
-        for (int c = 0; c < 4 * D; ++c) { o[c] = fma(s0, chi[c], o[c]); o[4 * D + c] = fma(-s1, chi[c], o[4 * D + c]); }
-        store_planes<ST_DEFAULT, 8 * D / RPV>(out + (size_t)f * 16, vh * 16, o);
+        for (int c = 0; c < D; ++c) {
+            o[2 * c] = fma(s0, chi[2 * c], o[2 * c]);
+            o[2 * c + 1] = fma(s0, chi[2 * c + 1], o[2 * c + 1]);
+            o[2 * D + 2 * c] = fma(s0, chi[2 * D + 2 * c], o[2 * D + 2 * c]);
+            o[2 * D + 2 * c + 1] = fma(s0, chi[2 * D + 2 * c + 1], o[2 * D + 2 * c + 1]);
+            acc_conj_c<-H::CRE, -H::CIM>(o[H::P0 * 2 * D + 2 * c], o[H::P0 * 2 * D + 2 * c + 1], chi[2 * c], chi[2 * c + 1], s1);
+            acc_conj_c<-H::CRE, -H::CIM>(o[H::P1 * 2 * D + 2 * c], o[H::P1 * 2 * D + 2 * c + 1], chi[2 * D + 2 * c], chi[2 * D + 2 * c + 1], s1 * sk1);
+        }
+        store_planes<ST_DEFAULT, 8 * D / RPV>(out + sx * 16, vh * 16, o);
     }
-    // slice T_l-1: forward hop to the next rank, (1-gamma_0) U_0(x) h = (chi0, chi1, chi0, chi1), own link
+    // last slice: forward hop to the next rank, chi = U_mu(x) h_recv with the OWN link; reconstruct with c = +c0
     {
-        const size_t sx = (size_t)(a.Tl - 1) * nf + (size_t)f;
+        const size_t sx = face_site<MU>(a, a.parity, 1, f);
         Real h[4 * D], u[LNREAL], h0[2 * D], h1[2 * D], c0[2 * D], c1[2 * D], o[8 * D];
         load_planes<LD_STREAM, 4 * D / RPV>(h, (const char *)a.recv_next + (size_t)f * 16, nf * 16, 0);
-        load_record<LD_STREAM, LNREAL>(u, (const char *)a.links + (size_t)(a.parity * 4) * LB * vh, vh, sx, 0);
+        load_record<LD_STREAM, LNREAL>(u, (const char *)a.links + (size_t)(a.parity * 4 + MU) * LB * vh, vh, sx, 0);
         load_record<LD_DEFAULT, 8 * D>(o, out, vh, sx, 0);
 #pragma unroll
         for (int c = 0; c < 2 * D; ++c) { h0[c] = h[c]; h1[c] = h[2 * D + c]; }
@@ -93,11 +153,13 @@ __global__ void __launch_bounds__(128) halo_apply_kernel(const HaloArgs a)
         link_mul<D, LK, false>(c1, u, h1);
         const Real s0 = be[0] * (Real)a.sign_next, s1 = be[1] * (Real)a.sign_next;
 #pragma unroll
-        for (int c = 0; c < 2 * D; ++c) {
-            o[c] = fma(s0, c0[c], o[c]);
-            o[2 * D + c] = fma(s0, c1[c], o[2 * D + c]);
-            o[4 * D + c] = fma(s1, c0[c], o[4 * D + c]);
-            o[6 * D + c] = fma(s1, c1[c], o[6 * D + c]);
+        for (int c = 0; c < D; ++c) {
+            o[2 * c] = fma(s0, c0[2 * c], o[2 * c]);
+            o[2 * c + 1] = fma(s0, c0[2 * c + 1], o[2 * c + 1]);
+            o[2 * D + 2 * c] = fma(s0, c1[2 * c], o[2 * D + 2 * c]);
+            o[2 * D + 2 * c + 1] = fma(s0, c1[2 * c + 1], o[2 * D + 2 * c + 1]);
+            acc_conj_c<H::CRE, H::CIM>(o[H::P0 * 2 * D + 2 * c], o[H::P0 * 2 * D + 2 * c + 1], c0[2 * c], c0[2 * c + 1], s1);
+            acc_conj_c<H::CRE, H::CIM>(o[H::P1 * 2 * D + 2 * c], o[H::P1 * 2 * D + 2 * c + 1], c1[2 * c], c1[2 * c + 1], s1 * sk1);
         }
         store_planes<ST_DEFAULT, 8 * D / RPV>(out + sx * 16, vh * 16, o);
     }

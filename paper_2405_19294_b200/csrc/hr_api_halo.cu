@@ -20,7 +20,9 @@ static hr_status check_links(const char *who, const hr_gauge *links, int parity)
     return use_device(links->ctx);
 }
 
-static void halo_common(HaloArgs &a, const hr_ctx *c, const hr_gauge *links, int parity)
+static long face_sites(const hr_ctx *c, int mu) { return c->Vh / c->dims[mu]; }
+
+static void halo_common(HaloArgs &a, const hr_ctx *c, const hr_gauge *links, int parity, int mu)
 {
     a.send_up = a.send_dn = nullptr;
     a.recv_prev = a.recv_next = nullptr;
@@ -29,8 +31,8 @@ static void halo_common(HaloArgs &a, const hr_ctx *c, const hr_gauge *links, int
     a.links = links->data;
     a.parity = parity;
     a.vh = c->Vh;
-    a.nface = (long)c->dims[1] * c->dims[2] * (c->dims[3] / 2);
-    a.Tl = c->dims[0];
+    a.nface = face_sites(c, mu);
+    a.T = c->dims[0]; a.X = c->dims[1]; a.Y = c->dims[2]; a.Zh = c->dims[3] / 2;
     a.beta[0] = a.beta[1] = -0.5;
     a.betaf[0] = a.betaf[1] = -0.5f;
     a.sign_prev = a.sign_next = 1;
@@ -38,15 +40,31 @@ static void halo_common(HaloArgs &a, const hr_ctx *c, const hr_gauge *links, int
 
 extern "C" {
 
-size_t hr_halo_bytes(const hr_ctx *ctx, hr_prec prec)
+size_t hr_face_bytes(const hr_ctx *ctx, hr_prec prec, int mu)
 {
-    if (!ctx || (prec != HR_F64 && prec != HR_F32)) return 0;
-    return (size_t)ctx->dims[1] * ctx->dims[2] * (ctx->dims[3] / 2) * 4 * ctx->d * prec_bytes(prec);
+    if (!ctx || (prec != HR_F64 && prec != HR_F32) || mu < 0 || mu > 3) return 0;
+    return (size_t)face_sites(ctx, mu) * 4 * ctx->d * prec_bytes(prec);
 }
+
+size_t hr_halo_bytes(const hr_ctx *ctx, hr_prec prec) { return hr_face_bytes(ctx, prec, 0); }
 
 hr_status hr_dphi_eo_halo_pack(void *send_up, void *send_dn, const void *in, const hr_gauge *links, int parity, void *stream)
 {
+    return hr_dphi_eo_face_pack(0, send_up, send_dn, in, links, parity, stream);
+}
+
+static hr_status check_mu(const char *who, const hr_gauge *links, int mu)
+{
+    if (mu < 0 || mu > 3) { set_error("%s: direction %d", who, mu); return HR_EINVAL; }
+    if (mu == 3 && (links->ctx->dims[2] & 1)) { set_error("%s: a split in z needs an even Y", who); return HR_EINVAL; }
+    return HR_OK;
+}
+
+hr_status hr_dphi_eo_face_pack(int mu, void *send_up, void *send_dn, const void *in, const hr_gauge *links, int parity, void *stream)
+{
     hr_status rc = check_links("hr_dphi_eo_halo_pack", links, parity);
+    if (rc != HR_OK) return rc;
+    rc = check_mu("hr_dphi_eo_face_pack", links, mu);
     if (rc != HR_OK) return rc;
     if (!send_up || !send_dn || !in) { set_error("hr_dphi_eo_halo_pack: NULL buffer"); return HR_EINVAL; }
     if (!aligned16(send_up) || !aligned16(send_dn) || !aligned16(in) || send_up == send_dn) {
@@ -54,30 +72,46 @@ hr_status hr_dphi_eo_halo_pack(void *send_up, void *send_dn, const void *in, con
         return HR_EINVAL;
     }
     HaloArgs a;
-    halo_common(a, links->ctx, links, parity);
+    halo_common(a, links->ctx, links, parity, mu);
     a.send_up = send_up;
     a.send_dn = send_dn;
     a.in = in;
-    return launch_halo(links->ctx, links->prec, true, a, (cudaStream_t)stream, link_src(links));
+    return launch_halo(links->ctx, links->prec, true, mu, a, (cudaStream_t)stream, link_src(links));
 }
 
 hr_status hr_dphi_eo_interior(void *out, const void *in, const hr_gauge *links, int parity, void *stream)
 {
+    return hr_dphi_eo_interior_mask(out, in, links, parity, 1, stream);
+}
+
+hr_status hr_dphi_eo_interior_mask(void *out, const void *in, const hr_gauge *links, int parity, int split_mask, void *stream)
+{
     hr_status rc = check_links("hr_dphi_eo_interior", links, parity);
     if (rc != HR_OK) return rc;
+    if (split_mask < 0 || split_mask > 15) { set_error("hr_dphi_eo_interior_mask: split_mask=%d", split_mask); return HR_EINVAL; }
     if (!out || !in || out == in || !aligned16(out) || !aligned16(in)) { set_error("hr_dphi_eo_interior: bad buffers"); return HR_EINVAL; }
     const hr_ctx *c = links->ctx;
     DphiArgs a;
     const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 };
     dphi_args(a, c, out, in, nullptr, links, parity, zero, mhalf);
-    a.bc[0] = 0; // a hop across the slab boundary contributes nothing here: hr_dphi_eo_halo_apply adds it
+    // a hop across the boundary of a split direction contributes nothing here: hr_dphi_eo_face_apply adds it
+    for (int mu = 0; mu < 4; ++mu)
+        if (split_mask & (1 << mu)) a.bc[mu] = 0;
     return launch_dphi(c, links->prec, a, (cudaStream_t)stream, link_src(links));
 }
 
 hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *recv_next, const hr_gauge *links, int parity,
                                 int first_rank, int last_rank, void *stream)
 {
+    return hr_dphi_eo_face_apply(0, out, recv_prev, recv_next, links, parity, first_rank, last_rank, stream);
+}
+
+hr_status hr_dphi_eo_face_apply(int mu, void *out, const void *recv_prev, const void *recv_next, const hr_gauge *links, int parity,
+                                int first_rank, int last_rank, void *stream)
+{
     hr_status rc = check_links("hr_dphi_eo_halo_apply", links, parity);
+    if (rc != HR_OK) return rc;
+    rc = check_mu("hr_dphi_eo_face_apply", links, mu);
     if (rc != HR_OK) return rc;
     if (!out || !recv_prev || !recv_next) { set_error("hr_dphi_eo_halo_apply: NULL buffer"); return HR_EINVAL; }
     if (!aligned16(out) || !aligned16(recv_prev) || !aligned16(recv_next)) {
@@ -86,13 +120,13 @@ hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *re
     }
     const hr_ctx *c = links->ctx;
     HaloArgs a;
-    halo_common(a, c, links, parity);
+    halo_common(a, c, links, parity, mu);
     a.out = out;
     a.recv_prev = recv_prev;
     a.recv_next = recv_next;
-    a.sign_prev = first_rank ? c->bc[0] : 1; // the global seam lies below rank 0's first slice ...
-    a.sign_next = last_rank ? c->bc[0] : 1;  // ... and above the last rank's last slice (reading C9)
-    return launch_halo(c, links->prec, false, a, (cudaStream_t)stream, link_src(links));
+    a.sign_prev = first_rank ? c->bc[mu] : 1; // the global seam lies below the first rank's first slice ...
+    a.sign_next = last_rank ? c->bc[mu] : 1;  // ... and above the last rank's last slice (reading C9)
+    return launch_halo(c, links->prec, false, mu, a, (cudaStream_t)stream, link_src(links));
 }
 
 // ---- face buffers in peer-accessible memory ---------------------------------------------------------------------

@@ -143,13 +143,13 @@ struct HaloArgs {
     void *out;             // apply: parity-p half field, already holding the interior result
     const void *links;
     int parity;            // p, parity of the OUTPUT sites of the Dphi_eo being assembled
-    long vh, nface;        // V_local/2, X*Y*Zh
-    int Tl;
+    long vh, nface;        // V_local/2; face sites of the direction (V_local/2 / L_mu)
+    int T, X, Y, Zh;       // local extents
     double beta[2];        // coefficient of the hop sum in the interior launch (-1/2 for plain Dphi)
     float betaf[2];
     int sign_prev, sign_next; // seam signs of the two faces (+-1)
 };
-hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, const HaloArgs &a, cudaStream_t st, int link_src);
+hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, int mu, const HaloArgs &a, cudaStream_t st, int link_src);
 
 // clover term (clover.cu): record of 8 d_R^2 reals per site, [parity] fields
 size_t clover_nreal(const hr_ctx *c);

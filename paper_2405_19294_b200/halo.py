@@ -200,3 +200,80 @@ class SlabCG:
             k += 1
             hist.append(rr / bb)
         return k, hist
+
+
+# ---- 4-D block decomposition ("4-D block partition, split t first, then z, y, x") ------------------
+def block_plan(rank: int, grid, dims_global) -> dict:
+    """Ranks form a grid (P_t, P_x, P_y, P_z), rank = ((c_t P_x + c_x) P_y + c_y) P_z + c_z; every rank owns a block of
+    dims_global / grid sites with EVEN local extents (site parity is global).  Per direction mu: the neighbour ranks
+    (periodic), whether this rank holds the first / last block (where the global seam bc[mu] sits) and whether the
+    direction is split at all (P_mu > 1; an unsplit direction stays periodic inside the rank)."""
+    grid = tuple(int(g) for g in grid)
+    dims_global = tuple(int(v) for v in dims_global)
+    world = grid[0] * grid[1] * grid[2] * grid[3]
+    if len(grid) != 4 or min(grid) < 1 or not (0 <= rank < world):
+        raise ValueError("bad rank/grid")
+    local = []
+    for mu in range(4):
+        if dims_global[mu] % grid[mu] or (dims_global[mu] // grid[mu]) % 2 or dims_global[mu] // grid[mu] < 2:
+            raise ValueError(f"extent {dims_global[mu]} of direction {mu} must split into {grid[mu]} blocks of even extent >= 2")
+        local.append(dims_global[mu] // grid[mu])
+    if grid[3] > 1 and local[2] % 2:
+        raise ValueError("a split in z needs an even local Y")
+    c = [0, 0, 0, 0]
+    r = rank
+    for mu in (3, 2, 1, 0):
+        c[mu] = r % grid[mu]
+        r //= grid[mu]
+
+    def rank_of(cc):
+        return ((cc[0] * grid[1] + cc[1]) * grid[2] + cc[2]) * grid[3] + cc[3]
+
+    prev, nxt = [], []
+    for mu in range(4):
+        a, b = list(c), list(c)
+        a[mu] = (c[mu] - 1) % grid[mu]
+        b[mu] = (c[mu] + 1) % grid[mu]
+        prev.append(rank_of(a))
+        nxt.append(rank_of(b))
+    return {"grid": grid, "coords": tuple(c), "dims_local": tuple(local), "origin": tuple(c[mu] * local[mu] for mu in range(4)),
+            "prev": prev, "next": nxt, "first": [c[mu] == 0 for mu in range(4)], "last": [c[mu] == grid[mu] - 1 for mu in range(4)],
+            "split": [mu for mu in range(4) if grid[mu] > 1], "mask": sum(1 << mu for mu in range(4) if grid[mu] > 1)}
+
+
+class BlockDphi:
+    """Distributed Dphi_eo of one rank of a 4-D block decomposition: for every split direction the four face buffers;
+    pack (all directions, same input) -> interior launch with the split directions masked || exchange -> apply
+    direction by direction on the same stream."""
+
+    def __init__(self, lat, prec: int, plan: dict, group=None):
+        import torch
+        from . import hr_face_bytes
+        self.lat, self.prec, self.plan, self.group = lat, prec, plan, group
+        dev = f"cuda:{lat.device}"
+        self.buf = {mu: [torch.empty(hr_face_bytes(lat.ctx, prec, mu), dtype=torch.uint8, device=dev) for _ in range(4)]
+                    for mu in plan["split"]}                      # send_up, send_dn, recv_prev, recv_next
+
+    def pack(self, inp, links: int, parity: int) -> None:
+        from . import hr_dphi_eo_face_pack
+        for mu, (su, sd, _, _) in self.buf.items():
+            hr_dphi_eo_face_pack(mu, su, sd, inp, links, parity, self.lat.stream())
+
+    def interior(self, out, inp, links: int, parity: int) -> None:
+        from . import hr_dphi_eo_interior_mask
+        hr_dphi_eo_interior_mask(out, inp, links, parity, self.plan["mask"], self.lat.stream())
+
+    def exchange(self) -> None:
+        for mu, (su, sd, rp, rn) in self.buf.items():
+            exchange(su, sd, rp, rn, {"prev": self.plan["prev"][mu], "next": self.plan["next"][mu]}, self.group)
+
+    def apply(self, out, links: int, parity: int) -> None:
+        from . import hr_dphi_eo_face_apply
+        for mu, (_, _, rp, rn) in self.buf.items():
+            hr_dphi_eo_face_apply(mu, out, rp, rn, links, parity, self.plan["first"][mu], self.plan["last"][mu], self.lat.stream())
+
+    def dphi_eo(self, out, inp, links: int, parity: int) -> None:
+        self.pack(inp, links, parity)
+        self.interior(out, inp, links, parity)
+        self.exchange()
+        self.apply(out, links, parity)

@@ -4,6 +4,7 @@ MAX over ranks of the measured time.  Checked here: replica seeds differ per ran
 max_over_ranks returns the slowest rank's time on every rank, value = units of all ranks / that time, and
 `bench.py --impl reference` lets rank 0 alone print a line."""
 import json
+import itertools
 import os
 import socket
 import subprocess
@@ -116,3 +117,18 @@ def test_slab_plan_rejects_bad_splits():
         with pytest.raises(ValueError):
             halo.slab_plan(0, world, T)
     assert halo.slab_plan(2, 4, 16) == {"T_local": 4, "t0": 8, "prev": 1, "next": 3, "first_rank": False, "last_rank": False}
+
+
+def test_block_plan_neighbours_and_errors():
+    import pytest
+    sys.path.insert(0, ROOT)
+    from paper_2405_19294_b200 import halo
+    p = halo.block_plan(5, (2, 2, 2, 1), (8, 8, 8, 4))          # rank 5 = coords (1, 0, 1, 0)
+    assert p["coords"] == (1, 0, 1, 0) and p["dims_local"] == (4, 4, 4, 4) and p["origin"] == (4, 0, 4, 0)
+    assert p["prev"] == [1, 7, 4, 5] and p["next"] == [1, 7, 4, 5] and p["split"] == [0, 1, 2] and p["mask"] == 7
+    assert p["first"] == [False, True, False, True] and p["last"] == [True, False, True, True]
+    for grid, dims in (((3, 1, 1, 1), (8, 4, 4, 4)), ((2, 1, 1, 1), (6, 4, 4, 4)), ((1, 1, 1, 4), (4, 4, 4, 4))):
+        with pytest.raises(ValueError):
+            halo.block_plan(0, grid, dims)
+    ranks = {tuple(halo.block_plan(r, (2, 1, 2, 2), (4, 4, 4, 4))["coords"]) for r in range(8)}
+    assert ranks == set(itertools.product((0, 1), (0,), (0, 1), (0, 1)))
