@@ -308,7 +308,8 @@ hr_status hr_dphi_eo_face_pack(int mu, void *send_up, void *send_dn, const void 
 hr_status hr_dphi_eo_interior_mask(void *out, const void *in, const hr_gauge *links, int parity, int split_mask, void *stream);
 hr_status hr_dphi_eo_face_apply(int mu, void *out, const void *recv_prev, const void *recv_next, const hr_gauge *links,
                                 int parity, int first_rank, int last_rank, void *stream);
-hr_status hr_halo_buffers_alloc(const hr_ctx *ctx, hr_prec prec, void **base);
+hr_status hr_halo_buffers_alloc(const hr_ctx *ctx, hr_prec prec, void **base);             /* direction t */
+hr_status hr_face_buffers_alloc(const hr_ctx *ctx, hr_prec prec, int mu, void **base);     /* 6 hr_face_bytes(mu) */
 void hr_halo_buffers_free(const hr_ctx *ctx, void *base);
 hr_status hr_ipc_export(const hr_ctx *ctx, const void *base, unsigned char handle[64]);
 hr_status hr_ipc_open(const hr_ctx *ctx, const unsigned char handle[64], void **peer_base);

@@ -91,6 +91,7 @@ _SIGNATURES = {
     "hr_dphi_eo_interior_mask": (_ci, [_vp, _vp, _vp, _ci, _ci, _vp]),
     "hr_dphi_eo_face_apply": (_ci, [_ci, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _vp]),
     "hr_halo_buffers_alloc": (_ci, [_vp, _ci, ctypes.POINTER(_vp)]),
+    "hr_face_buffers_alloc": (_ci, [_vp, _ci, _ci, ctypes.POINTER(_vp)]),
     "hr_halo_buffers_free": (None, [_vp, _vp]),
     "hr_ipc_export": (_ci, [_vp, _vp, ctypes.c_char_p]),
     "hr_ipc_open": (_ci, [_vp, ctypes.c_char_p, ctypes.POINTER(_vp)]),
@@ -371,6 +372,12 @@ def hr_dphi_eo_face_apply(mu: int, out, recv_prev, recv_next, links: int, parity
 def hr_halo_buffers_alloc(ctx: int, prec: int) -> int:
     p = _vp()
     _check(_lib.hr_halo_buffers_alloc(ctx, prec, ctypes.byref(p)))
+    return p.value
+
+
+def hr_face_buffers_alloc(ctx: int, prec: int, mu: int) -> int:
+    p = _vp()
+    _check(_lib.hr_face_buffers_alloc(ctx, prec, mu, ctypes.byref(p)))
     return p.value
 
 

@@ -133,14 +133,16 @@ hr_status hr_dphi_eo_face_apply(int mu, void *out, const void *recv_prev, const 
 // One cudaMalloc allocation of 6 face messages: [send_up | send_dn | recv_prev[0] | recv_next[0] | recv_prev[1] |
 // recv_next[1]] (the receive buffers are double-buffered by call parity, see halo.py).  A plain cudaMalloc base pointer
 // is what cudaIpcGetMemHandle wants; torch's caching allocator hands out sub-blocks.
-hr_status hr_halo_buffers_alloc(const hr_ctx *ctx, hr_prec prec, void **base)
+hr_status hr_halo_buffers_alloc(const hr_ctx *ctx, hr_prec prec, void **base) { return hr_face_buffers_alloc(ctx, prec, 0, base); }
+
+hr_status hr_face_buffers_alloc(const hr_ctx *ctx, hr_prec prec, int mu, void **base)
 {
-    if (!ctx || !base || (prec != HR_F64 && prec != HR_F32)) { set_error("hr_halo_buffers_alloc: bad argument"); return HR_EINVAL; }
+    if (!ctx || !base || (prec != HR_F64 && prec != HR_F32) || mu < 0 || mu > 3) { set_error("hr_face_buffers_alloc: bad argument"); return HR_EINVAL; }
     *base = nullptr;
     hr_status rc = use_device(ctx);
     if (rc != HR_OK) return rc;
-    cudaError_t e = cudaMalloc(base, 6 * hr_halo_bytes(ctx, prec));
-    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail("hr_halo_buffers_alloc: cudaMalloc", e); }
+    cudaError_t e = cudaMalloc(base, 6 * hr_face_bytes(ctx, prec, mu));
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail("hr_face_buffers_alloc: cudaMalloc", e); }
     return HR_OK;
 }
 

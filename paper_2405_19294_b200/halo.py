@@ -277,3 +277,66 @@ class BlockDphi:
         self.interior(out, inp, links, parity)
         self.exchange()
         self.apply(out, links, parity)
+
+
+class PeerBlockDphi:
+    """BlockDphi with the messages of every split direction written straight into the neighbours' receive buffers (CUDA IPC
+    peer memory, as PeerSlabDphi): one allocation of six messages per direction, receive buffers double-buffered by call
+    parity, ONE fence per call after all pack kernels."""
+
+    def __init__(self, lat, prec: int, plan: dict, group=None):
+        import torch.distributed as dist
+        from . import hr_face_buffers_alloc, hr_face_bytes, hr_ipc_export, hr_ipc_open
+        self.lat, self.prec, self.plan, self.group = lat, prec, plan, group
+        self.world = dist.get_world_size(group) if dist.is_available() and dist.is_initialized() else 1
+        self.calls = 0
+        self.nb = {mu: hr_face_bytes(lat.ctx, prec, mu) for mu in plan["split"]}
+        self.base = {mu: hr_face_buffers_alloc(lat.ctx, prec, mu) for mu in plan["split"]}
+        self._opened = []
+        self.prev_base, self.next_base = dict(self.base), dict(self.base)
+        if self.world == 1:
+            return
+        rank = dist.get_rank(group)
+        handles = [None] * self.world
+        dist.all_gather_object(handles, {mu: hr_ipc_export(lat.ctx, b) for mu, b in self.base.items()}, group=group)
+        mapped = {}
+
+        def peer(r, mu):
+            if r == rank:
+                return self.base[mu]
+            if (r, mu) not in mapped:
+                mapped[(r, mu)] = hr_ipc_open(lat.ctx, handles[r][mu])
+                self._opened.append(mapped[(r, mu)])
+            return mapped[(r, mu)]
+
+        for mu in plan["split"]:
+            self.prev_base[mu] = peer(plan["prev"][mu], mu)
+            self.next_base[mu] = peer(plan["next"][mu], mu)
+
+    fence = PeerSlabDphi.fence
+
+    def dphi_eo(self, out, inp, links: int, parity: int) -> None:
+        from . import hr_dphi_eo_face_apply, hr_dphi_eo_face_pack, hr_dphi_eo_interior_mask
+        st = self.lat.stream()
+        k = self.calls & 1
+        self.calls += 1
+        for mu in self.plan["split"]:              # my "up" message is the next rank's recv_prev[k], "down" the previous rank's recv_next[k]
+            nb = self.nb[mu]
+            hr_dphi_eo_face_pack(mu, self.next_base[mu] + (2 + 2 * k) * nb, self.prev_base[mu] + (3 + 2 * k) * nb, inp, links, parity, st)
+        hr_dphi_eo_interior_mask(out, inp, links, parity, self.plan["mask"], st)
+        self.fence()
+        for mu in self.plan["split"]:
+            nb = self.nb[mu]
+            hr_dphi_eo_face_apply(mu, out, self.base[mu] + (2 + 2 * k) * nb, self.base[mu] + (3 + 2 * k) * nb, links, parity,
+                                  self.plan["first"][mu], self.plan["last"][mu], st)
+
+    def close(self):
+        from . import hr_halo_buffers_free, hr_ipc_close
+        import torch
+        torch.cuda.synchronize(self.lat.device)
+        for p in self._opened:
+            hr_ipc_close(self.lat.ctx, p)
+        self._opened = []
+        for b in self.base.values():
+            hr_halo_buffers_free(self.lat.ctx, b)
+        self.base = {}

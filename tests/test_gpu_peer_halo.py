@@ -171,3 +171,110 @@ def test_two_processes_store_into_each_others_buffers(case):
         assert got[0]["cg"][1] == got[1]["cg"][1]                    # both ranks saw the same all-reduced scalars
         x = np.concatenate([got[r]["cg"][2] for r in range(world)])
         assert rel_l2(x, x_want) <= 1e-8
+
+
+# ---- 4-D blocks over peer memory: two processes, split in x, in z or in t ----------------------------------------------
+def _block_worker(rank, world, port, q, case):
+    try:
+        sys.path.insert(0, ROOT)
+        sys.path.insert(0, os.path.join(ROOT, "tests"))
+        import torch.distributed as dist
+        import paper_2405_19294_b200 as hr
+        from paper_2405_19294_b200 import halo
+        from gpu_common import GpuProblem
+        from test_gpu_blocks import _block, _half_to_lex, _lex_to_half
+        os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+        dist.init_process_group("gloo", rank=rank, world_size=world)
+        grid, dims, N, rep, prec, bc = case
+        d = oracle.rep_dim(N, oracle_rep_id(rep))
+        V = li.volume(dims)
+        U = li.haar_links(381, N, dims)
+        plan = halo.block_plan(rank, grid, dims)
+        ld = plan["dims_local"]
+        prob = GpuProblem(hr, ld, N, rep, prec, _block(U, dims, plan), bc=bc)
+        blk = halo.PeerBlockDphi(prob.lat, prob.prec, plan)
+        res = {}
+        for rounds in range(2):
+            for parity in (0, 1):
+                psi = li.gaussian_spinor(382 + parity + 2 * rounds, V // 2, d)
+                loc = _lex_to_half(ld, _block(_half_to_lex(dims, psi, 1 - parity), dims, plan), 1 - parity)
+                gin, out = prob.lat.spinor(prob.prec), prob.lat.spinor(prob.prec)
+                prob.lat.import_spinor(gin, prob.prec, loc, 1 - parity)
+                out.fill_(0xFF)
+                blk.dphi_eo(out, gin, prob.links, parity)
+                res[(rounds, parity)] = prob.lat.export_spinor(out, prob.prec, parity)
+        # distributed CG on the blocks
+        m0 = -0.2
+        b = li.gaussian_spinor(391, V // 2, d)
+        gb, gx = prob.lat.spinor(prob.prec), prob.lat.spinor(prob.prec)
+        prob.lat.import_spinor(gb, prob.prec, _lex_to_half(ld, _block(_half_to_lex(dims, b, 0), dims, plan), 0), 0)
+        gx.fill_(0xFF)
+        it, hist = halo.SlabCG(blk, prob.links, m0).solve(gx, gb, 1e-10, 400)
+        res["cg"] = (it, hist, prob.lat.export_spinor(gx, prob.prec, 0))
+        res["plan"] = plan
+        dist.barrier()
+        blk.close()
+        prob.close()
+        q.put((rank, res))
+        dist.destroy_process_group()
+    except BaseException as e:
+        q.put((rank, {"error": repr(e)}))
+        raise
+
+
+@pytest.mark.parametrize("case", [((1, 2, 1, 1), (4, 8, 4, 4), 3, "fund", "f64", (-1, -1, 1, 1)),
+                                  ((1, 1, 1, 2), (4, 4, 4, 8), 3, "fund", "f64", (-1, 1, 1, -1)),
+                                  ((2, 1, 1, 1), (8, 4, 4, 4), 2, "adj", "f64", (-1, 1, 1, 1))])
+def test_two_processes_blocks_over_peer_memory(case):
+    import torch
+    import torch.multiprocessing as mp
+    from test_gpu_blocks import _half_to_lex, _lex_to_half
+    assert torch.cuda.is_available()
+    from paper_2405_19294_b200 import build
+    build.build()
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_block_worker, args=(r, world, port, q, case)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = {}
+    for _ in range(world):
+        r, res = q.get(timeout=240)
+        if "error" in res:
+            for p in procs:
+                p.join(timeout=5)
+                if p.is_alive():
+                    p.terminate()
+            pytest.fail(f"rank {r}: {res['error']}")
+        got[r] = res
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    grid, dims, N, rep, prec, bc = case
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    R = oracle.represent(N, oracle_rep_id(rep), li.haar_links(381, N, dims))
+    V = li.volume(dims)
+
+    def stitch(key, parity):
+        lex = np.zeros((V, 4, d), dtype=np.complex128)
+        gl = lex.reshape(tuple(dims) + (4, d))
+        for r in range(world):
+            pl = got[r]["plan"]
+            ld, o = pl["dims_local"], pl["origin"]
+            val = got[r][key] if key != "cg" else got[r]["cg"][2]
+            loc = _half_to_lex(ld, val.astype(np.complex128), parity)
+            gl[o[0]:o[0] + ld[0], o[1]:o[1] + ld[1], o[2]:o[2] + ld[2], o[3]:o[3] + ld[3]] = loc.reshape(tuple(ld) + (4, d))
+        return _lex_to_half(dims, lex, parity)
+
+    for rounds in range(2):
+        for parity in (0, 1):
+            psi = li.gaussian_spinor(382 + parity + 2 * rounds, V // 2, d)
+            assert rel_l2(stitch((rounds, parity), parity), oracle.dphi_eo(dims, bc, R, parity, psi)) <= TOL[prec], (rounds, parity)
+    from oracle import solver
+    b = li.gaussian_spinor(391, V // 2, d)
+    x_want, it_want, hist_want = solver.cg_dhat(dims, bc, R, -0.2, b, 1e-10, 400)
+    assert got[0]["cg"][0] == got[1]["cg"][0] and abs(got[0]["cg"][0] - it_want) <= 1
+    n = min(got[0]["cg"][0], it_want) + 1
+    assert np.allclose(got[0]["cg"][1][:n], hist_want[:n], rtol=1e-6, atol=0)
+    assert rel_l2(stitch("cg", 0), x_want) <= 1e-8
