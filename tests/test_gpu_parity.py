@@ -200,11 +200,15 @@ def test_dirac_matches_oracle(hr, N, rep, prec):
     prob.close()
 
 
-def test_repeated_launches_are_bitwise_identical(hr):
-    """No atomics anywhere in the path: the result is deterministic (reading C15)."""
+@pytest.mark.parametrize("N,rep,variant", [(3, "fund", -1), (3, "sym", 6), (4, "sym", -1), (4, "adj", -1)])
+def test_repeated_launches_are_bitwise_identical(hr, N, rep, variant):
+    """No atomics anywhere in the path: the result is deterministic (reading C15) -- the one-thread-per-site kernel and
+    the colour-parallel kernel (its shared-memory exchange is ordered by barriers, not by arrival)."""
     dims = (8, 8, 8, 8)
-    U, psi = make_inputs(dims, 3, 71, 72, 3)
-    prob = GpuProblem(hr, dims, 3, "fund", "f64", U)
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U, psi = make_inputs(dims, N, 71, 72, d)
+    prob = GpuProblem(hr, dims, N, rep, "f64", U)
+    prob.lat.set_tuning("variant", variant)
     a = prob.dphi_eo(psi, 0)
     for _ in range(3):
         assert np.array_equal(prob.dphi_eo(psi, 0), a)
