@@ -6,6 +6,7 @@
 
 #include "dphi_pf_kernel.cuh"
 #include "dphi_cp_kernel.cuh"
+#include "dphi_cpo_kernel.cuh"
 #include "halo_kernel.cuh"
 
 namespace hr {
@@ -102,6 +103,9 @@ static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaS
     if constexpr (CP_OK) {
         if (variant == 6) return launch_cp<Real, D, LK, MASS, RED>(a, st);
     }
+    if constexpr (LK == LK_SYM_OTF || LK == LK_ASYM_OTF) {
+        if (variant == 6) return launch_cpo<Real, D, LK, MASS, RED>(a, st);
+    }
     if constexpr (D > 8) {
         if (variant == 0) return launch_one<Real, D, LK, 1, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
     } else
@@ -151,7 +155,7 @@ template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant)
 {
     constexpr int RPV = 16 / (int)sizeof(Real);
     if (variant < 0 || variant >= DPHI_NVARIANTS) return false;
-    if (variant == 6) return LK == LK_COMPLEX || LK == LK_REAL;
+    if (variant == 6) return LK == LK_COMPLEX || LK == LK_REAL || LK == LK_SYM_OTF || LK == LK_ASYM_OTF;
     if (D > 8) return variant == 0;
     if ((variant == 2 || variant == 3) && (2 * D) % RPV != 0) return false;
     if (variant == 5 && PfGeom<Real, D, LK>::smem_bytes(64) > kMaxDynSmem) return false;
