@@ -495,30 +495,21 @@ hr_status hr_qmr_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const 
         HR_CUDA(cudaStreamSynchronize(st));
         const double alpha = h[5] / delta;
         const double beta = k > 0 ? rho * delta / delta_prev : 0.0;
-        // vt = Dhat v - alpha v - beta v_prev = gamma5 w - alpha v - beta v_prev   (into w)
-        const double ma[2] = { -alpha, 0.0 }, mb[2] = { -beta, 0.0 };
-        rc = launch_lincomb(ctx, P, w, one, 1, w, ma, v, st);
+        // vt = Dhat v - alpha v - beta v_prev = gamma5 w - alpha v - beta v_prev (into w) and its two half norms: one kernel
+        rc = launch_qmr_lanczos(ctx, P, w, v, vp, alpha, beta, rs, rs.result, st);
         if (rc != HR_OK) return rc;
-        if (k > 0) {
-            rc = launch_lincomb(ctx, P, w, one, 0, w, mb, vp, st);
-            if (rc != HR_OK) return rc;
-        }
-        rc = halves(w, &up, &lo);
-        if (rc != HR_OK) return rc;
+        HR_CUDA(cudaMemcpyAsync(h, rs.result, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        HR_CUDA(cudaStreamSynchronize(st));
+        up = h[0]; lo = h[1];
         const double rho_next = sqrt(up + lo);
         const double theta = s2 * beta, t = c2 * beta;
         const double eps = c1 * t + s1 * alpha, zt = -s1 * t + c1 * alpha;
         const double zeta = sqrt(zt * zt + rho_next * rho_next);
         if (zeta == 0.0) break;
         const double c = zt / zeta, s = rho_next / zeta;
-        // p = (v - eps p1 - theta p2) / zeta, into p2's buffer (p_{k-2} is not needed again)
-        const double iz[2] = { 1.0 / zeta, 0.0 }, mt[2] = { -theta / zeta, 0.0 }, me[2] = { -eps / zeta, 0.0 };
-        rc = launch_lincomb(ctx, P, p2, iz, 0, v, mt, p2, st);
-        if (rc != HR_OK) return rc;
-        rc = launch_lincomb(ctx, P, p2, one, 0, p2, me, p1, st);
-        if (rc != HR_OK) return rc;
-        const double ce[2] = { c * eta, 0.0 };
-        rc = launch_lincomb(ctx, P, x_e, one, 0, x_e, ce, p2, st);                        // x += c eta p
+        // p = (v - eps p1 - theta p2) / zeta into p2's buffer (p_{k-2} is not needed again); x += c eta p;
+        // v_{k+1} = vt / rho_{k+1} into the old v_prev buffer: one kernel
+        rc = launch_qmr_update(ctx, P, p2, p1, v, x_e, vp, w, 1.0 / zeta, eps, theta, c * eta, rho_next > 0.0 ? 1.0 / rho_next : 0.0, st);
         if (rc != HR_OK) return rc;
         eta = -s * eta;
         ++k;
@@ -526,11 +517,7 @@ hr_status hr_qmr_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const 
         { void *q = p1; p1 = p2; p2 = q; }
         c2 = c1; s2 = s1; c1 = c; s1 = s;
         if (rho_next == 0.0) { rc = true_res2(bb, &res2); if (rc != HR_OK) return rc; have_res = true; break; }
-        // v_{k+1} = vt / rho_{k+1} into the old v_prev buffer (before the residual check below, which re-uses w);
         // delta_{k+1} = (|vt_up|^2 - |vt_lo|^2) / rho_{k+1}^2
-        const double ir[2] = { 1.0 / rho_next, 0.0 };
-        rc = launch_lincomb(ctx, P, vp, ir, 0, w, zero, nullptr, st);
-        if (rc != HR_OK) return rc;
         { void *q = v; v = vp; vp = q; }
         delta_prev = delta;
         delta = (up - lo) / (up + lo);

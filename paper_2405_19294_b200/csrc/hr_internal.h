@@ -171,6 +171,10 @@ hr_status launch_cvt(const hr_ctx *c, bool down, void *dst, const void *src, dou
 //   result[0..1] = <x, y> (result[0] = |x|^2 when x == y), device pointer
 hr_status launch_dot(const hr_ctx *c, hr_prec prec, const void *x, const void *y, const RedScratch &rs,
                      double *result_dev, cudaStream_t st);
+hr_status launch_qmr_lanczos(const hr_ctx *c, hr_prec prec, void *w, const void *v, const void *vp, double alpha, double beta,
+                             const RedScratch &rs, double *result_dev, cudaStream_t st);
+hr_status launch_qmr_update(const hr_ctx *c, hr_prec prec, void *p2, const void *p1, const void *v, void *x, void *vp, const void *w,
+                            double izeta, double eps, double theta, double ceta, double irho, cudaStream_t st);
 hr_status launch_dot_range(const hr_ctx *c, hr_prec prec, const void *x, const void *y, size_t first, size_t nvec,
                            const RedScratch &rs, double *result_dev, cudaStream_t st);
 // CG building blocks on the device-resident CgState (cg.cu)

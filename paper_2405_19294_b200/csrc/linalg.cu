@@ -191,6 +191,83 @@ hr_status launch_dot(const hr_ctx *c, hr_prec prec, const void *x, const void *y
     return prec == HR_F64 ? dot_t<double>(x, y, nvec, rs, result_dev, st) : dot_t<float>(x, y, nvec, rs, result_dev, st);
 }
 
+// ---- fused vector updates of the gamma5-QMR (hr_qmr_dhat; real coefficients) -----------------------------------------
+__device__ __forceinline__ double2 vscale(double a, double2 b) { return make_double2(a * b.x, a * b.y); }
+__device__ __forceinline__ float4 vscale(float a, float4 b) { return make_float4(a * b.x, a * b.y, a * b.z, a * b.w); }
+__device__ __forceinline__ double vnorm2(double2 a) { return a.x * a.x + a.y * a.y; }
+__device__ __forceinline__ double vnorm2(float4 a) { return (double)(a.x * a.x + a.y * a.y) + (double)(a.z * a.z + a.w * a.w); }
+
+// Lanczos step: w <- gamma5 w - alpha v - beta vp;  result = (|w_upper|^2, |w_lower|^2) of the new w   (3 reads, 1 write)
+template <typename Real>
+__global__ void __launch_bounds__(LIN_THREADS) qmr_lanczos_kernel(typename Vec16<Real>::type *w, const typename Vec16<Real>::type *v,
+                                                                  const typename Vec16<Real>::type *vp, Real alpha, Real beta,
+                                                                  size_t nvec, size_t half, double *partial, unsigned *ticket,
+                                                                  double *result)
+{
+    double r[2] = { 0.0, 0.0 };
+    const size_t stride = (size_t)gridDim.x * LIN_THREADS;
+    for (size_t i = (size_t)blockIdx.x * LIN_THREADS + threadIdx.x; i < nvec; i += stride) {
+        const bool lower = i >= half;
+        auto t = vadd(vscale(lower ? (Real)-1 : (Real)1, w[i]), vscale(-alpha, v[i]));
+        if (beta != (Real)0) t = vadd(t, vscale(-beta, vp[i]));
+        w[i] = t;
+        r[lower ? 1 : 0] += vnorm2(t);
+    }
+    if (grid_reduce<2>(r, partial, ticket)) { result[0] = r[0]; result[1] = r[1]; }
+}
+
+// direction, solution and next Lanczos vector:  p2 <- (v - eps p1 - theta p2) / zeta;  x += ceta p2;  vp <- w / rho
+// (5 reads, 3 writes)
+template <typename Real>
+__global__ void __launch_bounds__(LIN_THREADS) qmr_update_kernel(typename Vec16<Real>::type *p2, const typename Vec16<Real>::type *p1,
+                                                                 const typename Vec16<Real>::type *v, typename Vec16<Real>::type *x,
+                                                                 typename Vec16<Real>::type *vp, const typename Vec16<Real>::type *w,
+                                                                 Real izeta, Real eps, Real theta, Real ceta, Real irho, size_t nvec)
+{
+    const size_t i = (size_t)blockIdx.x * LIN_THREADS + threadIdx.x;
+    if (i >= nvec) return;
+    const auto p = vscale(izeta, vadd(v[i], vadd(vscale(-eps, p1[i]), vscale(-theta, p2[i]))));
+    p2[i] = p;
+    x[i] = vadd(x[i], vscale(ceta, p));
+    vp[i] = vscale(irho, w[i]);
+}
+
+template <typename Real>
+static hr_status qmr_lanczos_t(void *w, const void *v, const void *vp, double alpha, double beta, size_t nvec, const RedScratch &rs,
+                               double *result, cudaStream_t st)
+{
+    using V = typename Vec16<Real>::type;
+    qmr_lanczos_kernel<Real><<<reduce_grid(nvec), LIN_THREADS, 0, st>>>((V *)w, (const V *)v, (const V *)vp, (Real)alpha, (Real)beta, nvec,
+                                                                        nvec / 2, rs.partial, rs.ticket, result);
+    return check_launch("qmr_lanczos_kernel");
+}
+template <typename Real>
+static hr_status qmr_update_t(void *p2, const void *p1, const void *v, void *x, void *vp, const void *w, double izeta, double eps,
+                              double theta, double ceta, double irho, size_t nvec, cudaStream_t st)
+{
+    using V = typename Vec16<Real>::type;
+    const unsigned grid = (unsigned)((nvec + LIN_THREADS - 1) / LIN_THREADS);
+    qmr_update_kernel<Real><<<grid, LIN_THREADS, 0, st>>>((V *)p2, (const V *)p1, (const V *)v, (V *)x, (V *)vp, (const V *)w, (Real)izeta,
+                                                          (Real)eps, (Real)theta, (Real)ceta, (Real)irho, nvec);
+    return check_launch("qmr_update_kernel");
+}
+
+hr_status launch_qmr_lanczos(const hr_ctx *c, hr_prec prec, void *w, const void *v, const void *vp, double alpha, double beta,
+                             const RedScratch &rs, double *result_dev, cudaStream_t st)
+{
+    const size_t nvec = field_nvec(c, prec);
+    return prec == HR_F64 ? qmr_lanczos_t<double>(w, v, vp, alpha, beta, nvec, rs, result_dev, st)
+                          : qmr_lanczos_t<float>(w, v, vp, alpha, beta, nvec, rs, result_dev, st);
+}
+
+hr_status launch_qmr_update(const hr_ctx *c, hr_prec prec, void *p2, const void *p1, const void *v, void *x, void *vp, const void *w,
+                            double izeta, double eps, double theta, double ceta, double irho, cudaStream_t st)
+{
+    const size_t nvec = field_nvec(c, prec);
+    return prec == HR_F64 ? qmr_update_t<double>(p2, p1, v, x, vp, w, izeta, eps, theta, ceta, irho, nvec, st)
+                          : qmr_update_t<float>(p2, p1, v, x, vp, w, izeta, eps, theta, ceta, irho, nvec, st);
+}
+
 // <x, y> over the vectors [first, first + nvec) of the two fields (the upper / lower spin halves of a field are the first
 // and second half of its vectors: gamma5 is a sign pattern on them)
 hr_status launch_dot_range(const hr_ctx *c, hr_prec prec, const void *x, const void *y, size_t first, size_t nvec,
