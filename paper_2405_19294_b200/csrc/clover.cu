@@ -24,6 +24,32 @@ template <typename Real, int D, bool RL> struct CloverGeom {
     static constexpr int NREAL = 2 * BLK;
 };
 
+// one element of a link record in the plane layout of hr_internal.h (tail planes included), default caching
+template <int NREAL> __device__ __forceinline__ void load_real_any(double &r, const char *base, size_t vh, size_t s, int e)
+{
+    constexpr int NV = NREAL / 2;
+    if (NREAL % 2 == 0 || (e >> 1) < NV) r = *(const double *)(base + ((size_t)(e >> 1) * vh + s) * 16 + (size_t)(e & 1) * 8);
+    else r = *(const double *)(base + (size_t)NV * 16 * vh + s * 8);
+}
+template <int NREAL> __device__ __forceinline__ void load_real_any(float &r, const char *base, size_t vh, size_t s, int e)
+{
+    constexpr int NV = NREAL / 4, TAIL = NREAL - 4 * NV;
+    if (TAIL == 0 || (e >> 2) < NV) r = *(const float *)(base + ((size_t)(e >> 2) * vh + s) * 16 + (size_t)(e & 3) * 4);
+    else r = *(const float *)(base + (size_t)NV * 16 * vh + s * (size_t)(TAIL * 4) + (size_t)(e - 4 * NV) * 4);
+}
+template <int NREAL> __device__ __forceinline__ void load_cplx_any(double &re, double &im, const char *base, size_t vh, size_t s, int e)
+{
+    const double2 v = *(const double2 *)(base + ((size_t)e * vh + s) * 16);
+    re = v.x; im = v.y;
+}
+template <int NREAL> __device__ __forceinline__ void load_cplx_any(float &re, float &im, const char *base, size_t vh, size_t s, int e)
+{
+    constexpr int NV = NREAL / 4;
+    const float2 v = (NREAL % 4 == 0 || (e >> 1) < NV) ? *(const float2 *)(base + ((size_t)(e >> 1) * vh + s) * 16 + (size_t)(e & 1) * 8)
+                                                        : *(const float2 *)(base + (size_t)NV * 16 * vh + s * 8);
+    re = v.x; im = v.y;
+}
+
 // complex D x D matrices as Real[2*D*D], row-major (re, im)
 template <typename Real, int D, bool DA, bool DB>
 __device__ __forceinline__ void cmm(Real *o, const Real *a, const Real *b) // o = op(a) op(b), op = dagger if flagged
@@ -168,6 +194,146 @@ __global__ void __launch_bounds__(64) clover_build_kernel(const CloverArgs a)
     }
     const int qpar = (c[0] + c[1] + c[2] + c[3]) & 1;
     const size_t hs = (size_t)(i >> 1);
+    char *base = (char *)a.clover + (size_t)qpar * G::NREAL * sizeof(Real) * (size_t)a.vh;
+    store_record<G::NREAL>(base, (size_t)a.vh, hs, rec);
+}
+
+// ---- row-parallel build for d_R > 4 ------------------------------------------------------------------------------------
+// clover_build_kernel keeps d_R x d_R matrices in thread-local arrays and is bound by local-memory traffic from d_R = 6 on
+// (80 ms for the sextet at 24^3 x 48).  Here one thread owns ONE ROW of the plaquette products: row_i(M1 M2 M3 M4) =
+// ((e_i^T M1) M2) M3) M4 is three vector-matrix products with the vector (d_R complex) in registers and the matrices
+// streamed from the link field through L1 -- the d_R threads of a site (d_R warps of a CTA, lanes = consecutive sites:
+// coalesced element loads) read the same links.  clover_q_kernel writes the rows of Q_{mu nu} (sum of the four leaves)
+// of a chunk of sites to a scratch buffer; clover_pack_kernel forms F = (Q - Q^dagger)/(8i) and packs T as above.
+struct LeafFactor { signed char dm, dn, nu_dir, dag; };          // site offset (in mu, nu), link direction (0 mu / 1 nu), dagger
+__constant__ LeafFactor kLeaf[4][4] = {
+    { { 0, 0, 0, 0 }, { 1, 0, 1, 0 }, { 0, 1, 0, 1 }, { 0, 0, 1, 1 } },       // U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
+    { { 0, 0, 1, 0 }, { -1, 1, 0, 1 }, { -1, 0, 1, 1 }, { -1, 0, 0, 0 } },    // U_nu(x) U_mu(x-mu+nu)^dag U_nu(x-mu)^dag U_mu(x-mu)
+    { { -1, 0, 0, 1 }, { -1, -1, 1, 1 }, { -1, -1, 0, 0 }, { 0, -1, 1, 0 } }, // U_mu(x-mu)^dag U_nu(x-mu-nu)^dag U_mu(x-mu-nu) U_nu(x-nu)
+    { { 0, -1, 1, 1 }, { 0, -1, 0, 0 }, { 1, -1, 1, 0 }, { 0, 0, 0, 1 } } };  // U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag
+
+template <typename Real, int D, bool RL>
+__global__ void __launch_bounds__(32 * D) clover_q_kernel(const CloverArgs a, Real *scratch, long first, long n)
+{
+    constexpr int LNREAL = CloverGeom<Real, D, RL>::LNREAL;
+    const int lane = (int)threadIdx.x & 31, row = (int)threadIdx.x >> 5;
+    const long loc = (long)blockIdx.x * 32 + lane;
+    if (loc >= n) return;
+    const long idx = first + loc;                                  // even-odd site index: [parity][half index]
+    const int par = idx >= a.vh ? 1 : 0;
+    int c[4];
+    {
+        long r = idx - (long)par * a.vh;
+        const int Zh = a.Z / 2;
+        const int zh = (int)(r % Zh); r /= Zh;
+        c[2] = (int)(r % a.Y); r /= a.Y;
+        c[1] = (int)(r % a.X);
+        c[0] = (int)(r / a.X);
+        c[3] = 2 * zh + ((c[0] + c[1] + c[2] + par) & 1);
+    }
+    const int ext[4] = { a.T, a.X, a.Y, a.Z };
+    const size_t vh = (size_t)a.vh;
+    int plane = 0;
+    for (int mu = 0; mu < 4; ++mu)
+        for (int nu = mu + 1; nu < 4; ++nu, ++plane) {
+            Real q[2 * D];
+#pragma unroll
+            for (int j = 0; j < 2 * D; ++j) q[j] = 0;
+            for (int leaf = 0; leaf < 4; ++leaf) {
+                Real r[2 * D];
+                for (int f = 0; f < 4; ++f) {
+                    const LeafFactor lf = kLeaf[leaf][f];
+                    int y[4] = { c[0], c[1], c[2], c[3] };
+                    y[mu] = (y[mu] + lf.dm + ext[mu]) % ext[mu];
+                    y[nu] = (y[nu] + lf.dn + ext[nu]) % ext[nu];
+                    const int qy = (y[0] + y[1] + y[2] + y[3]) & 1;
+                    const size_t sy = (((size_t)y[0] * a.X + y[1]) * a.Y + y[2]) * (a.Z / 2) + y[3] / 2;
+                    const char *base = (const char *)a.links + (size_t)(qy * 4 + (lf.nu_dir ? nu : mu)) * LNREAL * sizeof(Real) * vh;
+                    const bool dag = lf.dag != 0;
+                    auto elem = [&](int k, int j, Real &re, Real &im) {       // op(M)[k][j]
+                        const int e = dag ? j * D + k : k * D + j;
+                        if constexpr (RL) { load_real_any<LNREAL>(re, base, vh, sy, e); im = 0; }
+                        else { load_cplx_any<LNREAL>(re, im, base, vh, sy, e); if (dag) im = -im; }
+                    };
+                    if (f == 0) {
+#pragma unroll
+                        for (int j = 0; j < D; ++j) elem(row, j, r[2 * j], r[2 * j + 1]);
+                    } else {
+                        Real rn[2 * D];
+#pragma unroll
+                        for (int j = 0; j < 2 * D; ++j) rn[j] = 0;
+#pragma unroll
+                        for (int k = 0; k < D; ++k)
+#pragma unroll
+                            for (int j = 0; j < D; ++j) {
+                                Real mr, mi;
+                                elem(k, j, mr, mi);
+                                rn[2 * j] = fma(r[2 * k], mr, fma(-r[2 * k + 1], mi, rn[2 * j]));
+                                rn[2 * j + 1] = fma(r[2 * k], mi, fma(r[2 * k + 1], mr, rn[2 * j + 1]));
+                            }
+#pragma unroll
+                        for (int j = 0; j < 2 * D; ++j) r[j] = rn[j];
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < 2 * D; ++j) q[j] += r[j];
+            }
+            // scratch: [plane][real index 2 (row D + j) + re/im][site of the chunk]
+#pragma unroll
+            for (int j = 0; j < 2 * D; ++j) scratch[((size_t)plane * 2 * D * D + (size_t)row * 2 * D + j) * (size_t)n + (size_t)loc] = q[j];
+        }
+}
+
+template <typename Real, int D, bool RL>
+__global__ void __launch_bounds__(64) clover_pack_kernel(const CloverArgs a, const Real *scratch, long first, long n)
+{
+    using G = CloverGeom<Real, D, RL>;
+    constexpr int M = 2 * D * D;
+    const long loc = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (loc >= n) return;
+    const long idx = first + loc;
+    const int qpar = idx >= a.vh ? 1 : 0;
+    const size_t hs = (size_t)(idx - (long)qpar * a.vh);
+    Real cf[2][3][M];
+    for (int b = 0; b < 2; ++b)
+        for (int k = 0; k < 3; ++k)
+            for (int e = 0; e < M; ++e) cf[b][k][e] = 0;
+    const int pk[6] = { 0, 1, 2, 2, 1, 0 };
+    const int su[6] = { 1, 1, 1, -1, 1, -1 };
+    const int sd[6] = { -1, -1, -1, -1, 1, -1 };
+    for (int plane = 0; plane < 6; ++plane) {
+        Real q[M];
+        for (int e = 0; e < M; ++e) q[e] = scratch[((size_t)plane * M + e) * (size_t)n + (size_t)loc];
+        for (int r = 0; r < D; ++r)
+            for (int s = 0; s < D; ++s) {
+                const Real gre = q[2 * (r * D + s)] - q[2 * (s * D + r)];
+                const Real gim = q[2 * (r * D + s) + 1] + q[2 * (s * D + r) + 1];
+                const Real fre = gim * (Real)0.125, fim = -gre * (Real)0.125;
+                cf[0][pk[plane]][2 * (r * D + s)] += su[plane] * fre;
+                cf[0][pk[plane]][2 * (r * D + s) + 1] += su[plane] * fim;
+                cf[1][pk[plane]][2 * (r * D + s)] += sd[plane] * fre;
+                cf[1][pk[plane]][2 * (r * D + s) + 1] += sd[plane] * fim;
+            }
+    }
+    const Real k = (Real)(-0.5 * a.csw);
+    Real rec[G::NREAL];
+    for (int b = 0; b < 2; ++b) {
+        const Real *A = cf[b][0], *B = cf[b][1], *C = cf[b][2];
+        auto elem = [&](int row, int col, Real &re, Real &im) {
+            const int sr = row / D, ar = row % D, sc = col / D, ac = col % D;
+            const int e = 2 * (ar * D + ac);
+            if (sr == 0 && sc == 0) { re = C[e]; im = C[e + 1]; }
+            else if (sr == 1 && sc == 1) { re = -C[e]; im = -C[e + 1]; }
+            else if (sr == 0 && sc == 1) { re = A[e] + B[e + 1]; im = A[e + 1] - B[e]; }
+            else { re = A[e] - B[e + 1]; im = A[e + 1] + B[e]; }
+            re *= k; im *= k;
+        };
+        Real *o = rec + b * G::BLK;
+        int w = 0;
+        for (int d = 0; d < 2 * D; ++d) { Real re, im; elem(d, d, re, im); o[w++] = re; }
+        for (int r = 0; r < 2 * D; ++r)
+            for (int s = r + 1; s < 2 * D; ++s) { Real re, im; elem(r, s, re, im); o[w++] = re; o[w++] = im; }
+    }
     char *base = (char *)a.clover + (size_t)qpar * G::NREAL * sizeof(Real) * (size_t)a.vh;
     store_record<G::NREAL>(base, (size_t)a.vh, hs, rec);
 }
@@ -373,6 +539,28 @@ static hr_status launched(const char *what)
 
 size_t clover_nreal(const hr_ctx *c) { return (size_t)8 * c->d * c->d; }
 
+// d_R > 4: rows of Q for a chunk of sites into a stream-ordered scratch allocation, then the packing kernel
+template <typename Real, int D, bool RL>
+static hr_status build_rows(const hr_ctx *c, const CloverArgs &a, cudaStream_t st)
+{
+    const long total = c->V;
+    const long chunk = total < (1L << 19) ? total : (1L << 19);
+    Real *scratch = nullptr;
+    cudaError_t e = cudaMallocAsync((void **)&scratch, (size_t)chunk * 6 * 2 * D * D * sizeof(Real), st);
+    if (e != cudaSuccess) { cudaGetLastError(); set_error("clover build: scratch allocation failed: %s", cudaGetErrorString(e)); return HR_ENOMEM; }
+    hr_status rc = HR_OK;
+    for (long first = 0; first < total && rc == HR_OK; first += chunk) {
+        const long n = total - first < chunk ? total - first : chunk;
+        clover_q_kernel<Real, D, RL><<<(unsigned)((n + 31) / 32), 32 * D, 0, st>>>(a, scratch, first, n);
+        rc = launched("clover_q_kernel");
+        if (rc != HR_OK) break;
+        clover_pack_kernel<Real, D, RL><<<(unsigned)((n + 63) / 64), 64, 0, st>>>(a, scratch, first, n);
+        rc = launched("clover_pack_kernel");
+    }
+    cudaFreeAsync(scratch, st);
+    return rc;
+}
+
 hr_status launch_clover_build(const hr_ctx *c, hr_prec prec, void *clover, const void *links, double csw, cudaStream_t st)
 {
     CloverArgs a;
@@ -383,6 +571,7 @@ hr_status launch_clover_build(const hr_ctx *c, hr_prec prec, void *clover, const
     const bool rl = c->real_links != 0;
 #define X(D, RL)                                                                                                      \
     if (c->d == D && rl == RL) {                                                                                      \
+        if (D > 4) return prec == HR_F64 ? build_rows<double, D, RL>(c, a, st) : build_rows<float, D, RL>(c, a, st);   \
         if (prec == HR_F64) clover_build_kernel<double, D, RL><<<grid, 64, 0, st>>>(a);                              \
         else clover_build_kernel<float, D, RL><<<grid, 64, 0, st>>>(a);                                              \
         return launched("clover_build_kernel");                                                                       \
