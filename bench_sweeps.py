@@ -1,15 +1,11 @@
 #!/usr/bin/env python
-"""Measurement of the NEXT-1 rows: the paper's second benchmark, the spinor linear
-algebra of PAPER.md:108-120 / Fig. 7 ("Copy spinor field", "g5 application", "g5 mulc add assign", norms and
-inner products; SU(3) fundamental), plus hr_dhat and one CG iteration.
+"""bench_sweeps.py -- companion measurements of bench.py (which stays the headline): the sweeps behind the tables of
+DESIGN.md and profiles/.  They import bench.py's configs, byte model and input recipe; nothing here is product code.
 
-    python -m paper_2405_19294_b200.bench_solver [--config 2|3|4|5] [--prec f64|f32] [--reps 50]
-
-Prints one JSON line per operation: algorithmic bytes (S = spinor bytes per site, Vh sites: copy/g5 2S,
-g5_mulc_add_assign 3S, norm2 1S, dot 2S; Dhat 2(8L+2S)+S; CG iteration 4(8L+2S) + 2S + 8S), the time per call
-from CUDA events on the launching stream (back to back, fields larger than L2 rotate through 4 buffer sets),
-GB/s and the fraction of the measured copy peak (MEASURED_PEAKS.json).  Inputs: the seeded synthetic fields
-of bench.py's configs.  bench.py stays the headline; this script is the Fig. 7 companion."""
+    python bench_sweeps.py volume  [--reps 200] [--sizes 8,12,...]      Dphi_eo and a copy against the lattice volume
+    python bench_sweeps.py large_n [--reps 50] [--variants ...]         Dphi_eo against d_R at constant memory moved (Fig. 6)
+    python bench_sweeps.py solver  [--config 2] [--prec f64] [--reps 50] spinor linear algebra, Dhat, solvers (Fig. 7)
+"""
 from __future__ import annotations
 
 import argparse
@@ -17,23 +13,178 @@ import json
 import os
 import sys
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
+def volume(argv):
+    """Volume dependence of Dphi_eo and of a streaming copy ("add 16^4, 32^4, 48^4 points
+    for the curve, cf. Fig. 7's volume dependence, PAPER.md:116"; at small local lattices "the execution time
+    is dominated by the kernel call overheads").
+    
+        python bench_sweeps.py volume [--reps 200]
+    
+    SU(3) fundamental, near-identity links (config 5's recipe), L^4 lattices, fp64 and fp32.  One JSON line per point:
+    time per hr_dphi_eo launch (CUDA events, back to back, alternating parity, 4 rotating buffer sets), contract and
+    compulsory GB/s, and hr_spinor_copy on the same half field."""
+    import torch
+    import bench as B
+    import lattice_inputs as li
+    import paper_2405_19294_b200 as hr
 
-def main():
+    ap = argparse.ArgumentParser(prog="bench_sweeps.py volume")
+    ap.add_argument("--reps", type=int, default=200)
+    ap.add_argument("--sizes", default="8,12,16,24,32,48,64")
+    args = ap.parse_args(argv)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench_sweeps volume: no CUDA device; the product path has no CPU fallback")
+    peak, _ = B.measured_peak()
+    for L in [int(x) for x in args.sizes.split(",")]:
+        dims = (L, L, L, L)
+        U = li.near_identity_links(1005, 3, dims, 0.3)
+        vh = li.volume(dims) // 2
+        psi = li.gaussian_spinor(2005, vh, 3)
+        for prec in ("f64", "f32"):
+            P = hr.PREC_NAMES[prec]
+            w = 8 if prec == "f64" else 4
+            S, Lb = 24 * w, 18 * w
+            lat = hr.Lattice(dims, B.BC, 3, "fund")
+            links = lat.gauge(True, P)
+            lat.import_gauge(links, U)
+            a = [lat.spinor(P) for _ in range(4)]
+            o = [lat.spinor(P) for _ in range(4)]
+            for k in range(4):
+                lat.import_spinor(a[k], P, psi, 0)
+            st = lat.stream()
+
+            def timed(fn):
+                for k in range(10):
+                    fn(k)
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for k in range(args.reps):
+                    fn(k)
+                e1.record()
+                torch.cuda.synchronize()
+                return e0.elapsed_time(e1) / args.reps
+
+            ms = timed(lambda k: hr.hr_dphi_eo(o[k % 4], a[k % 4], links, k & 1, st))
+            msc = timed(lambda k: hr.hr_spinor_copy(lat.ctx, P, o[k % 4], a[k % 4], st))
+            print(json.dumps({"workload": f"SU(3) fund {L}^4", "dtype": prec, "sites": vh, "dphi_us": ms * 1e3,
+                              "contract_gbs": vh * (8 * Lb + 9 * S) / (ms * 1e-3) / 1e9,
+                              "compulsory_gbs": vh * (8 * Lb + 2 * S) / (ms * 1e-3) / 1e9,
+                              "compulsory_frac_of_copy_peak": vh * (8 * Lb + 2 * S) / (ms * 1e-3) / 1e9 / peak,
+                              "copy_us": msc * 1e3, "copy_gbs": vh * 2 * S / (msc * 1e-3) / 1e9,
+                              "field_mb": (8 * Lb + 2 * S) * vh / 1e6}))
+            lat.close()
+
+
+
+# (N, rep, dims): compulsory bytes 1.6-1.9 GB in fp64 for every row
+CASES = [(2, "fund", (128, 32, 32, 32)), (3, "fund", (64, 32, 32, 32)), (4, "fund", (40, 32, 32, 32)),
+         (3, "sym", (48, 24, 24, 24)), (3, "adj", (48, 24, 24, 24)), (4, "sym", (56, 16, 16, 16)), (4, "adj", (48, 16, 16, 16))]
+NAMES = ["site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour"]
+
+
+def large_n(argv):
+    """Dphi_eo against the dimension d_R of the fermion representation, memory moved held about constant by shrinking the
+    lattice -- the experiment of the paper's Fig. 6 ("unimproved kernel blows up; improved is stable"),
+    here for every kernel flavour the library compiles for that d_R:
+    
+        site / site_ef   one thread per site (the paper's default kernel)
+        pair / pair_ef   two threads per site (d_R <= 8)
+        colour           one thread per (site, colour row): the large-d_R kernel (csrc/dphi_cp_kernel.cuh)
+    
+        python bench_sweeps.py large_n [--reps 50]
+    
+    Haar links, gaussian spinors, represented link field.  One JSON line per (representation, precision, variant): time per
+    hr_dphi_eo launch (CUDA events, back to back, alternating parity, rotating buffer sets), compulsory GB/s (every byte
+    once) and GFLOP/s with bench.py's per-site model."""
+    import torch
+    import bench as B
+    import lattice_inputs as li
+    import paper_2405_19294_b200 as hr
+
+    ap = argparse.ArgumentParser(prog="bench_sweeps.py large_n")
+    ap.add_argument("--reps", type=int, default=50)
+    ap.add_argument("--variants", default="0,1,2,3,6")
+    ap.add_argument("--cases", default="", help="comma list of d_R values to run (default: all)")
+    args = ap.parse_args(argv)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench_sweeps large_n: no CUDA device; the product path has no CPU fallback")
+    peak, _ = B.measured_peak()
+    only = [int(x) for x in args.cases.split(",") if x]
+    for N, rep, dims in CASES:
+        if only and B.REP_DIM[rep](N) not in only:
+            continue
+        U = li.haar_links(1006, N, dims)
+        vh = li.volume(dims) // 2
+        for prec in ("f64", "f32"):
+            P = hr.PREC_NAMES[prec]
+            bm = B.byte_model({"N": N, "rep": rep, "dims": dims}, prec)
+            lat = hr.Lattice(dims, B.BC, N, rep)
+            fund = lat.gauge(False, P)
+            lat.import_gauge(fund, U)
+            links = lat.gauge(True, P)
+            lat.represent_links(links, fund)
+            psi = li.gaussian_spinor(2006, vh, bm["d"])
+            a = [lat.spinor(P) for _ in range(2)]
+            o = [lat.spinor(P) for _ in range(2)]
+            for k in range(2):
+                lat.import_spinor(a[k], P, psi, 0)
+            st = lat.stream()
+            default = hr.hr_dphi_variant_name(lat.ctx, P)
+            for v in [int(x) for x in args.variants.split(",")]:
+                try:
+                    lat.set_tuning("variant", v)
+                    hr.hr_dphi_eo(o[0], a[0], links, 0, st)
+                except hr.HrError:
+                    continue
+                for k in range(5):
+                    hr.hr_dphi_eo(o[k % 2], a[k % 2], links, k & 1, st)
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for k in range(args.reps):
+                    hr.hr_dphi_eo(o[k % 2], a[k % 2], links, k & 1, st)
+                e1.record()
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1) / args.reps
+                cg = vh * bm["compulsory_bytes_per_site"] / (ms * 1e-3) / 1e9
+                print(json.dumps({"workload": f"SU({N}) {rep} {dims[1]}^3x{dims[0]}", "d_R": bm["d"], "dtype": prec,
+                                  "variant": NAMES[v], "default": NAMES[v] == default, "ms": ms,
+                                  "compulsory_mb": vh * bm["compulsory_bytes_per_site"] / 1e6, "compulsory_gbs": cg,
+                                  "compulsory_frac_of_copy_peak": cg / peak,
+                                  "gflops": vh * bm["dphi_flops_per_site"] / (ms * 1e-3) / 1e9}), flush=True)
+            lat.close()
+            torch.cuda.empty_cache()
+
+
+
+def solver(argv):
+    """Measurement of the NEXT-1 rows: the paper's second benchmark, the spinor linear
+    algebra of PAPER.md:108-120 / Fig. 7 ("Copy spinor field", "g5 application", "g5 mulc add assign", norms and
+    inner products; SU(3) fundamental), plus hr_dhat and one CG iteration.
+    
+        python bench_sweeps.py solver [--config 2|3|4|5] [--prec f64|f32] [--reps 50]
+    
+    Prints one JSON line per operation: algorithmic bytes (S = spinor bytes per site, Vh sites: copy/g5 2S,
+    g5_mulc_add_assign 3S, norm2 1S, dot 2S; Dhat 2(8L+2S)+S; CG iteration 4(8L+2S) + 2S + 8S), the time per call
+    from CUDA events on the launching stream (back to back, fields larger than L2 rotate through 4 buffer sets),
+    GB/s and the fraction of the measured copy peak (MEASURED_PEAKS.json).  Inputs: the seeded synthetic fields
+    of bench.py's configs.  bench.py stays the headline; this script is the Fig. 7 companion."""
     import torch
     import bench as B
     import paper_2405_19294_b200 as hr
 
-    ap = argparse.ArgumentParser()
+    ap = argparse.ArgumentParser(prog="bench_sweeps.py solver")
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--reps", type=int, default=50)
     ap.add_argument("--m0", type=float, default=0.1)
-    args = ap.parse_args()
+    args = ap.parse_args(argv)
     if not torch.cuda.is_available():
-        raise SystemExit("bench_solver: no CUDA device; the product path has no CPU fallback")
+        raise SystemExit("bench_sweeps solver: no CUDA device; the product path has no CPU fallback")
     cfg = B.CONFIGS[args.config]
     bm = B.byte_model(cfg, args.prec)
     P = hr.PREC_NAMES[args.prec]
@@ -210,5 +361,11 @@ def main():
     lat.close()
 
 
+
+
+SWEEPS = {"volume": volume, "large_n": large_n, "solver": solver}
+
 if __name__ == "__main__":
-    main()
+    if len(sys.argv) < 2 or sys.argv[1] not in SWEEPS:
+        raise SystemExit(__doc__)
+    SWEEPS[sys.argv[1]](sys.argv[2:])
