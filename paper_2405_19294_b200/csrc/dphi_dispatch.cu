@@ -6,12 +6,13 @@
 namespace hr {
 
 template <typename Real, int D, int LK>
-hr_status launch_dphi_t(int variant, int block, const DphiArgs &a, cudaStream_t st);
+hr_status launch_dphi_t(int variant, const LaunchTune &lt, const DphiArgs &a, cudaStream_t st);
 template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant);
+template <typename Real, int D, int LK> bool dphi_bulk_ok_t(const DphiArgs &a);
 
 template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, int mu, const HaloArgs &a, cudaStream_t st);
 
-static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour" };
+static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour", "bulk", "bulk2" };
 
 // Default variant per (d_R, link type, precision, volume): filled from measurements.
 static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
@@ -65,10 +66,11 @@ hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStre
         return HR_EUNSUPPORTED;
     }
     const int v = resolve_variant(c, prec, lk);
+    const LaunchTune lt = { c->block, c->bulk_rows, c->bulk_stages, c->bulk_ctas };
 #define X(D, LK)                                                                                          \
     if (c->d == D && lk == LK)                                                                            \
-        return prec == HR_F64 ? launch_dphi_t<double, D, LK>(v, c->block, a, st)                         \
-                              : launch_dphi_t<float, D, LK>(v, c->block, a, st);
+        return prec == HR_F64 ? launch_dphi_t<double, D, LK>(v, lt, a, st)                               \
+                              : launch_dphi_t<float, D, LK>(v, lt, a, st);
     HR_COMBOS(X)
 #undef X
     set_error("no Dphi kernel compiled for d_R=%d (link kind %d)", c->d, lk);

@@ -4,9 +4,14 @@
 #pragma once
 #include <type_traits>
 
+#include "dphi_kernel.cuh"
+#ifdef HR_BUILD_EXPERIMENTS
+// variants that were measured and lost everywhere (DESIGN.md sections 7, 14); kept as evidence, not in the default build
 #include "dphi_pf_kernel.cuh"
-#include "dphi_cp_kernel.cuh"
 #include "dphi_cpo_kernel.cuh"
+#endif
+#include "dphi_cp_kernel.cuh"
+#include "dphi_bulk_kernel.cuh"
 #include "halo_kernel.cuh"
 
 namespace hr {
@@ -20,10 +25,17 @@ namespace hr {
 //   5 site_pf   one thread per site, the next hop's operands prefetched with cp.async into a private,
 //               double-buffered shared-memory stage (dphi_pf_kernel.cuh)
 //   6 colour    one thread per (site, colour row): the large-d_R kernel (dphi_cp_kernel.cuh; represented links)
+//   7 bulk      persistent CTAs, operands of every hop staged in shared memory by TMA bulk copies (dphi_bulk_kernel.cuh)
+//   8 bulk2     the same with two consumer threads per site (one per half-spinor component)
 // d_R > 8 (SU(4) two-index symmetric, adjoint) compiles only 0 (the paper's "unimproved" kernel, for comparison) and 6.
-enum { DPHI_NVARIANTS = 7 };
-static const char *const kDphiVariantNames[DPHI_NVARIANTS] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour" };
-static const size_t kMaxDynSmem = 227 * 1024;
+// Variants 4, 5 and the colour-parallel on-the-fly kernel lost every measurement: they are compiled only with
+// -DHR_BUILD_EXPERIMENTS; the pair kernels (2, 3) only where they were ever competitive (d_R >= 6).
+enum { DPHI_NVARIANTS = 9 };
+#ifdef HR_BUILD_EXPERIMENTS
+static constexpr bool kExperiments = true;
+#else
+static constexpr bool kExperiments = false;
+#endif
 
 // registers: __launch_bounds__(MAXT, MINB) caps them at 65536 / (MAXT*MINB)
 template <typename Real, int D, int LK, int KSPLIT> struct Tune {
@@ -66,6 +78,7 @@ static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
     return HR_OK;
 }
 
+#ifdef HR_BUILD_EXPERIMENTS
 template <typename Real, int D, int LK, bool MASS, bool RED>
 static hr_status launch_pf(int block, const DphiArgs &a, cudaStream_t st)
 {
@@ -93,18 +106,28 @@ static hr_status launch_pf(int block, const DphiArgs &a, cudaStream_t st)
     if (e != cudaSuccess) { set_error("dphi_pf kernel launch failed: %s", cudaGetErrorString(e)); return HR_ECUDA; }
     return HR_OK;
 }
+#endif
 
 template <typename Real, int D, int LK, bool MASS, bool RED>
-static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaStream_t st)
+static hr_status launch_variant(int variant, const LaunchTune &lt, const DphiArgs &a, cudaStream_t st)
 {
     constexpr int RPV = 16 / (int)sizeof(Real);
-    constexpr bool PAIR_OK = (2 * D) % RPV == 0;
+    constexpr bool PAIR_OK = (2 * D) % RPV == 0 && (D >= 6 || kExperiments);
     constexpr bool CP_OK = (LK == LK_COMPLEX || LK == LK_REAL);
+    const int block = lt.block;
     if constexpr (CP_OK) {
         if (variant == 6) return launch_cp<Real, D, LK, MASS, RED>(a, st);
     }
+#ifdef HR_BUILD_EXPERIMENTS
     if constexpr (LK == LK_SYM_OTF || LK == LK_ASYM_OTF) {
         if (variant == 6) return launch_cpo<Real, D, LK, MASS, RED>(a, st);
+    }
+#endif
+    if constexpr (D <= 8) {
+        if (variant == 7) return launch_bulk<Real, D, LK, MASS, RED>(a, st, BulkTuning{ lt.bulk_rows, lt.bulk_stages, lt.bulk_ctas });
+        if constexpr ((2 * D) % RPV == 0 && (D >= 6 || LK == LK_SYM_OTF || LK == LK_ASYM_OTF)) {
+            if (variant == 8) return launch_bulk<Real, D, LK, MASS, RED, 2>(a, st, BulkTuning{ lt.bulk_rows, lt.bulk_stages, lt.bulk_ctas });
+        }
     }
     if constexpr (D > 8) {
         if (variant == 0) return launch_one<Real, D, LK, 1, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
@@ -118,10 +141,12 @@ static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaS
     case 3:
         if constexpr (PAIR_OK) return launch_one<Real, D, LK, 2, MASS, RED, LD_STREAM_EF, LD_KEEP, ST_STREAM>(block, a, st);
         break;
+#ifdef HR_BUILD_EXPERIMENTS
     case 4: return launch_one<Real, D, LK, 1, MASS, RED, LD_DEFAULT, LD_DEFAULT, ST_DEFAULT>(block, a, st);
     case 5:
         if constexpr (PfGeom<Real, D, LK>::smem_bytes(64) <= kMaxDynSmem) return launch_pf<Real, D, LK, MASS, RED>(block, a, st);
         break;
+#endif
     default: break;
     }
     set_error("dphi variant %d not available for d_R=%d, %s", variant, D, sizeof(Real) == 8 ? "fp64" : "fp32");
@@ -129,8 +154,9 @@ static hr_status launch_variant(int variant, int block, const DphiArgs &a, cudaS
 }
 
 template <typename Real, int D, int LK>
-hr_status launch_dphi_t(int variant, int block, const DphiArgs &a, cudaStream_t st)
+hr_status launch_dphi_t(int variant, const LaunchTune &lt, const DphiArgs &a, cudaStream_t st)
 {
+    const int block = lt.block;
     if (a.site_mode != 0) {
         // fused site-diagonal matrix: the `site` / `site_ef` kernels only, complex-link kinds with a clover field
         if constexpr ((LK == LK_COMPLEX || LK == LK_REAL) && D <= 8) {
@@ -146,20 +172,37 @@ hr_status launch_dphi_t(int variant, int block, const DphiArgs &a, cudaStream_t 
         set_error("fused site matrix: not available for this kernel variant / link kind");
         return HR_EUNSUPPORTED;
     }
-    if (a.self && a.red_result) return launch_variant<Real, D, LK, true, true>(variant, block, a, st);
-    if (a.self) return launch_variant<Real, D, LK, true, false>(variant, block, a, st);
-    return launch_variant<Real, D, LK, false, false>(variant, block, a, st);
+    if (a.self && a.red_result) return launch_variant<Real, D, LK, true, true>(variant, lt, a, st);
+    if (a.self) return launch_variant<Real, D, LK, true, false>(variant, lt, a, st);
+    return launch_variant<Real, D, LK, false, false>(variant, lt, a, st);
 }
 
 template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant)
 {
     constexpr int RPV = 16 / (int)sizeof(Real);
     if (variant < 0 || variant >= DPHI_NVARIANTS) return false;
-    if (variant == 6) return LK == LK_COMPLEX || LK == LK_REAL || LK == LK_SYM_OTF || LK == LK_ASYM_OTF;
+    if (variant == 6) return LK == LK_COMPLEX || LK == LK_REAL || (kExperiments && (LK == LK_SYM_OTF || LK == LK_ASYM_OTF));
+    if (variant == 7) return D <= 8;   // whether a tile can be aligned on THIS lattice is decided at launch (bulk_geometry)
+    if (variant == 8) return D <= 8 && (2 * D) % RPV == 0 && (D >= 6 || LK == LK_SYM_OTF || LK == LK_ASYM_OTF);
     if (D > 8) return variant == 0;
-    if ((variant == 2 || variant == 3) && (2 * D) % RPV != 0) return false;
-    if (variant == 5 && PfGeom<Real, D, LK>::smem_bytes(64) > kMaxDynSmem) return false;
+    if ((variant == 2 || variant == 3) && ((2 * D) % RPV != 0 || !(D >= 6 || kExperiments))) return false;
+    if (variant == 4 || variant == 5) {
+#ifdef HR_BUILD_EXPERIMENTS
+        return variant == 4 || PfGeom<Real, D, LK>::smem_bytes(64) <= kMaxDynSmem;
+#else
+        return false;
+#endif
+    }
     return true;
+}
+
+// can the bulk kernel tile this lattice (alignment of the tail planes, Zh <= 128)?
+template <typename Real, int D, int LK> bool dphi_bulk_ok_t(const DphiArgs &a)
+{
+    if constexpr (D <= 8) {
+        BulkArgs g;
+        return bulk_geometry<Real, D, LK>(a, g, kMaxDynSmem, 0, 0);
+    } else return false;
 }
 
 template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, int mu, const HaloArgs &a, cudaStream_t st)
@@ -185,8 +228,9 @@ template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, int m
 }
 
 #define HR_DPHI_INSTANCE(Real, D, LK)                                                                    \
-    template hr_status launch_dphi_t<Real, D, LK>(int, int, const DphiArgs &, cudaStream_t);             \
+    template hr_status launch_dphi_t<Real, D, LK>(int, const LaunchTune &, const DphiArgs &, cudaStream_t); \
     template bool dphi_variant_ok_t<Real, D, LK>(int);                                                    \
+    template bool dphi_bulk_ok_t<Real, D, LK>(const DphiArgs &);                                          \
     template hr_status launch_halo_t<Real, D, LK>(bool, int, const HaloArgs &, cudaStream_t);
 
 } // namespace hr
