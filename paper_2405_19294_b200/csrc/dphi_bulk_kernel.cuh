@@ -126,7 +126,10 @@ template <typename Real, int D, int LK> struct BulkGeom {
 // a broadcast --, one shuffle at the end): half the live state per thread and twice the warps, for the sites whose
 // arithmetic (on-the-fly representations, d_R >= 6) is too much for four warps per SM.
 template <typename Real, int D, int LK, bool MASS, bool RED, int KS>
-__global__ void __launch_bounds__((KS == 1 ? 32 + BulkGeom<Real, D, LK>::MAXN : 256), 1)
+#ifndef HR_BULK2_MINB
+#define HR_BULK2_MINB 1
+#endif
+__global__ void __launch_bounds__((KS == 1 ? 32 + BulkGeom<Real, D, LK>::MAXN : 256), (KS == 1 ? 1 : HR_BULK2_MINB))
 dphi_bulk_kernel(const DphiArgs a, const BulkArgs g, const __grid_constant__ BulkMaps maps)
 {
     static_assert(KS == 1 || (2 * D) % (16 / (int)sizeof(Real)) == 0, "two threads per site need vector-aligned spin components");
@@ -300,8 +303,8 @@ dphi_bulk_kernel(const DphiArgs a, const BulkArgs g, const __grid_constant__ Bul
                     }
                 }
                 [[maybe_unused]] const int jl = DIR == 0 ? i : j;
-                constexpr int P0 = (MU == 0 || MU == 3) ? 2 : 3;
-                constexpr int P1 = 5 - P0;
+                [[maybe_unused]] constexpr int P0 = (MU == 0 || MU == 3) ? 2 : 3;
+                [[maybe_unused]] constexpr int P1 = 5 - P0;
                 const Real sgn = (Real)sign;
                 constexpr bool STRAIGHT = (MU == 0 || MU == 3);
                 const int pk = STRAIGHT ? kk + 2 : 3 - kk;
@@ -421,8 +424,8 @@ dphi_bulk_kernel(const DphiArgs a, const BulkArgs g, const __grid_constant__ Bul
                     }
                 }
                 [[maybe_unused]] const int jl = DIR == 0 ? i : j;
-                constexpr int P0 = (MU == 0 || MU == 3) ? 2 : 3;
-                constexpr int P1 = 5 - P0;
+                [[maybe_unused]] constexpr int P0 = (MU == 0 || MU == 3) ? 2 : 3;
+                [[maybe_unused]] constexpr int P1 = 5 - P0;
                 const Real sgn = (Real)sign;
 
                 mbar_wait(full0 + 8 * stage, phase);

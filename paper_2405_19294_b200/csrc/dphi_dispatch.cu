@@ -8,15 +8,39 @@ namespace hr {
 template <typename Real, int D, int LK>
 hr_status launch_dphi_t(int variant, const LaunchTune &lt, const DphiArgs &a, cudaStream_t st);
 template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant);
-template <typename Real, int D, int LK> bool dphi_bulk_ok_t(const DphiArgs &a);
+template <typename Real, int D, int LK> bool dphi_bulk_ok_t(const DphiArgs &a, int ks);
 
 template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, int mu, const HaloArgs &a, cudaStream_t st);
 
-static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour", "bulk", "bulk2" };
+static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour", "bulk", "bulk2", "bulkx", "bulkx2" };
+
+#define HR_COMBOS(X)                                                                                      \
+    X(2, 0) X(3, 0) X(4, 0) X(6, 0) X(3, 1) X(8, 1) X(3, 2) X(6, 2) X(3, 3) X(6, 3) X(2, 4) X(3, 4) X(3, 5) X(8, 6) X(8, 7) X(10, 0) X(15, 1)
+
+// can the bulk kernel (variants 7 / 8, ks consumer threads per site) tile this lattice?
+static bool bulk_ok(const hr_ctx *c, hr_prec prec, int lk, int ks)
+{
+    DphiArgs a = {};
+    a.T = c->dims[0]; a.X = c->dims[1]; a.Y = c->dims[2]; a.Zh = c->dims[3] / 2; a.vh = c->Vh;
+#define X(D, LK)                                                                                          \
+    if (c->d == D && lk == LK) return prec == HR_F64 ? dphi_bulk_ok_t<double, D, LK>(a, ks) : dphi_bulk_ok_t<float, D, LK>(a, ks);
+    HR_COMBOS(X)
+#undef X
+    return false;
+}
 
 // Default variant per (d_R, link type, precision, volume): filled from measurements.
 static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
 {
+    // measured under sustained (power-capped) clocks, profiles/r2_staging.md: the TMA-staged kernels win where the site
+    // kernel is latency-bound at its 8 warps per SM -- row-compressed links in fp64 (+5-8 %), the fp32 sextet with
+    // represented links (+9 %), the fp64 sextet applied on the fly (+4 %)
+    if ((lk == 4 || lk == 5) && prec == HR_F64 && bulk_ok(c, prec, lk, 1)) return 7;
+    // d_R = 3 represented links in fp64 on lattices with Z <= 32 (tiles of 8 rows): +4-6 % (complex), +2 % (real) on 32^3x64,
+    // 32^3x256, 64^3x32(z); on Z = 64 lattices (64^4) the site kernel stays ahead
+    if ((lk == 0 || lk == 1) && c->d == 3 && prec == HR_F64 && c->dims[3] <= 32 && c->dims[3] >= 16 && bulk_ok(c, prec, lk, 1)) return 7;
+    if (lk == 2 && c->d == 6 && prec == HR_F64 && bulk_ok(c, prec, lk, 2)) return 8;
+    if (lk == 0 && c->d == 6 && prec == HR_F32 && bulk_ok(c, prec, lk, 2)) return 8;
     // on-the-fly two-index kernels hold an N x N link, not a d_R x d_R one: a whole site fits one thread
     if (lk == 2 || lk == 3 || lk == 4) return 0;
     if (lk == 6 || lk == 7) return prec == HR_F64 ? 2 : 0; // fp64 d_R = 8: two threads per site (measured)
@@ -35,6 +59,14 @@ static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
 }
 
 static int resolve_variant(const hr_ctx *c, hr_prec prec, int lk) { return c->variant >= 0 ? c->variant : default_variant(c, prec, lk); }
+// the variant for a launch that carries a fused site matrix: the staged kernels have no such epilogue, so where one of
+// them is the DEFAULT the site kernel it replaced takes these launches (an explicitly chosen variant is respected)
+static int resolve_variant_fused(const hr_ctx *c, hr_prec prec, int lk)
+{
+    const int v = resolve_variant(c, prec, lk);
+    if (c->variant < 0 && v >= 7) return (lk == 1 && c->d == 3) ? 1 : 0;
+    return v;
+}
 
 // link kind (dphi_kernel.cuh): 0 complex d_R x d_R, 1 real d_R x d_R (adjoint), 2 / 3 two-index symmetric /
 // antisymmetric applied on the fly from the fundamental link
@@ -55,9 +87,6 @@ int dphi_link_kind(const hr_ctx *c, int link_src)
     return -1;
 }
 
-#define HR_COMBOS(X)                                                                                      \
-    X(2, 0) X(3, 0) X(4, 0) X(6, 0) X(3, 1) X(8, 1) X(3, 2) X(6, 2) X(3, 3) X(6, 3) X(2, 4) X(3, 4) X(3, 5) X(8, 6) X(8, 7) X(10, 0) X(15, 1)
-
 hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStream_t st, int link_src)
 {
     const int lk = dphi_link_kind(c, link_src);
@@ -65,8 +94,8 @@ hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStre
         set_error("this kind of link field has no kernel for this representation (use hr_represent_links)");
         return HR_EUNSUPPORTED;
     }
-    const int v = resolve_variant(c, prec, lk);
-    const LaunchTune lt = { c->block, c->bulk_rows, c->bulk_stages, c->bulk_ctas };
+    const int v = a.site_mode != 0 ? resolve_variant_fused(c, prec, lk) : resolve_variant(c, prec, lk);
+    const LaunchTune lt = { c->block, c->bulk_rows, c->bulk_stages, c->bulk_ctas, c->bulk_strip };
 #define X(D, LK)                                                                                          \
     if (c->d == D && lk == LK)                                                                            \
         return prec == HR_F64 ? launch_dphi_t<double, D, LK>(v, lt, a, st)                               \
@@ -96,7 +125,7 @@ bool dphi_site_fusable(const hr_ctx *c, hr_prec prec, int link_src)
     // measured: fp64 d_R = 3 gains 18-30 %; fp32 (128-register cap) is no faster fused, and at
     // d_R >= 6 the block mat-vec spills in a kernel already at 255 registers
     if ((lk != 0 && lk != 1) || c->d > 4 || prec != HR_F64) return false;
-    const int v = resolve_variant(c, prec, lk);
+    const int v = resolve_variant_fused(c, prec, lk);
     return v == 0 || v == 1;
 }
 

@@ -150,10 +150,12 @@ __device__ __forceinline__ void twoindex_mul(Real (&chi)[2 * D], const Real *u, 
     // W = U (or U^dagger):  wr/wi[i][k], the imaginary part conjugated for the dagger
     auto wr = [&](int i, int k) -> Real { return DAG ? u[2 * (k * N + i)] : u[2 * (i * N + k)]; };
     auto wi = [&](int i, int k) -> Real { return DAG ? -u[2 * (k * N + i) + 1] : u[2 * (i * N + k) + 1]; };
-    // A = W Psi'
-    Real ar[N][N], ai[N][N];
+    // row by row:  A_i. = (W Psi')_i.  is used at once for  M'_ij = sum_l A_il W_jl  (j >= i: M' is (anti)symmetric), so only
+    // one row of A is ever live -- 2N reals instead of 2N^2 (the register budget of this kernel is what limits its warps)
+    int a = 0;
 #pragma unroll
-    for (int i = 0; i < N; ++i)
+    for (int i = 0; i < N; ++i) {
+        Real ar[N], ai[N];
 #pragma unroll
         for (int l = 0; l < N; ++l) {
             Real re = 0, im = 0;
@@ -163,25 +165,22 @@ __device__ __forceinline__ void twoindex_mul(Real (&chi)[2 * D], const Real *u, 
                 re = fma(wr(i, k), pr[k][l], re); re = fma(-wi(i, k), pi[k][l], re);
                 im = fma(wr(i, k), pi[k][l], im); im = fma(wi(i, k), pr[k][l], im);
             }
-            ar[i][l] = re; ai[i][l] = im;
+            ar[l] = re; ai[l] = im;
         }
-    // M' = A W^T, needed entries only
-    int a = 0;
-#pragma unroll
-    for (int i = 0; i < N; ++i)
 #pragma unroll
         for (int j = i; j < N; ++j) {
             if (!SYM && i == j) continue;
             Real re = 0, im = 0;
 #pragma unroll
             for (int l = 0; l < N; ++l) {
-                re = fma(ar[i][l], wr(j, l), re); re = fma(-ai[i][l], wi(j, l), re);
-                im = fma(ar[i][l], wi(j, l), im); im = fma(ai[i][l], wr(j, l), im);
+                re = fma(ar[l], wr(j, l), re); re = fma(-ai[l], wi(j, l), re);
+                im = fma(ar[l], wi(j, l), im); im = fma(ai[l], wr(j, l), im);
             }
             if (i == j) { re *= (Real)0.7071067811865476; im *= (Real)0.7071067811865476; }
             chi[2 * a] = re; chi[2 * a + 1] = im;
             ++a;
         }
+    }
 }
 
 // full N x N complex link from its first N-1 rows (N = 2, 3)

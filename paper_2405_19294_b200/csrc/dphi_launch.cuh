@@ -12,6 +12,7 @@
 #endif
 #include "dphi_cp_kernel.cuh"
 #include "dphi_bulk_kernel.cuh"
+#include "dphi_bulkx_kernel.cuh"
 #include "halo_kernel.cuh"
 
 namespace hr {
@@ -27,10 +28,13 @@ namespace hr {
 //   6 colour    one thread per (site, colour row): the large-d_R kernel (dphi_cp_kernel.cuh; represented links)
 //   7 bulk      persistent CTAs, operands of every hop staged in shared memory by TMA bulk copies (dphi_bulk_kernel.cuh)
 //   8 bulk2     the same with two consumer threads per site (one per half-spinor component)
+//   9 bulkx     bulk + the neighbour spinors of a time-slice kept in shared memory along a strip in x and re-used across
+//               sites (dphi_bulkx_kernel.cuh); d_R <= 4
+//  10 bulkx2    bulkx with two consumer threads per site
 // d_R > 8 (SU(4) two-index symmetric, adjoint) compiles only 0 (the paper's "unimproved" kernel, for comparison) and 6.
 // Variants 4, 5 and the colour-parallel on-the-fly kernel lost every measurement: they are compiled only with
 // -DHR_BUILD_EXPERIMENTS; the pair kernels (2, 3) only where they were ever competitive (d_R >= 6).
-enum { DPHI_NVARIANTS = 9 };
+enum { DPHI_NVARIANTS = 11 };
 #ifdef HR_BUILD_EXPERIMENTS
 static constexpr bool kExperiments = true;
 #else
@@ -129,6 +133,13 @@ static hr_status launch_variant(int variant, const LaunchTune &lt, const DphiArg
             if (variant == 8) return launch_bulk<Real, D, LK, MASS, RED, 2>(a, st, BulkTuning{ lt.bulk_rows, lt.bulk_stages, lt.bulk_ctas });
         }
     }
+    if constexpr (D <= 4) {
+        const BulkTuning bt{ lt.bulk_rows, lt.bulk_stages, lt.bulk_ctas };
+        if (variant == 9) return launch_bulkx<Real, D, LK, MASS, RED, 1>(a, st, bt, lt.bulk_strip);
+        if constexpr ((2 * D) % RPV == 0) {
+            if (variant == 10) return launch_bulkx<Real, D, LK, MASS, RED, 2>(a, st, bt, lt.bulk_strip);
+        }
+    }
     if constexpr (D > 8) {
         if (variant == 0) return launch_one<Real, D, LK, 1, MASS, RED, LD_STREAM, LD_DEFAULT, ST_DEFAULT>(block, a, st);
     } else
@@ -184,6 +195,8 @@ template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant)
     if (variant == 6) return LK == LK_COMPLEX || LK == LK_REAL || (kExperiments && (LK == LK_SYM_OTF || LK == LK_ASYM_OTF));
     if (variant == 7) return D <= 8;   // whether a tile can be aligned on THIS lattice is decided at launch (bulk_geometry)
     if (variant == 8) return D <= 8 && (2 * D) % RPV == 0 && (D >= 6 || LK == LK_SYM_OTF || LK == LK_ASYM_OTF);
+    if (variant == 9) return D <= 4;
+    if (variant == 10) return D <= 4 && (2 * D) % RPV == 0;
     if (D > 8) return variant == 0;
     if ((variant == 2 || variant == 3) && ((2 * D) % RPV != 0 || !(D >= 6 || kExperiments))) return false;
     if (variant == 4 || variant == 5) {
@@ -197,11 +210,11 @@ template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant)
 }
 
 // can the bulk kernel tile this lattice (alignment of the tail planes, Zh <= 128)?
-template <typename Real, int D, int LK> bool dphi_bulk_ok_t(const DphiArgs &a)
+template <typename Real, int D, int LK> bool dphi_bulk_ok_t(const DphiArgs &a, int ks)
 {
     if constexpr (D <= 8) {
         BulkArgs g;
-        return bulk_geometry<Real, D, LK>(a, g, kMaxDynSmem, 0, 0);
+        return bulk_geometry<Real, D, LK>(a, g, kMaxDynSmem - 1024, 0, 0, ks == 1 ? BulkGeom<Real, D, LK>::MAXN : 112);
     } else return false;
 }
 
@@ -230,7 +243,7 @@ template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, int m
 #define HR_DPHI_INSTANCE(Real, D, LK)                                                                    \
     template hr_status launch_dphi_t<Real, D, LK>(int, const LaunchTune &, const DphiArgs &, cudaStream_t); \
     template bool dphi_variant_ok_t<Real, D, LK>(int);                                                    \
-    template bool dphi_bulk_ok_t<Real, D, LK>(const DphiArgs &);                                          \
+    template bool dphi_bulk_ok_t<Real, D, LK>(const DphiArgs &, int);                                                \
     template hr_status launch_halo_t<Real, D, LK>(bool, int, const HaloArgs &, cudaStream_t);
 
 } // namespace hr

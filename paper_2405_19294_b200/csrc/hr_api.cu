@@ -177,7 +177,7 @@ hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N,
     c->block = 0;
     c->xblock = 0;
     c->cg_graph = 1;
-    c->bulk_rows = c->bulk_stages = c->bulk_ctas = 0;
+    c->bulk_rows = c->bulk_stages = c->bulk_ctas = c->bulk_strip = 0;
     c->ws_in = c->ws_out = c->ws_stage = nullptr;
     c->ws_spinor_bytes = c->ws_stage_bytes = 0;
     c->ws_prec = -1;
@@ -489,9 +489,9 @@ hr_status hr_ctx_set_tuning(hr_ctx *ctx, const char *key, int value)
         ctx->xblock = value;
         return HR_OK;
     }
-    if (!strcmp(key, "bulk_rows") || !strcmp(key, "bulk_stages") || !strcmp(key, "bulk_ctas")) {
+    if (!strcmp(key, "bulk_rows") || !strcmp(key, "bulk_stages") || !strcmp(key, "bulk_ctas") || !strcmp(key, "bulk_strip")) {
         if (value < 0 || value > 128) { set_error("hr_ctx_set_tuning: %s=%d", key, value); return HR_EINVAL; }
-        (key[5] == 'r' ? ctx->bulk_rows : key[5] == 's' ? ctx->bulk_stages : ctx->bulk_ctas) = value;
+        (key[5] == 'r' ? ctx->bulk_rows : !strcmp(key, "bulk_stages") ? ctx->bulk_stages : key[5] == 'c' ? ctx->bulk_ctas : ctx->bulk_strip) = value;
         return HR_OK;
     }
     if (!strcmp(key, "cg_graph")) {

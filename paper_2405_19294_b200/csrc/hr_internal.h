@@ -32,6 +32,7 @@ struct hr_ctx {
     int xblock;     // 0 = default (from the L2 working-set rule), else a divisor of X
     int cg_graph;   // 1 (default): the CG replays one captured iteration as a CUDA graph; 0: plain launches
     int bulk_rows, bulk_stages, bulk_ctas; // bulk kernel (variant 7): rows per tile / ring depth / CTAs per SM; 0 = default
+    int bulk_strip; // bulkx kernel (variants 9, 10): tiles per strip; 0 = default
     // host-path workspace (hr_dphi_eo_host)
     void *ws_in, *ws_out, *ws_stage;
     size_t ws_spinor_bytes, ws_stage_bytes;
@@ -118,6 +119,7 @@ struct CgState {
 struct LaunchTune {
     int block;                              // CTA size of the site / pair kernels; 0 = default
     int bulk_rows, bulk_stages, bulk_ctas;  // bulk kernel (dphi_bulk_kernel.cuh); 0 = default
+    int bulk_strip;                         // bulkx kernel (dphi_bulkx_kernel.cuh); 0 = default
 };
 static const size_t kMaxDynSmem = 227 * 1024;
 

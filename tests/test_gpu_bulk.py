@@ -55,7 +55,7 @@ def _bulk_or_skip(hr, prob, links, gin, parity):
 @pytest.mark.parametrize("N,rep", [(2, "fund"), (3, "fund"), (4, "fund"), (2, "adj"), (2, "sym"), (3, "sym"), (3, "asym"), (3, "adj"), (4, "asym")])
 @pytest.mark.parametrize("dims,bc", [((4, 4, 6, 8), BC_T), ((2, 2, 2, 2), (-1, -1, -1, -1)), ((6, 2, 4, 12), (1, -1, 1, -1)),
                                      ((4, 6, 8, 32), (1, 1, -1, 1)), ((2, 4, 2, 4), (-1, 1, 1, -1))])
-@pytest.mark.parametrize("variant", [7, 8])
+@pytest.mark.parametrize("variant", [7, 8, 9, 10])
 def test_bulk_kernel_matches_oracle(hr, dims, bc, N, rep, prec, variant):
     d = oracle.rep_dim(N, oracle_rep_id(rep))
     U = li.haar_links(701, N, dims)
@@ -66,8 +66,8 @@ def test_bulk_kernel_matches_oracle(hr, dims, bc, N, rep, prec, variant):
         prob.lat.set_tuning("variant", variant)
     except hr.HrError:
         prob.close()
-        pytest.skip("two consumer threads per site: compiled for d_R >= 6 with vector-aligned spin components only")
-    assert hr.hr_dphi_variant_name(prob.lat.ctx, prob.prec) == ("bulk" if variant == 7 else "bulk2")
+        pytest.skip("this variant is not compiled for this d_R / precision")
+    assert hr.hr_dphi_variant_name(prob.lat.ctx, prob.prec) == {7: "bulk", 8: "bulk2", 9: "bulkx", 10: "bulkx2"}[variant]
     ran = 0
     for parity in (0, 1):
         psi = li.gaussian_spinor(702 + parity, vh, d)
@@ -111,6 +111,42 @@ def test_bulk_tile_and_ring_geometry_do_not_change_the_result(hr, prec):
     prob.close()
 
 
+@pytest.mark.parametrize("variant", [9, 10])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_bulkx_strip_and_tile_geometry_do_not_change_the_result(hr, prec, variant):
+    """bulkx: rows per tile, tiles per strip and the x-block of the strip order are scheduling only (bitwise)."""
+    dims, N, rep = (4, 12, 8, 8), 3, "fund"
+    U = li.haar_links(713, N, dims)
+    vh = li.volume(dims) // 2
+    psi = li.gaussian_spinor(714, vh, 3)
+    want = oracle.dphi_eo(dims, (-1, -1, 1, -1), U, 0, psi)
+    prob = GpuProblem(hr, dims, N, rep, prec, U, bc=(-1, -1, 1, -1))
+    try:
+        prob.lat.set_tuning("variant", variant)
+    except hr.HrError:
+        prob.close()
+        pytest.skip("bulkx2 needs vector-aligned spin components")
+    gin = _put(prob, psi, 1)
+    if _bulk_or_skip(hr, prob, prob.links, gin, 0) is None:
+        prob.close()
+        pytest.skip("bulkx2 needs vector-aligned spin components (fp32: even d_R)")
+    ref = None
+    for xblock in (0, 12, 6, 4, 1):
+        for strip in (0, 1, 2, 3, 4, 6, 12):
+            for rows in (0, 1, 2, 4, 8):
+                prob.lat.set_tuning("xblock", xblock)
+                prob.lat.set_tuning("bulk_strip", strip)
+                prob.lat.set_tuning("bulk_rows", rows)
+                out = _new(prob)
+                prob.lat.dphi_eo(out, gin, prob.links, 0)
+                got = prob.lat.export_spinor(out, prob.prec, 0)
+                assert rel_l2(got, want) <= TOL[prec], (xblock, strip, rows)
+                if ref is None:
+                    ref = got
+                assert np.array_equal(got.view(np.uint8), ref.view(np.uint8)), (xblock, strip, rows)
+    prob.close()
+
+
 # many launches back to back on one stream: the ring's phase bits start afresh in every launch; repeated = bitwise equal
 def test_bulk_repeated_launches_are_bitwise_identical(hr):
     dims, N = (8, 8, 8, 16), 3
@@ -135,7 +171,7 @@ def test_bulk_repeated_launches_are_bitwise_identical(hr):
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("N,rep,src", [(3, "sym", "fund"), (2, "sym", "fund"), (3, "asym", "fund"), (4, "asym", "fund"), (3, "adj", "fund"),
                                        (3, "fund", "rows"), (2, "fund", "rows"), (2, "adj", "rows"), (3, "adj", "rows")])
-@pytest.mark.parametrize("variant", [7, 8])
+@pytest.mark.parametrize("variant", [7, 8, 9, 10])
 def test_bulk_kernel_with_on_the_fly_and_row_compressed_links(hr, N, rep, src, prec, variant):
     dims = (4, 4, 6, 8)
     d = oracle.rep_dim(N, oracle_rep_id(rep))
@@ -157,9 +193,9 @@ def test_bulk_kernel_with_on_the_fly_and_row_compressed_links(hr, N, rep, src, p
         psi = li.gaussian_spinor(732 + parity, vh, d)
         want = oracle.dphi_eo(dims, BC_T, R, parity, psi)
         got = _bulk_or_skip(hr, prob, links, _put(prob, psi, 1 - parity), parity)
-        if got is None and variant == 8:
+        if got is None and variant != 7:
             prob.close()
-            pytest.skip("bulk2 is not compiled for this link kind / precision")
+            pytest.skip("this variant is not compiled for this link kind / precision")
         assert got is not None
         assert rel_l2(got, want) <= TOL[prec], parity
     prob.close()
@@ -167,7 +203,7 @@ def test_bulk_kernel_with_on_the_fly_and_row_compressed_links(hr, N, rep, src, p
 
 # the epilogues: hr_dirac (self term), hr_dhat with and without gamma5, the CG (fused reduction + skip flag)
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("N,rep,variant", [(3, "fund", 7), (2, "adj", 7), (3, "sym", 7), (3, "sym", 8)])
+@pytest.mark.parametrize("N,rep,variant", [(3, "fund", 7), (2, "adj", 7), (3, "sym", 7), (3, "sym", 8), (3, "fund", 9), (3, "fund", 10), (2, "adj", 9), (2, "fund", 10)])
 def test_bulk_kernel_dirac_dhat_and_cg(hr, N, rep, prec, variant):
     dims, m0 = (4, 4, 4, 8), -0.3
     d = oracle.rep_dim(N, oracle_rep_id(rep))
@@ -177,6 +213,9 @@ def test_bulk_kernel_dirac_dhat_and_cg(hr, N, rep, prec, variant):
     vh = V // 2
     prob = GpuProblem(hr, dims, N, rep, prec, U)
     prob.lat.set_tuning("variant", variant)
+    if variant in (8, 10) and prec == "f32" and d % 2:
+        prob.close()
+        pytest.skip("two consumer threads per site need vector-aligned spin components (fp32: even d_R)")
     psi = li.gaussian_spinor(742, V, d)
     got = prob.dirac(m0, psi)
     assert rel_l2(got, oracle.dirac(dims, BC_T, R, m0, psi)) <= TOL[prec]
