@@ -398,7 +398,88 @@ def unregister_host(torch, arr):
 
 
 def run_sharded(args, hr, world, rank, local):
-    raise SystemExit("bench.py --sharded: not built yet")
+    """--sharded: ONE lattice cut into t-slabs over the ranks: every rank owns T/N
+    time-slices of the seeded global fields; a step is the link map on the slab + two distributed Dphi_eo -- half-spinor
+    faces projected and written straight into the neighbours' receive buffers by the pack kernel (CUDA IPC peer memory
+    over NVLink; --sharded-nccl: ncclSend/Recv on a side stream), interior launch meanwhile, apply after one fence.
+    value = contract bytes of the GLOBAL lattice / max-over-ranks time: "scaling": "strong"."""
+    import torch
+    import torch.distributed as dist
+    import lattice_inputs as li
+    from paper_2405_19294_b200 import halo
+
+    cfg, prec = CONFIGS[args.config], args.prec
+    P = hr.PREC_NAMES[prec]
+    bm = byte_model(cfg, prec)
+    plan = halo.slab_plan(rank, world, cfg["dims"][0])
+    ldims = (plan["T_local"],) + tuple(cfg["dims"][1:])
+    vl = li.volume(ldims)
+    sl, ss = cfg["seeds"]
+    gen = li.haar_links if cfg["kind"] == "haar" else (lambda s, N, dm, **kw: li.near_identity_links(s, N, dm, 0.3, **kw))
+    U = gen(sl, cfg["N"], ldims, first_site=rank * vl, nsites=vl)
+    psi = [li.gaussian_spinor(ss + 10 * p, vl // 2, bm["d"], first_site=rank * (vl // 2)) for p in (0, 1)]
+    lat = hr.Lattice(ldims, BC, cfg["N"], cfg["rep"], device=local)
+    fund, links = lat.gauge(False, P), lat.gauge(True, P)
+    lat.import_gauge(fund, U)
+    lat.represent_links(links, fund)
+    inp = [lat.spinor(P) for _ in range(NSET)]
+    out = [lat.spinor(P) for _ in range(NSET)]
+    for k in range(NSET):
+        lat.import_spinor(inp[k], P, psi[k & 1], 1 - (k & 1))
+    slab = (halo.SlabDphi if args.sharded_nccl else halo.PeerSlabDphi)(lat, P, plan)
+
+    def step(k):
+        lat.represent_links(links, fund)
+        slab.dphi_eo(out[(2 * k) % NSET], inp[(2 * k) % NSET], links, 0)
+        slab.dphi_eo(out[(2 * k + 1) % NSET], inp[(2 * k + 1) % NSET], links, 1)
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for k in range(args.warmup):
+        step(k)
+    sync_all()
+    n0 = hr.hr_launch_count()
+    with ClockSampler(local) as clk:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for k in range(args.steps):
+            step(k)
+        e1.record()
+        sync_all()
+    launches = hr.hr_launch_count() - n0
+    ms_step = max_over_ranks(e0.elapsed_time(e1), world, "cuda") / args.steps
+    # the same slab WITHOUT the decomposition (periodic in t inside the rank): what the faces cost
+    med, _, _ = bracket_protocol(torch, lambda k: lat.dphi_eo(out[k % NSET], inp[k % NSET], links, k & 1),
+                                 torch.empty(512 << 20, dtype=torch.uint8, device="cuda"), max(20, args.steps), brackets=3)
+    dmed, _, _ = bracket_protocol(torch, lambda k: slab.dphi_eo(out[k % NSET], inp[k % NSET], links, k & 1),
+                                  torch.empty(1, dtype=torch.uint8, device="cuda"), max(20, args.steps), brackets=3)
+    med, dmed = max_over_ranks(med, world, "cuda"), max_over_ranks(dmed, world, "cuda")
+    if rank == 0:
+        step_bytes = 4 * bm["V"] * bm["represent_bytes_per_link"] + bm["V"] * bm["dphi_bytes_per_site"]
+        comp = 4 * bm["V"] * bm["represent_bytes_per_link"] + bm["V"] * bm["compulsory_bytes_per_site"]
+        peak, peak_src = measured_peak()
+        print(json.dumps({
+            "metric": METRIC, "value": step_bytes / (ms_step * 1e-3) / 1e9, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": prec, "data": "synthetic", "config": config_keys(cfg, world, sharded=True),
+            "value_compulsory": comp / (ms_step * 1e-3) / 1e9, "clocks": clk.summary(), "gpu_launches": int(launches),
+            "e2e": None,
+            "sharded": {"exchange": "nccl send/recv on a side stream" if args.sharded_nccl else "peer stores from the pack kernel (CUDA IPC)",
+                        "local_dims": list(ldims), "halo_bytes_per_message": hr.hr_halo_bytes(lat.ctx, P),
+                        "dphi_eo_ms_distributed": dmed, "dphi_eo_ms_same_slab_undistributed": med,
+                        "decomposition_overhead": dmed / med - 1.0},
+            "roofline": {"bound": "hbm", "kernel": "interior Dphi launch + face pack / apply", "achieved": world * (vl // 2) * bm["compulsory_bytes_per_site"] / (dmed * 1e-3) / 1e9,
+                         "peak": peak * world, "unit": "GB/s", "frac": (vl // 2) * bm["compulsory_bytes_per_site"] / (dmed * 1e-3) / 1e9 / peak,
+                         "traffic": None, "peak_source": peak_src + " x n_gpus"}}))
+    if hasattr(slab, "close"):
+        slab.close()
+    lat.close()
+    if world > 1:
+        dist.destroy_process_group()
 
 
 def run_ours(args):
@@ -615,6 +696,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--sharded", action="store_true", help="N > 1: one lattice on t-slabs instead of replicas")
+    ap.add_argument("--sharded-nccl", action="store_true", help="--sharded with NCCL send/recv instead of peer stores")
     ap.add_argument("--sample-sites", type=int, default=1 << 18, help="--impl reference: output sites per parity and step")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -5,6 +5,7 @@ DESIGN.md and profiles/.  They import bench.py's configs, byte model and input r
     python bench_sweeps.py volume  [--reps 200] [--sizes 8,12,...]      Dphi_eo and a copy against the lattice volume
     python bench_sweeps.py large_n [--reps 50] [--variants ...]         Dphi_eo against d_R at constant memory moved (Fig. 6)
     python bench_sweeps.py solver  [--config 2] [--prec f64] [--reps 50] spinor linear algebra, Dhat, solvers (Fig. 7)
+    python bench_sweeps.py variants --cases '[...]' --sweeps '[...]'     kernel variants / tunings under sustained clocks
 """
 from __future__ import annotations
 
@@ -83,7 +84,7 @@ def volume(argv):
 # (N, rep, dims): compulsory bytes 1.6-1.9 GB in fp64 for every row
 CASES = [(2, "fund", (128, 32, 32, 32)), (3, "fund", (64, 32, 32, 32)), (4, "fund", (40, 32, 32, 32)),
          (3, "sym", (48, 24, 24, 24)), (3, "adj", (48, 24, 24, 24)), (4, "sym", (56, 16, 16, 16)), (4, "adj", (48, 16, 16, 16))]
-NAMES = ["site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour"]
+NAMES = ["site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour", "bulk", "bulk2", "bulkx", "bulkx2"]
 
 
 def large_n(argv):
@@ -363,7 +364,115 @@ def solver(argv):
 
 
 
-SWEEPS = {"volume": volume, "large_n": large_n, "solver": solver}
+
+def variants(argv):
+    """Dphi_eo under SUSTAINED clocks for every kernel variant / tuning asked for (the sweep behind DESIGN.md's default
+    table and profiles/r2_staging.md).  A B200 running this operator back to back sits at its 1 kW power cap with the
+    SM clock near 1.4-1.7 GHz; a kernel timed in a short burst runs at 1.97 GHz and reads 5-10 % faster.  Protocol per
+    point: 8 launches (burst), then half a bracket of warm-up launches and a bracket of `--secs` seconds timed with CUDA
+    events while NVML samples the SM clock.
+
+        python bench_sweeps.py variants --cases '[[5,"f64","repr"],[4,"f32","fund"],[2,"f64","rows",[64,32,32,32]]]' \
+               --sweeps '[{},{"variant":7},{"variant":8,"bulk_ctas":2}]' [--secs 0.5]
+
+    case = [bench.py config, precision, link source repr|fund|rows, optional dims]; a sweep entry sets hr_ctx_set_tuning keys
+    (variant, block, xblock, bulk_rows, bulk_stages, bulk_ctas, bulk_strip; {} = library defaults).  Inputs: one t-pair of the
+    config's seeded fields repeated along t (values do not influence timing).  One JSON line per point."""
+    import statistics
+    import time
+    import numpy as np
+    import pynvml
+    import torch
+    import bench as B
+    import lattice_inputs as li
+    import paper_2405_19294_b200 as hr
+
+    ap = argparse.ArgumentParser(prog="bench_sweeps.py variants")
+    ap.add_argument("--cases", required=True)
+    ap.add_argument("--sweeps", default="[{}]")
+    ap.add_argument("--secs", type=float, default=0.5)
+    args = ap.parse_args(argv)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench_sweeps variants: no CUDA device; the product path has no CPU fallback")
+    pynvml.nvmlInit()
+    H = pynvml.nvmlDeviceGetHandleByIndex(0)
+    peak, _ = B.measured_peak()
+    keys = ("variant", "block", "xblock", "bulk_rows", "bulk_stages", "bulk_ctas", "bulk_strip")
+
+    def timed(fn):
+        for k in range(3):
+            fn(k)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for k in range(8):
+            fn(k)
+        e1.record()
+        torch.cuda.synchronize()
+        burst = e0.elapsed_time(e1) / 8
+        n = max(10, int(args.secs * 1e3 / burst))
+        for k in range(max(5, n // 2)):
+            fn(k)
+        e0.record()
+        for k in range(n):
+            fn(k)
+        e1.record()
+        mhz = []
+        while not e1.query():
+            mhz.append(pynvml.nvmlDeviceGetClockInfo(H, pynvml.NVML_CLOCK_SM))
+            time.sleep(0.01)
+        torch.cuda.synchronize()
+        return burst, e0.elapsed_time(e1) / n, (statistics.median(mhz) if mhz else None)
+
+    for case in json.loads(args.cases):
+        cid, prec, src = case[:3]
+        cfg = dict(B.CONFIGS[cid])
+        if len(case) > 3:
+            cfg["dims"] = tuple(case[3])
+        P = hr.PREC_NAMES[prec]
+        dims = cfg["dims"]
+        vh = li.volume(dims) // 2
+        U, psi = B.make_fields(dict(cfg, dims=(2,) + tuple(dims[1:])))
+        U = np.concatenate([U] * (dims[0] // 2))
+        psi = [np.concatenate([p] * (dims[0] // 2)) for p in psi]
+        lat = hr.Lattice(dims, B.BC, cfg["N"], cfg["rep"])
+        fund, links = lat.gauge(False, P), lat.gauge(True, P)
+        lat.import_gauge(fund, U)
+        lat.represent_links(links, fund)
+        if src == "rows":
+            L = lat.gauge(2, P)
+            lat.compress_links(L, fund)
+        else:
+            L = fund if src == "fund" else links
+        inp = [lat.spinor(P) for _ in range(4)]
+        out = [lat.spinor(P) for _ in range(4)]
+        for k in range(4):
+            lat.import_spinor(inp[k], P, psi[k & 1], 1 - (k & 1))
+        st = lat.stream()
+        bm = B.byte_model(cfg, prec)
+        w = 8 if prec == "f64" else 4
+        lb = {"repr": bm["L"], "fund": bm["F"], "rows": 2 * cfg["N"] * (cfg["N"] - 1) * w}[src]
+        need = vh * (8 * lb + 2 * bm["S"])
+        for sw in json.loads(args.sweeps):
+            try:
+                for k in keys:
+                    lat.set_tuning(k, sw.get(k, -1 if k == "variant" else 0))
+                hr.hr_dphi_eo(out[0], inp[0], L, 0, st)
+                torch.cuda.synchronize()
+            except hr.HrError as exc:
+                print(json.dumps({"workload": cfg["name"], "dims": list(dims), "dtype": prec, "links": src, **sw, "unavailable": str(exc)[:90]}), flush=True)
+                continue
+            burst, ms, mhz = timed(lambda k: hr.hr_dphi_eo(out[k % 4], inp[k % 4], L, k & 1, st))
+            print(json.dumps({"workload": cfg["name"], "dims": list(dims), "dtype": prec, "links": src, **sw,
+                              "burst_ms": round(burst, 4), "burst_frac": round(need / burst / 1e6 / peak, 3),
+                              "sustained_ms": round(ms, 4), "sustained_frac": round(need / ms / 1e6 / peak, 3), "sm_mhz": mhz,
+                              "needed_mb": round(need / 1e6, 1)}), flush=True)
+        lat.close()
+        del inp, out, lat
+        torch.cuda.empty_cache()
+
+
+SWEEPS = {"volume": volume, "large_n": large_n, "solver": solver, "variants": variants}
 
 if __name__ == "__main__":
     if len(sys.argv) < 2 or sys.argv[1] not in SWEEPS:

@@ -215,6 +215,11 @@ hr_status hr_dhat(double m0, int g5, void *out_e, const void *in_e, void *tmp_o,
  * hr_dirac_solve solves the FULL system D x = b, D = (4+m0) + Dphi, fields [even half | odd half], through
  * the preconditioned one (reading C24):  Dhat x_e = (4+m0) b_e - Dphi_eo b_o ;  x_o = (b_o - Dphi_oe x_e)/(4+m0).
  * x must not alias b.  Not converged within maxiter is not an error: check iters / rel_res2.
+ * WHICH residual: rel_res2 of hr_dirac_solve is that of the system the iteration runs on -- the normal equations of the
+ * preconditioned system, |Dhat^dag (rhs_e - Dhat x_e)|^2 / |Dhat^dag rhs_e|^2 --, of hr_dirac_solve_bicgstab and
+ * hr_dirac_clover_solve that of the preconditioned system, |rhs_e - Dhat x_e|^2 / |rhs_e|^2; neither is |b - D x|^2 / |b|^2
+ * of the full system (the odd half is solved exactly given x_e, so the full residual lives on the even sites and equals
+ * |rhs_e - Dhat x_e| / (4+m0) there).  A caller who needs the full-system number applies hr_dirac to x once.
  */
 size_t hr_cg_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter);
 /*
@@ -228,6 +233,28 @@ hr_status hr_bicgstab_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, c
                            int maxiter, void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
 hr_status hr_cg_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links, double tol, int maxiter,
                      void *workspace, int *iters, double *rel_res2, double *hist, void *stream);
+/*
+ * hr_cg_dhat_dist -- the CG of hr_cg_dhat (reading C21: textbook CG on Dhat^dagger Dhat x = Dhat^dagger b, x0 = 0, stop at
+ * the first k with |r_k|^2 <= tol^2 |rhs|^2 or k = maxiter) on a lattice that is DISTRIBUTED over several ranks
+ * (DESIGN.md section 13).  The library owns every step of the algorithm -- the vector updates are its
+ * kernels on the local half fields, the scalar recurrences (alpha = rr / <p, A p>, beta = rr' / rr, the stopping test)
+ * run here -- and calls back for the two things only the caller can do:
+ *   dphi(user, out, in, parity):   the distributed Dphi_eo on the caller's decomposition (pack / exchange / interior /
+ *                                  apply, e.g. halo.py), enqueued on `stream`; out: parity-`parity` local half field.
+ *                                  Returns 0 on success.
+ *   allsum(user, vals, n):         sum of n host doubles over all ranks, in place (an all-reduce); returns 0 on success.
+ *                                  May be NULL on a single rank.
+ * x_e, b_e: local even half fields, precision `prec`.  workspace: hr_cg_dist_workspace_bytes(ctx, prec) bytes of device
+ * memory, 256-byte aligned.  iters / hist as hr_cg_dhat (hist: HOST array of maxiter+1 doubles or NULL).  Host-driven: two
+ * synchronisations of `stream` and two all-reduces per iteration (the sums must cross the ranks anyway).
+ * Errors: HR_EINVAL (NULL / misaligned / aliased arguments), HR_ECUDA (a callback failed or a CUDA call did).
+ */
+typedef int (*hr_dphi_fn)(void *user, void *out, const void *in, int parity);
+typedef int (*hr_allsum_fn)(void *user, double *vals, int n);
+size_t hr_cg_dist_workspace_bytes(const hr_ctx *ctx, hr_prec prec);
+hr_status hr_cg_dhat_dist(hr_ctx *ctx, hr_prec prec, double m0, void *x_e, const void *b_e, double tol, int maxiter,
+                          void *workspace, hr_dphi_fn dphi, hr_allsum_fn allsum, void *user, int *iters, double *hist,
+                          void *stream);
 /*
  * hr_qmr_dhat -- the gamma5-QMR ("QMR gamma_5 inverters"; reading C33): quasi-minimal residual method without
  * look-ahead on Dhat ITSELF, built on the Lanczos process in the indefinite inner product (x, y)_J = <x, gamma5 y>, in which
@@ -250,7 +277,9 @@ hr_status hr_dirac_solve(hr_ctx *ctx, double m0, void *x_full, const void *b_ful
  * the normalised residual) and the TRUE residual r = b - Dhat x recomputed in fp64 (links64) after every inner solve; stops
  * when |r|^2 <= tol^2 |b|^2 (fp64, true residual) or after maxiter inner iterations in total.  x_e, b_e: fp64 half
  * fields; workspace of hr_mixed_workspace_bytes(ctx, maxiter), 256-byte aligned.  iters: inner iterations in total,
- * outer_steps: number of defect corrections, rel_res2: true |r|^2 / |b|^2.  Synchronises once per outer step.
+ * outer_steps: number of defect corrections, rel_res2: true |r|^2 / |b|^2 of the x that is returned.  Synchronises once per
+ * outer step.  Also ends after 100 outer steps or when an inner solve makes no iteration; NOT converged is not an error:
+ * the caller compares rel_res2 with tol^2 (as for hr_cg_dhat: check iters / rel_res2).
  */
 size_t hr_mixed_workspace_bytes(const hr_ctx *ctx, int maxiter);
 hr_status hr_bicgstab_dhat_mixed(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const hr_gauge *links64,

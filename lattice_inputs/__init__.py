@@ -75,21 +75,22 @@ def _sun(seed, stream, kind, eps, N, first, count, out=None):
     return out
 
 
-def haar_links(seed: int, N: int, dims, out=None) -> np.ndarray:
-    """Haar-random SU(N) fundamental links, canonical [V][4][N][N] complex128."""
-    V = volume(dims)
+def haar_links(seed: int, N: int, dims, out=None, first_site: int = 0, nsites=None) -> np.ndarray:
+    """Haar-random SU(N) fundamental links, canonical [V][4][N][N] complex128 (or the nsites sites from first_site on of
+    that field: the generator is counter-based, any slice is reproducible on its own)."""
+    V = volume(dims) if nsites is None else int(nsites)
     if out is None:
         out = np.empty((V, 4, N, N), dtype=np.complex128)
-    _sun(seed, STREAM_LINKS, 0, 0.0, N, 0, 4 * V, out)
+    _sun(seed, STREAM_LINKS, 0, 0.0, N, 4 * first_site, 4 * V, out)
     return out
 
 
-def near_identity_links(seed: int, N: int, dims, eps: float = 0.3, out=None) -> np.ndarray:
-    """U = exp(i eps H), H Gaussian Hermitian traceless; canonical [V][4][N][N] complex128."""
-    V = volume(dims)
+def near_identity_links(seed: int, N: int, dims, eps: float = 0.3, out=None, first_site: int = 0, nsites=None) -> np.ndarray:
+    """U = exp(i eps H), H Gaussian Hermitian traceless; canonical [V][4][N][N] complex128 (or a slice, as haar_links)."""
+    V = volume(dims) if nsites is None else int(nsites)
     if out is None:
         out = np.empty((V, 4, N, N), dtype=np.complex128)
-    _sun(seed, STREAM_LINKS, 1, eps, N, 0, 4 * V, out)
+    _sun(seed, STREAM_LINKS, 1, eps, N, 4 * first_site, 4 * V, out)
     return out
 
 

@@ -80,6 +80,8 @@ _SIGNATURES = {
     "hr_dhat": (_ci, [_cd, _ci, _vp, _vp, _vp, _vp, _vp]),
     "hr_cg_workspace_bytes": (_sz, [_vp, _ci, _ci]),
     "hr_cg_dhat": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp, _vp]),
+    "hr_cg_dist_workspace_bytes": (_sz, [_vp, _ci]),
+    "hr_cg_dhat_dist": (_ci, [_vp, _ci, _cd, _vp, _vp, _cd, _ci, _vp, _vp, _vp, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp]),
     "hr_bicgstab_workspace_bytes": (_sz, [_vp, _ci, _ci]),
     "hr_bicgstab_dhat": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp, _vp]),
     "hr_qmr_workspace_bytes": (_sz, [_vp, _ci]),
@@ -311,6 +313,50 @@ def hr_cg_dhat(ctx: int, m0: float, x_e, b_e, links: int, tol: float, maxiter: i
     _check(_lib.hr_cg_dhat(ctx, float(m0), _ptr(x_e), _ptr(b_e), links, float(tol), int(maxiter), _ptr(workspace),
                            ctypes.byref(it), ctypes.byref(res), _ptr(hist), stream))
     return it.value, res.value, (hist[:it.value + 1] if want_hist else None)
+
+
+_DPHI_FN = ctypes.CFUNCTYPE(_ci, _vp, _vp, _vp, _ci)
+_ALLSUM_FN = ctypes.CFUNCTYPE(_ci, _vp, ctypes.POINTER(_cd), _ci)
+
+
+def hr_cg_dist_workspace_bytes(ctx: int, prec: int) -> int:
+    return int(_lib.hr_cg_dist_workspace_bytes(ctx, prec))
+
+
+def hr_cg_dhat_dist(ctx: int, prec: int, m0: float, x_e, b_e, tol: float, maxiter: int, workspace, dphi, allsum=None, stream: int = 0):
+    """CG on a distributed lattice, every step in libhr; `dphi(out_ptr, in_ptr, parity)` runs the caller's distributed
+    Dphi_eo on `stream`, `allsum(list of floats) -> list of floats` sums over the ranks (None: one rank).
+    Returns (iterations, [|r_k|^2 / |rhs|^2])."""
+    err = []
+
+    def _dphi(user, out, inp, parity):
+        try:
+            dphi(int(out), int(inp), int(parity))
+            return 0
+        except Exception as exc:  # an exception must not cross the C frames
+            err.append(exc)
+            return 1
+
+    def _allsum(user, vals, n):
+        try:
+            res = allsum([vals[i] for i in range(n)])
+            for i in range(n):
+                vals[i] = res[i]
+            return 0
+        except Exception as exc:
+            err.append(exc)
+            return 1
+
+    cb_d = _DPHI_FN(_dphi)
+    cb_a = _ALLSUM_FN(_allsum) if allsum is not None else None
+    iters = _ci(0)
+    hist = (_cd * (maxiter + 1))()
+    rc = _lib.hr_cg_dhat_dist(ctx, prec, m0, _ptr(x_e), _ptr(b_e), tol, maxiter, _ptr(workspace), ctypes.cast(cb_d, _vp),
+                              ctypes.cast(cb_a, _vp) if cb_a is not None else None, None, ctypes.byref(iters), hist, stream)
+    if err:
+        raise err[0]
+    _check(rc)
+    return iters.value, [hist[i] for i in range(iters.value + 1)]
 
 
 def hr_bicgstab_workspace_bytes(ctx: int, prec: int, maxiter: int) -> int:

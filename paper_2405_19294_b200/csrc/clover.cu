@@ -544,7 +544,12 @@ template <typename Real, int D, bool RL>
 static hr_status build_rows(const hr_ctx *c, const CloverArgs &a, cudaStream_t st)
 {
     const long total = c->V;
-    const long chunk = total < (1L << 19) ? total : (1L << 19);
+    // chunk sized by BYTES: 256 MiB of scratch at most (2^19 sites of d_R = 15 in fp64 were 11 GB next to the solver's
+    // workspaces), so that the hand-off from clover_q_kernel to clover_pack_kernel mostly stays in the 126 MB L2
+    const size_t per_site = (size_t)6 * 2 * D * D * sizeof(Real);
+    long chunk = (long)(((size_t)256 << 20) / per_site) / 32 * 32;
+    if (chunk < 32) chunk = 32;
+    if (chunk > total) chunk = total;
     Real *scratch = nullptr;
     cudaError_t e = cudaMallocAsync((void **)&scratch, (size_t)chunk * 6 * 2 * D * D * sizeof(Real), st);
     if (e != cudaSuccess) { cudaGetLastError(); set_error("clover build: scratch allocation failed: %s", cudaGetErrorString(e)); return HR_ENOMEM; }

@@ -42,6 +42,13 @@ static constexpr bool kExperiments = false;
 #endif
 
 // registers: __launch_bounds__(MAXT, MINB) caps them at 65536 / (MAXT*MINB)
+// LIVE in (96, 128] (the fp32 d_R = 3 kernels) at a 128-register cap: ptxas parks the upper halves of two or three
+// loop-invariant 64-bit addresses in local memory (2-3 STL at the top of the kernel, 2-3 LDL before the epilogue: 8-28
+// bytes per thread, L1-resident).  It does the same at a 168-register cap (checked: -DHR_MINB_128=3 gives "168 registers,
+// 8 bytes spill" -- the scheduler hoists loads until the budget is full), so the cap stays where the time is best.
+#ifndef HR_MINB_128
+#define HR_MINB_128 4
+#endif
 template <typename Real, int D, int LK, int KSPLIT> struct Tune {
     static constexpr int LNREAL = LinkGeom<LK, D>::NREAL;
     // live values of a thread, in 32-bit registers (accumulators + one spinor/half + one link)
@@ -52,7 +59,7 @@ template <typename Real, int D, int LK, int KSPLIT> struct Tune {
     // real-link d_R = 3 kernel (LIVE = 154) loses 3 % at a 168-register cap (it spills), hence the 150 threshold
     static constexpr int MINB = ((LK == LK_SYM_OTF || LK == LK_ASYM_OTF) && sizeof(Real) == 4 && KSPLIT == 1) ? 4 :
                                 (LK == LK_ADJ2_ROWS && sizeof(Real) == 8 && KSPLIT == 1) ? 2 :   // as the real-link kernel it expands to
-                                LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? 4 : LIVE <= 150 ? 3 : LIVE <= 255 ? 2 : 1;
+                                LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? HR_MINB_128 : LIVE <= 150 ? 3 : LIVE <= 255 ? 2 : 1;
 };
 
 template <typename Real, int D, int LK, int KSPLIT, bool MASS, bool RED, int LHINT, int SHINT, int STHINT, int CLV = 0>

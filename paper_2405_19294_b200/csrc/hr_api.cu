@@ -109,28 +109,51 @@ static hr_status transfer(const hr_ctx *c, FieldKind kind, bool import, int nrea
     };
     if (dev) return run(canon, 0, nsites);
 
-    // host canonical array: stage through device memory in chunks (set-up path)
-    long chunk = (long)(kStageBytes / site_bytes);
-    if (chunk < 1) chunk = 1;
-    if (chunk > nsites) chunk = nsites;
-    void *stage = nullptr;
-    HR_CUDA(cudaMalloc(&stage, (size_t)chunk * site_bytes));
-    hr_status out = HR_OK;
-    for (long first = 0; first < nsites && out == HR_OK; first += chunk) {
-        const long n = (nsites - first < chunk) ? nsites - first : chunk;
-        char *h = (char *)canon + (size_t)first * site_bytes;
-        cudaError_t e = cudaSuccess;
-        if (import) {
-            e = cudaMemcpyAsync(stage, h, (size_t)n * site_bytes, cudaMemcpyHostToDevice, st);
-            if (e == cudaSuccess) out = run(stage, first, n);
-        } else {
-            out = run(stage, first, n);
-            if (out == HR_OK) e = cudaMemcpyAsync(h, stage, (size_t)n * site_bytes, cudaMemcpyDeviceToHost, st);
+    // host canonical array: staged through two device buffers owned by the context; the host<->device copy of one chunk
+    // (copy stream) overlaps the pack / unpack kernel of the other (caller's stream); one synchronisation at the end
+    // (the host array must be reusable / valid when the call returns)
+    hr_ctx *mc = const_cast<hr_ctx *>(c);
+    if (!mc->stage[0]) {
+        HR_CUDA(cudaMalloc(&mc->stage[0], kStageBytes));
+        cudaError_t e = cudaMalloc(&mc->stage[1], kStageBytes);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&mc->copy_stream, cudaStreamNonBlocking);
+        for (int b = 0; b < 2 && e == cudaSuccess; ++b) {
+            e = cudaEventCreateWithFlags(&mc->ev_copied[b], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&mc->ev_used[b], cudaEventDisableTiming);
         }
-        if (e == cudaSuccess && out == HR_OK) e = cudaStreamSynchronize(st);
-        if (e != cudaSuccess) out = cuda_fail("staged canonical copy", e);
+        if (e != cudaSuccess) { cudaFree(mc->stage[0]); cudaFree(mc->stage[1]); mc->stage[0] = mc->stage[1] = nullptr; return cuda_fail("staging buffers", e); }
+        mc->stage_bytes = kStageBytes;
     }
-    cudaFree(stage);
+    long chunk = (long)(kStageBytes / site_bytes);
+    if (chunk < 1) { set_error("canonical record of %zu bytes exceeds the staging buffer", site_bytes); return HR_EUNSUPPORTED; }
+    if (chunk > nsites) chunk = nsites;
+    cudaStream_t cs = mc->copy_stream;
+    hr_status out = HR_OK;
+    cudaError_t e = cudaSuccess;
+    long k = 0;
+    for (long first = 0; first < nsites && out == HR_OK && e == cudaSuccess; first += chunk, ++k) {
+        const long n = (nsites - first < chunk) ? nsites - first : chunk;
+        const int b = (int)(k & 1);
+        char *h = (char *)canon + (size_t)first * site_bytes;
+        if (import) {
+            if (k >= 2) e = cudaStreamWaitEvent(cs, mc->ev_used[b], 0);                 // the pack of chunk k-2 has read stage[b]
+            if (e == cudaSuccess) e = cudaMemcpyAsync(mc->stage[b], h, (size_t)n * site_bytes, cudaMemcpyHostToDevice, cs);
+            if (e == cudaSuccess) e = cudaEventRecord(mc->ev_copied[b], cs);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(st, mc->ev_copied[b], 0);
+            if (e == cudaSuccess) out = run(mc->stage[b], first, n);
+            if (e == cudaSuccess && out == HR_OK) e = cudaEventRecord(mc->ev_used[b], st);
+        } else {
+            if (k >= 2) e = cudaStreamWaitEvent(st, mc->ev_copied[b], 0);               // the copy of chunk k-2 has left stage[b]
+            if (e == cudaSuccess) out = run(mc->stage[b], first, n);
+            if (e == cudaSuccess && out == HR_OK) e = cudaEventRecord(mc->ev_used[b], st);
+            if (e == cudaSuccess && out == HR_OK) e = cudaStreamWaitEvent(cs, mc->ev_used[b], 0);
+            if (e == cudaSuccess && out == HR_OK) e = cudaMemcpyAsync(h, mc->stage[b], (size_t)n * site_bytes, cudaMemcpyDeviceToHost, cs);
+            if (e == cudaSuccess && out == HR_OK) e = cudaEventRecord(mc->ev_copied[b], cs);
+        }
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(cs);
+    if (e != cudaSuccess) { cudaGetLastError(); if (out == HR_OK) out = cuda_fail("staged canonical copy", e); }
     return out;
 }
 
@@ -178,6 +201,9 @@ hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N,
     c->xblock = 0;
     c->cg_graph = 1;
     c->bulk_rows = c->bulk_stages = c->bulk_ctas = c->bulk_strip = 0;
+    c->stage[0] = c->stage[1] = nullptr;
+    c->stage_bytes = 0;
+    c->copy_stream = nullptr;
     c->ws_in = c->ws_out = c->ws_stage = nullptr;
     c->ws_spinor_bytes = c->ws_stage_bytes = 0;
     c->ws_prec = -1;
@@ -190,8 +216,14 @@ hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N,
 void hr_ctx_destroy(hr_ctx *ctx)
 {
     if (!ctx) return;
-    if (ctx->ws_in || ctx->ws_out || ctx->ws_stage || ctx->red_scratch) {
+    if (ctx->ws_in || ctx->ws_out || ctx->ws_stage || ctx->red_scratch || ctx->stage[0]) {
         if (cudaSetDevice(ctx->device) == cudaSuccess) {
+            if (ctx->stage[0]) {
+                cudaFree(ctx->stage[0]);
+                cudaFree(ctx->stage[1]);
+                for (int b = 0; b < 2; ++b) { cudaEventDestroy(ctx->ev_copied[b]); cudaEventDestroy(ctx->ev_used[b]); }
+                cudaStreamDestroy(ctx->copy_stream);
+            }
             cudaFree(ctx->ws_in);
             cudaFree(ctx->ws_out);
             cudaFree(ctx->ws_stage);
@@ -447,28 +479,21 @@ hr_status hr_dphi_eo_host(hr_ctx *ctx, void *out_canon, const void *in_canon, hr
     if (rc != HR_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t sb = hr_spinor_bytes(ctx, links->prec);
-    const size_t cb = hr_spinor_bytes(ctx, canon_prec);
-    if (ctx->ws_prec != (int)links->prec || ctx->ws_spinor_bytes != sb || ctx->ws_stage_bytes < cb) {
-        cudaFree(ctx->ws_in); cudaFree(ctx->ws_out); cudaFree(ctx->ws_stage);
-        ctx->ws_in = ctx->ws_out = ctx->ws_stage = nullptr;
+    if (ctx->ws_prec != (int)links->prec || ctx->ws_spinor_bytes != sb) {
+        cudaFree(ctx->ws_in); cudaFree(ctx->ws_out);
+        ctx->ws_in = ctx->ws_out = nullptr;
         ctx->ws_prec = -1;
         HR_CUDA(cudaMalloc(&ctx->ws_in, sb));
         HR_CUDA(cudaMalloc(&ctx->ws_out, sb));
-        HR_CUDA(cudaMalloc(&ctx->ws_stage, cb));
         ctx->ws_spinor_bytes = sb;
-        ctx->ws_stage_bytes = cb;
         ctx->ws_prec = (int)links->prec;
     }
-    HR_CUDA(cudaMemcpyAsync(ctx->ws_stage, in_canon, cb, cudaMemcpyHostToDevice, st));
-    rc = launch_pack_spinor(ctx, ctx->ws_in, links->prec, ctx->ws_stage, canon_prec, 0, ctx->Vh, st);
+    // chunked through the context's two staging buffers: copy of chunk k+1 || pack of chunk k, unpack of chunk k || copy of k-1
+    rc = transfer(ctx, FIELD_SPINOR, true, 8 * ctx->d, ctx->ws_in, links->prec, const_cast<void *>(in_canon), canon_prec, st);
     if (rc != HR_OK) return rc;
     rc = hr_dphi_eo(ctx->ws_out, ctx->ws_in, links, parity, stream);
     if (rc != HR_OK) return rc;
-    rc = launch_unpack_spinor(ctx, ctx->ws_out, links->prec, ctx->ws_stage, canon_prec, 0, ctx->Vh, st);
-    if (rc != HR_OK) return rc;
-    HR_CUDA(cudaMemcpyAsync(out_canon, ctx->ws_stage, cb, cudaMemcpyDeviceToHost, st));
-    HR_CUDA(cudaStreamSynchronize(st));
-    return HR_OK;
+    return transfer(ctx, FIELD_SPINOR, false, 8 * ctx->d, ctx->ws_out, links->prec, out_canon, canon_prec, st);
 }
 
 hr_status hr_ctx_set_tuning(hr_ctx *ctx, const char *key, int value)

@@ -263,6 +263,91 @@ hr_status hr_cg_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const h
     return cg_run(ctx, m0, x_e, links, tol, maxiter, ws, iters, rel_res2, hist, st);
 }
 
+size_t hr_cg_dist_workspace_bytes(const hr_ctx *ctx, hr_prec prec)
+{
+    if (!ctx || !valid_prec(prec)) return 0;
+    const size_t sb = ((size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec) + 255) & ~(size_t)255;
+    return 6 * sb;   // r, p, Ap, w, tmp_o, tmp_e
+}
+
+// CG on Dhat^dagger Dhat = (gamma5 Dhat)^2 with the operator's two Dphi_eo and the cross-rank sums supplied by the caller;
+// everything else -- vector updates, scalar recurrences, stopping test -- is done here (oracle/solver.py::cg_dhat, step by step)
+hr_status hr_cg_dhat_dist(hr_ctx *ctx, hr_prec prec, double m0, void *x_e, const void *b_e, double tol, int maxiter,
+                          void *workspace, hr_dphi_fn dphi, hr_allsum_fn allsum, void *user, int *iters, double *hist,
+                          void *stream)
+{
+    if (!ctx || !x_e || !b_e || !workspace || !dphi || !valid_prec(prec) || maxiter < 0 || !(tol >= 0)) {
+        set_error("hr_cg_dhat_dist: bad argument");
+        return HR_EINVAL;
+    }
+    if (x_e == b_e || !aligned16(x_e) || !aligned16(b_e) || ((uintptr_t)workspace & 255)) {
+        set_error("hr_cg_dhat_dist: x aliases b, or a buffer is misaligned (fields 16, workspace 256 bytes)");
+        return HR_EINVAL;
+    }
+    hr_status rc = use_device(ctx);
+    if (rc != HR_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    RedScratch rs;
+    rc = get_red_scratch(ctx, &rs, st);
+    if (rc != HR_OK) return rc;
+    const size_t sb = ((size_t)ctx->Vh * 8 * ctx->d * prec_bytes(prec) + 255) & ~(size_t)255;
+    char *ws = (char *)workspace;
+    void *r = ws, *p = ws + sb, *ap = ws + 2 * sb, *w = ws + 3 * sb, *tmp_o = ws + 4 * sb, *tmp_e = ws + 5 * sb;
+    const double m = 4.0 + m0, one[2] = { 1, 0 }, zero[2] = { 0, 0 }, mm[2] = { m * m, 0 }, minus[2] = { -1, 0 };
+
+    auto cb_fail = [&](const char *what) { set_error("hr_cg_dhat_dist: the %s callback failed", what); return HR_ECUDA; };
+    // out = gamma5 Dhat in,  Dhat = (4+m0)^2 - Dphi_eo Dphi_oe
+    auto g5dhat = [&](void *out, const void *in) -> hr_status {
+        if (dphi(user, tmp_o, in, 1) != 0) return cb_fail("dphi");
+        if (dphi(user, tmp_e, tmp_o, 0) != 0) return cb_fail("dphi");
+        hr_status q = launch_lincomb(ctx, prec, tmp_e, mm, 0, in, minus, tmp_e, st);
+        if (q != HR_OK) return q;
+        return launch_lincomb(ctx, prec, out, one, 1, tmp_e, zero, nullptr, st);
+    };
+    // global sum over the ranks of the local <a, b> (real part) -- |a|^2 when a == b
+    auto gdot = [&](const void *a, const void *b, double *out) -> hr_status {
+        hr_status q = launch_dot(ctx, prec, a, b, rs, rs.result, st);
+        if (q != HR_OK) return q;
+        double v[2];
+        q = deliver(v, rs.result, 2, st);
+        if (q != HR_OK) return q;
+        if (allsum && allsum(user, v, 1) != 0) return cb_fail("allsum");
+        *out = v[0];
+        return HR_OK;
+    };
+#define HR_TRY(x) do { hr_status q_ = (x); if (q_ != HR_OK) return q_; } while (0)
+    // rhs = Dhat^dagger b = gamma5 Dhat gamma5 b;  x = 0, r = p = rhs
+    HR_TRY(launch_lincomb(ctx, prec, w, one, 1, b_e, zero, nullptr, st));
+    HR_TRY(g5dhat(r, w));
+    HR_TRY(launch_lincomb(ctx, prec, p, one, 0, r, zero, nullptr, st));
+    HR_TRY(launch_lincomb(ctx, prec, x_e, zero, 0, r, zero, nullptr, st));
+    double bb = 0;
+    HR_TRY(gdot(r, r, &bb));
+    double rr = bb;
+    int k = 0;
+    if (hist) hist[0] = bb > 0 ? 1.0 : 0.0;
+    while (bb > 0 && k < maxiter && rr > tol * tol * bb) {
+        HR_TRY(g5dhat(w, p));
+        HR_TRY(g5dhat(ap, w));
+        double pap = 0;
+        HR_TRY(gdot(p, ap, &pap));
+        const double alpha = rr / pap;
+        const double pa[2] = { alpha, 0 }, na[2] = { -alpha, 0 };
+        HR_TRY(launch_lincomb(ctx, prec, x_e, one, 0, x_e, pa, p, st));
+        HR_TRY(launch_lincomb(ctx, prec, r, one, 0, r, na, ap, st));
+        double rr_new = 0;
+        HR_TRY(gdot(r, r, &rr_new));
+        const double beta[2] = { rr_new / rr, 0 };
+        HR_TRY(launch_lincomb(ctx, prec, p, one, 0, r, beta, p, st));
+        rr = rr_new;
+        ++k;
+        if (hist) hist[k] = rr / bb;
+    }
+#undef HR_TRY
+    if (iters) *iters = k;
+    return HR_OK;
+}
+
 size_t hr_bicgstab_workspace_bytes(const hr_ctx *ctx, hr_prec prec, int maxiter)
 {
     if (!ctx || !valid_prec(prec) || maxiter < 0) return 0;
@@ -728,7 +813,13 @@ hr_status hr_bicgstab_dhat_mixed(hr_ctx *ctx, double m0, void *x_e, const void *
         if (rc != HR_OK) return rc;
         rc = launch_lincomb(ctx, HR_F64, r, one, 0, b_e, mone, ax, st);                               // r = b - Dhat x
         if (rc != HR_OK) return rc;
-        if (it == 0) break;                                                                           // no progress possible
+        if (it == 0) {                                                                                // no progress possible:
+            rc = launch_dot(ctx, HR_F64, r, r, rs, rs.result, st);                                    // report the residual of
+            if (rc != HR_OK) return rc;                                                               // the x that is returned
+            HR_CUDA(cudaMemcpyAsync(&rr, rs.result, sizeof(double), cudaMemcpyDeviceToHost, st));
+            HR_CUDA(cudaStreamSynchronize(st));
+            break;
+        }
     }
     if (iters) *iters = total;
     if (outer_steps) *outer_steps = outer;

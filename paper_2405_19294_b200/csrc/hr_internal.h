@@ -37,6 +37,12 @@ struct hr_ctx {
     void *ws_in, *ws_out, *ws_stage;
     size_t ws_spinor_bytes, ws_stage_bytes;
     int ws_prec;
+    // staging of host canonical arrays (hr_gauge_import / export, hr_spinor_import / export, hr_dphi_eo_host): two device
+    // buffers and a copy stream, created on first use and kept, so that the copy of chunk k+1 overlaps the (un)packing of chunk k
+    void *stage[2];
+    size_t stage_bytes;
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_copied[2], ev_used[2];
     // reduction scratch (hr_spinor_dot / norm2, fused Dphi reductions, CG): per-CTA partial sums, the
     // self-resetting ticket counter and a small result area; created on first use, one stream at a time
     void *red_scratch;

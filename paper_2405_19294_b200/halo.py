@@ -37,6 +37,48 @@ def exchange(send_up, send_dn, recv_prev, recv_next, plan: dict, group=None):
         req.wait()
 
 
+class AsyncExchange:
+    """The NCCL exchange of a set of (send_up, send_dn, recv_prev, recv_next, prev, next) face buffers, started on a SIDE
+    stream that waits only for the pack kernels, so that the transfer runs while the interior kernel (enqueued on the
+    compute stream afterwards) computes -- PAPER.md:50: "compute the bulk while the messages are in flight".
+    (torch's NCCL stream waits for the stream that is current when batch_isend_irecv is called: issued from the compute
+    stream AFTER the interior launch the transfer would start only when the interior kernel has finished.)
+    start(): after the pack launches; finish(): makes the compute stream wait for the transfers, before the applies.
+    All directions go into ONE batch.  Matching between two ranks that are each other's previous AND next neighbour
+    (two blocks in a direction) relies on both posting [send up, recv prev, send down, recv next] in this order."""
+
+    def __init__(self, device, group=None):
+        import torch
+        self.torch, self.group = torch, group
+        self.side = torch.cuda.Stream(device=device)
+        self.packed = torch.cuda.Event()
+        self.reqs = []
+
+    def start(self, faces) -> None:
+        import torch.distributed as dist
+        torch = self.torch
+        world = dist.get_world_size(self.group) if dist.is_available() and dist.is_initialized() else 1
+        if world == 1:
+            for su, sd, rp, rn, _, _ in faces:
+                rp.copy_(su)
+                rn.copy_(sd)
+            self.reqs = []
+            return
+        ops = []
+        for su, sd, rp, rn, prev, nxt in faces:
+            ops += [dist.P2POp(dist.isend, su, nxt, self.group), dist.P2POp(dist.irecv, rp, prev, self.group),
+                    dist.P2POp(dist.isend, sd, prev, self.group), dist.P2POp(dist.irecv, rn, nxt, self.group)]
+        self.packed.record(torch.cuda.current_stream())
+        with torch.cuda.stream(self.side):
+            self.side.wait_event(self.packed)
+            self.reqs = dist.batch_isend_irecv(ops)
+
+    def finish(self) -> None:
+        for req in self.reqs:
+            req.wait()                       # the CURRENT (compute) stream waits for the transfer; no host wait
+        self.reqs = []
+
+
 class SlabDphi:
     """Distributed Dphi_eo of one rank: owns the four face buffers and sequences pack -> exchange || interior -> apply."""
 
@@ -47,13 +89,16 @@ class SlabDphi:
         n = hr_halo_bytes(lat.ctx, prec)
         dev = f"cuda:{lat.device}"
         self.send_up, self.send_dn, self.recv_prev, self.recv_next = (torch.empty(n, dtype=torch.uint8, device=dev) for _ in range(4))
+        self.xch = AsyncExchange(dev, group)
 
     def dphi_eo(self, out, inp, links: int, parity: int) -> None:
         from . import hr_dphi_eo_halo_apply, hr_dphi_eo_halo_pack, hr_dphi_eo_interior
         st = self.lat.stream()
         hr_dphi_eo_halo_pack(self.send_up, self.send_dn, inp, links, parity, st)
-        hr_dphi_eo_interior(out, inp, links, parity, st)      # enqueued first: NCCL's transfer overlaps with it
-        exchange(self.send_up, self.send_dn, self.recv_prev, self.recv_next, self.plan, self.group)
+        # pack -> [exchange on the side stream || interior on the compute stream] -> apply
+        self.xch.start([(self.send_up, self.send_dn, self.recv_prev, self.recv_next, self.plan["prev"], self.plan["next"])])
+        hr_dphi_eo_interior(out, inp, links, parity, st)
+        self.xch.finish()
         hr_dphi_eo_halo_apply(out, self.recv_prev, self.recv_next, links, parity, self.plan["first_rank"], self.plan["last_rank"], st)
 
 
@@ -135,71 +180,35 @@ class PeerSlabDphi:
 
 
 class SlabCG:
-    """Dhat x = b on a lattice cut into t-slabs (one per rank): CG on Dhat^dag Dhat x = Dhat^dag b (the
-    algorithm of hr_cg_dhat, readings C20-C22), every vector operation one of the library's kernels on the LOCAL slab,
-    the operator through `slab` (SlabDphi or PeerSlabDphi: two distributed Dphi_eo per Dhat), and the two scalars of an
-    iteration summed over the ranks with an all-reduce.  Host-driven (one scalar read per reduction): this is the
-    distributed counterpart of the single-GPU solver, not its tuned form."""
+    """Dhat x = b on a lattice cut into slabs or blocks (one per rank): hr_cg_dhat_dist (include/hr.h) -- the CG of
+    hr_cg_dhat, readings C20-C22, with every vector update AND every scalar recurrence inside libhr.  This class only
+    supplies the two callbacks the library cannot know: the distributed Dphi_eo (`slab`: SlabDphi, PeerSlabDphi, BlockDphi
+    or PeerBlockDphi) and the sum of a few doubles over the ranks (torch.distributed.all_reduce)."""
 
     def __init__(self, slab, links: int, m0: float, group=None):
         self.slab, self.links, self.m0, self.group = slab, links, float(m0), group
         self.lat, self.prec = slab.lat, slab.prec
-        self.tmp_o = self.lat.spinor(self.prec)
-        self.tmp_e = self.lat.spinor(self.prec)
 
-    def allsum(self, v: float) -> float:
+    def allsum(self, vals):
+        """Sum of a list of floats over the ranks (plumbing: one all-reduce)."""
         import torch
         import torch.distributed as dist
         if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(self.group) == 1:
-            return v
+            return list(vals)
         dev = f"cuda:{self.lat.device}" if dist.get_backend(self.group) == "nccl" else "cpu"
-        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        t = torch.tensor(list(vals), dtype=torch.float64, device=dev)
         dist.all_reduce(t, group=self.group)
-        return float(t.item())
-
-    def g5dhat(self, out, inp) -> None:
-        """out = gamma5 Dhat inp,  Dhat = (4+m0)^2 - Dphi_eo Dphi_oe  (Hermitian, reading C21)."""
-        from . import hr_spinor_g5, hr_spinor_lincomb
-        ctx, P, st = self.lat.ctx, self.prec, self.lat.stream()
-        self.slab.dphi_eo(self.tmp_o, inp, self.links, 1)
-        self.slab.dphi_eo(self.tmp_e, self.tmp_o, self.links, 0)
-        m = 4.0 + self.m0
-        hr_spinor_lincomb(ctx, P, self.tmp_e, m * m, 0, inp, -1.0, self.tmp_e, st)
-        hr_spinor_g5(ctx, P, out, self.tmp_e, st)
-
-    def norm2(self, v) -> float:
-        from . import hr_spinor_norm2
-        return self.allsum(hr_spinor_norm2(self.lat.ctx, self.prec, v, self.lat.stream()))
-
-    def redot(self, a, b) -> float:
-        from . import hr_spinor_dot
-        return self.allsum(hr_spinor_dot(self.lat.ctx, self.prec, a, b, self.lat.stream()).real)
+        return t.tolist()
 
     def solve(self, x, b, tol: float, maxiter: int):
         """x = Dhat^{-1} b (x0 = 0).  Returns (iterations, [|r_k|^2 / |rhs|^2])."""
-        from . import hr_spinor_copy, hr_spinor_g5, hr_spinor_lincomb, hr_spinor_mulc_add_assign
-        lat, ctx, P, st = self.lat, self.lat.ctx, self.prec, self.lat.stream()
-        r, p, ap, w = (lat.spinor(P) for _ in range(4))
-        # rhs = Dhat^dag b = g5 Dhat g5 b;  A = Dhat^dag Dhat = (g5 Dhat)^2
-        hr_spinor_g5(ctx, P, w, b, st)
-        self.g5dhat(r, w)
-        hr_spinor_copy(ctx, P, p, r, st)
-        hr_spinor_lincomb(ctx, P, x, 0.0, 0, r, stream=st)
-        rr = bb = self.norm2(r)
-        hist = [1.0 if bb > 0 else 0.0]
-        k = 0
-        while bb > 0 and k < maxiter and rr > tol * tol * bb:
-            self.g5dhat(w, p)
-            self.g5dhat(ap, w)
-            alpha = rr / self.redot(p, ap)
-            hr_spinor_mulc_add_assign(ctx, P, x, alpha, p, st)
-            hr_spinor_mulc_add_assign(ctx, P, r, -alpha, ap, st)
-            rr_new = self.norm2(r)
-            hr_spinor_lincomb(ctx, P, p, 1.0, 0, r, rr_new / rr, p, st)
-            rr = rr_new
-            k += 1
-            hist.append(rr / bb)
-        return k, hist
+        import torch
+        from . import hr_cg_dhat_dist, hr_cg_dist_workspace_bytes
+        lat = self.lat
+        ws = torch.empty(hr_cg_dist_workspace_bytes(lat.ctx, self.prec), dtype=torch.uint8, device=f"cuda:{lat.device}")
+        return hr_cg_dhat_dist(lat.ctx, self.prec, self.m0, x, b, tol, maxiter, ws,
+                               lambda out, inp, parity: self.slab.dphi_eo(out, inp, self.links, parity),
+                               self.allsum, lat.stream())
 
 
 # ---- 4-D block decomposition (SURVEY.md section 5: "4-D block partition, split t first, then z, y, x") ------------------
@@ -243,8 +252,8 @@ def block_plan(rank: int, grid, dims_global) -> dict:
 
 class BlockDphi:
     """Distributed Dphi_eo of one rank of a 4-D block decomposition: for every split direction the four face buffers;
-    pack (all directions, same input) -> interior launch with the split directions masked || exchange -> apply
-    direction by direction on the same stream."""
+    pack (all directions, same input) -> [exchange of all faces in one NCCL batch on a side stream || interior launch with
+    the split directions masked] -> apply direction by direction.  Unmeasured on more than one GPU (none in this run)."""
 
     def __init__(self, lat, prec: int, plan: dict, group=None):
         import torch
@@ -253,6 +262,7 @@ class BlockDphi:
         dev = f"cuda:{lat.device}"
         self.buf = {mu: [torch.empty(hr_face_bytes(lat.ctx, prec, mu), dtype=torch.uint8, device=dev) for _ in range(4)]
                     for mu in plan["split"]}                      # send_up, send_dn, recv_prev, recv_next
+        self.xch = AsyncExchange(dev, group)
 
     def pack(self, inp, links: int, parity: int) -> None:
         from . import hr_dphi_eo_face_pack
@@ -263,9 +273,8 @@ class BlockDphi:
         from . import hr_dphi_eo_interior_mask
         hr_dphi_eo_interior_mask(out, inp, links, parity, self.plan["mask"], self.lat.stream())
 
-    def exchange(self) -> None:
-        for mu, (su, sd, rp, rn) in self.buf.items():
-            exchange(su, sd, rp, rn, {"prev": self.plan["prev"][mu], "next": self.plan["next"][mu]}, self.group)
+    def faces(self):
+        return [(su, sd, rp, rn, self.plan["prev"][mu], self.plan["next"][mu]) for mu, (su, sd, rp, rn) in self.buf.items()]
 
     def apply(self, out, links: int, parity: int) -> None:
         from . import hr_dphi_eo_face_apply
@@ -274,8 +283,9 @@ class BlockDphi:
 
     def dphi_eo(self, out, inp, links: int, parity: int) -> None:
         self.pack(inp, links, parity)
-        self.interior(out, inp, links, parity)
-        self.exchange()
+        self.xch.start(self.faces())                 # one batch for all split directions, on the side stream
+        self.interior(out, inp, links, parity)       # ... while the interior kernel runs on the compute stream
+        self.xch.finish()
         self.apply(out, links, parity)
 
 
