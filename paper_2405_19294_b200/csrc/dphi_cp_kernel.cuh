@@ -95,7 +95,21 @@ template <typename Real, int D, bool RL> struct CpGeom {
     static constexpr int SITES = HR_CP_SITES;
     static constexpr int THREADS = (SITES * NG + 31) / 32 * 32;
     static constexpr int HB = 4;                     // hops per batch
-    static constexpr size_t smem_bytes() { return (size_t)HB * 2 * D * SITES * sizeof(CpPair<Real>); }
+    // Odd d_R with sub-vector link elements (SU(4) adjoint: 15 x 15 reals) cannot be read with whole vectors from a
+    // thread's own row or column: the CTA then copies the hop's link records of its sites into shared memory with
+    // coalesced 16-byte cp.async copies (every byte of every sector used once), double-buffered so that the copy of the next
+    // hop's links runs under the arithmetic of this one, and the threads pick their elements there.
+    // Measured, SU(4) adjoint 16^3 x 48: fp32 0.244 -> 0.223 ms (0.50 -> 0.55 of the copy peak), fp64 0.333 -> 0.428 ms --
+    // so fp32 only.  What binds this kernel is not the link loads but the shared-memory data pipe they share with the
+    // half-spinor exchange: every one of the 15 threads of a site reads all 30 entries h_{k,b} of a hop (7.2 KB per site
+    // and hop in fp64 against 1.8 KB of link), 5.7 GB per launch = 0.16 ms of the pipe at 128 B per clock and SM before a
+    // single link byte moves; staging adds 3.6 KB per site and hop and a barrier per hop.  The fix is fewer h reads
+    // (several rows per thread), which at d_R = 15 = 3 x 5 leaves 5 warps per SM next to 90 KB of buffers; not done.
+    static constexpr bool STAGE = RL && (D % 2 == 1) && D > 8 && sizeof(Real) == 4;
+    static constexpr int LNREAL_ = RL ? D * D : 2 * D * D;
+    static constexpr int NVT = (LNREAL_ + RPV - 1) / RPV;   // link planes including the tail plane
+    __host__ __device__ static constexpr size_t hs_bytes() { return (size_t)HB * 2 * D * SITES * sizeof(CpPair<Real>); }
+    static constexpr size_t smem_bytes() { return hs_bytes() + (STAGE ? 2 * ((size_t)NVT * SITES * 16 + SITES * sizeof(long)) : 0); }
     // registers: a thread's state does not grow with d_R, so the cap is chosen for occupancy (several CTAs per SM hide
     // the three barriers): HR_CP_REGS registers per thread per row
     // (measured on B200, bench_large_n: SU(4) sym d_R = 10 fp64 0.260 ms at 84, 0.275 at 160, 0.291 at 64; SU(4) adj
@@ -125,6 +139,8 @@ __global__ void __launch_bounds__((CpGeom<Real, D, RL>::THREADS), (CpGeom<Real, 
     if (a.skip != nullptr && *a.skip != 0) return;
     extern __shared__ __align__(16) unsigned char cp_smem[];
     CpPair<Real> *hs = reinterpret_cast<CpPair<Real> *>(cp_smem);          // [slot][k][b][site]
+    [[maybe_unused]] unsigned char *lk_sm = cp_smem + G::hs_bytes();        // STAGE: 2 x [plane][site] 16-byte vectors of one hop's links
+    [[maybe_unused]] long *sn_sm = reinterpret_cast<long *>(cp_smem + G::hs_bytes() + 2 * (size_t)G::NVT * SITES * 16);   // 2 x [site]
 
     const int sl = (int)threadIdx.x % SITES;
     const bool shadow = (int)threadIdx.x / SITES >= G::NG;
@@ -152,6 +168,42 @@ __global__ void __launch_bounds__((CpGeom<Real, D, RL>::THREADS), (CpGeom<Real, 
     for (int rr = 0; rr < RPT; ++rr)
 #pragma unroll
         for (int al = 0; al < 4; ++al) acc[rr][al][0] = acc[rr][al][1] = 0;
+
+    // STAGE: the link records of the CTA's sites for hop (MU, DIR) -> shared-memory buffer `buf`, asynchronously.
+    // publish: row group 0 writes each site's link index (own site for a forward hop, the neighbour for a backward hop);
+    // issue (after a barrier): all threads copy [planes][sites] with 16-byte cp.async, the tail plane with 4 / 8 bytes.
+    [[maybe_unused]] auto stage_publish = [&](auto mu_c, auto dir_c, int buf) {
+        constexpr int MU = decltype(mu_c)::value;
+        constexpr int DIR = decltype(dir_c)::value;
+        if ((int)threadIdx.x < SITES) {
+            long sn; int sign;
+            neighbour<MU, DIR>(a, g, s, sn, sign);
+            sn_sm[buf * SITES + sl] = DIR == 0 ? s : sn;
+        }
+    };
+    [[maybe_unused]] auto stage_issue = [&](auto mu_c, auto dir_c, int buf) {
+        constexpr int MU = decltype(mu_c)::value;
+        constexpr int DIR = decltype(dir_c)::value;
+        constexpr int NV = LNREAL / RPV, TAILB = (LNREAL - NV * RPV) * (int)sizeof(Real);
+        const char *lbase = (DIR == 0 ? lk_own : lk_nbr) + (size_t)MU * LB * vh;
+        const uint32_t dst0 = (uint32_t)__cvta_generic_to_shared(lk_sm + (size_t)buf * G::NVT * SITES * 16);
+        for (int idx = (int)threadIdx.x; idx < G::NVT * SITES; idx += G::THREADS) {
+            const int v = idx / SITES, j = idx - v * SITES;
+            const size_t sj = (size_t)sn_sm[buf * SITES + j];
+            if (v < NV)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst0 + (uint32_t)idx * 16u), "l"(lbase + ((size_t)v * vh + sj) * 16) : "memory");
+            else if constexpr (TAILB == 8)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst0 + (uint32_t)idx * 16u), "l"(lbase + (size_t)NV * 16 * vh + sj * 8) : "memory");
+            else if constexpr (TAILB == 4)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst0 + (uint32_t)idx * 16u), "l"(lbase + (size_t)NV * 16 * vh + sj * 4) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    if constexpr (G::STAGE) {
+        stage_publish(std::integral_constant<int, 0>{}, std::integral_constant<int, 0>{}, 0);
+        __syncthreads();
+        stage_issue(std::integral_constant<int, 0>{}, std::integral_constant<int, 0>{}, 0);
+    }
 
     // step 1 of a hop: my colours of the neighbour spinor -> my half-spinor entries -> shared memory
     auto project = [&](auto mu_c, auto dir_c, int slot, long &sn, int &sign) {
@@ -188,7 +240,20 @@ __global__ void __launch_bounds__((CpGeom<Real, D, RL>::THREADS), (CpGeom<Real, 
         const size_t ls = DIR == 0 ? (size_t)s : (size_t)sn;
         // the link elements of this thread, ul[rr][b]: rows r0+rr of U(s) (forward) or columns r0+rr of U(sn) (backward)
         Real ul[RPT][C * D];
-        if constexpr (DIR == 0) {
+        if constexpr (G::STAGE) {
+            static_assert(RPT == 1 && C == 1, "staged links: one real row per thread");
+            constexpr int H = 2 * MU + DIR;                                  // hops run in the order (mu, dir) = (0,0), (0,1), (1,0), ...
+            asm volatile("cp.async.wait_all;" ::: "memory");                 // my copies of this hop's links have landed
+            if constexpr (H < 7) stage_publish(std::integral_constant<int, (H + 1) / 2>{}, std::integral_constant<int, (H + 1) % 2>{}, (H + 1) & 1);
+            __syncthreads();                                                // everybody's copies are visible; everybody is done with hop H-1
+            if constexpr (H < 7) stage_issue(std::integral_constant<int, (H + 1) / 2>{}, std::integral_constant<int, (H + 1) % 2>{}, (H + 1) & 1);
+            const Real *lrec = reinterpret_cast<const Real *>(lk_sm + (size_t)(H & 1) * G::NVT * SITES * 16) + (size_t)sl * RPV;
+#pragma unroll
+            for (int b = 0; b < D; ++b) {
+                const int e = DIR == 0 ? r0 * D + b : b * D + r0;             // element e: plane e / RPV, word e % RPV
+                ul[0][b] = lrec[(size_t)(e / RPV) * SITES * RPV + (e % RPV)];
+            }
+        } else if constexpr (DIR == 0) {
 #pragma unroll
             for (int rr = 0; rr < RPT; ++rr) load_elems<ROW_AL ? LD_STREAM : EH, LNREAL, C, D, ROW_AL>(ul[rr], lbase, vh, ls, (r0 + rr) * D);
         } else {
