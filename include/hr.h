@@ -262,8 +262,10 @@ hr_status hr_cg_dhat_dist(hr_ctx *ctx, hr_prec prec, double m0, void *x_e, const
  * |eta_k| is the norm of the quasi-residual (|b - Dhat x_k| <= sqrt(k+1) |eta_k|); when |eta_k| <= tol |b| the TRUE
  * residual is computed (one more operator application) and the iteration ends if |b - Dhat x_k| <= tol |b|; it also ends at
  * k = maxiter, when the Krylov space is exhausted and at a Lanczos breakdown ((v_k, v_k)_J = 0).  The Lanczos scalars and the
- * Givens rotations live on the HOST: two synchronisations of `stream` per iteration; the vector work is two fused
- * kernels.  Arguments as hr_cg_dhat; workspace of hr_qmr_workspace_bytes(), 256-byte aligned.
+ * Givens rotations live on the DEVICE (a small state owned by the context), like the CG's: the host enqueues batches of 4, 8,
+ * ... 32 iterations -- per iteration two Dphi launches, two fused vector kernels and two one-thread kernels -- and reads the
+ * state once per batch; once a stop flag is set the rest of a batch returns at once.  Arguments as hr_cg_dhat; workspace of
+ * hr_qmr_workspace_bytes(), 256-byte aligned.
  *   rel_res2: TRUE |b - Dhat x|^2 / |b|^2 at exit.  hist (HOST, maxiter+1 doubles): |eta_k| / |b| for k = 0..iters.
  */
 size_t hr_qmr_workspace_bytes(const hr_ctx *ctx, hr_prec prec);

@@ -201,6 +201,8 @@ hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N,
     c->xblock = 0;
     c->cg_graph = 1;
     c->bulk_rows = c->bulk_stages = c->bulk_ctas = c->bulk_strip = 0;
+    c->qmr_state = nullptr;
+    c->qmr_state_bytes = 0;
     c->stage[0] = c->stage[1] = nullptr;
     c->stage_bytes = 0;
     c->copy_stream = nullptr;
@@ -216,8 +218,9 @@ hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N,
 void hr_ctx_destroy(hr_ctx *ctx)
 {
     if (!ctx) return;
-    if (ctx->ws_in || ctx->ws_out || ctx->ws_stage || ctx->red_scratch || ctx->stage[0]) {
+    if (ctx->ws_in || ctx->ws_out || ctx->ws_stage || ctx->red_scratch || ctx->stage[0] || ctx->qmr_state) {
         if (cudaSetDevice(ctx->device) == cudaSuccess) {
+            cudaFree(ctx->qmr_state);
             if (ctx->stage[0]) {
                 cudaFree(ctx->stage[0]);
                 cudaFree(ctx->stage[1]);

@@ -559,63 +559,67 @@ hr_status hr_qmr_dhat(hr_ctx *ctx, double m0, void *x_e, const void *b_e, const 
     if (iters) *iters = 0;
     if (rel_res2) *rel_res2 = bb > 0.0 ? 1.0 : 0.0;
     if (bb == 0.0) return HR_OK;
+    // the device-resident state (Lanczos scalars, rotations, history): owned by the context, grown with maxiter
+    const size_t need = (sizeof(QmrState) + ((size_t)maxiter + 2) * sizeof(double) + 255) & ~(size_t)255;
+    if (ctx->qmr_state_bytes < need) {
+        if (ctx->qmr_state) { HR_CUDA(cudaStreamSynchronize(st)); cudaFree(ctx->qmr_state); ctx->qmr_state = nullptr; ctx->qmr_state_bytes = 0; }
+        HR_CUDA(cudaMalloc(&ctx->qmr_state, need));
+        ctx->qmr_state_bytes = need;
+    }
+    QmrState *qs = (QmrState *)ctx->qmr_state;
     const double inv[2] = { 1.0 / bnorm, 0.0 };
-    rc = launch_lincomb(ctx, P, v, inv, 0, b_e, zero, nullptr, st);                       // v_1 = b / rho_1
+    // buffers by iteration parity: v_k in va (k even) / vb (k odd), v_{k-1} in the other; p_{k-1} in pa (k even) / pb, p_{k-2} in the other
+    void *va = v, *vb = vp, *pa = p1, *pb = p2;
+    rc = launch_lincomb(ctx, P, va, inv, 0, b_e, zero, nullptr, st);                      // v_1 = b / rho_1
     if (rc != HR_OK) return rc;
-    rc = launch_lincomb(ctx, P, p1, zero, 0, b_e, zero, nullptr, st);                     // p_0 = p_{-1} = 0
+    rc = launch_lincomb(ctx, P, pa, zero, 0, b_e, zero, nullptr, st);                     // p_0 = p_{-1} = 0
     if (rc != HR_OK) return rc;
-    rc = launch_lincomb(ctx, P, p2, zero, 0, b_e, zero, nullptr, st);
+    rc = launch_lincomb(ctx, P, pb, zero, 0, b_e, zero, nullptr, st);
     if (rc != HR_OK) return rc;
-    double c1 = 1.0, s1 = 0.0, c2 = 1.0, s2 = 0.0, eta = bnorm, rho = bnorm;
-    double delta_prev = 1.0, delta = (up - lo) / bb;
+    rc = launch_qmr_init(qs, bnorm, (up - lo) / bb, tol, maxiter, st);
+    if (rc != HR_OK) return rc;
+    // one iteration, with the buffer roles of iteration index kk: 2 Dphi launches (fused reduction -> (v, Dhat v)_J), the
+    // Lanczos kernel, the update kernel and two one-thread kernels for the scalar recurrences -- nothing returns to the host
+    auto enqueue = [&](int kk) -> hr_status {
+        void *vk = (kk & 1) ? vb : va, *vprev = (kk & 1) ? va : vb;
+        void *pk1 = (kk & 1) ? pb : pa, *pk2 = (kk & 1) ? pa : pb;
+        hr_status r = dhat_launches(ctx, m0, 1, w, vk, tmp, links, &rs, qs->red + 4, &qs->stop, st);   // w = gamma5 Dhat v
+        if (r != HR_OK) return r;
+        r = launch_qmr_scal_a(qs, st);
+        if (r != HR_OK) return r;
+        r = launch_qmr_lanczos(ctx, P, w, vk, vprev, qs, rs, st);    // vt = gamma5 w - alpha v - beta v_prev (into w) + its half norms
+        if (r != HR_OK) return r;
+        r = launch_qmr_scal_b(qs, st);
+        if (r != HR_OK) return r;
+        // p = (v - eps p_{k-1} - theta p_{k-2}) / zeta into p_{k-2}'s buffer; x += c eta p; v_{k+1} = vt / rho_{k+1} into v_{k-1}'s buffer
+        return launch_qmr_update(ctx, P, pk2, pk1, vk, x_e, vprev, w, qs, st);
+    };
+    QmrState hs;
     double res2 = 1.0;
     bool have_res = false;
-    int k = 0;
-    while (k < maxiter) {
-        if (delta == 0.0) break;                                                           // Lanczos breakdown
-        // w = gamma5 Dhat v, and <v, w> = (v, Dhat v)_J from the fused reduction of the second Dphi launch
-        rc = dhat_launches(ctx, m0, 1, w, v, tmp, links, &rs, rs.result + 4, nullptr, st);
-        if (rc != HR_OK) return rc;
-        HR_CUDA(cudaMemcpyAsync(h + 4, rs.result + 4, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    int k = 0, batch = 4;
+    for (;;) {
+        const int n = maxiter - k < batch ? maxiter - k : batch;
+        for (int j = 0; j < n; ++j) { rc = enqueue(k + j); if (rc != HR_OK) return rc; }
+        HR_CUDA(cudaMemcpyAsync(&hs, qs, sizeof(QmrState), cudaMemcpyDeviceToHost, st));
         HR_CUDA(cudaStreamSynchronize(st));
-        const double alpha = h[5] / delta;
-        const double beta = k > 0 ? rho * delta / delta_prev : 0.0;
-        // vt = Dhat v - alpha v - beta v_prev = gamma5 w - alpha v - beta v_prev (into w) and its two half norms: one kernel
-        rc = launch_qmr_lanczos(ctx, P, w, v, vp, alpha, beta, rs, rs.result, st);
-        if (rc != HR_OK) return rc;
-        HR_CUDA(cudaMemcpyAsync(h, rs.result, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        HR_CUDA(cudaStreamSynchronize(st));
-        up = h[0]; lo = h[1];
-        const double rho_next = sqrt(up + lo);
-        const double theta = s2 * beta, t = c2 * beta;
-        const double eps = c1 * t + s1 * alpha, zt = -s1 * t + c1 * alpha;
-        const double zeta = sqrt(zt * zt + rho_next * rho_next);
-        if (zeta == 0.0) break;
-        const double c = zt / zeta, s = rho_next / zeta;
-        // p = (v - eps p1 - theta p2) / zeta into p2's buffer (p_{k-2} is not needed again); x += c eta p;
-        // v_{k+1} = vt / rho_{k+1} into the old v_prev buffer: one kernel
-        rc = launch_qmr_update(ctx, P, p2, p1, v, x_e, vp, w, 1.0 / zeta, eps, theta, c * eta, rho_next > 0.0 ? 1.0 / rho_next : 0.0, st);
-        if (rc != HR_OK) return rc;
-        eta = -s * eta;
-        ++k;
-        if (hist) hist[k] = fabs(eta) / bnorm;
-        { void *q = p1; p1 = p2; p2 = q; }
-        c2 = c1; s2 = s1; c1 = c; s1 = s;
-        if (rho_next == 0.0) { rc = true_res2(bb, &res2); if (rc != HR_OK) return rc; have_res = true; break; }
-        // delta_{k+1} = (|vt_up|^2 - |vt_lo|^2) / rho_{k+1}^2
-        { void *q = v; v = vp; vp = q; }
-        delta_prev = delta;
-        delta = (up - lo) / (up + lo);
-        rho = rho_next;
-        if (fabs(eta) <= tol * bnorm) {
+        k = hs.k;
+        if (hs.stop == 1) {                                   // quasi-residual below tol: the TRUE residual decides
             rc = true_res2(bb, &res2);
             if (rc != HR_OK) return rc;
             have_res = true;
-            if (res2 <= tol * tol) break;
+            if (res2 <= tol * tol || k >= maxiter) break;
             have_res = false;
+            rc = launch_qmr_resume(qs, st);
+            if (rc != HR_OK) return rc;
+            if (k >= maxiter) break;
+            continue;
         }
+        if (hs.stop != 0 || k >= maxiter) break;
+        if (batch < 32) batch *= 2;
     }
     if (!have_res) { rc = true_res2(bb, &res2); if (rc != HR_OK) return rc; }
+    if (hist && k > 0) HR_CUDA(cudaMemcpy(hist + 1, reinterpret_cast<const double *>(qs + 1) + 1, (size_t)k * sizeof(double), cudaMemcpyDeviceToHost));
     if (iters) *iters = k;
     if (rel_res2) *rel_res2 = res2;
     return HR_OK;

@@ -43,6 +43,9 @@ struct hr_ctx {
     size_t stage_bytes;
     cudaStream_t copy_stream;
     cudaEvent_t ev_copied[2], ev_used[2];
+    // device-resident state of hr_qmr_dhat (QmrState + history), created on first use, grown with maxiter
+    void *qmr_state;
+    size_t qmr_state_bytes;
     // reduction scratch (hr_spinor_dot / norm2, fused Dphi reductions, CG): per-CTA partial sums, the
     // self-resetting ticket counter and a small result area; created on first use, one stream at a time
     void *red_scratch;
@@ -129,6 +132,20 @@ struct LaunchTune {
 };
 static const size_t kMaxDynSmem = 227 * 1024;
 
+// device-resident state of the gamma5-QMR (linalg.cu kernels, hr_qmr_dhat): the Lanczos scalars and Givens rotations never
+// leave the device; the host enqueues batches of iterations and reads this header once per batch
+struct QmrState {
+    double c1, s1, c2, s2, eta, rho, delta, delta_prev, bnorm, tol;
+    double alpha, beta;                      // of the current iteration: qmr_scal_a -> Lanczos kernel
+    double izeta, eps, theta, ceta, irho;    // qmr_scal_b -> update kernel
+    double red[8];                           // [0..1] |vt_up|^2, |vt_lo|^2 (Lanczos kernel); [4..6] fused Dphi reduction: [5] = (v, Dhat v)_J
+    int k, maxiter;
+    int stop;        // 0 running; 1 |eta_k| <= tol |b|: the host checks the TRUE residual; 2 breakdown (delta = 0 or zeta = 0);
+                     // 3 Krylov space exhausted (rho_{k+1} = 0); 4 k = maxiter.  Non-zero: every later kernel is a no-op
+    int do_update;   // the update kernel of the current iteration runs (0 for skipped iterations and after zeta = 0)
+    // hist[k] = |eta_k| / |b|, k = 0..maxiter, follows
+};
+
 // number of CTAs the reduction scratch provides partial-sum slots for
 static const unsigned kRedMaxBlocks = 1u << 20;
 struct RedScratch {
@@ -187,10 +204,15 @@ hr_status launch_cvt(const hr_ctx *c, bool down, void *dst, const void *src, dou
 //   result[0..1] = <x, y> (result[0] = |x|^2 when x == y), device pointer
 hr_status launch_dot(const hr_ctx *c, hr_prec prec, const void *x, const void *y, const RedScratch &rs,
                      double *result_dev, cudaStream_t st);
-hr_status launch_qmr_lanczos(const hr_ctx *c, hr_prec prec, void *w, const void *v, const void *vp, double alpha, double beta,
-                             const RedScratch &rs, double *result_dev, cudaStream_t st);
+// one QMR iteration's vector work and scalar recurrences on the device-resident QmrState
+hr_status launch_qmr_init(QmrState *qs, double bnorm, double delta0, double tol, int maxiter, cudaStream_t st);
+hr_status launch_qmr_scal_a(QmrState *qs, cudaStream_t st);
+hr_status launch_qmr_lanczos(const hr_ctx *c, hr_prec prec, void *w, const void *v, const void *vp, QmrState *qs, const RedScratch &rs,
+                             cudaStream_t st);
+hr_status launch_qmr_scal_b(QmrState *qs, cudaStream_t st);
 hr_status launch_qmr_update(const hr_ctx *c, hr_prec prec, void *p2, const void *p1, const void *v, void *x, void *vp, const void *w,
-                            double izeta, double eps, double theta, double ceta, double irho, cudaStream_t st);
+                            const QmrState *qs, cudaStream_t st);
+hr_status launch_qmr_resume(QmrState *qs, cudaStream_t st);
 hr_status launch_dot_range(const hr_ctx *c, hr_prec prec, const void *x, const void *y, size_t first, size_t nvec,
                            const RedScratch &rs, double *result_dev, cudaStream_t st);
 // CG building blocks on the device-resident CgState (cg.cu)

@@ -197,13 +197,14 @@ __device__ __forceinline__ float4 vscale(float a, float4 b) { return make_float4
 __device__ __forceinline__ double vnorm2(double2 a) { return a.x * a.x + a.y * a.y; }
 __device__ __forceinline__ double vnorm2(float4 a) { return (double)(a.x * a.x + a.y * a.y) + (double)(a.z * a.z + a.w * a.w); }
 
-// Lanczos step: w <- gamma5 w - alpha v - beta vp;  result = (|w_upper|^2, |w_lower|^2) of the new w   (3 reads, 1 write)
+// Lanczos step: w <- gamma5 w - alpha v - beta vp;  qs->red[0..1] = (|w_upper|^2, |w_lower|^2) of the new w   (3 reads, 1 write)
 template <typename Real>
 __global__ void __launch_bounds__(LIN_THREADS) qmr_lanczos_kernel(typename Vec16<Real>::type *w, const typename Vec16<Real>::type *v,
-                                                                  const typename Vec16<Real>::type *vp, Real alpha, Real beta,
-                                                                  size_t nvec, size_t half, double *partial, unsigned *ticket,
-                                                                  double *result)
+                                                                  const typename Vec16<Real>::type *vp, QmrState *qs,
+                                                                  size_t nvec, size_t half, double *partial, unsigned *ticket)
 {
+    if (qs->stop != 0) return;
+    const Real alpha = (Real)qs->alpha, beta = (Real)qs->beta;
     double r[2] = { 0.0, 0.0 };
     const size_t stride = (size_t)gridDim.x * LIN_THREADS;
     for (size_t i = (size_t)blockIdx.x * LIN_THREADS + threadIdx.x; i < nvec; i += stride) {
@@ -213,7 +214,7 @@ __global__ void __launch_bounds__(LIN_THREADS) qmr_lanczos_kernel(typename Vec16
         w[i] = t;
         r[lower ? 1 : 0] += vnorm2(t);
     }
-    if (grid_reduce<2>(r, partial, ticket)) { result[0] = r[0]; result[1] = r[1]; }
+    if (grid_reduce<2>(r, partial, ticket)) { qs->red[0] = r[0]; qs->red[1] = r[1]; }
 }
 
 // direction, solution and next Lanczos vector:  p2 <- (v - eps p1 - theta p2) / zeta;  x += ceta p2;  vp <- w / rho
@@ -222,50 +223,114 @@ template <typename Real>
 __global__ void __launch_bounds__(LIN_THREADS) qmr_update_kernel(typename Vec16<Real>::type *p2, const typename Vec16<Real>::type *p1,
                                                                  const typename Vec16<Real>::type *v, typename Vec16<Real>::type *x,
                                                                  typename Vec16<Real>::type *vp, const typename Vec16<Real>::type *w,
-                                                                 Real izeta, Real eps, Real theta, Real ceta, Real irho, size_t nvec)
+                                                                 const QmrState *qs, size_t nvec)
 {
+    if (qs->do_update == 0) return;
     const size_t i = (size_t)blockIdx.x * LIN_THREADS + threadIdx.x;
     if (i >= nvec) return;
+    const Real izeta = (Real)qs->izeta, eps = (Real)qs->eps, theta = (Real)qs->theta, ceta = (Real)qs->ceta, irho = (Real)qs->irho;
     const auto p = vscale(izeta, vadd(v[i], vadd(vscale(-eps, p1[i]), vscale(-theta, p2[i]))));
     p2[i] = p;
     x[i] = vadd(x[i], vscale(ceta, p));
     vp[i] = vscale(irho, w[i]);
 }
 
+// the scalar recurrences of reading C33 (oracle/solver.py::qmr_j, same order), one thread
+__global__ void qmr_init_kernel(QmrState *qs, double bnorm, double delta0, double tol, int maxiter)
+{
+    qs->c1 = 1.0; qs->s1 = 0.0; qs->c2 = 1.0; qs->s2 = 0.0;
+    qs->eta = bnorm; qs->rho = bnorm; qs->delta_prev = 1.0; qs->delta = delta0; qs->bnorm = bnorm; qs->tol = tol;
+    qs->k = 0; qs->maxiter = maxiter; qs->do_update = 0;
+    qs->stop = maxiter == 0 ? 4 : (delta0 == 0.0 ? 2 : 0);
+    double *hist = reinterpret_cast<double *>(qs + 1);
+    hist[0] = 1.0;
+}
+// after the Dhat launches: alpha_k = (v_k, Dhat v_k)_J / delta_k, beta_k = rho_k delta_k / delta_{k-1}
+__global__ void qmr_scal_a_kernel(QmrState *qs)
+{
+    if (qs->stop != 0) { qs->do_update = 0; return; }
+    qs->alpha = qs->red[5] / qs->delta;
+    qs->beta = qs->k > 0 ? qs->rho * qs->delta / qs->delta_prev : 0.0;
+}
+// after the Lanczos kernel: rho_{k+1}, the two old rotations applied to the new column, the new rotation, eta
+__global__ void qmr_scal_b_kernel(QmrState *qs)
+{
+    if (qs->stop != 0) { qs->do_update = 0; return; }
+    const double up = qs->red[0], lo = qs->red[1];
+    const double rho_next = sqrt(up + lo);
+    const double theta = qs->s2 * qs->beta, t = qs->c2 * qs->beta;
+    const double eps = qs->c1 * t + qs->s1 * qs->alpha, zt = -qs->s1 * t + qs->c1 * qs->alpha;
+    const double zeta = sqrt(zt * zt + rho_next * rho_next);
+    if (zeta == 0.0) { qs->stop = 2; qs->do_update = 0; return; }
+    const double c = zt / zeta, s = rho_next / zeta;
+    qs->izeta = 1.0 / zeta; qs->eps = eps; qs->theta = theta; qs->ceta = c * qs->eta;
+    qs->irho = rho_next > 0.0 ? 1.0 / rho_next : 0.0;
+    qs->do_update = 1;
+    qs->eta = -s * qs->eta;
+    const int k = ++qs->k;
+    double *hist = reinterpret_cast<double *>(qs + 1);
+    hist[k] = fabs(qs->eta) / qs->bnorm;
+    qs->c2 = qs->c1; qs->s2 = qs->s1; qs->c1 = c; qs->s1 = s;
+    if (rho_next == 0.0) { qs->stop = 3; return; }
+    qs->delta_prev = qs->delta;
+    qs->delta = (up - lo) / (up + lo);
+    qs->rho = rho_next;
+    if (fabs(qs->eta) <= qs->tol * qs->bnorm) qs->stop = 1;
+    else if (k >= qs->maxiter) qs->stop = 4;
+    else if (qs->delta == 0.0) qs->stop = 2;
+}
+// the host found the true residual above tol after a stop = 1: go on (or end at maxiter / at a breakdown)
+__global__ void qmr_resume_kernel(QmrState *qs)
+{
+    qs->do_update = 0;
+    qs->stop = qs->k >= qs->maxiter ? 4 : (qs->delta == 0.0 ? 2 : 0);
+}
+
+static hr_status check_small(const char *what)
+{
+    count_launch();
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) { set_error("%s launch failed: %s", what, cudaGetErrorString(e)); return HR_ECUDA; }
+    return HR_OK;
+}
+hr_status launch_qmr_init(QmrState *qs, double bnorm, double delta0, double tol, int maxiter, cudaStream_t st)
+{
+    qmr_init_kernel<<<1, 1, 0, st>>>(qs, bnorm, delta0, tol, maxiter);
+    return check_small("qmr_init_kernel");
+}
+hr_status launch_qmr_scal_a(QmrState *qs, cudaStream_t st) { qmr_scal_a_kernel<<<1, 1, 0, st>>>(qs); return check_small("qmr_scal_a_kernel"); }
+hr_status launch_qmr_scal_b(QmrState *qs, cudaStream_t st) { qmr_scal_b_kernel<<<1, 1, 0, st>>>(qs); return check_small("qmr_scal_b_kernel"); }
+hr_status launch_qmr_resume(QmrState *qs, cudaStream_t st) { qmr_resume_kernel<<<1, 1, 0, st>>>(qs); return check_small("qmr_resume_kernel"); }
+
 template <typename Real>
-static hr_status qmr_lanczos_t(void *w, const void *v, const void *vp, double alpha, double beta, size_t nvec, const RedScratch &rs,
-                               double *result, cudaStream_t st)
+static hr_status qmr_lanczos_t(void *w, const void *v, const void *vp, QmrState *qs, size_t nvec, const RedScratch &rs, cudaStream_t st)
 {
     using V = typename Vec16<Real>::type;
-    qmr_lanczos_kernel<Real><<<reduce_grid(nvec), LIN_THREADS, 0, st>>>((V *)w, (const V *)v, (const V *)vp, (Real)alpha, (Real)beta, nvec,
-                                                                        nvec / 2, rs.partial, rs.ticket, result);
+    qmr_lanczos_kernel<Real><<<reduce_grid(nvec), LIN_THREADS, 0, st>>>((V *)w, (const V *)v, (const V *)vp, qs, nvec, nvec / 2, rs.partial, rs.ticket);
     return check_launch("qmr_lanczos_kernel");
 }
 template <typename Real>
-static hr_status qmr_update_t(void *p2, const void *p1, const void *v, void *x, void *vp, const void *w, double izeta, double eps,
-                              double theta, double ceta, double irho, size_t nvec, cudaStream_t st)
+static hr_status qmr_update_t(void *p2, const void *p1, const void *v, void *x, void *vp, const void *w, const QmrState *qs, size_t nvec,
+                              cudaStream_t st)
 {
     using V = typename Vec16<Real>::type;
     const unsigned grid = (unsigned)((nvec + LIN_THREADS - 1) / LIN_THREADS);
-    qmr_update_kernel<Real><<<grid, LIN_THREADS, 0, st>>>((V *)p2, (const V *)p1, (const V *)v, (V *)x, (V *)vp, (const V *)w, (Real)izeta,
-                                                          (Real)eps, (Real)theta, (Real)ceta, (Real)irho, nvec);
+    qmr_update_kernel<Real><<<grid, LIN_THREADS, 0, st>>>((V *)p2, (const V *)p1, (const V *)v, (V *)x, (V *)vp, (const V *)w, qs, nvec);
     return check_launch("qmr_update_kernel");
 }
 
-hr_status launch_qmr_lanczos(const hr_ctx *c, hr_prec prec, void *w, const void *v, const void *vp, double alpha, double beta,
-                             const RedScratch &rs, double *result_dev, cudaStream_t st)
+hr_status launch_qmr_lanczos(const hr_ctx *c, hr_prec prec, void *w, const void *v, const void *vp, QmrState *qs, const RedScratch &rs,
+                             cudaStream_t st)
 {
     const size_t nvec = field_nvec(c, prec);
-    return prec == HR_F64 ? qmr_lanczos_t<double>(w, v, vp, alpha, beta, nvec, rs, result_dev, st)
-                          : qmr_lanczos_t<float>(w, v, vp, alpha, beta, nvec, rs, result_dev, st);
+    return prec == HR_F64 ? qmr_lanczos_t<double>(w, v, vp, qs, nvec, rs, st) : qmr_lanczos_t<float>(w, v, vp, qs, nvec, rs, st);
 }
 
 hr_status launch_qmr_update(const hr_ctx *c, hr_prec prec, void *p2, const void *p1, const void *v, void *x, void *vp, const void *w,
-                            double izeta, double eps, double theta, double ceta, double irho, cudaStream_t st)
+                            const QmrState *qs, cudaStream_t st)
 {
     const size_t nvec = field_nvec(c, prec);
-    return prec == HR_F64 ? qmr_update_t<double>(p2, p1, v, x, vp, w, izeta, eps, theta, ceta, irho, nvec, st)
-                          : qmr_update_t<float>(p2, p1, v, x, vp, w, izeta, eps, theta, ceta, irho, nvec, st);
+    return prec == HR_F64 ? qmr_update_t<double>(p2, p1, v, x, vp, w, qs, nvec, st) : qmr_update_t<float>(p2, p1, v, x, vp, w, qs, nvec, st);
 }
 
 // <x, y> over the vectors [first, first + nvec) of the two fields (the upper / lower spin halves of a field are the first
