@@ -280,7 +280,15 @@ def solver(argv):
     full_in.zero_()
     ops.append(("clover_build (per site of the FULL lattice: 4L + C)", 2 * (4 * L + Cb), lambda k: hr.hr_clover_build(cl, links, 1.0, st)))
     ops.append(("dirac (both parities: 2(8L+3S) per site pair)", 2 * (dphi_c + S), lambda k: hr.hr_dirac(args.m0, full_out, full_in, links, st)))
-    ops.append(("dirac_clover (both parities: 2(8L+3S + C+3S))", 2 * (dphi_c + S + Cb + 3 * S), lambda k: hr.hr_dirac_clover(args.m0, full_out, full_in, links, cl, st)))
+    # the site-diagonal matrix is fused into the Dphi epilogue where the library does so (fp64, d_R <= 4, site kernels: 2 launches
+    # instead of 4); the fused path moves FEWER bytes and gets its own model: 2(8L + 3S + C) against 2(8L + 3S) + 2(C + 3S)
+    hr.hr_clover_build(cl, links, 1.0, st)
+    n0 = hr.hr_launch_count()
+    hr.hr_dirac_clover(args.m0, full_out, full_in, links, cl, st)
+    fused = hr.hr_launch_count() - n0 == 2
+    ops.append(("dirac_clover, FUSED epilogue (both parities: 2(8L+3S+C))" if fused else "dirac_clover (both parities: 2(8L+3S + C+3S))",
+                2 * (dphi_c + S + Cb) if fused else 2 * (dphi_c + S + Cb + 3 * S),
+                lambda k: hr.hr_dirac_clover(args.m0, full_out, full_in, links, cl, st)))
     # even-odd preconditioned clover operator: 2 Dphi + 2 site-local launches;
     # algorithmic bytes per even site: 2(8L+2S) + (C+2S) + (C+3S)
     Ainv = torch.empty(hr.hr_clover_bytes(ctx, P), dtype=torch.uint8, device="cuda")
@@ -288,7 +296,8 @@ def solver(argv):
     hr.hr_clover_build(Asite, links, 1.0, st)
     hr.hr_clover_finalize(ctx, P, Asite, Ainv, args.m0, st)
     t2 = lat.spinor(P)
-    ops.append(("dhat_clover", 2 * dphi_c + 2 * Cb + 5 * S,
+    ops.append(("dhat_clover, FUSED epilogues (16L + 5S + 2C)" if fused else "dhat_clover (16L + 9S + 2C)",
+                2 * 8 * L + 5 * S + 2 * Cb if fused else 2 * 8 * L + 9 * S + 2 * Cb,
                 lambda k: hr.hr_dhat_clover(sets[k % nset][2], sets[k % nset][0], sets[k % nset][1], t2, links, Asite, Ainv, st)))
     common = {"workload": cfg["name"], "dtype": args.prec, "peak_gbs": peak, "peak_source": peak_src, "sites": vh}
     for name, bps, fn in ops:
