@@ -12,7 +12,7 @@ template <typename Real, int D, int LK> bool dphi_bulk_ok_t(const DphiArgs &a, i
 
 template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, int mu, const HaloArgs &a, cudaStream_t st);
 
-static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour", "bulk", "bulk2", "bulkx", "bulkx2" };
+static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour", "bulk", "bulk2", "bulkx", "bulkx2", "site_loop" };
 
 #define HR_COMBOS(X)                                                                                      \
     X(2, 0) X(3, 0) X(4, 0) X(6, 0) X(3, 1) X(8, 1) X(3, 2) X(6, 2) X(3, 3) X(6, 3) X(2, 4) X(3, 4) X(3, 5) X(8, 6) X(8, 7) X(10, 0) X(15, 1)

@@ -9,6 +9,7 @@
 // variants that were measured and lost everywhere (DESIGN.md sections 7, 14); kept as evidence, not in the default build
 #include "dphi_pf_kernel.cuh"
 #include "dphi_cpo_kernel.cuh"
+#include "dphi_loop_kernel.cuh"
 #endif
 #include "dphi_cp_kernel.cuh"
 #include "dphi_bulk_kernel.cuh"
@@ -31,10 +32,13 @@ namespace hr {
 //   9 bulkx     bulk + the neighbour spinors of a time-slice kept in shared memory along a strip in x and re-used across
 //               sites (dphi_bulkx_kernel.cuh); d_R <= 4
 //  10 bulkx2    bulkx with two consumer threads per site
+//  11 site_loop one thread per site, the four directions as a loop with run-time projectors (dphi_loop_kernel.cuh): a
+//               quarter of the code.  Measured 8-16 % SLOWER than `site` on every case (the loop stops ptxas hoisting the
+//               next direction's loads above this direction's arithmetic): -DHR_BUILD_EXPERIMENTS only
 // d_R > 8 (SU(4) two-index symmetric, adjoint) compiles only 0 (the paper's "unimproved" kernel, for comparison) and 6.
 // Variants 4, 5 and the colour-parallel on-the-fly kernel lost every measurement: they are compiled only with
 // -DHR_BUILD_EXPERIMENTS; the pair kernels (2, 3) only where they were ever competitive (d_R >= 6).
-enum { DPHI_NVARIANTS = 11 };
+enum { DPHI_NVARIANTS = 12 };
 #ifdef HR_BUILD_EXPERIMENTS
 static constexpr bool kExperiments = true;
 #else
@@ -119,6 +123,23 @@ static hr_status launch_pf(int block, const DphiArgs &a, cudaStream_t st)
 }
 #endif
 
+#ifdef HR_BUILD_EXPERIMENTS
+template <typename Real, int D, int LK, bool MASS, bool RED>
+static hr_status launch_loop(int block, const DphiArgs &a, cudaStream_t st)
+{
+    using T = Tune<Real, D, LK, 1>;
+    if (block <= 0) block = 64;
+    if (block > T::MAXT || (block % 32) != 0) { set_error("block=%d not supported by this variant (multiple of 32, <= %d)", block, T::MAXT); return HR_EINVAL; }
+    const long grid = (a.vh + block - 1) / block;
+    if (RED && (unsigned long)grid > kRedMaxBlocks) { set_error("fused Dphi reduction: too many CTAs"); return HR_EUNSUPPORTED; }
+    dphi_loop_kernel<Real, D, LK, MASS, RED, LD_STREAM, LD_DEFAULT, T::MAXT, T::MINB><<<(unsigned)grid, block, 0, st>>>(a);
+    count_launch();
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) { set_error("dphi loop kernel launch failed: %s", cudaGetErrorString(e)); return HR_ECUDA; }
+    return HR_OK;
+}
+#endif
+
 template <typename Real, int D, int LK, bool MASS, bool RED>
 static hr_status launch_variant(int variant, const LaunchTune &lt, const DphiArgs &a, cudaStream_t st)
 {
@@ -140,6 +161,11 @@ static hr_status launch_variant(int variant, const LaunchTune &lt, const DphiArg
             if (variant == 8) return launch_bulk<Real, D, LK, MASS, RED, 2>(a, st, BulkTuning{ lt.bulk_rows, lt.bulk_stages, lt.bulk_ctas });
         }
     }
+#ifdef HR_BUILD_EXPERIMENTS
+    if constexpr (D <= 8 && (2 * D) % RPV == 0) {
+        if (variant == 11) return launch_loop<Real, D, LK, MASS, RED>(block, a, st);
+    }
+#endif
     if constexpr (D <= 4) {
         const BulkTuning bt{ lt.bulk_rows, lt.bulk_stages, lt.bulk_ctas };
         if (variant == 9) return launch_bulkx<Real, D, LK, MASS, RED, 1>(a, st, bt, lt.bulk_strip);
@@ -204,6 +230,7 @@ template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant)
     if (variant == 8) return D <= 8 && (2 * D) % RPV == 0 && (D >= 6 || LK == LK_SYM_OTF || LK == LK_ASYM_OTF);
     if (variant == 9) return D <= 4;
     if (variant == 10) return D <= 4 && (2 * D) % RPV == 0;
+    if (variant == 11) return kExperiments && D <= 8 && (2 * D) % RPV == 0;
     if (D > 8) return variant == 0;
     if ((variant == 2 || variant == 3) && ((2 * D) % RPV != 0 || !(D >= 6 || kExperiments))) return false;
     if (variant == 4 || variant == 5) {

@@ -56,7 +56,7 @@ def test_no_call_writes_outside_its_output(hr, N, rep, prec):
         checks.append(g)
         return g
 
-    for variant in (0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10):
+    for variant in (0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11):
         try:
             lat.set_tuning("variant", variant)
             o = guarded(sb)

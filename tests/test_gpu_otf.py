@@ -51,7 +51,7 @@ def test_dphi_eo_from_fundamental_links_matches_oracle(hr, dims, N, rep, prec):
         psi = li.gaussian_spinor(202 + parity, vh, d)
         want = oracle.dphi_eo(dims, BC_T, R, parity, psi)
         gin = _put(prob, psi, 1 - parity)
-        for variant in (0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10):
+        for variant in (0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11):
             try:
                 prob.lat.set_tuning("variant", variant)
                 out = _new(prob)

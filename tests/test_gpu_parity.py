@@ -123,7 +123,7 @@ def test_dphi_eo_boundaries_and_small_extents(hr, dims, bc, parity):
     prob.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("N,rep", [(2, "fund"), (3, "fund"), (2, "adj"), (3, "sym"), (3, "adj"), (4, "sym"), (4, "adj")])
 def test_every_kernel_variant_matches_oracle(hr, N, rep, prec, variant):

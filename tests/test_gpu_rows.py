@@ -48,7 +48,7 @@ def test_dphi_eo_from_row_compressed_links(hr, dims, bc, N, rep, prec):
         want = oracle.dphi_eo(dims, bc, R, parity, psi)
         gin = prob.lat.spinor(prob.prec)
         prob.lat.import_spinor(gin, prob.prec, psi, 1 - parity)
-        for variant in (-1, 0, 1, 2, 3, 4, 5, 7, 9, 10):
+        for variant in (-1, 0, 1, 2, 3, 4, 5, 7, 9, 10, 11):
             try:
                 prob.lat.set_tuning("variant", variant)
                 out = prob.lat.spinor(prob.prec)

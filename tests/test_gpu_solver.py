@@ -136,7 +136,7 @@ def test_dhat_matches_oracle(hr, dims, N, rep, g5, prec):
     assert hr.hr_launch_count() == n0 + 2          # two Dphi launches, diagonal term and gamma5 fused
     assert rel_l2(f.get(out), want) <= TOL[prec]
     # every kernel variant computes the same operator
-    for variant in (0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10):
+    for variant in (0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11):
         try:
             prob.lat.set_tuning("variant", variant)
             out2 = f.new()
