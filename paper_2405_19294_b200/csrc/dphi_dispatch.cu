@@ -20,6 +20,9 @@ static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "sit
 // can the bulk kernel (variants 7 / 8, ks consumer threads per site) tile this lattice?
 static bool bulk_ok(const hr_ctx *c, hr_prec prec, int lk, int ks)
 {
+    // a persistent kernel wants several tiles per CTA: below 2^17 sites per parity (1024 tiles of 128) the defaults stay
+    // with the site / colour kernels (an explicitly chosen variant 7-10 runs on any lattice it can tile)
+    if (c->Vh < (1L << 17)) return false;
     DphiArgs a = {};
     a.T = c->dims[0]; a.X = c->dims[1]; a.Y = c->dims[2]; a.Zh = c->dims[3] / 2; a.vh = c->Vh;
 #define X(D, LK)                                                                                          \

@@ -3,6 +3,9 @@
 // (cudaGetDriverEntryPoint) so that libhr.so carries no link-time dependency on libcuda.
 #include <cuda.h>
 
+#include <cstring>
+#include <mutex>
+
 #include "hr_internal.h"
 
 namespace hr {
@@ -28,7 +31,34 @@ static encode_tiled_fn get_encode()
 // fields `field_stride` bytes apart (1 for a spinor half field; 8 for a gauge field).  Elements are 8-byte words (two per
 // site and plane); a box is `box_sites` consecutive sites of all planes of one field, landing in shared memory as
 // [plane][box_sites] 16-byte vectors.
+// Encoding is a pure function of its arguments and costs a driver call (microseconds, which a solver on a small lattice
+// would pay six times per launch): the last 64 descriptors are kept.
+struct MapKey { const void *base; size_t vh, field_stride; int nplanes, nfields, box; };
+static hr_status encode_uncached(void *map64, const void *base, size_t vh, int nplanes, int nfields, size_t field_stride, int box_sites);
+
 hr_status encode_plane_map(void *map64, const void *base, size_t vh, int nplanes, int nfields, size_t field_stride, int box_sites)
+{
+    static std::mutex mtx;
+    static MapKey keys[64];
+    static CUtensorMap maps[64];   // (CUtensorMap is declared 64-byte aligned)
+    static int used = 0, next = 0;
+    const MapKey k = { base, vh, field_stride, nplanes, nfields, box_sites };
+    std::lock_guard<std::mutex> lock(mtx);
+    for (int i = 0; i < used; ++i)
+        if (keys[i].base == k.base && keys[i].vh == k.vh && keys[i].field_stride == k.field_stride && keys[i].nplanes == k.nplanes &&
+            keys[i].nfields == k.nfields && keys[i].box == k.box) {
+            memcpy(map64, &maps[i], sizeof(CUtensorMap));
+            return HR_OK;
+        }
+    hr_status rc = encode_uncached(map64, base, vh, nplanes, nfields, field_stride, box_sites);
+    if (rc != HR_OK) return rc;
+    const int slot = used < 64 ? used++ : (next = (next + 1) % 64);
+    keys[slot] = k;
+    memcpy(&maps[slot], map64, sizeof(CUtensorMap));
+    return HR_OK;
+}
+
+static hr_status encode_uncached(void *map64, const void *base, size_t vh, int nplanes, int nfields, size_t field_stride, int box_sites)
 {
     encode_tiled_fn enc = get_encode();
     if (!enc) { set_error("bulk kernel: cuTensorMapEncodeTiled is not available from this driver"); return HR_EUNSUPPORTED; }
