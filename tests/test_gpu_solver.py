@@ -201,6 +201,55 @@ def test_cg_dhat_fp32_reaches_single_precision(hr):
     prob.close()
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_cg_dhat_dist_single_rank_follows_the_oracle_and_its_edge_cases(hr, prec):
+    """hr_cg_dhat_dist (the CG with the operator and the all-reduce as callbacks; every recurrence in libhr) on ONE rank,
+    where the distributed Dphi_eo is the plain hr_dphi_eo: iteration by iteration the oracle's CG (reading C21)."""
+    import torch
+    dims, N, m0 = (4, 4, 4, 8), 3, -0.3
+    U = li.haar_links(131, N, dims)
+    vh = li.volume(dims) // 2
+    b = li.gaussian_spinor(132, vh, 3)
+    prob = GpuProblem(hr, dims, N, "fund", prec, U)
+    f = Fields(hr, prob)
+    gb, gx = f.put(b), f.new()
+    ws = torch.empty(hr.hr_cg_dist_workspace_bytes(prob.lat.ctx, f.P), dtype=torch.uint8, device="cuda")
+    calls = []
+
+    def dphi(out, inp, parity):
+        calls.append(parity)
+        hr.hr_dphi_eo(out, inp, prob.links, parity, prob.lat.stream())
+
+    tol, maxit = (1e-10, 400) if prec == "f64" else (1e-5, 400)
+    x_o, it_o, hist_o = solver.cg_dhat(dims, BC_T, U, m0, b, tol, maxit)
+    it, hist = hr.hr_cg_dhat_dist(prob.lat.ctx, f.P, m0, gx, gb, tol, maxit, ws, dphi, None, prob.lat.stream())
+    assert abs(it - it_o) <= (1 if prec == "f64" else 2)
+    n = min(it, it_o, 8)
+    assert np.allclose(hist[:n + 1], hist_o[:n + 1], rtol=1e-6 if prec == "f64" else 1e-2)
+    assert rel_l2(f.get(gx), x_o) <= (1e-8 if prec == "f64" else 1e-3)
+    assert len(calls) == 2 + 4 * it and calls[:4] == [1, 0, 1, 0]        # rhs: one gamma5 Dhat (two Dphi_eo); per iteration two
+    # an all-reduce that doubles every sum is what two identical ranks would see: |rhs|^2, <p, Ap>, |r|^2 all scale, the
+    # iterates do not
+    it2, hist2 = hr.hr_cg_dhat_dist(prob.lat.ctx, f.P, m0, gx, gb, tol, maxit, ws, dphi, lambda v: [2.0 * t for t in v], prob.lat.stream())
+    assert it2 == it and np.allclose(hist2, hist, rtol=1e-12)
+    # edge cases: maxiter = 0, b = 0, tol >= 1
+    it0, h0 = hr.hr_cg_dhat_dist(prob.lat.ctx, f.P, m0, gx, gb, tol, 0, ws, dphi, None, prob.lat.stream())
+    assert it0 == 0 and h0 == [1.0] and not f.get(gx).any()
+    gz = f.put(np.zeros_like(b))
+    it0, h0 = hr.hr_cg_dhat_dist(prob.lat.ctx, f.P, m0, gx, gz, tol, 50, ws, dphi, None, prob.lat.stream())
+    assert it0 == 0 and h0 == [0.0] and not f.get(gx).any()
+    it0, _ = hr.hr_cg_dhat_dist(prob.lat.ctx, f.P, m0, gx, gb, 1.0, 50, ws, dphi, None, prob.lat.stream())
+    assert it0 == 0
+    # a failing callback surfaces as the Python exception, not as a crash across the C frames
+    def broken(out, inp, parity):
+        raise RuntimeError("exchange failed")
+    with pytest.raises(RuntimeError):
+        hr.hr_cg_dhat_dist(prob.lat.ctx, f.P, m0, gx, gb, tol, 5, ws, broken, None, prob.lat.stream())
+    with pytest.raises(hr.HrError):
+        hr.hr_cg_dhat_dist(prob.lat.ctx, f.P, m0, gb, gb, tol, 5, ws, dphi, None, prob.lat.stream())      # x aliases b
+    prob.close()
+
+
 def test_cg_edge_cases(hr):
     dims, N, m0 = (4, 4, 4, 4), 2, -0.4
     U = li.haar_links(5, N, dims)
