@@ -336,6 +336,12 @@ size_t hr_halo_bytes(const hr_ctx *ctx, hr_prec prec);
 size_t hr_face_bytes(const hr_ctx *ctx, hr_prec prec, int mu);
 hr_status hr_dphi_eo_face_pack(int mu, void *send_up, void *send_dn, const void *in, const hr_gauge *links, int parity,
                                void *stream);
+/* hr_dphi_eo_faces_pack -- hr_dphi_eo_face_pack for ALL split directions (bit mu of split_mask) in ONE launch: the faces of a
+ * 4-D block decomposition are packed from the same input field, and four launches of 7-40 us were
+ * launch-bound.  send_up[mu] / send_dn[mu]: the two messages of direction mu (device or peer memory, hr_face_bytes each);
+ * entries of unsplit directions are ignored.  Results are bitwise those of the per-direction calls. */
+hr_status hr_dphi_eo_faces_pack(int split_mask, void *const send_up[4], void *const send_dn[4], const void *in, const hr_gauge *links,
+                                int parity, void *stream);
 hr_status hr_dphi_eo_interior_mask(void *out, const void *in, const hr_gauge *links, int parity, int split_mask, void *stream);
 hr_status hr_dphi_eo_face_apply(int mu, void *out, const void *recv_prev, const void *recv_next, const hr_gauge *links,
                                 int parity, int first_rank, int last_rank, void *stream);

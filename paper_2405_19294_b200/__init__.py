@@ -90,6 +90,7 @@ _SIGNATURES = {
     "hr_halo_bytes": (_sz, [_vp, _ci]),
     "hr_face_bytes": (_sz, [_vp, _ci, _ci]),
     "hr_dphi_eo_face_pack": (_ci, [_ci, _vp, _vp, _vp, _vp, _ci, _vp]),
+    "hr_dphi_eo_faces_pack": (_ci, [_ci, ctypes.POINTER(_vp), ctypes.POINTER(_vp), _vp, _vp, _ci, _vp]),
     "hr_dphi_eo_interior_mask": (_ci, [_vp, _vp, _vp, _ci, _ci, _vp]),
     "hr_dphi_eo_face_apply": (_ci, [_ci, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _vp]),
     "hr_halo_buffers_alloc": (_ci, [_vp, _ci, ctypes.POINTER(_vp)]),
@@ -403,6 +404,15 @@ def hr_face_bytes(ctx: int, prec: int, mu: int) -> int:
 
 def hr_dphi_eo_face_pack(mu: int, send_up, send_dn, inp, links: int, parity: int, stream: int = 0) -> None:
     _check(_lib.hr_dphi_eo_face_pack(mu, _ptr(send_up), _ptr(send_dn), _ptr(inp), links, parity, stream))
+
+
+def hr_dphi_eo_faces_pack(split_mask: int, send_up: dict, send_dn: dict, inp, links: int, parity: int, stream: int = 0) -> None:
+    """send_up / send_dn: {mu: buffer} for the split directions (bits of split_mask)."""
+    up, dn = (_vp * 4)(), (_vp * 4)()
+    for mu in range(4):
+        up[mu] = _ptr(send_up.get(mu)) or None
+        dn[mu] = _ptr(send_dn.get(mu)) or None
+    _check(_lib.hr_dphi_eo_faces_pack(split_mask, up, dn, _ptr(inp), links, parity, stream))
 
 
 def hr_dphi_eo_interior_mask(out, inp, links: int, parity: int, split_mask: int, stream: int = 0) -> None:

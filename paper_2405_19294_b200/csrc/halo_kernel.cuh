@@ -61,14 +61,14 @@ template <int MU> struct HopTable {
     static constexpr int P1 = 5 - P0;
 };
 
+// both messages of face site f of direction MU
 template <typename Real, int D, int LK, int MU>
-__global__ void __launch_bounds__(128) halo_pack_kernel(const HaloArgs a)
+__device__ __forceinline__ void halo_pack_site(const HaloArgs &a, long f)
 {
     constexpr int LNREAL = LinkGeom<LK, D>::NREAL;
     constexpr int RPV = 16 / (int)sizeof(Real);
     constexpr size_t LB = (size_t)LNREAL * sizeof(Real);
     using H = HopTable<MU>;
-    const long f = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (f >= a.nface) return;
     const size_t vh = (size_t)a.vh, nf = (size_t)a.nface;
     const char *in = (const char *)a.in;
@@ -104,6 +104,35 @@ __global__ void __launch_bounds__(128) halo_pack_kernel(const HaloArgs a)
 #pragma unroll
         for (int c = 0; c < 2 * D; ++c) { chi[c] = c0[c]; chi[2 * D + c] = c1[c]; }
         store_planes<ST_DEFAULT, 4 * D / RPV>((char *)a.send_up + (size_t)f * 16, nf * 16, chi);
+    }
+}
+
+template <typename Real, int D, int LK, int MU>
+__global__ void __launch_bounds__(128) halo_pack_kernel(const HaloArgs a)
+{
+    halo_pack_site<Real, D, LK, MU>(a, (long)blockIdx.x * blockDim.x + threadIdx.x);
+}
+
+// the faces of ALL split directions in one launch (a 4-D block decomposition packs up to four directions from the same
+// input field: four launches of 7-40 us each were launch-bound).  The CTAs of direction
+// k are [first[k], first[k+1]): a CTA never straddles two directions, the switch is uniform.
+struct HaloMultiArgs {
+    HaloArgs a[4];
+    unsigned first[5];
+    int mu[4];
+    int ndir;
+};
+template <typename Real, int D, int LK>
+__global__ void __launch_bounds__(128) halo_pack_multi_kernel(const __grid_constant__ HaloMultiArgs g)
+{
+    int k = 0;
+    while (k + 1 < g.ndir && blockIdx.x >= g.first[k + 1]) ++k;
+    const long f = (long)(blockIdx.x - g.first[k]) * blockDim.x + threadIdx.x;
+    switch (g.mu[k]) {
+    case 0: halo_pack_site<Real, D, LK, 0>(g.a[k], f); break;
+    case 1: halo_pack_site<Real, D, LK, 1>(g.a[k], f); break;
+    case 2: halo_pack_site<Real, D, LK, 2>(g.a[k], f); break;
+    default: halo_pack_site<Real, D, LK, 3>(g.a[k], f); break;
     }
 }
 

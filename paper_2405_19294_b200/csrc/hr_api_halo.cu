@@ -79,6 +79,34 @@ hr_status hr_dphi_eo_face_pack(int mu, void *send_up, void *send_dn, const void 
     return launch_halo(links->ctx, links->prec, true, mu, a, (cudaStream_t)stream, link_src(links));
 }
 
+hr_status hr_dphi_eo_faces_pack(int split_mask, void *const send_up[4], void *const send_dn[4], const void *in, const hr_gauge *links,
+                                int parity, void *stream)
+{
+    hr_status rc = check_links("hr_dphi_eo_faces_pack", links, parity);
+    if (rc != HR_OK) return rc;
+    if (split_mask <= 0 || split_mask > 15 || !send_up || !send_dn || !in || !aligned16(in)) {
+        set_error("hr_dphi_eo_faces_pack: bad argument (split_mask 1..15, non-NULL buffers)");
+        return HR_EINVAL;
+    }
+    HaloArgs a[4];
+    int mus[4], n = 0;
+    for (int mu = 0; mu < 4; ++mu) {
+        if (!(split_mask & (1 << mu))) continue;
+        rc = check_mu("hr_dphi_eo_faces_pack", links, mu);
+        if (rc != HR_OK) return rc;
+        if (!send_up[mu] || !send_dn[mu] || !aligned16(send_up[mu]) || !aligned16(send_dn[mu]) || send_up[mu] == send_dn[mu]) {
+            set_error("hr_dphi_eo_faces_pack: buffers of direction %d must be distinct, non-NULL and 16-byte aligned", mu);
+            return HR_EINVAL;
+        }
+        halo_common(a[n], links->ctx, links, parity, mu);
+        a[n].send_up = send_up[mu];
+        a[n].send_dn = send_dn[mu];
+        a[n].in = in;
+        mus[n++] = mu;
+    }
+    return launch_halo_pack_multi(links->ctx, links->prec, a, mus, n, (cudaStream_t)stream, link_src(links));
+}
+
 hr_status hr_dphi_eo_interior(void *out, const void *in, const hr_gauge *links, int parity, void *stream)
 {
     return hr_dphi_eo_interior_mask(out, in, links, parity, 1, stream);

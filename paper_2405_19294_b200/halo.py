@@ -265,9 +265,9 @@ class BlockDphi:
         self.xch = AsyncExchange(dev, group)
 
     def pack(self, inp, links: int, parity: int) -> None:
-        from . import hr_dphi_eo_face_pack
-        for mu, (su, sd, _, _) in self.buf.items():
-            hr_dphi_eo_face_pack(mu, su, sd, inp, links, parity, self.lat.stream())
+        from . import hr_dphi_eo_faces_pack
+        hr_dphi_eo_faces_pack(self.plan["mask"], {mu: b[0] for mu, b in self.buf.items()}, {mu: b[1] for mu, b in self.buf.items()},
+                              inp, links, parity, self.lat.stream())         # all split directions in one launch
 
     def interior(self, out, inp, links: int, parity: int) -> None:
         from . import hr_dphi_eo_interior_mask
@@ -326,13 +326,13 @@ class PeerBlockDphi:
     fence = PeerSlabDphi.fence
 
     def dphi_eo(self, out, inp, links: int, parity: int) -> None:
-        from . import hr_dphi_eo_face_apply, hr_dphi_eo_face_pack, hr_dphi_eo_interior_mask
+        from . import hr_dphi_eo_face_apply, hr_dphi_eo_faces_pack, hr_dphi_eo_interior_mask
         st = self.lat.stream()
         k = self.calls & 1
         self.calls += 1
-        for mu in self.plan["split"]:              # my "up" message is the next rank's recv_prev[k], "down" the previous rank's recv_next[k]
-            nb = self.nb[mu]
-            hr_dphi_eo_face_pack(mu, self.next_base[mu] + (2 + 2 * k) * nb, self.prev_base[mu] + (3 + 2 * k) * nb, inp, links, parity, st)
+        # my "up" message is the next rank's recv_prev[k], "down" the previous rank's recv_next[k]; all directions in one launch
+        hr_dphi_eo_faces_pack(self.plan["mask"], {mu: self.next_base[mu] + (2 + 2 * k) * self.nb[mu] for mu in self.plan["split"]},
+                              {mu: self.prev_base[mu] + (3 + 2 * k) * self.nb[mu] for mu in self.plan["split"]}, inp, links, parity, st)
         hr_dphi_eo_interior_mask(out, inp, links, parity, self.plan["mask"], st)
         self.fence()
         for mu in self.plan["split"]:

@@ -124,3 +124,37 @@ def test_single_rank_block_in_one_direction_reproduces_dphi_eo(hr, mu):
         hr.hr_dphi_eo_face_apply(mu, out, up, dn, prob.links, parity, True, True, st)
         assert rel_l2(prob.lat.export_spinor(out, prob.prec, parity), oracle.dphi_eo(dims, bc, U, parity, psi)) <= TOL["f64"]
     prob.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("N,rep", [(3, "fund"), (2, "adj"), (3, "sym")])
+@pytest.mark.parametrize("mask", [1, 6, 9, 15])
+def test_fused_pack_of_all_directions_is_bitwise_the_per_direction_packs(hr, N, rep, mask, prec):
+    """hr_dphi_eo_faces_pack (one launch for every split direction) against hr_dphi_eo_face_pack direction by direction:
+    the same bytes in every message buffer, with ragged face counts (faces that are no multiple of the CTA size)."""
+    import torch
+    dims = (4, 6, 4, 10)
+    U = li.haar_links(901, N, dims)
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    vh = li.volume(dims) // 2
+    prob = GpuProblem(hr, dims, N, rep, prec, U)
+    lat, P, st = prob.lat, prob.prec, prob.lat.stream()
+    for parity in (0, 1):
+        gin = lat.spinor(P)
+        lat.import_spinor(gin, P, li.gaussian_spinor(902 + parity, vh, d), 1 - parity)
+        split = [mu for mu in range(4) if mask & (1 << mu)]
+        one = {mu: [torch.full((hr.hr_face_bytes(lat.ctx, P, mu),), 0xFF, dtype=torch.uint8, device="cuda") for _ in range(2)] for mu in split}
+        all_ = {mu: [torch.full((hr.hr_face_bytes(lat.ctx, P, mu),), 0xFF, dtype=torch.uint8, device="cuda") for _ in range(2)] for mu in split}
+        for mu in split:
+            hr.hr_dphi_eo_face_pack(mu, one[mu][0], one[mu][1], gin, prob.links, parity, st)
+        n0 = hr.hr_launch_count()
+        hr.hr_dphi_eo_faces_pack(mask, {mu: all_[mu][0] for mu in split}, {mu: all_[mu][1] for mu in split}, gin, prob.links, parity, st)
+        assert hr.hr_launch_count() == n0 + 1
+        for mu in split:
+            for k in (0, 1):
+                assert torch.equal(one[mu][k], all_[mu][k]), (mu, k)
+    with pytest.raises(hr.HrError):
+        hr.hr_dphi_eo_faces_pack(0, {}, {}, gin, prob.links, 0, st)                       # nothing to pack
+    with pytest.raises(hr.HrError):
+        hr.hr_dphi_eo_faces_pack(2, {}, {}, gin, prob.links, 0, st)                       # NULL buffers of a split direction
+    prob.close()
