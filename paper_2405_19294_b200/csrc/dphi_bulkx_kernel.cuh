@@ -11,8 +11,9 @@
 //  * a TILE is R z-rows (n = R * Zh sites) of one (t, x); a CTA processes a STRIP of Lx tiles x0 .. x0+Lx-1 at fixed
 //    (t, y0).  The input spinors of the time-slice live in BLOCKS: block(x) = rows y0-1 .. y0+R of column x (the R rows
 //    of the tile plus one halo row on either side: three TMA boxes).  Tile x reads block(x-1) for the -x hop, block(x+1)
-//    for the +x hop and block(x) for the +-y and +-z hops; moving on to x+1 only block(x+2) is new.  Four block slots
-//    (three live, one being filled) form a ring of their own.
+//    for the +x hop and block(x) for the +-y and +-z hops; moving on to x+1 only block(x+2) is new.  Three block slots
+//    form a ring of their own: the slot of block(x-1) is released right after the -x hop of tile x and refilled with
+//    block(x+2) while the +-y, +-z hops of this tile and the +-t hops of the next one run.
 //  * the +-t neighbours (no re-use inside a time-slice) and the eight links of a site go through per-hop rings exactly
 //    as in dphi_bulk_kernel.cuh.
 //  * spinor bytes through the crossbar per site: (1 + 2/R)(1 + 2/Lx) + 2 spinors instead of 8.
@@ -34,7 +35,7 @@ struct BulkxArgs {
     unsigned block_bytes, tslot_bytes, lslot_bytes;
 };
 
-enum { BULKX_NB = 4 };    // block slots: x-1, x, x+1 live + one being filled
+enum { BULKX_NB = 3 };    // block slots: x-1, x, x+1; the slot of x-1 is released right after the -x hop and refilled with x+2
 
 template <typename Real, int D, int LK> struct BulkxGeom {
     using G = BulkGeom<Real, D, LK>;
@@ -67,7 +68,7 @@ dphi_bulkx_kernel(const DphiArgs a, const BulkxArgs g, const __grid_constant__ B
     unsigned char *tsl0 = blk0 + (size_t)BULKX_NB * g.block_bytes;
     unsigned char *lsl0 = tsl0 + (size_t)nt * g.tslot_bytes;
     uint64_t *bars = reinterpret_cast<uint64_t *>(lsl0 + (size_t)nl * g.lslot_bytes);
-    // barriers: [full_b 4][empty_b 4][full_t nt][empty_t nt][full_l nl][empty_l nl]
+    // barriers: [full_b NB][empty_b NB][full_t nt][empty_t nt][full_l nl][empty_l nl]
     const uint32_t fullb = smem_addr(bars), emptyb = fullb + 8 * BULKX_NB;
     const uint32_t fullt = emptyb + 8 * BULKX_NB, emptyt = fullt + 8 * nt;
     const uint32_t fulll = emptyt + 8 * nt, emptyl = fulll + 8 * nl;
@@ -97,7 +98,9 @@ dphi_bulkx_kernel(const DphiArgs a, const BulkxArgs g, const __grid_constant__ B
         y0 = yb * R;
     };
 
-    unsigned qb = 0;                      // block sequence number: slot = q & 3, phase = (q >> 2) & 1
+    unsigned qb = 0;                      // block sequence number: slot = q % NB, phase = (q / NB) & 1
+    auto bslot = [](unsigned q) { return q % (unsigned)BULKX_NB; };
+    auto bphase = [](unsigned q) { return (q / (unsigned)BULKX_NB) & 1u; };
     int ts = 0, ls = 0;                   // slots of the +-t ring and of the link ring
     uint32_t tph = 0, lph = 0;
     auto adv_t = [&]() { if (++ts == nt) { ts = 0; tph ^= 1u; } };
@@ -118,8 +121,8 @@ dphi_bulkx_kernel(const DphiArgs a, const BulkxArgs g, const __grid_constant__ B
                 auto issue_block = [&](int xx) {
                     const int xw = xx < 0 ? xx + a.X : (xx >= a.X ? xx - a.X : xx);
                     const long col = ((long)t * a.X + xw) * a.Y;
-                    const unsigned slot = qb & 3u;
-                    mbar_wait(emptyb + 8 * slot, ((qb >> 2) & 1u) ^ 1u);
+                    const unsigned slot = bslot(qb);
+                    mbar_wait(emptyb + 8 * slot, bphase(qb) ^ 1u);
                     const uint32_t fb = fullb + 8 * slot;
                     mbar_arrive_expect_tx(fb, blk_tx);
                     const uint32_t dst = smem_addr(blk0 + (size_t)slot * g.block_bytes);
@@ -194,15 +197,15 @@ dphi_bulkx_kernel(const DphiArgs a, const BulkxArgs g, const __grid_constant__ B
             decode(strip, t, x0, y0);
             const int y = y0 + row;
             // the first two blocks of the strip
-            mbar_wait(fullb + 8 * (qb & 3u), (qb >> 2) & 1u);
-            mbar_wait(fullb + 8 * ((qb + 1) & 3u), ((qb + 1) >> 2) & 1u);
+            mbar_wait(fullb + 8 * bslot(qb), bphase(qb));
+            mbar_wait(fullb + 8 * bslot(qb + 1), bphase(qb + 1));
             for (int jx = 0; jx < g.Lx; ++jx, ++qb) {
                 const int x = x0 + jx;
                 const int b = (t + x + y + a.parity) & 1;
                 const size_t s = (size_t)((((long)t * a.X + x) * a.Y + y0) * Zh + i);
-                const unsigned char *blk_m = blk0 + (size_t)(qb & 3u) * g.block_bytes;          // column x-1
-                const unsigned char *blk_c = blk0 + (size_t)((qb + 1) & 3u) * g.block_bytes;    // column x
-                const unsigned char *blk_p = blk0 + (size_t)((qb + 2) & 3u) * g.block_bytes;    // column x+1
+                const unsigned char *blk_m = blk0 + (size_t)bslot(qb) * g.block_bytes;          // column x-1
+                const unsigned char *blk_c = blk0 + (size_t)bslot(qb + 1) * g.block_bytes;      // column x
+                const unsigned char *blk_p = blk0 + (size_t)bslot(qb + 2) * g.block_bytes;      // column x+1
 
                 // accumulators: KS = 1: acc[0..3] = out_0..3.  KS = 2: acc[0] -> out_k, acc[1] -> out_{k+2} (mu = 0,3),
                 // acc[2] -> out_{3-k} (mu = 1,2; handed to the partner lane at the end)
@@ -226,7 +229,7 @@ dphi_bulkx_kernel(const DphiArgs a, const BulkxArgs g, const __grid_constant__ B
                         sp = tsl0 + (size_t)ts * g.tslot_bytes + (size_t)i * 16;
                     } else if constexpr (MU == 1) {
                         sign = (DIR == 0 ? x == a.X - 1 : x == 0) ? a.bc[1] : 1;
-                        if constexpr (DIR == 0) mbar_wait(fullb + 8 * ((qb + 2) & 3u), ((qb + 2) >> 2) & 1u);   // the new block
+                        if constexpr (DIR == 0) mbar_wait(fullb + 8 * bslot(qb + 2), bphase(qb + 2));   // the new block
                         sp = (DIR == 0 ? blk_p : blk_m) + halo_b + (size_t)i * 16;
                     } else if constexpr (MU == 2) {
                         sign = (DIR == 0 ? y == a.Y - 1 : y == 0) ? a.bc[2] : 1;
@@ -275,6 +278,7 @@ dphi_bulkx_kernel(const DphiArgs a, const BulkxArgs g, const __grid_constant__ B
                         if (lane == 0) {
                             mbar_arrive(emptyl + 8 * ls);
                             if constexpr (MU == 0) mbar_arrive(emptyt + 8 * ts);
+                            if constexpr (MU == 1 && DIR == 1) mbar_arrive(emptyb + 8 * bslot(qb));   // column x-1: last use
                         }
                     };
                     if constexpr (KS == 1) {
@@ -314,11 +318,10 @@ dphi_bulkx_kernel(const DphiArgs a, const BulkxArgs g, const __grid_constant__ B
                 hop(I2{}, I0{}); hop(I2{}, I1{});
                 hop(I3{}, I0{}); hop(I3{}, I1{});
 
-                // column x-1 is done with (at the end of a strip: all three)
-                __syncwarp();
-                if (lane == 0) {
-                    mbar_arrive(emptyb + 8 * (qb & 3u));
-                    if (jx == g.Lx - 1) { mbar_arrive(emptyb + 8 * ((qb + 1) & 3u)); mbar_arrive(emptyb + 8 * ((qb + 2) & 3u)); }
+                // at the end of a strip the other two blocks are done with as well
+                if (jx == g.Lx - 1) {
+                    __syncwarp();
+                    if (lane == 0) { mbar_arrive(emptyb + 8 * bslot(qb + 1)); mbar_arrive(emptyb + 8 * bslot(qb + 2)); }
                 }
 
                 // epilogue (a6): as dphi_kernel
@@ -413,9 +416,9 @@ static bool bulkx_geometry(const DphiArgs &a, BulkxArgs &g, size_t smem_max, int
     for (int r = 1; r <= a.Y; ++r) {
         if (a.Y % r) continue;
         if (r * a.Zh > maxn) break;
-        // four block slots + at least 2 +-t slots and 4 link slots
+        // the block slots + at least 2 +-t slots and 3 link slots
         const size_t need = (size_t)BULKX_NB * GX::block_bytes(r * a.Zh, a.Zh) + 2 * (size_t)GX::tslot_bytes(r * a.Zh) +
-                            4 * (size_t)GX::lslot_bytes(r * a.Zh) + 512;
+                            3 * (size_t)GX::lslot_bytes(r * a.Zh) + 512;
         if (need > smem_max) break;
         if (want_rows > 0 && r > want_rows) break;
         R = r;
@@ -440,8 +443,8 @@ static bool bulkx_geometry(const DphiArgs &a, BulkxArgs &g, size_t smem_max, int
     g.lslot_bytes = GX::lslot_bytes(g.n);
     // the rest of shared memory goes to the two rings (a tile uses 2 +-t slots and 8 link slots): the deepest pair that fits
     const size_t rest = smem_max - 512 - (size_t)BULKX_NB * g.block_bytes;
-    static const int kRings[][2] = { { 2, 4 }, { 2, 5 }, { 2, 6 }, { 3, 6 }, { 3, 7 }, { 3, 8 }, { 3, 9 }, { 4, 9 }, { 4, 10 }, { 4, 11 }, { 4, 12 } };
-    int nt = 2, nl = 4;
+    static const int kRings[][2] = { { 2, 3 }, { 2, 4 }, { 2, 5 }, { 2, 6 }, { 3, 6 }, { 3, 7 }, { 3, 8 }, { 3, 9 }, { 4, 9 }, { 4, 10 }, { 4, 11 }, { 4, 12 } };
+    int nt = 2, nl = 3;
     for (const auto &rg : kRings)
         if ((size_t)rg[0] * g.tslot_bytes + (size_t)rg[1] * g.lslot_bytes <= rest) { nt = rg[0]; nl = rg[1]; }
     g.nt = nt;
