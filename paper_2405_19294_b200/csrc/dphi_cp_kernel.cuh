@@ -80,8 +80,13 @@ template <typename Real, int D, bool RL> struct CpGeom {
     static constexpr int EPV = RPV / C;              // link elements per 16-byte vector
     // colour rows per thread: 2 when that turns the spinor entries (fp32) and the column entries of a backward hop
     // (fp32 complex, fp64 real) into whole 16-byte vectors -- needs an even d_R; 1 otherwise
+// rows per thread at odd d_R divisible by 3 with real fp64 links (SU(4) adjoint): 3 was measured (a third of the h reads):
+// 0.333 -> 0.626 ms -- 255 registers, 400 bytes of spills and 5 warps per SM -- so 1
+#ifndef HR_CP_RPT_ODD
+#define HR_CP_RPT_ODD 1
+#endif
 #ifndef HR_CP_RPT
-#define HR_CP_RPT ((D % 2 == 0 && (sizeof(Real) == 4 || RL)) ? 2 : 1)
+#define HR_CP_RPT ((D % 2 == 0 && (sizeof(Real) == 4 || RL)) ? 2 : (RL && D % 3 == 0 && D > 8 && sizeof(Real) == 8) ? HR_CP_RPT_ODD : 1)
 #endif
     static constexpr int RPT = HR_CP_RPT;
     static constexpr int NG = D / RPT;               // row groups = threads per site
@@ -117,7 +122,7 @@ template <typename Real, int D, bool RL> struct CpGeom {
 #ifndef HR_CP_REGS
 #define HR_CP_REGS 84
 #endif
-    static constexpr int REGS = HR_CP_REGS * (RPT == 2 ? 3 : 2) / 2;
+    static constexpr int REGS = RPT >= 3 ? 255 : HR_CP_REGS * (RPT == 2 ? 3 : 2) / 2;
     static constexpr int MINB = 65536 / (THREADS * REGS) < 1 ? 1 : 65536 / (THREADS * REGS);
 };
 
