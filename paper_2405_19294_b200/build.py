@@ -23,6 +23,7 @@ INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",
+    "-Xfatbin=-compress-all",     # the 46 instantiation units are 177 MB of SASS + line tables uncompressed, 60 MB compressed
     "-Xcompiler", "-fPIC",
     "-I", INCLUDE,
 ] + (os.environ.get("HR_EXTRA_NVCC_FLAGS", "").split())
