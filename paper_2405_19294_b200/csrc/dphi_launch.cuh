@@ -50,6 +50,9 @@ static constexpr bool kExperiments = false;
 // loop-invariant 64-bit addresses in local memory (2-3 STL at the top of the kernel, 2-3 LDL before the epilogue: 8-28
 // bytes per thread, L1-resident).  It does the same at a 168-register cap (checked: -DHR_MINB_128=3 gives "168 registers,
 // 8 bytes spill" -- the scheduler hoists loads until the budget is full), so the cap stays where the time is best.
+#ifndef HR_OTF32_MINB
+#define HR_OTF32_MINB 4
+#endif
 #ifndef HR_MINB_128
 #define HR_MINB_128 4
 #endif
@@ -61,7 +64,7 @@ template <typename Real, int D, int LK, int KSPLIT> struct Tune {
     static constexpr int MAXT = 128;
     // measured (profiles/): the fp32 on-the-fly kernels gain 7 % from a 128-register cap (16 warps per SM); the fp64
     // real-link d_R = 3 kernel (LIVE = 154) loses 3 % at a 168-register cap (it spills), hence the 150 threshold
-    static constexpr int MINB = ((LK == LK_SYM_OTF || LK == LK_ASYM_OTF) && sizeof(Real) == 4 && KSPLIT == 1) ? 4 :
+    static constexpr int MINB = ((LK == LK_SYM_OTF || LK == LK_ASYM_OTF) && sizeof(Real) == 4 && KSPLIT == 1) ? HR_OTF32_MINB :
                                 (LK == LK_ADJ2_ROWS && sizeof(Real) == 8 && KSPLIT == 1) ? 2 :   // as the real-link kernel it expands to
                                 LIVE <= 64 ? 8 : LIVE <= 80 ? 6 : LIVE <= 96 ? 5 : LIVE <= 128 ? HR_MINB_128 : LIVE <= 150 ? 3 : LIVE <= 255 ? 2 : 1;
 };
