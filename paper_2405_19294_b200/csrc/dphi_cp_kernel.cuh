@@ -79,42 +79,47 @@ template <typename Real, int D, bool RL> struct CpGeom {
     static constexpr int C = RL ? 1 : 2;             // reals per link element
     static constexpr int EPV = RPV / C;              // link elements per 16-byte vector
     // colour rows per thread: 2 when that turns the spinor entries (fp32) and the column entries of a backward hop
-    // (fp32 complex, fp64 real) into whole 16-byte vectors -- needs an even d_R; 1 otherwise
-// rows per thread at odd d_R divisible by 3 with real fp64 links (SU(4) adjoint): 3 was measured (a third of the h reads):
-// 0.333 -> 0.626 ms -- 255 registers, 400 bytes of spills and 5 warps per SM -- so 1
-#ifndef HR_CP_RPT_ODD
-#define HR_CP_RPT_ODD 1
+    // (fp32 complex, fp64 real) into whole 16-byte vectors -- needs an even d_R; 1 otherwise.
+    // PAD: real links of an odd d_R > 8 (SU(4) adjoint, 15 x 15) are stored with rows of LD = d_R + 1 reals (LinkGeom::LD).
+    // With RPT = 4 (fp32) / 2 (fp64) rows per thread and r0 a multiple of RPT, both a thread's rows of U (forward hop) and
+    // its RPT columns of every row of U (backward hop: rows of U^T) are whole 16-byte vectors at compile-time plane offsets
+    // from one per-thread base.  The last row group is ragged (rows 12, 13, 14 and a dummy): the dummy row loads nothing,
+    // holds zeros in the half-spinor exchange and stores nothing.
+    // Before (round 1 / early round 2: unpadded rows, RPT = 1): every link element was a 4- / 8-byte load at a run-time
+    // plane and word (12 integer instructions per load) and all 15 threads of a site re-read the 30 half-spinor entries of
+    // a hop from shared memory (7.2 KB per site and hop in fp64 against 1.8 KB of link): L1 pipe 90 % busy, 0.74 (fp64) /
+    // 0.50 (fp32; 0.55 with the links staged through shared memory by cp.async) of the copy peak.  Now, SU(4) adjoint
+    // 16^3 x 48 on the UNPADDED 8L + 2S bytes: fp64 0.333 -> 0.281 ms (0.87), fp32 0.223 -> 0.150 ms (0.82); the padded
+    // bytes cap that figure at 225 / 240 = 0.94.  Sweep (profiles/r2_large_n.md): fp64 RPT 2 / chunk 16 / 16 sites per CTA;
+    // fp32 RPT 4 / chunk 8 / 32 sites; 128 registers (100 and 84 spill: 0.75 / 0.61; RPT = 4 in fp64 needs 168: 0.85).
+#ifndef HR_CP_RPT_PAD64
+#define HR_CP_RPT_PAD64 2
+#endif
+#ifndef HR_CP_RPT_PAD32
+#define HR_CP_RPT_PAD32 4
 #endif
 #ifndef HR_CP_RPT
-#define HR_CP_RPT ((D % 2 == 0 && (sizeof(Real) == 4 || RL)) ? 2 : (RL && D % 3 == 0 && D > 8 && sizeof(Real) == 8) ? HR_CP_RPT_ODD : 1)
+#define HR_CP_RPT (PAD ? (sizeof(Real) == 8 ? HR_CP_RPT_PAD64 : HR_CP_RPT_PAD32) : (D % 2 == 0 && (sizeof(Real) == 4 || RL)) ? 2 : 1)
 #endif
+    static constexpr int LD = LinkGeom<RL ? LK_REAL : LK_COMPLEX, D>::LD;
+    static constexpr bool PAD = LD != D;
     static constexpr int RPT = HR_CP_RPT;
-    static constexpr int NG = D / RPT;               // row groups = threads per site
-    static_assert(D % RPT == 0, "rows per thread must divide d_R");
+    static constexpr int NG = (D + RPT - 1) / RPT;   // row groups = threads per site
+    static constexpr int DP = NG * RPT;              // colours in the half-spinor exchange (D, or D + dummies when PAD)
+    static_assert(D % RPT == 0 || PAD, "rows per thread must divide d_R");
+    static_assert(!PAD || (RPT % RPV == 0 && LD % RPV == 0), "padded rows: a thread's rows / columns must be whole vectors");
     // sites per CTA: a warp covers 32 sites of one row group, or (more than 12 groups, where 32 x groups threads would
-    // leave one CTA per SM alone with its barriers) 16 sites of two groups; THREADS is padded to whole warps, the padding
-    // threads shadow the last group and store nothing
+    // leave one CTA per SM alone with its barriers; fp64 PAD: measured) 16 sites of two groups; THREADS is padded to whole
+    // warps, the padding threads shadow the last group and store nothing
 #ifndef HR_CP_SITES
-#define HR_CP_SITES (NG > 12 ? 16 : 32)
+#define HR_CP_SITES ((NG > 12 || (PAD && sizeof(Real) == 8)) ? 16 : 32)
 #endif
     static constexpr int SITES = HR_CP_SITES;
     static constexpr int THREADS = (SITES * NG + 31) / 32 * 32;
     static constexpr int HB = 4;                     // hops per batch
-    // Odd d_R with sub-vector link elements (SU(4) adjoint: 15 x 15 reals) cannot be read with whole vectors from a
-    // thread's own row or column: the CTA then copies the hop's link records of its sites into shared memory with
-    // coalesced 16-byte cp.async copies (every byte of every sector used once), double-buffered so that the copy of the next
-    // hop's links runs under the arithmetic of this one, and the threads pick their elements there.
-    // Measured, SU(4) adjoint 16^3 x 48: fp32 0.244 -> 0.223 ms (0.50 -> 0.55 of the copy peak), fp64 0.333 -> 0.428 ms --
-    // so fp32 only.  What binds this kernel is not the link loads but the shared-memory data pipe they share with the
-    // half-spinor exchange: every one of the 15 threads of a site reads all 30 entries h_{k,b} of a hop (7.2 KB per site
-    // and hop in fp64 against 1.8 KB of link), 5.7 GB per launch = 0.16 ms of the pipe at 128 B per clock and SM before a
-    // single link byte moves; staging adds 3.6 KB per site and hop and a barrier per hop.  The fix is fewer h reads
-    // (several rows per thread), which at d_R = 15 = 3 x 5 leaves 5 warps per SM next to 90 KB of buffers; not done.
-    static constexpr bool STAGE = RL && (D % 2 == 1) && D > 8 && sizeof(Real) == 4;
-    static constexpr int LNREAL_ = RL ? D * D : 2 * D * D;
-    static constexpr int NVT = (LNREAL_ + RPV - 1) / RPV;   // link planes including the tail plane
-    __host__ __device__ static constexpr size_t hs_bytes() { return (size_t)HB * 2 * D * SITES * sizeof(CpPair<Real>); }
-    static constexpr size_t smem_bytes() { return hs_bytes() + (STAGE ? 2 * ((size_t)NVT * SITES * 16 + SITES * sizeof(long)) : 0); }
+    static constexpr int LNREAL_ = RL ? D * LD : 2 * D * D;
+    __host__ __device__ static constexpr size_t hs_bytes() { return (size_t)HB * 2 * DP * SITES * sizeof(CpPair<Real>); }
+    static constexpr size_t smem_bytes() { return hs_bytes(); }
     // registers: a thread's state does not grow with d_R, so the cap is chosen for occupancy (several CTAs per SM hide
     // the three barriers): HR_CP_REGS registers per thread per row
     // (measured on B200, bench_large_n: SU(4) sym d_R = 10 fp64 0.260 ms at 84, 0.275 at 160, 0.291 at 64; SU(4) adj
@@ -122,7 +127,16 @@ template <typename Real, int D, bool RL> struct CpGeom {
 #ifndef HR_CP_REGS
 #define HR_CP_REGS 84
 #endif
-    static constexpr int REGS = RPT >= 3 ? 255 : HR_CP_REGS * (RPT == 2 ? 3 : 2) / 2;
+#ifndef HR_CP_REGS_PAD   // PAD: 8 RPT accumulators + 4 RPT partial sums + one chunk of RPT x CB link elements
+#define HR_CP_REGS_PAD 128
+#endif
+    static constexpr int REGS = PAD ? HR_CP_REGS_PAD : HR_CP_REGS * (RPT == 2 ? 3 : 2) / 2;
+    // link columns per chunk of a forward hop: the whole row, or 8 when the rows are padded (two chunks of 16)
+#ifndef HR_CP_CHUNK
+#define HR_CP_CHUNK (PAD ? (sizeof(Real) == 8 ? 16 : 8) : D)
+#endif
+    static constexpr int CB = HR_CP_CHUNK;
+    static_assert(LD % CB == 0 && (!PAD || CB % RPV == 0), "the chunk must divide the row and be whole vectors");
     static constexpr int MINB = 65536 / (THREADS * REGS) < 1 ? 1 : 65536 / (THREADS * REGS);
 };
 
@@ -132,7 +146,9 @@ __global__ void __launch_bounds__((CpGeom<Real, D, RL>::THREADS), (CpGeom<Real, 
     static_assert(!RED || MASS, "the fused reduction needs the self field");
     using G = CpGeom<Real, D, RL>;
     constexpr int SITES = G::SITES, RPT = G::RPT, C = G::C, EPV = G::EPV, RPV = G::RPV;
-    constexpr int LNREAL = RL ? D * D : 2 * D * D;
+    constexpr int LNREAL = G::LNREAL_;
+    constexpr int LD = G::LD, DP = G::DP;
+    constexpr bool PAD = G::PAD;
     constexpr size_t LB = (size_t)LNREAL * sizeof(Real);
     // spinor entries of RPT consecutive colours form whole vectors?  (fp64: a complex IS a vector; fp32: pairs)
     constexpr bool SPIN_AL = (2 * RPT) % RPV == 0;
@@ -144,8 +160,6 @@ __global__ void __launch_bounds__((CpGeom<Real, D, RL>::THREADS), (CpGeom<Real, 
     if (a.skip != nullptr && *a.skip != 0) return;
     extern __shared__ __align__(16) unsigned char cp_smem[];
     CpPair<Real> *hs = reinterpret_cast<CpPair<Real> *>(cp_smem);          // [slot][k][b][site]
-    [[maybe_unused]] unsigned char *lk_sm = cp_smem + G::hs_bytes();        // STAGE: 2 x [plane][site] 16-byte vectors of one hop's links
-    [[maybe_unused]] long *sn_sm = reinterpret_cast<long *>(cp_smem + G::hs_bytes() + 2 * (size_t)G::NVT * SITES * 16);   // 2 x [site]
 
     const int sl = (int)threadIdx.x % SITES;
     const bool shadow = (int)threadIdx.x / SITES >= G::NG;
@@ -174,42 +188,6 @@ __global__ void __launch_bounds__((CpGeom<Real, D, RL>::THREADS), (CpGeom<Real, 
 #pragma unroll
         for (int al = 0; al < 4; ++al) acc[rr][al][0] = acc[rr][al][1] = 0;
 
-    // STAGE: the link records of the CTA's sites for hop (MU, DIR) -> shared-memory buffer `buf`, asynchronously.
-    // publish: row group 0 writes each site's link index (own site for a forward hop, the neighbour for a backward hop);
-    // issue (after a barrier): all threads copy [planes][sites] with 16-byte cp.async, the tail plane with 4 / 8 bytes.
-    [[maybe_unused]] auto stage_publish = [&](auto mu_c, auto dir_c, int buf) {
-        constexpr int MU = decltype(mu_c)::value;
-        constexpr int DIR = decltype(dir_c)::value;
-        if ((int)threadIdx.x < SITES) {
-            long sn; int sign;
-            neighbour<MU, DIR>(a, g, s, sn, sign);
-            sn_sm[buf * SITES + sl] = DIR == 0 ? s : sn;
-        }
-    };
-    [[maybe_unused]] auto stage_issue = [&](auto mu_c, auto dir_c, int buf) {
-        constexpr int MU = decltype(mu_c)::value;
-        constexpr int DIR = decltype(dir_c)::value;
-        constexpr int NV = LNREAL / RPV, TAILB = (LNREAL - NV * RPV) * (int)sizeof(Real);
-        const char *lbase = (DIR == 0 ? lk_own : lk_nbr) + (size_t)MU * LB * vh;
-        const uint32_t dst0 = (uint32_t)__cvta_generic_to_shared(lk_sm + (size_t)buf * G::NVT * SITES * 16);
-        for (int idx = (int)threadIdx.x; idx < G::NVT * SITES; idx += G::THREADS) {
-            const int v = idx / SITES, j = idx - v * SITES;
-            const size_t sj = (size_t)sn_sm[buf * SITES + j];
-            if (v < NV)
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst0 + (uint32_t)idx * 16u), "l"(lbase + ((size_t)v * vh + sj) * 16) : "memory");
-            else if constexpr (TAILB == 8)
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst0 + (uint32_t)idx * 16u), "l"(lbase + (size_t)NV * 16 * vh + sj * 8) : "memory");
-            else if constexpr (TAILB == 4)
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst0 + (uint32_t)idx * 16u), "l"(lbase + (size_t)NV * 16 * vh + sj * 4) : "memory");
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-    };
-    if constexpr (G::STAGE) {
-        stage_publish(std::integral_constant<int, 0>{}, std::integral_constant<int, 0>{}, 0);
-        __syncthreads();
-        stage_issue(std::integral_constant<int, 0>{}, std::integral_constant<int, 0>{}, 0);
-    }
-
     // step 1 of a hop: my colours of the neighbour spinor -> my half-spinor entries -> shared memory
     auto project = [&](auto mu_c, auto dir_c, int slot, long &sn, int &sign) {
         constexpr int MU = decltype(mu_c)::value;
@@ -221,15 +199,28 @@ __global__ void __launch_bounds__((CpGeom<Real, D, RL>::THREADS), (CpGeom<Real, 
         constexpr int P1 = 5 - P0;
         neighbour<MU, DIR>(a, g, s, sn, sign);
         Real p[4][2 * RPT];
+        if constexpr (PAD) {
+            // r0 is a multiple of RPV / 2 complex entries: entry al D + r0 + rr sits at a compile-time plane and half from
+            // the thread's base; a dummy row (r0 + rr >= D) reads nothing and contributes zeros
+            const char *inb = in + (size_t)(2 * r0 / RPV) * vh * 16;
 #pragma unroll
-        for (int al = 0; al < 4; ++al) load_elems<LD_DEFAULT, 8 * D, 2, RPT, SPIN_AL>(p[al], in, vh, (size_t)sn, al * D + r0);
+            for (int al = 0; al < 4; ++al)
+#pragma unroll
+                for (int rr = 0; rr < RPT; ++rr) {
+                    p[al][2 * rr] = 0; p[al][2 * rr + 1] = 0;
+                    if (r0 + rr < D) load_cplx<LD_DEFAULT, 8 * D>(p[al][2 * rr], p[al][2 * rr + 1], inb, vh, (size_t)sn, al * D + rr, 0);
+                }
+        } else {
+#pragma unroll
+            for (int al = 0; al < 4; ++al) load_elems<LD_DEFAULT, 8 * D, 2, RPT, SPIN_AL>(p[al], in, vh, (size_t)sn, al * D + r0);
+        }
 #pragma unroll
         for (int rr = 0; rr < RPT; ++rr) {
             CpPair<Real> h0, h1;
             add_c<CRE, CIM>(h0.re, h0.im, p[0][2 * rr], p[0][2 * rr + 1], p[P0][2 * rr], p[P0][2 * rr + 1], (Real)1);
             add_c<CRE, CIM>(h1.re, h1.im, p[1][2 * rr], p[1][2 * rr + 1], p[P1][2 * rr], p[P1][2 * rr + 1], (Real)(MU >= 2 ? -1 : 1));
-            hs[((slot * 2 + 0) * D + r0 + rr) * SITES + sl] = h0;
-            hs[((slot * 2 + 1) * D + r0 + rr) * SITES + sl] = h1;
+            hs[((slot * 2 + 0) * DP + r0 + rr) * SITES + sl] = h0;
+            hs[((slot * 2 + 1) * DP + r0 + rr) * SITES + sl] = h1;
         }
     };
     // step 2: chi_{k,r} = sum_b M_{r,b} h_{k,b},  M = U(s) (forward) or U(sn)^dagger (backward); reconstruct
@@ -243,54 +234,67 @@ __global__ void __launch_bounds__((CpGeom<Real, D, RL>::THREADS), (CpGeom<Real, 
         constexpr int P1 = 5 - P0;
         const char *lbase = (DIR == 0 ? lk_own : lk_nbr) + (size_t)MU * LB * vh;
         const size_t ls = DIR == 0 ? (size_t)s : (size_t)sn;
-        // the link elements of this thread, ul[rr][b]: rows r0+rr of U(s) (forward) or columns r0+rr of U(sn) (backward)
-        Real ul[RPT][C * D];
-        if constexpr (G::STAGE) {
-            static_assert(RPT == 1 && C == 1, "staged links: one real row per thread");
-            constexpr int H = 2 * MU + DIR;                                  // hops run in the order (mu, dir) = (0,0), (0,1), (1,0), ...
-            asm volatile("cp.async.wait_all;" ::: "memory");                 // my copies of this hop's links have landed
-            if constexpr (H < 7) stage_publish(std::integral_constant<int, (H + 1) / 2>{}, std::integral_constant<int, (H + 1) % 2>{}, (H + 1) & 1);
-            __syncthreads();                                                // everybody's copies are visible; everybody is done with hop H-1
-            if constexpr (H < 7) stage_issue(std::integral_constant<int, (H + 1) / 2>{}, std::integral_constant<int, (H + 1) % 2>{}, (H + 1) & 1);
-            const Real *lrec = reinterpret_cast<const Real *>(lk_sm + (size_t)(H & 1) * G::NVT * SITES * 16) + (size_t)sl * RPV;
-#pragma unroll
-            for (int b = 0; b < D; ++b) {
-                const int e = DIR == 0 ? r0 * D + b : b * D + r0;             // element e: plane e / RPV, word e % RPV
-                ul[0][b] = lrec[(size_t)(e / RPV) * SITES * RPV + (e % RPV)];
-            }
-        } else if constexpr (DIR == 0) {
-#pragma unroll
-            for (int rr = 0; rr < RPT; ++rr) load_elems<ROW_AL ? LD_STREAM : EH, LNREAL, C, D, ROW_AL>(ul[rr], lbase, vh, ls, (r0 + rr) * D);
-        } else {
-#pragma unroll
-            for (int b = 0; b < D; ++b) {
-                Real t[C * RPT];
-                load_elems<COL_AL ? LD_STREAM : EH, LNREAL, C, RPT, COL_AL>(t, lbase, vh, ls, b * D + r0);
-#pragma unroll
-                for (int rr = 0; rr < RPT; ++rr)
-#pragma unroll
-                    for (int c = 0; c < C; ++c) ul[rr][C * b + c] = t[C * rr + c];
-            }
-        }
+        // the link elements of this thread, ul[rr][b]: rows r0+rr of U(s) (forward) or columns r0+rr of U(sn) (backward),
+        // CB columns b at a time
+        constexpr int CB = G::CB;
         Real ch[RPT][4];                                                   // chi_0 (re, im), chi_1 (re, im)
 #pragma unroll
         for (int rr = 0; rr < RPT; ++rr) ch[rr][0] = ch[rr][1] = ch[rr][2] = ch[rr][3] = 0;
+        // PAD: per-thread bases -- rows r0.. of U start RPT * LD / RPV planes apart, columns r0.. of a row r0 / RPV planes in
+        [[maybe_unused]] const char *lrow = lbase + ((size_t)(r0 * LD / RPV) * vh + ls) * 16;
+        [[maybe_unused]] const char *lcol = lbase + ((size_t)(r0 / RPV) * vh + ls) * 16;
 #pragma unroll
-        for (int b = 0; b < D; ++b) {
-            const CpPair<Real> h0 = hs[((slot * 2 + 0) * D + b) * SITES + sl];
-            const CpPair<Real> h1 = hs[((slot * 2 + 1) * D + b) * SITES + sl];
+        for (int b0 = 0; b0 < LD; b0 += CB) {
+            Real ul[RPT][C * CB];
+            if constexpr (PAD && DIR == 0) {
 #pragma unroll
-            for (int rr = 0; rr < RPT; ++rr) {
-                if constexpr (RL) {
-                    const Real u = ul[rr][b];
-                    ch[rr][0] = fma(u, h0.re, ch[rr][0]); ch[rr][1] = fma(u, h0.im, ch[rr][1]);
-                    ch[rr][2] = fma(u, h1.re, ch[rr][2]); ch[rr][3] = fma(u, h1.im, ch[rr][3]);
-                } else {
-                    const Real ur = ul[rr][2 * b], ui = DIR == 1 ? -ul[rr][2 * b + 1] : ul[rr][2 * b + 1]; // backward: conj
-                    ch[rr][0] = fma(ur, h0.re, ch[rr][0]); ch[rr][0] = fma(-ui, h0.im, ch[rr][0]);
-                    ch[rr][1] = fma(ur, h0.im, ch[rr][1]); ch[rr][1] = fma(ui, h0.re, ch[rr][1]);
-                    ch[rr][2] = fma(ur, h1.re, ch[rr][2]); ch[rr][2] = fma(-ui, h1.im, ch[rr][2]);
-                    ch[rr][3] = fma(ur, h1.im, ch[rr][3]); ch[rr][3] = fma(ui, h1.re, ch[rr][3]);
+                for (int rr = 0; rr < RPT; ++rr) {
+#pragma unroll
+                    for (int b = 0; b < CB; ++b) ul[rr][b] = 0;
+                    if (r0 + rr < D) load_planes<LD_STREAM, CB / RPV>(ul[rr], lrow + (size_t)((rr * LD + b0) / RPV) * vh * 16, vh * 16, 0);
+                }
+            } else if constexpr (PAD) {
+#pragma unroll
+                for (int b = 0; b < CB; ++b) {
+                    if (b0 + b >= D) continue;                               // the padding column pairs with the dummy colour: nothing to add
+                    Real t[RPT];
+                    load_planes<LD_STREAM, RPT / RPV>(t, lcol + (size_t)((b0 + b) * LD / RPV) * vh * 16, vh * 16, 0);
+#pragma unroll
+                    for (int rr = 0; rr < RPT; ++rr) ul[rr][b] = t[rr];
+                }
+            } else if constexpr (DIR == 0) {
+#pragma unroll
+                for (int rr = 0; rr < RPT; ++rr)
+                    load_elems<(ROW_AL && CB == D) ? LD_STREAM : EH, LNREAL, C, CB, ROW_AL && CB == D>(ul[rr], lbase, vh, ls, (r0 + rr) * D + b0);
+            } else {
+#pragma unroll
+                for (int b = 0; b < CB; ++b) {
+                    Real t[C * RPT];
+                    load_elems<COL_AL ? LD_STREAM : EH, LNREAL, C, RPT, COL_AL>(t, lbase, vh, ls, (b0 + b) * D + r0);
+#pragma unroll
+                    for (int rr = 0; rr < RPT; ++rr)
+#pragma unroll
+                        for (int c = 0; c < C; ++c) ul[rr][C * b + c] = t[C * rr + c];
+                }
+            }
+#pragma unroll
+            for (int b = 0; b < CB; ++b) {
+                if (b0 + b >= D) continue;
+                const CpPair<Real> h0 = hs[((slot * 2 + 0) * DP + b0 + b) * SITES + sl];
+                const CpPair<Real> h1 = hs[((slot * 2 + 1) * DP + b0 + b) * SITES + sl];
+#pragma unroll
+                for (int rr = 0; rr < RPT; ++rr) {
+                    if constexpr (RL) {
+                        const Real u = ul[rr][b];
+                        ch[rr][0] = fma(u, h0.re, ch[rr][0]); ch[rr][1] = fma(u, h0.im, ch[rr][1]);
+                        ch[rr][2] = fma(u, h1.re, ch[rr][2]); ch[rr][3] = fma(u, h1.im, ch[rr][3]);
+                    } else {
+                        const Real ur = ul[rr][2 * b], ui = DIR == 1 ? -ul[rr][2 * b + 1] : ul[rr][2 * b + 1]; // backward: conj
+                        ch[rr][0] = fma(ur, h0.re, ch[rr][0]); ch[rr][0] = fma(-ui, h0.im, ch[rr][0]);
+                        ch[rr][1] = fma(ur, h0.im, ch[rr][1]); ch[rr][1] = fma(ui, h0.re, ch[rr][1]);
+                        ch[rr][2] = fma(ur, h1.re, ch[rr][2]); ch[rr][2] = fma(-ui, h1.im, ch[rr][2]);
+                        ch[rr][3] = fma(ur, h1.im, ch[rr][3]); ch[rr][3] = fma(ui, h1.re, ch[rr][3]);
+                    }
                 }
             }
         }
@@ -326,7 +330,14 @@ __global__ void __launch_bounds__((CpGeom<Real, D, RL>::THREADS), (CpGeom<Real, 
         Real o[2 * RPT];
         if constexpr (MASS) {
             Real sf[2 * RPT];
-            load_elems<LD_STREAM, 8 * D, 2, RPT, SPIN_AL>(sf, (const char *)a.self, vh, (size_t)s, al * D + r0);
+            if constexpr (PAD) {
+                const char *sb = (const char *)a.self + (size_t)(2 * r0 / RPV) * vh * 16;
+#pragma unroll
+                for (int rr = 0; rr < RPT; ++rr) {
+                    sf[2 * rr] = 0; sf[2 * rr + 1] = 0;
+                    if (r0 + rr < D) load_cplx<LD_STREAM, 8 * D>(sf[2 * rr], sf[2 * rr + 1], sb, vh, (size_t)s, al * D + rr, 0);
+                }
+            } else load_elems<LD_STREAM, 8 * D, 2, RPT, SPIN_AL>(sf, (const char *)a.self, vh, (size_t)s, al * D + r0);
             const Real alc = coef_alpha<Real>(a, al >> 1), bec = coef_beta<Real>(a, al >> 1);
 #pragma unroll
             for (int rr = 0; rr < RPT; ++rr) {
@@ -345,12 +356,25 @@ __global__ void __launch_bounds__((CpGeom<Real, D, RL>::THREADS), (CpGeom<Real, 
         }
         if (live) {
             const int e = al * D + r0;                                     // first complex entry
-            if constexpr (SPIN_AL) {
+            if constexpr (PAD) {
+                char *ob = (char *)a.out + ((size_t)(2 * r0 / RPV) * vh + (size_t)s) * 16;
+#pragma unroll
+                for (int rr = 0; rr < RPT; ++rr) {
+                    if (r0 + rr >= D) continue;
+                    constexpr int CPV = RPV / 2;                           // complex entries per vector
+                    const int ee = al * D + rr;                            // compile-time after unrolling
+                    char *q = ob + (size_t)(ee / CPV) * vh * 16 + (size_t)(ee % CPV) * (2 * sizeof(Real));
+                    if constexpr (sizeof(Real) == 8) st16<ST_DEFAULT>(q, o[2 * rr], o[2 * rr + 1]);
+                    else *reinterpret_cast<float2 *>(q) = make_float2((float)o[2 * rr], (float)o[2 * rr + 1]);
+                }
+            } else if constexpr (SPIN_AL) {
                 store_planes<ST_DEFAULT, 2 * RPT / RPV>((char *)a.out + ((size_t)(2 * e / RPV) * vh + (size_t)s) * 16, vh * 16, o);
-            } else {                                                       // fp32, one colour: half a vector
-                static_assert(sizeof(Real) == 4 && RPT == 1, "unaligned spinor entries: fp32, one row per thread");
-                *reinterpret_cast<float2 *>((char *)a.out + ((size_t)(e >> 1) * vh + (size_t)s) * 16 + (size_t)(e & 1) * 8) =
-                    make_float2((float)o[0], (float)o[1]);
+            } else {                                                       // fp32, an odd number of colours: half vectors
+                static_assert(sizeof(Real) == 4, "unaligned spinor entries: fp32 only");
+#pragma unroll
+                for (int rr = 0; rr < RPT; ++rr)
+                    *reinterpret_cast<float2 *>((char *)a.out + ((size_t)((e + rr) >> 1) * vh + (size_t)s) * 16 + (size_t)((e + rr) & 1) * 8) =
+                        make_float2((float)o[2 * rr], (float)o[2 * rr + 1]);
             }
         }
     }

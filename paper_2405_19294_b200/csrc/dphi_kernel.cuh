@@ -60,17 +60,18 @@ __device__ __forceinline__ void acc_conj_c(Real &ore, Real &oim, Real xre, Real 
     }
 }
 
-// chi = U h (DAG = false) or U^dagger h (DAG = true); U complex [D][D] (re,im) or real [D][D]
-template <int D, bool RL, bool DAG, typename Real>
+// chi = U h (DAG = false) or U^dagger h (DAG = true); U complex [D][D] (re,im) or real [D][LDM] (LDM: row stride, LinkGeom::LD)
+template <int D, bool RL, bool DAG, typename Real, int LDM = D>
 __device__ __forceinline__ void colour_mul(Real (&chi)[2 * D], const Real *u, const Real (&h)[2 * D])
 {
+    static_assert(RL || LDM == D, "padded rows: real links only");
 #pragma unroll
     for (int i = 0; i < D; ++i) {
         Real re = 0, im = 0;
 #pragma unroll
         for (int j = 0; j < D; ++j) {
             if constexpr (RL) {
-                const Real r = DAG ? u[j * D + i] : u[i * D + j];
+                const Real r = DAG ? u[j * LDM + i] : u[i * LDM + j];
                 re = fma(r, h[2 * j], re);
                 im = fma(r, h[2 * j + 1], im);
             } else {
@@ -118,7 +119,9 @@ template <int LK, int D> struct LinkGeom {
                            : LK == LK_ASYM_OTF ? (D == 3 ? 3 : D == 6 ? 4 : 0)
                            : LK == LK_ADJ2_ROWS ? (D == 3 ? 2 : 0)
                            : (LK == LK_ADJ3_OTF || LK == LK_ADJ3_ROWS) ? (D == 8 ? 3 : 0) : D;
-    static constexpr int NREAL = LK == LK_REAL ? D * D : LK == LK_COMPLEX ? 2 * D * D
+    // row stride of the represented real link: d_R + 1 for an odd d_R > 8 (hr_internal.h link_ld), the extra entry is zero
+    static constexpr int LD = (LK == LK_REAL && (D & 1) && D > 8) ? D + 1 : D;
+    static constexpr int NREAL = LK == LK_REAL ? D * LD : LK == LK_COMPLEX ? 2 * D * D
                                : (LK == LK_ROWS || LK == LK_ADJ2_ROWS || LK == LK_ADJ3_ROWS) ? 2 * N * (N - 1) : 2 * N * N;
     static_assert(N > 0, "no such two-index representation");
 };
@@ -280,7 +283,7 @@ __device__ __forceinline__ void adj3_mul(Real (&chi)[16], const Real *u, const R
 template <int D, int LK, bool DAG, typename Real>
 __device__ __forceinline__ void link_mul(Real (&chi)[2 * D], const Real *u, const Real (&h)[2 * D])
 {
-    if constexpr (LK == LK_COMPLEX || LK == LK_REAL) colour_mul<D, LK == LK_REAL, DAG>(chi, u, h);
+    if constexpr (LK == LK_COMPLEX || LK == LK_REAL) colour_mul<D, LK == LK_REAL, DAG, Real, LinkGeom<LK, D>::LD>(chi, u, h);
     else if constexpr (LK == LK_ROWS) {
         Real f[2 * D * D];
         rebuild_rows<D>(f, u);     // identical for both half-spinor components of a hop: the compiler merges the two

@@ -98,12 +98,16 @@ static hr_status transfer(const hr_ctx *c, FieldKind kind, bool import, int nrea
     rc = pointer_on_device(canon, &dev);
     if (rc != HR_OK) return rc;
     const long nsites = kind == FIELD_GAUGE ? c->V : c->Vh;
-    const size_t site_bytes = (size_t)(kind == FIELD_GAUGE ? 4 : 1) * nreal * prec_bytes(cprec);
+    // a represented real link field with padded rows (link_ld): internal rows of ld reals, canonical rows of d_R
+    const bool padded = kind == FIELD_GAUGE && link_ld(c) != c->d && nreal == c->d * link_ld(c);
+    const int ld = padded ? link_ld(c) : 0, dcol = padded ? c->d : 0;
+    const int cnreal = padded ? c->d * c->d : nreal;
+    const size_t site_bytes = (size_t)(kind == FIELD_GAUGE ? 4 : 1) * cnreal * prec_bytes(cprec);
 
     auto run = [&](void *canon_dev, long first, long n) -> hr_status {
         if (kind == FIELD_GAUGE)
-            return import ? launch_pack_gauge(c, nreal, internal, prec, canon_dev, cprec, first, n, st)
-                          : launch_unpack_gauge(c, nreal, internal, prec, canon_dev, cprec, first, n, st);
+            return import ? launch_pack_gauge(c, nreal, ld, dcol, internal, prec, canon_dev, cprec, first, n, st)
+                          : launch_unpack_gauge(c, nreal, ld, dcol, internal, prec, canon_dev, cprec, first, n, st);
         return import ? launch_pack_spinor(c, internal, prec, canon_dev, cprec, first, n, st)
                       : launch_unpack_spinor(c, internal, prec, canon_dev, cprec, first, n, st);
     };

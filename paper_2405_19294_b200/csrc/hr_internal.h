@@ -59,7 +59,7 @@ struct hr_gauge {
     void *data;
     int owns;
     size_t bytes;
-    int nreal; // reals per link
+    int nreal; // reals per link, internal record (link_nreal)
 };
 
 namespace hr {
@@ -76,11 +76,24 @@ void dphi_args(DphiArgs &a, const hr_ctx *c, void *out, const void *in, const vo
 static inline size_t prec_bytes(hr_prec p) { return p == HR_F64 ? 8 : 4; }
 // link-field kinds (hr_gauge::represented): 0 fundamental N x N, 1 represented d_R x d_R, 2 fundamental stored as its
 // first N-1 rows (the last row of an SU(N) matrix is fixed by the others; N = 2, 3)
-static inline int link_nreal(const hr_ctx *c, int represented)
+// Row stride of a represented link in the INTERNAL layout.  Real links of an odd d_R > 8 (SU(4) adjoint: 15 x 15) are kept
+// with rows of d_R + 1 reals, the last one zero: a row, and a group of 2 (fp64) / 4 (fp32) columns of a row, is then a whole
+// number of 16-byte vectors, which is what lets the colour-parallel kernel read U and U^T with vector loads
+// (dphi_cp_kernel.cuh).  +6.7 % link bytes; the canonical (import / export) record stays d_R x d_R.  LinkGeom::LD is the
+// device-side twin.
+static inline int link_ld(const hr_ctx *c) { return (c->real_links && (c->d & 1) && c->d > 8) ? c->d + 1 : c->d; }
+// reals per link of the canonical record
+static inline int link_nreal_canon(const hr_ctx *c, int represented)
 {
     if (represented == 2) return 2 * c->N * (c->N - 1);
     if (!represented) return 2 * c->N * c->N;
     return c->real_links ? c->d * c->d : 2 * c->d * c->d;
+}
+// reals per link of the internal record
+static inline int link_nreal(const hr_ctx *c, int represented)
+{
+    if (represented == 1 && c->real_links) return c->d * link_ld(c);
+    return link_nreal_canon(c, represented);
 }
 
 // ---- launch entry points implemented in the kernel translation units ----------------------------
@@ -243,9 +256,11 @@ hr_status launch_pack_spinor(const hr_ctx *c, void *dst, hr_prec prec, const voi
                              long first_site, long nsites, cudaStream_t st);
 hr_status launch_unpack_spinor(const hr_ctx *c, const void *src, hr_prec prec, void *canon_dev, hr_prec cprec,
                                long first_site, long nsites, cudaStream_t st);
-hr_status launch_pack_gauge(const hr_ctx *c, int nreal, void *dst, hr_prec prec, const void *canon_dev,
+// nreal: reals of the internal record; ld / dcol: internal row stride and canonical row length when they differ (link_ld),
+// 0 / 0 otherwise
+hr_status launch_pack_gauge(const hr_ctx *c, int nreal, int ld, int dcol, void *dst, hr_prec prec, const void *canon_dev,
                             hr_prec cprec, long first_site, long nsites, cudaStream_t st);
-hr_status launch_unpack_gauge(const hr_ctx *c, int nreal, const void *src, hr_prec prec, void *canon_dev,
+hr_status launch_unpack_gauge(const hr_ctx *c, int nreal, int ld, int dcol, const void *src, hr_prec prec, void *canon_dev,
                               hr_prec cprec, long first_site, long nsites, cudaStream_t st);
 
 } // namespace hr

@@ -103,7 +103,10 @@ template <int N, int SIGN, typename R, int D> __device__ __forceinline__ void re
 
 template <int N, int REP> struct RepGeom {
     static constexpr int D = REP == HR_REP_FUND ? N : REP == HR_REP_ADJ ? N * N - 1 : REP == HR_REP_SYM ? N * (N + 1) / 2 : N * (N - 1) / 2;
-    static constexpr int NOUT = REP == HR_REP_ADJ ? D * D : 2 * D * D;
+    static constexpr int NREP = REP == HR_REP_ADJ ? D * D : 2 * D * D;   // reals of the represented matrix
+    // internal row stride of a real link (hr_internal.h link_ld): d_R + 1 for an odd d_R > 8, the extra entry zero
+    static constexpr int LD = (REP == HR_REP_ADJ && (D & 1) && D > 8) ? D + 1 : D;
+    static constexpr int NOUT = REP == HR_REP_ADJ ? D * LD : 2 * D * D;     // reals of the internal record
 };
 
 template <int N, int REP, typename RI, typename RO>
@@ -117,7 +120,7 @@ __global__ void __launch_bounds__(128) represent_kernel(const char *__restrict__
     const long s = idx - q * vh;
     RI u[NIN];
     load_record<LD_STREAM, NIN>(u, fund + (size_t)q * NIN * sizeof(RI) * vh, (size_t)vh, (size_t)s, 0);
-    RI r[G::NOUT];
+    RI r[G::NREP];
     if constexpr (REP == HR_REP_FUND) {
 #pragma unroll
         for (int e = 0; e < NIN; ++e) r[e] = u[e];
@@ -127,8 +130,15 @@ __global__ void __launch_bounds__(128) represent_kernel(const char *__restrict__
         rep_twoindex<N, REP == HR_REP_SYM ? 1 : -1, RI, G::D>(u, r);
     }
     RO o[G::NOUT];
+    if constexpr (G::LD == G::D) {
 #pragma unroll
-    for (int e = 0; e < G::NOUT; ++e) o[e] = (RO)r[e];
+        for (int e = 0; e < G::NOUT; ++e) o[e] = (RO)r[e];
+    } else {
+#pragma unroll
+        for (int a = 0; a < G::D; ++a)
+#pragma unroll
+            for (int b = 0; b < G::LD; ++b) o[a * G::LD + b] = b < G::D ? (RO)r[a * G::D + b] : (RO)0;
+    }
     store_record<G::NOUT>(repr + (size_t)q * G::NOUT * sizeof(RO) * vh, (size_t)vh, (size_t)s, o);
 }
 
