@@ -68,7 +68,10 @@ void hr_ctx_destroy(hr_ctx *ctx); /* also frees the host-path workspace, if one 
 int hr_rep_dim(const hr_ctx *ctx);          /* d_R */
 int hr_links_are_real(const hr_ctx *ctx);   /* 1 for the adjoint (reading C7), else 0 */
 size_t hr_half_volume(const hr_ctx *ctx);   /* V/2 = output sites of one hr_dphi_eo */
-size_t hr_gauge_bytes(const hr_ctx *ctx, int represented, hr_prec prec); /* whole field, both parities */
+size_t hr_gauge_bytes(const hr_ctx *ctx, int represented, hr_prec prec); /* whole field, both parities, INTERNAL layout:
+                                             * represented real links of an odd d_R > 8 (SU(4) adjoint) are held with rows
+                                             * of d_R + 1 reals (the last one zero); the canonical record that
+                                             * hr_gauge_import / hr_gauge_export exchange stays d_R x d_R */
 size_t hr_spinor_bytes(const hr_ctx *ctx, hr_prec prec);                 /* ONE parity: V/2 sites      */
 
 /*
