@@ -196,6 +196,19 @@ hr_status hr_spinor_g5_mulc_add_assign(const hr_ctx *ctx, hr_prec prec, void *ou
  */
 hr_status hr_spinor_dot(hr_ctx *ctx, hr_prec prec, const void *x, const void *y, double *result, void *stream);
 hr_status hr_spinor_norm2(hr_ctx *ctx, hr_prec prec, const void *x, double *result, void *stream);
+/*
+ * hr_spinor_dot_noalloc -- hr_spinor_dot for callers that may not allocate (CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): same one-pass reduction, same result (result_dev[0] + i result_dev[1] = <x, y>; x == y gives the
+ * norm with result_dev[1] = 0), but the per-CTA partial sums live in a 33 KB file-scope device array of libhr.so instead
+ * of the context's cudaMalloc'ed scratch.  The call makes no cudaMalloc / cudaFree and no synchronisation.
+ *   x, y        DEVICE half fields, internal layout, 16-byte aligned, hr_spinor_bytes(ctx, prec) each; not modified
+ *   result_dev  DEVICE memory, 2 doubles, written by the kernel on `stream` (host pointers are rejected: HR_EINVAL)
+ * Limits: half fields of at most hr_spinor_dot_noalloc_max_bytes() = 4 GiB; beyond that HR_EUNSUPPORTED, nothing launched.
+ * The array is shared by every call on a device: calls that can overlap on the GPU (different streams without an ordering
+ * between them, concurrent host threads) race on it -- order them on one stream or with events.
+ */
+size_t hr_spinor_dot_noalloc_max_bytes(void);
+hr_status hr_spinor_dot_noalloc(hr_ctx *ctx, hr_prec prec, const void *x, const void *y, double *result_dev, void *stream);
 
 /*
  * hr_dhat -- the even-odd preconditioned operator on EVEN sites (reading C20):

@@ -77,6 +77,8 @@ _SIGNATURES = {
     "hr_spinor_g5_mulc_add_assign": (_ci, [_vp, _ci, _vp, _cd, _cd, _vp, _vp]),
     "hr_spinor_dot": (_ci, [_vp, _ci, _vp, _vp, _vp, _vp]),
     "hr_spinor_norm2": (_ci, [_vp, _ci, _vp, _vp, _vp]),
+    "hr_spinor_dot_noalloc_max_bytes": (_sz, []),
+    "hr_spinor_dot_noalloc": (_ci, [_vp, _ci, _vp, _vp, _vp, _vp]),
     "hr_dhat": (_ci, [_cd, _ci, _vp, _vp, _vp, _vp, _vp]),
     "hr_cg_workspace_bytes": (_sz, [_vp, _ci, _ci]),
     "hr_cg_dhat": (_ci, [_vp, _cd, _vp, _vp, _vp, _cd, _ci, _vp, ctypes.POINTER(_ci), ctypes.POINTER(_cd), _vp, _vp]),
@@ -288,6 +290,15 @@ def hr_spinor_dot(ctx: int, prec: int, x, y, stream: int = 0, result=None):
     r = _D2()
     _check(_lib.hr_spinor_dot(ctx, prec, _ptr(x), _ptr(y), ctypes.addressof(r), stream))
     return complex(r[0], r[1])
+
+
+def hr_spinor_dot_noalloc_max_bytes() -> int:
+    return _lib.hr_spinor_dot_noalloc_max_bytes()
+
+
+def hr_spinor_dot_noalloc(ctx: int, prec: int, x, y, result, stream: int = 0) -> None:
+    """<x, y> into the device buffer `result` (2 doubles); allocates nothing, does not synchronise (include/hr.h)."""
+    _check(_lib.hr_spinor_dot_noalloc(ctx, prec, _ptr(x), _ptr(y), _ptr(result), stream))
 
 
 def hr_spinor_norm2(ctx: int, prec: int, x, stream: int = 0, result=None):
