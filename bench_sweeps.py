@@ -384,7 +384,7 @@ def variants(argv):
         python bench_sweeps.py variants --cases '[[5,"f64","repr"],[4,"f32","fund"],[2,"f64","rows",[64,32,32,32]]]' \
                --sweeps '[{},{"variant":7},{"variant":8,"bulk_ctas":2}]' [--secs 0.5]
 
-    case = [bench.py config, precision, link source repr|fund|rows, optional dims]; a sweep entry sets hr_ctx_set_tuning keys
+    case = [bench.py config (or {"N": .., "rep": ..} with dims), precision, link source repr|fund|rows, optional dims]; a sweep entry sets hr_ctx_set_tuning keys
     (variant, block, xblock, bulk_rows, bulk_stages, bulk_ctas, bulk_strip; {} = library defaults).  Inputs: one t-pair of the
     config's seeded fields repeated along t (values do not influence timing).  One JSON line per point."""
     import statistics
@@ -435,7 +435,10 @@ def variants(argv):
 
     for case in json.loads(args.cases):
         cid, prec, src = case[:3]
-        cfg = dict(B.CONFIGS[cid])
+        if isinstance(cid, dict):   # {"N": 4, "rep": "fund"}: a gauge group / representation outside BASELINE.json's configs
+            cfg = dict(name="SU(%d) %s" % (cid["N"], cid["rep"]), kind="haar", seeds=(1007, 2007), **cid)
+        else:
+            cfg = dict(B.CONFIGS[cid])
         if len(case) > 3:
             cfg["dims"] = tuple(case[3])
         P = hr.PREC_NAMES[prec]

@@ -33,6 +33,28 @@ static bool bulk_ok(const hr_ctx *c, hr_prec prec, int lk, int ks)
     return false;
 }
 
+// sites of the tile the two-threads-per-site bulk kernel (variant 8) would use on this lattice: whole rows of Zh sites, a
+// divisor of Y of them, at most 112 sites (dphi_bulk_kernel.cuh, bulk_geometry); 0 = none
+static int bulk2_tile_sites(const hr_ctx *c)
+{
+    const int Y = c->dims[2], Zh = c->dims[3] / 2;
+    int best = 0;
+    for (int r = 1; r <= Y && r * Zh <= 112; ++r)
+        if (Y % r == 0) best = r * Zh;
+    return best;
+}
+
+// bulk2 where its tile fills the CTA, else bulk, else -1.  Measured (profiles/r2_staging.md, "geometry"): with 96-112 sites per
+// tile (24^3 x 48: 8 rows of 12) bulk2 is 9-15 % ahead of the site kernel; on Z = 16 / 32 / 64 lattices its largest tile that
+// divides Y has 64 sites -- 4 consumer warps -- and it LOSES 5-13 %, while bulk (one thread per site, 128-site tiles) is level
+// with or ahead of the site kernel.
+static int staged_variant(const hr_ctx *c, hr_prec prec, int lk)
+{
+    if (bulk2_tile_sites(c) >= 96 && bulk_ok(c, prec, lk, 2)) return 8;
+    if (bulk_ok(c, prec, lk, 1)) return 7;
+    return -1;
+}
+
 // Default variant per (d_R, link type, precision, volume): filled from measurements.
 static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
 {
@@ -43,8 +65,14 @@ static int default_variant(const hr_ctx *c, hr_prec prec, int lk)
     // d_R = 3 represented links in fp64 on lattices with Z <= 32 (tiles of 8 rows): +4-6 % (complex), +2 % (real) on 32^3x64,
     // 32^3x256, 64^3x32(z); on Z = 64 lattices (64^4) the site kernel stays ahead
     if ((lk == 0 || lk == 1) && c->d == 3 && prec == HR_F64 && c->dims[3] <= 32 && c->dims[3] >= 16 && bulk_ok(c, prec, lk, 1)) return 7;
-    if (lk == 2 && c->d == 6 && prec == HR_F64 && bulk_ok(c, prec, lk, 2)) return 8;
-    if (lk == 0 && c->d == 6 && prec == HR_F32 && bulk_ok(c, prec, lk, 2)) return 8;
+    // sextet: fp64 applied on the fly, fp32 with represented links; SU(3) adjoint (real 8 x 8 links) in fp32 (24^3 x 48:
+    // 0.159 -> 0.145 ms with bulk2; 32^4: 0.247 -> 0.236 ms with bulk)
+    if (((lk == 2 && c->d == 6 && prec == HR_F64) || (lk == 0 && c->d == 6 && prec == HR_F32) || (lk == 1 && c->d == 8 && prec == HR_F32))) {
+        const int v = staged_variant(c, prec, lk);
+        if (v >= 0) return v;
+    }
+    // SU(4) fundamental in fp64, Z <= 32: +1-2 % (40 x 32^3 0.291 -> 0.284 ms, 64 x 32^2 x 16 0.230 -> 0.227 ms)
+    if (lk == 0 && c->d == 4 && prec == HR_F64 && c->dims[3] <= 32 && c->dims[3] >= 16 && bulk_ok(c, prec, lk, 1)) return 7;
     // on-the-fly two-index kernels hold an N x N link, not a d_R x d_R one: a whole site fits one thread
     if (lk == 2 || lk == 3 || lk == 4) return 0;
     if (lk == 6 || lk == 7) return prec == HR_F64 ? 2 : 0; // fp64 d_R = 8: two threads per site (measured)

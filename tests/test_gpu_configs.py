@@ -76,7 +76,7 @@ def test_config4_su3_sextet_24x24x24x48(hr, prec):
 
 
 # the large representations at the sizes bench_large_n times (the paper's Fig. 6 experiment), default
-# kernel = colour-parallel: every output site against the oracle
+# kernel = colour-parallel or, for d_R = 8 in fp32, bulk2: every output site against the oracle
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("N,rep,dims", [(3, "adj", (48, 24, 24, 24)), (4, "sym", (56, 16, 16, 16)), (4, "adj", (48, 16, 16, 16))])
 def test_large_representations_at_the_benchmarked_sizes(hr, N, rep, dims, prec):
@@ -84,7 +84,8 @@ def test_large_representations_at_the_benchmarked_sizes(hr, N, rep, dims, prec):
     U, psi = inputs(f"large{N}{rep}", dims, N, d, 1006, 2006)
     import paper_2405_19294_b200 as lib
     lat = lib.Lattice(dims, BC_T, N, rep)
-    want_kernel = "colour" if (prec == "f64" or d > 8) else "site_ef"
+    # fp32 SU(3) adjoint on 24^3 x 48: the TMA-staged two-threads-per-site kernel since round 2 (tiles of 8 rows x 12 sites)
+    want_kernel = "colour" if (prec == "f64" or d > 8) else "bulk2"
     assert lib.hr_dphi_variant_name(lat.ctx, lib.PREC_NAMES[prec]) == want_kernel
     lat.close()
     check_full(hr, dims, N, rep, prec, U, psi, check_links=True)
