@@ -361,6 +361,14 @@ hr_status hr_dphi_eo_faces_pack(int split_mask, void *const send_up[4], void *co
 hr_status hr_dphi_eo_interior_mask(void *out, const void *in, const hr_gauge *links, int parity, int split_mask, void *stream);
 hr_status hr_dphi_eo_face_apply(int mu, void *out, const void *recv_prev, const void *recv_next, const hr_gauge *links,
                                 int parity, int first_rank, int last_rank, void *stream);
+/* hr_dphi_eo_faces_apply -- hr_dphi_eo_face_apply for ALL split directions (bit mu of split_mask) in ONE launch.  An edge or
+ * corner site of the block receives a term from each of its faces; every boundary site is updated by exactly one thread, which
+ * adds the terms of its faces in ascending mu, so the result is bitwise that of the per-direction calls made in ascending mu.
+ * recv_prev[mu] / recv_next[mu]: the messages received from the previous / next rank in mu (hr_face_bytes each; entries of
+ * unsplit directions are ignored); bit mu of first_mask / last_mask: this rank is the first / last along mu (its outer face
+ * carries the seam sign bc[mu]).  `out` already holds hr_dphi_eo_interior_mask's result; no synchronisation. */
+hr_status hr_dphi_eo_faces_apply(int split_mask, void *out, const void *const recv_prev[4], const void *const recv_next[4],
+                                 const hr_gauge *links, int parity, int first_mask, int last_mask, void *stream);
 hr_status hr_halo_buffers_alloc(const hr_ctx *ctx, hr_prec prec, void **base);             /* direction t */
 hr_status hr_face_buffers_alloc(const hr_ctx *ctx, hr_prec prec, int mu, void **base);     /* 6 hr_face_bytes(mu) */
 void hr_halo_buffers_free(const hr_ctx *ctx, void *base);

@@ -93,6 +93,7 @@ _SIGNATURES = {
     "hr_face_bytes": (_sz, [_vp, _ci, _ci]),
     "hr_dphi_eo_face_pack": (_ci, [_ci, _vp, _vp, _vp, _vp, _ci, _vp]),
     "hr_dphi_eo_faces_pack": (_ci, [_ci, ctypes.POINTER(_vp), ctypes.POINTER(_vp), _vp, _vp, _ci, _vp]),
+    "hr_dphi_eo_faces_apply": (_ci, [_ci, _vp, ctypes.POINTER(_vp), ctypes.POINTER(_vp), _vp, _ci, _ci, _ci, _vp]),
     "hr_dphi_eo_interior_mask": (_ci, [_vp, _vp, _vp, _ci, _ci, _vp]),
     "hr_dphi_eo_face_apply": (_ci, [_ci, _vp, _vp, _vp, _vp, _ci, _ci, _ci, _vp]),
     "hr_halo_buffers_alloc": (_ci, [_vp, _ci, ctypes.POINTER(_vp)]),
@@ -434,6 +435,16 @@ def hr_dphi_eo_face_apply(mu: int, out, recv_prev, recv_next, links: int, parity
                           stream: int = 0) -> None:
     _check(_lib.hr_dphi_eo_face_apply(mu, _ptr(out), _ptr(recv_prev), _ptr(recv_next), links, parity, int(first_rank),
                                       int(last_rank), stream))
+
+
+def hr_dphi_eo_faces_apply(split_mask: int, out, recv_prev: dict, recv_next: dict, links: int, parity: int, first_mask: int,
+                           last_mask: int, stream: int = 0) -> None:
+    """recv_prev / recv_next: {mu: buffer} for the split directions; first_mask / last_mask: bit mu = first / last rank along mu."""
+    rp, rn = (_vp * 4)(), (_vp * 4)()
+    for mu in range(4):
+        rp[mu] = _ptr(recv_prev.get(mu)) or None
+        rn[mu] = _ptr(recv_next.get(mu)) or None
+    _check(_lib.hr_dphi_eo_faces_apply(split_mask, _ptr(out), rp, rn, links, parity, int(first_mask), int(last_mask), stream))
 
 
 def hr_halo_buffers_alloc(ctx: int, prec: int) -> int:

@@ -11,7 +11,7 @@ template <typename Real, int D, int LK> bool dphi_variant_ok_t(int variant);
 template <typename Real, int D, int LK> bool dphi_bulk_ok_t(const DphiArgs &a, int ks);
 
 template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, int mu, const HaloArgs &a, cudaStream_t st);
-template <typename Real, int D, int LK> hr_status launch_halo_pack_multi_t(const HaloArgs *a, const int *mu, int ndir, cudaStream_t st);
+template <typename Real, int D, int LK> hr_status launch_halo_multi_t(bool pack, const HaloArgs *a, const int *mu, int ndir, cudaStream_t st);
 
 static const char *const kNames[] = { "site", "site_ef", "pair", "pair_ef", "site_l1", "site_pf", "colour", "bulk", "bulk2", "bulkx", "bulkx2", "site_loop" };
 
@@ -150,12 +150,12 @@ hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, int mu, const Ha
     return HR_EUNSUPPORTED;
 }
 
-hr_status launch_halo_pack_multi(const hr_ctx *c, hr_prec prec, const HaloArgs *a, const int *mu, int ndir, cudaStream_t st, int link_src)
+hr_status launch_halo_multi(const hr_ctx *c, hr_prec prec, bool pack, const HaloArgs *a, const int *mu, int ndir, cudaStream_t st, int link_src)
 {
     const int lk = dphi_link_kind(c, link_src);
 #define X(D, LK)                                                                                          \
     if (c->d == D && lk == LK)                                                                            \
-        return prec == HR_F64 ? launch_halo_pack_multi_t<double, D, LK>(a, mu, ndir, st) : launch_halo_pack_multi_t<float, D, LK>(a, mu, ndir, st);
+        return prec == HR_F64 ? launch_halo_multi_t<double, D, LK>(pack, a, mu, ndir, st) : launch_halo_multi_t<float, D, LK>(pack, a, mu, ndir, st);
     HR_COMBOS(X)
 #undef X
     set_error("no halo kernel compiled for d_R=%d (link kind %d)", c->d, lk);

@@ -277,21 +277,25 @@ template <typename Real, int D, int LK> hr_status launch_halo_t(bool pack, int m
     return HR_OK;
 }
 
-template <typename Real, int D, int LK> hr_status launch_halo_pack_multi_t(const HaloArgs *a, const int *mu, int ndir, cudaStream_t st)
+// pack == true: the messages of all split directions; false: their face terms added to out (halo_kernel.cuh); mu ascending
+template <typename Real, int D, int LK> hr_status launch_halo_multi_t(bool pack, const HaloArgs *a, const int *mu, int ndir, cudaStream_t st)
 {
     HaloMultiArgs g;
     g.ndir = ndir;
     g.first[0] = 0;
+    for (int m = 0; m < 4; ++m) g.slot[m] = -1;
     for (int k = 0; k < ndir; ++k) {
         g.a[k] = a[k];
         g.mu[k] = mu[k];
+        g.slot[mu[k]] = k;
         g.first[k + 1] = g.first[k] + (unsigned)((a[k].nface + 127) / 128);
     }
     for (int k = ndir; k < 4; ++k) { g.a[k] = a[0]; g.mu[k] = 0; g.first[k + 1] = g.first[ndir]; }
-    halo_pack_multi_kernel<Real, D, LK><<<g.first[ndir], 128, 0, st>>>(g);
+    if (pack) halo_pack_multi_kernel<Real, D, LK><<<g.first[ndir], 128, 0, st>>>(g);
+    else halo_apply_multi_kernel<Real, D, LK><<<g.first[ndir], 128, 0, st>>>(g);
     count_launch();
     cudaError_t e = cudaPeekAtLastError();
-    if (e != cudaSuccess) { set_error("halo multi-direction pack launch failed: %s", cudaGetErrorString(e)); return HR_ECUDA; }
+    if (e != cudaSuccess) { set_error("halo multi-direction %s launch failed: %s", pack ? "pack" : "apply", cudaGetErrorString(e)); return HR_ECUDA; }
     return HR_OK;
 }
 
@@ -300,6 +304,6 @@ template <typename Real, int D, int LK> hr_status launch_halo_pack_multi_t(const
     template bool dphi_variant_ok_t<Real, D, LK>(int);                                                    \
     template bool dphi_bulk_ok_t<Real, D, LK>(const DphiArgs &, int);                                                \
     template hr_status launch_halo_t<Real, D, LK>(bool, int, const HaloArgs &, cudaStream_t);             \
-    template hr_status launch_halo_pack_multi_t<Real, D, LK>(const HaloArgs *, const int *, int, cudaStream_t);
+    template hr_status launch_halo_multi_t<Real, D, LK>(bool, const HaloArgs *, const int *, int, cudaStream_t);
 
 } // namespace hr

@@ -121,6 +121,7 @@ struct HaloMultiArgs {
     unsigned first[5];
     int mu[4];
     int ndir;
+    int slot[4];   // direction mu -> its entry of a[], -1 if mu is not split (fused apply)
 };
 template <typename Real, int D, int LK>
 __global__ void __launch_bounds__(128) halo_pack_multi_kernel(const __grid_constant__ HaloMultiArgs g)
@@ -136,60 +137,149 @@ __global__ void __launch_bounds__(128) halo_pack_multi_kernel(const __grid_const
     }
 }
 
+// The two face terms of direction MU, added to the site's spinor o[] held in registers (shared by the per-direction and the
+// fused apply kernels, so that both perform the same sequence of roundings):
+//   apply_prev  first slice: backward hop from the previous rank; reconstruct with c = -c0:
+//               out_k += chi_k, out_{p(k)} += sk_k conj(-c0) chi_k
+//   apply_next  last slice: forward hop to the next rank, chi = U_mu(x) h_recv with the OWN link; reconstruct with c = +c0
 template <typename Real, int D, int LK, int MU>
-__global__ void __launch_bounds__(128) halo_apply_kernel(const HaloArgs a)
+__device__ __forceinline__ void apply_prev(Real (&o)[8 * D], const HaloArgs &a, size_t f, const Real (&be)[2])
+{
+    constexpr int RPV = 16 / (int)sizeof(Real);
+    using H = HopTable<MU>;
+    const Real sk1 = (Real)(MU >= 2 ? -1 : 1);
+    Real chi[4 * D];
+    load_planes<LD_STREAM, 4 * D / RPV>(chi, (const char *)a.recv_prev + f * 16, (size_t)a.nface * 16, 0);
+    const Real s0 = be[0] * (Real)a.sign_prev, s1 = be[1] * (Real)a.sign_prev;
+#pragma unroll
+    for (int c = 0; c < D; ++c) {
+        o[2 * c] = fma(s0, chi[2 * c], o[2 * c]);
+        o[2 * c + 1] = fma(s0, chi[2 * c + 1], o[2 * c + 1]);
+        o[2 * D + 2 * c] = fma(s0, chi[2 * D + 2 * c], o[2 * D + 2 * c]);
+        o[2 * D + 2 * c + 1] = fma(s0, chi[2 * D + 2 * c + 1], o[2 * D + 2 * c + 1]);
+        acc_conj_c<-H::CRE, -H::CIM>(o[H::P0 * 2 * D + 2 * c], o[H::P0 * 2 * D + 2 * c + 1], chi[2 * c], chi[2 * c + 1], s1);
+        acc_conj_c<-H::CRE, -H::CIM>(o[H::P1 * 2 * D + 2 * c], o[H::P1 * 2 * D + 2 * c + 1], chi[2 * D + 2 * c], chi[2 * D + 2 * c + 1], s1 * sk1);
+    }
+}
+template <typename Real, int D, int LK, int MU>
+__device__ __forceinline__ void apply_next(Real (&o)[8 * D], const HaloArgs &a, size_t f, size_t sx, const Real (&be)[2])
 {
     constexpr int LNREAL = LinkGeom<LK, D>::NREAL;
     constexpr int RPV = 16 / (int)sizeof(Real);
     constexpr size_t LB = (size_t)LNREAL * sizeof(Real);
     using H = HopTable<MU>;
-    const long f = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (f >= a.nface) return;
-    const size_t vh = (size_t)a.vh, nf = (size_t)a.nface;
-    Real be[2];
+    const Real sk1 = (Real)(MU >= 2 ? -1 : 1);
+    const size_t vh = (size_t)a.vh;
+    Real h[4 * D], u[LNREAL], h0[2 * D], h1[2 * D], c0[2 * D], c1[2 * D];
+    load_planes<LD_STREAM, 4 * D / RPV>(h, (const char *)a.recv_next + f * 16, (size_t)a.nface * 16, 0);
+    load_record<LD_STREAM, LNREAL>(u, (const char *)a.links + (size_t)(a.parity * 4 + MU) * LB * vh, vh, sx, 0);
+#pragma unroll
+    for (int c = 0; c < 2 * D; ++c) { h0[c] = h[c]; h1[c] = h[2 * D + c]; }
+    link_mul<D, LK, false>(c0, u, h0);
+    link_mul<D, LK, false>(c1, u, h1);
+    const Real s0 = be[0] * (Real)a.sign_next, s1 = be[1] * (Real)a.sign_next;
+#pragma unroll
+    for (int c = 0; c < D; ++c) {
+        o[2 * c] = fma(s0, c0[2 * c], o[2 * c]);
+        o[2 * c + 1] = fma(s0, c0[2 * c + 1], o[2 * c + 1]);
+        o[2 * D + 2 * c] = fma(s0, c1[2 * c], o[2 * D + 2 * c]);
+        o[2 * D + 2 * c + 1] = fma(s0, c1[2 * c + 1], o[2 * D + 2 * c + 1]);
+        acc_conj_c<H::CRE, H::CIM>(o[H::P0 * 2 * D + 2 * c], o[H::P0 * 2 * D + 2 * c + 1], c0[2 * c], c0[2 * c + 1], s1);
+        acc_conj_c<H::CRE, H::CIM>(o[H::P1 * 2 * D + 2 * c], o[H::P1 * 2 * D + 2 * c + 1], c1[2 * c], c1[2 * c + 1], s1 * sk1);
+    }
+}
+
+template <typename Real> __device__ __forceinline__ void halo_beta(Real (&be)[2], const HaloArgs &a)
+{
     if constexpr (sizeof(Real) == 8) { be[0] = (Real)a.beta[0]; be[1] = (Real)a.beta[1]; }
     else { be[0] = a.betaf[0]; be[1] = a.betaf[1]; }
-    const Real sk1 = (Real)(MU >= 2 ? -1 : 1);
+}
+
+template <typename Real, int D, int LK, int MU>
+__global__ void __launch_bounds__(128) halo_apply_kernel(const HaloArgs a)
+{
+    constexpr int RPV = 16 / (int)sizeof(Real);
+    const long f = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= a.nface) return;
+    const size_t vh = (size_t)a.vh;
+    Real be[2];
+    halo_beta(be, a);
     char *out = (char *)a.out;
-    // first slice: backward hop from the previous rank; reconstruct with c = -c0:  out_k += chi_k, out_{p(k)} += sk_k conj(-c0) chi_k
     {
         const size_t sx = face_site<MU>(a, a.parity, 0, f);
-        Real chi[4 * D], o[8 * D];
-        load_planes<LD_STREAM, 4 * D / RPV>(chi, (const char *)a.recv_prev + (size_t)f * 16, nf * 16, 0);
+        Real o[8 * D];
         load_record<LD_DEFAULT, 8 * D>(o, out, vh, sx, 0);
-        const Real s0 = be[0] * (Real)a.sign_prev, s1 = be[1] * (Real)a.sign_prev;
-#pragma unroll
-        for (int c = 0; c < D; ++c) {
-            o[2 * c] = fma(s0, chi[2 * c], o[2 * c]);
-            o[2 * c + 1] = fma(s0, chi[2 * c + 1], o[2 * c + 1]);
-            o[2 * D + 2 * c] = fma(s0, chi[2 * D + 2 * c], o[2 * D + 2 * c]);
-            o[2 * D + 2 * c + 1] = fma(s0, chi[2 * D + 2 * c + 1], o[2 * D + 2 * c + 1]);
-            acc_conj_c<-H::CRE, -H::CIM>(o[H::P0 * 2 * D + 2 * c], o[H::P0 * 2 * D + 2 * c + 1], chi[2 * c], chi[2 * c + 1], s1);
-            acc_conj_c<-H::CRE, -H::CIM>(o[H::P1 * 2 * D + 2 * c], o[H::P1 * 2 * D + 2 * c + 1], chi[2 * D + 2 * c], chi[2 * D + 2 * c + 1], s1 * sk1);
-        }
+        apply_prev<Real, D, LK, MU>(o, a, (size_t)f, be);
         store_planes<ST_DEFAULT, 8 * D / RPV>(out + sx * 16, vh * 16, o);
     }
-    // last slice: forward hop to the next rank, chi = U_mu(x) h_recv with the OWN link; reconstruct with c = +c0
     {
         const size_t sx = face_site<MU>(a, a.parity, 1, f);
-        Real h[4 * D], u[LNREAL], h0[2 * D], h1[2 * D], c0[2 * D], c1[2 * D], o[8 * D];
-        load_planes<LD_STREAM, 4 * D / RPV>(h, (const char *)a.recv_next + (size_t)f * 16, nf * 16, 0);
-        load_record<LD_STREAM, LNREAL>(u, (const char *)a.links + (size_t)(a.parity * 4 + MU) * LB * vh, vh, sx, 0);
+        Real o[8 * D];
         load_record<LD_DEFAULT, 8 * D>(o, out, vh, sx, 0);
-#pragma unroll
-        for (int c = 0; c < 2 * D; ++c) { h0[c] = h[c]; h1[c] = h[2 * D + c]; }
-        link_mul<D, LK, false>(c0, u, h0);
-        link_mul<D, LK, false>(c1, u, h1);
-        const Real s0 = be[0] * (Real)a.sign_next, s1 = be[1] * (Real)a.sign_next;
-#pragma unroll
-        for (int c = 0; c < D; ++c) {
-            o[2 * c] = fma(s0, c0[2 * c], o[2 * c]);
-            o[2 * c + 1] = fma(s0, c0[2 * c + 1], o[2 * c + 1]);
-            o[2 * D + 2 * c] = fma(s0, c1[2 * c], o[2 * D + 2 * c]);
-            o[2 * D + 2 * c + 1] = fma(s0, c1[2 * c + 1], o[2 * D + 2 * c + 1]);
-            acc_conj_c<H::CRE, H::CIM>(o[H::P0 * 2 * D + 2 * c], o[H::P0 * 2 * D + 2 * c + 1], c0[2 * c], c0[2 * c + 1], s1);
-            acc_conj_c<H::CRE, H::CIM>(o[H::P1 * 2 * D + 2 * c], o[H::P1 * 2 * D + 2 * c + 1], c1[2 * c], c1[2 * c + 1], s1 * sk1);
-        }
+        apply_next<Real, D, LK, MU>(o, a, (size_t)f, sx, be);
+        store_planes<ST_DEFAULT, 8 * D / RPV>(out + sx * 16, vh * 16, o);
+    }
+}
+
+// The face terms of ALL split directions in one launch.  A site on an edge or corner of the block receives a term from each
+// of its faces, and out += term is not associative: to stay bitwise equal to the per-direction launches (ascending mu, each
+// a read-modify-write of out) every boundary site is updated by exactly ONE thread, which adds the terms of all its faces in
+// ascending mu with the spinor in registers.  Threads are laid out as in halo_pack_multi_kernel -- thread (k, f) visits the
+// two sites f of the first and last slice of direction mu_k -- and thread (k, f) OWNS a site iff the site lies on no face of
+// a split direction below mu_k; the others skip it.  Face index of a site in direction mu = the inverse of face_site.
+template <typename Real, int D, int LK, int MU>
+__device__ __forceinline__ void apply_dir(Real (&o)[8 * D], const HaloMultiArgs &g, int t, int x, int y, int zh, int b, size_t sx,
+                                          const Real (&be)[2])
+{
+    const int slot = g.slot[MU];
+    if (slot < 0) return;
+    const HaloArgs &a = g.a[slot];
+    bool lo, hi;
+    size_t f;
+    if constexpr (MU == 0) { lo = t == 0; hi = t == a.T - 1; f = ((size_t)x * a.Y + y) * a.Zh + zh; }
+    else if constexpr (MU == 1) { lo = x == 0; hi = x == a.X - 1; f = ((size_t)t * a.Y + y) * a.Zh + zh; }
+    else if constexpr (MU == 2) { lo = y == 0; hi = y == a.Y - 1; f = ((size_t)t * a.X + x) * a.Zh + zh; }
+    else { lo = zh == 0 && b == 0; hi = zh == a.Zh - 1 && b == 1; f = ((size_t)t * a.X + x) * (a.Y / 2) + y / 2; }
+    if (lo) apply_prev<Real, D, LK, MU>(o, a, f, be);
+    if (hi) apply_next<Real, D, LK, MU>(o, a, f, sx, be);
+}
+
+template <typename Real, int D, int LK>
+__global__ void __launch_bounds__(128) halo_apply_multi_kernel(const __grid_constant__ HaloMultiArgs g)
+{
+    constexpr int RPV = 16 / (int)sizeof(Real);
+    int k = 0;
+    while (k + 1 < g.ndir && blockIdx.x >= g.first[k + 1]) ++k;
+    const HaloArgs &a = g.a[k];
+    const long f = (long)(blockIdx.x - g.first[k]) * blockDim.x + threadIdx.x;
+    if (f >= a.nface) return;
+    const int mu = g.mu[k];
+    const size_t vh = (size_t)a.vh;
+    Real be[2];
+    halo_beta(be, a);
+    char *out = (char *)a.out;
+#pragma unroll 1
+    for (int side = 0; side < 2; ++side) {
+        const size_t sx = mu == 0 ? face_site<0>(a, a.parity, side, f) : mu == 1 ? face_site<1>(a, a.parity, side, f)
+                        : mu == 2 ? face_site<2>(a, a.parity, side, f) : face_site<3>(a, a.parity, side, f);
+        unsigned r = (unsigned)sx;
+        const int zh = (int)(r % (unsigned)a.Zh); r /= (unsigned)a.Zh;
+        const int y = (int)(r % (unsigned)a.Y); r /= (unsigned)a.Y;
+        const int x = (int)(r % (unsigned)a.X);
+        const int t = (int)(r / (unsigned)a.X);
+        const int b = (t + x + y + a.parity) & 1;
+        // owner: no face of a split direction below mu holds this site
+        bool mine = true;
+        if (mu > 0 && g.slot[0] >= 0 && (t == 0 || t == a.T - 1)) mine = false;
+        if (mu > 1 && g.slot[1] >= 0 && (x == 0 || x == a.X - 1)) mine = false;
+        if (mu > 2 && g.slot[2] >= 0 && (y == 0 || y == a.Y - 1)) mine = false;
+        if (!mine) continue;
+        Real o[8 * D];
+        load_record<LD_DEFAULT, 8 * D>(o, out, vh, sx, 0);
+        apply_dir<Real, D, LK, 0>(o, g, t, x, y, zh, b, sx, be);
+        apply_dir<Real, D, LK, 1>(o, g, t, x, y, zh, b, sx, be);
+        apply_dir<Real, D, LK, 2>(o, g, t, x, y, zh, b, sx, be);
+        apply_dir<Real, D, LK, 3>(o, g, t, x, y, zh, b, sx, be);
         store_planes<ST_DEFAULT, 8 * D / RPV>(out + sx * 16, vh * 16, o);
     }
 }

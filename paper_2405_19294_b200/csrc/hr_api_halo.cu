@@ -104,7 +104,7 @@ hr_status hr_dphi_eo_faces_pack(int split_mask, void *const send_up[4], void *co
         a[n].in = in;
         mus[n++] = mu;
     }
-    return launch_halo_pack_multi(links->ctx, links->prec, a, mus, n, (cudaStream_t)stream, link_src(links));
+    return launch_halo_multi(links->ctx, links->prec, true, a, mus, n, (cudaStream_t)stream, link_src(links));
 }
 
 hr_status hr_dphi_eo_interior(void *out, const void *in, const hr_gauge *links, int parity, void *stream)
@@ -155,6 +155,39 @@ hr_status hr_dphi_eo_face_apply(int mu, void *out, const void *recv_prev, const 
     a.sign_prev = first_rank ? c->bc[mu] : 1; // the global seam lies below the first rank's first slice ...
     a.sign_next = last_rank ? c->bc[mu] : 1;  // ... and above the last rank's last slice (reading C9)
     return launch_halo(c, links->prec, false, mu, a, (cudaStream_t)stream, link_src(links));
+}
+
+hr_status hr_dphi_eo_faces_apply(int split_mask, void *out, const void *const recv_prev[4], const void *const recv_next[4],
+                                 const hr_gauge *links, int parity, int first_mask, int last_mask, void *stream)
+{
+    hr_status rc = check_links("hr_dphi_eo_faces_apply", links, parity);
+    if (rc != HR_OK) return rc;
+    if (split_mask <= 0 || split_mask > 15 || !out || !recv_prev || !recv_next || !aligned16(out)) {
+        set_error("hr_dphi_eo_faces_apply: bad argument (split_mask 1..15, non-NULL buffers)");
+        return HR_EINVAL;
+    }
+    const hr_ctx *c = links->ctx;
+    HaloArgs a[4];
+    int mus[4], n = 0;
+    for (int mu = 0; mu < 4; ++mu) {
+        if (!(split_mask & (1 << mu))) continue;
+        rc = check_mu("hr_dphi_eo_faces_apply", links, mu);
+        if (rc != HR_OK) return rc;
+        if (!recv_prev[mu] || !recv_next[mu] || !aligned16(recv_prev[mu]) || !aligned16(recv_next[mu])) {
+            set_error("hr_dphi_eo_faces_apply: buffers of direction %d must be non-NULL and 16-byte aligned", mu);
+            return HR_EINVAL;
+        }
+        halo_common(a[n], c, links, parity, mu);
+        a[n].out = out;
+        a[n].recv_prev = recv_prev[mu];
+        a[n].recv_next = recv_next[mu];
+        a[n].sign_prev = (first_mask & (1 << mu)) ? c->bc[mu] : 1;
+        a[n].sign_next = (last_mask & (1 << mu)) ? c->bc[mu] : 1;
+        mus[n++] = mu;
+    }
+    // one split direction: the per-direction kernel (compile-time direction) is 2 us faster and bitwise the same
+    if (n == 1) return launch_halo(c, links->prec, false, mus[0], a[0], (cudaStream_t)stream, link_src(links));
+    return launch_halo_multi(c, links->prec, false, a, mus, n, (cudaStream_t)stream, link_src(links));
 }
 
 // ---- face buffers in peer-accessible memory ---------------------------------------------------------------------

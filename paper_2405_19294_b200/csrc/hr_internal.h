@@ -196,7 +196,7 @@ struct HaloArgs {
     int sign_prev, sign_next; // seam signs of the two faces (+-1)
 };
 hr_status launch_halo(const hr_ctx *c, hr_prec prec, bool pack, int mu, const HaloArgs &a, cudaStream_t st, int link_src);
-hr_status launch_halo_pack_multi(const hr_ctx *c, hr_prec prec, const HaloArgs *a, const int *mu, int ndir, cudaStream_t st, int link_src);
+hr_status launch_halo_multi(const hr_ctx *c, hr_prec prec, bool pack, const HaloArgs *a, const int *mu, int ndir, cudaStream_t st, int link_src);
 
 // clover term (clover.cu): record of 8 d_R^2 reals per site, [parity] fields
 size_t clover_nreal(const hr_ctx *c);

@@ -250,10 +250,14 @@ def block_plan(rank: int, grid, dims_global) -> dict:
             "split": [mu for mu in range(4) if grid[mu] > 1], "mask": sum(1 << mu for mu in range(4) if grid[mu] > 1)}
 
 
+def _mask(flags) -> int:
+    return sum(1 << mu for mu in range(4) if flags[mu])
+
+
 class BlockDphi:
     """Distributed Dphi_eo of one rank of a 4-D block decomposition: for every split direction the four face buffers;
     pack (all directions, same input) -> [exchange of all faces in one NCCL batch on a side stream || interior launch with
-    the split directions masked] -> apply direction by direction.  Unmeasured on more than one GPU (none in this run)."""
+    the split directions masked] -> apply (all directions, one launch).  Unmeasured on more than one GPU (none in this run)."""
 
     def __init__(self, lat, prec: int, plan: dict, group=None):
         import torch
@@ -277,9 +281,9 @@ class BlockDphi:
         return [(su, sd, rp, rn, self.plan["prev"][mu], self.plan["next"][mu]) for mu, (su, sd, rp, rn) in self.buf.items()]
 
     def apply(self, out, links: int, parity: int) -> None:
-        from . import hr_dphi_eo_face_apply
-        for mu, (_, _, rp, rn) in self.buf.items():
-            hr_dphi_eo_face_apply(mu, out, rp, rn, links, parity, self.plan["first"][mu], self.plan["last"][mu], self.lat.stream())
+        from . import hr_dphi_eo_faces_apply
+        hr_dphi_eo_faces_apply(self.plan["mask"], out, {mu: b[2] for mu, b in self.buf.items()}, {mu: b[3] for mu, b in self.buf.items()},
+                               links, parity, _mask(self.plan["first"]), _mask(self.plan["last"]), self.lat.stream())   # one launch
 
     def dphi_eo(self, out, inp, links: int, parity: int) -> None:
         self.pack(inp, links, parity)
@@ -326,7 +330,7 @@ class PeerBlockDphi:
     fence = PeerSlabDphi.fence
 
     def dphi_eo(self, out, inp, links: int, parity: int) -> None:
-        from . import hr_dphi_eo_face_apply, hr_dphi_eo_faces_pack, hr_dphi_eo_interior_mask
+        from . import hr_dphi_eo_faces_apply, hr_dphi_eo_faces_pack, hr_dphi_eo_interior_mask
         st = self.lat.stream()
         k = self.calls & 1
         self.calls += 1
@@ -335,10 +339,9 @@ class PeerBlockDphi:
                               {mu: self.prev_base[mu] + (3 + 2 * k) * self.nb[mu] for mu in self.plan["split"]}, inp, links, parity, st)
         hr_dphi_eo_interior_mask(out, inp, links, parity, self.plan["mask"], st)
         self.fence()
-        for mu in self.plan["split"]:
-            nb = self.nb[mu]
-            hr_dphi_eo_face_apply(mu, out, self.base[mu] + (2 + 2 * k) * nb, self.base[mu] + (3 + 2 * k) * nb, links, parity,
-                                  self.plan["first"][mu], self.plan["last"][mu], st)
+        hr_dphi_eo_faces_apply(self.plan["mask"], out, {mu: self.base[mu] + (2 + 2 * k) * self.nb[mu] for mu in self.plan["split"]},
+                               {mu: self.base[mu] + (3 + 2 * k) * self.nb[mu] for mu in self.plan["split"]}, links, parity,
+                               _mask(self.plan["first"]), _mask(self.plan["last"]), st)
 
     def close(self):
         from . import hr_halo_buffers_free, hr_ipc_close

@@ -158,3 +158,48 @@ def test_fused_pack_of_all_directions_is_bitwise_the_per_direction_packs(hr, N, 
     with pytest.raises(hr.HrError):
         hr.hr_dphi_eo_faces_pack(2, {}, {}, gin, prob.links, 0, st)                       # NULL buffers of a split direction
     prob.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("N,rep", [(3, "fund"), (2, "adj"), (3, "sym")])
+@pytest.mark.parametrize("dims,mask", [((4, 6, 4, 10), 1), ((4, 6, 4, 10), 6), ((4, 6, 4, 10), 9), ((4, 6, 4, 10), 15), ((4, 6, 4, 10), 8),
+                                       ((2, 2, 2, 2), 15), ((2, 4, 2, 4), 11), ((6, 2, 4, 2), 14)])
+def test_fused_apply_of_all_directions_is_bitwise_the_per_direction_applies(hr, N, rep, dims, mask, prec):
+    """hr_dphi_eo_faces_apply (one launch; every boundary site updated by one thread, its faces in ascending mu) against
+    hr_dphi_eo_face_apply direction by direction in ascending mu: the same bytes in `out` -- edge and corner sites, extents
+    of 2 (a site's two neighbours in a direction are both off the block), ragged face counts, every mix of seam flags."""
+    import torch
+    bc = (-1, 1, -1, -1)
+    U = li.haar_links(911, N, dims)
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    vh = li.volume(dims) // 2
+    prob = GpuProblem(hr, dims, N, rep, prec, U, bc=bc)
+    lat, P, st = prob.lat, prob.prec, prob.lat.stream()
+    split = [mu for mu in range(4) if mask & (1 << mu)]
+    for parity, (first, last) in itertools.product((0, 1), ((mask, mask), (0, mask), (mask & 5, mask & 10))):
+        gin = lat.spinor(P)
+        lat.import_spinor(gin, P, li.gaussian_spinor(912 + parity, vh, d), 1 - parity)
+        msg = {mu: [torch.empty(hr.hr_face_bytes(lat.ctx, P, mu), dtype=torch.uint8, device="cuda") for _ in range(2)] for mu in split}
+        hr.hr_dphi_eo_faces_pack(mask, {mu: m[0] for mu, m in msg.items()}, {mu: m[1] for mu, m in msg.items()}, gin, prob.links, parity, st)
+        base = lat.spinor(P)
+        hr.hr_dphi_eo_interior_mask(base, gin, prob.links, parity, mask, st)
+        one, fused = base.clone(), base.clone()
+        for mu in split:                                            # the rank is its own neighbour in every direction
+            hr.hr_dphi_eo_face_apply(mu, one, msg[mu][0], msg[mu][1], prob.links, parity, bool(first & (1 << mu)), bool(last & (1 << mu)), st)
+        n0 = hr.hr_launch_count()
+        hr.hr_dphi_eo_faces_apply(mask, fused, {mu: m[0] for mu, m in msg.items()}, {mu: m[1] for mu, m in msg.items()}, prob.links, parity,
+                                  first, last, st)
+        assert hr.hr_launch_count() == n0 + 1
+        torch.cuda.synchronize()
+        assert torch.equal(one, fused), (parity, first, last)
+        assert not torch.equal(fused, base)
+        if first == mask and last == mask:                          # and the whole sequence is hr_dphi_eo
+            full = lat.spinor(P)
+            lat.dphi_eo(full, gin, prob.links, parity)
+            a, b = lat.export_spinor(fused, P, parity), lat.export_spinor(full, P, parity)
+            assert rel_l2(a, b) <= TOL[prec]
+    with pytest.raises(hr.HrError):
+        hr.hr_dphi_eo_faces_apply(0, fused, {}, {}, prob.links, 0, 0, 0, st)
+    with pytest.raises(hr.HrError):
+        hr.hr_dphi_eo_faces_apply(2, fused, {}, {}, prob.links, 0, 0, 0, st)
+    prob.close()
