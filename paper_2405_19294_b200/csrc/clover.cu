@@ -198,6 +198,178 @@ __global__ void __launch_bounds__(64) clover_build_kernel(const CloverArgs a)
     store_record<G::NREAL>(base, (size_t)a.vh, hs, rec);
 }
 
+// ---- plane-parallel build for d_R <= 4 -----------------------------------------------------------------------------------
+// One thread per (site, plane (mu, nu)): Q_{mu nu}(x) = the sum of the four plaquette leaves around x, each
+// ((M1 M2) M3) M4 with the links loaded just before the product that needs them and the link shared by two consecutive
+// leaves (U_nu(x), U_mu(x-mu), U_nu(x-nu)) kept in registers: 13 link loads and 12 products per thread, live state
+// q + two partial products + two links.  The plane is uniform over a CTA (blockIdx.y) and a compile-time constant of the
+// code path; neighbour sites come from the lexicographic index by adding a stride (the wrap is a compare, not a modulo).
+// Q goes to the scratch layout of clover_q_kernel, clover_pack_kernel finishes.  (clover_build_kernel above holds all six
+// planes of a site in one thread: 252 registers and 1.5 KB of local memory in fp64, and four integer divisions per link.)
+template <typename Real, int D, bool RL, int MU, int NU>
+__device__ __forceinline__ void clover_plane(const CloverArgs &a, const int (&c)[4], int par, long lex, Real (&q)[2 * D * D])
+{
+    constexpr int M = 2 * D * D;
+    constexpr int LNREAL = CloverGeom<Real, D, RL>::LNREAL;
+    const size_t vh = (size_t)a.vh;
+    const int ext[4] = { a.T, a.X, a.Y, a.Z };
+    const long str[4] = { (long)a.X * a.Y * a.Z, (long)a.Y * a.Z, (long)a.Z, 1 };
+    // displacement of the lexicographic index by +-1 in mu / nu
+    const long dmu[3] = { c[MU] == 0 ? (long)(ext[MU] - 1) * str[MU] : -str[MU], 0, c[MU] == ext[MU] - 1 ? -(long)(ext[MU] - 1) * str[MU] : str[MU] };
+    const long dnu[3] = { c[NU] == 0 ? (long)(ext[NU] - 1) * str[NU] : -str[NU], 0, c[NU] == ext[NU] - 1 ? -(long)(ext[NU] - 1) * str[NU] : str[NU] };
+    auto link = [&](Real (&m)[M], int dm, int dn, int dir) {
+        const size_t s = (size_t)((lex + dmu[dm + 1] + dnu[dn + 1]) >> 1);
+        const int qy = par ^ ((dm + dn) & 1);
+        const char *base = (const char *)a.links + (size_t)(qy * 4 + dir) * LNREAL * sizeof(Real) * vh;
+        if constexpr (RL) {
+            Real r[LNREAL];
+            load_record<LD_DEFAULT, LNREAL>(r, base, vh, s, 0);
+#pragma unroll
+            for (int e = 0; e < D * D; ++e) { m[2 * e] = r[e]; m[2 * e + 1] = 0; }
+        } else {
+            load_record<LD_DEFAULT, LNREAL>(m, base, vh, s, 0);
+        }
+    };
+    Real p[M], r[M], u[M], v[M];
+#pragma unroll
+    for (int e = 0; e < M; ++e) q[e] = 0;
+    // U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
+    link(u, 0, 0, MU); link(v, 1, 0, NU);
+    cmm<Real, D, false, false>(p, u, v);
+    link(u, 0, 1, MU);
+    cmm<Real, D, false, true>(r, p, u);
+    link(v, 0, 0, NU);                                           // U_nu(x): also the first factor of the next leaf
+    cmm<Real, D, false, true>(p, r, v);
+#pragma unroll
+    for (int e = 0; e < M; ++e) q[e] += p[e];
+    // U_nu(x) U_mu(x-mu+nu)^dag U_nu(x-mu)^dag U_mu(x-mu)
+    link(u, -1, 1, MU);
+    cmm<Real, D, false, true>(p, v, u);
+    link(u, -1, 0, NU);
+    cmm<Real, D, false, true>(r, p, u);
+    link(v, -1, 0, MU);                                          // U_mu(x-mu): first factor of the next leaf
+    cmm<Real, D, false, false>(p, r, v);
+#pragma unroll
+    for (int e = 0; e < M; ++e) q[e] += p[e];
+    // U_mu(x-mu)^dag U_nu(x-mu-nu)^dag U_mu(x-mu-nu) U_nu(x-nu)
+    link(u, -1, -1, NU);
+    cmm<Real, D, true, true>(p, v, u);
+    link(u, -1, -1, MU);
+    cmm<Real, D, false, false>(r, p, u);
+    link(v, 0, -1, NU);                                          // U_nu(x-nu): first factor of the next leaf
+    cmm<Real, D, false, false>(p, r, v);
+#pragma unroll
+    for (int e = 0; e < M; ++e) q[e] += p[e];
+    // U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag
+    link(u, 0, -1, MU);
+    cmm<Real, D, true, false>(p, v, u);
+    link(u, 1, -1, NU);
+    cmm<Real, D, false, false>(r, p, u);
+    link(v, 0, 0, MU);
+    cmm<Real, D, false, true>(p, r, v);
+#pragma unroll
+    for (int e = 0; e < M; ++e) q[e] += p[e];
+}
+
+template <typename Real, int D, bool RL>
+__global__ void __launch_bounds__(64) clover_plane_kernel(const CloverArgs a, Real *scratch, long first, long n)
+{
+    constexpr int M = 2 * D * D;
+    const long loc = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (loc >= n) return;
+    const long idx = first + loc;                                  // even-odd site index: [parity][half index]
+    const int par = idx >= a.vh ? 1 : 0;
+    int c[4];
+    long lex;
+    {
+        long r = idx - (long)par * a.vh;
+        const int Zh = a.Z / 2;
+        const int zh = (int)(r % Zh); r /= Zh;
+        c[2] = (int)(r % a.Y); r /= a.Y;
+        c[1] = (int)(r % a.X);
+        c[0] = (int)(r / a.X);
+        c[3] = 2 * zh + ((c[0] + c[1] + c[2] + par) & 1);
+        lex = (((long)c[0] * a.X + c[1]) * a.Y + c[2]) * a.Z + c[3];
+    }
+    Real q[M];
+    const int plane = (int)blockIdx.y;                             // (0,1) (0,2) (0,3) (1,2) (1,3) (2,3)
+    switch (plane) {
+    case 0: clover_plane<Real, D, RL, 0, 1>(a, c, par, lex, q); break;
+    case 1: clover_plane<Real, D, RL, 0, 2>(a, c, par, lex, q); break;
+    case 2: clover_plane<Real, D, RL, 0, 3>(a, c, par, lex, q); break;
+    case 3: clover_plane<Real, D, RL, 1, 2>(a, c, par, lex, q); break;
+    case 4: clover_plane<Real, D, RL, 1, 3>(a, c, par, lex, q); break;
+    default: clover_plane<Real, D, RL, 2, 3>(a, c, par, lex, q); break;
+    }
+    // F = (Q - Q^dag)/(8i):  F_re = Im(Q - Q^dag)/8, F_im = -Re(Q - Q^dag)/8  (as clover_build_kernel / clover_pack_kernel)
+    // scratch: [plane][real index 2 (row D + col) + re/im][site of the chunk]
+#pragma unroll
+    for (int r = 0; r < D; ++r)
+#pragma unroll
+        for (int c2 = 0; c2 < D; ++c2) {
+            const Real gre = q[2 * (r * D + c2)] - q[2 * (c2 * D + r)];
+            const Real gim = q[2 * (r * D + c2) + 1] + q[2 * (c2 * D + r) + 1];
+            scratch[((size_t)plane * M + 2 * (r * D + c2)) * (size_t)n + (size_t)loc] = gim * (Real)0.125;
+            scratch[((size_t)plane * M + 2 * (r * D + c2) + 1) * (size_t)n + (size_t)loc] = -gre * (Real)0.125;
+        }
+}
+
+// T from the six F of clover_plane_kernel, d_R <= 4: one thread per site, every index a compile-time constant (no local
+// arrays); an element of T is formed from the two or four F entries it needs (coalesced loads from the scratch, which the
+// plane kernel has just left in L2) and leaves through a 16-byte vector as soon as the vector is complete.
+//   up: A = F01 - F23, B = F02 + F13, C = F03 - F12;   dn: A = -F01 - F23, B = -F02 + F13, C = -F03 - F12
+//   T_b = -(c_sw/2) [[C, A - iB], [A + iB, -C]], packed: the 2 d_R diagonal entries, then the strict upper triangle
+template <typename Real, int D, bool RL>
+__global__ void __launch_bounds__(128) clover_pack_f_kernel(const CloverArgs a, const Real *scratch, long first, long n)
+{
+    using G = CloverGeom<Real, D, RL>;
+    constexpr int M = 2 * D * D, RPV = 16 / (int)sizeof(Real);
+    const long loc = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (loc >= n) return;
+    const long idx = first + loc;
+    const int qpar = idx >= a.vh ? 1 : 0;
+    const size_t hs = (size_t)(idx - (long)qpar * a.vh), vh = (size_t)a.vh;
+    char *out = (char *)a.clover + (size_t)qpar * G::NREAL * sizeof(Real) * vh + hs * 16;
+    const Real k = (Real)(-0.5 * a.csw);
+    auto F = [&](int plane, int e) -> Real { return scratch[((size_t)plane * M + e) * (size_t)n + (size_t)loc]; };
+    // planes: 0 (0,1)  1 (0,2)  2 (0,3)  3 (1,2)  4 (1,3)  5 (2,3)
+    static_assert(G::BLK % RPV == 0, "a block is a whole number of vectors");
+#pragma unroll 1
+    for (int b = 0; b < 2; ++b) {
+        const Real sg = b ? (Real)-1 : (Real)1;                    // sign of F01, F02, F03 in the block
+        char *ob = out + (size_t)(b * (G::BLK / RPV)) * vh * 16;
+        Real buf[RPV];
+        int w = 0;                                                 // position in the block: compile-time once unrolled
+        auto put = [&](Real v) {
+            buf[w % RPV] = v;
+            if (++w % RPV == 0) {
+                if constexpr (sizeof(Real) == 8) st16<ST_DEFAULT>(ob + (size_t)(w / RPV - 1) * vh * 16, buf[0], buf[1]);
+                else st16<ST_DEFAULT>(ob + (size_t)(w / RPV - 1) * vh * 16, buf[0], buf[1], buf[2], buf[3]);
+            }
+        };
+        auto elem = [&](int row, int col, Real &re, Real &im) {
+            const int sr = row / D, ar = row % D, sc = col / D, ac = col % D;
+            const int e = 2 * (ar * D + ac);
+            if (sr == sc) {                                         // +-C, C = +-F03 - F12
+                const Real cr = sg * F(2, e) - F(3, e), ci = sg * F(2, e + 1) - F(3, e + 1);
+                re = sr ? -cr : cr; im = sr ? -ci : ci;
+            } else {                                                // (0,1): A - iB,  A = +-F01 - F23, B = +-F02 + F13
+                const Real Ar = sg * F(0, e) - F(5, e), Ai = sg * F(0, e + 1) - F(5, e + 1);
+                const Real Br = sg * F(1, e) + F(4, e), Bi = sg * F(1, e + 1) + F(4, e + 1);
+                re = Ar + Bi; im = Ai - Br;
+            }
+            re *= k; im *= k;
+        };
+#pragma unroll
+        for (int d = 0; d < 2 * D; ++d) { Real re, im; elem(d, d, re, im); put(re); }
+#pragma unroll
+        for (int r = 0; r < 2 * D; ++r)
+#pragma unroll
+            for (int c2 = 0; c2 < 2 * D; ++c2)                      // rectangular bounds: the compiler unrolls them fully
+                if (c2 > r) { Real re, im; elem(r, c2, re, im); put(re); put(im); }
+    }
+}
+
 // ---- row-parallel build for d_R > 4 ------------------------------------------------------------------------------------
 // clover_build_kernel keeps d_R x d_R matrices in thread-local arrays and is bound by local-memory traffic from d_R = 6 on
 // (80 ms for the sextet at 24^3 x 48).  Here one thread owns ONE ROW of the plaquette products: row_i(M1 M2 M3 M4) =
@@ -540,7 +712,7 @@ static hr_status launched(const char *what)
 size_t clover_nreal(const hr_ctx *c) { return (size_t)8 * c->d * c->d; }
 
 // d_R > 4: rows of Q for a chunk of sites into a stream-ordered scratch allocation, then the packing kernel
-template <typename Real, int D, bool RL>
+template <typename Real, int D, bool RL, bool PLANES = false>
 static hr_status build_rows(const hr_ctx *c, const CloverArgs &a, cudaStream_t st)
 {
     const long total = c->V;
@@ -556,11 +728,13 @@ static hr_status build_rows(const hr_ctx *c, const CloverArgs &a, cudaStream_t s
     hr_status rc = HR_OK;
     for (long first = 0; first < total && rc == HR_OK; first += chunk) {
         const long n = total - first < chunk ? total - first : chunk;
-        clover_q_kernel<Real, D, RL><<<(unsigned)((n + 31) / 32), 32 * D, 0, st>>>(a, scratch, first, n);
-        rc = launched("clover_q_kernel");
+        if constexpr (PLANES) clover_plane_kernel<Real, D, RL><<<dim3((unsigned)((n + 63) / 64), 6), 64, 0, st>>>(a, scratch, first, n);
+        else clover_q_kernel<Real, D, RL><<<(unsigned)((n + 31) / 32), 32 * D, 0, st>>>(a, scratch, first, n);
+        rc = launched(PLANES ? "clover_plane_kernel" : "clover_q_kernel");
         if (rc != HR_OK) break;
-        clover_pack_kernel<Real, D, RL><<<(unsigned)((n + 63) / 64), 64, 0, st>>>(a, scratch, first, n);
-        rc = launched("clover_pack_kernel");
+        if constexpr (PLANES) clover_pack_f_kernel<Real, D, RL><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(a, scratch, first, n);
+        else clover_pack_kernel<Real, D, RL><<<(unsigned)((n + 63) / 64), 64, 0, st>>>(a, scratch, first, n);
+        rc = launched(PLANES ? "clover_pack_f_kernel" : "clover_pack_kernel");
     }
     cudaFreeAsync(scratch, st);
     return rc;
@@ -577,8 +751,11 @@ hr_status launch_clover_build(const hr_ctx *c, hr_prec prec, void *clover, const
 #define X(D, RL)                                                                                                      \
     if (c->d == D && rl == RL) {                                                                                      \
         if (D > 4) return prec == HR_F64 ? build_rows<double, D, RL>(c, a, st) : build_rows<float, D, RL>(c, a, st);   \
-        if (prec == HR_F64) clover_build_kernel<double, D, RL><<<grid, 64, 0, st>>>(a);                              \
-        else clover_build_kernel<float, D, RL><<<grid, 64, 0, st>>>(a);                                              \
+        /* plane-parallel form where it wins (measured): complex d_R = 3, and d_R = 4 in fp64 */ \
+        if ((D == 3 && !RL) || (D == 4 && prec == HR_F64))                                                             \
+            return prec == HR_F64 ? build_rows<double, (D <= 4 ? D : 2), RL, true>(c, a, st) : build_rows<float, (D <= 4 ? D : 2), RL, true>(c, a, st); \
+        if (prec == HR_F64) clover_build_kernel<double, (D <= 4 ? D : 2), RL><<<grid, 64, 0, st>>>(a);               \
+        else clover_build_kernel<float, (D <= 4 ? D : 2), RL><<<grid, 64, 0, st>>>(a);                               \
         return launched("clover_build_kernel");                                                                       \
     }
     X(2, false) X(3, false) X(4, false) X(6, false) X(3, true) X(8, true)
