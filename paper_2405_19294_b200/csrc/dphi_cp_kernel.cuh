@@ -99,7 +99,13 @@ template <typename Real, int D, bool RL> struct CpGeom {
 #define HR_CP_RPT_PAD32 4
 #endif
 #ifndef HR_CP_RPT
-#define HR_CP_RPT (PAD ? (sizeof(Real) == 8 ? HR_CP_RPT_PAD64 : HR_CP_RPT_PAD32) : (D % 2 == 0 && (sizeof(Real) == 4 || RL)) ? 2 : 1)
+// two rows per thread for complex fp64 links too (a complex entry is already a whole vector; what is gained is half the
+// shared-memory reads of the half-spinor exchange and two link rows in flight per thread): measured, SU(3) sextet 24^3 x 48
+// 0.301 -> 0.290 ms (0.90 -> 0.94), SU(4) sextet d_R = 10 0.260 -> 0.264 ms -- so at d_R = 6 only
+#ifndef HR_CP_RPT2_F64C
+#define HR_CP_RPT2_F64C (D == 6)
+#endif
+#define HR_CP_RPT (PAD ? (sizeof(Real) == 8 ? HR_CP_RPT_PAD64 : HR_CP_RPT_PAD32) : (D % 2 == 0 && (sizeof(Real) == 4 || RL || HR_CP_RPT2_F64C)) ? 2 : 1)
 #endif
     static constexpr int LD = LinkGeom<RL ? LK_REAL : LK_COMPLEX, D>::LD;
     static constexpr bool PAD = LD != D;
