@@ -45,6 +45,38 @@ def test_import_export_roundtrip_bit_exact(hr, N, rep, prec):
     lat.close()
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("N,rep", COMBOS)
+def test_represented_field_import_export_and_use(hr, N, rep, prec):
+    """A REPRESENTED link field handed in by the caller (hr_gauge_import into a represented handle) instead of being made by
+    hr_represent_links: bit-exact round trip of the canonical d_R x d_R records -- for the SU(4) adjoint the internal record
+    has rows of d_R + 1 reals (include/hr.h, hr_gauge_bytes) and the canonical one does not -- and Dphi_eo on the imported
+    field equals the oracle."""
+    dims = (4, 2, 6, 10)
+    lat = hr.Lattice(dims, BC_T, N, rep)
+    p = hr.PREC_NAMES[prec]
+    R64 = oracle.represent(N, oracle_rep_id(rep), li.haar_links(13, N, dims))
+    if rep == "adj":
+        R = np.ascontiguousarray(R64.real).astype(np.float64 if prec == "f64" else np.float32)
+    else:
+        R = R64.astype(np.complex128 if prec == "f64" else np.complex64)
+    g = lat.gauge(True, p)
+    w = 8 if prec == "f64" else 4
+    ld = lat.d + 1 if (rep == "adj" and lat.d % 2 == 1 and lat.d > 8) else lat.d
+    assert hr.hr_gauge_bytes(lat.ctx, 1, p) == li.volume(dims) * 4 * lat.d * ld * w * (1 if rep == "adj" else 2)
+    lat.import_gauge(g, R)
+    back = lat.export_gauge(g, True, p)
+    assert back.dtype == R.dtype and back.shape == R.shape and np.array_equal(back, R)
+    for parity in (0, 1):
+        psi = li.gaussian_spinor(14 + parity, lat.vh, lat.d)
+        inp, out = lat.spinor(p), lat.spinor(p)
+        out.fill_(0xFF)
+        lat.import_spinor(inp, p, psi, 1 - parity)
+        lat.dphi_eo(out, inp, g, parity)
+        assert rel_l2(lat.export_spinor(out, p, parity), oracle.dphi_eo(dims, BC_T, R64, parity, psi)) <= TOL[prec]
+    lat.close()
+
+
 def test_import_from_device_canonical_equals_import_from_host(hr):
     import torch
     dims = (4, 4, 4, 6)
