@@ -37,7 +37,8 @@ def _bufs(hr, prob, n=4):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("N,rep,fundlinks", [(3, "fund", False), (2, "adj", False), (3, "sym", False), (3, "sym", True), (4, "asym", True)])
+@pytest.mark.parametrize("N,rep,fundlinks", [(3, "fund", False), (2, "adj", False), (3, "sym", False), (3, "sym", True), (4, "asym", True),
+                                            (4, "adj", False)])      # SU(4) adjoint: link records with padded rows
 @pytest.mark.parametrize("dims,bc", [((4, 4, 6, 8), BC_T), ((2, 2, 4, 2), (-1, 1, -1, 1)), ((6, 2, 2, 10), (1, 1, 1, 1))])
 def test_single_rank_slab_reproduces_dphi_eo(hr, dims, bc, N, rep, fundlinks, prec):
     from paper_2405_19294_b200 import halo
