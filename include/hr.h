@@ -150,8 +150,12 @@ hr_status hr_dirac(double m0, void *out_full, const void *in_full, const hr_gaug
  * (1-parity) half spinor `in_canon` (host, ideally pinned) to the device, packs it, runs hr_dphi_eo,
  * unpacks and copies the canonical result into `out_canon` (host).  `links` stays resident on the
  * device (a gauge field changes once per molecular-dynamics step, a spinor every call).  The
- * workspace (two internal half spinors + one staging buffer) is created on first use and cached in
- * the ctx.  Synchronises `stream` before returning.
+ * workspace (two internal half spinors + two 256 MiB staging buffers, two copy streams) is created on
+ * first use and cached in the ctx.  With host arrays and at least 8 time slices the call is a pipeline
+ * over chunks of time slices: upload of chunk k+1 || pack, Dphi_eo on the output slices of chunk k-1,
+ * unpack || download of chunk k-2 (the same result as the single launch up to the kernel variant's
+ * rounding).  Device pointers are accepted too (no staging).  Synchronises `stream` before returning:
+ * the host arrays are valid / reusable then.
  */
 hr_status hr_dphi_eo_host(hr_ctx *ctx, void *out_canon, const void *in_canon, hr_prec canon_prec,
                           const hr_gauge *links, int parity, void *stream);

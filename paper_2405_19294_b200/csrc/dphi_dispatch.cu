@@ -126,7 +126,9 @@ hr_status launch_dphi(const hr_ctx *c, hr_prec prec, const DphiArgs &a, cudaStre
         set_error("this kind of link field has no kernel for this representation (use hr_represent_links)");
         return HR_EUNSUPPORTED;
     }
-    const int v = a.site_mode != 0 ? resolve_variant_fused(c, prec, lk) : resolve_variant(c, prec, lk);
+    int v = a.site_mode != 0 ? resolve_variant_fused(c, prec, lk) : resolve_variant(c, prec, lk);
+    // a launch over a range of time slices (hr_dphi_eo_host's pipeline): the one-thread-per-site kernels take it
+    if (a.Tl != a.T && v != 0 && v != 1) v = (lk == 1 && c->d == 3) ? 1 : 0;
     const LaunchTune lt = { c->block, c->bulk_rows, c->bulk_stages, c->bulk_ctas, c->bulk_strip };
 #define X(D, LK)                                                                                          \
     if (c->d == D && lk == LK)                                                                            \

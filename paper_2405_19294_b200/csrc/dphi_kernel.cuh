@@ -491,8 +491,8 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
     const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
     long s = tid / KSPLIT;
     const int k = (int)(tid % KSPLIT);
-    const bool live = s < a.vh;
-    if (!live) s = a.vh - 1; // keep the pair convergent for the final shuffle; stores are predicated
+    const bool live = s < a.nsite;
+    if (!live) s = a.nsite - 1; // keep the pair convergent for the final shuffle; stores are predicated
 
     // Thread order -> site (a3).  Threads walk the lattice as [x / Xb][t][x % Xb][y][zh] while the
     // storage order stays [t][x][y][zh]: the +-t neighbours of a site are then Xb*Y*Zh threads away
@@ -504,8 +504,8 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
         g.zh = (int)(r % (unsigned)a.Zh); r /= (unsigned)a.Zh;
         g.y = (int)(r % (unsigned)a.Y); r /= (unsigned)a.Y;
         const int xl = (int)(r % (unsigned)a.Xb); r /= (unsigned)a.Xb;
-        g.t = (int)(r % (unsigned)a.T);
-        g.x = (int)(r / (unsigned)a.T) * a.Xb + xl;
+        g.t = a.t0 + (int)(r % (unsigned)a.Tl);              // the launch covers the slices [t0, t0 + Tl): all of them, or a chunk
+        g.x = (int)(r / (unsigned)a.Tl) * a.Xb + xl;
         g.b = (g.t + g.x + g.y + a.parity) & 1;
         s = (((long)g.t * a.X + g.x) * a.Y + g.y) * a.Zh + g.zh;
     }

@@ -80,7 +80,7 @@ static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
         set_error("block=%d not supported by this variant (multiple of 32, <= %d)", block, T::MAXT);
         return HR_EINVAL;
     }
-    const long nthreads = a.vh * KSPLIT;
+    const long nthreads = a.nsite * KSPLIT;
     const long grid = (nthreads + block - 1) / block;
     if (RED && (unsigned long)grid > kRedMaxBlocks) {
         set_error("fused Dphi reduction: %ld CTAs exceed the reduction scratch (%u)", grid, kRedMaxBlocks);

@@ -87,6 +87,25 @@ static const size_t kStageBytes = (size_t)256 << 20;
 
 enum FieldKind { FIELD_GAUGE, FIELD_SPINOR };
 
+// the context's two staging buffers, copy streams and events (first use of a host-pointer path)
+static hr_status ensure_staging(hr_ctx *mc)
+{
+    if (mc->stage[0]) return HR_OK;
+    HR_CUDA(cudaMalloc(&mc->stage[0], kStageBytes));
+    cudaError_t e = cudaMalloc(&mc->stage[1], kStageBytes);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&mc->copy_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&mc->copy_stream2, cudaStreamNonBlocking);
+    for (int b = 0; b < 2 && e == cudaSuccess; ++b) {
+        e = cudaEventCreateWithFlags(&mc->ev_copied[b], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&mc->ev_used[b], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&mc->ev_out_ready[b], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&mc->ev_out_copied[b], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) { cudaFree(mc->stage[0]); cudaFree(mc->stage[1]); mc->stage[0] = mc->stage[1] = nullptr; return cuda_fail("staging buffers", e); }
+    mc->stage_bytes = kStageBytes;
+    return HR_OK;
+}
+
 // canonical (host or device) <-> internal.  `nsites_total` = sites of the canonical array
 // (gauge: V full-lattice sites, 4 records each; spinor: Vh half-lattice sites of `parity`).
 static hr_status transfer(const hr_ctx *c, FieldKind kind, bool import, int nreal, void *internal, hr_prec prec,
@@ -117,17 +136,8 @@ static hr_status transfer(const hr_ctx *c, FieldKind kind, bool import, int nrea
     // (copy stream) overlaps the pack / unpack kernel of the other (caller's stream); one synchronisation at the end
     // (the host array must be reusable / valid when the call returns)
     hr_ctx *mc = const_cast<hr_ctx *>(c);
-    if (!mc->stage[0]) {
-        HR_CUDA(cudaMalloc(&mc->stage[0], kStageBytes));
-        cudaError_t e = cudaMalloc(&mc->stage[1], kStageBytes);
-        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&mc->copy_stream, cudaStreamNonBlocking);
-        for (int b = 0; b < 2 && e == cudaSuccess; ++b) {
-            e = cudaEventCreateWithFlags(&mc->ev_copied[b], cudaEventDisableTiming);
-            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&mc->ev_used[b], cudaEventDisableTiming);
-        }
-        if (e != cudaSuccess) { cudaFree(mc->stage[0]); cudaFree(mc->stage[1]); mc->stage[0] = mc->stage[1] = nullptr; return cuda_fail("staging buffers", e); }
-        mc->stage_bytes = kStageBytes;
-    }
+    rc = ensure_staging(mc);
+    if (rc != HR_OK) return rc;
     long chunk = (long)(kStageBytes / site_bytes);
     if (chunk < 1) { set_error("canonical record of %zu bytes exceeds the staging buffer", site_bytes); return HR_EUNSUPPORTED; }
     if (chunk > nsites) chunk = nsites;
@@ -210,6 +220,7 @@ hr_status hr_ctx_create(hr_ctx **ctx, const int dims[4], const int bc[4], int N,
     c->stage[0] = c->stage[1] = nullptr;
     c->stage_bytes = 0;
     c->copy_stream = nullptr;
+    c->copy_stream2 = nullptr;
     c->ws_in = c->ws_out = c->ws_stage = nullptr;
     c->ws_spinor_bytes = c->ws_stage_bytes = 0;
     c->ws_prec = -1;
@@ -228,8 +239,12 @@ void hr_ctx_destroy(hr_ctx *ctx)
             if (ctx->stage[0]) {
                 cudaFree(ctx->stage[0]);
                 cudaFree(ctx->stage[1]);
-                for (int b = 0; b < 2; ++b) { cudaEventDestroy(ctx->ev_copied[b]); cudaEventDestroy(ctx->ev_used[b]); }
+                for (int b = 0; b < 2; ++b) {
+                    cudaEventDestroy(ctx->ev_copied[b]); cudaEventDestroy(ctx->ev_used[b]);
+                    cudaEventDestroy(ctx->ev_out_ready[b]); cudaEventDestroy(ctx->ev_out_copied[b]);
+                }
                 cudaStreamDestroy(ctx->copy_stream);
+                cudaStreamDestroy(ctx->copy_stream2);
             }
             cudaFree(ctx->ws_in);
             cudaFree(ctx->ws_out);
@@ -408,6 +423,9 @@ void dphi_args(DphiArgs &a, const hr_ctx *c, void *out, const void *in, const vo
     a.skip = nullptr;
     a.site_mat = nullptr;
     a.site_mode = 0;
+    a.t0 = 0;
+    a.Tl = a.T;
+    a.nsite = a.vh;
 }
 
 // Reduction scratch of the ctx: [3 * kRedMaxBlocks doubles of per-CTA partials][16 doubles of results][ticket].
@@ -495,12 +513,83 @@ hr_status hr_dphi_eo_host(hr_ctx *ctx, void *out_canon, const void *in_canon, hr
         ctx->ws_spinor_bytes = sb;
         ctx->ws_prec = (int)links->prec;
     }
-    // chunked through the context's two staging buffers: copy of chunk k+1 || pack of chunk k, unpack of chunk k || copy of k-1
-    rc = transfer(ctx, FIELD_SPINOR, true, 8 * ctx->d, ctx->ws_in, links->prec, const_cast<void *>(in_canon), canon_prec, st);
+    bool in_dev = false, out_dev = false;
+    rc = pointer_on_device(in_canon, &in_dev);
+    if (rc == HR_OK) rc = pointer_on_device(out_canon, &out_dev);
     if (rc != HR_OK) return rc;
-    rc = hr_dphi_eo(ctx->ws_out, ctx->ws_in, links, parity, stream);
+    // Host arrays on a lattice with enough time slices: a three-stream pipeline over chunks of time slices,
+    //   host -> device copy of input chunk k+1  ||  pack k, Dphi_eo on the OUTPUT slices of chunk k-1, unpack  ||  device -> host
+    //   copy of output chunk k-2
+    // so that the two directions of the PCIe link are busy at once (PAPER.md:50 in miniature: compute what is there while the
+    // rest travels).  Output chunk j needs the input chunks j-1, j, j+1 (hops in t, periodic), so chunks 1 .. C-2 follow the
+    // uploads and the chunks C-1 and 0 come last.  Each staging buffer is used in halves (double buffering per direction).
+    const long slice = ctx->Vh / ctx->dims[0];                                   // half-lattice sites of one time slice
+    const size_t rec = (size_t)8 * ctx->d * prec_bytes(canon_prec);              // canonical bytes per site
+    long ct = (long)((kStageBytes / 2) / ((size_t)slice * rec));                 // time slices per chunk
+    if (ct > ctx->dims[0] / 8) ct = ctx->dims[0] / 8;
+    const int T = ctx->dims[0];
+    const int C = ct >= 1 ? (int)((T + ct - 1) / ct) : 0;
+    if (in_dev || out_dev || C < 3 || dphi_link_kind(ctx, link_src(links)) < 0) {
+        // device arrays, or a lattice too short in t: whole-field upload, one launch, whole-field download
+        rc = transfer(ctx, FIELD_SPINOR, true, 8 * ctx->d, ctx->ws_in, links->prec, const_cast<void *>(in_canon), canon_prec, st);
+        if (rc != HR_OK) return rc;
+        rc = hr_dphi_eo(ctx->ws_out, ctx->ws_in, links, parity, stream);
+        if (rc != HR_OK) return rc;
+        return transfer(ctx, FIELD_SPINOR, false, 8 * ctx->d, ctx->ws_out, links->prec, out_canon, canon_prec, st);
+    }
+    rc = ensure_staging(ctx);
     if (rc != HR_OK) return rc;
-    return transfer(ctx, FIELD_SPINOR, false, 8 * ctx->d, ctx->ws_out, links->prec, out_canon, canon_prec, st);
+    cudaStream_t cin = ctx->copy_stream, cout = ctx->copy_stream2;
+    char *sin[2] = { (char *)ctx->stage[0], (char *)ctx->stage[0] + kStageBytes / 2 };
+    char *sout[2] = { (char *)ctx->stage[1], (char *)ctx->stage[1] + kStageBytes / 2 };
+    cudaError_t e = cudaSuccess;
+    int nexp = 0;
+    auto chunk_t0 = [&](int k) { return (int)(k * ct); };
+    auto chunk_tl = [&](int k) { return (int)((k + 1) * ct <= T ? ct : T - k * ct); };
+    auto import_chunk = [&](int k) -> hr_status {
+        const int b = k & 1;
+        const long first = (long)chunk_t0(k) * slice, n = (long)chunk_tl(k) * slice;
+        if (k >= 2) e = cudaStreamWaitEvent(cin, ctx->ev_used[b], 0);               // the pack of chunk k-2 has read this half
+        if (e == cudaSuccess) e = cudaMemcpyAsync(sin[b], (const char *)in_canon + (size_t)first * rec, (size_t)n * rec, cudaMemcpyHostToDevice, cin);
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_copied[b], cin);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->ev_copied[b], 0);
+        if (e != cudaSuccess) return cuda_fail("hr_dphi_eo_host: upload", e);
+        hr_status r = launch_pack_spinor(ctx, ctx->ws_in, links->prec, sin[b], canon_prec, first, n, st);
+        if (r == HR_OK && (e = cudaEventRecord(ctx->ev_used[b], st)) != cudaSuccess) r = cuda_fail("hr_dphi_eo_host: upload", e);
+        return r;
+    };
+    auto compute_export = [&](int j) -> hr_status {
+        const int m = nexp++ & 1;
+        const long first = (long)chunk_t0(j) * slice, n = (long)chunk_tl(j) * slice;
+        DphiArgs a;
+        const double zero[2] = { 0.0, 0.0 }, mhalf[2] = { -0.5, -0.5 };
+        dphi_args(a, ctx, ctx->ws_out, ctx->ws_in, nullptr, links, parity, zero, mhalf);
+        a.t0 = chunk_t0(j); a.Tl = chunk_tl(j); a.nsite = n;
+        hr_status r = launch_dphi(ctx, links->prec, a, st, link_src(links));
+        if (r != HR_OK) return r;
+        if (nexp > 2) e = cudaStreamWaitEvent(st, ctx->ev_out_copied[m], 0);        // the download two chunks ago has left this half
+        if (e != cudaSuccess) return cuda_fail("hr_dphi_eo_host: download", e);
+        r = launch_unpack_spinor(ctx, ctx->ws_out, links->prec, sout[m], canon_prec, first, n, st);
+        if (r != HR_OK) return r;
+        e = cudaEventRecord(ctx->ev_out_ready[m], st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(cout, ctx->ev_out_ready[m], 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync((char *)out_canon + (size_t)first * rec, sout[m], (size_t)n * rec, cudaMemcpyDeviceToHost, cout);
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_out_copied[m], cout);
+        return e == cudaSuccess ? HR_OK : cuda_fail("hr_dphi_eo_host: download", e);
+    };
+    for (int k = 0; k < C && rc == HR_OK; ++k) {
+        rc = import_chunk(k);
+        if (rc == HR_OK && k >= 2) rc = compute_export(k - 1);
+    }
+    if (rc == HR_OK) rc = compute_export(C - 1);
+    if (rc == HR_OK) rc = compute_export(0);
+    // the host arrays must be valid / reusable when the call returns
+    cudaError_t e1 = cudaStreamSynchronize(st), e2 = cudaStreamSynchronize(cin), e3 = cudaStreamSynchronize(cout);
+    if (rc == HR_OK && (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess)) {
+        cudaGetLastError();
+        rc = cuda_fail("hr_dphi_eo_host: pipeline", e1 != cudaSuccess ? e1 : e2 != cudaSuccess ? e2 : e3);
+    }
+    return rc;
 }
 
 hr_status hr_ctx_set_tuning(hr_ctx *ctx, const char *key, int value)

@@ -43,6 +43,9 @@ struct hr_ctx {
     size_t stage_bytes;
     cudaStream_t copy_stream;
     cudaEvent_t ev_copied[2], ev_used[2];
+    // hr_dphi_eo_host's pipeline: a second copy stream (device -> host) and its events (created with the staging buffers)
+    cudaStream_t copy_stream2;
+    cudaEvent_t ev_out_ready[2], ev_out_copied[2];
     // device-resident state of hr_qmr_dhat (QmrState + history), created on first use, grown with maxiter
     void *qmr_state;
     size_t qmr_state_bytes;
@@ -121,6 +124,10 @@ struct DphiArgs {
     // site_mode 1: out = alpha self + beta hops + M self;  2: out = M (beta hops);  0: none.  One-thread-per-site kernels.
     const void *site_mat;
     int site_mode;
+    // output sites of this launch: the time slices [t0, t0 + Tl) -- the whole lattice (0, T) except for the chunks of
+    // hr_dphi_eo_host's copy / compute pipeline; nsite = Tl X Y Zh.  One-thread-per-site kernels only (launch_dphi checks).
+    int t0, Tl;
+    long nsite;
 };
 
 // device-resident state of the CG (cg.cu); the host only reads it

@@ -248,18 +248,32 @@ def test_repeated_launches_are_bitwise_identical(hr, N, rep, variant):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_host_entry_point_matches_oracle(hr, prec):
-    """hr_dphi_eo_host: canonical host buffers in, canonical host buffers out (the e2e call of bench.py)."""
+@pytest.mark.parametrize("dims,N,rep", [((4, 4, 6, 8), 3, "fund"),      # T < 8: whole-field upload, one launch, download
+                                        ((8, 4, 6, 8), 3, "fund"),      # 8 chunks of one time slice
+                                        ((26, 2, 2, 4), 3, "fund"),     # chunks of 3 slices, a ragged last chunk of 2
+                                        ((16, 2, 4, 2), 2, "adj"),      # real links
+                                        ((10, 4, 2, 6), 3, "sym"),      # default kernel = colour: the chunks take the site kernel
+                                        ((12, 2, 2, 4), 4, "adj")])
+def test_host_entry_point_matches_oracle(hr, dims, N, rep, prec):
+    """hr_dphi_eo_host: canonical host buffers in, canonical host buffers out (the e2e call of bench.py) -- from 8 time slices
+    on a pipeline over chunks of slices (upload || pack, Dphi on the chunk's output slices, unpack || download), the chunks
+    0 and C-1 last; every output site, both parities, antiperiodic t."""
     import torch
-    dims = (4, 4, 6, 8)
-    U, psi = make_inputs(dims, 3, 81, 82, 3)
-    want = oracle.dphi_eo(dims, BC_T, U, 1, psi)
-    prob = GpuProblem(hr, dims, 3, "fund", prec, U)
+    d = oracle.rep_dim(N, oracle_rep_id(rep))
+    U = li.haar_links(81, N, dims)
+    R = oracle.represent(N, oracle_rep_id(rep), U)
+    prob = GpuProblem(hr, dims, N, rep, prec, U)
     cdt = torch.complex128 if prec == "f64" else torch.complex64
-    inp = torch.from_numpy(psi).to(cdt).pin_memory()
-    out = torch.empty_like(inp).pin_memory()
-    hr.hr_dphi_eo_host(prob.lat.ctx, out, inp, hr.PREC_NAMES[prec], prob.links, 1, prob.lat.stream())
-    assert rel_l2(out.numpy(), want) <= TOL[prec]
+    for parity in (0, 1):
+        psi = li.gaussian_spinor(82 + parity, li.volume(dims) // 2, d)
+        want = oracle.dphi_eo(dims, BC_T, R, parity, psi)
+        inp = torch.from_numpy(psi).to(cdt).pin_memory()
+        out = torch.full_like(inp, float("nan")).pin_memory()
+        hr.hr_dphi_eo_host(prob.lat.ctx, out, inp, hr.PREC_NAMES[prec], prob.links, parity, prob.lat.stream())
+        assert rel_l2(out.numpy(), want) <= TOL[prec]
+        again = torch.full_like(inp, float("nan")).pin_memory()            # a second call re-uses the staging buffers and events
+        hr.hr_dphi_eo_host(prob.lat.ctx, again, inp, hr.PREC_NAMES[prec], prob.links, parity, prob.lat.stream())
+        assert torch.equal(out, again)
     prob.close()
 
 
