@@ -43,7 +43,7 @@ def test_version_string(hr):
 @pytest.mark.parametrize("N,rep,d,real", [
     (2, "fund", 2, 0), (2, "adj", 3, 1), (2, "sym", 3, 0),
     (3, "fund", 3, 0), (3, "adj", 8, 1), (3, "sym", 6, 0), (3, "asym", 3, 0),
-    (4, "fund", 4, 0), (4, "asym", 6, 0)])
+    (4, "fund", 4, 0), (4, "asym", 6, 0), (4, "sym", 10, 0), (4, "adj", 15, 1)])
 def test_ctx_geometry_and_sizes(hr, N, rep, d, real):
     dims = (4, 2, 6, 8)
     ctx = hr.hr_ctx_create(dims, (-1, 1, 1, 1), N, hr.REP_NAMES[rep], 0)
@@ -55,7 +55,8 @@ def test_ctx_geometry_and_sizes(hr, N, rep, d, real):
         for prec, w in ((hr.HR_F64, 8), (hr.HR_F32, 4)):
             assert hr.hr_spinor_bytes(ctx, prec) == (V // 2) * 4 * d * 2 * w          # S = 4 d_R complex per site
             assert hr.hr_gauge_bytes(ctx, 0, prec) == V * 4 * N * N * 2 * w            # F = N^2 complex
-            L = d * d * w * (1 if real else 2)                                         # real adjoint: half the bytes (C7)
+            ld = d + 1 if (real and d % 2 == 1 and d > 8) else d                        # SU(4) adjoint: internal rows of 16 reals
+            L = d * ld * w * (1 if real else 2)                                        # real adjoint: half the bytes (C7)
             assert hr.hr_gauge_bytes(ctx, 1, prec) == V * 4 * L
     finally:
         hr.hr_ctx_destroy(ctx)
@@ -75,6 +76,30 @@ def test_ctx_create_rejects_bad_arguments(hr, dims, bc, N, rep, status):
         hr.hr_ctx_create(dims, bc, N, rep, 0)
     assert e.value.status == status
     assert hr.hr_last_error() != ""
+
+
+@pytest.mark.parametrize("dims,N,rep,f64,f32", [
+    ((64, 64, 64, 64), 3, "fund", "site", "site"),          # config 5
+    ((64, 32, 32, 32), 3, "fund", "bulk", "site"),          # config 2: Z <= 32
+    ((32, 32, 32, 32), 2, "adj", "bulk", "site_ef"),        # config 3
+    ((48, 24, 24, 24), 3, "sym", "colour", "bulk2"),        # config 4: bulk2's tile is 8 rows x 12 sites
+    ((32, 32, 32, 32), 3, "sym", "colour", "bulk"),         # Zh = 16: bulk2's tile would have 64 sites -> bulk
+    ((48, 24, 24, 24), 3, "adj", "colour", "bulk2"),
+    ((32, 32, 32, 32), 3, "adj", "colour", "bulk"),
+    ((40, 32, 32, 32), 4, "fund", "bulk", "site"),
+    ((16, 32, 64, 64), 4, "fund", "site", "site"),          # Z = 64: the site kernel stays
+    ((56, 16, 16, 16), 4, "sym", "colour", "colour"),
+    ((48, 16, 16, 16), 4, "adj", "colour", "colour"),
+    ((8, 8, 8, 8), 3, "sym", "colour", "site_ef"),          # below 2^17 sites per parity: no persistent kernel
+    ((4, 4, 4, 4), 3, "fund", "site", "site")])
+def test_default_kernel_table(hr, dims, N, rep, f64, f32):
+    """The measured default kernel per (d_R, link type, precision, lattice shape): DESIGN.md "Kernels", profiles/r2_staging.md."""
+    ctx = hr.hr_ctx_create(dims, (-1, 1, 1, 1), N, hr.REP_NAMES[rep], 0)
+    try:
+        assert hr.hr_dphi_variant_name(ctx, hr.HR_F64) == f64
+        assert hr.hr_dphi_variant_name(ctx, hr.HR_F32) == f32
+    finally:
+        hr.hr_ctx_destroy(ctx)
 
 
 def test_tuning_keys_validated(hr):
