@@ -125,6 +125,10 @@ template <typename Real, int D, int LK> struct BulkGeom {
 // pair structure of dphi_kernel: no redundant spinor reads, both lanes read the same link vectors from shared memory --
 // a broadcast --, one shuffle at the end): half the live state per thread and twice the warps, for the sites whose
 // arithmetic (on-the-fly representations, d_R >= 6) is too much for four warps per SM.
+// KS = 2 tiles stop at 112 sites = 7 consumer warps + the producer warp = 8 warps, two per SM sub-partition, each with up to
+// 255 registers.  A 128-site tile would be 9 warps: three of them share one sub-partition's 16384 registers, i.e. at most 170
+// per thread (this is why ptxas budgets __launch_bounds__(288) like 384 threads; with __maxnreg__(224) instead the launch
+// fails with "too many resources requested") -- and at 168 registers these kernels spill.
 template <typename Real, int D, int LK, bool MASS, bool RED, int KS>
 #ifndef HR_BULK2_MINB
 #define HR_BULK2_MINB 1
