@@ -277,6 +277,22 @@ def test_host_entry_point_matches_oracle(hr, dims, N, rep, prec):
     prob.close()
 
 
+@pytest.mark.parametrize("dims", [(4, 4, 6, 8), (12, 2, 4, 6)])
+def test_host_entry_point_converts_the_canonical_precision(hr, dims):
+    """hr_dphi_eo_host with fp32 canonical arrays on an fp64 field (and the other way round): the conversion happens in the
+    pack / unpack kernels, whole-field and pipelined path alike; the error is the rounding of the fp32 side."""
+    import torch
+    U, psi = make_inputs(dims, 3, 85, 86, 3)
+    want = oracle.dphi_eo(dims, BC_T, U, 0, psi)
+    for prec, cdt in (("f64", torch.complex64), ("f32", torch.complex128)):
+        prob = GpuProblem(hr, dims, 3, "fund", prec, U)
+        inp = torch.from_numpy(psi).to(cdt).pin_memory()
+        out = torch.full_like(inp, float("nan")).pin_memory()
+        hr.hr_dphi_eo_host(prob.lat.ctx, out, inp, hr.HR_F32 if cdt == torch.complex64 else hr.HR_F64, prob.links, 0, prob.lat.stream())
+        assert rel_l2(out.numpy(), want) <= TOL["f32"]
+        prob.close()
+
+
 def test_argument_errors_on_the_gpu(hr):
     dims = (4, 4, 4, 4)
     U, psi = make_inputs(dims, 3, 91, 92, 3)
