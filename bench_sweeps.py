@@ -22,7 +22,7 @@ def volume(argv):
     for the curve, cf. Fig. 7's volume dependence, PAPER.md:116"; at small local lattices "the execution time
     is dominated by the kernel call overheads").
     
-        python bench_sweeps.py volume [--reps 200]
+        python bench_sweeps.py volume [--reps 200] [--graph]
     
     SU(3) fundamental, near-identity links (config 5's recipe), L^4 lattices, fp64 and fp32.  One JSON line per point:
     time per hr_dphi_eo launch (CUDA events, back to back, alternating parity, 4 rotating buffer sets), contract and
@@ -35,6 +35,7 @@ def volume(argv):
     ap = argparse.ArgumentParser(prog="bench_sweeps.py volume")
     ap.add_argument("--reps", type=int, default=200)
     ap.add_argument("--sizes", default="8,12,16,24,32,48,64")
+    ap.add_argument("--graph", action="store_true", help="also time 50 launches replayed from one CUDA graph (no host work between kernels)")
     args = ap.parse_args(argv)
     if not torch.cuda.is_available():
         raise SystemExit("bench_sweeps volume: no CUDA device; the product path has no CPU fallback")
@@ -69,9 +70,34 @@ def volume(argv):
                 torch.cuda.synchronize()
                 return e0.elapsed_time(e1) / args.reps
 
+            def timed_graph(fn, n=50):
+                # the same launches captured ONCE into a CUDA graph and replayed: no host work between the kernels, i.e. the
+                # time the GPU itself needs per launch (what a solver that replays a captured iteration sees)
+                s = torch.cuda.Stream()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.stream(s):
+                    fn_s = lambda k: fn(k, s.cuda_stream)
+                    for k in range(4):
+                        fn_s(k)
+                    s.synchronize()
+                    with torch.cuda.graph(g, stream=s):
+                        for k in range(n):
+                            fn_s(k)
+                    g.replay()
+                    s.synchronize()
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(s)
+                    for _ in range(max(1, args.reps // n)):
+                        g.replay()
+                    e1.record(s)
+                    s.synchronize()
+                return e0.elapsed_time(e1) / (max(1, args.reps // n) * n)
+
             ms = timed(lambda k: hr.hr_dphi_eo(o[k % 4], a[k % 4], links, k & 1, st))
             msc = timed(lambda k: hr.hr_spinor_copy(lat.ctx, P, o[k % 4], a[k % 4], st))
+            msg = timed_graph(lambda k, sp: hr.hr_dphi_eo(o[k % 4], a[k % 4], links, k & 1, sp)) if args.graph else None
             print(json.dumps({"workload": f"SU(3) fund {L}^4", "dtype": prec, "sites": vh, "dphi_us": ms * 1e3,
+                              "dphi_graph_us": None if msg is None else msg * 1e3, "kernel": lat.variant_name(P),
                               "contract_gbs": vh * (8 * Lb + 9 * S) / (ms * 1e-3) / 1e9,
                               "compulsory_gbs": vh * (8 * Lb + 2 * S) / (ms * 1e-3) / 1e9,
                               "compulsory_frac_of_copy_peak": vh * (8 * Lb + 2 * S) / (ms * 1e-3) / 1e9 / peak,

@@ -30,6 +30,13 @@
 #include <type_traits>
 
 #include "hr_internal.h"
+
+// HR_PDL: the one-thread-per-site / pair kernels are launched with programmatic stream serialization, so that back-to-back
+// Dphi launches overlap the launch latency of one with the tail of the other (small lattices: "dominated by the
+// kernel call overheads")
+#ifndef HR_PDL
+#define HR_PDL 1
+#endif
 #include "packed_f32.cuh"
 
 namespace hr {
@@ -481,6 +488,13 @@ __global__ void __launch_bounds__(MAXT, MINB) dphi_kernel(const DphiArgs a)
 {
     static_assert(!RED || MASS, "the fused reduction needs the self field");
     static_assert(CLV == 0 || (KSPLIT == 1 && !RED && (CLV != 1 || MASS) && (CLV != 2 || !MASS)), "fused site matrix: site kernels only");
+#if HR_PDL
+    // programmatic dependent launch (launch_one sets the stream-serialization attribute): this grid may be SCHEDULED while
+    // the previous kernel of the stream is still draining; nothing is read or written before the wait, which returns when
+    // that kernel has completed and its memory operations are visible.  launch_dependents lets the NEXT kernel do the same.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;");
+#endif
     if (a.skip != nullptr && *a.skip != 0) return;
     constexpr int LNREAL = LinkGeom<LK, D>::NREAL;         // reals per link record read by the kernel
     constexpr int RPV = 16 / (int)sizeof(Real);

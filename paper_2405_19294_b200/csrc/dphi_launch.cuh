@@ -86,7 +86,24 @@ static hr_status launch_one(int block, const DphiArgs &a, cudaStream_t st)
         set_error("fused Dphi reduction: %ld CTAs exceed the reduction scratch (%u)", grid, kRedMaxBlocks);
         return HR_EUNSUPPORTED;
     }
+#if HR_PDL
+    {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)grid);
+        cfg.blockDim = dim3((unsigned)block);
+        cfg.dynamicSmemBytes = 0;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        cudaError_t le = cudaLaunchKernelEx(&cfg, dphi_kernel<Real, D, LK, KSPLIT, MASS, RED, LHINT, SHINT, STHINT, T::MAXT, T::MINB, CLV>, a);
+        if (le != cudaSuccess) { set_error("dphi kernel launch failed: %s", cudaGetErrorString(le)); cudaGetLastError(); return HR_ECUDA; }
+    }
+#else
     dphi_kernel<Real, D, LK, KSPLIT, MASS, RED, LHINT, SHINT, STHINT, T::MAXT, T::MINB, CLV><<<(unsigned)grid, block, 0, st>>>(a);
+#endif
     count_launch();
     cudaError_t e = cudaPeekAtLastError();
     if (e != cudaSuccess) {
