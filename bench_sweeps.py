@@ -193,7 +193,7 @@ def solver(argv):
     algebra of PAPER.md:108-120 / Fig. 7 ("Copy spinor field", "g5 application", "g5 mulc add assign", norms and
     inner products; SU(3) fundamental), plus hr_dhat and one CG iteration.
     
-        python bench_sweeps.py solver [--config 2|3|4|5] [--prec f64|f32] [--reps 50]
+        python bench_sweeps.py solver [--config 2|3|4|5] [--prec f64|f32] [--reps 50] [--dims t,x,y,z]
     
     Prints one JSON line per operation: algorithmic bytes (S = spinor bytes per site, Vh sites: copy/g5 2S,
     g5_mulc_add_assign 3S, norm2 1S, dot 2S; Dhat 2(8L+2S)+S; CG iteration 4(8L+2S) + 2S + 8S), the time per call
@@ -209,10 +209,14 @@ def solver(argv):
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--reps", type=int, default=50)
     ap.add_argument("--m0", type=float, default=0.1)
+    ap.add_argument("--dims", default="", help="t,x,y,z: the config's gauge group and representation on another lattice")
     args = ap.parse_args(argv)
     if not torch.cuda.is_available():
         raise SystemExit("bench_sweeps solver: no CUDA device; the product path has no CPU fallback")
-    cfg = B.CONFIGS[args.config]
+    cfg = dict(B.CONFIGS[args.config])
+    if args.dims:
+        cfg["dims"] = tuple(int(x) for x in args.dims.split(","))
+        cfg["name"] = "%s on %s" % (cfg["name"], "x".join(str(x) for x in cfg["dims"]))
     bm = B.byte_model(cfg, args.prec)
     P = hr.PREC_NAMES[args.prec]
     peak, peak_src = B.measured_peak()
