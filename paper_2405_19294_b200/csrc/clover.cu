@@ -632,6 +632,89 @@ __global__ void __launch_bounds__(64) clover_exp_kernel(char *clover, long vh, d
 // preconditioned operator with a clover term needs A_oo^{-1}).  One thread per (site, chirality block); the n x n
 // block (n = 2 d_R <= 16) is inverted by Gauss-Jordan elimination with partial pivoting in fp64 (the inverse of a
 // Hermitian matrix is Hermitian, so it packs the same way).  Set-up kernel.
+// Inverse of a Hermitian POSITIVE DEFINITE n x n block in registers, every index a compile-time constant: A = L L^H
+// (Cholesky, no pivoting needed for a positive definite matrix), M = L^{-1}, A^{-1} = M^H M.  Packed storage as the clover
+// field: n real diagonal entries, then the strict upper triangle row by row.  Lower-triangular factors are stored at the
+// transposed position: X[i][j], i > j, at up(j, i).  Returns false -- and the caller falls back to Gauss-Jordan with partial
+// pivoting -- as soon as a pivot is not safely positive (A = (4+m0) + T is positive definite for any physical mass; a
+// negative or tiny shifted mass makes it indefinite).
+template <int N> __host__ __device__ constexpr int up(int r, int c) { return r * (2 * N - r - 1) / 2 + (c - r - 1); }
+
+template <int N>
+__device__ __forceinline__ bool hpd_inverse(const double (&ad)[N], const double (&ar)[N * (N - 1) / 2], const double (&ai)[N * (N - 1) / 2],
+                                            double (&od)[N], double (&orr)[N * (N - 1) / 2], double (&oi)[N * (N - 1) / 2])
+{
+    constexpr int NU = N * (N - 1) / 2;
+    double lr[NU], li[NU], id[N];
+    bool ok = true;
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+        double sdiag = ad[j];
+#pragma unroll
+        for (int k = 0; k < N; ++k)
+            if (k < j) sdiag -= lr[up<N>(k, j)] * lr[up<N>(k, j)] + li[up<N>(k, j)] * li[up<N>(k, j)];
+        ok = ok && (sdiag > 1e-12 * fabs(ad[j])) && (sdiag > 1e-300);
+        id[j] = rsqrt(ok ? sdiag : 1.0);
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+            if (i > j) {                                           // L[i][j] = (conj(A[j][i]) - sum_k L[i][k] conj(L[j][k])) / L[j][j]
+                double re = ar[up<N>(j, i)], im = -ai[up<N>(j, i)];
+#pragma unroll
+                for (int k = 0; k < N; ++k)
+                    if (k < j) {
+                        const double a = lr[up<N>(k, i)], b = li[up<N>(k, i)], c = lr[up<N>(k, j)], d = li[up<N>(k, j)];
+                        re -= a * c + b * d;
+                        im -= b * c - a * d;
+                    }
+                lr[up<N>(j, i)] = re * id[j];
+                li[up<N>(j, i)] = im * id[j];
+            }
+    }
+    if (!ok) return false;
+    // M = L^{-1}: M[j][j] = 1 / L[j][j],  M[i][j] = -(1 / L[i][i]) sum_{k = j}^{i-1} L[i][k] M[k][j]
+    double mr[NU], mi[NU];
+#pragma unroll
+    for (int j = 0; j < N; ++j)
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+            if (i > j) {
+                double re = lr[up<N>(j, i)] * id[j], im = li[up<N>(j, i)] * id[j];
+#pragma unroll
+                for (int k = 0; k < N; ++k)
+                    if (k > j && k < i) {
+                        const double a = lr[up<N>(k, i)], b = li[up<N>(k, i)], c = mr[up<N>(j, k)], d = mi[up<N>(j, k)];
+                        re += a * c - b * d;
+                        im += a * d + b * c;
+                    }
+                mr[up<N>(j, i)] = -id[i] * re;
+                mi[up<N>(j, i)] = -id[i] * im;
+            }
+    // A^{-1} = M^H M:  (r, c), r <= c:  sum_{k >= c} conj(M[k][r]) M[k][c]
+#pragma unroll
+    for (int r = 0; r < N; ++r) {
+        double dsum = id[r] * id[r];
+#pragma unroll
+        for (int k = 0; k < N; ++k)
+            if (k > r) dsum += mr[up<N>(r, k)] * mr[up<N>(r, k)] + mi[up<N>(r, k)] * mi[up<N>(r, k)];
+        od[r] = dsum;
+#pragma unroll
+        for (int c = 0; c < N; ++c)
+            if (c > r) {
+                double re = mr[up<N>(r, c)] * id[c], im = -mi[up<N>(r, c)] * id[c];   // k = c: conj(M[c][r]) M[c][c]
+#pragma unroll
+                for (int k = 0; k < N; ++k)
+                    if (k > c) {
+                        const double a = mr[up<N>(r, k)], b = mi[up<N>(r, k)], cc = mr[up<N>(c, k)], d = mi[up<N>(c, k)];
+                        re += a * cc + b * d;
+                        im += a * d - b * cc;
+                    }
+                orr[up<N>(r, c)] = re;
+                oi[up<N>(r, c)] = im;
+            }
+    }
+    return true;
+}
+
 template <typename Real, int D>
 __global__ void __launch_bounds__(64) clover_finalize_kernel(char *clover, char *inverse, long vh, double m)
 {
@@ -645,6 +728,28 @@ __global__ void __launch_bounds__(64) clover_finalize_kernel(char *clover, char 
     const size_t pb = (size_t)vh * 16;
     Real t[BLK];
     load_planes<LD_DEFAULT, NVB>(t, clover + off, pb, 0);
+    if constexpr (D <= 3) {
+        // fast path: positive definite block, everything in registers
+        constexpr int NU = N2 * (N2 - 1) / 2;
+        double ad[N2], ar[NU], ai[NU], od[N2], orr[NU], oi[NU];
+#pragma unroll
+        for (int d = 0; d < N2; ++d) ad[d] = (double)(Real)((double)t[d] + m);      // the stored A = m + T, rounded to Real as below
+#pragma unroll
+        for (int e = 0; e < NU; ++e) { ar[e] = (double)t[N2 + 2 * e]; ai[e] = (double)t[N2 + 2 * e + 1]; }
+        if (hpd_inverse<N2>(ad, ar, ai, od, orr, oi)) {
+            Real a_out[BLK], inv_out[BLK];
+#pragma unroll
+            for (int d = 0; d < N2; ++d) { a_out[d] = (Real)ad[d]; inv_out[d] = (Real)od[d]; }
+#pragma unroll
+            for (int e = 0; e < NU; ++e) {
+                a_out[N2 + 2 * e] = t[N2 + 2 * e]; a_out[N2 + 2 * e + 1] = t[N2 + 2 * e + 1];
+                inv_out[N2 + 2 * e] = (Real)orr[e]; inv_out[N2 + 2 * e + 1] = (Real)oi[e];
+            }
+            store_planes<ST_DEFAULT, NVB>(clover + off, pb, a_out);
+            store_planes<ST_DEFAULT, NVB>(inverse + off, pb, inv_out);
+            return;
+        }
+    }
     double x[M], y[M];
     for (int i = 0; i < M; ++i) { x[i] = 0; y[i] = 0; }
     {
