@@ -715,6 +715,9 @@ __device__ __forceinline__ bool hpd_inverse(const double (&ad)[N], const double 
     return true;
 }
 
+#ifndef HR_CLV_CHOL_MAXD
+#define HR_CLV_CHOL_MAXD 4
+#endif
 template <typename Real, int D>
 __global__ void __launch_bounds__(64) clover_finalize_kernel(char *clover, char *inverse, long vh, double m)
 {
@@ -728,7 +731,7 @@ __global__ void __launch_bounds__(64) clover_finalize_kernel(char *clover, char 
     const size_t pb = (size_t)vh * 16;
     Real t[BLK];
     load_planes<LD_DEFAULT, NVB>(t, clover + off, pb, 0);
-    if constexpr (D <= 3) {
+    if constexpr (D <= HR_CLV_CHOL_MAXD) {
         // fast path: positive definite block, everything in registers
         constexpr int NU = N2 * (N2 - 1) / 2;
         double ad[N2], ar[NU], ai[NU], od[N2], orr[NU], oi[NU];
