@@ -570,6 +570,35 @@ __global__ void __launch_bounds__(128) clover_apply_kernel(const CloverArgs a)
 // X = T / (m 2^6) is exponentiated by a 10-term Taylor series of expm1 (|X| < 0.1: remainder < 1e-22) and the result
 // is squared six times in the expm1 form  e(2X) = e(X)^2 + 2 e(X)  (no cancellation against the identity), then
 // packed back.  Set-up kernel: runtime loops over local arrays.
+// position of (r, c), r < c, in the packed strict upper triangle (row by row) of an N x N Hermitian matrix
+template <int N> __host__ __device__ constexpr int up(int r, int c) { return r * (2 * N - r - 1) / 2 + (c - r - 1); }
+
+// A Hermitian N x N matrix in registers: N real diagonal entries and the strict upper triangle; every index compile-time.
+template <int N> struct Herm {
+    double d[N], re[N * (N - 1) / 2], im[N * (N - 1) / 2];
+    __device__ __forceinline__ double er(int r, int c) const { return r == c ? d[r] : r < c ? re[up<N>(r, c)] : re[up<N>(c, r)]; }
+    __device__ __forceinline__ double ei(int r, int c) const { return r == c ? 0.0 : r < c ? im[up<N>(r, c)] : -im[up<N>(c, r)]; }
+};
+// C = A B for COMMUTING Hermitian A, B (polynomials of one matrix): the product is Hermitian, only its upper triangle is formed
+template <int N> __device__ __forceinline__ void herm_mul(Herm<N> &c, const Herm<N> &a, const Herm<N> &b)
+{
+#pragma unroll
+    for (int r = 0; r < N; ++r)
+#pragma unroll
+        for (int cc = 0; cc < N; ++cc)
+            if (cc >= r) {
+                double sr = 0, si = 0;
+#pragma unroll
+                for (int k = 0; k < N; ++k) {
+                    const double ar = a.er(r, k), ai = a.ei(r, k), br = b.er(k, cc), bi = b.ei(k, cc);
+                    sr += ar * br - ai * bi;
+                    if (cc > r) si += ar * bi + ai * br;
+                }
+                if (cc == r) c.d[r] = sr;
+                else { c.re[up<N>(r, cc)] = sr; c.im[up<N>(r, cc)] = si; }
+            }
+}
+
 template <typename Real, int D>
 __global__ void __launch_bounds__(64) clover_exp_kernel(char *clover, long vh, double m)
 {
@@ -583,6 +612,44 @@ __global__ void __launch_bounds__(64) clover_exp_kernel(char *clover, long vh, d
     const size_t pb = (size_t)vh * 16;
     Real t[BLK];
     load_planes<LD_DEFAULT, NVB>(t, rec, pb, 0);
+    if constexpr (D <= 3) {
+        // d_R <= 3: the same algorithm on Hermitian matrices held in registers (X, its powers and expm1(X) are Hermitian and
+        // commute): expm1(X) by Horner, s_k = (X + X s_{k+1}) / k from s_11 = 0 down to s_1, then six squarings
+        constexpr int NU = N2 * (N2 - 1) / 2;
+        const double sc = 1.0 / (m * 64.0);
+        Herm<N2> x, e, q;
+#pragma unroll
+        for (int d = 0; d < N2; ++d) x.d[d] = (double)t[d] * sc;
+#pragma unroll
+        for (int u = 0; u < NU; ++u) { x.re[u] = (double)t[N2 + 2 * u] * sc; x.im[u] = (double)t[N2 + 2 * u + 1] * sc; }
+#pragma unroll
+        for (int d = 0; d < N2; ++d) e.d[d] = x.d[d] * 0.1;
+#pragma unroll
+        for (int u = 0; u < NU; ++u) { e.re[u] = x.re[u] * 0.1; e.im[u] = x.im[u] * 0.1; }
+#pragma unroll 1
+        for (int k = 9; k >= 1; --k) {
+            herm_mul<N2>(q, x, e);
+            const double ik = 1.0 / k;
+#pragma unroll
+            for (int d = 0; d < N2; ++d) e.d[d] = (x.d[d] + q.d[d]) * ik;
+#pragma unroll
+            for (int u = 0; u < NU; ++u) { e.re[u] = (x.re[u] + q.re[u]) * ik; e.im[u] = (x.im[u] + q.im[u]) * ik; }
+        }
+#pragma unroll 1
+        for (int sq = 0; sq < 6; ++sq) {                               // expm1(2X) = expm1(X)^2 + 2 expm1(X)
+            herm_mul<N2>(q, e, e);
+#pragma unroll
+            for (int d = 0; d < N2; ++d) e.d[d] = q.d[d] + 2.0 * e.d[d];
+#pragma unroll
+            for (int u = 0; u < NU; ++u) { e.re[u] = q.re[u] + 2.0 * e.re[u]; e.im[u] = q.im[u] + 2.0 * e.im[u]; }
+        }
+#pragma unroll
+        for (int d = 0; d < N2; ++d) t[d] = (Real)(m * e.d[d]);
+#pragma unroll
+        for (int u = 0; u < NU; ++u) { t[N2 + 2 * u] = (Real)(m * e.re[u]); t[N2 + 2 * u + 1] = (Real)(m * e.im[u]); }
+        store_planes<ST_DEFAULT, NVB>(rec, pb, t);
+        return;
+    }
     double x[M], e[M], p[M], q[M];
     const double sc = 1.0 / (m * 64.0);
     for (int i = 0; i < M; ++i) x[i] = 0;
@@ -638,8 +705,6 @@ __global__ void __launch_bounds__(64) clover_exp_kernel(char *clover, long vh, d
 // transposed position: X[i][j], i > j, at up(j, i).  Returns false -- and the caller falls back to Gauss-Jordan with partial
 // pivoting -- as soon as a pivot is not safely positive (A = (4+m0) + T is positive definite for any physical mass; a
 // negative or tiny shifted mass makes it indefinite).
-template <int N> __host__ __device__ constexpr int up(int r, int c) { return r * (2 * N - r - 1) / 2 + (c - r - 1); }
-
 template <int N>
 __device__ __forceinline__ bool hpd_inverse(const double (&ad)[N], const double (&ar)[N * (N - 1) / 2], const double (&ai)[N * (N - 1) / 2],
                                             double (&od)[N], double (&orr)[N * (N - 1) / 2], double (&oi)[N * (N - 1) / 2])
