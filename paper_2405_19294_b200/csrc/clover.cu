@@ -695,6 +695,103 @@ __global__ void __launch_bounds__(64) clover_exp_kernel(char *clover, long vh, d
     store_planes<ST_DEFAULT, NVB>(rec, pb, t);
 }
 
+// d_R >= 4: ONE WARP per block.  The thread-per-block kernel above keeps four dense n x n complex matrices (n = 2 d_R = 12: 9 KB)
+// in local memory and takes 93 ms for the sextet at 24^3 x 48.  Here the three matrices of the Horner / squaring scheme
+// (X, E, Q; dense, n^2 complex each) live in shared memory, the n (n + 1) / 2 upper-triangle entries of a product of two
+// commuting Hermitian matrices are shared out over the 32 lanes (the lower triangle is the mirror image), and the record
+// is read and written by the lanes vector by vector.  Same algorithm, same fp64 arithmetic.
+#ifndef HR_CLV_EXP_PAD
+#define HR_CLV_EXP_PAD 1
+#endif
+template <int D> struct ExpWarp { static constexpr int WARPS = D >= 8 ? 2 : 4; };   // 3 n^2 complex per warp: 12 KB at n = 16
+template <typename Real, int D>
+__global__ void __launch_bounds__(32 * ExpWarp<D>::WARPS) clover_exp_warp_kernel(char *clover, long vh, double m)
+{
+    constexpr int N2 = 2 * D, LDA = N2 + HR_CLV_EXP_PAD, NC = N2 * LDA, NE = N2 * (N2 + 1) / 2, BLK = 4 * D * D, RPV = 16 / (int)sizeof(Real), NVB = BLK / RPV;
+    constexpr int WARPS = ExpWarp<D>::WARPS;
+    __shared__ double2 mat[WARPS][3][NC];                          // X, E, Q
+    __shared__ unsigned char rc_of[NE][2];                         // upper-triangle entry (diagonal first, then row by row) -> (r, c)
+    const int warp = (int)threadIdx.x >> 5, lane = (int)threadIdx.x & 31;
+    for (int e = (int)threadIdx.x; e < NE; e += (int)blockDim.x) {
+        if (e < N2) { rc_of[e][0] = rc_of[e][1] = (unsigned char)e; }
+        else {
+            int u = e - N2, r = 0;
+            while (u >= N2 - 1 - r) { u -= N2 - 1 - r; ++r; }
+            rc_of[e][0] = (unsigned char)r; rc_of[e][1] = (unsigned char)(r + 1 + u);
+        }
+    }
+    __syncthreads();
+    const long blk = (long)blockIdx.x * WARPS + warp;              // over 2 parities x vh sites x 2 blocks
+    if (blk >= 4 * vh) return;
+    const int b = (int)(blk & 1);
+    const long site = blk >> 1;
+    const long par = site / vh, s = site - par * vh;
+    char *rec = clover + (size_t)par * 2 * BLK * sizeof(Real) * (size_t)vh + (size_t)s * 16 + (size_t)(b * NVB) * (size_t)vh * 16;
+    const size_t pb = (size_t)vh * 16;
+    double2 *X = mat[warp][0], *E = mat[warp][1], *Q = mat[warp][2];
+    const double sc = 1.0 / (m * 64.0);
+    // packed real w of the record: w < N2 the diagonal entry w; else entry N2 + (w - N2) / 2 of rc_of, re or im
+    for (int v = lane; v < NVB; v += 32) {
+        Real tv[RPV];
+        load_planes<LD_DEFAULT, 1>(tv, rec + (size_t)v * pb, pb, 0);
+#pragma unroll
+        for (int i = 0; i < RPV; ++i) {
+            const int w = v * RPV + i;
+            const double val = (double)tv[i] * sc;
+            if (w < N2) X[w * LDA + w] = make_double2(val, 0.0);
+            else {
+                const int e = N2 + ((w - N2) >> 1), r = rc_of[e][0], c = rc_of[e][1];
+                if (((w - N2) & 1) == 0) { X[r * LDA + c].x = val; X[c * LDA + r].x = val; }
+                else { X[r * LDA + c].y = val; X[c * LDA + r].y = -val; }
+            }
+        }
+    }
+    __syncwarp();
+    auto mul = [&](double2 *o, const double2 *a, const double2 *bb) {   // o = a bb, commuting Hermitian matrices
+        for (int e = lane; e < NE; e += 32) {
+            const int r = rc_of[e][0], c = rc_of[e][1];
+            double re = 0, im = 0;
+#pragma unroll
+            for (int k = 0; k < N2; ++k) {
+                const double2 x = a[r * LDA + k], y = bb[k * LDA + c];
+                re += x.x * y.x - x.y * y.y;
+                im += x.x * y.y + x.y * y.x;
+            }
+            if (r == c) o[r * LDA + r] = make_double2(re, 0.0);
+            else { o[r * LDA + c] = make_double2(re, im); o[c * LDA + r] = make_double2(re, -im); }
+        }
+        __syncwarp();
+    };
+    for (int i = lane; i < NC; i += 32) E[i] = make_double2(X[i].x * 0.1, X[i].y * 0.1);
+    __syncwarp();
+    for (int k = 9; k >= 1; --k) {                                     // Horner: s_k = (X + X s_{k+1}) / k
+        mul(Q, X, E);
+        const double ik = 1.0 / k;
+        for (int i = lane; i < NC; i += 32) E[i] = make_double2((X[i].x + Q[i].x) * ik, (X[i].y + Q[i].y) * ik);
+        __syncwarp();
+    }
+    for (int sq = 0; sq < 6; ++sq) {                                   // expm1(2X) = expm1(X)^2 + 2 expm1(X)
+        mul(Q, E, E);
+        for (int i = lane; i < NC; i += 32) E[i] = make_double2(Q[i].x + 2.0 * E[i].x, Q[i].y + 2.0 * E[i].y);
+        __syncwarp();
+    }
+    for (int v = lane; v < NVB; v += 32) {
+        Real tv[RPV];
+#pragma unroll
+        for (int i = 0; i < RPV; ++i) {
+            const int w = v * RPV + i;
+            double val;
+            if (w < N2) val = E[w * LDA + w].x;
+            else {
+                const int e = N2 + ((w - N2) >> 1), r = rc_of[e][0], c = rc_of[e][1];
+                val = ((w - N2) & 1) == 0 ? E[r * LDA + c].x : E[r * LDA + c].y;
+            }
+            tv[i] = (Real)(m * val);
+        }
+        store_planes<ST_DEFAULT, 1>(rec + (size_t)v * pb, pb, tv);
+    }
+}
+
 // T (or E) -> A = (4+m0) + T in place, and A^{-1} into a second field of the same layout (reading C32: the even-odd
 // preconditioned operator with a clover term needs A_oo^{-1}).  One thread per (site, chirality block); the n x n
 // block (n = 2 d_R <= 16) is inverted by Gauss-Jordan elimination with partial pivoting in fp64 (the inverse of a
@@ -937,13 +1034,23 @@ hr_status launch_clover_build(const hr_ctx *c, hr_prec prec, void *clover, const
     return HR_EUNSUPPORTED;
 }
 
+#ifndef HR_CLV_EXP_WARP_MIND   // smallest d_R that takes the warp-per-block kernel
+#define HR_CLV_EXP_WARP_MIND 4
+#endif
 hr_status launch_clover_exp(const hr_ctx *c, hr_prec prec, void *clover, double m, cudaStream_t st)
 {
     const unsigned grid = (unsigned)((4 * c->Vh + 63) / 64);
 #define X(D)                                                                                                          \
     if (c->d == D) {                                                                                                  \
-        if (prec == HR_F64) clover_exp_kernel<double, D><<<grid, 64, 0, st>>>((char *)clover, c->Vh, m);             \
-        else clover_exp_kernel<float, D><<<grid, 64, 0, st>>>((char *)clover, c->Vh, m);                             \
+        if (D >= HR_CLV_EXP_WARP_MIND) {                                                                              \
+            constexpr int W = ExpWarp<(D >= 4 ? D : 4)>::WARPS;                                                       \
+            const unsigned gw = (unsigned)((4 * c->Vh + W - 1) / W);                                                  \
+            if (prec == HR_F64) clover_exp_warp_kernel<double, (D >= 4 ? D : 4)><<<gw, 32 * W, 0, st>>>((char *)clover, c->Vh, m); \
+            else clover_exp_warp_kernel<float, (D >= 4 ? D : 4)><<<gw, 32 * W, 0, st>>>((char *)clover, c->Vh, m);    \
+            return launched("clover_exp_warp_kernel");                                                                \
+        }                                                                                                             \
+        if (prec == HR_F64) clover_exp_kernel<double, (D < HR_CLV_EXP_WARP_MIND ? D : 2)><<<grid, 64, 0, st>>>((char *)clover, c->Vh, m); \
+        else clover_exp_kernel<float, (D < HR_CLV_EXP_WARP_MIND ? D : 2)><<<grid, 64, 0, st>>>((char *)clover, c->Vh, m); \
         return launched("clover_exp_kernel");                                                                         \
     }
     X(2) X(3) X(4) X(6) X(8)
