@@ -968,6 +968,173 @@ __global__ void __launch_bounds__(64) clover_finalize_kernel(char *clover, char 
     store_planes<ST_DEFAULT, NVB>(inverse + off, pb, t);
 }
 
+// d_R >= 6: ONE WARP per block, matrices in shared memory (the thread-per-block kernel above takes 42 ms for the sextet at
+// 24^3 x 48 and 106 ms for the SU(3) adjoint).  A = (4+m0) + T is factored in place, A = L L^H (right-looking Cholesky: the
+// pivot, the column scaling and the rank-1 update of the trailing triangle each shared out over the lanes), M = L^{-1} by
+// forward substitution (one lane per column), A^{-1} = M^H M (upper-triangle entries over the lanes).  A block that is not
+// safely positive definite is inverted by lane 0 with the pivoted Gauss-Jordan elimination of the kernel above, on the same
+// shared-memory matrices (any physical mass gives positive definite blocks; the path exists for correctness).
+template <int D> struct FinWarp { static constexpr int WARPS = D >= 8 ? 2 : 4; };
+template <typename Real, int D>
+__global__ void __launch_bounds__(32 * FinWarp<D>::WARPS) clover_finalize_warp_kernel(char *clover, char *inverse, long vh, double m)
+{
+    constexpr int N2 = 2 * D, LDA = N2 + 1, NC = N2 * LDA, NE = N2 * (N2 + 1) / 2, BLK = 4 * D * D, RPV = 16 / (int)sizeof(Real), NVB = BLK / RPV;
+    constexpr int WARPS = FinWarp<D>::WARPS;
+    __shared__ double2 mat[WARPS][2][NC];                          // A -> L (lower triangle), M / A^{-1}
+    __shared__ double idiag[WARPS][N2];                            // 1 / L[j][j]
+    __shared__ unsigned char rc_of[NE][2];                         // entry (diagonal first, then the upper triangle row by row) -> (r, c)
+    const int warp = (int)threadIdx.x >> 5, lane = (int)threadIdx.x & 31;
+    for (int e = (int)threadIdx.x; e < NE; e += (int)blockDim.x) {
+        if (e < N2) { rc_of[e][0] = rc_of[e][1] = (unsigned char)e; }
+        else {
+            int u = e - N2, r = 0;
+            while (u >= N2 - 1 - r) { u -= N2 - 1 - r; ++r; }
+            rc_of[e][0] = (unsigned char)r; rc_of[e][1] = (unsigned char)(r + 1 + u);
+        }
+    }
+    __syncthreads();
+    const long blk = (long)blockIdx.x * WARPS + warp;
+    if (blk >= 4 * vh) return;
+    const int b = (int)(blk & 1);
+    const long site = blk >> 1;
+    const long par = site / vh, s = site - par * vh;
+    const size_t off = (size_t)par * 2 * BLK * sizeof(Real) * (size_t)vh + (size_t)s * 16 + (size_t)(b * NVB) * (size_t)vh * 16;
+    const size_t pb = (size_t)vh * 16;
+    double2 *A = mat[warp][0], *Mi = mat[warp][1];
+    double *id = idiag[warp];
+    // load T, form A = m + T (the diagonal rounded to Real as it is stored), write A back, keep A dense in shared memory
+    auto load_a = [&](bool write_back) {
+        for (int v = lane; v < NVB; v += 32) {
+            Real tv[RPV];
+            load_planes<LD_DEFAULT, 1>(tv, clover + off + (size_t)v * pb, pb, 0);
+            bool touched = false;
+#pragma unroll
+            for (int i = 0; i < RPV; ++i) {
+                const int w = v * RPV + i;
+                if (w < N2) {
+                    if (write_back) { tv[i] = (Real)((double)tv[i] + m); touched = true; }
+                    A[w * LDA + w] = make_double2((double)tv[i], 0.0);
+                } else {
+                    const int e = N2 + ((w - N2) >> 1), r = rc_of[e][0], c = rc_of[e][1];
+                    const double val = (double)tv[i];
+                    if (((w - N2) & 1) == 0) { A[r * LDA + c].x = val; A[c * LDA + r].x = val; }
+                    else { A[r * LDA + c].y = val; A[c * LDA + r].y = -val; }
+                }
+            }
+            if (write_back && touched) store_planes<ST_DEFAULT, 1>(clover + off + (size_t)v * pb, pb, tv);
+        }
+        __syncwarp();
+    };
+    load_a(true);
+    if (lane < N2) Mi[lane * LDA + lane].x = A[lane * LDA + lane].x;   // the original diagonal, for the relative pivot test
+    __syncwarp();
+    bool ok = true;
+    for (int j = 0; j < N2; ++j) {
+        const double piv = A[j * LDA + j].x;
+        ok = ok && (piv > 1e-12 * fabs(Mi[j * LDA + j].x)) && (piv > 1e-300);
+        const double inv = rsqrt(ok ? piv : 1.0);
+        __syncwarp();
+        if (lane == 0) id[j] = inv;
+        for (int i = j + 1 + lane; i < N2; i += 32) { double2 &x = A[i * LDA + j]; x.x *= inv; x.y *= inv; }   // L[i][j]
+        __syncwarp();
+        for (int e = lane; e < NE; e += 32) {                          // A[i][k] -= L[i][j] conj(L[k][j]),  j < k <= i
+            const int k = rc_of[e][0], i = rc_of[e][1];
+            if (k > j) {
+                const double2 li = A[i * LDA + j], lk = A[k * LDA + j];
+                double2 &x = A[i * LDA + k];
+                x.x -= li.x * lk.x + li.y * lk.y;
+                x.y -= li.y * lk.x - li.x * lk.y;
+            }
+        }
+        __syncwarp();
+    }
+    if (ok) {
+        // M = L^{-1}: lane j owns column j
+        if (lane < N2) {
+            const int j = lane;
+            Mi[j * LDA + j] = make_double2(id[j], 0.0);
+            for (int i = j + 1; i < N2; ++i) {
+                double re = 0, im = 0;
+                for (int k = j; k < i; ++k) {
+                    const double2 l = A[i * LDA + k], x = Mi[k * LDA + j];
+                    re += l.x * x.x - l.y * x.y;
+                    im += l.x * x.y + l.y * x.x;
+                }
+                Mi[i * LDA + j] = make_double2(-id[i] * re, -id[i] * im);
+            }
+        }
+        __syncwarp();
+        // A^{-1}(r, c) = sum_{k >= c} conj(M[k][r]) M[k][c], r <= c: into the upper triangle of A's storage
+        for (int e = lane; e < NE; e += 32) {
+            const int r = rc_of[e][0], c = rc_of[e][1];
+            double re = 0, im = 0;
+            for (int k = c; k < N2; ++k) {
+                const double2 x = Mi[k * LDA + r], y = Mi[k * LDA + c];
+                re += x.x * y.x + x.y * y.y;
+                im += x.x * y.y - x.y * y.x;
+            }
+            A[r * LDA + c] = make_double2(re, r == c ? 0.0 : im);       // the upper triangle of A is free (L lives below)
+        }
+        __syncwarp();
+    } else {
+        // not positive definite: Gauss-Jordan with partial pivoting by one lane (x = A, y = identity -> A^{-1}), result into A
+        load_a(false);
+        if (lane == 0) {
+            double2 *x = A, *y = Mi;
+            for (int i = 0; i < N2; ++i)
+                for (int k = 0; k < N2; ++k) y[i * LDA + k] = make_double2(i == k ? 1.0 : 0.0, 0.0);
+            for (int col = 0; col < N2; ++col) {
+                int pv = col;
+                double best = -1.0;
+                for (int r = col; r < N2; ++r) {
+                    const double v = x[r * LDA + col].x * x[r * LDA + col].x + x[r * LDA + col].y * x[r * LDA + col].y;
+                    if (v > best) { best = v; pv = r; }
+                }
+                if (pv != col)
+                    for (int k = 0; k < N2; ++k) {
+                        double2 tmp = x[col * LDA + k]; x[col * LDA + k] = x[pv * LDA + k]; x[pv * LDA + k] = tmp;
+                        tmp = y[col * LDA + k]; y[col * LDA + k] = y[pv * LDA + k]; y[pv * LDA + k] = tmp;
+                    }
+                const double pr = x[col * LDA + col].x, pi = x[col * LDA + col].y;
+                const double den = pr * pr + pi * pi, ir = pr / den, ii = -pi / den;
+                for (int k = 0; k < N2; ++k) {
+                    double2 v = x[col * LDA + k];
+                    x[col * LDA + k] = make_double2(v.x * ir - v.y * ii, v.x * ii + v.y * ir);
+                    v = y[col * LDA + k];
+                    y[col * LDA + k] = make_double2(v.x * ir - v.y * ii, v.x * ii + v.y * ir);
+                }
+                for (int r = 0; r < N2; ++r) {
+                    if (r == col) continue;
+                    const double fr = x[r * LDA + col].x, fi = x[r * LDA + col].y;
+                    for (int k = 0; k < N2; ++k) {
+                        const double2 av = x[col * LDA + k], bv = y[col * LDA + k];
+                        x[r * LDA + k].x -= fr * av.x - fi * av.y; x[r * LDA + k].y -= fr * av.y + fi * av.x;
+                        y[r * LDA + k].x -= fr * bv.x - fi * bv.y; y[r * LDA + k].y -= fr * bv.y + fi * bv.x;
+                    }
+                }
+            }
+            for (int i = 0; i < N2; ++i)
+                for (int k = i; k < N2; ++k) x[i * LDA + k] = y[i * LDA + k];
+        }
+        __syncwarp();
+    }
+    for (int v = lane; v < NVB; v += 32) {
+        Real tv[RPV];
+#pragma unroll
+        for (int i = 0; i < RPV; ++i) {
+            const int w = v * RPV + i;
+            double val;
+            if (w < N2) val = A[w * LDA + w].x;
+            else {
+                const int e = N2 + ((w - N2) >> 1), r = rc_of[e][0], c = rc_of[e][1];
+                val = ((w - N2) & 1) == 0 ? A[r * LDA + c].x : A[r * LDA + c].y;
+            }
+            tv[i] = (Real)val;
+        }
+        store_planes<ST_DEFAULT, 1>(inverse + off + (size_t)v * pb, pb, tv);
+    }
+}
+
 static hr_status launched(const char *what)
 {
     count_launch();
@@ -1064,8 +1231,15 @@ hr_status launch_clover_finalize(const hr_ctx *c, hr_prec prec, void *clover, vo
     const unsigned grid = (unsigned)((4 * c->Vh + 63) / 64);
 #define X(D)                                                                                                          \
     if (c->d == D) {                                                                                                  \
-        if (prec == HR_F64) clover_finalize_kernel<double, D><<<grid, 64, 0, st>>>((char *)clover, (char *)inverse, c->Vh, m); \
-        else clover_finalize_kernel<float, D><<<grid, 64, 0, st>>>((char *)clover, (char *)inverse, c->Vh, m);       \
+        if (D >= 6) {                                                                                                 \
+            constexpr int W = FinWarp<(D >= 6 ? D : 6)>::WARPS;                                                       \
+            const unsigned gw = (unsigned)((4 * c->Vh + W - 1) / W);                                                  \
+            if (prec == HR_F64) clover_finalize_warp_kernel<double, (D >= 6 ? D : 6)><<<gw, 32 * W, 0, st>>>((char *)clover, (char *)inverse, c->Vh, m); \
+            else clover_finalize_warp_kernel<float, (D >= 6 ? D : 6)><<<gw, 32 * W, 0, st>>>((char *)clover, (char *)inverse, c->Vh, m); \
+            return launched("clover_finalize_warp_kernel");                                                           \
+        }                                                                                                             \
+        if (prec == HR_F64) clover_finalize_kernel<double, (D < 6 ? D : 2)><<<grid, 64, 0, st>>>((char *)clover, (char *)inverse, c->Vh, m); \
+        else clover_finalize_kernel<float, (D < 6 ? D : 2)><<<grid, 64, 0, st>>>((char *)clover, (char *)inverse, c->Vh, m); \
         return launched("clover_finalize_kernel");                                                                    \
     }
     X(2) X(3) X(4) X(6) X(8)
