@@ -14,6 +14,8 @@
 // hundreds of times per field in a solve), written with runtime loops over d_R.
 // clover_apply_kernel: out += T in, one thread per (site, chirality block), Hermitian block mat-vec unrolled on d_R;
 // algorithmic bytes per site: C + 3S (clover record, in, out read, out written).
+#include <type_traits>
+
 #include "hr_internal.h"
 
 namespace hr {
@@ -454,6 +456,103 @@ __global__ void __launch_bounds__(32 * D) clover_q_kernel(const CloverArgs a, Re
 #pragma unroll
             for (int j = 0; j < 2 * D; ++j) scratch[((size_t)plane * 2 * D * D + (size_t)row * 2 * D + j) * (size_t)n + (size_t)loc] = q[j];
         }
+}
+
+// clover_q_kernel with the links staged through shared memory: there the d_R row-threads of a site each fetch
+// all d_R^2 elements of every factor from L1 (d_R times the same matrix: 2736 element loads per thread at d_R = 6, one per four
+// FMAs -- the load/store unit binds it: 3.2 ms per 77k-site chunk).  Here the CTA (32 sites x d_R rows) copies a factor's
+// matrices once, d_R elements per thread, into one of two shared-memory buffers [element][site] and every row-thread reads
+// its operands from there (consecutive lanes = consecutive 16-byte words: conflict-free); the copy of the next factor is
+// issued before the arithmetic of this one, one barrier per factor.  Same products in the same order: same bits.
+template <typename Real> struct StagedReal { Real x; static constexpr Real y = 0; };   // a real link element (adjoint representation)
+template <typename Real, int D, bool RL>
+__global__ void __launch_bounds__(32 * D) clover_q_staged_kernel(const CloverArgs a, Real *scratch, long first, long n)
+{
+    constexpr int LNREAL = CloverGeom<Real, D, RL>::LNREAL;
+    using C2c = typename std::conditional<sizeof(Real) == 8, double2, float2>::type;
+    using C2r = typename std::conditional<RL, StagedReal<Real>, C2c>::type;
+    __shared__ C2r stg[2][D * D][32];
+    const int lane = (int)threadIdx.x & 31, row = (int)threadIdx.x >> 5;
+    long loc = (long)blockIdx.x * 32 + lane;
+    const bool live = loc < n;
+    if (!live) loc = n - 1;                                        // every thread stays for the barriers
+    const long idx = first + loc;                                  // even-odd site index: [parity][half index]
+    const int par = idx >= a.vh ? 1 : 0;
+    int c[4];
+    {
+        long r = idx - (long)par * a.vh;
+        const int Zh = a.Z / 2;
+        const int zh = (int)(r % Zh); r /= Zh;
+        c[2] = (int)(r % a.Y); r /= a.Y;
+        c[1] = (int)(r % a.X);
+        c[0] = (int)(r / a.X);
+        c[3] = 2 * zh + ((c[0] + c[1] + c[2] + par) & 1);
+    }
+    const int ext[4] = { a.T, a.X, a.Y, a.Z };
+    const size_t vh = (size_t)a.vh;
+    // factor g = ((plane * 4 + leaf) * 4 + f), g = 0 .. 95: copy my d_R elements (row `row` of the stored matrix) into buffer g & 1
+    auto stage = [&](int g) {
+        const int f = g & 3, leaf = (g >> 2) & 3, plane = g >> 4;
+        const int mu = plane < 3 ? 0 : plane < 5 ? 1 : 2, nu = plane < 3 ? plane + 1 : plane < 5 ? plane - 1 : 3;
+        const LeafFactor lf = kLeaf[leaf][f];
+        int y[4] = { c[0], c[1], c[2], c[3] };
+        y[mu] = (y[mu] + lf.dm + ext[mu]) % ext[mu];
+        y[nu] = (y[nu] + lf.dn + ext[nu]) % ext[nu];
+        const int qy = (y[0] + y[1] + y[2] + y[3]) & 1;
+        const size_t sy = (((size_t)y[0] * a.X + y[1]) * a.Y + y[2]) * (a.Z / 2) + y[3] / 2;
+        const char *base = (const char *)a.links + (size_t)(qy * 4 + (lf.nu_dir ? nu : mu)) * LNREAL * sizeof(Real) * vh;
+#pragma unroll
+        for (int j = 0; j < D; ++j) {
+            C2r v;
+            if constexpr (RL) load_real_any<LNREAL>(v.x, base, vh, sy, row * D + j);
+            else { Real re, im; load_cplx_any<LNREAL>(re, im, base, vh, sy, row * D + j); v.x = re; v.y = im; }
+            stg[g & 1][row * D + j][lane] = v;
+        }
+    };
+    stage(0);
+    __syncthreads();
+    Real q[2 * D], r[2 * D];
+    for (int g = 0; g < 96; ++g) {
+        const int f = g & 3, leaf = (g >> 2) & 3, plane = g >> 4;
+        if (g + 1 < 96) stage(g + 1);                                  // the other buffer: free since the barrier of factor g - 1
+        const bool dag = kLeaf[leaf][f].dag != 0;
+        const C2r (*m)[32] = stg[g & 1];
+        if (f == 0 && leaf == 0) {
+#pragma unroll
+            for (int j = 0; j < 2 * D; ++j) q[j] = 0;
+        }
+        if (f == 0) {                                                  // r = row `row` of op(M)
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                const C2r v = dag ? m[j * D + row][lane] : m[row * D + j][lane];
+                r[2 * j] = v.x; r[2 * j + 1] = dag ? -v.y : v.y;
+            }
+        } else {                                                       // r = r op(M)
+            Real rn[2 * D];
+#pragma unroll
+            for (int j = 0; j < 2 * D; ++j) rn[j] = 0;
+#pragma unroll
+            for (int k = 0; k < D; ++k)
+#pragma unroll
+                for (int j = 0; j < D; ++j) {
+                    const C2r v = dag ? m[j * D + k][lane] : m[k * D + j][lane];
+                    const Real mr = v.x, mi = dag ? -v.y : v.y;
+                    rn[2 * j] = fma(r[2 * k], mr, fma(-r[2 * k + 1], mi, rn[2 * j]));
+                    rn[2 * j + 1] = fma(r[2 * k], mi, fma(r[2 * k + 1], mr, rn[2 * j + 1]));
+                }
+#pragma unroll
+            for (int j = 0; j < 2 * D; ++j) r[j] = rn[j];
+        }
+        if (f == 3) {
+#pragma unroll
+            for (int j = 0; j < 2 * D; ++j) q[j] += r[j];
+            if (leaf == 3 && live) {
+#pragma unroll
+                for (int j = 0; j < 2 * D; ++j) scratch[((size_t)plane * 2 * D * D + (size_t)row * 2 * D + j) * (size_t)n + (size_t)loc] = q[j];
+            }
+        }
+        __syncthreads();                                               // buffer g & 1 may be overwritten, buffer (g + 1) & 1 is complete
+    }
 }
 
 template <typename Real, int D, bool RL>
@@ -1166,6 +1265,7 @@ static hr_status build_rows(const hr_ctx *c, const CloverArgs &a, cudaStream_t s
     for (long first = 0; first < total && rc == HR_OK; first += chunk) {
         const long n = total - first < chunk ? total - first : chunk;
         if constexpr (PLANES) clover_plane_kernel<Real, D, RL><<<dim3((unsigned)((n + 63) / 64), 6), 64, 0, st>>>(a, scratch, first, n);
+        else if constexpr (D >= 6) clover_q_staged_kernel<Real, D, RL><<<(unsigned)((n + 31) / 32), 32 * D, 0, st>>>(a, scratch, first, n);
         else clover_q_kernel<Real, D, RL><<<(unsigned)((n + 31) / 32), 32 * D, 0, st>>>(a, scratch, first, n);
         rc = launched(PLANES ? "clover_plane_kernel" : "clover_q_kernel");
         if (rc != HR_OK) break;
