@@ -291,3 +291,35 @@ def test_fused_and_unfused_clover_paths_agree(hr, variant):
     assert hr.hr_launch_count() - n0 == (2 if variant in (0, 1) else 4)
     assert rel_l2(lat.export_spinor(out, P, 0), clover.dhat_clover(dims, BC_T, U, m0, csw, psi[:V // 2])) <= TOL["f64"]
     prob.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("N,rep", [(3, "fund"), (4, "fund"), (3, "sym"), (3, "adj")])
+def test_clover_setup_kernels_are_bitwise_repeatable(hr, N, rep, prec):
+    """hr_clover_build / hr_clover_exp / hr_clover_finalize run the same arithmetic in the same order every time -- in
+    registers (d_R <= 3 / 4), or shared out over the lanes of a warp or the row-threads of a CTA through shared memory
+    (d_R >= 4 / 6): a missing barrier in those would show up as bytes that change from run to run (compute-sanitizer's
+    racecheck is not available on this pool).  Ragged sizes: the last CTA / warp group is partial."""
+    import torch
+    dims = (6, 2, 6, 2)                                        # 72 sites per parity: no multiple of 32, 4 or 2 warps' worth
+    prob = GpuProblem(hr, dims, N, rep, prec, li.haar_links(451, N, dims))
+    lat, P, st = prob.lat, prob.prec, prob.lat.stream()
+    nb = hr.hr_clover_bytes(lat.ctx, P)
+    runs = []
+    for _ in range(3):
+        T = torch.full((nb,), 0xFF, dtype=torch.uint8, device="cuda")
+        Ainv = torch.full((nb,), 0xFF, dtype=torch.uint8, device="cuda")
+        hr.hr_clover_build(T, prob.links, 1.2, st)
+        E = T.clone()
+        hr.hr_clover_exp(lat.ctx, P, E, -0.25, st)
+        A = E.clone()
+        hr.hr_clover_finalize(lat.ctx, P, A, Ainv, -0.25, st)
+        torch.cuda.synchronize()
+        runs.append((T, E, A, Ainv))
+    for k in (1, 2):
+        for a, b in zip(runs[0], runs[k]):
+            assert torch.equal(a, b)
+    for t in runs[0]:                                          # every byte was written (0xFF.. is a NaN pattern in both precisions)
+        v = t.view(torch.float64 if prec == "f64" else torch.float32)
+        assert not torch.isnan(v).any()
+    prob.close()
