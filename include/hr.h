@@ -404,7 +404,8 @@ hr_status hr_dphi_eo_halo_apply(void *out, const void *recv_prev, const void *re
  * A(x) = (4+m0) + T(x)  [or (4+m0) exp(T/(4+m0)) after hr_clover_exp]  and  D_sw = [[A_ee, Dphi_eo], [Dphi_oe, A_oo]],
  *     Dhat_sw = A_ee - Dphi_eo A_oo^{-1} Dphi_oe                                  (Schur complement on the even sites).
  * hr_clover_finalize: IN PLACE site_term (T or E, as written by hr_clover_build / hr_clover_exp) -> A = (4+m0) + it, and
- *     A^{-1} (every 2 d_R x 2 d_R block inverted by Gauss-Jordan elimination in fp64) into site_inverse, a second buffer
+ *     A^{-1} (every 2 d_R x 2 d_R block inverted in fp64: Cholesky where it is positive definite -- any physical mass --, else
+ *     Gauss-Jordan elimination with partial pivoting) into site_inverse, a second buffer
  *     of hr_clover_bytes().  After this call the buffers serve hr_dhat_clover / hr_dirac_clover_solve (NOT
  *     hr_dirac_clover, which expects T and adds 4+m0 itself).
  * hr_dhat_clover: out_e = Dhat_sw in_e; two Dphi launches and two site-local launches; tmp_o, tmp2_o: odd-parity half
