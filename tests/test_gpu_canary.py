@@ -35,7 +35,7 @@ class Guarded:
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("N,rep", [(3, "fund"), (2, "adj"), (3, "sym")])
+@pytest.mark.parametrize("N,rep", [(3, "fund"), (2, "adj"), (3, "sym"), (3, "adj"), (4, "fund"), (4, "adj")])
 def test_no_call_writes_outside_its_output(hr, N, rep, prec):
     dims = (6, 2, 6, 10)                       # V/2 = 360: 2 full CTAs + a ragged tail of 104 sites
     U = li.haar_links(501, N, dims)
@@ -77,8 +77,21 @@ def test_no_call_writes_outside_its_output(hr, N, rep, prec):
     hr.hr_dphi_eo_halo_pack(up.t, dn.t, gin, prob.links, 0, st)
     o = guarded(sb); hr.hr_dphi_eo_interior(o.t, gin, prob.links, 0, st)
     hr.hr_dphi_eo_halo_apply(o.t, up.t, dn.t, prob.links, 0, True, True, st)
-    cl = guarded(hr.hr_clover_bytes(ctx, P)); hr.hr_clover_build(cl.t, prob.links, 1.0, st)
-    o = guarded(2 * sb); hr.hr_dirac_clover(0.1, o.t, full_in, prob.links, cl.t, st)
+    if d <= 8:                                  # the clover kernels stop at d_R = 8
+        cl = guarded(hr.hr_clover_bytes(ctx, P)); hr.hr_clover_build(cl.t, prob.links, 1.0, st)
+        o = guarded(2 * sb); hr.hr_dirac_clover(0.1, o.t, full_in, prob.links, cl.t, st)
+        hr.hr_clover_exp(ctx, P, cl.t, 0.1, st)                      # in place
+        inv = guarded(hr.hr_clover_bytes(ctx, P)); hr.hr_clover_finalize(ctx, P, cl.t, inv.t, 0.1, st)
+        bad = guarded(hr.hr_clover_bytes(ctx, P)); hr.hr_clover_build(bad.t, prob.links, 1.0, st)
+        inv2 = guarded(hr.hr_clover_bytes(ctx, P)); hr.hr_clover_finalize(ctx, P, bad.t, inv2.t, -8.0, st)   # the pivoted path
+    # the faces of all four directions in one launch each (round 2), the rank being its own neighbour
+    fb = {mu: hr.hr_face_bytes(ctx, P, mu) for mu in range(4)}
+    fu = {mu: guarded(fb[mu]) for mu in range(4)}
+    fd = {mu: guarded(fb[mu]) for mu in range(4)}
+    hr.hr_dphi_eo_faces_pack(15, {mu: g.t for mu, g in fu.items()}, {mu: g.t for mu, g in fd.items()}, gin, prob.links, 0, st)
+    o = guarded(sb); hr.hr_dphi_eo_interior_mask(o.t, gin, prob.links, 0, 15, st)
+    hr.hr_dphi_eo_faces_apply(15, o.t, {mu: g.t for mu, g in fu.items()}, {mu: g.t for mu, g in fd.items()}, prob.links, 0, 15, 15, st)
+    r2 = guarded(16); hr.hr_spinor_dot_noalloc(ctx, P, gin, gin, r2.t, st)
     g = guarded(hr.hr_gauge_bytes(ctx, 1, P))
     h = hr.hr_gauge_alloc(ctx, 1, P, g.t)
     hr.hr_represent_links(h, prob.fund, st)
