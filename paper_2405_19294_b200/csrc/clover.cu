@@ -1288,8 +1288,8 @@ hr_status launch_clover_build(const hr_ctx *c, hr_prec prec, void *clover, const
 #define X(D, RL)                                                                                                      \
     if (c->d == D && rl == RL) {                                                                                      \
         if (D > 4) return prec == HR_F64 ? build_rows<double, D, RL>(c, a, st) : build_rows<float, D, RL>(c, a, st);   \
-        /* plane-parallel form where it wins (measured): complex d_R = 3, and d_R = 4 in fp64 */ \
-        if ((D == 3 && !RL) || (D == 4 && prec == HR_F64))                                                             \
+        /* plane-parallel form where it wins (measured): complex d_R = 3, and d_R = 4 */         \
+        if ((D == 3 && !RL) || D == 4)                                                                                 \
             return prec == HR_F64 ? build_rows<double, (D <= 4 ? D : 2), RL, true>(c, a, st) : build_rows<float, (D <= 4 ? D : 2), RL, true>(c, a, st); \
         if (prec == HR_F64) clover_build_kernel<double, (D <= 4 ? D : 2), RL><<<grid, 64, 0, st>>>(a);               \
         else clover_build_kernel<float, (D <= 4 ? D : 2), RL><<<grid, 64, 0, st>>>(a);                               \

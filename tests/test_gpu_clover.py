@@ -59,7 +59,7 @@ def test_dirac_clover_matches_oracle(hr, dims, N, rep, prec):
     cl.fill_(0xFF)
     n0 = hr.hr_launch_count()
     hr.hr_clover_build(cl, prob.links, csw, lat.stream())
-    two = d > 4 or (d == 3 and rep != "adj") or (d == 4 and prec == "f64")   # plane- or row-parallel Q kernel + packing kernel; else one kernel
+    two = d >= 4 or (d == 3 and rep != "adj")                     # plane- or row-parallel Q kernel + packing kernel; else one kernel
     assert hr.hr_launch_count() == n0 + (2 if two else 1)
     gin = _full(prob, psi)
     gout, gref = lat.spinor(P, full=True), lat.spinor(P, full=True)
