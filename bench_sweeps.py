@@ -299,6 +299,16 @@ def solver(argv):
         face_bytes[f"face_pack {nm}"] = nf_mu * (2 * S + Lk + S)
         face_bytes[f"face_apply {nm}"] = nf_mu * (S + Lk + 4 * S)
         face_sites[f"face_pack {nm}"] = face_sites[f"face_apply {nm}"] = nf_mu
+    if cfg["dims"][2] % 2 == 0:
+        # the faces of all four directions in ONE launch each (hr_dphi_eo_faces_pack / _apply): bytes = the sum of the per-direction ones
+        fb[0] = hb
+        fup, fdn = {mu: fb[mu][0] for mu in range(4)}, {mu: fb[mu][1] for mu in range(4)}
+        ops.append(("faces_pack t+x+y+z (one launch)", None, lambda k: hr.hr_dphi_eo_faces_pack(15, fup, fdn, sets[k % nset][0], links, k & 1, st)))
+        ops.append(("faces_apply t+x+y+z (one launch)", None,
+                    lambda k: hr.hr_dphi_eo_faces_apply(15, sets[k % nset][2], fup, fdn, links, k & 1, 15, 15, st)))
+        face_bytes["faces_pack t+x+y+z (one launch)"] = face_bytes["halo_pack"] + sum(face_bytes[f"face_pack {nm}"] for nm in "xyz")
+        face_bytes["faces_apply t+x+y+z (one launch)"] = face_bytes["halo_apply"] + sum(face_bytes[f"face_apply {nm}"] for nm in "xyz")
+        face_sites["faces_pack t+x+y+z (one launch)"] = face_sites["faces_apply t+x+y+z (one launch)"] = nface + sum(vh // cfg["dims"][mu] for mu in (1, 2, 3))
     ops.append(("dphi_eo_interior, all four directions masked", dphi_c,
                 lambda k: hr.hr_dphi_eo_interior_mask(sets[k % nset][2], sets[k % nset][0], links, k & 1, 15, st)))
     # NEXT-4: clover term.  build: reads the represented links (each link is used by many leaves; algorithmic bytes
