@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(64) clover_build_kernel(const CloverArgs a)
 // leaves (U_nu(x), U_mu(x-mu), U_nu(x-nu)) kept in registers: 13 link loads and 12 products per thread, live state
 // q + two partial products + two links.  The plane is uniform over a CTA (blockIdx.y) and a compile-time constant of the
 // code path; neighbour sites come from the lexicographic index by adding a stride (the wrap is a compare, not a modulo).
-// Q goes to the scratch layout of clover_q_kernel, clover_pack_kernel finishes.  (clover_build_kernel above holds all six
+// F goes to the scratch layout of clover_q_kernel, clover_pack_f_kernel finishes.  (clover_build_kernel above holds all six
 // planes of a site in one thread: 252 registers and 1.5 KB of local memory in fp64, and four integer divisions per link.)
 template <typename Real, int D, bool RL, int MU, int NU>
 __device__ __forceinline__ void clover_plane(const CloverArgs &a, const int (&c)[4], int par, long lex, Real (&q)[2 * D * D])
@@ -303,7 +303,7 @@ __global__ void __launch_bounds__(64) clover_plane_kernel(const CloverArgs a, Re
     case 4: clover_plane<Real, D, RL, 1, 3>(a, c, par, lex, q); break;
     default: clover_plane<Real, D, RL, 2, 3>(a, c, par, lex, q); break;
     }
-    // F = (Q - Q^dag)/(8i):  F_re = Im(Q - Q^dag)/8, F_im = -Re(Q - Q^dag)/8  (as clover_build_kernel / clover_pack_kernel)
+    // F = (Q - Q^dag)/(8i):  F_re = Im(Q - Q^dag)/8, F_im = -Re(Q - Q^dag)/8  (as clover_build_kernel / clover_pack_vec_kernel)
     // scratch: [plane][real index 2 (row D + col) + re/im][site of the chunk]
 #pragma unroll
     for (int r = 0; r < D; ++r)
@@ -378,7 +378,7 @@ __global__ void __launch_bounds__(128) clover_pack_f_kernel(const CloverArgs a, 
 // ((e_i^T M1) M2) M3) M4 is three vector-matrix products with the vector (d_R complex) in registers and the matrices
 // streamed from the link field through L1 -- the d_R threads of a site (d_R warps of a CTA, lanes = consecutive sites:
 // coalesced element loads) read the same links.  clover_q_kernel writes the rows of Q_{mu nu} (sum of the four leaves)
-// of a chunk of sites to a scratch buffer; clover_pack_kernel forms F = (Q - Q^dagger)/(8i) and packs T as above.
+// of a chunk of sites to a scratch buffer; clover_pack_vec_kernel forms F = (Q - Q^dagger)/(8i) and packs T as above.
 struct LeafFactor { signed char dm, dn, nu_dir, dag; };          // site offset (in mu, nu), link direction (0 mu / 1 nu), dagger
 __constant__ LeafFactor kLeaf[4][4] = {
     { { 0, 0, 0, 0 }, { 1, 0, 1, 0 }, { 0, 1, 0, 1 }, { 0, 0, 1, 1 } },       // U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
@@ -555,58 +555,53 @@ __global__ void __launch_bounds__(32 * D) clover_q_staged_kernel(const CloverArg
     }
 }
 
+// T from the six Q of the row-parallel kernels, any d_R: one thread per (site, 16-byte vector of the packed record) -- no
+// per-thread matrices at all (its predecessor held cf[2][3][2 d_R^2] per thread in local memory: 5.8 KB of stack at d_R = 6).  A
+// thread decodes which packed reals its vector holds, forms each from the F entries it needs (F = (Q - Q^dag)/(8i) on the
+// fly: two Q loads per F entry, coalesced over the sites of the chunk) and stores the vector; consecutive threads are
+// consecutive sites of the same vector, so loads and stores are coalesced.
 template <typename Real, int D, bool RL>
-__global__ void __launch_bounds__(64) clover_pack_kernel(const CloverArgs a, const Real *scratch, long first, long n)
+__global__ void __launch_bounds__(128) clover_pack_vec_kernel(const CloverArgs a, const Real *scratch, long first, long n)
 {
     using G = CloverGeom<Real, D, RL>;
-    constexpr int M = 2 * D * D;
-    const long loc = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (loc >= n) return;
+    constexpr int M = 2 * D * D, N2 = 2 * D, RPV = 16 / (int)sizeof(Real), NVREC = G::NREAL / RPV, NVBLK = G::BLK / RPV;
+    const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= n * NVREC) return;
+    const int v = (int)(tid / n);                                  // vector of the record
+    const long loc = tid - (long)v * n;
     const long idx = first + loc;
     const int qpar = idx >= a.vh ? 1 : 0;
-    const size_t hs = (size_t)(idx - (long)qpar * a.vh);
-    Real cf[2][3][M];
-    for (int b = 0; b < 2; ++b)
-        for (int k = 0; k < 3; ++k)
-            for (int e = 0; e < M; ++e) cf[b][k][e] = 0;
-    const int pk[6] = { 0, 1, 2, 2, 1, 0 };
-    const int su[6] = { 1, 1, 1, -1, 1, -1 };
-    const int sd[6] = { -1, -1, -1, -1, 1, -1 };
-    for (int plane = 0; plane < 6; ++plane) {
-        Real q[M];
-        for (int e = 0; e < M; ++e) q[e] = scratch[((size_t)plane * M + e) * (size_t)n + (size_t)loc];
-        for (int r = 0; r < D; ++r)
-            for (int s = 0; s < D; ++s) {
-                const Real gre = q[2 * (r * D + s)] - q[2 * (s * D + r)];
-                const Real gim = q[2 * (r * D + s) + 1] + q[2 * (s * D + r) + 1];
-                const Real fre = gim * (Real)0.125, fim = -gre * (Real)0.125;
-                cf[0][pk[plane]][2 * (r * D + s)] += su[plane] * fre;
-                cf[0][pk[plane]][2 * (r * D + s) + 1] += su[plane] * fim;
-                cf[1][pk[plane]][2 * (r * D + s)] += sd[plane] * fre;
-                cf[1][pk[plane]][2 * (r * D + s) + 1] += sd[plane] * fim;
-            }
+    const size_t hs = (size_t)(idx - (long)qpar * a.vh), vh = (size_t)a.vh;
+    const int b = v / NVBLK;                                       // chirality block
+    const Real sg = b ? (Real)-1 : (Real)1, kk = (Real)(-0.5 * a.csw);
+    auto Q = [&](int plane, int e) -> Real { return scratch[((size_t)plane * M + e) * (size_t)n + (size_t)loc]; };
+    auto Fre = [&](int plane, int r, int c) -> Real { return (Q(plane, 2 * (r * D + c) + 1) + Q(plane, 2 * (c * D + r) + 1)) * (Real)0.125; };
+    auto Fim = [&](int plane, int r, int c) -> Real { return -(Q(plane, 2 * (r * D + c)) - Q(plane, 2 * (c * D + r))) * (Real)0.125; };
+    // planes: 0 (0,1)  1 (0,2)  2 (0,3)  3 (1,2)  4 (1,3)  5 (2,3);  up: A = F01 - F23, B = F02 + F13, C = F03 - F12, dn: F0k -> -F0k
+    auto elem = [&](int row, int col, int part) -> Real {          // part 0 re, 1 im of T_b[row][col], row <= col
+        const int sr = row / D, ar = row % D, sc = col / D, ac = col % D;
+        Real val;
+        if (sr == sc) {
+            const Real c = part == 0 ? sg * Fre(2, ar, ac) - Fre(3, ar, ac) : sg * Fim(2, ar, ac) - Fim(3, ar, ac);
+            val = sr ? -c : c;
+        } else if (part == 0) val = (sg * Fre(0, ar, ac) - Fre(5, ar, ac)) + (sg * Fim(1, ar, ac) + Fim(4, ar, ac));   // Re(A - iB) = A_re + B_im
+        else val = (sg * Fim(0, ar, ac) - Fim(5, ar, ac)) - (sg * Fre(1, ar, ac) + Fre(4, ar, ac));                    // Im(A - iB) = A_im - B_re
+        return val * kk;
+    };
+    Real out[RPV];
+#pragma unroll
+    for (int i = 0; i < RPV; ++i) {
+        const int w = (v - b * NVBLK) * RPV + i;                   // packed real of the block
+        if (w < N2) out[i] = elem(w, w, 0);
+        else {
+            int u = (w - N2) >> 1, r = 0;
+            while (u >= N2 - 1 - r) { u -= N2 - 1 - r; ++r; }
+            out[i] = elem(r, r + 1 + u, (w - N2) & 1);
+        }
     }
-    const Real k = (Real)(-0.5 * a.csw);
-    Real rec[G::NREAL];
-    for (int b = 0; b < 2; ++b) {
-        const Real *A = cf[b][0], *B = cf[b][1], *C = cf[b][2];
-        auto elem = [&](int row, int col, Real &re, Real &im) {
-            const int sr = row / D, ar = row % D, sc = col / D, ac = col % D;
-            const int e = 2 * (ar * D + ac);
-            if (sr == 0 && sc == 0) { re = C[e]; im = C[e + 1]; }
-            else if (sr == 1 && sc == 1) { re = -C[e]; im = -C[e + 1]; }
-            else if (sr == 0 && sc == 1) { re = A[e] + B[e + 1]; im = A[e + 1] - B[e]; }
-            else { re = A[e] - B[e + 1]; im = A[e + 1] + B[e]; }
-            re *= k; im *= k;
-        };
-        Real *o = rec + b * G::BLK;
-        int w = 0;
-        for (int d = 0; d < 2 * D; ++d) { Real re, im; elem(d, d, re, im); o[w++] = re; }
-        for (int r = 0; r < 2 * D; ++r)
-            for (int s = r + 1; s < 2 * D; ++s) { Real re, im; elem(r, s, re, im); o[w++] = re; o[w++] = im; }
-    }
-    char *base = (char *)a.clover + (size_t)qpar * G::NREAL * sizeof(Real) * (size_t)a.vh;
-    store_record<G::NREAL>(base, (size_t)a.vh, hs, rec);
+    char *dst = (char *)a.clover + (size_t)qpar * G::NREAL * sizeof(Real) * vh + ((size_t)v * vh + hs) * 16;
+    if constexpr (sizeof(Real) == 8) st16<ST_DEFAULT>(dst, out[0], out[1]);
+    else st16<ST_DEFAULT>(dst, out[0], out[1], out[2], out[3]);
 }
 
 // out += T in on one parity (clover/in/out point at that parity's half fields).  One thread per (site, chirality
@@ -1253,7 +1248,7 @@ static hr_status build_rows(const hr_ctx *c, const CloverArgs &a, cudaStream_t s
 {
     const long total = c->V;
     // chunk sized by BYTES: 256 MiB of scratch at most (2^19 sites of d_R = 15 in fp64 were 11 GB next to the solver's
-    // workspaces), so that the hand-off from clover_q_kernel to clover_pack_kernel mostly stays in the 126 MB L2
+    // workspaces), so that the hand-off from the Q kernel to the packing kernel partly stays in the 126 MB L2
     const size_t per_site = (size_t)6 * 2 * D * D * sizeof(Real);
     long chunk = (long)(((size_t)256 << 20) / per_site) / 32 * 32;
     if (chunk < 32) chunk = 32;
@@ -1270,8 +1265,11 @@ static hr_status build_rows(const hr_ctx *c, const CloverArgs &a, cudaStream_t s
         rc = launched(PLANES ? "clover_plane_kernel" : "clover_q_kernel");
         if (rc != HR_OK) break;
         if constexpr (PLANES) clover_pack_f_kernel<Real, D, RL><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(a, scratch, first, n);
-        else clover_pack_kernel<Real, D, RL><<<(unsigned)((n + 63) / 64), 64, 0, st>>>(a, scratch, first, n);
-        rc = launched(PLANES ? "clover_pack_f_kernel" : "clover_pack_kernel");
+        else {
+            constexpr int NVREC = CloverGeom<Real, D, RL>::NREAL / (16 / (int)sizeof(Real));
+            clover_pack_vec_kernel<Real, D, RL><<<(unsigned)((n * NVREC + 127) / 128), 128, 0, st>>>(a, scratch, first, n);
+        }
+        rc = launched(PLANES ? "clover_pack_f_kernel" : "clover_pack_vec_kernel");
     }
     cudaFreeAsync(scratch, st);
     return rc;
